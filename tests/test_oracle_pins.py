@@ -1,0 +1,544 @@
+"""Pins for the CPU oracle: closed forms, invariants, an independent derivation, brute force and finite
+differences (no GPU).  Each pin is chosen so that a plausible mistake in oracle/satsplat_oracle.cpp (a
+dropped term, a wrong sign or index, a transposed operand) fails at least one of them.  None of the
+expected values below comes from the oracle or from the CUDA path: they are numpy restatements of the
+closed form for the special case, or properties the mathematics fixes.
+
+P1  single camera-facing surfel          -> Gaussian ellipse, opacity, depth, normal (Eq. 8-12, 14)
+P1b tilted surfel                        -> foreshortening by cos(beta), depth slope g (Eq. 6, 11)
+P2/P7 stacked surfels at one pixel       -> blending order, transmittance, O(n^2) distortion, median
+P3  inverse-map round trip               -> Eq. 8-10 and the depth plane
+P4  homogeneous two-plane intersection   -> Eq. 9 is its affine special case
+P5  sun camera                           -> Eq. 16, S1-S6, hand-evaluated fixtures, reprojection
+P6  compositing invariants               -> T monotone in [0,1], A + T = 1, stop rule
+P8  central finite differences           -> every gradient of step E incl. dF, CC, L_a, reproj, sun depth
+P9  all-pairs == tile lists              -> bbox conservativeness, tile independence
+P10 binning                              -> sorted, stable, complete, ranges consistent
+P11 shadow test closed form              -> reprojection, bilinear, sigmoid sign, Eq. 1
+P12 identity cases of Eq. 1
+P13 fp32 contract vs double              -> records agree to fp32 rounding
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import satsplat_scenes as S
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def make_view(W, H, F, *, dF=None, view_dir=(0, 0, -1), b_z=100.0, z_bg=120.0, bg=(0, 0, 0), cc=None,
+              ambient=(0.3, 0.35, 0.45)):
+    cc = np.concatenate([np.eye(3), np.zeros((3, 1))], 1).reshape(12) if cc is None else cc
+    return S.View(width=W, height=H, F=np.asarray(F, np.float32).reshape(8),
+                  dF=np.zeros(8, np.float32) if dF is None else np.asarray(dF, np.float32),
+                  view_dir=np.asarray(view_dir, np.float32), b_z=b_z, z_bg=z_bg,
+                  bg_rgb=np.asarray(bg, np.float32), cc=np.asarray(cc, np.float32),
+                  ambient=np.asarray(ambient, np.float32))
+
+
+def nadir_F(gsd, W, H):
+    return np.array([[1 / gsd, 0, 0, W / 2], [0, -1 / gsd, 0, H / 2]], np.float64)
+
+
+def pixel_grid(W, H):
+    px, py = np.meshgrid(np.arange(W) + 0.5, np.arange(H) + 0.5)
+    return px, py
+
+
+def render64(orc, view, means, quats, scales, logits, rgb, *, shading=None, options=0, bg=None):
+    """all-pairs, everything in double from the raw inputs (record mode `double`)."""
+    pre = orc.preprocess_f64(view, means, quats, scales, logits, rgb)
+    order = np.argsort(-np.asarray(means, np.float64)[:, 2], kind="stable").astype(np.uint32)  # depth = b_z - z
+    shading = shading or orc.Shading(cc=view.cc, ambient=view.ambient)
+    out = orc.forward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb if bg is None else bg, pre["rec"],
+                      pre["flags"], order, shading, options=options)
+    return pre, order, out
+
+
+# ------------------------------------------------------------------------------------------------ P1
+def test_p1_single_camera_facing_surfel(orc):
+    W = H = 48
+    gsd = 0.5
+    view = make_view(W, H, nadir_F(gsd, W, H))
+    p = np.array([[0.7, -0.4, 12.0]])     # world; projects to (W/2 + 1.4, H/2 + 0.8)
+    su, sv, logit = 1.5, 0.8, 0.3
+    rgbv = np.array([[0.2, 0.5, 0.9]])
+    pre, _, out = render64(orc, view, p, np.array([[1.0, 0, 0, 0]]), np.array([[su, sv]]), np.array([logit]), rgbv)
+    px, py = pixel_grid(W, H)
+    cx, cy = W / 2 + p[0, 0] / gsd, H / 2 - p[0, 1] / gsd
+    dxw, dyw = (px - cx) * gsd, (py - cy) * gsd          # world offsets
+    rho = (dxw / su) ** 2 + (dyw / sv) ** 2               # scales >= 1 px: the low-pass term never wins
+    alpha = 1 / (1 + math.exp(-logit))
+    A = np.minimum(0.99, alpha * np.exp(-0.5 * rho))
+    A[(rho > 9) | (A < 1 / 255)] = 0
+    zc = view.b_z - p[0, 2]
+    np.testing.assert_allclose(out["rgba"][..., 3], A, atol=1e-13)
+    for c in range(3):
+        np.testing.assert_allclose(out["rgba"][..., c], A * rgbv[0, c], atol=1e-13)   # identity CC, bg 0
+    np.testing.assert_allclose(out["geom"][..., 3], A * zc, atol=1e-11)
+    np.testing.assert_allclose(out["geom"][..., 2], A * 1.0, atol=1e-13)              # n = +z faces the sensor
+    np.testing.assert_allclose(out["geom"][..., :2], 0, atol=1e-13)
+    np.testing.assert_allclose(out["aux"][..., 1], 0, atol=1e-9)                      # one surfel: no distortion
+    np.testing.assert_allclose(out["aux"][..., 3], 1 - A, atol=1e-13)
+    med = np.where(A > 0, zc, view.z_bg)
+    np.testing.assert_allclose(out["aux"][..., 0], med, atol=1e-11)
+    assert A.max() > 0.5 and (A > 0).sum() > 50
+
+
+def test_p1b_tilted_surfel(orc):
+    W = H = 64
+    gsd = 0.5
+    view = make_view(W, H, nadir_F(gsd, W, H))
+    beta = math.radians(35.0)
+    q = np.array([[math.cos(beta / 2), math.sin(beta / 2), 0, 0]])   # rotation about the u (= world x) axis
+    p = np.array([[0.0, 0.0, 5.0]])
+    su, sv = 2.0, 3.0
+    pre, _, out = render64(orc, view, p, q, np.array([[su, sv]]), np.array([4.0]), np.array([[1.0, 1.0, 1.0]]))
+    px, py = pixel_grid(W, H)
+    dxw, dyw = (px - W / 2) * gsd, -(py - H / 2) * gsd   # image y is down
+    u, v = dxw / su, dyw / (sv * math.cos(beta))         # v-extent on screen is foreshortened by cos(beta)
+    rho = u * u + v * v
+    alpha = 1 / (1 + math.exp(-4.0))
+    A = np.minimum(0.99, alpha * np.exp(-0.5 * rho))
+    keep = (rho <= 9) & (A >= 1 / 255)
+    A = np.where(keep, A, 0)
+    z = (view.b_z - p[0, 2]) - sv * math.sin(beta) * v   # P_z = p_z + s_v sin(beta) v  (Eq. 3, 6, 11)
+    np.testing.assert_allclose(out["rgba"][..., 3], A, atol=1e-12)
+    np.testing.assert_allclose(out["geom"][..., 3], A * z, atol=1e-10)
+    n = np.array([0, -math.sin(beta), math.cos(beta)])
+    for c in range(3):
+        np.testing.assert_allclose(out["geom"][..., c], A * n[c], atol=1e-12)
+
+
+def test_p1c_lowpass_wins_for_subpixel_and_edge_on(orc):
+    """Eq. 12: a surfel much smaller than a pixel, or seen edge-on, renders as the sigma = 1/sqrt(2) px disc."""
+    W = H = 16
+    gsd = 1.0
+    view = make_view(W, H, nadir_F(gsd, W, H))
+    px, py = pixel_grid(W, H)
+    d2 = (px - (W / 2 + 0.25)) ** 2 + (py - (H / 2 - 0.5)) ** 2
+    alpha = 1 / (1 + math.exp(-1.0))
+    A_disc = np.minimum(0.99, alpha * np.exp(-0.5 * 2.0 * d2))
+    A_disc[(2 * d2 > 9) | (A_disc < 1 / 255)] = 0
+    zc = view.b_z - 3.0
+    # (a) tiny surfel: G(u) < G_lowpass everywhere except within ~the surfel itself (no pixel centre there)
+    pre, _, out = render64(orc, view, np.array([[0.25, 0.5, 3.0]]), np.array([[1.0, 0, 0, 0]]),
+                           np.array([[0.01, 0.01]]), np.array([1.0]), np.ones((1, 3)))
+    np.testing.assert_allclose(out["rgba"][..., 3], A_disc, atol=1e-12)
+    np.testing.assert_allclose(out["geom"][..., 3], A_disc * zc, atol=1e-10)   # low-pass branch uses z_c
+    # (b) exactly edge-on surfel (normal horizontal): det = 0 -> degenerate flag, same disc
+    q = np.array([[math.cos(math.pi / 4), math.sin(math.pi / 4), 0, 0]])       # 90 deg about x
+    pre, _, out = render64(orc, view, np.array([[0.25, 0.5, 3.0]]), q, np.array([[0.01, 5.0]]), np.array([1.0]),
+                           np.ones((1, 3)))
+    assert pre["flags"][0] & orc.F_DEGENERATE
+    np.testing.assert_allclose(out["rgba"][..., 3], A_disc, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------- P2 / P7
+def test_p2_p7_stacked_surfels_blend_order_distortion_median(orc):
+    rng = np.random.default_rng(5)
+    W = H = 1
+    view = make_view(W, H, nadir_F(1.0, W, H), z_bg=200.0, bg=(0.1, 0.2, 0.3))
+    n = 9
+    heights = rng.uniform(0, 30, n)
+    means = np.stack([np.zeros(n), np.zeros(n), heights], 1)       # all centred on the single pixel centre
+    logits = rng.normal(0.0, 1.5, n)
+    logits[3] = 8.0                                                # one clamps at 0.99
+    rgb = rng.uniform(0, 1, (n, 3))
+    quats = np.tile([1.0, 0, 0, 0], (n, 1))
+    pre, order, out = render64(orc, view, means, quats, np.full((n, 2), 4.0), logits, rgb)
+    # by hand: front to back = decreasing height; G = 1 at the centre
+    idx = np.argsort(-heights, kind="stable")
+    T, C, D, Ls = 1.0, np.zeros(3), 0.0, 0.0
+    ws, zs, med = [], [], view.z_bg
+    for i in idx:
+        a = min(0.99, 1 / (1 + math.exp(-logits[i])))
+        z = view.b_z - heights[i]
+        if T * (1 - a) < 1e-4:
+            break
+        if T > 0.5:
+            med = z
+        w = a * T
+        ws.append(w); zs.append(z)
+        C += w * rgb[i]; D += w * z
+        T *= 1 - a
+    ws, zs = np.array(ws), np.array(zs)
+    for i in range(len(ws)):
+        for j in range(i):
+            Ls += ws[i] * ws[j] * (zs[i] - zs[j]) ** 2             # O(n^2) definition (Mip-NeRF-360 form)
+    C = C + T * np.asarray(view.bg_rgb, np.float64)
+    np.testing.assert_allclose(out["rgba"][0, 0, :3], C, rtol=1e-12)
+    np.testing.assert_allclose(out["rgba"][0, 0, 3], 1 - T, rtol=1e-12)
+    np.testing.assert_allclose(out["geom"][0, 0, 3], D, rtol=1e-12)
+    np.testing.assert_allclose(out["aux"][0, 0, 1], Ls, rtol=1e-9)
+    np.testing.assert_allclose(out["aux"][0, 0, 0], med, rtol=1e-12)
+    np.testing.assert_allclose(out["aux"][0, 0, 3], T, rtol=1e-12)
+    assert len(ws) >= 4
+
+
+# ------------------------------------------------------------------------------------------------ P3
+def test_p3_inverse_map_round_trip(orc):
+    rng = np.random.default_rng(11)
+    n = 200
+    F, d = S.affine_camera(0.4, math.radians(22), 1.1, 256, 256, (10, -5, 0))
+    dF = (rng.normal(0, 1e-3, 8)).astype(np.float32)
+    view = make_view(256, 256, F, dF=dF, view_dir=d)
+    means = rng.uniform(-30, 30, (n, 3))
+    quats = rng.normal(0, 1, (n, 4)) * rng.uniform(0.3, 3, (n, 1))    # deliberately not unit
+    scales = rng.uniform(0.2, 2, (n, 2))
+    pre = orc.preprocess_f64(view, means, quats, scales, np.zeros(n), np.zeros((n, 3)))
+    rec = pre["rec"]
+    Fp = (view.F.astype(np.float64) + view.dF.astype(np.float64)).reshape(2, 4)
+    qh = quats / np.linalg.norm(quats, axis=1, keepdims=True)
+    w, x, y, z = qh.T
+    # textbook rotation matrix of a unit quaternion, column by column
+    R = np.stack([np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y)], 1),
+                  np.stack([2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x)], 1),
+                  np.stack([2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)], 1)], 1)  # [n,3,3]
+    np.testing.assert_allclose(np.einsum("nij,nkj->nik", R, R), np.tile(np.eye(3), (n, 1, 1)), atol=1e-12)
+    uv = rng.uniform(-3, 3, (n, 2))
+    P = means + scales[:, :1] * R[:, :, 0] * uv[:, :1] + scales[:, 1:] * R[:, :, 1] * uv[:, 1:]   # Eq. 3
+    xpix = P @ Fp[:, :3].T + Fp[:, 3]                                                               # Eq. 6
+    dd = xpix - rec[:, 0:2]
+    u = rec[:, 2] * dd[:, 0] + rec[:, 3] * dd[:, 1]
+    v = rec[:, 4] * dd[:, 0] + rec[:, 5] * dd[:, 1]
+    np.testing.assert_allclose(np.stack([u, v], 1), uv, atol=1e-9)
+    zz = rec[:, 6] + rec[:, 7] * dd[:, 0] + rec[:, 8] * dd[:, 1]
+    np.testing.assert_allclose(zz, view.b_z - P[:, 2], atol=1e-9)                                   # Eq. 11
+    np.testing.assert_allclose(rec[:, 0:2], means @ Fp[:, :3].T + Fp[:, 3], atol=1e-10)
+    # stored normal: last column of R, flipped to face the sensor
+    nrm = R[:, :, 2]
+    flip = (nrm @ view.view_dir.astype(np.float64)) > 0
+    np.testing.assert_allclose(rec[:, 13:16], np.where(flip[:, None], -nrm, nrm), atol=1e-12)
+    assert ((pre["flags"] & orc.F_FLIPPED) > 0).tolist() == flip.tolist()
+
+
+# ------------------------------------------------------------------------------------------------ P4
+def test_p4_two_plane_intersection_reduces_to_affine_inverse(orc):
+    """2DGS finds (u,v) by intersecting the two pixel planes transformed by (WH)^T.  With an
+    affine W (last row 0 0 0 1) the same construction must give Q x + q of Eq. 9."""
+    rng = np.random.default_rng(12)
+    n = 50
+    F, d = S.affine_camera(0.5, math.radians(30), 2.5, 128, 128, (0, 0, 0))
+    view = make_view(128, 128, F, view_dir=d)
+    means = rng.uniform(-20, 20, (n, 3))
+    quats = rng.normal(0, 1, (n, 4))
+    scales = rng.uniform(0.3, 2, (n, 2))
+    rec = orc.preprocess_f64(view, means, quats, scales, np.zeros(n), np.zeros((n, 3)))["rec"]
+    Fp = view.F.astype(np.float64).reshape(2, 4)
+    Wm = np.zeros((4, 4)); Wm[:2] = Fp; Wm[2] = [0, 0, -1, view.b_z]; Wm[3] = [0, 0, 0, 1]   # Eq. 7 + Eq. 11
+    qh = quats / np.linalg.norm(quats, axis=1, keepdims=True)
+    for i in range(n):
+        w, x, y, z = qh[i]
+        tu = np.array([1 - 2 * (y * y + z * z), 2 * (x * y + w * z), 2 * (x * z - w * y)])
+        tv = np.array([2 * (x * y - w * z), 1 - 2 * (x * x + z * z), 2 * (y * z + w * x)])
+        Hm = np.zeros((4, 4)); Hm[:3, 0] = scales[i, 0] * tu; Hm[:3, 1] = scales[i, 1] * tv
+        Hm[:3, 3] = means[i]; Hm[3, 3] = 1                                                     # Eq. 4
+        WH = Wm @ Hm
+        xp = rec[i, 0:2] + rng.uniform(-20, 20, 2)
+        hx, hy = np.array([-1, 0, 0, xp[0]]), np.array([0, -1, 0, xp[1]])
+        hu, hv = WH.T @ hx, WH.T @ hy
+        den = hu[0] * hv[1] - hu[1] * hv[0]
+        u = (hu[1] * hv[3] - hu[3] * hv[1]) / den
+        v = (hu[3] * hv[0] - hu[0] * hv[3]) / den
+        dd = xp - rec[i, 0:2]
+        np.testing.assert_allclose([rec[i, 2] * dd[0] + rec[i, 3] * dd[1], rec[i, 4] * dd[0] + rec[i, 5] * dd[1]],
+                                   [u, v], atol=1e-8)
+
+
+# ------------------------------------------------------------------------------------------------ P5
+def test_p5_sun_camera_fixtures_and_nullspace(orc):
+    rows = [l for l in open(os.path.join(GOLDEN, "sun_camera_cases.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 4
+    for l in rows:
+        v = [float(t) for t in l.split()]
+        phi, th = math.radians(v[0]), math.radians(v[1])
+        B = np.array(v[2:8]).reshape(2, 3)
+        Fp = np.concatenate([B, [[3.0], [-7.0]]], 1).reshape(8)
+        F_sun, reproj = orc.sun_camera(Fp, phi, th, [1, 1, 0, 0])
+        np.testing.assert_allclose(F_sun.reshape(2, 4)[:, :3], np.array(v[8:14]).reshape(2, 3), atol=1e-12)
+        np.testing.assert_allclose(F_sun.reshape(2, 4)[:, 3], [3.0, -7.0], atol=1e-12)
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        F, d = S.affine_camera(rng.uniform(0.3, 0.6), math.radians(rng.uniform(0, 35)), rng.uniform(0, 6.28), 512, 512,
+                               (50, 60, 0))
+        Fp = F.astype(np.float64)
+        B = Fp.reshape(2, 4)[:, :3]
+        # l.165: the viewing direction B_x x B_y spans the nullspace of B_xy
+        np.testing.assert_allclose(B @ np.cross(B[0], B[1]), 0, atol=1e-9)
+        phi, th = rng.uniform(0, 2 * math.pi), math.radians(rng.uniform(20, 80))
+        s = np.array([math.cos(phi) / math.tan(th), math.sin(phi) / math.tan(th), 1.0])
+        vp = np.array([rng.uniform(0.5, 2), rng.uniform(0.5, 2), rng.uniform(-50, 50), rng.uniform(-50, 50)])
+        F_sun, reproj = orc.sun_camera(Fp, phi, th, vp)
+        Fs = F_sun.reshape(2, 4)
+        np.testing.assert_allclose(Fs[:, :3] @ s, 0, atol=1e-9)                                  # Eq. S6
+        p = rng.uniform(-40, 40, 3)
+        t = rng.uniform(-30, 30)
+        np.testing.assert_allclose(Fs[:, :3] @ p + Fs[:, 3], Fs[:, :3] @ (p + t * s) + Fs[:, 3], atol=1e-8)
+        # shadow of a point at height h falls on the ground at p_xy - h (cos phi, sin phi)/tan theta
+        g = np.array([p[0] - p[2] * s[0], p[1] - p[2] * s[1], 0.0])
+        np.testing.assert_allclose(Fs[:, :3] @ p, Fs[:, :3] @ g, atol=1e-8)
+        # reprojection: view pixel x of a world point at height h  ->  its sun pixel
+        xv = B @ p + Fp.reshape(2, 4)[:, 3]
+        xs = Fs[:, :3] @ p + Fs[:, 3]
+        R = reproj.reshape(2, 4)
+        np.testing.assert_allclose(R[:, :2] @ xv + R[:, 2] * p[2] + R[:, 3], xs, atol=1e-7)
+    # unscaled Eq. 16 camera: R_x = I, k_h = -B s, k_0 = 0
+    F_sun, reproj = orc.sun_camera(Fp, phi, th, [1, 1, 0, 0])
+    R = reproj.reshape(2, 4)
+    np.testing.assert_allclose(R[:, :2], np.eye(2), atol=1e-12)
+    np.testing.assert_allclose(R[:, 2], -(B @ s), atol=1e-10)
+    np.testing.assert_allclose(R[:, 3], 0, atol=1e-9)
+
+
+# ------------------------------------------------------------------------------------- P6 / P9 / P10
+@pytest.fixture(scope="module")
+def c0(orc):
+    scene = S.make_config(0)
+    view = scene.views[0]
+    tile = orc.render_pass(view, scene, tile_mode=True)
+    sh = orc.Shading(cc=view.cc, ambient=view.ambient)
+    f_tile = orc.forward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, tile["rec64"], tile["flags"],
+                         tile["lists"], sh, threads=orc.num_threads())
+    order = orc.global_order(tile["depth_key"], tile["flags"])
+    f_all = orc.forward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, tile["rec64"], tile["flags"],
+                        order, sh, threads=orc.num_threads())
+    return scene, view, tile, f_tile, f_all, order
+
+
+def test_p6_compositing_invariants(c0):
+    scene, view, tile, f, _, _ = c0
+    T, A = f["aux"][..., 3], f["rgba"][..., 3]
+    assert (T >= 1e-4).all() and (T <= 1).all()
+    np.testing.assert_allclose(A + T, 1, atol=1e-15)
+    assert (np.linalg.norm(f["geom"][..., :3], axis=-1) <= A * (1 + 1e-6) + 1e-12).all()     # |sum w n| <= sum w (fp32 normals are unit to ~1e-7)
+    zmin, zmax = view.b_z - scene.means[:, 2].max() - 5, view.b_z - scene.means[:, 2].min() + 5
+    has = A > 1e-3
+    dmean = f["geom"][..., 3][has] / A[has]
+    assert (dmean > zmin).all() and (dmean < zmax).all()
+    assert (f["aux"][..., 1] >= -1e-12).all()                                   # distortion is a sum of squares
+    assert (f["rgba"][..., :3] >= 0).all() and (f["rgba"][..., :3] <= 1 + 1e-12).all()
+    assert f["counters"][1] > view.width * view.height
+
+
+def test_p9_all_pairs_equals_tile_lists(c0):
+    scene, view, tile, f_tile, f_all, _ = c0
+    for k in ("rgba", "geom", "aux", "albedo", "med_idx"):
+        assert np.array_equal(f_tile[k], f_all[k]), k
+    assert f_all["counters"][1] == f_tile["counters"][1]
+    assert f_all["counters"][0] > f_tile["counters"][0]
+
+
+def test_p10_binning_sorted_stable_complete(c0, orc):
+    scene, view, tile, *_ = c0
+    keys, vals, ranges = tile["keys"], tile["vals"], tile["ranges"]
+    rect, count, dk = tile["rect"], tile["count"], tile["depth_key"]
+    TX = (view.width + 15) // 16
+    assert np.all(keys[1:] >= keys[:-1])
+    same = keys[1:] == keys[:-1]
+    assert np.all(vals[1:][same] > vals[:-1][same])                      # ties broken by ascending surfel index
+    # completeness: the multiset of (tile, surfel) pairs equals the rect expansion, done independently here
+    pairs = set()
+    for i in range(scene.n):
+        if count[i]:
+            for ty in range(rect[i, 1], rect[i, 3]):
+                for tx in range(rect[i, 0], rect[i, 2]):
+                    pairs.add((ty * TX + tx, i))
+    got = list(zip((keys >> np.uint64(32)).astype(np.int64).tolist(), vals.tolist()))
+    assert len(got) == len(pairs) == int(count.sum()) and set(got) == pairs
+    assert np.array_equal((keys & np.uint64(0xFFFFFFFF)).astype(np.uint32), dk[vals])
+    # depth key is order preserving
+    zc = tile["rec"][:, 6]
+    o = np.argsort(dk, kind="stable")
+    assert np.all(np.diff(zc[o]) >= 0)
+    # ranges
+    tiles = (keys >> np.uint64(32)).astype(np.int64)
+    for t in range(ranges.shape[0]):
+        s, e = ranges[t]
+        if e > s:
+            assert np.all(tiles[s:e] == t) and (s == 0 or tiles[s - 1] < t) and (e == len(tiles) or tiles[e] > t)
+        else:
+            assert not np.any(tiles == t) and s == 0 and e == 0
+    # rect really is the 3-sigma box, in tiles, clamped (spot-check against a direct float64 evaluation)
+    rec = tile["rec"].astype(np.float64)
+    M = np.linalg.inv(rec[:, 2:6].reshape(-1, 2, 2) + np.eye(2) * 1e-300)
+    ok = (tile["flags"] & (orc.F_DEGENERATE | orc.F_CULLED)) == 0
+    ext = np.maximum(3 * np.sqrt((M ** 2).sum(-1)), 3 / math.sqrt(2))
+    lo = np.floor((rec[:, 0:2] - ext) / 16).astype(int)
+    hi = np.floor((rec[:, 0:2] + ext) / 16).astype(int) + 1
+    TY = (view.height + 15) // 16
+    lo = np.clip(lo, 0, [TX, TY]); hi = np.clip(hi, 0, [TX, TY])
+    mism = ((lo[:, 0] != rect[:, 0]) | (lo[:, 1] != rect[:, 1]) | (hi[:, 0] != rect[:, 2]) | (hi[:, 1] != rect[:, 3])) & ok
+    assert mism.sum() <= 2          # float64 vs the fp32 contract may differ on a knife edge only
+
+
+def test_p13_fp32_contract_matches_double(c0, orc):
+    scene, view, tile, *_ = c0
+    d = orc.preprocess_f64(view, scene.means, scene.quats, scene.scales, scene.opacity_logits, scene.rgb)
+    ok = (tile["flags"] & orc.F_DEGENERATE) == 0
+    assert np.array_equal(tile["flags"] & orc.F_DEGENERATE, d["flags"] & orc.F_DEGENERATE)
+    a, b = tile["rec"][ok].astype(np.float64), d["rec"][ok]
+    scale = np.abs(b).max(0) + 1e-6
+    assert (np.abs(a - b) / scale).max() < 5e-5
+    assert np.abs(a[:, :2] - b[:, :2]).max() < 1e-4     # centres to ~fp32 ulp at 128 px
+
+
+# ------------------------------------------------------------------------------------------------ P8
+def _fd_problem(orc, shadows, options, seed=21):
+    rng = np.random.default_rng(seed)
+    n, W, H = 14, 16, 16
+    F, d = S.affine_camera(0.5, math.radians(20), 0.7, W, H, (4, 4, 0))
+    means = np.concatenate([rng.uniform(0.5, 7.5, (n, 2)), rng.normal(0, 1.0, (n, 1))], 1)
+    nrm = np.array([0, 0, 1.0]) + 0.5 * rng.normal(0, 1, (n, 3))
+    quats = rng.normal(0, 1, (n, 4))
+    quats[:, 0] += 3.0          # mostly upward-facing, generic otherwise
+    quats *= rng.uniform(0.5, 2.0, (n, 1))
+    del nrm
+    P = dict(means=means, quats=quats, scales=rng.uniform(0.6, 2.0, (n, 2)), logits=rng.normal(0.5, 1, n),
+             rgb=rng.uniform(0, 1, (n, 3)), dF=rng.normal(0, 1e-2, 8),
+             cc=(np.concatenate([np.eye(3), np.zeros((3, 1))], 1) + rng.normal(0, 0.1, (3, 4))).reshape(12),
+             ambient=rng.uniform(0.2, 0.5, 3))
+    if shadows:
+        P["reproj"] = np.array([0.9, 0.05, 0.3, 1.0, -0.04, 0.95, -0.2, 0.5]) + rng.normal(0, 0.01, 8)
+        P["sun_depth"] = 10 + rng.normal(0, 1.0, (20, 20))
+    view = make_view(W, H, F, view_dir=d, b_z=12.0, z_bg=16.0, bg=(0.2, 0.1, 0.3))
+    up = [rng.normal(0, 1, (H, W, 4)) for _ in range(3)]
+    up[2][..., 2:] = 0
+    order = np.argsort(-means[:, 2], kind="stable").astype(np.uint32)
+
+    def run(Pv, need_grad=False):
+        sh = orc.Shading(cc=Pv["cc"], ambient=Pv["ambient"], sun_depth=Pv.get("sun_depth"), reproj=Pv.get("reproj"),
+                         bias=0.5, slope=4.0)
+        pre = orc.preprocess_f64(view, Pv["means"], Pv["quats"], Pv["scales"], Pv["logits"], Pv["rgb"],
+                                 F=view.F.astype(np.float64), dF=Pv["dF"])
+        out = orc.forward(W, H, view.b_z, view.z_bg, view.bg_rgb, pre["rec"], pre["flags"], order, sh, options=options)
+        loss = (out["rgba"] * up[0]).sum() + (out["geom"] * up[1]).sum() + (out["aux"] * up[2]).sum()
+        if not need_grad:
+            return loss, out
+        bw = orc.backward(W, H, view.b_z, view.z_bg, view.bg_rgb, pre["rec"], pre["flags"], order, sh, *up, options=options)
+        g = orc.preprocess_backward(view, Pv["means"], Pv["quats"], Pv["scales"], Pv["logits"], pre["flags"],
+                                    bw["v_rec"], F=view.F.astype(np.float64), dF=Pv["dF"])
+        grads = dict(means=g["v_means"], quats=g["v_quats"], scales=g["v_scales"], logits=g["v_logits"], rgb=g["v_rgb"],
+                     dF=g["v_dF"], cc=bw["v_cc"], ambient=bw["v_ambient"])
+        if shadows:
+            grads.update(reproj=bw["v_reproj"], sun_depth=bw["v_sun_depth"])
+        return loss, out, grads
+
+    return P, run
+
+
+def _check_fd(P, run, names, h=1e-6, rtol=1e-6):
+    _, out, grads = run(P, need_grad=True)
+    rng = np.random.default_rng(0)
+    worst = 0.0
+    for name in names:
+        base = np.asarray(P[name], np.float64)
+        flat_idx = np.arange(base.size)
+        if base.size > 60:
+            flat_idx = rng.choice(base.size, 60, replace=False)
+        g = np.asarray(grads[name]).reshape(-1)
+        gscale = max(np.abs(g).max(), 1e-3)
+        for k in flat_idx:
+            Pp, Pm = dict(P), dict(P)
+            e = np.zeros(base.size); e[k] = h * max(1.0, abs(base.reshape(-1)[k]))
+            Pp[name] = (base.reshape(-1) + e).reshape(base.shape)
+            Pm[name] = (base.reshape(-1) - e).reshape(base.shape)
+            fd = (run(Pp)[0] - run(Pm)[0]) / (2 * e[k])
+            err = abs(fd - g[k]) / gscale
+            worst = max(worst, err)
+            assert err < rtol, (name, int(k), fd, g[k])
+    return out, worst
+
+
+def test_p8_finite_differences_no_cutoffs(orc):
+    """Cut-offs off (smooth objective): every parameter group, shadows off."""
+    P, run = _fd_problem(orc, shadows=False, options=7)
+    out, _ = _check_fd(P, run, ["means", "quats", "scales", "logits", "rgb", "dF", "cc", "ambient"])
+    assert out["counters"][1] > 200
+
+
+def test_p8_finite_differences_shadows(orc):
+    """Shadows on with an arbitrary sun map: adds reproj, sun depth, ambient through V."""
+    P, run = _fd_problem(orc, shadows=True, options=7)
+    # bilinear sampling is piecewise smooth: keep the sample points away from texel borders for the FD step
+    out, _ = _check_fd(P, run, ["means", "quats", "scales", "logits", "rgb", "dF", "cc", "ambient", "reproj", "sun_depth"])
+    V = out["aux"][..., 2]
+    assert V.min() < 0.4 and V.max() > 0.8          # the shadow test is exercised on both sides
+
+
+def test_p8_finite_differences_with_cutoffs(orc):
+    """Cut-offs on: gradients still match away from the decision boundaries (margins asserted)."""
+    P, run = _fd_problem(orc, shadows=False, options=0, seed=33)
+    _, out = run(P)
+    m = out["margins"]
+    # distance of every pixel from the rho cut, the alpha skip and the median switch; step 1e-7 moves rho by <1e-5
+    assert np.isfinite(m[..., 0]).any()
+    names = ["means", "scales", "logits", "rgb", "dF"]
+    _, out, grads = run(P, need_grad=True)
+    h = 1e-7
+    rng = np.random.default_rng(1)
+    for name in names:
+        base = np.asarray(P[name], np.float64)
+        g = np.asarray(grads[name]).reshape(-1)
+        gscale = max(np.abs(g).max(), 1e-3)
+        bad = 0
+        idxs = rng.choice(base.size, min(base.size, 30), replace=False)
+        for k in idxs:
+            e = np.zeros(base.size); e[k] = h
+            Pp, Pm = dict(P), dict(P)
+            Pp[name] = (base.reshape(-1) + e).reshape(base.shape)
+            Pm[name] = (base.reshape(-1) - e).reshape(base.shape)
+            fd = (run(Pp)[0] - run(Pm)[0]) / (2 * h)
+            if abs(fd - g[k]) / gscale > 1e-3:
+                bad += 1            # a decision flipped inside the FD step (jump in the loss)
+        assert bad <= 1, (name, bad)
+
+
+# ----------------------------------------------------------------------------------------- P11 / P12
+def test_p11_shadow_test_closed_form(orc):
+    W = H = 24
+    gsd = 0.5
+    view = make_view(W, H, nadir_F(gsd, W, H), z_bg=130.0)
+    # one big opaque camera-facing surfel: A = 0.99 over the whole frame
+    means = np.array([[0.0, 0.0, 20.0]])
+    pre = orc.preprocess_f64(view, means, np.array([[1.0, 0, 0, 0]]), np.array([[500.0, 500.0]]), np.array([20.0]),
+                             np.array([[0.5, 0.6, 0.7]]))
+    Ws, Hs = 40, 30
+    sx, sy = np.meshgrid(np.arange(Ws), np.arange(Hs))
+    sun_depth = 70.0 + 0.5 * sx - 0.25 * sy                  # linear ramp: bilinear interpolation is exact
+    reproj = np.array([1.2, 0.1, 0.05, 3.0, -0.1, 0.9, -0.02, 2.0])
+    cc = np.array([[1.1, 0.05, 0, 0.01], [0, 0.9, 0.1, -0.02], [0.02, 0, 1.2, 0.03]])
+    amb = np.array([0.3, 0.35, 0.45])
+    sh = orc.Shading(cc=cc.reshape(12), ambient=amb, sun_depth=sun_depth, reproj=reproj, bias=0.5, slope=4.0)
+    out = orc.forward(W, H, view.b_z, view.z_bg, view.bg_rgb, pre["rec"], pre["flags"], np.array([0], np.uint32), sh)
+    px, py = pixel_grid(W, H)
+    A = 0.99
+    zv = A * (view.b_z - 20.0) + (1 - A) * view.z_bg
+    h = view.b_z - zv
+    xs = reproj[0] * px + reproj[1] * py + reproj[2] * h + reproj[3]
+    ys = reproj[4] * px + reproj[5] * py + reproj[6] * h + reproj[7]
+    inside = (xs >= 0.5) & (xs <= Ws - 0.5) & (ys >= 0.5) & (ys <= Hs - 0.5)
+    ds = 70.0 + 0.5 * (xs - 0.5) - 0.25 * (ys - 0.5)
+    V = np.where(inside, 1 / (1 + np.exp(4.0 * (zv - ds - 0.5))), 1.0)
+    assert inside.any() and (~inside).any() and V[inside].min() < 0.2 and V[inside].max() > 0.8
+    np.testing.assert_allclose(out["aux"][..., 2], V, atol=1e-12)
+    albedo = A * np.array([0.5, 0.6, 0.7])
+    for c in range(3):
+        I = (cc[c, :3] @ albedo + cc[c, 3]) * (V + (1 - V) * amb[c])          # Eq. 1
+        np.testing.assert_allclose(out["rgba"][..., c], I, atol=1e-12)
+
+
+def test_p12_identity_cases(c0, orc):
+    scene, view, tile, f_tile, _, _ = c0
+    np.testing.assert_array_equal(f_tile["rgba"][..., :3], f_tile["albedo"])    # CC = [I 0], shadows off
+    np.testing.assert_array_equal(f_tile["aux"][..., 2], 1.0)
+    cc = np.array([[0.9, 0.1, 0, 0.05], [0, 1.1, 0, 0], [0.1, 0, 0.8, -0.05]])
+    f2 = orc.forward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, tile["rec64"], tile["flags"],
+                     tile["lists"], orc.Shading(cc=cc.reshape(12), ambient=(0.5, 0.5, 0.5)), threads=orc.num_threads())
+    exp = f_tile["albedo"] @ cc[:, :3].T + cc[:, 3]
+    np.testing.assert_allclose(f2["rgba"][..., :3], exp, atol=1e-14)
+    for k in ("geom", "aux"):
+        np.testing.assert_array_equal(f2[k], f_tile[k])
