@@ -1,0 +1,190 @@
+/* satsplat.h — C ABI of the B200-native affine-2DGS rasteriser (SatSplat hot path, arxiv/paper_2606_28581).
+ *
+ * Boundary of the product: plain C, plain pointers and sizes, no C++ or torch types.  Every pointer
+ * argument says whether it is a HOST or a DEVICE pointer.  Citations are PAPER.md line numbers
+ * (/root/reference/PAPER.md at build time) plus the equation they fall in.
+ *
+ * Conventions
+ *   - Every function returns an int: SATSPLAT_OK (0) or a negative SATSPLAT_E_* code.  No exception or C++
+ *     type crosses the ABI.  satsplat_last_error(ctx) returns a message owned by the context.
+ *   - Ownership: the caller owns every input and output buffer.  The opaque satsplat_ctx owns only scratch
+ *     (per-surfel records, tile rects, counts/offsets, key/value double buffers, tile ranges, per-pixel
+ *     state, per-surfel gradient records), sized ONCE at satsplat_create from
+ *     (max_surfels, max_width, max_height, max_duplicates).  The hot calls (preprocess / shadow_map /
+ *     render_forward / render_backward / shadow_map_backward) allocate nothing, never synchronise with the
+ *     host, and enqueue all work on the caller's stream.  Exceeding max_duplicates sets a device flag that
+ *     satsplat_sync_status surfaces as SATSPLAT_E_CAPACITY (outputs of that pass are then undefined but no
+ *     out-of-bounds access happens).
+ *   - One context per camera pass in flight: the view pass and the sun pass of one training iteration use
+ *     two contexts so that both stay alive for the backward.
+ *   - Layouts: fp32, row-major, contiguous, 16-byte aligned device buffers.
+ *       surfels  means[N,3]  quats[N,4] (w,x,y,z; need not be unit)  scales[N,2] (linear, > 0, world units)
+ *                opacity_logits[N]  rgb[N,3]                                        (PAPER.md:69-79 Eq. 3-4, :145)
+ *       images   [H,W,4] float4 groups:
+ *                out_rgba = (I_r, I_g, I_b, A)       Eq. 1 colour (:59) and alpha = 1 - T
+ *                out_geom = (N_x, N_y, N_z, D)       blended world normal (:133) and expected depth sum w z (Eq. 14)
+ *                out_aux  = (median depth, distortion, V, T)   V = sun visibility (:55), T = final transmittance
+ *     Pixel (i,j) has its centre at (i+0.5, j+0.5), x to the right, y down.  F maps WORLD UNITS DIRECTLY TO
+ *     THESE PIXEL COORDINATES (the caller folds the paper's NDC step, :63, into F).
+ *   - Gradient outputs are ACCUMULATED INTO (+=) caller-zeroed buffers, because the view pass and the sun
+ *     pass both contribute to the same surfel gradients.
+ *   - Method constants: 16x16 tiles (:140); sigma = 1/sqrt(2) px (Eq. 12);
+ *     rho cut-off 9; alpha skip 1/255; alpha clamp 0.99; transmittance stop 1e-4; |det| <= 1e-6 => degenerate.
+ */
+#ifndef SATSPLAT_H_
+#define SATSPLAT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SATSPLAT_OK 0
+#define SATSPLAT_E_INVALID (-1)  /* null pointer, bad shape, N or image larger than the context was created for */
+#define SATSPLAT_E_CAPACITY (-2) /* duplicated keys K exceeded max_duplicates (reported by satsplat_sync_status) */
+#define SATSPLAT_E_CUDA (-3)     /* a CUDA runtime call failed; message in satsplat_last_error */
+#define SATSPLAT_E_STATE (-4)    /* calls out of order (e.g. render_forward before preprocess) */
+
+typedef struct satsplat_ctx satsplat_ctx;
+typedef void* satsplat_stream; /* a cudaStream_t (0 = default stream) */
+
+/* One affine camera (PAPER.md:63-65 Eq. 2, :97-105 Eq. 6-7, :155-163 Eq. 15).  HOST struct, passed by pointer. */
+typedef struct {
+  int32_t width, height; /* pixels; tiles are 16x16 (:140) */
+  float F[8];            /* 2x4 row-major [B_xy | b_xy]: world -> pixel                      (Eq. 2, 7) */
+  float dF[8];           /* 2x4 delta; the effective camera is F' = F + dF (fp32 add)        (Eq. 15)   */
+  float view_dir[3];     /* unit viewing direction, sensor -> scene (prop. to B_x x B_y)     (:165)     */
+  float b_z;             /* max_altitude: depth z = b_z - world_z                            (Eq. 11)   */
+  float z_bg;            /* background depth composited behind the last surfel                          */
+  float bg_rgb[3];       /* background albedo                                                           */
+} satsplat_camera;
+
+/* Image formation I = (C A + c) (.) (V + (1 - V) L_a)  (Eq. 1) and the soft shadow test
+ * V = sigmoid(-slope (z_view - d_sun(x_s) - depth_bias)) with x_s = R_x x + k_h h + k_0 (:153, :165-167).
+ * HOST struct; sun_depth is a DEVICE pointer. */
+typedef struct {
+  float cc[12];           /* 3x4 row-major [C | c]; identity + zero bias = no correction */
+  float ambient[3];       /* L_a */
+  int32_t shadows_on;     /* 0: V == 1 everywhere and the sun fields are ignored */
+  int32_t sun_width, sun_height;
+  const float* sun_depth; /* DEVICE [sun_height, sun_width]: background-composited sun-view depth (satsplat_shadow_map) */
+  float reproj[8];        /* 2x4 [R_x | k_h | k_0] from satsplat_sun_camera */
+  float depth_bias, slope;
+} satsplat_shading;
+
+/* ---- lifetime ------------------------------------------------------------------------------------------ */
+/* Allocates all scratch on `device` (cudaMalloc; the only allocating call).  max_duplicates bounds K, the
+ * number of (tile, surfel) pairs of one pass. */
+int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t max_width, int32_t max_height,
+                    int64_t max_duplicates);
+void satsplat_destroy(satsplat_ctx* ctx);
+const char* satsplat_last_error(const satsplat_ctx* ctx); /* never NULL; ctx may be NULL */
+int64_t satsplat_scratch_bytes(const satsplat_ctx* ctx);  /* device bytes owned by the context */
+
+/* ---- camera helper (host arithmetic only) -------------------------------------------------------------- */
+/* Sun-direction affine camera of PAPER.md:165-173 Eq. 16 / :317-345 Eq. S1-S6: B_sun = B' (I - [0 0 s]),
+ * s = (cos(az)/tan(el), sin(az)/tan(el), 1), B' = B + dB of `view`; followed by the 2-D viewport
+ * x_px = viewport[0..1] (.) x + viewport[2..3] that fits the flattened scene into sun_w x sun_h.  Azimuth from +X
+ * toward +Y, elevation above the horizon, radians.  sun_out gets dF = 0, the depth row of `view` (the sun depth
+ * is the original elevation, :167) and view_dir = -(cos az cos el, sin az cos el, sin el).  reproj_out is the
+ * 2x4 map view pixel + height -> sun pixel used by the shadow test.  All HOST pointers. */
+int satsplat_sun_camera(const satsplat_camera* view, float azimuth, float elevation, int32_t sun_w, int32_t sun_h,
+                        const float viewport[4], satsplat_camera* sun_out, float reproj_out[8]);
+
+/* ---- hot path ------------------------------------------------------------------------------------------ */
+/* (a1)+(a2) per-surfel preprocess and binning (PAPER.md:97-131 Eq. 6-12; :140).  Per surfel: rotation from the
+ * quaternion, M = B' R S' (Eq. 8), Q = M^-1 (Eq. 10), centre c, height depth z_c (Eq. 11), depth slope, opacity,
+ * sensor-facing normal, 3-sigma extent widened to the low-pass disc of Eq. 12, tile rect and count; then exclusive
+ * scan, key duplication (tile << 32 | order-preserving depth bits), stable radix sort and per-tile ranges.
+ * All array arguments are DEVICE pointers; `cam` is a HOST pointer.  Requires N <= max_surfels and
+ * cam->width/height <= max_width/max_height.  The five surfel buffers must stay valid and unmodified until the
+ * backward of this pass has been enqueued (the per-surfel chain rule re-reads them). */
+int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
+                        const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
+                        satsplat_stream stream);
+
+/* (a3)+(a5) per-16x16-tile front-to-back compositing (Eq. 14) of colour, alpha, expected depth,
+ * normal, median depth and the depth-distortion term, with the Eq. 1 colour correction and shadow test fused
+ * into the epilogue.  Outputs are DEVICE [H,W,4] buffers (any may be NULL to skip the store); `shading` HOST. */
+int satsplat_render_forward(satsplat_ctx* ctx, const satsplat_shading* shading, float* out_rgba, float* out_geom,
+                            float* out_aux, satsplat_stream stream);
+
+/* Depth-only compositing on a preprocessed SUN context: sun_depth_out[Hs,Ws] = D + T z_bg (DEVICE pointer). */
+int satsplat_shadow_map(satsplat_ctx* sun_ctx, float* sun_depth_out, satsplat_stream stream);
+
+/* (a4) backward of satsplat_render_forward: epilogue backward (v_cc, v_ambient, v_reproj, scatter into
+ * v_sun_depth), compositing backward in reverse order with warp-shuffle reduction before any atomics, then the
+ * per-surfel chain to (means, quats, scales, logits, rgb) and the reduction to v_dF (Eq. 15).
+ * Upstream v_rgba / v_geom / v_aux: DEVICE [H,W,4], any may be NULL (= zero); v_aux channels (d median,
+ * d distortion, ignored, ignored).  All v_* outputs are DEVICE pointers, accumulated into (+=); any may be NULL
+ * (v_sun_depth / v_reproj must be non-NULL only if the caller wants them). */
+int satsplat_render_backward(satsplat_ctx* ctx, const satsplat_shading* shading, const float* v_rgba,
+                             const float* v_geom, const float* v_aux, float* v_means, float* v_quats,
+                             float* v_scales, float* v_opacity_logits, float* v_rgb, float* v_dF /*[8]*/,
+                             float* v_cc /*[12]*/, float* v_ambient /*[3]*/, float* v_sun_depth /*[Hs,Ws]*/,
+                             float* v_reproj /*[8]*/, satsplat_stream stream);
+
+/* Backward of satsplat_shadow_map: v_sun_depth DEVICE [Hs,Ws]; surfel gradients and v_dF_sun (gradient w.r.t.
+ * the sun camera's 2x4) accumulated into DEVICE buffers. */
+int satsplat_shadow_map_backward(satsplat_ctx* sun_ctx, const float* v_sun_depth, float* v_means, float* v_quats,
+                                 float* v_scales, float* v_opacity_logits, float* v_dF_sun /*[8]*/,
+                                 satsplat_stream stream);
+
+/* One whole training-view iteration with HOST buffers (end-to-end leg of the benchmark): copies the surfels and
+ * upstream gradients host->device, runs sun pass (if shading->shadows_on; `sun_cam` then non-NULL and
+ * shading->sun_depth ignored) + view pass forward + backward of both, copies images and gradients back, and
+ * synchronises `stream`.  h_* are HOST pointers (pinned memory recommended); h_grads = packed
+ * [N*13 + 8 + 12 + 3] floats: means(3N) quats(4N) scales(2N) logits(N) rgb(3N) dF(8) cc(12) ambient(3).
+ * `sun_ctx` may be NULL when shadows are off. */
+int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
+                            const satsplat_camera* sun_cam, const satsplat_shading* shading, int64_t N,
+                            const float* h_means, const float* h_quats, const float* h_scales,
+                            const float* h_opacity_logits, const float* h_rgb, const float* h_v_rgba,
+                            const float* h_v_geom, const float* h_v_aux, float* h_out_rgba, float* h_out_geom,
+                            float* h_out_aux, float* h_grads, satsplat_stream stream);
+
+/* ---- status, test and profiling access ------------------------------------------------------------------ */
+/* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
+ * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */
+int satsplat_sync_status(satsplat_ctx* ctx, int64_t* K, satsplat_stream stream);
+
+/* Pointers into the context's scratch for the bit-exact binning checks (DEVICE pointers returned through HOST
+ * pointer arguments; valid until the next preprocess on this context; K read with a stream sync):
+ * keys[K] = (tile << 32) | depth bits, sorted; vals[K] surfel ids; tile_ranges[tiles,2]; rects[N,4] uint16
+ * (tx0,ty0,tx1,ty1); counts[N] uint32. */
+int satsplat_debug_bins(satsplat_ctx* ctx, int64_t* K, const uint64_t** keys, const uint32_t** vals,
+                        const uint32_t** tile_ranges, const uint16_t** rects, const uint32_t** counts,
+                        satsplat_stream stream);
+
+/* Copies the per-surfel records of the last preprocess into records_out (DEVICE [N,16] fp32) in the canonical
+ * order (c_x, c_y, Q00, Q01, Q10, Q11, z_c, g0, g1, alpha, r, g, b, n_x, n_y, n_z) and flags_out (DEVICE [N] uint8:
+ * bit0 culled, bit1 degenerate, bit2 normal flipped). */
+int satsplat_debug_records(satsplat_ctx* ctx, float* records_out, uint8_t* flags_out, satsplat_stream stream);
+
+/* Per-pixel planes of the last forward: n_visited[H,W] (tile-list entries visited, including the one that
+ * triggered the transmittance stop) and n_contrib[H,W] (composited entries); DEVICE int32 pointers owned by
+ * the context.  Their sums are the evaluated / contributing pair counts the roofline is quoted against. */
+int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const int32_t** n_contrib);
+
+/* Per-stage device times of the most recent hot call on this context, measured with CUDA events on the
+ * caller's stream when profiling is enabled (costs event records, no host sync until the query).
+ * Stage ids: SATSPLAT_STAGE_*.  ms_out HOST [SATSPLAT_NUM_STAGES]; stages that did not run report 0. */
+#define SATSPLAT_STAGE_PREPROCESS 0
+#define SATSPLAT_STAGE_SCAN 1
+#define SATSPLAT_STAGE_DUPLICATE 2
+#define SATSPLAT_STAGE_SORT 3
+#define SATSPLAT_STAGE_RANGES 4
+#define SATSPLAT_STAGE_BLEND_FWD 5
+#define SATSPLAT_STAGE_BLEND_BWD 6
+#define SATSPLAT_STAGE_CHAIN_BWD 7
+#define SATSPLAT_NUM_STAGES 8
+int satsplat_set_profiling(satsplat_ctx* ctx, int32_t enabled);
+int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out);
+
+const char* satsplat_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SATSPLAT_H_ */

@@ -1,0 +1,275 @@
+"""paper_2606_28581_b200 — thin Python binding of libsatsplat.so (the C ABI of include/satsplat.h).
+
+Argument marshalling only: every step of the path runs in the hand-written sm_100a kernels under csrc/.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback: if the CUDA library
+is missing or fails to load, importing a compute entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libsatsplat.so")
+_LIB = None
+
+OK, E_INVALID, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4
+STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_fwd", "blend_bwd", "chain_bwd")
+
+
+class SatsplatError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"satsplat error {code}: {msg}")
+        self.code = code
+
+
+class Camera(C.Structure):
+    """satsplat_camera (include/satsplat.h)."""
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("F", C.c_float * 8), ("dF", C.c_float * 8),
+                ("view_dir", C.c_float * 3), ("b_z", C.c_float), ("z_bg", C.c_float), ("bg_rgb", C.c_float * 3)]
+
+    @classmethod
+    def make(cls, width, height, F, dF=None, view_dir=(0, 0, -1), b_z=0.0, z_bg=0.0, bg_rgb=(0, 0, 0)):
+        c = cls()
+        c.width, c.height = int(width), int(height)
+        c.F[:] = [float(x) for x in F]
+        c.dF[:] = [0.0] * 8 if dF is None else [float(x) for x in dF]
+        c.view_dir[:] = [float(x) for x in view_dir]
+        c.b_z, c.z_bg = float(b_z), float(z_bg)
+        c.bg_rgb[:] = [float(x) for x in bg_rgb]
+        return c
+
+    @classmethod
+    def from_view(cls, v):
+        """From a satsplat_scenes.View-like object (duck typed)."""
+        return cls.make(v.width, v.height, v.F, v.dF, v.view_dir, v.b_z, v.z_bg, v.bg_rgb)
+
+
+class Shading(C.Structure):
+    """satsplat_shading (include/satsplat.h)."""
+    _fields_ = [("cc", C.c_float * 12), ("ambient", C.c_float * 3), ("shadows_on", C.c_int32),
+                ("sun_width", C.c_int32), ("sun_height", C.c_int32), ("sun_depth", C.c_void_p),
+                ("reproj", C.c_float * 8), ("depth_bias", C.c_float), ("slope", C.c_float)]
+
+    @classmethod
+    def make(cls, cc=None, ambient=(0, 0, 0), sun_depth=None, reproj=None, depth_bias=0.5, slope=4.0):
+        s = cls()
+        s.cc[:] = [1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0] if cc is None else [float(x) for x in cc]
+        s.ambient[:] = [float(x) for x in ambient]
+        s.shadows_on = 0
+        if sun_depth is not None:
+            _check(sun_depth, torch.float32, 2)
+            s.shadows_on = 1
+            s.sun_height, s.sun_width = int(sun_depth.shape[0]), int(sun_depth.shape[1])
+            s.sun_depth = sun_depth.data_ptr()
+            s._keep = sun_depth
+        s.reproj[:] = [0.0] * 8 if reproj is None else [float(x) for x in reproj]
+        s.depth_bias, s.slope = float(depth_bias), float(slope)
+        return s
+
+
+def build(force: bool = False) -> str:
+    from .build import build as _b
+    return _b(force=force)
+
+
+def lib():
+    """Load libsatsplat.so; raises if it is missing (no fallback path exists)."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(_SO):
+            raise ImportError(f"{_SO} not built: run `python -m paper_2606_28581_b200.build` (needs nvcc); there is no CPU fallback")
+        L = C.CDLL(_SO)
+        L.satsplat_last_error.restype = C.c_char_p
+        L.satsplat_last_error.argtypes = [C.c_void_p]
+        L.satsplat_version.restype = C.c_char_p
+        L.satsplat_scratch_bytes.restype = C.c_int64
+        L.satsplat_scratch_bytes.argtypes = [C.c_void_p]
+        L.satsplat_destroy.restype = None
+        L.satsplat_destroy.argtypes = [C.c_void_p]
+        vp, i64, i32, f32 = C.c_void_p, C.c_int64, C.c_int32, C.c_float
+        L.satsplat_create.argtypes = [C.POINTER(vp), C.c_int, i64, i32, i32, i64]
+        L.satsplat_sun_camera.argtypes = [C.POINTER(Camera), f32, f32, i32, i32, C.POINTER(f32), C.POINTER(Camera), C.POINTER(f32)]
+        L.satsplat_preprocess.argtypes = [vp, C.POINTER(Camera), i64, vp, vp, vp, vp, vp, vp]
+        L.satsplat_render_forward.argtypes = [vp, C.POINTER(Shading), vp, vp, vp, vp]
+        L.satsplat_shadow_map.argtypes = [vp, vp, vp]
+        L.satsplat_render_backward.argtypes = [vp, C.POINTER(Shading)] + [vp] * 14
+        L.satsplat_shadow_map_backward.argtypes = [vp] * 8
+        L.satsplat_iteration_host.argtypes = [vp, vp, C.POINTER(Camera), C.POINTER(Camera), C.POINTER(Shading), i64] + [vp] * 13
+        L.satsplat_sync_status.argtypes = [vp, C.POINTER(i64), vp]
+        L.satsplat_debug_bins.argtypes = [vp, C.POINTER(i64)] + [C.POINTER(vp)] * 5 + [vp]
+        L.satsplat_debug_records.argtypes = [vp, vp, vp, vp]
+        L.satsplat_debug_planes.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+        L.satsplat_set_profiling.argtypes = [vp, i32]
+        L.satsplat_stage_ms.argtypes = [vp, C.POINTER(f32)]
+        _LIB = L
+    return _LIB
+
+
+def version() -> str:
+    return lib().satsplat_version().decode()
+
+
+def _check(t, dtype, ndim=None):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    if ndim is not None and t.dim() != ndim:
+        raise ValueError("expected %d dims" % ndim)
+    return t
+
+
+def _ptr(t, dtype=torch.float32):
+    return None if t is None else _check(t, dtype).data_ptr()
+
+
+class _DevBytes:
+    """Raw device memory exposed through __cuda_array_interface__ so torch can view (then clone) it."""
+
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, True), "version": 2}
+
+
+def _wrap(ptr, nbytes, dev):
+    if nbytes <= 0:
+        return torch.empty(0, dtype=torch.uint8, device=dev)
+    return torch.as_tensor(_DevBytes(ptr, nbytes), device=dev).clone()
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def sun_camera(view: Camera, azimuth, elevation, sun_w, sun_h, viewport):
+    """satsplat_sun_camera: returns (sun Camera, reproj list[8])."""
+    out, rep = Camera(), (C.c_float * 8)()
+    vp = (C.c_float * 4)(*[float(x) for x in viewport])
+    rc = lib().satsplat_sun_camera(C.byref(view), float(azimuth), float(elevation), int(sun_w), int(sun_h), vp, C.byref(out), rep)
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+    return out, list(rep)
+
+
+class Context:
+    """satsplat_ctx: scratch arena for one camera pass (create once, reuse every iteration)."""
+
+    def __init__(self, max_surfels, max_width, max_height, max_duplicates, device=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_28581_b200 needs a CUDA device (there is no CPU fallback)")
+        self._h = C.c_void_p()
+        self.device = int(device)
+        rc = lib().satsplat_create(C.byref(self._h), self.device, int(max_surfels), int(max_width), int(max_height), int(max_duplicates))
+        if rc:
+            raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+        self._keep = {}
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().satsplat_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _rc(self, rc):
+        if rc:
+            raise SatsplatError(rc, lib().satsplat_last_error(self._h).decode())
+
+    @property
+    def scratch_bytes(self):
+        return int(lib().satsplat_scratch_bytes(self._h))
+
+    # ---- hot path ----
+    def preprocess(self, cam: Camera, means, quats, scales, opacity_logits, rgb, stream=None):
+        n = int(means.shape[0])
+        self._keep["in"] = (means, quats, scales, opacity_logits, rgb)   # must outlive the backward
+        self.cam, self.n = cam, n
+        self._rc(lib().satsplat_preprocess(self._h, C.byref(cam), n, _ptr(means), _ptr(quats), _ptr(scales),
+                                           _ptr(opacity_logits), _ptr(rgb), _stream(stream)))
+
+    def render_forward(self, shading: Shading, out_rgba=None, out_geom=None, out_aux=None, stream=None):
+        self._rc(lib().satsplat_render_forward(self._h, C.byref(shading), _ptr(out_rgba), _ptr(out_geom), _ptr(out_aux), _stream(stream)))
+
+    def shadow_map(self, sun_depth_out, stream=None):
+        self._rc(lib().satsplat_shadow_map(self._h, _ptr(sun_depth_out), _stream(stream)))
+
+    def render_backward(self, shading: Shading, v_rgba, v_geom, v_aux, v_means, v_quats, v_scales, v_opacity_logits, v_rgb,
+                        v_dF=None, v_cc=None, v_ambient=None, v_sun_depth=None, v_reproj=None, stream=None):
+        self._rc(lib().satsplat_render_backward(self._h, C.byref(shading), _ptr(v_rgba), _ptr(v_geom), _ptr(v_aux), _ptr(v_means),
+                                                _ptr(v_quats), _ptr(v_scales), _ptr(v_opacity_logits), _ptr(v_rgb), _ptr(v_dF),
+                                                _ptr(v_cc), _ptr(v_ambient), _ptr(v_sun_depth), _ptr(v_reproj), _stream(stream)))
+
+    def shadow_map_backward(self, v_sun_depth, v_means, v_quats, v_scales, v_opacity_logits, v_dF_sun=None, stream=None):
+        self._rc(lib().satsplat_shadow_map_backward(self._h, _ptr(v_sun_depth), _ptr(v_means), _ptr(v_quats), _ptr(v_scales),
+                                                    _ptr(v_opacity_logits), _ptr(v_dF_sun), _stream(stream)))
+
+    # ---- status / test access ----
+    def sync_status(self, stream=None) -> int:
+        k = C.c_int64()
+        self._rc(lib().satsplat_sync_status(self._h, C.byref(k), _stream(stream)))
+        return int(k.value)
+
+    def debug_bins(self, stream=None):
+        """Copies of (keys[K] int64-viewed uint64, vals[K], ranges[tiles,2], rects[N,4], counts[N]) as torch tensors."""
+        k = C.c_int64()
+        ptrs = [C.c_void_p() for _ in range(5)]
+        self._rc(lib().satsplat_debug_bins(self._h, C.byref(k), *[C.byref(p) for p in ptrs], _stream(stream)))
+        K = int(k.value)
+        tiles = ((self.cam.width + 15) // 16) * ((self.cam.height + 15) // 16)
+        dev = torch.device("cuda", self.device)
+
+        def copy(ptr, nbytes, dtype):
+            return _wrap(ptr.value, nbytes, dev).view(dtype)
+
+        keys = copy(ptrs[0], K * 8, torch.int64)
+        vals = copy(ptrs[1], K * 4, torch.int32)
+        ranges = copy(ptrs[2], tiles * 8, torch.int32).view(tiles, 2)
+        rects = copy(ptrs[3], self.n * 8, torch.int16).view(self.n, 4)
+        counts = copy(ptrs[4], self.n * 4, torch.int32)
+        return K, keys, vals, ranges, rects, counts
+
+    def debug_records(self, stream=None):
+        dev = torch.device("cuda", self.device)
+        rec = torch.empty(self.n, 16, dtype=torch.float32, device=dev)
+        flags = torch.empty(self.n, dtype=torch.uint8, device=dev)
+        self._rc(lib().satsplat_debug_records(self._h, rec.data_ptr(), flags.data_ptr(), _stream(stream)))
+        return rec, flags
+
+    def debug_planes(self):
+        """(n_visited[H,W], n_contrib[H,W]) int32 copies."""
+        a, b = C.c_void_p(), C.c_void_p()
+        self._rc(lib().satsplat_debug_planes(self._h, C.byref(a), C.byref(b)))
+        H, W = self.cam.height, self.cam.width
+        dev = torch.device("cuda", self.device)
+        torch.cuda.synchronize()
+        outs = [_wrap(p.value, H * W * 4, dev).view(torch.int32).view(H, W) for p in (a, b)]
+        return outs
+
+    def set_profiling(self, enabled: bool):
+        self._rc(lib().satsplat_set_profiling(self._h, 1 if enabled else 0))
+
+    def stage_ms(self):
+        ms = (C.c_float * len(STAGES))()
+        self._rc(lib().satsplat_stage_ms(self._h, ms))
+        return dict(zip(STAGES, [float(x) for x in ms]))
+
+
+def iteration_host(ctx: Context, sun_ctx, cam: Camera, sun_cam, shading: Shading, n, h_means, h_quats, h_scales, h_logits,
+                   h_rgb, h_v_rgba, h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, stream=None):
+    """satsplat_iteration_host: one full training-view iteration with HOST (pinned CPU) tensors."""
+    def hp(t):
+        if t is None:
+            return None
+        if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+            raise ValueError("expected contiguous fp32 CPU tensors")
+        return t.data_ptr()
+    rc = lib().satsplat_iteration_host(ctx._h, None if sun_ctx is None else sun_ctx._h, C.byref(cam),
+                                       None if sun_cam is None else C.byref(sun_cam), C.byref(shading), int(n), hp(h_means),
+                                       hp(h_quats), hp(h_scales), hp(h_logits), hp(h_rgb), hp(h_v_rgba), hp(h_v_geom),
+                                       hp(h_v_aux), hp(h_out_rgba), hp(h_out_geom), hp(h_out_aux), hp(h_grads), _stream(stream))
+    ctx._rc(rc)

@@ -1,0 +1,456 @@
+// api.cu — the C ABI of include/satsplat.h: context (scratch arena), argument checks, launch sequencing.
+// No kernel lives here; every step of the path runs in the kernels of the other translation units.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "internal.cuh"
+
+using namespace satsplat;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(satsplat_ctx* c, int code, const char* fmt, const char* a = "") {
+  char* dst = c ? c->err : g_err;
+  snprintf(dst, 512, fmt, a);
+  return code;
+}
+
+#define CU(call)                                                                       \
+  do {                                                                                 \
+    cudaError_t e_ = (call);                                                           \
+    if (e_ != cudaSuccess) return fail(ctx, SATSPLAT_E_CUDA, #call ": %s", cudaGetErrorString(e_)); \
+  } while (0)
+
+template <typename T>
+cudaError_t dalloc(satsplat_ctx* c, T** p, size_t n) {
+  const size_t bytes = ((n * sizeof(T) + 255) / 256) * 256;
+  cudaError_t e = cudaMalloc((void**)p, bytes ? bytes : 256);
+  if (e == cudaSuccess) c->scratch_bytes += (int64_t)(bytes ? bytes : 256);
+  return e;
+}
+
+void set_camera(satsplat_ctx* c, const satsplat_camera* cam) {
+  DevCamera& d = c->cam;
+  d.W = cam->width;
+  d.H = cam->height;
+  d.TX = (cam->width + kTile - 1) / kTile;
+  d.TY = (cam->height + kTile - 1) / kTile;
+  for (int i = 0; i < 8; ++i) d.Fp[i] = cam->F[i] + cam->dF[i];  // Eq. 15 (one fp32 rounding)
+  for (int i = 0; i < 3; ++i) d.vd[i] = cam->view_dir[i];
+  d.b_z = cam->b_z;
+  d.z_bg = cam->z_bg;
+  for (int i = 0; i < 3; ++i) d.bg[i] = cam->bg_rgb[i];
+}
+
+DevShading make_shading(const satsplat_shading* s) {
+  DevShading d;
+  memset(&d, 0, sizeof(d));
+  if (!s) {
+    d.cc[0] = d.cc[5] = d.cc[10] = 1.f;
+    return d;
+  }
+  memcpy(d.cc, s->cc, sizeof(d.cc));
+  memcpy(d.ambient, s->ambient, sizeof(d.ambient));
+  d.shadows_on = s->shadows_on ? 1 : 0;
+  d.sun_w = s->sun_width;
+  d.sun_h = s->sun_height;
+  d.sun_depth = s->sun_depth;
+  memcpy(d.reproj, s->reproj, sizeof(d.reproj));
+  d.bias = s->depth_bias;
+  d.slope = s->slope;
+  return d;
+}
+
+struct StageTimer {
+  satsplat_ctx* c;
+  cudaStream_t s;
+  int stage;
+  StageTimer(satsplat_ctx* c_, int stage_, cudaStream_t s_) : c(c_), s(s_), stage(stage_) {
+    if (c->profiling) { cudaEventRecord(c->ev[2 * stage], s); }
+  }
+  ~StageTimer() {
+    if (c->profiling) { cudaEventRecord(c->ev[2 * stage + 1], s); c->ev_used[stage] = 1; }
+  }
+};
+
+void clear_stage_marks(satsplat_ctx* c, std::initializer_list<int> stages) {
+  for (int s : stages) c->ev_used[s] = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* satsplat_version(void) { return "satsplat-b200 0.1 (sm_100a)"; }
+
+const char* satsplat_last_error(const satsplat_ctx* ctx) { return ctx ? ctx->err : g_err; }
+
+int64_t satsplat_scratch_bytes(const satsplat_ctx* ctx) { return ctx ? ctx->scratch_bytes : 0; }
+
+int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t max_w, int32_t max_h,
+                    int64_t max_dup) {
+  if (!out) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_create: out is NULL");
+  *out = nullptr;
+  if (max_surfels < 0 || max_surfels >= (1ll << 31) || max_w <= 0 || max_h <= 0 || max_dup < 0 || max_dup >= (1ll << 32) - 1 ||
+      max_w > 65535 * kTile || max_h > 65535 * kTile)
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_create: size out of range");
+  satsplat_ctx* ctx = (satsplat_ctx*)calloc(1, sizeof(satsplat_ctx));
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_create: out of host memory");
+  ctx->device = device;
+  ctx->max_surfels = max_surfels;
+  ctx->max_dup = max_dup;
+  ctx->max_w = max_w;
+  ctx->max_h = max_h;
+  cudaError_t e = cudaSetDevice(device);
+  const size_t N = (size_t)max_surfels, K = (size_t)max_dup;
+  const size_t tiles = (size_t)((max_w + kTile - 1) / kTile) * (size_t)((max_h + kTile - 1) / kTile);
+  const size_t px = (size_t)max_w * (size_t)max_h;
+#define A(call) if (e == cudaSuccess) e = (call)
+  A(dalloc(ctx, &ctx->rec, N * 4));
+  A(dalloc(ctx, &ctx->rect, N * 4));
+  A(dalloc(ctx, &ctx->count, N));
+  A(dalloc(ctx, &ctx->offset, N + 1));
+  A(dalloc(ctx, &ctx->depth_key, N));
+  A(dalloc(ctx, &ctx->flags, N));
+  A(dalloc(ctx, &ctx->vrec, N * 16));
+  A(dalloc(ctx, &ctx->block_sums, N / 4096 + 2));
+  A(dalloc(ctx, &ctx->keys[0], K));
+  A(dalloc(ctx, &ctx->keys[1], K));
+  A(dalloc(ctx, &ctx->vals[0], K));
+  A(dalloc(ctx, &ctx->vals[1], K));
+  A(dalloc(ctx, &ctx->hist, (size_t)256 * kSortBlocks));
+  A(dalloc(ctx, &ctx->ranges, tiles * 2));
+  A(dalloc(ctx, &ctx->status, 1));
+  A(dalloc(ctx, &ctx->px_a, px));
+  A(dalloc(ctx, &ctx->px_b, px));
+  A(dalloc(ctx, &ctx->px_i, px));
+  A(dalloc(ctx, &ctx->px_visited, px));
+  A(dalloc(ctx, &ctx->px_contrib, px));
+  A(dalloc(ctx, &ctx->red_buf, 64));
+  A(cudaMemset(ctx->vrec, 0, N * 16 * sizeof(float) ? N * 16 * sizeof(float) : 4));
+  A(cudaMemset(ctx->status, 0, sizeof(Status)));
+  for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i) A(cudaEventCreate(&ctx->ev[i]));
+#undef A
+  if (e != cudaSuccess) {
+    fail(nullptr, SATSPLAT_E_CUDA, "satsplat_create: %s", cudaGetErrorString(e));
+    satsplat_destroy(ctx);
+    return SATSPLAT_E_CUDA;
+  }
+  strcpy(ctx->err, "ok");
+  *out = ctx;
+  return SATSPLAT_OK;
+}
+
+void satsplat_destroy(satsplat_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  void* ptrs[] = {ctx->rec, ctx->rect, ctx->count, ctx->offset, ctx->depth_key, ctx->flags, ctx->vrec, ctx->block_sums,
+                  ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->px_a,
+                  ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in, ctx->e2e_up,
+                  ctx->e2e_out, ctx->e2e_grads};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
+    if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  free(ctx);
+}
+
+int satsplat_sun_camera(const satsplat_camera* view, float azimuth, float elevation, int32_t sun_w, int32_t sun_h,
+                        const float viewport[4], satsplat_camera* sun_out, float reproj_out[8]) {
+  if (!view || !viewport || !sun_out || !reproj_out || sun_w <= 0 || sun_h <= 0)
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: bad argument");
+  const double te = tan((double)elevation);
+  if (!(fabs(te) > 1e-12)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: elevation must be non-zero");
+  double Fp[8];
+  for (int i = 0; i < 8; ++i) Fp[i] = (double)(float)(view->F[i] + view->dF[i]);  // the camera the rasteriser uses
+  const double s[3] = {cos((double)azimuth) / te, sin((double)azimuth) / te, 1.0};  // Eq. S2
+  double S[2][4];
+  for (int r = 0; r < 2; ++r) {
+    const double* B = Fp + 4 * r;
+    const double Bs = B[0] * s[0] + B[1] * s[1] + B[2] * s[2];
+    const double sc = viewport[r], tr = viewport[2 + r];
+    S[r][0] = sc * B[0];
+    S[r][1] = sc * B[1];
+    S[r][2] = sc * (B[2] - Bs);  // Eq. 16: B (I - [0 0 s])
+    S[r][3] = sc * B[3] + tr;
+  }
+  const double det = Fp[0] * Fp[5] - Fp[1] * Fp[4];
+  if (!(fabs(det) > 0)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: singular view camera");
+  const double Bi[2][2] = {{Fp[5] / det, -Fp[1] / det}, {-Fp[4] / det, Fp[0] / det}};
+  memset(sun_out, 0, sizeof(*sun_out));
+  sun_out->width = sun_w;
+  sun_out->height = sun_h;
+  for (int r = 0; r < 2; ++r) {
+    for (int c = 0; c < 4; ++c) sun_out->F[4 * r + c] = (float)S[r][c];
+    const double Rx0 = S[r][0] * Bi[0][0] + S[r][1] * Bi[1][0];
+    const double Rx1 = S[r][0] * Bi[0][1] + S[r][1] * Bi[1][1];
+    reproj_out[4 * r + 0] = (float)Rx0;
+    reproj_out[4 * r + 1] = (float)Rx1;
+    reproj_out[4 * r + 2] = (float)(S[r][2] - (Rx0 * Fp[2] + Rx1 * Fp[6]));
+    reproj_out[4 * r + 3] = (float)(S[r][3] - (Rx0 * Fp[3] + Rx1 * Fp[7]));
+  }
+  const double ce = cos((double)elevation);
+  sun_out->view_dir[0] = (float)(-cos((double)azimuth) * ce);
+  sun_out->view_dir[1] = (float)(-sin((double)azimuth) * ce);
+  sun_out->view_dir[2] = (float)(-sin((double)elevation));
+  sun_out->b_z = view->b_z;
+  sun_out->z_bg = view->z_bg;
+  return SATSPLAT_OK;
+}
+
+int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
+                        const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
+                        satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_preprocess: ctx is NULL");
+  if (!cam || N < 0 || (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb)))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: NULL argument");
+  if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: N exceeds max_surfels");
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > ctx->max_w || cam->height > ctx->max_h)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: image size exceeds the context");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  set_camera(ctx, cam);
+  ctx->N = N;
+  ctx->in_means = means; ctx->in_quats = quats; ctx->in_scales = scales; ctx->in_logits = opacity_logits;
+  ctx->preprocessed = 0;
+  ctx->forwarded = 0;
+  clear_stage_marks(ctx, {0, 1, 2, 3, 4, 5, 6, 7});
+  { StageTimer t(ctx, SATSPLAT_STAGE_PREPROCESS, s); CU(launch_preprocess(ctx, N, means, quats, scales, opacity_logits, rgb, s)); }
+  { StageTimer t(ctx, SATSPLAT_STAGE_SCAN, s); CU(launch_scan(ctx, N, s)); }
+  { StageTimer t(ctx, SATSPLAT_STAGE_DUPLICATE, s); CU(launch_duplicate(ctx, N, s)); }
+  { StageTimer t(ctx, SATSPLAT_STAGE_SORT, s); CU(launch_sort(ctx, s)); }
+  { StageTimer t(ctx, SATSPLAT_STAGE_RANGES, s); CU(launch_ranges(ctx, s)); }
+  ctx->preprocessed = 1;
+  return SATSPLAT_OK;
+}
+
+int satsplat_render_forward(satsplat_ctx* ctx, const satsplat_shading* shading, float* out_rgba, float* out_geom,
+                            float* out_aux, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_forward: ctx is NULL");
+  if (!ctx->preprocessed) return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_forward: call satsplat_preprocess first");
+  if (shading && shading->shadows_on && (!shading->sun_depth || shading->sun_width <= 0 || shading->sun_height <= 0))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_forward: shadows_on without a sun depth map");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  const DevShading sh = make_shading(shading);
+  clear_stage_marks(ctx, {5, 6, 7});
+  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, out_rgba, out_geom, out_aux, nullptr, false, s)); }
+  ctx->forwarded = 1;
+  ctx->depth_only = 0;
+  return SATSPLAT_OK;
+}
+
+int satsplat_shadow_map(satsplat_ctx* ctx, float* sun_depth_out, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_shadow_map: ctx is NULL");
+  if (!sun_depth_out) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_shadow_map: output is NULL");
+  if (!ctx->preprocessed) return fail(ctx, SATSPLAT_E_STATE, "satsplat_shadow_map: call satsplat_preprocess first");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  const DevShading sh = make_shading(nullptr);
+  clear_stage_marks(ctx, {5, 6, 7});
+  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, nullptr, nullptr, nullptr, sun_depth_out, true, s)); }
+  ctx->forwarded = 1;
+  ctx->depth_only = 1;
+  return SATSPLAT_OK;
+}
+
+int satsplat_render_backward(satsplat_ctx* ctx, const satsplat_shading* shading, const float* v_rgba,
+                             const float* v_geom, const float* v_aux, float* v_means, float* v_quats,
+                             float* v_scales, float* v_opacity_logits, float* v_rgb, float* v_dF, float* v_cc,
+                             float* v_ambient, float* v_sun_depth, float* v_reproj, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_backward: ctx is NULL");
+  if (!ctx->forwarded || ctx->depth_only)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_backward: call satsplat_render_forward first");
+  if (shading && shading->shadows_on && !shading->sun_depth)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_backward: shadows_on without a sun depth map");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  const DevShading sh = make_shading(shading);
+  clear_stage_marks(ctx, {6, 7});
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
+    CU(launch_blend_backward(ctx, sh, v_rgba, v_geom, v_aux, nullptr, false, v_cc, v_ambient, v_sun_depth, v_reproj, s));
+    if (v_cc) CU(launch_add_small(v_cc, ctx->red_buf, 12, s));
+    if (v_ambient) CU(launch_add_small(v_ambient, ctx->red_buf + 12, 3, s));
+    if (v_reproj) CU(launch_add_small(v_reproj, ctx->red_buf + 15, 8, s));
+  }
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
+    CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
+                             v_opacity_logits, v_rgb, v_dF, s));
+  }
+  return SATSPLAT_OK;
+}
+
+int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, float* v_means, float* v_quats,
+                                 float* v_scales, float* v_opacity_logits, float* v_dF_sun, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_shadow_map_backward: ctx is NULL");
+  if (!v_sun_depth) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_shadow_map_backward: v_sun_depth is NULL");
+  if (!ctx->forwarded || !ctx->depth_only)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_shadow_map_backward: call satsplat_shadow_map first");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  const DevShading sh = make_shading(nullptr);
+  clear_stage_marks(ctx, {6, 7});
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
+    CU(launch_blend_backward(ctx, sh, nullptr, nullptr, nullptr, v_sun_depth, true, nullptr, nullptr, nullptr, nullptr, s));
+  }
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
+    CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
+                             v_opacity_logits, nullptr, v_dF_sun, s));
+  }
+  return SATSPLAT_OK;
+}
+
+int satsplat_sync_status(satsplat_ctx* ctx, int64_t* K, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sync_status: ctx is NULL");
+  CU(cudaSetDevice(ctx->device));
+  Status st;
+  CU(cudaMemcpyAsync(&st, ctx->status, sizeof(Status), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  if (K) *K = (int64_t)st.K;
+  if (st.overflow) return fail(ctx, SATSPLAT_E_CAPACITY, "duplicated keys exceed max_duplicates");
+  return SATSPLAT_OK;
+}
+
+int satsplat_debug_bins(satsplat_ctx* ctx, int64_t* K, const uint64_t** keys, const uint32_t** vals,
+                        const uint32_t** tile_ranges, const uint16_t** rects, const uint32_t** counts,
+                        satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_debug_bins: ctx is NULL");
+  if (!ctx->preprocessed) return fail(ctx, SATSPLAT_E_STATE, "satsplat_debug_bins: call satsplat_preprocess first");
+  int64_t k = 0;
+  const int rc = satsplat_sync_status(ctx, &k, stream);
+  if (K) *K = k;
+  if (keys) *keys = ctx->keys[ctx->sorted];
+  if (vals) *vals = ctx->vals[ctx->sorted];
+  if (tile_ranges) *tile_ranges = ctx->ranges;
+  if (rects) *rects = ctx->rect;
+  if (counts) *counts = ctx->count;
+  return rc;
+}
+
+int satsplat_debug_records(satsplat_ctx* ctx, float* records_out, uint8_t* flags_out, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_debug_records: ctx is NULL");
+  if (!records_out) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_debug_records: records_out is NULL");
+  if (!ctx->preprocessed) return fail(ctx, SATSPLAT_E_STATE, "satsplat_debug_records: call satsplat_preprocess first");
+  CU(cudaSetDevice(ctx->device));
+  CU(launch_export_records(ctx, records_out, flags_out, (cudaStream_t)stream));
+  return SATSPLAT_OK;
+}
+
+int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const int32_t** n_contrib) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_debug_planes: ctx is NULL");
+  if (!ctx->forwarded) return fail(ctx, SATSPLAT_E_STATE, "satsplat_debug_planes: no forward pass yet");
+  if (n_visited) *n_visited = ctx->px_visited;
+  if (n_contrib) *n_contrib = ctx->px_contrib;
+  return SATSPLAT_OK;
+}
+
+int satsplat_set_profiling(satsplat_ctx* ctx, int32_t enabled) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_set_profiling: ctx is NULL");
+  ctx->profiling = enabled ? 1 : 0;
+  for (int i = 0; i < SATSPLAT_NUM_STAGES; ++i) ctx->ev_used[i] = 0;
+  return SATSPLAT_OK;
+}
+
+int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out) {
+  if (!ctx || !ms_out) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_stage_ms: NULL argument");
+  CU(cudaSetDevice(ctx->device));
+  for (int i = 0; i < SATSPLAT_NUM_STAGES; ++i) {
+    ms_out[i] = 0.f;
+    if (ctx->profiling && ctx->ev_used[i]) {
+      CU(cudaEventSynchronize(ctx->ev[2 * i + 1]));
+      CU(cudaEventElapsedTime(&ms_out[i], ctx->ev[2 * i], ctx->ev[2 * i + 1]));
+    }
+  }
+  return SATSPLAT_OK;
+}
+
+int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
+                            const satsplat_camera* sun_cam, const satsplat_shading* shading, int64_t N,
+                            const float* h_means, const float* h_quats, const float* h_scales,
+                            const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                            const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                            float* h_grads, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_iteration_host: ctx is NULL");
+  if (!cam || !shading || !h_means || !h_quats || !h_scales || !h_logits || !h_rgb || !h_grads || N <= 0)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: NULL argument");
+  if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: N exceeds max_surfels");
+  const bool shadows = shading->shadows_on != 0;
+  if (shadows && (!sun_ctx || !sun_cam)) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: shadows need sun_ctx and sun_cam");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  const size_t n = (size_t)N, px = (size_t)cam->width * cam->height;
+  const size_t spx = shadows ? (size_t)sun_cam->width * sun_cam->height : 0;
+  if (!ctx->e2e_in) {  // staging buffers: allocated on first use, sized for the context's maxima
+    const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
+    CU(dalloc(ctx, &ctx->e2e_in, (size_t)ctx->max_surfels * 13));
+    CU(dalloc(ctx, &ctx->e2e_up, mpx * 12));
+    CU(dalloc(ctx, &ctx->e2e_out, mpx * 12));
+    CU(dalloc(ctx, &ctx->e2e_grads, (size_t)ctx->max_surfels * 13 + 32));
+  }
+  float* d_means = ctx->e2e_in;
+  float* d_quats = d_means + 3 * (size_t)ctx->max_surfels;
+  float* d_scales = d_quats + 4 * (size_t)ctx->max_surfels;
+  float* d_logits = d_scales + 2 * (size_t)ctx->max_surfels;
+  float* d_rgb = d_logits + (size_t)ctx->max_surfels;
+  CU(cudaMemcpyAsync(d_means, h_means, n * 12, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(d_quats, h_quats, n * 16, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(d_scales, h_scales, n * 8, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(d_logits, h_logits, n * 4, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(d_rgb, h_rgb, n * 12, cudaMemcpyHostToDevice, s));
+  float* d_up[3] = {nullptr, nullptr, nullptr};
+  const float* h_up[3] = {h_v_rgba, h_v_geom, h_v_aux};
+  for (int k = 0; k < 3; ++k)
+    if (h_up[k]) {
+      d_up[k] = ctx->e2e_up + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+      CU(cudaMemcpyAsync(d_up[k], h_up[k], px * 16, cudaMemcpyHostToDevice, s));
+    }
+  float* d_out[3];
+  for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+  float* g = ctx->e2e_grads;
+  CU(cudaMemsetAsync(g, 0, (n * 13 + 23) * sizeof(float), s));
+  float *g_means = g, *g_quats = g + 3 * n, *g_scales = g + 7 * n, *g_logits = g + 9 * n, *g_rgb = g + 10 * n;
+  float *g_dF = g + 13 * n, *g_cc = g_dF + 8, *g_amb = g_cc + 12;
+  satsplat_shading sh = *shading;
+  float* d_sun = nullptr;
+  float* d_vsun = nullptr;
+  int rc;
+  if (shadows) {
+    if (!sun_ctx->e2e_out) {
+      const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
+      CU(dalloc(sun_ctx, &sun_ctx->e2e_out, mpx * 2));
+    }
+    d_sun = sun_ctx->e2e_out;
+    d_vsun = d_sun + (size_t)sun_ctx->max_w * sun_ctx->max_h;
+    if ((rc = satsplat_preprocess(sun_ctx, sun_cam, N, d_means, d_quats, d_scales, d_logits, d_rgb, stream))) return rc;
+    if ((rc = satsplat_shadow_map(sun_ctx, d_sun, stream))) return rc;
+    CU(cudaMemsetAsync(d_vsun, 0, spx * sizeof(float), s));
+    sh.sun_depth = d_sun;
+    sh.sun_width = sun_cam->width;
+    sh.sun_height = sun_cam->height;
+  }
+  if ((rc = satsplat_preprocess(ctx, cam, N, d_means, d_quats, d_scales, d_logits, d_rgb, stream))) return rc;
+  if ((rc = satsplat_render_forward(ctx, &sh, d_out[0], d_out[1], d_out[2], stream))) return rc;
+  if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_means, g_quats, g_scales, g_logits, g_rgb, g_dF,
+                                     g_cc, g_amb, d_vsun, nullptr, stream)))
+    return rc;
+  if (shadows) {
+    // the sun camera is derived from F' (cascade, Fig. 1); its 2x4 gradient is not chained here (NEXT-2)
+    if ((rc = satsplat_shadow_map_backward(sun_ctx, d_vsun, g_means, g_quats, g_scales, g_logits, nullptr, stream))) return rc;
+  }
+  float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};
+  for (int k = 0; k < 3; ++k)
+    if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s));
+  CU(cudaMemcpyAsync(h_grads, g, (n * 13 + 23) * sizeof(float), cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  return SATSPLAT_OK;
+}
+
+}  // extern "C"

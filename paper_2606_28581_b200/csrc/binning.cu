@@ -1,0 +1,346 @@
+// binning.cu — (a2) exclusive scan of tile counts, key duplication, stable LSD radix sort of
+// (tile id << 32 | depth bits) keys with surfel-id payloads, and per-tile range detection (PAPER.md:140:
+// "sorted based on the depth of their centers and organized into tiles").  Integer work: bit-exact.
+//
+// No host synchronisation anywhere: K (the number of duplicated keys) lives in device memory, every kernel
+// below runs on a fixed grid and reads K itself.  All stages are HBM/L2-bandwidth bound.
+#include "internal.cuh"
+
+namespace satsplat {
+
+// ------------------------------------------------------------------------------------------------------------
+// exclusive scan of count[N] -> offset[N+1]; three small kernels (block sums, top-level scan, apply)
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;
+constexpr int kScanTile = kScanThreads * kScanItems;  // 4096
+
+__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += t;
+  }
+  return v;
+}
+
+// block-wide exclusive scan of one value per thread (256 threads); returns exclusive prefix, total in *total
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s_warp, uint32_t* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t inc = warp_inclusive_scan(v, lane);
+  if (lane == 31) s_warp[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    const uint32_t w = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0u;
+    const uint32_t wi = warp_inclusive_scan(w, lane);
+    s_warp[lane] = wi - w;
+    if (lane == 31) s_warp[32] = wi;
+  }
+  __syncthreads();
+  const uint32_t res = s_warp[warp] + inc - v;
+  *total = s_warp[32];
+  __syncthreads();
+  return res;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_block_sums_kernel(int N, const uint32_t* __restrict__ count,
+                                                                       uint32_t* __restrict__ block_sums) {
+  __shared__ uint32_t s_warp[33];
+  const int base = blockIdx.x * kScanTile;
+  uint32_t sum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    const int i = base + k * kScanThreads + threadIdx.x;
+    if (i < N) sum += count[i];
+  }
+  uint32_t total;
+  block_exclusive_scan(sum, s_warp, &total);
+  if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) scan_top_kernel(int nblocks, uint32_t* __restrict__ block_sums, Status* status,
+                                                         uint32_t capacity) {
+  __shared__ uint32_t s_warp[33];
+  // one block; each thread owns a contiguous chunk
+  const int per = (nblocks + 1023) / 1024;
+  const int b0 = threadIdx.x * per;
+  uint32_t sum = 0;
+  for (int k = 0; k < per; ++k)
+    if (b0 + k < nblocks) sum += block_sums[b0 + k];
+  uint32_t total;
+  uint32_t run = block_exclusive_scan(sum, s_warp, &total);
+  for (int k = 0; k < per; ++k)
+    if (b0 + k < nblocks) {
+      const uint32_t v = block_sums[b0 + k];
+      block_sums[b0 + k] = run;
+      run += v;
+    }
+  if (threadIdx.x == 0) {
+    status->K = total;
+    status->overflow = total > capacity ? 1u : 0u;
+  }
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(int N, const uint32_t* __restrict__ count,
+                                                                  const uint32_t* __restrict__ block_sums,
+                                                                  uint32_t* __restrict__ offset) {
+  __shared__ uint32_t s_warp[33];
+  // blocked arrangement: thread t owns items [t*16, t*16+16) of the tile so that a single block scan suffices
+  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+  uint32_t v[kScanItems];
+  uint32_t sum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; k += 4) {
+    if (base + k + 3 < N) {
+      const uint4 t = *reinterpret_cast<const uint4*>(count + base + k);
+      v[k] = t.x; v[k + 1] = t.y; v[k + 2] = t.z; v[k + 3] = t.w;
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[k + j] = (base + k + j < N) ? count[base + k + j] : 0u;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) sum += v[k];
+  uint32_t total;
+  uint32_t run = block_exclusive_scan(sum, s_warp, &total) + block_sums[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    if (base + k < N) offset[base + k] = run;
+    run += v[k];
+  }
+  if (base <= N - 1 && base + kScanItems > N - 1) offset[N] = run;  // total after the last element
+}
+
+cudaError_t launch_scan(satsplat_ctx* c, int64_t N, cudaStream_t s) {
+  const int nblocks = (int)((N + kScanTile - 1) / kScanTile);
+  if (nblocks == 0) {
+    cudaMemsetAsync(c->status, 0, sizeof(Status), s);
+    return cudaMemsetAsync(c->offset, 0, sizeof(uint32_t), s);
+  }
+  scan_block_sums_kernel<<<nblocks, kScanThreads, 0, s>>>((int)N, c->count, c->block_sums);
+  scan_top_kernel<<<1, 1024, 0, s>>>(nblocks, c->block_sums, c->status, (uint32_t)c->max_dup);
+  scan_apply_kernel<<<nblocks, kScanThreads, 0, s>>>((int)N, c->count, c->block_sums, c->offset);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// key duplication: surfel i writes count[i] keys (row-major over its tile rect) at offset[i].  One warp per 32
+// surfels; surfels with many tiles are expanded cooperatively by the whole warp so that no thread serialises a
+// 4000-tile splat (oversized Gaussians).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kDupCoopThreshold = 16;
+
+__global__ void __launch_bounds__(256) duplicate_kernel(int N, int TX, const ushort4* __restrict__ rect,
+                                                        const uint32_t* __restrict__ count,
+                                                        const uint32_t* __restrict__ offset,
+                                                        const uint32_t* __restrict__ depth_key, uint64_t* __restrict__ keys,
+                                                        uint32_t* __restrict__ vals, uint32_t capacity) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  uint32_t cnt = 0, off = 0, dk = 0;
+  ushort4 r = make_ushort4(0, 0, 0, 0);
+  if (i < N) {
+    cnt = count[i];
+    if (cnt) { off = offset[i]; dk = depth_key[i]; r = rect[i]; }
+  }
+  if (cnt && off + cnt > capacity) cnt = 0;  // overflow: flagged by the scan, nothing written out of bounds
+  // small splats: the owning thread writes them
+  if (cnt && cnt <= kDupCoopThreshold) {
+    uint32_t o = off;
+    for (int ty = r.y; ty < r.w; ++ty)
+      for (int tx = r.x; tx < r.z; ++tx) {
+        keys[o] = ((uint64_t)(uint32_t)(ty * TX + tx) << 32) | dk;
+        vals[o] = (uint32_t)i;
+        ++o;
+      }
+  }
+  // large splats: whole warp, coalesced
+  unsigned big = __ballot_sync(0xffffffffu, cnt > kDupCoopThreshold);
+  while (big) {
+    const int src = __ffs(big) - 1;
+    big &= big - 1;
+    const uint32_t c2 = __shfl_sync(0xffffffffu, cnt, src);
+    const uint32_t o2 = __shfl_sync(0xffffffffu, off, src);
+    const uint32_t k2 = __shfl_sync(0xffffffffu, dk, src);
+    const int x0 = __shfl_sync(0xffffffffu, (int)r.x, src), y0 = __shfl_sync(0xffffffffu, (int)r.y, src);
+    const int x1 = __shfl_sync(0xffffffffu, (int)r.z, src);
+    const int id = (blockIdx.x * blockDim.x + (threadIdx.x & ~31)) + src;
+    const int w = x1 - x0;
+    for (uint32_t e = lane; e < c2; e += 32) {
+      const int ty = y0 + (int)(e / (uint32_t)w), tx = x0 + (int)(e % (uint32_t)w);
+      keys[o2 + e] = ((uint64_t)(uint32_t)(ty * TX + tx) << 32) | k2;
+      vals[o2 + e] = (uint32_t)id;
+    }
+  }
+}
+
+cudaError_t launch_duplicate(satsplat_ctx* c, int64_t N, cudaStream_t s) {
+  if (N == 0) return cudaSuccess;
+  duplicate_kernel<<<(int)((N + 255) / 256), 256, 0, s>>>((int)N, c->cam.TX, reinterpret_cast<const ushort4*>(c->rect),
+                                                          c->count, c->offset, c->depth_key, c->keys[0], c->vals[0],
+                                                          (uint32_t)c->max_dup);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// stable LSD radix sort, 8 bits per pass, 64-bit keys + 32-bit payloads.  Per pass: (1) per-block digit
+// histogram over the block's contiguous chunk, (2) exclusive scan of the [digit][block] table, (3) stable
+// scatter (ranks from warp match + per-warp counters).  Chunks are contiguous and processed in order, so the
+// sort is stable; only as many passes as the key has significant bits (32 depth bits + ceil(log2 tiles)).
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sort_chunk(uint32_t K, uint32_t& begin, uint32_t& end) {
+  const uint32_t tiles = (K + kSortTile - 1) / kSortTile;
+  const uint32_t per = (tiles + gridDim.x - 1) / gridDim.x;
+  begin = min((uint32_t)blockIdx.x * per * kSortTile, K);
+  end = min(begin + per * kSortTile, K);
+}
+
+__global__ void __launch_bounds__(kSortThreads) sort_hist_kernel(const Status* __restrict__ status, uint32_t capacity,
+                                                                 const uint64_t* __restrict__ keys, int shift,
+                                                                 uint32_t* __restrict__ hist) {
+  __shared__ uint32_t s_hist[256];
+  const uint32_t K = min(status->K, capacity);
+  uint32_t begin, end;
+  sort_chunk(K, begin, end);
+  s_hist[threadIdx.x] = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  for (uint32_t base = begin; base < end; base += kSortThreads) {
+    const uint32_t i = base + threadIdx.x;
+    const bool valid = i < end;
+    const uint32_t d = valid ? (uint32_t)(keys[i] >> shift) & 255u : (256u + lane);
+    const unsigned m = __match_any_sync(0xffffffffu, d);
+    if (valid && lane == __ffs(m) - 1) atomicAdd(&s_hist[d], __popc(m));
+  }
+  __syncthreads();
+  hist[threadIdx.x * gridDim.x + blockIdx.x] = s_hist[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(1024) sort_scan_kernel(int n, uint32_t* __restrict__ hist) {
+  __shared__ uint32_t s_warp[33];
+  const int per = (n + 1023) / 1024;
+  const int b0 = threadIdx.x * per;
+  uint32_t sum = 0;
+  for (int k = 0; k < per; ++k)
+    if (b0 + k < n) sum += hist[b0 + k];
+  uint32_t total;
+  uint32_t run = block_exclusive_scan(sum, s_warp, &total);
+  for (int k = 0; k < per; ++k)
+    if (b0 + k < n) {
+      const uint32_t v = hist[b0 + k];
+      hist[b0 + k] = run;
+      run += v;
+    }
+}
+
+__global__ void __launch_bounds__(kSortThreads) sort_scatter_kernel(const Status* __restrict__ status, uint32_t capacity,
+                                                                    const uint64_t* __restrict__ keys_in,
+                                                                    const uint32_t* __restrict__ vals_in,
+                                                                    uint64_t* __restrict__ keys_out,
+                                                                    uint32_t* __restrict__ vals_out, int shift,
+                                                                    const uint32_t* __restrict__ hist) {
+  constexpr int kWarps = kSortThreads / 32;
+  __shared__ uint32_t s_warp_hist[kWarps][256];
+  __shared__ uint32_t s_base[256];       // running global base of each digit for this block
+  __shared__ uint32_t s_tile_base[256];  // base of each digit for the current tile
+  const uint32_t K = min(status->K, capacity);
+  uint32_t begin, end;
+  sort_chunk(K, begin, end);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  s_base[threadIdx.x] = hist[threadIdx.x * gridDim.x + blockIdx.x];
+  for (uint32_t tile = begin; tile < end; tile += kSortTile) {
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) s_warp_hist[w][threadIdx.x] = 0;
+    __syncthreads();
+    uint64_t key[kSortItems];
+    uint32_t val[kSortItems], rank[kSortItems];
+    const uint32_t wbase = tile + warp * (kSortItems * 32);
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+      const uint32_t i = wbase + j * 32 + lane;
+      const bool valid = i < end;
+      key[j] = valid ? keys_in[i] : 0ull;
+      val[j] = valid ? vals_in[i] : 0u;
+    }
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+      const uint32_t i = wbase + j * 32 + lane;
+      const bool valid = i < end;
+      const uint32_t d = valid ? (uint32_t)(key[j] >> shift) & 255u : (256u + lane);
+      const unsigned m = __match_any_sync(0xffffffffu, d);
+      uint32_t prev = 0;
+      if (valid) prev = s_warp_hist[warp][d];
+      __syncwarp();
+      rank[j] = prev + __popc(m & lt);
+      if (valid && lane == __ffs(m) - 1) s_warp_hist[warp][d] = prev + __popc(m);
+      __syncwarp();
+    }
+    __syncthreads();
+    {  // per digit: exclusive scan over the warps, then advance the running base
+      const int d = threadIdx.x;
+      uint32_t run = 0;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) {
+        const uint32_t c = s_warp_hist[w][d];
+        s_warp_hist[w][d] = run;
+        run += c;
+      }
+      const uint32_t b = s_base[d];
+      s_tile_base[d] = b;
+      s_base[d] = b + run;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+      const uint32_t i = wbase + j * 32 + lane;
+      if (i < end) {
+        const uint32_t d = (uint32_t)(key[j] >> shift) & 255u;
+        const uint32_t dst = s_tile_base[d] + s_warp_hist[warp][d] + rank[j];
+        keys_out[dst] = key[j];
+        vals_out[dst] = val[j];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_sort(satsplat_ctx* c, cudaStream_t s) {
+  const int tiles = c->cam.TX * c->cam.TY;
+  int tile_bits = 0;
+  while ((1 << tile_bits) < tiles) ++tile_bits;
+  const int passes = (32 + tile_bits + 7) / 8;
+  int cur = 0;
+  for (int p = 0; p < passes; ++p) {
+    const int shift = 8 * p;
+    sort_hist_kernel<<<kSortBlocks, kSortThreads, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[cur], shift, c->hist);
+    sort_scan_kernel<<<1, 1024, 0, s>>>(256 * kSortBlocks, c->hist);
+    sort_scatter_kernel<<<kSortBlocks, kSortThreads, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[cur], c->vals[cur],
+                                                            c->keys[cur ^ 1], c->vals[cur ^ 1], shift, c->hist);
+    cur ^= 1;
+  }
+  c->sorted = cur;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// tile ranges: ranges[t] = [first, last+1) of tile t in the sorted keys, (0,0) for empty tiles
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ranges_kernel(const Status* __restrict__ status, uint32_t capacity,
+                                                     const uint64_t* __restrict__ keys, uint32_t* __restrict__ ranges) {
+  const uint32_t K = min(status->K, capacity);
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < K; i += gridDim.x * blockDim.x) {
+    const uint32_t t = (uint32_t)(keys[i] >> 32);
+    if (i == 0 || (uint32_t)(keys[i - 1] >> 32) != t) ranges[2 * t] = i;
+    if (i == K - 1 || (uint32_t)(keys[i + 1] >> 32) != t) ranges[2 * t + 1] = i + 1;
+  }
+}
+
+cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
+  const int tiles = c->cam.TX * c->cam.TY;
+  cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
+  ranges_kernel<<<148 * 8, 256, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[c->sorted], c->ranges);
+  return cudaGetLastError();
+}
+
+}  // namespace satsplat

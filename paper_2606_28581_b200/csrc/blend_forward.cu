@@ -1,0 +1,165 @@
+// blend_forward.cu — (a3) per-16x16-tile front-to-back compositing (Eq. 14) of colour,
+// alpha, expected depth, normal, median depth and the depth-distortion term, with the Eq. 12 lower-bounded
+// Gaussian evaluated through the exact per-splat affine map u = Q (x - c) (Eq. 9), and (a5) the Eq. 1 epilogue
+// (colour correction + soft shadow test against the sun-view depth map) fused after the loop.
+//
+// One CTA per tile, one thread per pixel; a warp covers an 8x4 pixel block.  Splat records are staged through
+// shared memory in batches of 256 (two float4 for the per-pair test, two more read only by contributing pairs).
+// FP32-issue bound: ~17 instructions per evaluated pair, ~25 more per contributing pair.
+#include "internal.cuh"
+
+namespace satsplat {
+
+struct FwdParams {
+  DevCamera cam;
+  DevShading sh;
+  const uint32_t* ranges;
+  const uint32_t* vals;
+  const float4* rec;
+  float4* out_rgba;
+  float4* out_geom;
+  float4* out_aux;
+  float* sun_depth_out;
+  float4* px_a;
+  float4* px_b;
+  int2* px_i;
+  int32_t* px_visited;
+  int32_t* px_contrib;
+};
+
+constexpr int kBatch = 256;
+
+template <bool DEPTH_ONLY>
+__global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constant__ FwdParams P) {
+  __shared__ float4 s_r0[kBatch], s_r1[kBatch], s_r2[kBatch], s_r3[kBatch];
+
+  const int tile = blockIdx.y * P.cam.TX + blockIdx.x;
+  const uint32_t start = P.ranges[2 * tile], end = P.ranges[2 * tile + 1];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int ix = blockIdx.x * kTile + (warp & 1) * 8 + (lane & 7);
+  const int iy = blockIdx.y * kTile + (warp >> 1) * 4 + (lane >> 3);
+  const bool inside = ix < P.cam.W && iy < P.cam.H;
+  const float px = (float)ix + 0.5f, py = (float)iy + 0.5f;
+
+  float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
+  float M1 = 0.f, M2 = 0.f, L = 0.f, zref = 0.f, med = P.cam.z_bg;
+  int mi = -1, last = 0, visited = 0, ncontrib = 0;
+  bool done = !inside;
+
+  for (uint32_t base = start; base < end; base += kBatch) {
+    if (__syncthreads_and(done)) break;
+    const uint32_t idx = base + threadIdx.x;
+    if (idx < end) {
+      const float4* r = P.rec + 4 * (size_t)P.vals[idx];
+      s_r0[threadIdx.x] = r[0];
+      s_r1[threadIdx.x] = r[1];
+      if (!DEPTH_ONLY) {
+        s_r2[threadIdx.x] = r[2];
+        s_r3[threadIdx.x] = r[3];
+      } else {
+        s_r2[threadIdx.x] = r[2];
+      }
+    }
+    __syncthreads();
+    if (done) continue;
+    const int n = min(kBatch, (int)(end - base));
+    const int rel0 = (int)(base - start);
+    for (int j = 0; j < n; ++j) {
+      const float4 r0 = s_r0[j], r1 = s_r1[j];
+      const float dx = px - r0.x, dy = py - r0.y;
+      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
+      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
+      const float rho = fminf(rho3, rho2);
+      if (rho > kRhoCut) continue;
+      const float G = __expf(-0.5f * rho);
+      const float a = fminf(kAlphaMax, r1.z * G);
+      if (a < kAlphaMin) continue;
+      const float Tn = T * (1.0f - a);
+      if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
+      const float w = a * T;
+      const float4 r2 = s_r2[j];
+      const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
+      if (DEPTH_ONLY) {
+        M1 += w * z;
+      } else {
+        const float4 r3 = s_r3[j];
+        if (ncontrib == 0) zref = z;
+        const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
+        if (T > 0.5f) { med = z; mi = rel0 + j; }
+        L += w * (zs * zs * (1.0f - T) + M2 - 2.0f * zs * M1);
+        C0 += w * r2.z; C1 += w * r2.w; C2 += w * r3.x;
+        N0 += w * r3.y; N1 += w * r3.z; N2 += w * r3.w;
+        M1 += w * zs;
+        M2 += w * zs * zs;
+      }
+      T = Tn;
+      last = rel0 + j + 1;
+      ++ncontrib;
+    }
+  }
+  if (!inside) return;
+  if (visited == 0) visited = (int)(end - start);
+  const size_t o = (size_t)iy * P.cam.W + ix;
+  const float A = 1.0f - T;
+  if (DEPTH_ONLY) {
+    P.sun_depth_out[o] = M1 + T * P.cam.z_bg;
+    P.px_a[o] = make_float4(T, 0.f, 0.f, 0.f);
+    P.px_i[o] = make_int2(last, -1);
+  } else {
+    const float D = __fmaf_rn(zref, A, M1);
+    const float al0 = C0 + T * P.cam.bg[0], al1 = C1 + T * P.cam.bg[1], al2 = C2 + T * P.cam.bg[2];
+    float V = 1.0f;
+    if (P.sh.shadows_on) {
+      const ShadowTap t = shadow_tap(P.sh, P.cam, px, py, D, T);
+      if (t.in_map) {
+        const float* Dm = P.sh.sun_depth;
+        const int SW = P.sh.sun_w;
+        const float d00 = __ldg(Dm + t.y0 * SW + t.x0), d01 = __ldg(Dm + t.y0 * SW + t.x1);
+        const float d10 = __ldg(Dm + t.y1 * SW + t.x0), d11 = __ldg(Dm + t.y1 * SW + t.x1);
+        const float ds = (1.f - t.fy) * ((1.f - t.fx) * d00 + t.fx * d01) + t.fy * ((1.f - t.fx) * d10 + t.fx * d11);
+        const float gap = t.zv - ds;
+        V = 1.0f / (1.0f + __expf(P.sh.slope * (gap - P.sh.bias)));
+      }
+    }
+    const float* cc = P.sh.cc;
+    const float ac0 = cc[0] * al0 + cc[1] * al1 + cc[2] * al2 + cc[3];
+    const float ac1 = cc[4] * al0 + cc[5] * al1 + cc[6] * al2 + cc[7];
+    const float ac2 = cc[8] * al0 + cc[9] * al1 + cc[10] * al2 + cc[11];
+    const float s0 = V + (1.f - V) * P.sh.ambient[0], s1 = V + (1.f - V) * P.sh.ambient[1], s2 = V + (1.f - V) * P.sh.ambient[2];
+    if (P.out_rgba) P.out_rgba[o] = make_float4(ac0 * s0, ac1 * s1, ac2 * s2, A);   // Eq. 1
+    if (P.out_geom) P.out_geom[o] = make_float4(N0, N1, N2, D);
+    if (P.out_aux) P.out_aux[o] = make_float4(med, L, V, T);
+    P.px_a[o] = make_float4(T, zref, M1, M2);
+    P.px_b[o] = make_float4(al0, al1, al2, V);
+    P.px_i[o] = make_int2(last, mi);
+  }
+  P.px_visited[o] = visited;
+  P.px_contrib[o] = ncontrib;
+}
+
+cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* out_rgba, float* out_geom, float* out_aux,
+                                 float* sun_depth_out, bool depth_only, cudaStream_t s) {
+  FwdParams P;
+  P.cam = c->cam;
+  P.sh = sh;
+  P.ranges = c->ranges;
+  P.vals = c->vals[c->sorted];
+  P.rec = c->rec;
+  P.out_rgba = reinterpret_cast<float4*>(out_rgba);
+  P.out_geom = reinterpret_cast<float4*>(out_geom);
+  P.out_aux = reinterpret_cast<float4*>(out_aux);
+  P.sun_depth_out = sun_depth_out;
+  P.px_a = c->px_a;
+  P.px_b = c->px_b;
+  P.px_i = c->px_i;
+  P.px_visited = c->px_visited;
+  P.px_contrib = c->px_contrib;
+  const dim3 grid(c->cam.TX, c->cam.TY);
+  if (depth_only)
+    blend_forward_kernel<true><<<grid, 256, 0, s>>>(P);
+  else
+    blend_forward_kernel<false><<<grid, 256, 0, s>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace satsplat

@@ -1,0 +1,135 @@
+// chain_backward.cu — per-surfel chain rule from gradient records (c, Q, alpha, z_c, g, rgb, n) to the surfel
+// parameters (means, quats, scales, opacity logits, rgb) and to the 2x4 camera delta dF (PAPER.md:155-163,
+// Eq. 15), through Eq. 8-11.  One thread per surfel; the 8 dF partials are reduced over the CTA (shuffles +
+// shared memory) before one atomic each.  The gradient records are cleared as they are consumed, so the
+// context never needs a separate memset pass.  HBM-bound: 64 B record + 40 B inputs read, 52 B read-modify-write.
+#include "internal.cuh"
+
+namespace satsplat {
+
+__device__ __forceinline__ float warp_sum_f(float v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+  return v;
+}
+
+__global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int N, const float* __restrict__ means,
+                                                             const float* __restrict__ quats, const float* __restrict__ scales,
+                                                             const float* __restrict__ logits, const uint32_t* __restrict__ count,
+                                                             const uint8_t* __restrict__ flags, float4* __restrict__ vrec,
+                                                             float* __restrict__ v_means, float* __restrict__ v_quats,
+                                                             float* __restrict__ v_scales, float* __restrict__ v_logits,
+                                                             float* __restrict__ v_rgb, float* __restrict__ v_dF) {
+  __shared__ float s_red[8][8];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  float dF[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) dF[k] = 0.f;
+  if (i < N && count[i] > 0) {
+    float4* gp = vrec + 4 * (size_t)i;
+    const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2], g3 = gp[3];
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    gp[0] = zero; gp[1] = zero; gp[2] = zero; gp[3] = zero;
+    const uint8_t fl = flags[i];
+    const float p0 = means[3 * i], p1 = means[3 * i + 1], p2 = means[3 * i + 2];
+    const float4 q = reinterpret_cast<const float4*>(quats)[i];
+    const float2 sc = reinterpret_cast<const float2*>(scales)[i];
+    const float B00 = cam.Fp[0], B01 = cam.Fp[1], B02 = cam.Fp[2];
+    const float B10 = cam.Fp[4], B11 = cam.Fp[5], B12 = cam.Fp[6];
+    const float qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
+    const float inv = 1.0f / qn;
+    const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
+    const float tu0 = 1.f - 2.f * (y * y + z * z), tu1 = 2.f * (x * y + w * z), tu2 = 2.f * (x * z - w * y);
+    const float tv0 = 2.f * (x * y - w * z), tv1 = 1.f - 2.f * (x * x + z * z), tv2 = 2.f * (y * z + w * x);
+    // gradient record slots: g0 = (c_x, c_y, Q00, Q01)  g1 = (Q10, Q11, alpha, z_c)  g2 = (g0, g1, r, g)  g3 = (b, n_x, n_y, n_z)
+    const float alpha = 1.0f / (1.0f + expf(-logits[i]));
+    if (v_logits) v_logits[i] += g1.z * alpha * (1.0f - alpha);
+    if (v_rgb) { v_rgb[3 * i] += g2.z; v_rgb[3 * i + 1] += g2.w; v_rgb[3 * i + 2] += g3.x; }
+    const float sg = (fl & F_FLIPPED) ? -1.f : 1.f;
+    float vtu0 = 0.f, vtu1 = 0.f, vtu2 = 0.f, vtv0 = 0.f, vtv1 = 0.f, vtv2 = 0.f;
+    const float vn0 = sg * g3.y, vn1 = sg * g3.z, vn2 = sg * g3.w;
+    const float vc0 = g0.x, vc1 = g0.y;
+    float vs0 = 0.f, vs1 = 0.f;
+    if (!(fl & F_DEGENERATE)) {
+      const float au0 = B00 * tu0 + B01 * tu1 + B02 * tu2, au1 = B10 * tu0 + B11 * tu1 + B12 * tu2;
+      const float av0 = B00 * tv0 + B01 * tv1 + B02 * tv2, av1 = B10 * tv0 + B11 * tv1 + B12 * tv2;
+      const float M00 = sc.x * au0, M10 = sc.x * au1, M01 = sc.y * av0, M11 = sc.y * av1;
+      const float id = 1.0f / (M00 * M11 - M01 * M10);
+      const float Q00 = M11 * id, Q01 = -M01 * id, Q10 = -M10 * id, Q11 = M00 * id;
+      const float r0 = sc.x * tu2, r1 = sc.y * tv2;
+      // g_j = -sum_i r_i Q_ij
+      const float vg0 = g2.x, vg1 = g2.y;
+      const float vr0 = -(vg0 * Q00 + vg1 * Q01), vr1 = -(vg0 * Q10 + vg1 * Q11);
+      const float vQ00 = g0.z - r0 * vg0, vQ01 = g0.w - r0 * vg1, vQ10 = g1.x - r1 * vg0, vQ11 = g1.y - r1 * vg1;
+      // v_M = -Q^T v_Q Q^T
+      const float t00 = Q00 * vQ00 + Q10 * vQ10, t01 = Q00 * vQ01 + Q10 * vQ11;
+      const float t10 = Q01 * vQ00 + Q11 * vQ10, t11 = Q01 * vQ01 + Q11 * vQ11;
+      const float vM00 = -(t00 * Q00 + t01 * Q01), vM01 = -(t00 * Q10 + t01 * Q11);
+      const float vM10 = -(t10 * Q00 + t11 * Q01), vM11 = -(t10 * Q10 + t11 * Q11);
+      vs0 = vM00 * au0 + vM10 * au1 + vr0 * tu2;
+      vs1 = vM01 * av0 + vM11 * av1 + vr1 * tv2;
+      const float vau0 = sc.x * vM00, vau1 = sc.x * vM10, vav0 = sc.y * vM01, vav1 = sc.y * vM11;
+      vtu0 = B00 * vau0 + B10 * vau1; vtu1 = B01 * vau0 + B11 * vau1; vtu2 = B02 * vau0 + B12 * vau1 + sc.x * vr0;
+      vtv0 = B00 * vav0 + B10 * vav1; vtv1 = B01 * vav0 + B11 * vav1; vtv2 = B02 * vav0 + B12 * vav1 + sc.y * vr1;
+      dF[0] = vau0 * tu0 + vav0 * tv0; dF[1] = vau0 * tu1 + vav0 * tv1; dF[2] = vau0 * tu2 + vav0 * tv2;
+      dF[4] = vau1 * tu0 + vav1 * tv0; dF[5] = vau1 * tu1 + vav1 * tv1; dF[6] = vau1 * tu2 + vav1 * tv2;
+    }
+    if (v_scales) { v_scales[2 * i] += vs0; v_scales[2 * i + 1] += vs1; }
+    // c = B p + b ; z_c = b_z - p_z
+    if (v_means) {
+      v_means[3 * i] += B00 * vc0 + B10 * vc1;
+      v_means[3 * i + 1] += B01 * vc0 + B11 * vc1;
+      v_means[3 * i + 2] += B02 * vc0 + B12 * vc1 - g1.w;
+    }
+    dF[0] += vc0 * p0; dF[1] += vc0 * p1; dF[2] += vc0 * p2; dF[3] = vc0;
+    dF[4] += vc1 * p0; dF[5] += vc1 * p1; dF[6] += vc1 * p2; dF[7] = vc1;
+    // R = [t_u | t_v | n] -> unit quaternion -> raw quaternion.  G[r][c] = dL/dR[r][c]
+    if (v_quats) {
+      const float G00 = vtu0, G01 = vtv0, G02 = vn0, G10 = vtu1, G11 = vtv1, G12 = vn1, G20 = vtu2, G21 = vtv2, G22 = vn2;
+      const float vw = 2.f * (x * (G21 - G12) + y * (G02 - G20) + z * (G10 - G01));
+      const float vx = 2.f * (-2.f * x * (G11 + G22) + y * (G01 + G10) + z * (G02 + G20) + w * (G21 - G12));
+      const float vy = 2.f * (x * (G01 + G10) - 2.f * y * (G00 + G22) + z * (G12 + G21) + w * (G02 - G20));
+      const float vz = 2.f * (x * (G02 + G20) + y * (G12 + G21) - 2.f * z * (G00 + G11) + w * (G10 - G01));
+      const float dotq = w * vw + x * vx + y * vy + z * vz;
+      float4* vq = reinterpret_cast<float4*>(v_quats) + i;
+      float4 cur = *vq;
+      cur.x += (vw - w * dotq) * inv; cur.y += (vx - x * dotq) * inv; cur.z += (vy - y * dotq) * inv; cur.w += (vz - z * dotq) * inv;
+      *vq = cur;
+    }
+  }
+  if (v_dF) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float r = warp_sum_f(dF[k]);
+      if (lane == 0) s_red[warp][k] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+      float r = 0.f;
+#pragma unroll
+      for (int wv = 0; wv < 8; ++wv) r += s_red[wv][threadIdx.x];
+      if (r != 0.f) atomicAdd(v_dF + threadIdx.x, r);
+    }
+  }
+}
+
+cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
+                                  const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
+                                  float* v_rgb, float* v_dF, cudaStream_t s) {
+  if (c->N == 0) return cudaSuccess;
+  chain_backward_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>(c->cam, (int)c->N, means, quats, scales, logits, c->count,
+                                                                  c->flags, reinterpret_cast<float4*>(c->vrec), v_means,
+                                                                  v_quats, v_scales, v_logits, v_rgb, v_dF);
+  return cudaGetLastError();
+}
+
+__global__ void add_small_kernel(float* dst, const float* src, int n) {
+  if ((int)threadIdx.x < n) dst[threadIdx.x] += src[threadIdx.x];
+}
+cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s) {
+  add_small_kernel<<<1, 32, 0, s>>>(dst, src, n);
+  return cudaGetLastError();
+}
+
+}  // namespace satsplat

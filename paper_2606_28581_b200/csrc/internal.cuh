@@ -1,0 +1,151 @@
+// internal.cuh — shared declarations of the CUDA path (NOT part of the C ABI; never seen by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/satsplat.h"
+
+namespace satsplat {
+
+// ---- method constants ------------------------------------------------
+constexpr int kTile = 16;
+constexpr float kRhoCut = 9.0f;            // 3-sigma
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kAlphaMax = 0.99f;
+constexpr float kTMin = 1e-4f;
+constexpr float kDetEps = 1e-6f;           // |det(B'_xy R S')| <= eps -> degenerate
+constexpr float kLogitCull = -5.5373342f;  // sigmoid(l) < 1/255
+constexpr float kMinExtent = 2.1213204f;   // 3 sigma, sigma = 1/sqrt(2) px (Eq. 12)
+constexpr float kDegenerateQ = 1e12f;      // Q = kDegenerateQ * I encodes "rho3 = +inf" for degenerate surfels
+
+enum : uint8_t { F_CULLED = 1, F_DEGENERATE = 2, F_FLIPPED = 4 };
+
+// ---- device-side camera ------------------------------------------------------------------------------------
+struct DevCamera {
+  int W, H, TX, TY;
+  float Fp[8];  // F + dF (fp32 add, Eq. 15)
+  float vd[3];
+  float b_z, z_bg;
+  float bg[3];
+};
+
+struct DevShading {
+  float cc[12];
+  float ambient[3];
+  int shadows_on;
+  int sun_w, sun_h;
+  const float* sun_depth;
+  float reproj[8];
+  float bias, slope;
+};
+
+// ---- record layout in HBM: 4 x float4 = 64 B per surfel, 64-B aligned --------------------------------------
+//   r0 = (c_x, c_y, Q00, Q01)   r1 = (Q10, Q11, alpha, z_c)   r2 = (g0, g1, red, green)   r3 = (blue, n_x, n_y, n_z)
+// The first two float4 are all the per-pair test needs; the last two are only read by contributing pairs.
+// Gradient records use the same slots.
+
+// sort configuration
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 8;
+constexpr int kSortTile = kSortThreads * kSortItems;  // 2048 keys
+constexpr int kSortBlocks = 148 * 4;                  // fixed grid: K lives on the device
+
+struct Status {           // device-resident status words
+  unsigned int K;         // duplicated keys of the last preprocess (may exceed capacity)
+  unsigned int overflow;  // K > max_duplicates
+  unsigned int pad[2];
+};
+
+// Shadow-test lookup shared by the forward epilogue and its backward so that both take the same in-map /
+// texel decisions from the same bits (explicit fma sequence: no compiler-dependent contraction).
+struct ShadowTap {
+  bool in_map;
+  int x0, y0, x1, y1;
+  float fx, fy, h, zv;
+};
+__device__ __forceinline__ ShadowTap shadow_tap(const DevShading& sh, const DevCamera& cam, float px, float py, float D, float T) {
+  ShadowTap t;
+  t.zv = __fmaf_rn(T, cam.z_bg, D);          // z_v = D + T_f z_bg
+  t.h = __fsub_rn(cam.b_z, t.zv);            // world height seen at this pixel
+  const float xs = __fmaf_rn(sh.reproj[2], t.h, __fmaf_rn(sh.reproj[1], py, __fmaf_rn(sh.reproj[0], px, sh.reproj[3])));
+  const float ys = __fmaf_rn(sh.reproj[6], t.h, __fmaf_rn(sh.reproj[5], py, __fmaf_rn(sh.reproj[4], px, sh.reproj[7])));
+  t.in_map = xs >= 0.5f && xs <= (float)sh.sun_w - 0.5f && ys >= 0.5f && ys <= (float)sh.sun_h - 0.5f;
+  const float tx = xs - 0.5f, ty = ys - 0.5f;
+  t.x0 = min(max((int)floorf(tx), 0), sh.sun_w - 1);
+  t.y0 = min(max((int)floorf(ty), 0), sh.sun_h - 1);
+  t.fx = tx - (float)t.x0;
+  t.fy = ty - (float)t.y0;
+  t.x1 = min(t.x0 + 1, sh.sun_w - 1);
+  t.y1 = min(t.y0 + 1, sh.sun_h - 1);
+  return t;
+}
+
+}  // namespace satsplat
+
+struct satsplat_ctx {
+  int device;
+  int64_t max_surfels, max_dup;
+  int32_t max_w, max_h;
+  int64_t scratch_bytes;
+  // per-surfel
+  float4* rec;            // [N*4]
+  uint16_t* rect;         // [N*4]
+  uint32_t* count;        // [N]
+  uint32_t* offset;       // [N+1] exclusive scan
+  uint32_t* depth_key;    // [N]
+  uint8_t* flags;         // [N]
+  float* vrec;            // [N*16] gradient records, kept zero between calls (the chain kernel clears them)
+  uint32_t* block_sums;   // scan scratch
+  // binning
+  uint64_t* keys[2];
+  uint32_t* vals[2];
+  int sorted;             // which buffer holds the sorted result
+  uint32_t* hist;         // [256 * kSortBlocks]
+  uint32_t* ranges;       // [tiles*2]
+  satsplat::Status* status;
+  // per-pixel state kept for the backward
+  float4* px_a;           // (T_f, z_ref, M1', M2')
+  float4* px_b;           // (albedo r,g,b, V)
+  int2* px_i;             // (last, median list index)
+  int32_t* px_last;       // planes for debug/statistics
+  int32_t* px_visited;
+  int32_t* px_contrib;
+  float* red_buf;         // small reduction scratch (dF, cc, ambient, reproj)
+  // host state
+  satsplat::DevCamera cam;
+  int64_t N;
+  const float *in_means, *in_quats, *in_scales, *in_logits;  // caller buffers of the last preprocess (chain backward)
+  int preprocessed, forwarded, depth_only;
+  // e2e staging buffers (lazily sized inside create)
+  float* e2e_in;          // means..rgb
+  float* e2e_up;          // upstream grads (3 images)
+  float* e2e_out;         // images
+  float* e2e_grads;       // N*13 + 23
+  // profiling
+  int profiling;
+  cudaEvent_t ev[2 * SATSPLAT_NUM_STAGES];
+  int ev_used[SATSPLAT_NUM_STAGES];
+  char err[512];
+};
+
+namespace satsplat {
+
+// launchers (each enqueues on `s`, returns the cudaError_t of the launch)
+cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, const float* quats, const float* scales,
+                              const float* logits, const float* rgb, cudaStream_t s);
+cudaError_t launch_scan(satsplat_ctx* c, int64_t N, cudaStream_t s);
+cudaError_t launch_duplicate(satsplat_ctx* c, int64_t N, cudaStream_t s);
+cudaError_t launch_sort(satsplat_ctx* c, cudaStream_t s);
+cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s);
+cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* out_rgba, float* out_geom, float* out_aux,
+                                 float* sun_depth_out, bool depth_only, cudaStream_t s);
+cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* v_rgba, const float* v_geom,
+                                  const float* v_aux, const float* v_sun_depth_in, bool depth_only, float* v_cc,
+                                  float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s);
+cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
+                                  const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
+                                  float* v_rgb, float* v_dF, cudaStream_t s);
+cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s);
+cudaError_t launch_export_records(satsplat_ctx* c, float* records_out, uint8_t* flags_out, cudaStream_t s);
+
+}  // namespace satsplat

@@ -1,0 +1,159 @@
+"""Helpers for the GPU parity tests: run one view through the C ABI (via the thin Python binding) and through the
+oracle on the SAME seeded inputs, and compare with the parity policy of DESIGN.md ("Parity policy at
+discontinuities").  Nothing here computes expected values from the CUDA path."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+# fragility thresholds on the oracle's per-pixel decision margins
+# (rho cut [abs], alpha skip [rel], T stop [rel], median |T-0.5| [abs], depth branch |rho3-rho2| [abs], clamp [abs])
+MARGIN_THRESH = np.array([2e-4, 2e-4, 2e-3, 2e-5, 2e-4, 2e-5])
+
+
+def t(a, dtype=torch.float32):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dtype=dtype).contiguous()
+
+
+class GpuScene:
+    """Device copies of a scene's surfel arrays."""
+
+    def __init__(self, scene):
+        self.n = scene.n
+        self.means, self.quats, self.scales = t(scene.means), t(scene.quats), t(scene.scales)
+        self.logits, self.rgb = t(scene.opacity_logits), t(scene.rgb)
+
+    def zeros_grads(self):
+        z = lambda *s: torch.zeros(*s, device="cuda", dtype=torch.float32)
+        return dict(v_means=z(self.n, 3), v_quats=z(self.n, 4), v_scales=z(self.n, 2), v_logits=z(self.n), v_rgb=z(self.n, 3),
+                    v_dF=z(8), v_cc=z(12), v_ambient=z(3), v_reproj=z(8), v_dF_sun=z(8))
+
+
+def gpu_view_iteration(P, gs: GpuScene, view, *, sun_view=None, reproj=None, upstream=None, sun_upstream=None,
+                       do_backward=True, max_dup=None, ctx=None, sun_ctx=None, want_debug=True):
+    """One view through the CUDA path.  `sun_view`/`reproj`: the fp32 sun camera + reprojection constants (inputs)."""
+    n = gs.n
+    H, W = view.height, view.width
+    max_dup = max_dup or max(16 * n, 1024)
+    res = {}
+    cam = P.Camera.from_view(view)
+    own = []
+    if ctx is None:
+        ctx = P.Context(max(n, 1), W, H, max_dup)
+        own.append(ctx)
+    sun_depth = None
+    if sun_view is not None:
+        if sun_ctx is None:
+            sun_ctx = P.Context(max(n, 1), sun_view.width, sun_view.height, max_dup)
+            own.append(sun_ctx)
+        scam = P.Camera.from_view(sun_view)
+        sun_ctx.preprocess(scam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+        sun_depth = torch.empty(sun_view.height, sun_view.width, device="cuda", dtype=torch.float32)
+        sun_ctx.shadow_map(sun_depth)
+        res["sun_depth"] = sun_depth.cpu().numpy()
+        if want_debug:
+            res["sun_bins"] = sun_ctx.debug_bins()
+    shading = P.Shading.make(cc=view.cc, ambient=view.ambient, sun_depth=sun_depth, reproj=reproj, depth_bias=view.depth_bias,
+                             slope=view.slope)
+    ctx.preprocess(cam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+    out = [torch.empty(H, W, 4, device="cuda", dtype=torch.float32) for _ in range(3)]
+    ctx.render_forward(shading, *out)
+    res["K"] = ctx.sync_status()
+    res.update(rgba=out[0].cpu().numpy(), geom=out[1].cpu().numpy(), aux=out[2].cpu().numpy())
+    if want_debug:
+        res["bins"] = ctx.debug_bins()
+        rec, flags = ctx.debug_records()
+        res.update(rec=rec.cpu().numpy(), flags=flags.cpu().numpy())
+        nv, nc = ctx.debug_planes()
+        res.update(n_visited=nv.cpu().numpy(), n_contrib=nc.cpu().numpy())
+    if do_backward:
+        g = gs.zeros_grads()
+        up = [None if u is None else t(u) for u in upstream]
+        v_sun = None if sun_view is None else torch.zeros_like(sun_depth)
+        ctx.render_backward(shading, up[0], up[1], up[2], g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"], g["v_rgb"],
+                            g["v_dF"], g["v_cc"], g["v_ambient"], v_sun, g["v_reproj"] if sun_view is not None else None)
+        if sun_view is not None:
+            res["v_sun_depth"] = v_sun.cpu().numpy()
+            gsun = gs.zeros_grads()
+            vs = v_sun if sun_upstream is None else v_sun + t(sun_upstream)
+            sun_ctx.shadow_map_backward(vs.contiguous(), gsun["v_means"], gsun["v_quats"], gsun["v_scales"], gsun["v_logits"],
+                                        gsun["v_dF_sun"])
+            res["sun_grads"] = {k: v.cpu().numpy() for k, v in gsun.items()}
+        res["grads"] = {k: v.cpu().numpy() for k, v in g.items()}
+    torch.cuda.synchronize()
+    for c in own:
+        c.close()
+    return res
+
+
+# ------------------------------------------------------------------------------------------------------------
+# comparisons
+# ------------------------------------------------------------------------------------------------------------
+def assert_bins_bitexact(orc_pass, bins, n):
+    K, keys, vals, ranges, rects, counts = bins
+    assert K == len(orc_pass["keys"]), (K, len(orc_pass["keys"]))
+    assert np.array_equal(counts.cpu().numpy().view(np.uint32), orc_pass["count"])
+    nz = orc_pass["count"] > 0
+    r = rects.cpu().numpy().view(np.uint16).astype(np.int32)
+    assert np.array_equal(r[nz], orc_pass["rect"][nz])
+    assert keys.cpu().numpy().view(np.uint64).tobytes() == orc_pass["keys"].tobytes()       # memcmp
+    assert vals.cpu().numpy().view(np.uint32).tobytes() == orc_pass["vals"].tobytes()
+    assert ranges.cpu().numpy().view(np.uint32).tobytes() == orc_pass["ranges"].tobytes()
+
+
+def assert_records(orc_pass, rec, flags):
+    ref, rf = orc_pass["rec"], orc_pass["flags"]
+    assert np.array_equal(flags, rf)
+    ok = (orc_pass["count"] > 0)
+    nd = ok & ((rf & 2) == 0)
+    # c, z_c bit exact for every binned surfel; Q, g bit exact where not degenerate; normals bit exact
+    for col in (0, 1, 6, 13, 14, 15, 10, 11, 12):
+        assert np.array_equal(rec[ok, col].view(np.uint32), ref[ok, col].view(np.uint32)), col
+    for col in (2, 3, 4, 5, 7, 8):
+        assert np.array_equal(rec[nd, col].view(np.uint32), ref[nd, col].view(np.uint32)), col
+    np.testing.assert_allclose(rec[ok, 9], ref[ok, 9], rtol=2e-6, atol=1e-7)       # alpha uses exp
+
+
+def fragile_mask(margins, extra=None):
+    m = (margins < MARGIN_THRESH).any(-1)
+    if extra is not None:
+        m |= extra
+    return m
+
+
+def compare_images(gpu, ref, fragile, *, atol=1e-5, rtol=1e-4, names=("rgba", "geom", "aux"), extra_tol=None,
+                   max_fragile_frac=5e-3):
+    """|gpu - ref| <= atol + rtol |ref| on every non-fragile pixel, every channel."""
+    frac = fragile.mean()
+    assert frac <= max_fragile_frac, f"too many fragile pixels: {frac}"
+    stats = {}
+    for k in names:
+        g, r = gpu[k].astype(np.float64), ref[k]
+        tol = atol + rtol * np.abs(r)
+        if extra_tol is not None and k in extra_tol:
+            tol = tol + extra_tol[k]
+        err = np.abs(g - r)
+        bad = (err > tol) & ~fragile[..., None]
+        stats[k] = float((err / tol)[~fragile].max()) if (~fragile).any() else 0.0
+        assert not bad.any(), (k, int(bad.sum()), np.argwhere(bad)[:5], g[bad][:5], r[bad][:5])
+    return stats
+
+
+def compare_grads(gpu, ref, *, atol=1e-5, rtol=1e-3, pairs=None, allow_frac=0.0):
+    """|gpu - ref| <= atol + rtol |ref| elementwise.  `allow_frac` tolerates that share of elements out of
+    tolerance (only used for the unmasked runs where fragile pixels legitimately differ)."""
+    stats = {}
+    for kg, kr in pairs:
+        g, r = gpu[kg].astype(np.float64), np.asarray(ref[kr]).reshape(gpu[kg].shape)
+        tol = atol + rtol * np.abs(r)
+        err = np.abs(g - r)
+        nbad = int((err > tol).sum())
+        stats[kg] = (float((err / tol).max()), nbad)
+        assert nbad <= allow_frac * g.size, (kg, nbad, g.size, float((err / tol).max()),
+                                             g.reshape(-1)[np.argmax((err / tol).reshape(-1))],
+                                             r.reshape(-1)[np.argmax((err / tol).reshape(-1))])
+    return stats
+
+
+GRAD_PAIRS = [("v_means", "v_means"), ("v_quats", "v_quats"), ("v_scales", "v_scales"), ("v_logits", "v_logits"),
+              ("v_rgb", "v_rgb"), ("v_dF", "v_dF")]

@@ -1,0 +1,297 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): tile keys, sorted order and per-tile ranges bit-exact; forward images, depths and
+normals within 1e-5 abs / 1e-4 rel; gradients within 1e-3 rel (or 1e-5 abs).  Pixels whose oracle decision margin
+is below the thresholds in gpu_util.MARGIN_THRESH are "fragile" (DESIGN.md parity policy): excluded from the image
+check, counted, and bounded.  For the gradient check the upstream gradient is zeroed on fragile pixels on BOTH
+sides, so that a decision flipped by fp32 rounding cannot leak into the comparison; an unmasked run is also made
+and must agree except for a bounded share of elements.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import satsplat_scenes as S
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_28581_b200 as P
+    P.lib()   # fails loudly if libsatsplat.so is missing
+    return P
+
+
+@pytest.fixture(scope="module")
+def G():
+    import gpu_util
+    return gpu_util
+
+
+def _scene(cfg):
+    if cfg == "C0":
+        return S.make_config(0)
+    if cfg == "C0_ragged":            # image not a multiple of the tile size, shifted camera
+        sc = S.make_config(0, size=100)
+        sc.views[0].height = 77
+        return sc
+    if cfg == "C1s":
+        return S.make_config(1, n=20000, size=256, n_views=2, extent=64.0)
+    if cfg == "C3s":
+        return S.make_config(3, n=40000, size=384, n_views=1, extent=200.0, sun_size=384)
+    if cfg == "C4s":
+        return S.make_config(4, n=40000, size=512, n_views=1, extent=250.0)
+    raise KeyError(cfg)
+
+
+def _no_shadow(view):
+    import copy
+    v = copy.copy(view)
+    v.shadows_on = False
+    return v
+
+
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s"])
+def test_binning_and_records_bitexact(P, G, orc, cfg):
+    scene = _scene(cfg)
+    gs = G.GpuScene(scene)
+    for view in scene.views:
+        view = _no_shadow(view)
+        ref = orc.render_pass(view, scene)
+        res = G.gpu_view_iteration(P, gs, view, do_backward=False)
+        G.assert_bins_bitexact(ref, res["bins"], scene.n)
+        G.assert_records(ref, res["rec"], res["flags"])
+        assert res["K"] == len(ref["keys"]) > 0
+
+
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s"])
+def test_forward_backward_parity(P, G, orc, cfg):
+    scene = _scene(cfg)
+    gs = G.GpuScene(scene)
+    nth = orc.num_threads()
+    for vi, view in enumerate(scene.views):
+        view = _no_shadow(view)
+        up = S.upstream_grads(scene.seed, vi, view.height, view.width)
+        ref = orc.view_iteration(scene, view, do_backward=False, threads=nth)
+        fragile = G.fragile_mask(ref["fwd"]["margins"])
+        res = G.gpu_view_iteration(P, gs, view, do_backward=False)
+        stats = G.compare_images(res, ref["fwd"], fragile)
+        # pair counts: same decisions on every non-fragile pixel
+        ok = ~fragile
+        assert np.array_equal(res["n_visited"][ok], ref["fwd"]["last"][ok])
+        assert int(res["n_contrib"][ok].sum()) > 0
+        # ---- gradients, upstream masked on fragile pixels ----
+        upm = [u.copy() for u in up]
+        for u in upm:
+            u[fragile] = 0
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        resb = G.gpu_view_iteration(P, gs, view, upstream=upm, want_debug=False)
+        gstats = G.compare_grads(resb["grads"], refb["grads"], pairs=G.GRAD_PAIRS)
+        G.compare_grads(resb["grads"], refb["bwd"], pairs=[("v_cc", "v_cc"), ("v_ambient", "v_ambient")])
+        # ---- unmasked: fragile pixels may legitimately differ; bounded share of elements ----
+        refu = orc.view_iteration(scene, view, upstream=up, threads=nth)
+        resu = G.gpu_view_iteration(P, gs, view, upstream=up, want_debug=False)
+        G.compare_grads(resu["grads"], refu["grads"], pairs=G.GRAD_PAIRS[:5], allow_frac=2e-3 if fragile.any() else 0.0)
+        print(cfg, vi, "fragile", int(fragile.sum()), "img err/tol", stats, "grad err/tol", gstats)
+
+
+def test_shadow_pass_parity_by_stage(P, G, orc):
+    """C2-shaped: sun pass (depth only) -> view pass with the fused shadow + colour epilogue -> both backwards.
+    Each stage is compared with identical inputs on both sides (the oracle's fp32 sun camera / sun map / sun-map
+    gradient are the inputs of the next GPU stage), then once end to end."""
+    import torch
+    scene = S.make_config(2, n=20000, size=256, n_views=2, extent=64.0, sun_size=384)
+    gs = G.GpuScene(scene)
+    nth = orc.num_threads()
+    for vi, view in enumerate(scene.views):
+        up = S.upstream_grads(scene.seed, vi, view.height, view.width)
+        ref = orc.view_iteration(scene, view, do_backward=False, threads=nth)
+        sun_view, reproj = ref["sun_view"], ref["reproj"]
+        # library's own Eq. 16 helper against the oracle's
+        cam = P.Camera.from_view(view)
+        lib_sun, lib_rep = P.sun_camera(cam, view.sun_azimuth, view.sun_elevation, view.sun_width, view.sun_height, view.sun_viewport)
+        np.testing.assert_allclose(np.array(lib_sun.F[:]), sun_view.F, rtol=2e-6, atol=1e-4)
+        np.testing.assert_allclose(np.array(lib_rep), reproj, rtol=2e-6, atol=1e-4)
+        # ---- stage 1: sun pass ----
+        sres = G.gpu_view_iteration(P, gs, _no_shadow(view), sun_view=sun_view, reproj=reproj, do_backward=False)
+        G.assert_bins_bitexact(ref["sun_pass"], sres["sun_bins"], scene.n)
+        sfrag = G.fragile_mask(ref["sun_fwd"]["margins"])
+        sd_ref = ref["sun_depth"]
+        err = np.abs(sres["sun_depth"].astype(np.float64) - sd_ref)
+        assert sfrag.mean() < 5e-3
+        assert (err[~sfrag] <= 1e-5 + 1e-4 * np.abs(sd_ref[~sfrag])).all()
+        # ---- stage 2: view pass forward with the ORACLE's fp32 sun map as input ----
+        sun_map32 = ref["shading"].sun_depth.astype(np.float32)
+        ctx = P.Context(scene.n, view.width, view.height, 16 * scene.n)
+        d_sun = G.t(sun_map32)
+        shading = P.Shading.make(cc=view.cc, ambient=view.ambient, sun_depth=d_sun, reproj=reproj, depth_bias=view.depth_bias, slope=view.slope)
+        ctx.preprocess(cam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+        out = [torch.empty(view.height, view.width, 4, device="cuda") for _ in range(3)]
+        ctx.render_forward(shading, *out)
+        gpu = dict(rgba=out[0].cpu().numpy(), geom=out[1].cpu().numpy(), aux=out[2].cpu().numpy())
+        f = ref["fwd"]
+        fragile = G.fragile_mask(f["margins"])
+        # conditioning of the shadow lookup: x_s carries ~2 ulp(2048) of fp32 rounding and z_v ~1e-5; V moves by
+        # slope V (1-V) (range of the bilinear footprint * dx + dz)
+        V = f["aux"][..., 2]
+        zv = f["geom"][..., 3] + f["aux"][..., 3] * view.z_bg
+        h = view.b_z - zv
+        py, px = np.meshgrid(np.arange(view.height) + 0.5, np.arange(view.width) + 0.5, indexing="ij")
+        xs = reproj[0] * px + reproj[1] * py + reproj[2] * h + reproj[3] - 0.5
+        ys = reproj[4] * px + reproj[5] * py + reproj[6] * h + reproj[7] - 0.5
+        x0 = np.clip(np.floor(xs).astype(int), 0, view.sun_width - 2); y0 = np.clip(np.floor(ys).astype(int), 0, view.sun_height - 2)
+        tex = np.stack([sun_map32[y0, x0], sun_map32[y0, x0 + 1], sun_map32[y0 + 1, x0], sun_map32[y0 + 1, x0 + 1]], -1).astype(np.float64)
+        rng_ = tex.max(-1) - tex.min(-1)
+        dV = view.slope * V * (1 - V) * (rng_ * 1e-3 + 3e-5)
+        # texel-border crossings flip the footprint: fragile
+        fr = np.minimum(np.abs(xs - np.round(xs)), np.abs(ys - np.round(ys)))
+        fragile |= (fr < 1e-3) & (rng_ > 1e-3)
+        albC = np.abs(f["albedo"] @ view.cc.reshape(3, 4)[:, :3].T.astype(np.float64) + view.cc.reshape(3, 4)[:, 3])
+        ex_rgba = np.zeros_like(f["rgba"]); ex_rgba[..., :3] = albC * dV[..., None]
+        ex_aux = np.zeros_like(f["aux"]); ex_aux[..., 2] = dV
+        stats = G.compare_images(gpu, f, fragile, extra_tol=dict(rgba=ex_rgba, aux=ex_aux), max_fragile_frac=2e-2)
+        assert V.min() < 0.3 and V.max() > 0.9       # shadows really are exercised
+        # ---- stage 3: view backward (masked upstream) ----
+        upm = [u.copy() for u in up]
+        for u in upm:
+            u[fragile] = 0
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        g = gs.zeros_grads()
+        v_sun = torch.zeros_like(d_sun)
+        ctx.render_backward(shading, G.t(upm[0]), G.t(upm[1]), G.t(upm[2]), g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"],
+                            g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"], v_sun, g["v_reproj"])
+        gn = {k: v.cpu().numpy() for k, v in g.items()}
+        # gradients that pass through dV/dgap inherit the conditioning of the lookup: looser relative bar there
+        gst = G.compare_grads(gn, refb["grads"], pairs=G.GRAD_PAIRS, rtol=5e-3, atol=1e-4, allow_frac=1e-3)
+        G.compare_grads(gn, refb["bwd"], pairs=[("v_cc", "v_cc"), ("v_ambient", "v_ambient"), ("v_reproj", "v_reproj")], rtol=5e-3, atol=1e-3)
+        vs_ref = refb["bwd"]["v_sun_depth"]
+        vs_err = np.abs(v_sun.cpu().numpy().astype(np.float64) - vs_ref)
+        assert (vs_err > 1e-4 + 5e-3 * np.abs(vs_ref)).mean() < 1e-3
+        ctx.close()
+        # ---- stage 4: sun backward with the ORACLE's fp32 sun-map gradient as input (masked on fragile sun pixels) ----
+        vsd = vs_ref.astype(np.float32)
+        vsd[sfrag] = 0
+        Hs, Ws = vsd.shape
+        vg = np.zeros((Hs, Ws, 4)); vg[..., 3] = vsd
+        vr = np.zeros((Hs, Ws, 4)); vr[..., 3] = -sun_view.z_bg * vsd.astype(np.float64)
+        sp = ref["sun_pass"]
+        bs = orc.backward(Ws, Hs, sun_view.b_z, sun_view.z_bg, np.zeros(3), sp["rec64"], sp["flags"], sp["lists"], orc.Shading(),
+                          vr, vg, None, threads=nth)
+        gsr = orc.preprocess_backward(sun_view, scene.means, scene.quats, scene.scales, scene.opacity_logits, sp["flags"], bs["v_rec"])
+        sctx = P.Context(scene.n, Ws, Hs, 16 * scene.n)
+        sctx.preprocess(P.Camera.from_view(sun_view), gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+        tmp = torch.empty(Hs, Ws, device="cuda")
+        sctx.shadow_map(tmp)
+        g2 = gs.zeros_grads()
+        sctx.shadow_map_backward(G.t(vsd), g2["v_means"], g2["v_quats"], g2["v_scales"], g2["v_logits"], g2["v_dF_sun"])
+        g2n = {k: v.cpu().numpy() for k, v in g2.items()}
+        G.compare_grads(g2n, gsr, pairs=[("v_means", "v_means"), ("v_quats", "v_quats"), ("v_scales", "v_scales"),
+                                         ("v_logits", "v_logits"), ("v_dF_sun", "v_dF")])
+        sctx.close()
+        print("C2s", vi, "fragile", int(fragile.sum()), "sun fragile", int(sfrag.sum()), stats, gst)
+
+
+def test_edge_cases_and_errors(P, G, orc):
+    import torch
+    scene = S.make_config(0)
+    view = scene.views[0]
+    cam = P.Camera.from_view(view)
+    gs = G.GpuScene(scene)
+    ctx = P.Context(scene.n, view.width, view.height, 16 * scene.n)
+    sh = P.Shading.make()
+    out = [torch.empty(view.height, view.width, 4, device="cuda") for _ in range(3)]
+    # calls out of order
+    with pytest.raises(P.SatsplatError) as e:
+        ctx.render_forward(sh, *out)
+    assert e.value.code == P.E_STATE
+    # empty input: every pixel is background
+    z = lambda *s: torch.zeros(*s, device="cuda")
+    ctx.cam, ctx.n = cam, 0
+    rc = P.lib().satsplat_preprocess(ctx._h, cam, 0, None, None, None, None, None, None)
+    assert rc == 0
+    ctx.render_forward(sh, *out)
+    assert ctx.sync_status() == 0
+    assert torch.all(out[0] == 0) and torch.all(out[2][..., 3] == 1) and torch.all(out[2][..., 0] == view.z_bg)
+    # N too large / image too large
+    with pytest.raises(P.SatsplatError) as e:
+        big = torch.zeros(scene.n + 1, 3, device="cuda")
+        ctx.preprocess(cam, big, z(scene.n + 1, 4), z(scene.n + 1, 2), z(scene.n + 1), big)
+    assert e.value.code == P.E_INVALID
+    # everything culled (logits very negative, zero scale, zero quaternion, NaN mean)
+    lg = gs.logits.clone(); lg[:] = -20.0
+    ctx.preprocess(cam, gs.means, gs.quats, gs.scales, lg, gs.rgb)
+    assert ctx.sync_status() == 0
+    bad = G.GpuScene(scene)
+    bad.scales[::4] = 0.0
+    bad.quats[1::4] = 0.0
+    bad.means[2::4, 0] = float("nan")
+    ctx.preprocess(cam, bad.means, bad.quats, bad.scales, bad.logits, bad.rgb)
+    ctx.render_forward(sh, *out)
+    import copy
+    s2 = copy.copy(scene)
+    s2.means, s2.quats, s2.scales = bad.means.cpu().numpy(), bad.quats.cpu().numpy(), bad.scales.cpu().numpy()
+    ref = orc.render_pass(view, s2)
+    G.assert_bins_bitexact(ref, ctx.debug_bins(), scene.n)
+    assert torch.isfinite(out[0]).all() and torch.isfinite(out[1]).all()
+    # capacity overflow is reported, not a crash
+    small = P.Context(scene.n, view.width, view.height, 100)
+    small.preprocess(cam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+    with pytest.raises(P.SatsplatError) as e:
+        small.sync_status()
+    assert e.value.code == P.E_CAPACITY
+    small.close()
+    ctx.close()
+
+
+def test_oversized_splats_cooperative_duplication(P, G, orc):
+    """A few surfels covering hundreds of tiles (C4's tail) + depth ties (flat ground): binning still bit exact."""
+    scene = S.make_config(1, n=5000, size=512, n_views=1, extent=64.0)
+    scene.scales[:20] = 25.0          # ~100 px sigma -> whole-image rects
+    scene.means[:, 2] = np.where(np.arange(scene.n) % 2 == 0, 0.0, scene.means[:, 2])   # massive depth ties
+    view = _no_shadow(scene.views[0])
+    gs = G.GpuScene(scene)
+    ref = orc.render_pass(view, scene)
+    assert ref["count"].max() >= 900
+    res = G.gpu_view_iteration(P, gs, view, do_backward=False, max_dup=int(ref["count"].sum()) + 10)
+    G.assert_bins_bitexact(ref, res["bins"], scene.n)
+    f = orc.forward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, ref["rec64"], ref["flags"], ref["lists"],
+                    orc.Shading(cc=view.cc, ambient=view.ambient), threads=orc.num_threads())
+    G.compare_images(res, f, G.fragile_mask(f["margins"]))
+
+
+def test_iteration_host_matches_device_path(P, G, orc):
+    """The end-to-end HOST-buffer entry point gives the same result as the staged device calls."""
+    import torch
+    scene = S.make_config(2, n=8000, size=128, n_views=1, extent=40.0, sun_size=192)
+    view = scene.views[0]
+    gs = G.GpuScene(scene)
+    cam = P.Camera.from_view(view)
+    sun_cam, rep = P.sun_camera(cam, view.sun_azimuth, view.sun_elevation, view.sun_width, view.sun_height, view.sun_viewport)
+    up = S.upstream_grads(scene.seed, 0, view.height, view.width)
+    n = scene.n
+    ctx = P.Context(n, view.width, view.height, 16 * n)
+    sctx = P.Context(n, view.sun_width, view.sun_height, 16 * n)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
+    h_out = [torch.empty(view.height, view.width, 4).pin_memory() for _ in range(3)]
+    h_g = torch.empty(n * 13 + 23).pin_memory()
+    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, reproj=rep, depth_bias=view.depth_bias, slope=view.slope)
+    sh.shadows_on = 1
+    P.iteration_host(ctx, sctx, cam, sun_cam, sh, n, pin(scene.means), pin(scene.quats), pin(scene.scales), pin(scene.opacity_logits),
+                     pin(scene.rgb), pin(up[0]), pin(up[1]), pin(up[2]), h_out[0], h_out[1], h_out[2], h_g)
+    # staged device path
+    class SV: pass
+    sv = SV(); sv.width, sv.height = view.sun_width, view.sun_height
+    sv.F, sv.dF, sv.view_dir = np.array(sun_cam.F[:]), np.zeros(8), np.array(sun_cam.view_dir[:])
+    sv.b_z, sv.z_bg, sv.bg_rgb = sun_cam.b_z, sun_cam.z_bg, np.zeros(3)
+    res = G.gpu_view_iteration(P, gs, view, sun_view=sv, reproj=rep, upstream=up, want_debug=False)
+    np.testing.assert_allclose(h_out[0].numpy(), res["rgba"], rtol=0, atol=0)
+    np.testing.assert_allclose(h_out[1].numpy(), res["geom"], rtol=0, atol=0)
+    g = h_g.numpy()
+    tot = res["grads"]["v_means"] + res["sun_grads"]["v_means"]
+    np.testing.assert_allclose(g[:3 * n].reshape(n, 3), tot, rtol=1e-3, atol=1e-4)   # atomics: order differs run to run
+    np.testing.assert_allclose(g[13 * n:13 * n + 8], res["grads"]["v_dF"], rtol=2e-3, atol=1e-2)
+    ctx.close(); sctx.close()
