@@ -128,7 +128,7 @@ class _DevBytes:
     """Raw device memory exposed through __cuda_array_interface__ so torch can view (then clone) it."""
 
     def __init__(self, ptr, nbytes):
-        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, True), "version": 2}
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
 
 
 def _wrap(ptr, nbytes, dev):

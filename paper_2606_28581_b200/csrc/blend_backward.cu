@@ -3,7 +3,7 @@
 // Per pixel: epilogue backward first (gradients of the 3x4 colour correction, the ambient light, the
 // reprojection constants; scatter into the sun-depth gradient), then the tile list is walked in REVERSE order:
 // T_i is recovered as T_{i+1}/(1 - a_i), the suffix sum S_i = sum_{k>i} w_k phi_k is carried, and each
-// contributing (pixel, surfel) pair produces 16 gradient values in the record layout (c, Q, alpha, z_c, g, rgb, n).
+// contributing (pixel, surfel) pair produces 16 gradient values (c, M = Q^-1, alpha, z_c, r, rgb, n) in the record slots.
 // Those are reduced across the warp with a transposed shuffle butterfly (16 shuffles instead of 80), across
 // the CTA's warps with shared-memory atomics, and only then flushed once per (tile, surfel) with coalesced
 // global atomics into the per-surfel gradient records.  FP32-issue + atomics bound.
@@ -254,11 +254,14 @@ __global__ void __launch_bounds__(256) blend_backward_kernel(const __grid_consta
         g[7] = v_z;
         float vd0, vd1;
         if (!lowpass) {
+          // z = z_c + g.d = z_c - r.(u,v): accumulate the gradients of M = Q^-1 and r directly,
+          //   v_d = Q^T (v_uv - v_z r) = v_z g + Q^T v_uv,   v_M = -v_d (u,v)^T,   v_r = -v_z (u,v)
+          // (no multiplication by Q^2 afterwards: well conditioned for nearly edge-on surfels)
           const float vu = 2.0f * u * v_rho, vv = 2.0f * v * v_rho;
-          g[8] = v_z * dx; g[9] = v_z * dy;
           vd0 = v_z * r2.x + r0.z * vu + r1.x * vv;
           vd1 = v_z * r2.y + r0.w * vu + r1.y * vv;
-          g[2] = vu * dx; g[3] = vu * dy; g[4] = vv * dx; g[5] = vv * dy;
+          g[2] = -vd0 * u; g[3] = -vd0 * v; g[4] = -vd1 * u; g[5] = -vd1 * v;
+          g[8] = -v_z * u; g[9] = -v_z * v;
         } else {
           vd0 = 4.0f * dx * v_rho;
           vd1 = 4.0f * dy * v_rho;

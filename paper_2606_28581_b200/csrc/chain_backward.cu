@@ -1,4 +1,4 @@
-// chain_backward.cu — per-surfel chain rule from gradient records (c, Q, alpha, z_c, g, rgb, n) to the surfel
+// chain_backward.cu — per-surfel chain rule from gradient records (c, M, alpha, z_c, r, rgb, n) to the surfel
 // parameters (means, quats, scales, opacity logits, rgb) and to the 2x4 camera delta dF (PAPER.md:155-163,
 // Eq. 15), through Eq. 8-11.  One thread per surfel; the 8 dF partials are reduced over the CTA (shuffles +
 // shared memory) before one atomic each.  The gradient records are cleared as they are consumed, so the
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
     const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
     const float tu0 = 1.f - 2.f * (y * y + z * z), tu1 = 2.f * (x * y + w * z), tu2 = 2.f * (x * z - w * y);
     const float tv0 = 2.f * (x * y - w * z), tv1 = 1.f - 2.f * (x * x + z * z), tv2 = 2.f * (y * z + w * x);
-    // gradient record slots: g0 = (c_x, c_y, Q00, Q01)  g1 = (Q10, Q11, alpha, z_c)  g2 = (g0, g1, r, g)  g3 = (b, n_x, n_y, n_z)
+    // gradient record slots: g0 = (c_x, c_y, M00, M01)  g1 = (M10, M11, alpha, z_c)  g2 = (r_0, r_1, red, green)  g3 = (blue, n_x, n_y, n_z)
     const float alpha = 1.0f / (1.0f + expf(-logits[i]));
     if (v_logits) v_logits[i] += g1.z * alpha * (1.0f - alpha);
     if (v_rgb) { v_rgb[3 * i] += g2.z; v_rgb[3 * i + 1] += g2.w; v_rgb[3 * i + 2] += g3.x; }
@@ -53,19 +53,9 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
     if (!(fl & F_DEGENERATE)) {
       const float au0 = B00 * tu0 + B01 * tu1 + B02 * tu2, au1 = B10 * tu0 + B11 * tu1 + B12 * tu2;
       const float av0 = B00 * tv0 + B01 * tv1 + B02 * tv2, av1 = B10 * tv0 + B11 * tv1 + B12 * tv2;
-      const float M00 = sc.x * au0, M10 = sc.x * au1, M01 = sc.y * av0, M11 = sc.y * av1;
-      const float id = 1.0f / (M00 * M11 - M01 * M10);
-      const float Q00 = M11 * id, Q01 = -M01 * id, Q10 = -M10 * id, Q11 = M00 * id;
-      const float r0 = sc.x * tu2, r1 = sc.y * tv2;
-      // g_j = -sum_i r_i Q_ij
-      const float vg0 = g2.x, vg1 = g2.y;
-      const float vr0 = -(vg0 * Q00 + vg1 * Q01), vr1 = -(vg0 * Q10 + vg1 * Q11);
-      const float vQ00 = g0.z - r0 * vg0, vQ01 = g0.w - r0 * vg1, vQ10 = g1.x - r1 * vg0, vQ11 = g1.y - r1 * vg1;
-      // v_M = -Q^T v_Q Q^T
-      const float t00 = Q00 * vQ00 + Q10 * vQ10, t01 = Q00 * vQ01 + Q10 * vQ11;
-      const float t10 = Q01 * vQ00 + Q11 * vQ10, t11 = Q01 * vQ01 + Q11 * vQ11;
-      const float vM00 = -(t00 * Q00 + t01 * Q01), vM01 = -(t00 * Q10 + t01 * Q11);
-      const float vM10 = -(t10 * Q00 + t11 * Q01), vM11 = -(t10 * Q10 + t11 * Q11);
+      // gradient record slots 2..5 hold v_M (M = B' R S' = Q^-1), slots 8..9 hold v_r (r = (s_u t_u.z, s_v t_v.z))
+      const float vM00 = g0.z, vM01 = g0.w, vM10 = g1.x, vM11 = g1.y;
+      const float vr0 = g2.x, vr1 = g2.y;
       vs0 = vM00 * au0 + vM10 * au1 + vr0 * tu2;
       vs1 = vM01 * av0 + vM11 * av1 + vr1 * tv2;
       const float vau0 = sc.x * vM00, vau1 = sc.x * vM10, vav0 = sc.y * vM01, vav1 = sc.y * vM11;
