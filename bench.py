@@ -1,0 +1,417 @@
+#!/usr/bin/env python
+"""bench.py — affine-2DGS fwd+bwd on the benchmark-shaped site (BASELINE.json configs[3]: 1M surfels, 2048^2 views).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (hand-written sm_100a kernels)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands, on the host cores
+
+A "step" is one full training-view iteration of the hot path: sun pass (preprocess,
+binning, depth-only compositing) -> view pass (preprocess, binning, compositing of colour/alpha/depth/normal/
+median/distortion with the fused colour-correction + shadow epilogue) -> backward of both passes (epilogue
+backward, reverse compositing, per-surfel chain, dF / CC reductions).  Views cycle through the config's 20 views.
+Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "affine-2DGS fwd+bwd throughput at 1M surfels, 2048^2 view (C3 full iteration incl. shadow pass)"
+UNIT = "Mpixel/s"
+# algorithmic work per pair: FP32 flops, FMA = 2
+FLOP_EVAL = 26.0          # per evaluated (pixel, list entry) pair: Eq. 9 + Eq. 12 + exp + alpha tests
+FLOP_CONTRIB_FWD = 40.0   # extra per contributing pair, forward
+FLOP_CONTRIB_BWD = 110.0  # extra per contributing pair, backward
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz = 74.4
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = the metric's config)")
+    ap.add_argument("--surfels", type=int, default=None, help="override N (debug)")
+    ap.add_argument("--size", type=int, default=None, help="override view size (debug)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def make_scene(args):
+    import satsplat_scenes as S
+    kw = {}
+    if args.surfels:
+        kw["n"] = args.surfels
+    if args.size:
+        kw["size"] = args.size
+        kw["sun_size"] = args.size
+    return S.make_config(args.config, **kw)
+
+
+def views_for_rank(rank: int, world: int, n_views: int, steps: int):
+    """View index of every step of this rank: ranks start on different views and stride by the world size, so
+    that the ranks of one job render disjoint views (independent units, no data-path collective)."""
+    return [(rank + s * world) % n_views for s in range(steps)]
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index):
+        self.index, self.proc, self.rows = index, None, []
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+# ------------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample
+# ------------------------------------------------------------------------------------------------------------
+def oracle_iteration_seconds(scene, view_index):
+    import satsplat_scenes as S
+    from oracle import oracle as orc
+    view = scene.views[view_index]
+    up = S.upstream_grads(scene.seed, view_index, view.height, view.width)
+    nth = orc.num_threads()
+    t0 = time.perf_counter()
+    orc.view_iteration(scene, view, upstream=up, threads=nth)
+    return time.perf_counter() - t0, nth
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    orc.build()
+    scene = make_scene(args)
+    steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)   # bounded: each step is ~10 s of CPU work
+    for w in range(warm):
+        oracle_iteration_seconds(scene, w % len(scene.views))
+    ts = []
+    for s in range(steps):
+        dt, nth = oracle_iteration_seconds(scene, s % len(scene.views))
+        ts.append(dt)
+    v = scene.views[0]
+    ms = 1e3 * float(np.mean(ts))
+    val = v.width * v.height / 1e6 / (ms / 1e3)
+    sample = f"{steps} full view iteration(s) of the workload (views 0..{steps - 1} of {len(scene.views)}), all {nth} host threads"
+    line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=0, steps=steps, warmup=warm, ms_per_step=ms,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=workload_config(scene, args, 1),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=nth, kind="oracle", sample=sample),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+def workload_config(scene, args, world):
+    v = scene.views[0]
+    return dict(workload=f"C{args.config} benchmark-shaped site (BASELINE.json configs[{args.config}])", surfels=scene.n,
+                view=f"{v.width}x{v.height}", sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
+                views=len(scene.views), shadows=bool(v.shadows_on), parallelism=f"views sharded over {world} rank(s), no collective",
+                l2="per-step working set (records, keys, per-pixel state, images: >0.8 GB) exceeds the 126 MB L2; views cycle")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------------------
+class Job:
+    """Device-resident state of one rank: surfels, two contexts (view + sun), outputs, gradient buffers."""
+
+    def __init__(self, P, torch, scene, device):
+        self.P, self.torch, self.scene = P, torch, scene
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(device)
+        self.means, self.quats, self.scales = dev(scene.means), dev(scene.quats), dev(scene.scales)
+        self.logits, self.rgb = dev(scene.opacity_logits), dev(scene.rgb)
+        n, v = scene.n, scene.views[0]
+        self.n, self.W, self.H = n, v.width, v.height
+        self.shadows = bool(v.shadows_on)
+        max_dup = 8 * n + 4096
+        self.ctx = P.Context(n, v.width, v.height, max_dup, device=device.index)
+        self.sctx = P.Context(n, v.sun_width, v.sun_height, max_dup, device=device.index) if self.shadows else None
+        z = lambda *s: torch.zeros(*s, device=device, dtype=torch.float32)
+        self.out = [torch.empty(v.height, v.width, 4, device=device) for _ in range(3)]
+        self.sun_depth = z(v.sun_height, v.sun_width) if self.shadows else None
+        self.v_sun = z(v.sun_height, v.sun_width) if self.shadows else None
+        self.g = dict(m=z(n, 3), q=z(n, 4), s=z(n, 2), l=z(n), c=z(n, 3), dF=z(8), cc=z(12), amb=z(3))
+        self.cams, self.up = {}, {}
+        self.device = device
+
+    def prepare_view(self, vi):
+        if vi in self.cams:
+            return
+        P, torch, v = self.P, self.torch, self.scene.views[vi]
+        cam = P.Camera.from_view(v)
+        sun_cam, rep = (P.sun_camera(cam, v.sun_azimuth, v.sun_elevation, v.sun_width, v.sun_height, v.sun_viewport)
+                        if self.shadows else (None, None))
+        self.cams[vi] = (cam, sun_cam, rep)
+        gen = torch.Generator(device=self.device)
+        gen.manual_seed(self.scene.seed + 1000 + 7919 * vi)
+        up = [torch.randn(v.height, v.width, 4, device=self.device, generator=gen) for _ in range(3)]
+        up[2][..., 2:] = 0
+        self.up[vi] = up
+
+    def shading(self, vi, with_sun=True):
+        v = self.scene.views[vi]
+        rep = self.cams[vi][2]
+        return self.P.Shading.make(cc=v.cc, ambient=v.ambient, sun_depth=self.sun_depth if (self.shadows and with_sun) else None,
+                                   reproj=rep, depth_bias=v.depth_bias, slope=v.slope)
+
+    def forward(self, vi):
+        cam, sun_cam, _ = self.cams[vi]
+        if self.shadows:
+            self.sctx.preprocess(sun_cam, self.means, self.quats, self.scales, self.logits, self.rgb)
+            self.sctx.shadow_map(self.sun_depth)
+        sh = self.shading(vi)
+        self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb)
+        self.ctx.render_forward(sh, *self.out)
+        return sh
+
+    def step(self, vi):
+        g = self.g
+        for t in g.values():
+            t.zero_()
+        sh = self.forward(vi)
+        up = self.up[vi]
+        if self.shadows:
+            self.v_sun.zero_()
+        self.ctx.render_backward(sh, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"], g["cc"], g["amb"],
+                                 self.v_sun, None)
+        if self.shadows:
+            self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], None)
+
+
+def timed(torch, dist, world, fn, items):
+    """Time fn(item) over items with CUDA events on the current stream; barrier + synchronize on both sides;
+    returns the max over ranks of the elapsed milliseconds."""
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for it in items:
+        fn(it)
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms
+
+
+def stage_profile(job, vi, peaks):
+    """Per-stage device ms (CUDA events recorded by the library on the launching stream), pair counts, and the
+    algorithmic work of each kernel for view `vi`."""
+    torch, P = job.torch, job.P
+    job.ctx.set_profiling(True)
+    if job.sctx:
+        job.sctx.set_profiling(True)
+    job.step(vi)
+    torch.cuda.synchronize()
+    ms_view = job.ctx.stage_ms()
+    ms_sun = job.sctx.stage_ms() if job.sctx else {}
+    job.ctx.set_profiling(False)
+    if job.sctx:
+        job.sctx.set_profiling(False)
+    nv, nc = job.ctx.debug_planes()
+    pairs = dict(view_evaluated=int(nv.sum().item()), view_contributing=int(nc.sum().item()), view_K=job.ctx.sync_status())
+    if job.sctx:
+        snv, snc = job.sctx.debug_planes()
+        pairs.update(sun_evaluated=int(snv.sum().item()), sun_contributing=int(snc.sum().item()), sun_K=job.sctx.sync_status())
+    n, K = job.n, pairs["view_K"]
+    tiles = ((job.W + 15) // 16) * ((job.H + 15) // 16)
+    passes = (32 + max(1, (tiles - 1).bit_length()) + 7) // 8
+    px = job.W * job.H
+    # algorithmic bytes: per surfel / per key / per pixel figures of SURVEY.md 8(d)
+    work = {
+        "preprocess": ("hbm", n * 137.0),
+        "scan": ("hbm", n * 12.0),
+        "duplicate": ("hbm", n * 16.0 + K * 12.0),
+        "sort": ("hbm", K * (passes * 36.0)),
+        "ranges": ("hbm", K * 8.0 + tiles * 8.0),
+        "blend_fwd": ("alu", pairs["view_evaluated"] * FLOP_EVAL + pairs["view_contributing"] * FLOP_CONTRIB_FWD),
+        "blend_bwd": ("alu", pairs["view_evaluated"] * FLOP_EVAL + pairs["view_contributing"] * FLOP_CONTRIB_BWD),
+        "chain_bwd": ("hbm", n * (64.0 * 2 + 40.0 + 52.0 * 2)),
+    }
+    stages = {}
+    for k, ms in ms_view.items():
+        bound, w = work[k]
+        ach = w / (ms * 1e-3) / (1e12 if bound == "alu" else 1e9) if ms > 0 else 0.0
+        peak = FP32_PEAK_TFLOPS if bound == "alu" else peaks["hbm_gbs"]
+        stages[k] = dict(ms=ms, sun_ms=ms_sun.get(k, 0.0), bound=bound, achieved=ach, peak=peak,
+                         unit="TFLOP/s" if bound == "alu" else "GB/s", frac=ach / peak if peak else None)
+    return stages, pairs, px
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_28581_b200 as P
+    P.lib()   # no CUDA library -> fail loudly (there is no fallback)
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device"
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    peaks = load_peaks()
+    scene = make_scene(args)
+    job = Job(P, torch, scene, device)
+    nviews = len(scene.views)
+    warm_views = views_for_rank(rank, world, nviews, args.warmup)
+    step_views = views_for_rank(rank + args.warmup * world, world, nviews, args.steps)
+    for vi in set(warm_views + step_views):
+        job.prepare_view(vi)
+    for vi in warm_views:
+        job.step(vi)
+    torch.cuda.synchronize()
+    k_ok = job.ctx.sync_status()     # raises on capacity overflow
+    launches0 = P.kernel_launches()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_total = timed(torch, dist, world, job.step, step_views)
+    launches = P.kernel_launches() - launches0
+    clocks = sampler.stop()
+    ms_fwd = timed(torch, dist, world, job.forward, step_views)
+    px = job.W * job.H
+    ms_step = ms_total / args.steps
+    value = world * px / 1e6 / (ms_step * 1e-3)
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms_step,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=workload_config(scene, args, world), clocks=clocks, gpu_launches=int(launches),
+                fwd_ms_per_step=ms_fwd / args.steps, fwd_mpixel_s=world * px / 1e6 / (ms_fwd / args.steps * 1e-3))
+    if rank == 0:
+        stages, pairs, _ = stage_profile(job, step_views[0], peaks)
+        dom = max(stages, key=lambda k: stages[k]["ms"])
+        d = stages[dom]
+        line["roofline"] = dict(kernel=dom, bound=d["bound"], achieved=d["achieved"], peak=d["peak"], unit=d["unit"], frac=d["frac"],
+                                traffic=None, peak_source=("derived: 148 SM x 128 lanes x 2 x 1.965 GHz" if d["bound"] == "alu"
+                                                           else peaks["source"] + " HBM copy"),
+                                kernel_ms=d["ms"])
+        line["stages"] = stages
+        line["pairs"] = pairs
+        sun_ms = sum(s["sun_ms"] for s in stages.values())
+        view_ms = sum(s["ms"] for s in stages.values())
+        # whole-iteration roofline: sum over kernels of their own roofline time (both passes)
+        roof_ms = 0.0
+        for k, s in stages.items():
+            if s["frac"]:
+                roof_ms += s["ms"] * s["frac"]
+        line["iteration"] = dict(view_pass_kernel_ms=view_ms, sun_pass_kernel_ms=sun_ms, view_pass_roofline_ms=roof_ms,
+                                 view_pass_frac_of_roofline=roof_ms / view_ms if view_ms else None,
+                                 scratch_gb=(job.ctx.scratch_bytes + (job.sctx.scratch_bytes if job.sctx else 0)) / 1e9,
+                                 peak_mem_gb=torch.cuda.max_memory_allocated() / 1e9 + (job.ctx.scratch_bytes + (job.sctx.scratch_bytes if job.sctx else 0)) / 1e9)
+    # ---- end to end through the C ABI with HOST buffers ----
+    if not args.no_e2e:
+        vi = step_views[0]
+        v = scene.views[vi]
+        pin = lambda t: t.detach().cpu().contiguous().pin_memory()
+        h_in = [pin(x) for x in (job.means, job.quats, job.scales, job.logits, job.rgb)]
+        h_up = [pin(u) for u in job.up[vi]]
+        h_out = [torch.empty(v.height, v.width, 4).pin_memory() for _ in range(3)]
+        h_g = torch.empty(scene.n * 13 + 23).pin_memory()
+        cam, sun_cam, rep = job.cams[vi]
+        sh = P.Shading.make(cc=v.cc, ambient=v.ambient, reproj=rep, depth_bias=v.depth_bias, slope=v.slope)
+        sh.shadows_on = 1 if job.shadows else 0
+
+        def e2e_step(_):
+            P.iteration_host(job.ctx, job.sctx, cam, sun_cam, sh, scene.n, *h_in, *h_up, *h_out, h_g)
+        for _ in range(2):
+            e2e_step(0)
+        n_e2e = max(3, min(args.steps, 10))
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for i in range(n_e2e):
+            e2e_step(i)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = scene.n * 56 + 3 * px * 16
+        d2h = 3 * px * 16 + (scene.n * 13 + 23) * 4
+        line["e2e"] = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                           ms_per_step=1e3 * dt / n_e2e, steps=n_e2e, api="satsplat_iteration_host (pinned host buffers)")
+    # ---- the oracle beside it (rank 0, N = 1 only) ----
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as orc
+        orc.build()
+        dt, nth = oracle_iteration_seconds(scene, step_views[0])
+        line["cpu_baseline"] = dict(value=px / 1e6 / dt, unit=UNIT, cores=nth, kind="oracle", seconds=dt,
+                                    sample=f"1 full view iteration (view {step_views[0]} of {nviews}) of the same workload, {nth} threads")
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -184,6 +184,9 @@ int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out);
 
 const char* satsplat_version(void);
 
+/* Cumulative number of CUDA kernels this library has launched in this process (all contexts). */
+int64_t satsplat_kernel_launches(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -86,6 +86,7 @@ def lib():
         L.satsplat_last_error.argtypes = [C.c_void_p]
         L.satsplat_version.restype = C.c_char_p
         L.satsplat_scratch_bytes.restype = C.c_int64
+        L.satsplat_kernel_launches.restype = C.c_int64
         L.satsplat_scratch_bytes.argtypes = [C.c_void_p]
         L.satsplat_destroy.restype = None
         L.satsplat_destroy.argtypes = [C.c_void_p]
@@ -106,6 +107,10 @@ def lib():
         L.satsplat_stage_ms.argtypes = [vp, C.POINTER(f32)]
         _LIB = L
     return _LIB
+
+
+def kernel_launches() -> int:
+    return int(lib().satsplat_kernel_launches())
 
 
 def version() -> str:

@@ -9,6 +9,10 @@
 
 using namespace satsplat;
 
+namespace satsplat {
+long long g_kernel_launches = 0;
+}
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -86,6 +90,8 @@ void clear_stage_marks(satsplat_ctx* c, std::initializer_list<int> stages) {
 extern "C" {
 
 const char* satsplat_version(void) { return "satsplat-b200 0.1 (sm_100a)"; }
+
+int64_t satsplat_kernel_launches(void) { return (int64_t)g_kernel_launches; }
 
 const char* satsplat_last_error(const satsplat_ctx* ctx) { return ctx ? ctx->err : g_err; }
 

@@ -117,6 +117,7 @@ cudaError_t launch_scan(satsplat_ctx* c, int64_t N, cudaStream_t s) {
     cudaMemsetAsync(c->status, 0, sizeof(Status), s);
     return cudaMemsetAsync(c->offset, 0, sizeof(uint32_t), s);
   }
+  g_kernel_launches += 3;
   scan_block_sums_kernel<<<nblocks, kScanThreads, 0, s>>>((int)N, c->count, c->block_sums);
   scan_top_kernel<<<1, 1024, 0, s>>>(nblocks, c->block_sums, c->status, (uint32_t)c->max_dup);
   scan_apply_kernel<<<nblocks, kScanThreads, 0, s>>>((int)N, c->count, c->block_sums, c->offset);
@@ -176,6 +177,7 @@ __global__ void __launch_bounds__(256) duplicate_kernel(int N, int TX, const ush
 
 cudaError_t launch_duplicate(satsplat_ctx* c, int64_t N, cudaStream_t s) {
   if (N == 0) return cudaSuccess;
+  ++g_kernel_launches;
   duplicate_kernel<<<(int)((N + 255) / 256), 256, 0, s>>>((int)N, c->cam.TX, reinterpret_cast<const ushort4*>(c->rect),
                                                           c->count, c->offset, c->depth_key, c->keys[0], c->vals[0],
                                                           (uint32_t)c->max_dup);
@@ -216,21 +218,33 @@ __global__ void __launch_bounds__(kSortThreads) sort_hist_kernel(const Status* _
   hist[threadIdx.x * gridDim.x + blockIdx.x] = s_hist[threadIdx.x];
 }
 
+// exclusive scan of the [digit][block] table (n = 256 * kSortBlocks entries) by ONE 1024-thread CTA with coalesced
+// accesses: warp w owns the contiguous segment [w*seg, (w+1)*seg) and walks it 32 entries at a time.
 __global__ void __launch_bounds__(1024) sort_scan_kernel(int n, uint32_t* __restrict__ hist) {
   __shared__ uint32_t s_warp[33];
-  const int per = (n + 1023) / 1024;
-  const int b0 = threadIdx.x * per;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int seg = ((n + 31) / 32 + 31) / 32 * 32;   // per-warp segment, multiple of 32
+  const int begin = warp * seg, end = min(begin + seg, n);
   uint32_t sum = 0;
-  for (int k = 0; k < per; ++k)
-    if (b0 + k < n) sum += hist[b0 + k];
-  uint32_t total;
-  uint32_t run = block_exclusive_scan(sum, s_warp, &total);
-  for (int k = 0; k < per; ++k)
-    if (b0 + k < n) {
-      const uint32_t v = hist[b0 + k];
-      hist[b0 + k] = run;
-      run += v;
-    }
+  for (int i = begin + lane; i < end; i += 32) sum += hist[i];
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  if (lane == 0) s_warp[warp] = sum;
+  __syncthreads();
+  if (warp == 0) {
+    const uint32_t w = s_warp[lane];
+    const uint32_t wi = warp_inclusive_scan(w, lane);
+    s_warp[lane] = wi - w;
+  }
+  __syncthreads();
+  uint32_t run = s_warp[warp];
+  for (int i0 = begin; i0 < end; i0 += 32) {
+    const int i = i0 + lane;
+    const uint32_t v = i < end ? hist[i] : 0u;
+    const uint32_t inc = warp_inclusive_scan(v, lane);
+    if (i < end) hist[i] = run + inc - v;
+    run += __shfl_sync(0xffffffffu, inc, 31);
+  }
 }
 
 __global__ void __launch_bounds__(kSortThreads) sort_scatter_kernel(const Status* __restrict__ status, uint32_t capacity,
@@ -313,6 +327,7 @@ cudaError_t launch_sort(satsplat_ctx* c, cudaStream_t s) {
   int cur = 0;
   for (int p = 0; p < passes; ++p) {
     const int shift = 8 * p;
+    g_kernel_launches += 3;
     sort_hist_kernel<<<kSortBlocks, kSortThreads, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[cur], shift, c->hist);
     sort_scan_kernel<<<1, 1024, 0, s>>>(256 * kSortBlocks, c->hist);
     sort_scatter_kernel<<<kSortBlocks, kSortThreads, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[cur], c->vals[cur],
@@ -339,6 +354,7 @@ __global__ void __launch_bounds__(256) ranges_kernel(const Status* __restrict__ 
 cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
   cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
+  ++g_kernel_launches;
   ranges_kernel<<<148 * 8, 256, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[c->sorted], c->ranges);
   return cudaGetLastError();
 }

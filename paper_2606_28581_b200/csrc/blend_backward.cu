@@ -78,8 +78,9 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 template <bool DEPTH_ONLY>
-__global__ void __launch_bounds__(256) blend_backward_kernel(const __grid_constant__ BwdParams P) {
+__global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_constant__ BwdParams P) {
   __shared__ float4 s_r0[kBatchB], s_r1[kBatchB], s_r2[kBatchB], s_r3[kBatchB];
+  __shared__ float4 s_bb[kBatchB];
   __shared__ uint32_t s_id[kBatchB];
   __shared__ float s_grad[kBatchB * 16];
   __shared__ float s_red[8][24];
@@ -93,6 +94,8 @@ __global__ void __launch_bounds__(256) blend_backward_kernel(const __grid_consta
   const bool inside = ix < P.cam.W && iy < P.cam.H;
   const float px = (float)ix + 0.5f, py = (float)iy + 0.5f;
   const size_t o = (size_t)iy * P.cam.W + ix;
+  const float wx0 = (float)(blockIdx.x * kTile + (warp & 1) * 8) + 0.5f, wx1 = wx0 + 7.0f;
+  const float wy0 = (float)(blockIdx.y * kTile + (warp >> 1) * 4) + 0.5f, wy1 = wy0 + 3.0f;
 
   // ---- per-pixel state and epilogue backward ----
   float T = 1.f, Tf = 1.f, zref = 0.f, M1 = 0.f, M2 = 0.f, A = 0.f;
@@ -203,13 +206,26 @@ __global__ void __launch_bounds__(256) blend_backward_kernel(const __grid_consta
       const uint32_t id = P.vals[start + rel0 + threadIdx.x];
       const float4* r = P.rec + 4 * (size_t)id;
       s_id[threadIdx.x] = id;
-      s_r0[threadIdx.x] = r[0];
-      s_r1[threadIdx.x] = r[1];
+      const float4 q0 = r[0], q1 = r[1];
+      s_r0[threadIdx.x] = q0;
+      s_r1[threadIdx.x] = q1;
+      s_bb[threadIdx.x] = splat_bbox(q0, q1);
       s_r2[threadIdx.x] = r[2];
       if (!DEPTH_ONLY) s_r3[threadIdx.x] = r[3];
     }
     __syncthreads();
-    for (int j = n - 1; j >= 0; --j) {
+    const int wlast = __reduce_max_sync(0xffffffffu, last);   // nothing beyond this index matters to this warp
+    for (int g0 = ((n - 1) >> 5) << 5; g0 >= 0; g0 -= 32) {
+      bool hit = false;
+      if (g0 + lane < n && rel0 + g0 + lane < wlast) {
+        const float4 bb = s_bb[g0 + lane];
+        hit = bb.x <= wx1 && bb.y >= wx0 && bb.z <= wy1 && bb.w >= wy0;
+      }
+      unsigned mask = __ballot_sync(0xffffffffu, hit);
+      while (mask) {
+      const int bit = 31 - __clz(mask);
+      mask &= ~(1u << bit);
+      const int j = g0 + bit;
       const float4 r0 = s_r0[j], r1 = s_r1[j];
       const float dx = px - r0.x, dy = py - r0.y;
       const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
@@ -271,6 +287,7 @@ __global__ void __launch_bounds__(256) blend_backward_kernel(const __grid_consta
       }
       const float tot = warp_reduce16_transposed(g, lane);
       if (!(lane & 1) && tot != 0.f) atomicAdd(&s_grad[j * 16 + slot], tot);
+      }
     }
     __syncthreads();
     // flush this batch: one coalesced atomic per non-zero gradient component of each (tile, surfel) pair
@@ -308,6 +325,7 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.red = want_red ? c->red_buf : nullptr;
   if (want_red) cudaMemsetAsync(c->red_buf, 0, 32 * sizeof(float), s);
   const dim3 grid(c->cam.TX, c->cam.TY);
+  ++g_kernel_launches;
   if (depth_only)
     blend_backward_kernel<true><<<grid, 256, 0, s>>>(P);
   else

@@ -108,6 +108,7 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
                                   const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
                                   float* v_rgb, float* v_dF, cudaStream_t s) {
   if (c->N == 0) return cudaSuccess;
+  ++g_kernel_launches;
   chain_backward_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>(c->cam, (int)c->N, means, quats, scales, logits, c->count,
                                                                   c->flags, reinterpret_cast<float4*>(c->vrec), v_means,
                                                                   v_quats, v_scales, v_logits, v_rgb, v_dF);
@@ -118,6 +119,7 @@ __global__ void add_small_kernel(float* dst, const float* src, int n) {
   if ((int)threadIdx.x < n) dst[threadIdx.x] += src[threadIdx.x];
 }
 cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s) {
+  ++g_kernel_launches;
   add_small_kernel<<<1, 32, 0, s>>>(dst, src, n);
   return cudaGetLastError();
 }

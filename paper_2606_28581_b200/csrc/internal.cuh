@@ -48,13 +48,28 @@ struct DevShading {
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 8;
 constexpr int kSortTile = kSortThreads * kSortItems;  // 2048 keys
-constexpr int kSortBlocks = 148 * 4;                  // fixed grid: K lives on the device
+constexpr int kSortBlocks = 148 * 2;                  // fixed grid: K lives on the device
 
 struct Status {           // device-resident status words
   unsigned int K;         // duplicated keys of the last preprocess (may exceed capacity)
   unsigned int overflow;  // K > max_duplicates
   unsigned int pad[2];
 };
+
+// Conservative screen-space bounding box (x_min, x_max, y_min, y_max) of the pixel centres a splat can touch
+// (rho <= 9 under Eq. 12): the 3-sigma ellipse of M = Q^-1, widened to the 3-sigma low-pass disc, slightly inflated
+// so that fp32 rounding can never drop a contributor.  Used only to skip work; the per-pixel rho test decides.
+__device__ __forceinline__ float4 splat_bbox(const float4 r0, const float4 r1) {
+  const float det = r0.z * r1.y - r0.w * r1.x;
+  const float id = 3.0f / fabsf(det);
+  float ex = id * sqrtf(r1.y * r1.y + r0.w * r0.w);   // 3 |row 0 of M|
+  float ey = id * sqrtf(r1.x * r1.x + r0.z * r0.z);   // 3 |row 1 of M|
+  ex = fmaxf(ex, kMinExtent) * 1.0001f + 1e-3f;
+  ey = fmaxf(ey, kMinExtent) * 1.0001f + 1e-3f;
+  if (!(ex < 1e30f)) ex = 1e30f;                       // NaN / inf (det underflow) -> never culled
+  if (!(ey < 1e30f)) ey = 1e30f;
+  return make_float4(r0.x - ex, r0.x + ex, r0.y - ey, r0.y + ey);
+}
 
 // Shadow-test lookup shared by the forward epilogue and its backward so that both take the same in-map /
 // texel decisions from the same bits (explicit fma sequence: no compiler-dependent contraction).
@@ -129,6 +144,8 @@ struct satsplat_ctx {
 };
 
 namespace satsplat {
+
+extern long long g_kernel_launches;  // cumulative kernel launches of this process (bench.py's gpu_launches)
 
 // launchers (each enqueues on `s`, returns the cudaError_t of the launch)
 cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, const float* quats, const float* scales,

@@ -105,6 +105,7 @@ cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, co
   if (N == 0) return cudaSuccess;
   const int threads = 256;
   const int blocks = (int)((N + threads - 1) / threads);
+  ++g_kernel_launches;
   preprocess_kernel<<<blocks, threads, 0, s>>>(c->cam, (int)N, means, quats, scales, logits, rgb, c->rec,
                                                reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags);
   return cudaGetLastError();
@@ -131,6 +132,7 @@ __global__ void export_records_kernel(int N, const float4* __restrict__ rec, con
 
 cudaError_t launch_export_records(satsplat_ctx* c, float* records_out, uint8_t* flags_out, cudaStream_t s) {
   if (c->N == 0) return cudaSuccess;
+  ++g_kernel_launches;
   export_records_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>((int)c->N, c->rec, c->count, c->flags, records_out, flags_out);
   return cudaGetLastError();
 }
