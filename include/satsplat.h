@@ -182,6 +182,18 @@ int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const in
 int satsplat_set_profiling(satsplat_ctx* ctx, int32_t enabled);
 int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out);
 
+/* Options (HOST call; takes effect at the next satsplat_preprocess).
+ *   SATSPLAT_OPT_BINNING: how (a2) builds the sorted (tile, depth, surfel) list.  Both give the same, unique,
+ *     bit-exact result (keys, order, ranges):
+ *       SATSPLAT_BINNING_TILESORT (default) per-tile counts with atomics -> tile scan (= ranges) -> scatter -> one
+ *                                           shared-memory sort per tile by (depth bits, surfel id); 4 launches
+ *       SATSPLAT_BINNING_RADIX              per-surfel scan -> key duplication -> stable 8-bit LSD radix sort of the
+ *                                           64-bit keys -> range detection; the general-purpose device sort */
+#define SATSPLAT_OPT_BINNING 0
+#define SATSPLAT_BINNING_TILESORT 0
+#define SATSPLAT_BINNING_RADIX 1
+int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value);
+
 const char* satsplat_version(void);
 
 /* Cumulative number of CUDA kernels this library has launched in this process (all contexts). */

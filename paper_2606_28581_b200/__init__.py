@@ -16,6 +16,7 @@ _SO = os.path.join(_HERE, "libsatsplat.so")
 _LIB = None
 
 OK, E_INVALID, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4
+OPT_BINNING, BINNING_TILESORT, BINNING_RADIX = 0, 0, 1
 STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_fwd", "blend_bwd", "chain_bwd")
 
 
@@ -104,6 +105,7 @@ def lib():
         L.satsplat_debug_records.argtypes = [vp, vp, vp, vp]
         L.satsplat_debug_planes.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
         L.satsplat_set_profiling.argtypes = [vp, i32]
+        L.satsplat_set_option.argtypes = [vp, i32, i32]
         L.satsplat_stage_ms.argtypes = [vp, C.POINTER(f32)]
         _LIB = L
     return _LIB
@@ -254,6 +256,9 @@ class Context:
         torch.cuda.synchronize()
         outs = [_wrap(p.value, H * W * 4, dev).view(torch.int32).view(H, W) for p in (a, b)]
         return outs
+
+    def set_option(self, option: int, value: int):
+        self._rc(lib().satsplat_set_option(self._h, int(option), int(value)))
 
     def set_profiling(self, enabled: bool):
         self._rc(lib().satsplat_set_profiling(self._h, 1 if enabled else 0))

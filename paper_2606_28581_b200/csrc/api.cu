@@ -131,6 +131,11 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->hist, (size_t)256 * kSortBlocks));
   A(dalloc(ctx, &ctx->ranges, tiles * 2));
   A(dalloc(ctx, &ctx->status, 1));
+  A(dalloc(ctx, &ctx->tile_count, tiles));
+  A(dalloc(ctx, &ctx->tile_start, tiles));
+  A(dalloc(ctx, &ctx->worklist, tiles));
+  A(dalloc(ctx, &ctx->wl_count, 4));
+  A(cudaMemset(ctx->tile_count, 0, tiles * sizeof(uint32_t)));
   A(dalloc(ctx, &ctx->px_a, px));
   A(dalloc(ctx, &ctx->px_b, px));
   A(dalloc(ctx, &ctx->px_i, px));
@@ -155,7 +160,8 @@ void satsplat_destroy(satsplat_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   void* ptrs[] = {ctx->rec, ctx->rect, ctx->count, ctx->offset, ctx->depth_key, ctx->flags, ctx->vrec, ctx->block_sums,
-                  ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->px_a,
+                  ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->tile_count,
+                  ctx->tile_start, ctx->worklist, ctx->wl_count, ctx->px_a,
                   ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in, ctx->e2e_up,
                   ctx->e2e_out, ctx->e2e_grads};
   for (void* p : ptrs)
@@ -225,11 +231,20 @@ int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N
   ctx->preprocessed = 0;
   ctx->forwarded = 0;
   clear_stage_marks(ctx, {0, 1, 2, 3, 4, 5, 6, 7});
-  { StageTimer t(ctx, SATSPLAT_STAGE_PREPROCESS, s); CU(launch_preprocess(ctx, N, means, quats, scales, opacity_logits, rgb, s)); }
-  { StageTimer t(ctx, SATSPLAT_STAGE_SCAN, s); CU(launch_scan(ctx, N, s)); }
-  { StageTimer t(ctx, SATSPLAT_STAGE_DUPLICATE, s); CU(launch_duplicate(ctx, N, s)); }
-  { StageTimer t(ctx, SATSPLAT_STAGE_SORT, s); CU(launch_sort(ctx, s)); }
-  { StageTimer t(ctx, SATSPLAT_STAGE_RANGES, s); CU(launch_ranges(ctx, s)); }
+  if (ctx->binning_mode == SATSPLAT_BINNING_TILESORT) {
+    // tile_count is all zero here: create() clears it, tile_scan turns it into the scatter cursor and the tile
+    // sort clears it again, all on this stream
+    { StageTimer t(ctx, SATSPLAT_STAGE_PREPROCESS, s); CU(launch_preprocess(ctx, N, means, quats, scales, opacity_logits, rgb, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_SCAN, s); CU(launch_tile_scan(ctx, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_DUPLICATE, s); CU(launch_tile_scatter(ctx, N, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_SORT, s); CU(launch_tile_sort(ctx, s)); }
+  } else {
+    { StageTimer t(ctx, SATSPLAT_STAGE_PREPROCESS, s); CU(launch_preprocess(ctx, N, means, quats, scales, opacity_logits, rgb, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_SCAN, s); CU(launch_scan(ctx, N, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_DUPLICATE, s); CU(launch_duplicate(ctx, N, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_SORT, s); CU(launch_sort(ctx, s)); }
+    { StageTimer t(ctx, SATSPLAT_STAGE_RANGES, s); CU(launch_ranges(ctx, s)); }
+  }
   ctx->preprocessed = 1;
   return SATSPLAT_OK;
 }
@@ -356,6 +371,17 @@ int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const in
   if (n_visited) *n_visited = ctx->px_visited;
   if (n_contrib) *n_contrib = ctx->px_contrib;
   return SATSPLAT_OK;
+}
+
+int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_set_option: ctx is NULL");
+  if (option == SATSPLAT_OPT_BINNING && (value == SATSPLAT_BINNING_TILESORT || value == SATSPLAT_BINNING_RADIX)) {
+    ctx->binning_mode = value;
+    ctx->preprocessed = 0;
+    ctx->forwarded = 0;
+    return SATSPLAT_OK;
+  }
+  return fail(ctx, SATSPLAT_E_INVALID, "satsplat_set_option: unknown option or value");
 }
 
 int satsplat_set_profiling(satsplat_ctx* ctx, int32_t enabled) {

@@ -359,4 +359,294 @@ cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
   return cudaGetLastError();
 }
 
+// ============================================================================================================
+// Tile-sort binning (default mode): the same unique result as the stable radix sort above — entries ordered by
+// (tile id, depth bits, surfel id) — but built the way the data wants on B200: the (tile, surfel) pairs of one
+// view (2 M at C3) sit in L2, so instead of 6 full radix passes we
+//   1. count pairs per tile with fire-and-forget RED atomics (fused into the preprocess kernel),
+//   2. exclusive-scan the per-tile counts (this IS the tile-range table),
+//   3. scatter (depth bits << 32 | surfel id) entries into their tile's segment in arrival order,
+//   4. sort every segment in shared memory by the 64-bit (depth, id) composite, one warp per tile.
+// Arrival order is nondeterministic, the sorted result is not: (depth, id) is a total order and each surfel occurs
+// at most once per tile.  4 launches instead of 25, ~10x less traffic.
+// ============================================================================================================
+
+// single CTA: exclusive scan of tile_count[tiles]; writes ranges, K, overflow; resets the cursors and the worklist.
+// Chunks of 1024 x 8 counters are staged through shared memory so that every global access is coalesced.
+constexpr int kTileScanItems = 8;
+__global__ void __launch_bounds__(1024) tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_start,
+                                                         uint32_t* __restrict__ ranges, Status* status, uint32_t capacity,
+                                                         uint32_t* __restrict__ wl_count) {
+  __shared__ uint32_t s_warp[33];
+  __shared__ uint32_t s_cnt[1024 * kTileScanItems + 8];
+  __shared__ uint32_t s_total;
+  constexpr int kChunk = 1024 * kTileScanItems;
+  // pass 1: total (decides overflow before any range is written)
+  uint32_t sum = 0;
+  for (int i = threadIdx.x; i < tiles; i += 1024) sum += tile_count[i];
+  uint32_t total;
+  block_exclusive_scan(sum, s_warp, &total);
+  const bool overflow = total > capacity;
+  uint32_t carry = 0;
+  for (int base = 0; base < tiles; base += kChunk) {
+    const int n = min(kChunk, tiles - base);
+    for (int i = threadIdx.x; i < n; i += 1024) {
+      s_cnt[i] = tile_count[base + i];
+      tile_count[base + i] = 0;                     // becomes the scatter cursor
+    }
+    __syncthreads();
+    uint32_t v[kTileScanItems], part = 0;
+#pragma unroll
+    for (int k = 0; k < kTileScanItems; ++k) {
+      const int i = threadIdx.x * kTileScanItems + k;
+      v[k] = i < n ? s_cnt[i] : 0u;
+      part += v[k];
+    }
+    uint32_t chunk_total;
+    uint32_t run = carry + block_exclusive_scan(part, s_warp, &chunk_total);
+#pragma unroll
+    for (int k = 0; k < kTileScanItems; ++k) {
+      const int i = threadIdx.x * kTileScanItems + k;
+      if (i < n) s_cnt[i] = run;                    // exclusive prefix, back in place
+      run += v[k];
+    }
+    if (threadIdx.x == 1023) s_total = run;         // = carry + chunk_total
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += 1024) {
+      const uint32_t st = s_cnt[i];
+      const uint32_t en = (i + 1 < n) ? s_cnt[i + 1] : s_total;
+      tile_start[base + i] = st;
+      const bool empty = en == st || overflow;      // overflow: nothing is rendered (outputs undefined, no OOB access)
+      reinterpret_cast<uint2*>(ranges)[base + i] = empty ? make_uint2(0u, 0u) : make_uint2(st, en);
+    }
+    carry += chunk_total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    status->K = total;
+    status->overflow = overflow ? 1u : 0u;
+    wl_count[0] = 0;
+    wl_count[1] = 0;
+  }
+}
+
+__global__ void __launch_bounds__(256) tile_scatter_kernel(int N, int TX, const ushort4* __restrict__ rect,
+                                                           const uint32_t* __restrict__ count,
+                                                           const uint32_t* __restrict__ depth_key,
+                                                           const uint32_t* __restrict__ tile_start, uint32_t* __restrict__ cursor,
+                                                           const Status* __restrict__ status, uint64_t* __restrict__ entries) {
+  if (status->overflow) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  uint32_t cnt = 0, dk = 0;
+  ushort4 r = make_ushort4(0, 0, 0, 0);
+  if (i < N) {
+    cnt = count[i];
+    if (cnt) { dk = depth_key[i]; r = rect[i]; }
+  }
+  if (cnt && cnt <= kDupCoopThreshold) {
+    const uint64_t e = ((uint64_t)dk << 32) | (uint32_t)i;
+    for (int ty = r.y; ty < r.w; ++ty)
+      for (int tx = r.x; tx < r.z; ++tx) {
+        const int t = ty * TX + tx;
+        entries[tile_start[t] + atomicAdd(cursor + t, 1u)] = e;
+      }
+  }
+  unsigned big = __ballot_sync(0xffffffffu, cnt > kDupCoopThreshold);
+  while (big) {
+    const int src = __ffs(big) - 1;
+    big &= big - 1;
+    const uint32_t c2 = __shfl_sync(0xffffffffu, cnt, src);
+    const uint32_t k2 = __shfl_sync(0xffffffffu, dk, src);
+    const int x0 = __shfl_sync(0xffffffffu, (int)r.x, src), y0 = __shfl_sync(0xffffffffu, (int)r.y, src);
+    const int x1 = __shfl_sync(0xffffffffu, (int)r.z, src);
+    const uint32_t id = (uint32_t)((blockIdx.x * blockDim.x + (threadIdx.x & ~31)) + src);
+    const int w = x1 - x0;
+    const uint64_t e = ((uint64_t)k2 << 32) | id;
+    for (uint32_t q = lane; q < c2; q += 32) {
+      const int t = (y0 + (int)(q / (uint32_t)w)) * TX + x0 + (int)(q % (uint32_t)w);
+      entries[tile_start[t] + atomicAdd(cursor + t, 1u)] = e;
+    }
+  }
+}
+
+// Bitonic sort, all comparisons ascending (flip + half-cleaner form), so indices >= n behave as +inf padding and
+// are simply skipped.  `buf` may point to shared or global memory; `sync` is __syncwarp or __syncthreads.
+template <typename Sync>
+__device__ __forceinline__ void bitonic_sort_asc(uint64_t* buf, uint32_t n, uint32_t tid, uint32_t nthreads, Sync sync) {
+  uint32_t P = 2;
+  while (P < n) P <<= 1;
+  for (uint32_t k = 2; k <= P; k <<= 1) {
+    {  // flip: a = base + off, b = base + k - 1 - off
+      const uint32_t h = k >> 1;
+      for (uint32_t i = tid; i < (P >> 1); i += nthreads) {
+        const uint32_t base = (i / h) * k, off = i & (h - 1);
+        const uint32_t a = base + off, b = base + k - 1 - off;
+        if (b < n) {
+          const uint64_t x = buf[a], y = buf[b];
+          if (x > y) { buf[a] = y; buf[b] = x; }
+        }
+      }
+      sync();
+    }
+    for (uint32_t j = k >> 2; j > 0; j >>= 1) {
+      for (uint32_t i = tid; i < (P >> 1); i += nthreads) {
+        const uint32_t a = ((i & ~(j - 1)) << 1) | (i & (j - 1)), b = a + j;
+        if (b < n) {
+          const uint64_t x = buf[a], y = buf[b];
+          if (x > y) { buf[a] = y; buf[b] = x; }
+        }
+      }
+      sync();
+    }
+  }
+}
+
+constexpr int kTileSortWarps = 8;         // warps (= tiles) per CTA
+constexpr int kTileSortWarpMax = 1024;    // entries one warp sorts in registers (32 per lane)
+constexpr int kTileSortCtaMax = 16384;    // entries one CTA sorts in shared memory (large-tile kernel)
+
+// Warp-wide bitonic sort of 32*E 64-bit values held in registers, blocked layout: element index of v[e] is
+// lane*E + e.  Strides >= E exchange through shuffles (run-time loop: the body is the same for every stride), strides
+// below E are register-to-register.  Only the loop over e is unrolled, so the code stays small (an earlier fully
+// unrolled version spent 40 % of its issue slots waiting on the instruction cache, profiles/r1_binning.md).
+template <int E>
+__device__ __forceinline__ void warp_bitonic_regs(uint64_t (&v)[E], int lane) {
+  for (int k = 2; k <= 32 * E; k <<= 1) {
+    for (int j = k >> 1; j >= E; j >>= 1) {           // partner in another lane (k > j >= E: direction is per lane)
+      const int m = j / E;
+      const bool take_min = ((lane & m) == 0) == (((lane * E) & k) == 0);
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const uint64_t x = v[e];
+        const uint64_t y = __shfl_xor_sync(0xffffffffu, x, m);
+        v[e] = ((x < y) == take_min) ? x : y;
+      }
+    }
+#pragma unroll
+    for (int js = E >> 1; js >= 1; js >>= 1) {        // partner in this lane's registers
+      if (js < k) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          if ((e & js) == 0) {
+            const bool up = (((lane * E + e) & k) == 0);
+            const uint64_t x = v[e], y = v[e | js];
+            const bool sw = (x > y) == up;
+            v[e] = sw ? y : x;
+            v[e | js] = sw ? x : y;
+          }
+        }
+      }
+    }
+  }
+}
+
+template <int E>
+__device__ __noinline__ void tile_sort_warp(const uint64_t* __restrict__ in, uint32_t n, uint64_t hi, uint64_t* __restrict__ keys,
+                                            uint32_t* __restrict__ vals, int lane) {
+  uint64_t v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const uint32_t i = lane * E + e;
+    v[e] = i < n ? in[i] : ~0ull;                     // +inf padding sorts to the end (real entries are unique)
+  }
+  warp_bitonic_regs<E>(v, lane);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const uint32_t i = lane * E + e;
+    if (i < n) {
+      keys[i] = hi | (v[e] >> 32);
+      vals[i] = (uint32_t)v[e];
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tiles, const uint32_t* __restrict__ ranges,
+                                                                        const uint64_t* __restrict__ entries,
+                                                                        uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                                        uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count,
+                                                                        uint32_t* __restrict__ cursor) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = blockIdx.x * kTileSortWarps + warp;
+  if (t >= tiles) return;
+  if (lane == 0) cursor[t] = 0;   // leave the per-tile counters zero for the next preprocess on this context
+  const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
+  if (n == 0) return;
+  if (n > (uint32_t)kTileSortWarpMax) {
+    if (lane == 0) worklist[atomicAdd(wl_count, 1u)] = (uint32_t)t;
+    return;
+  }
+  const uint64_t hi = (uint64_t)(uint32_t)t << 32;
+  const uint64_t* in = entries + s;
+  uint64_t* ko = keys + s;
+  uint32_t* vo = vals + s;
+  if (n <= 64) tile_sort_warp<2>(in, n, hi, ko, vo, lane);
+  else if (n <= 256) tile_sort_warp<8>(in, n, hi, ko, vo, lane);
+  else tile_sort_warp<32>(in, n, hi, ko, vo, lane);
+}
+
+// tiles with more than kTileSortWarpMax entries (oversized splats; tiny images): one 1024-thread CTA
+// per worklist item, in shared memory up to kTileSortCtaMax entries, else in place in global memory.
+__global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* __restrict__ ranges, uint64_t* __restrict__ entries,
+                                                               uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                               const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
+  extern __shared__ uint64_t s_big[];
+  __shared__ uint32_t s_item;
+  const uint32_t total = wl_count[0];
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_item = atomicAdd(wl_count + 1, 1u);
+    __syncthreads();
+    const uint32_t item = s_item;
+    if (item >= total) return;
+    const uint32_t t = worklist[item];
+    const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
+    uint64_t* buf;
+    if (n <= (uint32_t)kTileSortCtaMax) {
+      buf = s_big;
+      for (uint32_t i = threadIdx.x; i < n; i += 1024) buf[i] = entries[s + i];
+    } else {
+      buf = entries + s;
+    }
+    __syncthreads();
+    bitonic_sort_asc(buf, n, threadIdx.x, 1024, [] { __syncthreads(); });
+    const uint64_t hi = (uint64_t)t << 32;
+    for (uint32_t i = threadIdx.x; i < n; i += 1024) {
+      const uint64_t v = buf[i];
+      keys[s + i] = hi | (v >> 32);
+      vals[s + i] = (uint32_t)v;
+    }
+  }
+}
+
+cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s) {
+  const int tiles = c->cam.TX * c->cam.TY;
+  ++g_kernel_launches;
+  tile_scan_kernel<<<1, 1024, 0, s>>>(tiles, c->tile_count, c->tile_start, c->ranges, c->status, (uint32_t)c->max_dup, c->wl_count);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s) {
+  if (N == 0) return cudaSuccess;
+  ++g_kernel_launches;
+  tile_scatter_kernel<<<(int)((N + 255) / 256), 256, 0, s>>>((int)N, c->cam.TX, reinterpret_cast<const ushort4*>(c->rect), c->count,
+                                                             c->depth_key, c->tile_start, c->tile_count, c->status, c->keys[1]);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
+  const int tiles = c->cam.TX * c->cam.TY;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
+    attr_set = true;
+  }
+  g_kernel_launches += 2;
+  tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(
+      tiles, c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count, c->tile_count);
+  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  c->sorted = 0;
+  return cudaGetLastError();
+}
+
 }  // namespace satsplat

@@ -117,6 +117,11 @@ struct satsplat_ctx {
   int sorted;             // which buffer holds the sorted result
   uint32_t* hist;         // [256 * kSortBlocks]
   uint32_t* ranges;       // [tiles*2]
+  uint32_t* tile_count;   // [tiles] tile-sort binning: pair count per tile, then the scatter cursor
+  uint32_t* tile_start;   // [tiles] exclusive scan of tile_count
+  uint32_t* worklist;     // [tiles] tiles too long for the one-warp sort
+  uint32_t* wl_count;     // [2] worklist length, consumer cursor
+  int binning_mode;       // SATSPLAT_BINNING_TILESORT (default) or SATSPLAT_BINNING_RADIX
   satsplat::Status* status;
   // per-pixel state kept for the backward
   float4* px_a;           // (T_f, z_ref, M1', M2')
@@ -154,6 +159,9 @@ cudaError_t launch_scan(satsplat_ctx* c, int64_t N, cudaStream_t s);
 cudaError_t launch_duplicate(satsplat_ctx* c, int64_t N, cudaStream_t s);
 cudaError_t launch_sort(satsplat_ctx* c, cudaStream_t s);
 cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s);
+cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s);
+cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s);
+cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s);
 cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* out_rgba, float* out_geom, float* out_aux,
                                  float* sun_depth_out, bool depth_only, cudaStream_t s);
 cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* v_rgba, const float* v_geom,

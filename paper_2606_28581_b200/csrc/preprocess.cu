@@ -23,9 +23,10 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
                                                          const float* __restrict__ logits, const float* __restrict__ rgb,
                                                          float4* __restrict__ rec, ushort4* __restrict__ rect,
                                                          uint32_t* __restrict__ count, uint32_t* __restrict__ depth_key,
-                                                         uint8_t* __restrict__ flags) {
+                                                         uint8_t* __restrict__ flags, uint32_t* __restrict__ tile_count) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
+  int cnt = 0, tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
+  if (i < N) {
   const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
   const float4 q = reinterpret_cast<const float4*>(quats)[i];
   const float2 sc = reinterpret_cast<const float2*>(scales)[i];
@@ -61,7 +62,6 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   // 8. cull
   const bool cull = logit < kLogitCull || !(n2 > 0.0f) || !(sc.x > 0.0f) || !(sc.y > 0.0f) || !isfinite(n2) ||
                     !isfinite(cx) || !isfinite(cy) || !isfinite(extx) || !isfinite(exty) || !isfinite(zc);
-  int tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
   if (!cull) {
     // 7. tile rect
     tx0 = min(max(tile_of(__fsub_rn(cx, extx), cam.TX), 0), cam.TX);
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   } else {
     fl |= F_CULLED;
   }
-  const int cnt = cull ? 0 : max(tx1 - tx0, 0) * max(ty1 - ty0, 0);
+  cnt = cull ? 0 : max(tx1 - tx0, 0) * max(ty1 - ty0, 0);
   rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
   count[i] = (uint32_t)cnt;
   depth_key[i] = k;
@@ -98,6 +98,24 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
     r[2] = make_float4(g0, g1, rgb[3 * i], rgb[3 * i + 1]);
     r[3] = make_float4(rgb[3 * i + 2], n0, n1, nz);
   }
+  }
+  // tile-sort binning: count the (tile, surfel) pairs per tile with fire-and-forget RED atomics; surfels covering
+  // many tiles (oversized splats) are expanded by the whole warp
+  if (tile_count == nullptr) return;
+  if (cnt > 0 && cnt <= 16) {
+    for (int ty = ty0; ty < ty1; ++ty)
+      for (int tx = tx0; tx < tx1; ++tx) atomicAdd(tile_count + ty * cam.TX + tx, 1u);
+  }
+  unsigned big = __ballot_sync(0xffffffffu, cnt > 16);
+  const int lane = threadIdx.x & 31;
+  while (big) {
+    const int src = __ffs(big) - 1;
+    big &= big - 1;
+    const int c2 = __shfl_sync(0xffffffffu, cnt, src);
+    const int x0 = __shfl_sync(0xffffffffu, tx0, src), y0 = __shfl_sync(0xffffffffu, ty0, src);
+    const int w = __shfl_sync(0xffffffffu, tx1, src) - x0;
+    for (int q = lane; q < c2; q += 32) atomicAdd(tile_count + (y0 + q / w) * cam.TX + x0 + q % w, 1u);
+  }
 }
 
 cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, const float* quats, const float* scales,
@@ -107,7 +125,8 @@ cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, co
   const int blocks = (int)((N + threads - 1) / threads);
   ++g_kernel_launches;
   preprocess_kernel<<<blocks, threads, 0, s>>>(c->cam, (int)N, means, quats, scales, logits, rgb, c->rec,
-                                               reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags);
+                                               reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags,
+                                               c->binning_mode == SATSPLAT_BINNING_TILESORT ? c->tile_count : nullptr);
   return cudaGetLastError();
 }
 

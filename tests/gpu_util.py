@@ -30,7 +30,7 @@ class GpuScene:
 
 
 def gpu_view_iteration(P, gs: GpuScene, view, *, sun_view=None, reproj=None, upstream=None, sun_upstream=None,
-                       do_backward=True, max_dup=None, ctx=None, sun_ctx=None, want_debug=True):
+                       do_backward=True, max_dup=None, ctx=None, sun_ctx=None, want_debug=True, binning=None):
     """One view through the CUDA path.  `sun_view`/`reproj`: the fp32 sun camera + reprojection constants (inputs)."""
     n = gs.n
     H, W = view.height, view.width
@@ -41,11 +41,15 @@ def gpu_view_iteration(P, gs: GpuScene, view, *, sun_view=None, reproj=None, ups
     if ctx is None:
         ctx = P.Context(max(n, 1), W, H, max_dup)
         own.append(ctx)
+    if binning is not None:
+        ctx.set_option(P.OPT_BINNING, binning)
     sun_depth = None
     if sun_view is not None:
         if sun_ctx is None:
             sun_ctx = P.Context(max(n, 1), sun_view.width, sun_view.height, max_dup)
             own.append(sun_ctx)
+        if binning is not None:
+            sun_ctx.set_option(P.OPT_BINNING, binning)
         scam = P.Camera.from_view(sun_view)
         sun_ctx.preprocess(scam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
         sun_depth = torch.empty(sun_view.height, sun_view.width, device="cuda", dtype=torch.float32)
