@@ -427,6 +427,8 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int tiles, uint32_t* __
     status->overflow = overflow ? 1u : 0u;
     wl_count[0] = 0;
     wl_count[1] = 0;
+    wl_count[2] = 0;
+    wl_count[3] = 0;
   }
 }
 
@@ -561,6 +563,10 @@ __device__ __noinline__ void tile_sort_warp(const uint64_t* __restrict__ in, uin
   }
 }
 
+// Tiles are dispatched by list length so that each kernel keeps the register budget (and occupancy) of its own
+// variants: <= 256 entries here (2/4/8 registers per lane), 257..1024 in tile_sort_mid_kernel (16/32 per lane),
+// longer ones in tile_sort_large_kernel (one CTA per tile).  Worklists: [0, tiles) mid, [tiles, 2 tiles) large;
+// wl_count = {mid length, mid cursor, large length, large cursor}.
 __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tiles, const uint32_t* __restrict__ ranges,
                                                                         const uint64_t* __restrict__ entries,
                                                                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
@@ -572,17 +578,35 @@ __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tile
   if (lane == 0) cursor[t] = 0;   // leave the per-tile counters zero for the next preprocess on this context
   const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
   if (n == 0) return;
-  if (n > (uint32_t)kTileSortWarpMax) {
-    if (lane == 0) worklist[atomicAdd(wl_count, 1u)] = (uint32_t)t;
+  if (n > 256u) {
+    if (lane == 0) {
+      if (n > (uint32_t)kTileSortWarpMax) worklist[tiles + atomicAdd(wl_count + 2, 1u)] = (uint32_t)t;
+      else worklist[atomicAdd(wl_count, 1u)] = (uint32_t)t;
+    }
     return;
   }
   const uint64_t hi = (uint64_t)(uint32_t)t << 32;
-  const uint64_t* in = entries + s;
-  uint64_t* ko = keys + s;
-  uint32_t* vo = vals + s;
-  if (n <= 64) tile_sort_warp<2>(in, n, hi, ko, vo, lane);
-  else if (n <= 256) tile_sort_warp<8>(in, n, hi, ko, vo, lane);
-  else tile_sort_warp<32>(in, n, hi, ko, vo, lane);
+  if (n <= 64) tile_sort_warp<2>(entries + s, n, hi, keys + s, vals + s, lane);
+  else if (n <= 128) tile_sort_warp<4>(entries + s, n, hi, keys + s, vals + s, lane);
+  else tile_sort_warp<8>(entries + s, n, hi, keys + s, vals + s, lane);
+}
+
+__global__ void __launch_bounds__(128) tile_sort_mid_kernel(const uint32_t* __restrict__ ranges, const uint64_t* __restrict__ entries,
+                                                            uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                            const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t total = wl_count[0];
+  for (;;) {
+    uint32_t item = 0;
+    if (lane == 0) item = atomicAdd(wl_count + 1, 1u);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= total) return;
+    const uint32_t t = worklist[item];
+    const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
+    const uint64_t hi = (uint64_t)t << 32;
+    if (n <= 512) tile_sort_warp<16>(entries + s, n, hi, keys + s, vals + s, lane);
+    else tile_sort_warp<32>(entries + s, n, hi, keys + s, vals + s, lane);
+  }
 }
 
 // tiles with more than kTileSortWarpMax entries (oversized splats; tiny images): one 1024-thread CTA
@@ -592,10 +616,10 @@ __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* _
                                                                const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
   extern __shared__ uint64_t s_big[];
   __shared__ uint32_t s_item;
-  const uint32_t total = wl_count[0];
+  const uint32_t total = wl_count[2];
   for (;;) {
     __syncthreads();
-    if (threadIdx.x == 0) s_item = atomicAdd(wl_count + 1, 1u);
+    if (threadIdx.x == 0) s_item = atomicAdd(wl_count + 3, 1u);
     __syncthreads();
     const uint32_t item = s_item;
     if (item >= total) return;
@@ -641,10 +665,12 @@ cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
     cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
     attr_set = true;
   }
-  g_kernel_launches += 2;
+  g_kernel_launches += 3;
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(
       tiles, c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count, c->tile_count);
-  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_mid_kernel<<<148 * 4, 128, 0, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist + tiles,
+                                                               c->wl_count);
   c->sorted = 0;
   return cudaGetLastError();
 }

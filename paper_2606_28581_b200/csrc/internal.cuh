@@ -119,8 +119,8 @@ struct satsplat_ctx {
   uint32_t* ranges;       // [tiles*2]
   uint32_t* tile_count;   // [tiles] tile-sort binning: pair count per tile, then the scatter cursor
   uint32_t* tile_start;   // [tiles] exclusive scan of tile_count
-  uint32_t* worklist;     // [tiles] tiles too long for the one-warp sort
-  uint32_t* wl_count;     // [2] worklist length, consumer cursor
+  uint32_t* worklist;     // [2*tiles] tiles too long for the small-tile sort: mid list, then large list
+  uint32_t* wl_count;     // [4] mid length, mid cursor, large length, large cursor
   int binning_mode;       // SATSPLAT_BINNING_TILESORT (default) or SATSPLAT_BINNING_RADIX
   satsplat::Status* status;
   // per-pixel state kept for the backward
