@@ -27,11 +27,12 @@ sys.path.insert(0, ROOT)
 
 METRIC = "affine-2DGS fwd+bwd throughput at 1M surfels, 2048^2 view (C3 full iteration incl. shadow pass)"
 UNIT = "Mpixel/s"
-# algorithmic work per pair: FP32 flops, FMA = 2
-FLOP_EVAL = 26.0          # per evaluated (pixel, list entry) pair: Eq. 9 + Eq. 12 + exp + alpha tests
-FLOP_CONTRIB_FWD = 40.0   # extra per contributing pair, forward
-FLOP_CONTRIB_BWD = 110.0  # extra per contributing pair, backward
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz = 74.4
+# algorithmic work per pair: FP32-pipe lane-instructions of the paper's per-pixel loop
+INST_EVAL = 17.0          # per evaluated (pixel, list entry) pair: Eq. 9 + Eq. 12 + ex2 + alpha tests
+INST_CONTRIB_FWD = 25.0   # extra per contributing pair, forward (view pass; the depth-only sun pass: 6)
+INST_CONTRIB_BWD = 90.0   # extra per contributing pair, backward (view pass; sun pass: 50)
+INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN = 6.0, 50.0
+FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.965 GHz = 37.2 T lane-instr/s
 
 
 def parse():
@@ -231,6 +232,15 @@ class Job:
             self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], None)
 
 
+def max_over_ranks(torch, dist, world, value, device):
+    """MAX all-reduce of a per-rank scalar (device timings are reported as the max over ranks)."""
+    if world <= 1:
+        return float(value)
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def timed(torch, dist, world, fn, items):
     """Time fn(item) over items with CUDA events on the current stream; barrier + synchronize on both sides;
     returns the max over ranks of the elapsed milliseconds."""
@@ -246,12 +256,7 @@ def timed(torch, dist, world, fn, items):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    return ms
+    return max_over_ranks(torch, dist, world, e0.elapsed_time(e1), "cuda")
 
 
 def stage_profile(job, vi, peaks):
@@ -284,17 +289,17 @@ def stage_profile(job, vi, peaks):
         "duplicate": ("hbm", n * 16.0 + K * 12.0),
         "sort": ("hbm", K * (passes * 36.0)),
         "ranges": ("hbm", K * 8.0 + tiles * 8.0),
-        "blend_fwd": ("alu", pairs["view_evaluated"] * FLOP_EVAL + pairs["view_contributing"] * FLOP_CONTRIB_FWD),
-        "blend_bwd": ("alu", pairs["view_evaluated"] * FLOP_EVAL + pairs["view_contributing"] * FLOP_CONTRIB_BWD),
+        "blend_fwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_FWD),
+        "blend_bwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_BWD),
         "chain_bwd": ("hbm", n * (64.0 * 2 + 40.0 + 52.0 * 2)),
     }
     stages = {}
     for k, ms in ms_view.items():
         bound, w = work[k]
         ach = w / (ms * 1e-3) / (1e12 if bound == "alu" else 1e9) if ms > 0 else 0.0
-        peak = FP32_PEAK_TFLOPS if bound == "alu" else peaks["hbm_gbs"]
+        peak = FP32_PEAK_TINST if bound == "alu" else peaks["hbm_gbs"]
         stages[k] = dict(ms=ms, sun_ms=ms_sun.get(k, 0.0), bound=bound, achieved=ach, peak=peak,
-                         unit="TFLOP/s" if bound == "alu" else "GB/s", frac=ach / peak if peak else None)
+                         unit="Tinst/s" if bound == "alu" else "GB/s", frac=ach / peak if peak else None)
     return stages, pairs, px
 
 
@@ -342,7 +347,7 @@ def run_ours(args):
         dom = max(stages, key=lambda k: stages[k]["ms"])
         d = stages[dom]
         line["roofline"] = dict(kernel=dom, bound=d["bound"], achieved=d["achieved"], peak=d["peak"], unit=d["unit"], frac=d["frac"],
-                                traffic=None, peak_source=("derived: 148 SM x 128 lanes x 2 x 1.965 GHz" if d["bound"] == "alu"
+                                traffic=None, peak_source=("derived: 148 SM x 128 FP32 lanes x 1.965 GHz (DESIGN.md section 5)" if d["bound"] == "alu"
                                                            else peaks["source"] + " HBM copy"),
                                 kernel_ms=d["ms"])
         line["stages"] = stages
@@ -384,10 +389,7 @@ def run_ours(args):
             e2e_step(i)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(torch, dist, world, dt, "cuda")
         h2d = scene.n * 56 + 3 * px * 16
         d2h = 3 * px * 16 + (scene.n * 13 + 23) * 4
         line["e2e"] = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,

@@ -32,7 +32,9 @@ constexpr int kBatch = 256;
 
 template <bool DEPTH_ONLY>
 __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constant__ FwdParams P) {
-  __shared__ float4 s_r0[kBatch], s_r1[kBatch], s_r2[kBatch], s_r3[kBatch], s_bb[kBatch];
+  // one 64-B record per staged entry (AoS: the four float4 of an entry share one address computation) + its bbox
+  __shared__ float4 s_rec[kBatch][4];
+  __shared__ float4 s_bb[kBatch];
 
   const int tile = blockIdx.y * P.cam.TX + blockIdx.x;
   const uint32_t start = P.ranges[2 * tile], end = P.ranges[2 * tile + 1];
@@ -55,16 +57,12 @@ __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constan
     const uint32_t idx = base + threadIdx.x;
     if (idx < end) {
       const float4* r = P.rec + 4 * (size_t)P.vals[idx];
-      const float4 q0 = r[0], q1 = r[1];
-      s_r0[threadIdx.x] = q0;
-      s_r1[threadIdx.x] = q1;
+      const float4 q0 = r[0], q1 = r[1], q2 = r[2];
+      s_rec[threadIdx.x][0] = q0;
+      s_rec[threadIdx.x][1] = q1;
+      s_rec[threadIdx.x][2] = q2;
+      if (!DEPTH_ONLY) s_rec[threadIdx.x][3] = r[3];
       s_bb[threadIdx.x] = splat_bbox(q0, q1);
-      if (!DEPTH_ONLY) {
-        s_r2[threadIdx.x] = r[2];
-        s_r3[threadIdx.x] = r[3];
-      } else {
-        s_r2[threadIdx.x] = r[2];
-      }
     }
     __syncthreads();
     const int n = min(kBatch, (int)(end - base));
@@ -81,25 +79,25 @@ __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constan
       while (mask) {
         const int j = g0 + __ffs(mask) - 1;
         mask &= mask - 1;
-        if (done) continue;
-        const float4 r0 = s_r0[j], r1 = s_r1[j];
+        const float4* e = s_rec[j];
+        const float4 r0 = e[0], r1 = e[1];
         const float dx = px - r0.x, dy = py - r0.y;
         const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
         const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
         const float rho = fminf(rho3, rho2);
-        if (rho > kRhoCut) continue;
-        const float G = __expf(-0.5f * rho);
+        if (done || rho > kRhoCut) continue;
+        const float G = fast_exp2(rho * kNegHalfLog2e);                         // exp(-rho/2)
         const float a = fminf(kAlphaMax, r1.z * G);
         if (a < kAlphaMin) continue;
         const float Tn = T * (1.0f - a);
-        if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
+        if (Tn < kTMin) { done = true; visited = rel0 + j + 1; continue; }
         const float w = a * T;
-        const float4 r2 = s_r2[j];
+        const float4 r2 = e[2];
         const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
         if (DEPTH_ONLY) {
           M1 += w * z;
         } else {
-          const float4 r3 = s_r3[j];
+          const float4 r3 = e[3];
           if (ncontrib == 0) zref = z;
           const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
           if (T > 0.5f) { med = z; mi = rel0 + j; }

@@ -18,7 +18,16 @@ constexpr float kLogitCull = -5.5373342f;  // sigmoid(l) < 1/255
 constexpr float kMinExtent = 2.1213204f;   // 3 sigma, sigma = 1/sqrt(2) px (Eq. 12)
 constexpr float kDegenerateQ = 1e12f;      // Q = kDegenerateQ * I encodes "rho3 = +inf" for degenerate surfels
 
+constexpr float kNegHalfLog2e = -0.72134752044448170368f;   // exp(-rho/2) = 2^(rho * kNegHalfLog2e)
+
 enum : uint8_t { F_CULLED = 1, F_DEGENERATE = 2, F_FLIPPED = 4 };
+
+// 2^x, one MUFU.EX2 (x is in [-6.5, 0] here: no range reduction, no denormals)
+__device__ __forceinline__ float fast_exp2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 
 // ---- device-side camera ------------------------------------------------------------------------------------
 struct DevCamera {

@@ -1,0 +1,65 @@
+"""Multi-GPU path of bench.py on CPU: world_size-2 `gloo` processes (the path shards by view).
+Checks that the ranks of one job render disjoint views that together cover the steps, and that the reported time
+is the max over ranks."""
+import os
+import socket
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    import bench
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        steps, warm, n_views = 6, 3, 20
+        warm_views = bench.views_for_rank(rank, world, n_views, warm)
+        step_views = bench.views_for_rank(rank + warm * world, world, n_views, steps)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, (warm_views, step_views))
+        ms = bench.max_over_ranks(torch, dist, world, 10.0 + 5.0 * rank, "cpu")
+        if rank == 0:
+            out.put((gathered, ms))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(120)
+def test_views_shard_over_two_ranks_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    gathered, ms = q.get(timeout=100)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    (w0, s0), (w1, s1) = gathered
+    assert ms == 15.0                                 # max over ranks, not rank 0's own 10.0
+    assert len(s0) == len(s1) == 6 and len(w0) == len(w1) == 3
+    for a, b in zip(s0, s1):                          # same step: different views on the two ranks
+        assert a != b
+    assert set(s0).isdisjoint(s1) and set(w0).isdisjoint(w1)
+    assert sorted(w0 + w1 + s0 + s1) == list(range(18))   # consecutive views, no gap, no overlap
+
+
+def test_views_for_rank_single_process_cycles():
+    import bench
+    assert bench.views_for_rank(0, 1, 20, 23) == [i % 20 for i in range(23)]
+    assert bench.views_for_rank(3, 8, 20, 3) == [3, 11, 19]
