@@ -122,7 +122,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->offset, N + 1));
   A(dalloc(ctx, &ctx->depth_key, N));
   A(dalloc(ctx, &ctx->flags, N));
-  A(dalloc(ctx, &ctx->vrec, N * 16));
+  A(dalloc(ctx, &ctx->vrec, N * satsplat::kVrec));
   A(dalloc(ctx, &ctx->block_sums, N / 4096 + 2));
   A(dalloc(ctx, &ctx->keys[0], K));
   A(dalloc(ctx, &ctx->keys[1], K));
@@ -142,7 +142,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->px_visited, px));
   A(dalloc(ctx, &ctx->px_contrib, px));
   A(dalloc(ctx, &ctx->red_buf, 64));
-  A(cudaMemset(ctx->vrec, 0, N * 16 * sizeof(float) ? N * 16 * sizeof(float) : 4));
+  A(cudaMemset(ctx->vrec, 0, N ? N * satsplat::kVrec * sizeof(float) : 4));
   A(cudaMemset(ctx->status, 0, sizeof(Status)));
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i) A(cudaEventCreate(&ctx->ev[i]));
 #undef A

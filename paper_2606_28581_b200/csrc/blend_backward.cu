@@ -2,11 +2,13 @@
 //
 // Per pixel: epilogue backward first (gradients of the 3x4 colour correction, the ambient light, the
 // reprojection constants; scatter into the sun-depth gradient), then the tile list is walked in REVERSE order:
-// T_i is recovered as T_{i+1}/(1 - a_i), the suffix sum S_i = sum_{k>i} w_k phi_k is carried, and each
-// contributing (pixel, surfel) pair produces 16 gradient values (c, M = Q^-1, alpha, z_c, r, rgb, n) in the record slots.
-// Those are reduced across the warp with a transposed shuffle butterfly (16 shuffles instead of 80), across
-// the CTA's warps with shared-memory atomics, and only then flushed once per (tile, surfel) with coalesced
-// global atomics into the per-surfel gradient records.  FP32-issue + atomics bound.
+// T_i is recovered as T_{i+1}/(1 - a_i) and the suffix sum S_i = sum_{k>i} w_k phi_k is carried.  The walk only
+// produces, per contributing (pixel, surfel) pair, the three scalars the gradients are linear in (dL/d rho,
+// dL/d z, w) and the pair's local coordinates; the lanes of a warp that hit the same surfel append them,
+// ballot-compacted, to a small per-warp segment buffer in shared memory.  Every four segments the warp turns
+// into four teams of 8 lanes: a team walks one segment with all lanes busy, accumulates the 18 gradient moments
+// of that surfel, reduces them over its 8 lanes (transposed butterfly) and adds them to the surfel's moment
+// record with 16-byte vector REDs.  FP32-issue bound.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -30,45 +32,25 @@ struct BwdParams {
 };
 
 constexpr int kBatchB = 256;
+constexpr int kSegs = 4;    // (warp, surfel) segments per accumulation round: four teams of 8 lanes
 
-// Sum 16 per-lane values over the warp.  On return lane l (l even) holds the total of slot
-// ((l>>4)&1)*8 + ((l>>3)&1)*4 + ((l>>2)&1)*2 + ((l>>1)&1) in v[0].
-__device__ __forceinline__ float warp_reduce16_transposed(float (&v)[16], int lane) {
-  {
-    const bool hi = lane & 16;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      const float send = hi ? v[k] : v[k + 8];
-      const float keep = hi ? v[k + 8] : v[k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-  }
-  {
-    const bool hi = lane & 8;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const float send = hi ? v[k] : v[k + 4];
-      const float keep = hi ? v[k + 4] : v[k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-    }
-  }
-  {
-    const bool hi = lane & 4;
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const float send = hi ? v[k] : v[k + 2];
-      const float keep = hi ? v[k + 2] : v[k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    }
-  }
-  {
-    const bool hi = lane & 2;
-    const float send = hi ? v[0] : v[1];
-    const float keep = hi ? v[1] : v[0];
-    v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-  }
-  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-  return v[0];
+// ---- per-surfel gradient record (internal; consumed and cleared by chain_backward_kernel) -----------------------
+// The blend backward does not form the 16 parameter gradients per (pixel, surfel) pair.  Every per-pair gradient
+// is a per-pair scalar times a polynomial in the surfel-local coordinates (u, v) = Q (x - c), so it accumulates
+// 18 moments per surfel and the chain kernel (once per surfel) turns them into gradients:
+//   s = dL/d rho (0 where alpha' is clamped), t = dL/d z, w = blend weight;   np = Eq. 9 term active, lp = low-pass
+//    0 sum_np s u u    1 sum_np s u v    2 sum_np s v v    3 sum_np s u
+//    4 sum_np s v      5 sum_np t u      6 sum_np t v      7 sum_np t
+//    8 sum_lp s dx     9 sum_lp s dy    10 sum t          11 sum s
+//   12..14 sum w v_albedo              15..17 sum w v_normal            18, 19 unused
+// All products are formed from the same fp32 (u, v) the per-pair form would use, so this is the per-pair sum with
+// the common factors (Q, g, alpha) pulled out: same conditioning for nearly edge-on surfels.
+
+__device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
+  asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(a), "f"(b) : "memory");
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -77,12 +59,54 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
+// Sum 16 per-lane values over a team of 8 consecutive lanes.  On return every lane holds, in v[0..3], the team
+// totals of slots base..base+3 with base = ((lane>>2)&1)*8 + ((lane>>1)&1)*4 (lanes 2k and 2k+1 hold the same four).
+__device__ __forceinline__ void team8_reduce16(float (&v)[16], int lane) {
+  {
+    const bool hi = lane & 4;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float send = hi ? v[k] : v[k + 8];
+      const float keep = hi ? v[k + 8] : v[k];
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+  }
+  {
+    const bool hi = lane & 2;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float send = hi ? v[k] : v[k + 4];
+      const float keep = hi ? v[k + 4] : v[k];
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], 1);
+}
+
+// Sum 32 per-lane values over the warp: on return lane l holds the total of slot l.
+__device__ __forceinline__ float warp_reduce32_transposed(float (&v)[32], int lane) {
+#pragma unroll
+  for (int h = 16; h >= 1; h >>= 1) {
+    const bool hi = lane & h;
+#pragma unroll
+    for (int k = 0; k < h; ++k) {
+      const float send = hi ? v[k] : v[k + h];
+      const float keep = hi ? v[k + h] : v[k];
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, h);
+    }
+  }
+  return v[0];
+}
+
 template <bool DEPTH_ONLY>
 __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_constant__ BwdParams P) {
-  __shared__ float4 s_r0[kBatchB], s_r1[kBatchB], s_r2[kBatchB], s_r3[kBatchB];
+  constexpr int kRecV = DEPTH_ONLY ? 3 : 4;
+  __shared__ float4 s_rec[kBatchB][kRecV];
   __shared__ float4 s_bb[kBatchB];
   __shared__ uint32_t s_id[kBatchB];
-  __shared__ float s_grad[kBatchB * 16];
+  __shared__ float4 s_p4[8][kSegs * 32];   // per warp: pending pairs (s, t, w, source lane | low-pass flag)
+  __shared__ float2 s_p2[8][kSegs * 32];   //           and their local coordinates: (u, v), or (dx, dy) for low-pass pairs
   __shared__ float s_red[8][24];
   __shared__ int s_max[8];
 
@@ -101,9 +125,6 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
   float T = 1.f, Tf = 1.f, zref = 0.f, M1 = 0.f, M2 = 0.f, A = 0.f;
   float va0 = 0.f, va1 = 0.f, va2 = 0.f, vN0 = 0.f, vN1 = 0.f, vN2 = 0.f, vD = 0.f, vL = 0.f, vmed = 0.f, vT = 0.f;
   int last = 0, mi = -1;
-  float red[23];
-#pragma unroll
-  for (int k = 0; k < 23; ++k) red[k] = 0.f;
   if (inside) {
     const float4 a = P.px_a[o];
     const int2 li = P.px_i[o];
@@ -112,7 +133,14 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
       // sun_depth = sum w (z - z_bg) + z_bg  (since sum w + T_f = 1): phi = v (z - z_bg), no T_f term
       vD = P.v_sun_in[o];
       zref = P.cam.z_bg;
-    } else {
+    }
+  }
+  if (!DEPTH_ONLY) {
+    float red[32];
+#pragma unroll
+    for (int k = 0; k < 32; ++k) red[k] = 0.f;
+    if (inside) {
+      const float4 a = P.px_a[o];
       zref = a.y; M1 = a.z; M2 = a.w;
       const float4 b = P.px_b[o];
       float vI0 = 0.f, vI1 = 0.f, vI2 = 0.f, vA = 0.f;
@@ -167,20 +195,17 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
       vT += -vA + va0 * P.cam.bg[0] + va1 * P.cam.bg[1] + va2 * P.cam.bg[2];   // A = 1 - T_f ; albedo = C + T_f bg
       vT -= vD * zref;                                                          // D = M1' + z_ref (1 - T_f)
     }
-  }
-  // ---- reduce the 23 epilogue gradients over the CTA, one atomic each ----
-  if (!DEPTH_ONLY && P.red) {
+    // ---- reduce the 23 epilogue gradients over the CTA (transposed butterfly, then shared memory), one atomic each ----
+    if (P.red) {
+      const float r = warp_reduce32_transposed(red, lane);
+      if (lane < 24) s_red[warp][lane] = r;
+      __syncthreads();
+      if (threadIdx.x < 23) {
+        float r = 0.f;
 #pragma unroll
-    for (int k = 0; k < 23; ++k) {
-      const float r = warp_sum(red[k]);
-      if (lane == 0) s_red[warp][k] = r;
-    }
-    __syncthreads();
-    if (threadIdx.x < 23) {
-      float r = 0.f;
-#pragma unroll
-      for (int w = 0; w < 8; ++w) r += s_red[w][threadIdx.x];
-      if (r != 0.f) atomicAdd(P.red + threadIdx.x, r);
+        for (int w = 0; w < 8; ++w) r += s_red[w][threadIdx.x];
+        if (r != 0.f) atomicAdd(P.red + threadIdx.x, r);
+      }
     }
   }
   // ---- CTA-wide maximum of `last` ----
@@ -188,7 +213,6 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
     const int m = __reduce_max_sync(0xffffffffu, last);
     if (lane == 0) s_max[warp] = m;
   }
-  for (int k = threadIdx.x; k < kBatchB * 16; k += 256) s_grad[k] = 0.f;
   __syncthreads();
   int max_last = 0;
 #pragma unroll
@@ -196,7 +220,63 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
 
   const float TfvT = Tf * vT;
   float Ssum = 0.f;
-  const int slot = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const int team = lane >> 3, tl = lane & 7;
+  float4* const p4 = s_p4[warp];
+  float2* const p2 = s_p2[warp];
+  // pending (warp, surfel) segments: team q keeps surfel id and pair count of segment q in its lanes' registers
+  int nseg = 0, wmax = 0, my_cnt = 0;
+  uint32_t my_id = 0;
+
+  // Accumulate the pending segments: team q walks the pairs of segment q (8 at a time), sums the 18 moments,
+  // reduces them over its 8 lanes and adds them to the surfel's gradient record with vector REDs.
+  auto flush = [&]() {
+    __syncwarp();
+    float acc[16], e0 = 0.f, e1 = 0.f;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) acc[k] = 0.f;
+    for (int i0 = 0; i0 < wmax; i0 += 8) {   // warp-uniform trip count: the loop body shuffles
+      const int i = i0 + tl;
+      float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+      float2 ab = make_float2(0.f, 0.f);
+      if (i < my_cnt) { q = p4[team * 32 + i]; ab = p2[team * 32 + i]; }
+      const int info = __float_as_int(q.w);
+      const bool lp = info & 32;
+      const float s_np = lp ? 0.f : q.x, s_lp = lp ? q.x : 0.f, t_np = lp ? 0.f : q.y;
+      const float su = s_np * ab.x, sv = s_np * ab.y;
+      acc[0] += su * ab.x; acc[1] += su * ab.y; acc[2] += sv * ab.y; acc[3] += su;
+      acc[4] += sv; acc[5] += t_np * ab.x; acc[6] += t_np * ab.y; acc[7] += t_np;
+      acc[8] += s_lp * ab.x; acc[9] += s_lp * ab.y; acc[10] += q.y; acc[11] += q.x;
+      if (!DEPTH_ONLY) {
+        const int src = info & 31;
+        acc[12] += q.z * __shfl_sync(0xffffffffu, va0, src);
+        acc[13] += q.z * __shfl_sync(0xffffffffu, va1, src);
+        acc[14] += q.z * __shfl_sync(0xffffffffu, va2, src);
+        acc[15] += q.z * __shfl_sync(0xffffffffu, vN0, src);
+        e0 += q.z * __shfl_sync(0xffffffffu, vN1, src);
+        e1 += q.z * __shfl_sync(0xffffffffu, vN2, src);
+      }
+    }
+    team8_reduce16(acc, lane);
+    if (!DEPTH_ONLY) {
+#pragma unroll
+      for (int d = 4; d > 0; d >>= 1) {
+        e0 += __shfl_xor_sync(0xffffffffu, e0, d);
+        e1 += __shfl_xor_sync(0xffffffffu, e1, d);
+      }
+    }
+    if (my_cnt > 0) {
+      float* dst = P.vrec + (size_t)my_id * kVrec;
+      const int base = ((tl >> 2) & 1) * 8 + ((tl >> 1) & 1) * 4;
+      if (!(tl & 1)) {
+        if (!DEPTH_ONLY || base < 12) red_add_v4(dst + base, acc[0], acc[1], acc[2], acc[3]);
+      } else if (!DEPTH_ONLY && tl == 1) {
+        red_add_v2(dst + 16, e0, e1);
+      }
+    }
+    nseg = 0; wmax = 0; my_cnt = 0;
+    __syncwarp();
+  };
 
   const int nb = (max_last + kBatchB - 1) / kBatchB;
   for (int b = nb - 1; b >= 0; --b) {
@@ -207,11 +287,11 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
       const float4* r = P.rec + 4 * (size_t)id;
       s_id[threadIdx.x] = id;
       const float4 q0 = r[0], q1 = r[1];
-      s_r0[threadIdx.x] = q0;
-      s_r1[threadIdx.x] = q1;
+      s_rec[threadIdx.x][0] = q0;
+      s_rec[threadIdx.x][1] = q1;
+      s_rec[threadIdx.x][2] = r[2];
+      if (!DEPTH_ONLY) s_rec[threadIdx.x][3] = r[3];
       s_bb[threadIdx.x] = splat_bbox(q0, q1);
-      s_r2[threadIdx.x] = r[2];
-      if (!DEPTH_ONLY) s_r3[threadIdx.x] = r[3];
     }
     __syncthreads();
     const int wlast = __reduce_max_sync(0xffffffffu, last);   // nothing beyond this index matters to this warp
@@ -223,84 +303,55 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
       }
       unsigned mask = __ballot_sync(0xffffffffu, hit);
       while (mask) {
-      const int bit = 31 - __clz(mask);
-      mask &= ~(1u << bit);
-      const int j = g0 + bit;
-      const float4 r0 = s_r0[j], r1 = s_r1[j];
-      const float dx = px - r0.x, dy = py - r0.y;
-      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
-      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);
-      const float rho = fminf(rho3, rho2);
-      const float G = __expf(-0.5f * rho);
-      const float aG = r1.z * G;
-      const float a = fminf(kAlphaMax, aG);
-      const bool active = (rel0 + j < last) && (rho <= kRhoCut) && (a >= kAlphaMin);
-      if (!__any_sync(0xffffffffu, active)) continue;
-      float g[16];
-#pragma unroll
-      for (int k = 0; k < 16; ++k) g[k] = 0.f;
-      if (active) {
-        const float4 r2 = s_r2[j];
-        const bool lowpass = !(rho3 <= rho2);
-        const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
-        const float zs = z - zref;
-        const float om = 1.0f - a;
-        const float Ti = T / om;
-        const float w = a * Ti;
-        float phi, v_z;
-        if (DEPTH_ONLY) {
-          phi = vD * zs;
-          v_z = w * vD;
-        } else {
-          const float4 r3 = s_r3[j];
-          const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
-          phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
-          v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((rel0 + j == mi) ? vmed : 0.f);
-          g[10] = w * va0; g[11] = w * va1; g[12] = w * va2;
-          g[13] = w * vN0; g[14] = w * vN1; g[15] = w * vN2;
+        const int bit = 31 - __clz(mask);
+        mask &= ~(1u << bit);
+        const int j = g0 + bit;
+        const float4* e = s_rec[j];
+        const float4 r0 = e[0], r1 = e[1];
+        const float dx = px - r0.x, dy = py - r0.y;
+        const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
+        const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);
+        const float rho = fminf(rho3, rho2);
+        const float aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
+        const float a = fminf(kAlphaMax, aG);
+        const bool active = (rel0 + j < last) && (rho <= kRhoCut) && (a >= kAlphaMin);
+        const unsigned hm = __ballot_sync(0xffffffffu, active);
+        if (hm == 0) continue;
+        if (active) {
+          const float4 r2 = e[2];
+          const bool lowpass = !(rho3 <= rho2);
+          const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
+          const float zs = z - zref;
+          const float rc = __fdividef(1.0f, 1.0f - a);
+          const float Ti = T * rc;
+          const float w = a * Ti;
+          float phi, v_z;
+          if (DEPTH_ONLY) {
+            phi = vD * zs;
+            v_z = w * vD;
+          } else {
+            const float4 r3 = e[3];
+            const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
+            phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
+            v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((rel0 + j == mi) ? vmed : 0.f);
+          }
+          const float v_a = Ti * phi - (Ssum + TfvT) * rc;
+          Ssum += w * phi;
+          T = Ti;
+          const float v_rho = (aG < kAlphaMax) ? -0.5f * aG * v_a : 0.f;   // alpha' = alpha G unless clamped
+          const int pos = nseg * 32 + __popc(hm & lt_mask);
+          p4[pos] = make_float4(v_rho, v_z, w, __int_as_float(lane | (lowpass ? 32 : 0)));
+          p2[pos] = lowpass ? make_float2(dx, dy) : make_float2(u, v);
         }
-        const float v_a = Ti * phi - (Ssum + TfvT) / om;
-        Ssum += w * phi;
-        T = Ti;
-        float v_rho = 0.f;
-        if (aG < kAlphaMax) {
-          g[6] = G * v_a;
-          v_rho = -0.5f * G * r1.z * v_a;
-        }
-        g[7] = v_z;
-        float vd0, vd1;
-        if (!lowpass) {
-          // z = z_c + g.d = z_c - r.(u,v): accumulate the gradients of M = Q^-1 and r directly,
-          //   v_d = Q^T (v_uv - v_z r) = v_z g + Q^T v_uv,   v_M = -v_d (u,v)^T,   v_r = -v_z (u,v)
-          // (no multiplication by Q^2 afterwards: well conditioned for nearly edge-on surfels)
-          const float vu = 2.0f * u * v_rho, vv = 2.0f * v * v_rho;
-          vd0 = v_z * r2.x + r0.z * vu + r1.x * vv;
-          vd1 = v_z * r2.y + r0.w * vu + r1.y * vv;
-          g[2] = -vd0 * u; g[3] = -vd0 * v; g[4] = -vd1 * u; g[5] = -vd1 * v;
-          g[8] = -v_z * u; g[9] = -v_z * v;
-        } else {
-          vd0 = 4.0f * dx * v_rho;
-          vd1 = 4.0f * dy * v_rho;
-        }
-        g[0] = -vd0;
-        g[1] = -vd1;
-      }
-      const float tot = warp_reduce16_transposed(g, lane);
-      if (!(lane & 1) && tot != 0.f) atomicAdd(&s_grad[j * 16 + slot], tot);
-      }
-    }
-    __syncthreads();
-    // flush this batch: one coalesced atomic per non-zero gradient component of each (tile, surfel) pair
-#pragma unroll 4
-    for (int k = threadIdx.x; k < n * 16; k += 256) {
-      const float gval = s_grad[k];
-      if (gval != 0.f) {
-        atomicAdd(P.vrec + 16 * (size_t)s_id[k >> 4] + (k & 15), gval);
-        s_grad[k] = 0.f;
+        const int cnt = __popc(hm);
+        if (team == nseg) { my_cnt = cnt; my_id = s_id[j]; }
+        wmax = max(wmax, cnt);
+        if (++nseg == kSegs) flush();
       }
     }
     __syncthreads();
   }
+  if (nseg) flush();
 }
 
 cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* v_rgba, const float* v_geom,

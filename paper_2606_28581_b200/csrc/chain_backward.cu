@@ -1,8 +1,9 @@
-// chain_backward.cu — per-surfel chain rule from gradient records (c, M, alpha, z_c, r, rgb, n) to the surfel
-// parameters (means, quats, scales, opacity logits, rgb) and to the 2x4 camera delta dF (PAPER.md:155-163,
-// Eq. 15), through Eq. 8-11.  One thread per surfel; the 8 dF partials are reduced over the CTA (shuffles +
-// shared memory) before one atomic each.  The gradient records are cleared as they are consumed, so the
-// context never needs a separate memset pass.  HBM-bound: 64 B record + 40 B inputs read, 52 B read-modify-write.
+// chain_backward.cu — per-surfel chain rule from the gradient moment records of the blend backward (layout in
+// blend_backward.cu) to the record gradients (c, M = Q^-1, alpha, z_c, r, rgb, n) and on to the surfel parameters
+// (means, quats, scales, opacity logits, rgb) and the 2x4 camera delta dF (Eq. 15), through
+// Eq. 8-11.  One thread per surfel; the 8 dF partials are reduced over the CTA (shuffles + shared memory) before
+// one atomic each.  The moment records are cleared as they are consumed, so the context never needs a separate
+// memset pass.  HBM-bound: 80 B moments read + cleared, 48 B record + 40 B inputs read, 52 B read-modify-write.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -16,7 +17,8 @@ __device__ __forceinline__ float warp_sum_f(float v) {
 __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int N, const float* __restrict__ means,
                                                              const float* __restrict__ quats, const float* __restrict__ scales,
                                                              const float* __restrict__ logits, const uint32_t* __restrict__ count,
-                                                             const uint8_t* __restrict__ flags, float4* __restrict__ vrec,
+                                                             const uint8_t* __restrict__ flags, const float4* __restrict__ rec,
+                                                             float4* __restrict__ vrec,
                                                              float* __restrict__ v_means, float* __restrict__ v_quats,
                                                              float* __restrict__ v_scales, float* __restrict__ v_logits,
                                                              float* __restrict__ v_rgb, float* __restrict__ v_dF) {
@@ -26,11 +28,34 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
 #pragma unroll
   for (int k = 0; k < 8; ++k) dF[k] = 0.f;
   if (i < N && count[i] > 0) {
-    float4* gp = vrec + 4 * (size_t)i;
-    const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2], g3 = gp[3];
+    float4* gp = vrec + (kVrec / 4) * (size_t)i;
+    const float4 m0 = gp[0], m1 = gp[1], m2 = gp[2], m3 = gp[3], m4 = gp[4];
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    gp[0] = zero; gp[1] = zero; gp[2] = zero; gp[3] = zero;
+    gp[0] = zero; gp[1] = zero; gp[2] = zero; gp[3] = zero; gp[4] = zero;
     const uint8_t fl = flags[i];
+    // moments -> record gradients, slots g0 = (c_x, c_y, M00, M01)  g1 = (M10, M11, alpha, z_c)  g2 = (r_0, r_1, red, green)
+    // g3 = (blue, n_x, n_y, n_z).  Per pair: v_uv = 2 s (u,v); v_d = t g + Q^T v_uv (4 s d for low-pass pairs);
+    // v_c = -v_d; v_M = -v_d (u,v)^T; v_r = -t (u,v); v_alpha = G v_a = -2 s / alpha; v_zc = t.
+    float4 g0, g1, g2, g3;
+    {
+      const float4 r0 = rec[4 * (size_t)i], r1 = rec[4 * (size_t)i + 1], r2 = rec[4 * (size_t)i + 2];
+      const float Q00 = r0.z, Q01 = r0.w, Q10 = r1.x, Q11 = r1.y, ga = r2.x, gb = r2.y;
+      const float suu = m0.x, suv = m0.y, svv = m0.z, Su = m0.w, Sv = m1.x, Tu = m1.y, Tv = m1.z, T0np = m1.w;
+      g0.x = -(4.0f * m2.x); g0.y = -(4.0f * m2.y);
+      g0.z = 0.f; g0.w = 0.f; g1.x = 0.f; g1.y = 0.f; g2.x = 0.f; g2.y = 0.f;
+      if (!(fl & F_DEGENERATE)) {
+        g0.x -= T0np * ga + 2.0f * (Q00 * Su + Q10 * Sv);
+        g0.y -= T0np * gb + 2.0f * (Q01 * Su + Q11 * Sv);
+        g0.z = -(ga * Tu + 2.0f * (Q00 * suu + Q10 * suv));
+        g0.w = -(ga * Tv + 2.0f * (Q00 * suv + Q10 * svv));
+        g1.x = -(gb * Tu + 2.0f * (Q01 * suu + Q11 * suv));
+        g1.y = -(gb * Tv + 2.0f * (Q01 * suv + Q11 * svv));
+        g2.x = -Tu; g2.y = -Tv;
+      }
+      g1.z = -2.0f * m2.w / r1.z;
+      g1.w = m2.z;
+      g2.z = m3.x; g2.w = m3.y; g3.x = m3.z; g3.y = m3.w; g3.z = m4.x; g3.w = m4.y;
+    }
     const float p0 = means[3 * i], p1 = means[3 * i + 1], p2 = means[3 * i + 2];
     const float4 q = reinterpret_cast<const float4*>(quats)[i];
     const float2 sc = reinterpret_cast<const float2*>(scales)[i];
@@ -110,7 +135,7 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
   if (c->N == 0) return cudaSuccess;
   ++g_kernel_launches;
   chain_backward_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>(c->cam, (int)c->N, means, quats, scales, logits, c->count,
-                                                                  c->flags, reinterpret_cast<float4*>(c->vrec), v_means,
+                                                                  c->flags, c->rec, reinterpret_cast<float4*>(c->vrec), v_means,
                                                                   v_quats, v_scales, v_logits, v_rgb, v_dF);
   return cudaGetLastError();
 }

@@ -51,7 +51,8 @@ struct DevShading {
 // ---- record layout in HBM: 4 x float4 = 64 B per surfel, 64-B aligned --------------------------------------
 //   r0 = (c_x, c_y, Q00, Q01)   r1 = (Q10, Q11, alpha, z_c)   r2 = (g0, g1, red, green)   r3 = (blue, n_x, n_y, n_z)
 // The first two float4 are all the per-pair test needs; the last two are only read by contributing pairs.
-// Gradient records use the same slots.
+// Gradient records (vrec) are kVrec floats of per-surfel moments: layout in blend_backward.cu.
+constexpr int kVrec = 20;
 
 // sort configuration
 constexpr int kSortThreads = 256;
@@ -118,7 +119,7 @@ struct satsplat_ctx {
   uint32_t* offset;       // [N+1] exclusive scan
   uint32_t* depth_key;    // [N]
   uint8_t* flags;         // [N]
-  float* vrec;            // [N*16] gradient records, kept zero between calls (the chain kernel clears them)
+  float* vrec;            // [N*kVrec] gradient moment records, kept zero between calls (the chain kernel clears them)
   uint32_t* block_sums;   // scan scratch
   // binning
   uint64_t* keys[2];
