@@ -5,9 +5,9 @@
 // T_i is recovered as T_{i+1}/(1 - a_i) and the suffix sum S_i = sum_{k>i} w_k phi_k is carried.  The walk only
 // produces, per contributing (pixel, surfel) pair, the three scalars the gradients are linear in (dL/d rho,
 // dL/d z, w) and the pair's local coordinates; the lanes of a warp that hit the same surfel append them,
-// ballot-compacted, to a small per-warp segment buffer in shared memory.  Every four segments the warp turns
-// into four teams of 8 lanes: a team walks one segment with all lanes busy, accumulates the 18 gradient moments
-// of that surfel, reduces them over its 8 lanes (transposed butterfly) and adds them to the surfel's moment
+// ballot-compacted, to a small per-warp segment buffer in shared memory.  Every eight segments the warp turns
+// into eight teams of 4 lanes: a team walks one segment with all lanes busy, accumulates the 18 gradient moments
+// of that surfel, reduces them over its 4 lanes (transposed butterfly) and adds them to the surfel's moment
 // record with 16-byte vector REDs.  FP32-issue bound.
 #include "internal.cuh"
 
@@ -31,8 +31,20 @@ struct BwdParams {
   float* red;              // [23] = cc(12) ambient(3) reproj(8), accumulated with atomics (may be NULL)
 };
 
-constexpr int kBatchB = 256;
-constexpr int kSegs = 4;    // (warp, surfel) segments per accumulation round: four teams of 8 lanes
+#ifndef SATSPLAT_BWD_WARPS
+#define SATSPLAT_BWD_WARPS 8
+#endif
+#ifndef SATSPLAT_BWD_MINB
+#define SATSPLAT_BWD_MINB 3
+#endif
+constexpr int kWarpsB = SATSPLAT_BWD_WARPS;   // warps per CTA: 8 = one 16x16 tile, 4 = its upper or lower half
+constexpr int kThreadsB = 32 * kWarpsB;
+constexpr int kBatchB = kThreadsB;
+#ifndef SATSPLAT_BWD_TEAM
+#define SATSPLAT_BWD_TEAM 4
+#endif
+constexpr int kTeam = SATSPLAT_BWD_TEAM;   // lanes per team (4 or 8)
+constexpr int kSegs = 32 / kTeam;         // (warp, surfel) segments per accumulation round: one per team
 
 // ---- per-surfel gradient record (internal; consumed and cleared by chain_backward_kernel) -----------------------
 // The blend backward does not form the 16 parameter gradients per (pixel, surfel) pair.  Every per-pair gradient
@@ -59,29 +71,32 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-// Sum 16 per-lane values over a team of 8 consecutive lanes.  On return every lane holds, in v[0..3], the team
-// totals of slots base..base+3 with base = ((lane>>2)&1)*8 + ((lane>>1)&1)*4 (lanes 2k and 2k+1 hold the same four).
-__device__ __forceinline__ void team8_reduce16(float (&v)[16], int lane) {
+// Sum 16 per-lane values over a team of kTeam consecutive lanes.  On return every lane holds, in v[0..3], the team
+// totals of slots base..base+3: kTeam = 8: base = ((lane>>2)&1)*8 + ((lane>>1)&1)*4 (lanes 2k, 2k+1 hold the same
+// four); kTeam = 4: base = ((lane>>1)&1)*8 + (lane&1)*4 (every lane holds a different four).
+__device__ __forceinline__ void team_reduce16(float (&v)[16], int lane) {
   {
-    const bool hi = lane & 4;
+    const bool hi = lane & (kTeam / 2);
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
       const float send = hi ? v[k] : v[k + 8];
       const float keep = hi ? v[k + 8] : v[k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, kTeam / 2);
     }
   }
   {
-    const bool hi = lane & 2;
+    const bool hi = lane & (kTeam / 4);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const float send = hi ? v[k] : v[k + 4];
       const float keep = hi ? v[k + 4] : v[k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, kTeam / 4);
     }
   }
+  if (kTeam == 8) {
 #pragma unroll
-  for (int k = 0; k < 4; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], 1);
+    for (int k = 0; k < 4; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], 1);
+  }
 }
 
 // Sum 32 per-lane values over the warp: on return lane l holds the total of slot l.
@@ -100,26 +115,29 @@ __device__ __forceinline__ float warp_reduce32_transposed(float (&v)[32], int la
 }
 
 template <bool DEPTH_ONLY>
-__global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_constant__ BwdParams P) {
+__global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_kernel(const __grid_constant__ BwdParams P) {
   constexpr int kRecV = DEPTH_ONLY ? 3 : 4;
   __shared__ float4 s_rec[kBatchB][kRecV];
   __shared__ float4 s_bb[kBatchB];
   __shared__ uint32_t s_id[kBatchB];
-  __shared__ float4 s_p4[8][kSegs * 32];   // per warp: pending pairs (s, t, w, source lane | low-pass flag)
-  __shared__ float2 s_p2[8][kSegs * 32];   //           and their local coordinates: (u, v), or (dx, dy) for low-pass pairs
-  __shared__ float s_red[8][24];
-  __shared__ int s_max[8];
+  // per warp: pending pairs (s, t, w, source lane | low-pass flag) and their local coordinates: (u, v), or (dx, dy)
+  // for low-pass pairs; kSegs segments of up to 32 pairs each (dynamic shared memory: kPairBytes per CTA)
+  extern __shared__ float4 s_dyn[];
+  __shared__ float s_red[kWarpsB][24];
+  __shared__ int s_max[kWarpsB];
 
-  const int tile = blockIdx.y * P.cam.TX + blockIdx.x;
-  const uint32_t start = P.ranges[2 * tile];
+  // CTA blockIdx.y holds warps [blockIdx.y * kWarpsB, +kWarpsB) of tile column blockIdx.x; a tile has 8 warps (8x4 px each)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int ix = blockIdx.x * kTile + (warp & 1) * 8 + (lane & 7);
-  const int iy = blockIdx.y * kTile + (warp >> 1) * 4 + (lane >> 3);
+  const int gw = blockIdx.y * kWarpsB + warp, ty = gw >> 3, wi = gw & 7;
+  const int tile = ty * P.cam.TX + blockIdx.x;
+  const uint32_t start = P.ranges[2 * tile];
+  const int bx0 = blockIdx.x * kTile + (wi & 1) * 8, by0 = ty * kTile + (wi >> 1) * 4;
+  const int ix = bx0 + (lane & 7), iy = by0 + (lane >> 3);
   const bool inside = ix < P.cam.W && iy < P.cam.H;
   const float px = (float)ix + 0.5f, py = (float)iy + 0.5f;
   const size_t o = (size_t)iy * P.cam.W + ix;
-  const float wx0 = (float)(blockIdx.x * kTile + (warp & 1) * 8) + 0.5f, wx1 = wx0 + 7.0f;
-  const float wy0 = (float)(blockIdx.y * kTile + (warp >> 1) * 4) + 0.5f, wy1 = wy0 + 3.0f;
+  const float wx0 = (float)bx0 + 0.5f, wx1 = wx0 + 7.0f;
+  const float wy0 = (float)by0 + 0.5f, wy1 = wy0 + 3.0f;
 
   // ---- per-pixel state and epilogue backward ----
   float T = 1.f, Tf = 1.f, zref = 0.f, M1 = 0.f, M2 = 0.f, A = 0.f;
@@ -203,7 +221,7 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
       if (threadIdx.x < 23) {
         float r = 0.f;
 #pragma unroll
-        for (int w = 0; w < 8; ++w) r += s_red[w][threadIdx.x];
+        for (int w = 0; w < kWarpsB; ++w) r += s_red[w][threadIdx.x];
         if (r != 0.f) atomicAdd(P.red + threadIdx.x, r);
       }
     }
@@ -216,14 +234,14 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
   __syncthreads();
   int max_last = 0;
 #pragma unroll
-  for (int w = 0; w < 8; ++w) max_last = max(max_last, s_max[w]);
+  for (int w = 0; w < kWarpsB; ++w) max_last = max(max_last, s_max[w]);
 
   const float TfvT = Tf * vT;
   float Ssum = 0.f;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const int team = lane >> 3, tl = lane & 7;
-  float4* const p4 = s_p4[warp];
-  float2* const p2 = s_p2[warp];
+  const int team = lane / kTeam, tl = lane % kTeam;
+  float4* const p4 = s_dyn + warp * (kSegs * 32);
+  float2* const p2 = reinterpret_cast<float2*>(s_dyn + kWarpsB * (kSegs * 32)) + warp * (kSegs * 32);
   // pending (warp, surfel) segments: team q keeps surfel id and pair count of segment q in its lanes' registers
   int nseg = 0, wmax = 0, my_cnt = 0;
   uint32_t my_id = 0;
@@ -235,7 +253,7 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
     float acc[16], e0 = 0.f, e1 = 0.f;
 #pragma unroll
     for (int k = 0; k < 16; ++k) acc[k] = 0.f;
-    for (int i0 = 0; i0 < wmax; i0 += 8) {   // warp-uniform trip count: the loop body shuffles
+    for (int i0 = 0; i0 < wmax; i0 += kTeam) {   // warp-uniform trip count: the loop body shuffles
       const int i = i0 + tl;
       float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
       float2 ab = make_float2(0.f, 0.f);
@@ -257,21 +275,27 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
         e1 += q.z * __shfl_sync(0xffffffffu, vN2, src);
       }
     }
-    team8_reduce16(acc, lane);
+    team_reduce16(acc, lane);
     if (!DEPTH_ONLY) {
 #pragma unroll
-      for (int d = 4; d > 0; d >>= 1) {
+      for (int d = kTeam / 2; d > 0; d >>= 1) {
         e0 += __shfl_xor_sync(0xffffffffu, e0, d);
         e1 += __shfl_xor_sync(0xffffffffu, e1, d);
       }
     }
     if (my_cnt > 0) {
       float* dst = P.vrec + (size_t)my_id * kVrec;
-      const int base = ((tl >> 2) & 1) * 8 + ((tl >> 1) & 1) * 4;
-      if (!(tl & 1)) {
+      if (kTeam == 8) {
+        const int base = ((tl >> 2) & 1) * 8 + ((tl >> 1) & 1) * 4;
+        if (!(tl & 1)) {
+          if (!DEPTH_ONLY || base < 12) red_add_v4(dst + base, acc[0], acc[1], acc[2], acc[3]);
+        } else if (!DEPTH_ONLY && tl == 1) {
+          red_add_v2(dst + 16, e0, e1);
+        }
+      } else {
+        const int base = ((tl >> 1) & 1) * 8 + (tl & 1) * 4;
         if (!DEPTH_ONLY || base < 12) red_add_v4(dst + base, acc[0], acc[1], acc[2], acc[3]);
-      } else if (!DEPTH_ONLY && tl == 1) {
-        red_add_v2(dst + 16, e0, e1);
+        if (!DEPTH_ONLY && tl == 3) red_add_v2(dst + 16, e0, e1);
       }
     }
     nseg = 0; wmax = 0; my_cnt = 0;
@@ -322,7 +346,7 @@ __global__ void __launch_bounds__(256, 3) blend_backward_kernel(const __grid_con
           const bool lowpass = !(rho3 <= rho2);
           const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
           const float zs = z - zref;
-          const float rc = __fdividef(1.0f, 1.0f - a);
+          const float rc = fast_rcp(1.0f - a);
           const float Ti = T * rc;
           const float w = a * Ti;
           float phi, v_z;
@@ -375,12 +399,19 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   const bool want_red = !depth_only && (v_cc || v_ambient || v_reproj);
   P.red = want_red ? c->red_buf : nullptr;
   if (want_red) cudaMemsetAsync(c->red_buf, 0, 32 * sizeof(float), s);
-  const dim3 grid(c->cam.TX, c->cam.TY);
+  const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));
+  constexpr int kPairBytes = kWarpsB * kSegs * 32 * (int)(sizeof(float4) + sizeof(float2));
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(blend_backward_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
+    cudaFuncSetAttribute(blend_backward_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
+    attr_set = true;
+  }
   ++g_kernel_launches;
   if (depth_only)
-    blend_backward_kernel<true><<<grid, 256, 0, s>>>(P);
+    blend_backward_kernel<true><<<grid, kThreadsB, kPairBytes, s>>>(P);
   else
-    blend_backward_kernel<false><<<grid, 256, 0, s>>>(P);
+    blend_backward_kernel<false><<<grid, kThreadsB, kPairBytes, s>>>(P);
   return cudaGetLastError();
 }
 

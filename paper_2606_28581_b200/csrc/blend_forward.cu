@@ -4,9 +4,11 @@
 // (colour correction + soft shadow test against the sun-view depth map) fused after the loop.
 //
 // One CTA per tile, one thread per pixel; a warp covers an 8x4 pixel block.  Splat records are staged through
-// shared memory in batches of 256 together with a conservative bounding box; each warp first culls the batch
-// against its own 8x4 block (one splat per lane, ballot) and walks only the survivors, in order (two float4 for the per-pair test, two more read only by contributing pairs).
-// FP32-issue bound: ~17 instructions per evaluated pair, ~25 more per contributing pair.
+// shared memory in batches of 256 together with a conservative bounding box.  Per group of 32 entries, lane l turns
+// entry l's box into the bit mask of the block's pixels it covers; a 32x32 bit transpose across the warp (5 shuffles)
+// hands every pixel the mask of entries whose box covers it, and each pixel then walks only its own candidates, in
+// list order (the walk diverges across lanes; the per-pair test and the blend are exactly those of Eq. 9/12/14).
+// FP32-issue bound.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -30,10 +32,33 @@ struct FwdParams {
 
 constexpr int kBatch = 256;
 
+// 32x32 bit-matrix transpose across the warp: lane l passes row l, and receives column l (bit b = bit l of lane b's row).
+__device__ __forceinline__ uint32_t warp_transpose_bits(uint32_t x, int lane) {
+  uint32_t m = 0x0000FFFFu;
+#pragma unroll
+  for (int j = 16; j >= 1; j >>= 1) {
+    const uint32_t y = __shfl_xor_sync(0xffffffffu, x, j);
+    x = (lane & j) ? ((x & ~m) | ((y >> j) & m)) : ((x & m) | ((y << j) & ~m));
+    m ^= m << (j >> 1);
+  }
+  return x;
+}
+
+// Bit p (p = 8 * row + column) set iff pixel p of the 8x4 block whose first pixel centre is (wx0, wy0) lies inside the
+// bounding box bb = (x_min, x_max, y_min, y_max).
+__device__ __forceinline__ uint32_t block_cover_mask(const float4 bb, float wx0, float wy0) {
+  const int c0 = (int)fmaxf(ceilf(bb.x - wx0), 0.0f), c1 = (int)fminf(floorf(bb.y - wx0), 7.0f);
+  const int r0 = (int)fmaxf(ceilf(bb.z - wy0), 0.0f), r1 = (int)fminf(floorf(bb.w - wy0), 3.0f);
+  if (c0 > c1 || r0 > r1) return 0u;
+  const uint32_t cols = (2u << c1) - (1u << c0);
+  const uint32_t rows = (2u << r1) - (1u << r0);
+  return cols * ((rows * 0x00204081u) & 0x01010101u);
+}
+
 template <bool DEPTH_ONLY>
-__global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constant__ FwdParams P) {
-  // one 64-B record per staged entry (AoS: the four float4 of an entry share one address computation) + its bbox
-  __shared__ float4 s_rec[kBatch][4];
+__global__ void __launch_bounds__(256, 4) blend_forward_kernel(const __grid_constant__ FwdParams P) {
+  // staged records as four float4 planes (lanes of a warp read different entries at the same time) + bounding boxes
+  __shared__ float4 s_r0[kBatch], s_r1[kBatch], s_r2[kBatch], s_r3[DEPTH_ONLY ? 1 : kBatch];
   __shared__ float4 s_bb[kBatch];
 
   const int tile = blockIdx.y * P.cam.TX + blockIdx.x;
@@ -43,9 +68,9 @@ __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constan
   const int iy = blockIdx.y * kTile + (warp >> 1) * 4 + (lane >> 3);
   const bool inside = ix < P.cam.W && iy < P.cam.H;
   const float px = (float)ix + 0.5f, py = (float)iy + 0.5f;
-  // pixel-centre extent of this warp's 8x4 block
-  const float wx0 = (float)(blockIdx.x * kTile + (warp & 1) * 8) + 0.5f, wx1 = wx0 + 7.0f;
-  const float wy0 = (float)(blockIdx.y * kTile + (warp >> 1) * 4) + 0.5f, wy1 = wy0 + 3.0f;
+  // first pixel centre of this warp's 8x4 block
+  const float wx0 = (float)(blockIdx.x * kTile + (warp & 1) * 8) + 0.5f;
+  const float wy0 = (float)(blockIdx.y * kTile + (warp >> 1) * 4) + 0.5f;
 
   float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
   float M1 = 0.f, M2 = 0.f, L = 0.f, zref = 0.f, med = P.cam.z_bg;
@@ -57,47 +82,46 @@ __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constan
     const uint32_t idx = base + threadIdx.x;
     if (idx < end) {
       const float4* r = P.rec + 4 * (size_t)P.vals[idx];
-      const float4 q0 = r[0], q1 = r[1], q2 = r[2];
-      s_rec[threadIdx.x][0] = q0;
-      s_rec[threadIdx.x][1] = q1;
-      s_rec[threadIdx.x][2] = q2;
-      if (!DEPTH_ONLY) s_rec[threadIdx.x][3] = r[3];
+      const float4 q0 = r[0], q1 = r[1];
+      s_r0[threadIdx.x] = q0;
+      s_r1[threadIdx.x] = q1;
+      s_r2[threadIdx.x] = r[2];
+      if (!DEPTH_ONLY) s_r3[threadIdx.x] = r[3];
       s_bb[threadIdx.x] = splat_bbox(q0, q1);
     }
     __syncthreads();
     const int n = min(kBatch, (int)(end - base));
     const int rel0 = (int)(base - start);
-    if (__all_sync(0xffffffffu, done)) continue;   // this warp's 8x4 pixels are all finished
     for (int g0 = 0; g0 < n; g0 += 32) {
-      // hierarchical culling: each lane tests one staged splat against the warp's 8x4 pixel block
-      bool hit = false;
-      if (g0 + lane < n) {
-        const float4 bb = s_bb[g0 + lane];
-        hit = bb.x <= wx1 && bb.y >= wx0 && bb.z <= wy1 && bb.w >= wy0;
-      }
-      unsigned mask = __ballot_sync(0xffffffffu, hit);
-      while (mask) {
-        const int j = g0 + __ffs(mask) - 1;
-        mask &= mask - 1;
-        const float4* e = s_rec[j];
-        const float4 r0 = e[0], r1 = e[1];
+      if (__all_sync(0xffffffffu, done)) break;   // this warp's 8x4 pixels are all finished
+      // per-pixel candidate lists of this group of 32 entries: lane l turns entry l's bounding box into the mask of
+      // block pixels it covers; the transpose hands every pixel the mask of entries that cover it
+      uint32_t cover = 0u;
+      if (g0 + lane < n) cover = block_cover_mask(s_bb[g0 + lane], wx0, wy0);
+      uint32_t m = warp_transpose_bits(cover, lane);
+      if (done) m = 0u;
+      // every pixel walks its own candidates, in list order
+      while (m) {
+        const int j = g0 + __ffs(m) - 1;
+        m &= m - 1;
+        const float4 r0 = s_r0[j], r1 = s_r1[j];
         const float dx = px - r0.x, dy = py - r0.y;
         const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
         const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
         const float rho = fminf(rho3, rho2);
-        if (done || rho > kRhoCut) continue;
+        if (!(rho <= kRhoCut)) continue;
         const float G = fast_exp2(rho * kNegHalfLog2e);                         // exp(-rho/2)
         const float a = fminf(kAlphaMax, r1.z * G);
         if (a < kAlphaMin) continue;
         const float Tn = T * (1.0f - a);
-        if (Tn < kTMin) { done = true; visited = rel0 + j + 1; continue; }
+        if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
         const float w = a * T;
-        const float4 r2 = e[2];
+        const float4 r2 = s_r2[j];
         const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
         if (DEPTH_ONLY) {
           M1 += w * z;
         } else {
-          const float4 r3 = e[3];
+          const float4 r3 = s_r3[j];
           if (ncontrib == 0) zref = z;
           const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
           if (T > 0.5f) { med = z; mi = rel0 + j; }
@@ -111,7 +135,6 @@ __global__ void __launch_bounds__(256) blend_forward_kernel(const __grid_constan
         last = rel0 + j + 1;
         ++ncontrib;
       }
-      if (__all_sync(0xffffffffu, done)) break;
     }
   }
   if (!inside) return;

@@ -29,6 +29,13 @@ __device__ __forceinline__ float fast_exp2(float x) {
   return y;
 }
 
+// 1/x, one MUFU.RCP (x is in [0.01, 1] here)
+__device__ __forceinline__ float fast_rcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // ---- device-side camera ------------------------------------------------------------------------------------
 struct DevCamera {
   int W, H, TX, TY;
