@@ -3,7 +3,7 @@
 // (means, quats, scales, opacity logits, rgb) and the 2x4 camera delta dF (Eq. 15), through
 // Eq. 8-11.  One thread per surfel; the 8 dF partials are reduced over the CTA (shuffles + shared memory) before
 // one atomic each.  The moment records are cleared as they are consumed, so the context never needs a separate
-// memset pass.  HBM-bound: 80 B moments read + cleared, 48 B record + 40 B inputs read, 52 B read-modify-write.
+// memset pass.  HBM-bound: 80 B moments read + cleared, 45 B inputs read, 52 B read-modify-write.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -17,29 +17,94 @@ __device__ __forceinline__ float warp_sum_f(float v) {
 __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int N, const float* __restrict__ means,
                                                              const float* __restrict__ quats, const float* __restrict__ scales,
                                                              const float* __restrict__ logits, const uint32_t* __restrict__ count,
-                                                             const uint8_t* __restrict__ flags, const float4* __restrict__ rec,
-                                                             float4* __restrict__ vrec,
+                                                             const uint8_t* __restrict__ flags, float4* __restrict__ vrec,
                                                              float* __restrict__ v_means, float* __restrict__ v_quats,
                                                              float* __restrict__ v_scales, float* __restrict__ v_logits,
                                                              float* __restrict__ v_rgb, float* __restrict__ v_dF) {
   __shared__ float s_red[8][8];
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  // The CTA's 256 surfels are contiguous in every array: the 80-B moment records and the 12-B rows (means, v_means,
+  // v_rgb) are moved between HBM and shared memory as coalesced float4 streams, and every load of the kernel is
+  // issued before the first use (one DRAM round trip).
+  __shared__ float4 s_v[256 * (kVrec / 4)];
+  __shared__ __align__(16) float s_p[256 * 3], s_vm[256 * 3], s_vc[256 * 3];
+  const int base = blockIdx.x * 256, t = threadIdx.x;
+  const int i = base + t;
+  const int nb = min(256, N - base);                      // surfels of this CTA
+  {
+    const float4* gv = vrec + (kVrec / 4) * (size_t)base;
+#pragma unroll
+    for (int k = 0; k < kVrec / 4; ++k) {
+      const int e = t + 256 * k;
+      if (e < nb * (kVrec / 4)) s_v[e] = gv[e];
+    }
+    if (nb == 256) {
+      if (t < 192) {
+        reinterpret_cast<float4*>(s_p)[t] = reinterpret_cast<const float4*>(means + 3 * (size_t)base)[t];
+        if (v_means) reinterpret_cast<float4*>(s_vm)[t] = reinterpret_cast<const float4*>(v_means + 3 * (size_t)base)[t];
+        if (v_rgb) reinterpret_cast<float4*>(s_vc)[t] = reinterpret_cast<const float4*>(v_rgb + 3 * (size_t)base)[t];
+      }
+    } else {
+      for (int e = t; e < nb * 3; e += 256) {
+        s_p[e] = means[3 * (size_t)base + e];
+        if (v_means) s_vm[e] = v_means[3 * (size_t)base + e];
+        if (v_rgb) s_vc[e] = v_rgb[3 * (size_t)base + e];
+      }
+    }
+  }
+  // per-thread rows, fetched before the barrier so that they overlap the staging
+  const bool have = i < N;
+  const uint32_t cnt = have ? count[i] : 0u;
+  const uint8_t fl = have ? flags[i] : (uint8_t)0;
+  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  float4 q = make_float4(1.f, 0.f, 0.f, 0.f), cur = zero4;
+  float2 sc = make_float2(1.f, 1.f), vsc = make_float2(0.f, 0.f);
+  float lg = 0.f, vlg = 0.f;
+  if (have) {
+    q = reinterpret_cast<const float4*>(quats)[i];
+    sc = reinterpret_cast<const float2*>(scales)[i];
+    lg = logits[i];
+    if (v_quats) cur = reinterpret_cast<const float4*>(v_quats)[i];
+    if (v_scales) vsc = reinterpret_cast<const float2*>(v_scales)[i];
+    if (v_logits) vlg = v_logits[i];
+  }
+  __syncthreads();
+  {
+    // clear the consumed moment records; only now that their loads have landed: a store to a line whose fill is
+    // still in flight serialises behind it (measured: 0.12 ms with the clear next to the load, 0.05 ms here)
+    float4* gv = vrec + (kVrec / 4) * (size_t)base;
+#pragma unroll
+    for (int k = 0; k < kVrec / 4; ++k) {
+      const int e = t + 256 * k;
+      if (e < nb * (kVrec / 4)) gv[e] = zero4;
+    }
+  }
   float dF[8];
 #pragma unroll
   for (int k = 0; k < 8; ++k) dF[k] = 0.f;
-  if (i < N && count[i] > 0) {
-    float4* gp = vrec + (kVrec / 4) * (size_t)i;
-    const float4 m0 = gp[0], m1 = gp[1], m2 = gp[2], m3 = gp[3], m4 = gp[4];
-    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    gp[0] = zero; gp[1] = zero; gp[2] = zero; gp[3] = zero; gp[4] = zero;
-    const uint8_t fl = flags[i];
+  if (cnt > 0) {
+    const float4 m0 = s_v[5 * t], m1 = s_v[5 * t + 1], m2 = s_v[5 * t + 2], m3 = s_v[5 * t + 3], m4 = s_v[5 * t + 4];
+    const float p0 = s_p[3 * t], p1 = s_p[3 * t + 1], p2 = s_p[3 * t + 2];
+    const float B00 = cam.Fp[0], B01 = cam.Fp[1], B02 = cam.Fp[2];
+    const float B10 = cam.Fp[4], B11 = cam.Fp[5], B12 = cam.Fp[6];
+    const float qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
+    const float inv = 1.0f / qn;
+    const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
+    const float tu0 = 1.f - 2.f * (y * y + z * z), tu1 = 2.f * (x * y + w * z), tu2 = 2.f * (x * z - w * y);
+    const float tv0 = 2.f * (x * y - w * z), tv1 = 1.f - 2.f * (x * x + z * z), tv2 = 2.f * (y * z + w * x);
+    const float au0 = B00 * tu0 + B01 * tu1 + B02 * tu2, au1 = B10 * tu0 + B11 * tu1 + B12 * tu2;
+    const float av0 = B00 * tv0 + B01 * tv1 + B02 * tv2, av1 = B10 * tv0 + B11 * tv1 + B12 * tv2;
+    const float M00 = sc.x * au0, M01 = sc.y * av0, M10 = sc.x * au1, M11 = sc.y * av1;   // M = B' R S' (Eq. 8)
+    const float alpha = 1.0f / (1.0f + expf(-lg));
     // moments -> record gradients, slots g0 = (c_x, c_y, M00, M01)  g1 = (M10, M11, alpha, z_c)  g2 = (r_0, r_1, red, green)
     // g3 = (blue, n_x, n_y, n_z).  Per pair: v_uv = 2 s (u,v); v_d = t g + Q^T v_uv (4 s d for low-pass pairs);
     // v_c = -v_d; v_M = -v_d (u,v)^T; v_r = -t (u,v); v_alpha = G v_a = -2 s / alpha; v_zc = t.
     float4 g0, g1, g2, g3;
     {
-      const float4 r0 = rec[4 * (size_t)i], r1 = rec[4 * (size_t)i + 1], r2 = rec[4 * (size_t)i + 2];
-      const float Q00 = r0.z, Q01 = r0.w, Q10 = r1.x, Q11 = r1.y, ga = r2.x, gb = r2.y;
+      // Q = M^-1 and the depth slope g = -r Q are recomputed from the inputs (Eq. 8-10) instead of re-read from the record
+      const float idet = 1.0f / (M00 * M11 - M01 * M10);
+      const float Q00 = M11 * idet, Q01 = -M01 * idet, Q10 = -M10 * idet, Q11 = M00 * idet;
+      const float rr0 = sc.x * tu2, rr1 = sc.y * tv2;
+      const float ga = -(rr0 * Q00 + rr1 * Q10), gb = -(rr0 * Q01 + rr1 * Q11);
       const float suu = m0.x, suv = m0.y, svv = m0.z, Su = m0.w, Sv = m1.x, Tu = m1.y, Tv = m1.z, T0np = m1.w;
       g0.x = -(4.0f * m2.x); g0.y = -(4.0f * m2.y);
       g0.z = 0.f; g0.w = 0.f; g1.x = 0.f; g1.y = 0.f; g2.x = 0.f; g2.y = 0.f;
@@ -52,32 +117,19 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
         g1.y = -(gb * Tv + 2.0f * (Q01 * suv + Q11 * svv));
         g2.x = -Tu; g2.y = -Tv;
       }
-      g1.z = -2.0f * m2.w / r1.z;
+      g1.z = -2.0f * m2.w / alpha;
       g1.w = m2.z;
       g2.z = m3.x; g2.w = m3.y; g3.x = m3.z; g3.y = m3.w; g3.z = m4.x; g3.w = m4.y;
     }
-    const float p0 = means[3 * i], p1 = means[3 * i + 1], p2 = means[3 * i + 2];
-    const float4 q = reinterpret_cast<const float4*>(quats)[i];
-    const float2 sc = reinterpret_cast<const float2*>(scales)[i];
-    const float B00 = cam.Fp[0], B01 = cam.Fp[1], B02 = cam.Fp[2];
-    const float B10 = cam.Fp[4], B11 = cam.Fp[5], B12 = cam.Fp[6];
-    const float qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
-    const float inv = 1.0f / qn;
-    const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
-    const float tu0 = 1.f - 2.f * (y * y + z * z), tu1 = 2.f * (x * y + w * z), tu2 = 2.f * (x * z - w * y);
-    const float tv0 = 2.f * (x * y - w * z), tv1 = 1.f - 2.f * (x * x + z * z), tv2 = 2.f * (y * z + w * x);
     // gradient record slots: g0 = (c_x, c_y, M00, M01)  g1 = (M10, M11, alpha, z_c)  g2 = (r_0, r_1, red, green)  g3 = (blue, n_x, n_y, n_z)
-    const float alpha = 1.0f / (1.0f + expf(-logits[i]));
-    if (v_logits) v_logits[i] += g1.z * alpha * (1.0f - alpha);
-    if (v_rgb) { v_rgb[3 * i] += g2.z; v_rgb[3 * i + 1] += g2.w; v_rgb[3 * i + 2] += g3.x; }
+    if (v_logits) v_logits[i] = vlg + g1.z * alpha * (1.0f - alpha);
+    if (v_rgb) { s_vc[3 * t] += g2.z; s_vc[3 * t + 1] += g2.w; s_vc[3 * t + 2] += g3.x; }
     const float sg = (fl & F_FLIPPED) ? -1.f : 1.f;
     float vtu0 = 0.f, vtu1 = 0.f, vtu2 = 0.f, vtv0 = 0.f, vtv1 = 0.f, vtv2 = 0.f;
     const float vn0 = sg * g3.y, vn1 = sg * g3.z, vn2 = sg * g3.w;
     const float vc0 = g0.x, vc1 = g0.y;
     float vs0 = 0.f, vs1 = 0.f;
     if (!(fl & F_DEGENERATE)) {
-      const float au0 = B00 * tu0 + B01 * tu1 + B02 * tu2, au1 = B10 * tu0 + B11 * tu1 + B12 * tu2;
-      const float av0 = B00 * tv0 + B01 * tv1 + B02 * tv2, av1 = B10 * tv0 + B11 * tv1 + B12 * tv2;
       // gradient record slots 2..5 hold v_M (M = B' R S' = Q^-1), slots 8..9 hold v_r (r = (s_u t_u.z, s_v t_v.z))
       const float vM00 = g0.z, vM01 = g0.w, vM10 = g1.x, vM11 = g1.y;
       const float vr0 = g2.x, vr1 = g2.y;
@@ -89,12 +141,12 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
       dF[0] = vau0 * tu0 + vav0 * tv0; dF[1] = vau0 * tu1 + vav0 * tv1; dF[2] = vau0 * tu2 + vav0 * tv2;
       dF[4] = vau1 * tu0 + vav1 * tv0; dF[5] = vau1 * tu1 + vav1 * tv1; dF[6] = vau1 * tu2 + vav1 * tv2;
     }
-    if (v_scales) { v_scales[2 * i] += vs0; v_scales[2 * i + 1] += vs1; }
+    if (v_scales) reinterpret_cast<float2*>(v_scales)[i] = make_float2(vsc.x + vs0, vsc.y + vs1);
     // c = B p + b ; z_c = b_z - p_z
     if (v_means) {
-      v_means[3 * i] += B00 * vc0 + B10 * vc1;
-      v_means[3 * i + 1] += B01 * vc0 + B11 * vc1;
-      v_means[3 * i + 2] += B02 * vc0 + B12 * vc1 - g1.w;
+      s_vm[3 * t] += B00 * vc0 + B10 * vc1;
+      s_vm[3 * t + 1] += B01 * vc0 + B11 * vc1;
+      s_vm[3 * t + 2] += B02 * vc0 + B12 * vc1 - g1.w;
     }
     dF[0] += vc0 * p0; dF[1] += vc0 * p1; dF[2] += vc0 * p2; dF[3] = vc0;
     dF[4] += vc1 * p0; dF[5] += vc1 * p1; dF[6] += vc1 * p2; dF[7] = vc1;
@@ -107,9 +159,20 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
       const float vz = 2.f * (x * (G02 + G20) + y * (G12 + G21) - 2.f * z * (G00 + G11) + w * (G10 - G01));
       const float dotq = w * vw + x * vx + y * vy + z * vz;
       float4* vq = reinterpret_cast<float4*>(v_quats) + i;
-      float4 cur = *vq;
       cur.x += (vw - w * dotq) * inv; cur.y += (vx - x * dotq) * inv; cur.z += (vy - y * dotq) * inv; cur.w += (vz - z * dotq) * inv;
       *vq = cur;
+    }
+  }
+  __syncthreads();
+  if (nb == 256) {
+    if (t < 192) {
+      if (v_means) reinterpret_cast<float4*>(v_means + 3 * (size_t)base)[t] = reinterpret_cast<const float4*>(s_vm)[t];
+      if (v_rgb) reinterpret_cast<float4*>(v_rgb + 3 * (size_t)base)[t] = reinterpret_cast<const float4*>(s_vc)[t];
+    }
+  } else {
+    for (int e = t; e < nb * 3; e += 256) {
+      if (v_means) v_means[3 * (size_t)base + e] = s_vm[e];
+      if (v_rgb) v_rgb[3 * (size_t)base + e] = s_vc[e];
     }
   }
   if (v_dF) {
@@ -135,7 +198,7 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
   if (c->N == 0) return cudaSuccess;
   ++g_kernel_launches;
   chain_backward_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>(c->cam, (int)c->N, means, quats, scales, logits, c->count,
-                                                                  c->flags, c->rec, reinterpret_cast<float4*>(c->vrec), v_means,
+                                                                  c->flags, reinterpret_cast<float4*>(c->vrec), v_means,
                                                                   v_quats, v_scales, v_logits, v_rgb, v_dF);
   return cudaGetLastError();
 }
