@@ -24,10 +24,13 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
                                                          float4* __restrict__ rec, ushort4* __restrict__ rect,
                                                          uint32_t* __restrict__ count, uint32_t* __restrict__ depth_key,
                                                          uint8_t* __restrict__ flags, uint32_t* __restrict__ tile_count) {
+  // records leave through shared memory so that the CTA's 256 x 64 B go out as one contiguous float4 stream
+  __shared__ float4 s_rec[256 * 4];
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   int cnt = 0, tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
   if (i < N) {
   const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
+  const float cr = rgb[3 * i], cg = rgb[3 * i + 1], cb = rgb[3 * i + 2];
   const float4 q = reinterpret_cast<const float4*>(quats)[i];
   const float2 sc = reinterpret_cast<const float2*>(scales)[i];
   const float logit = logits[i];
@@ -91,13 +94,21 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   if (dotv > 0.0f) { n0 = -n0; n1 = -n1; nz = -nz; fl |= F_FLIPPED; }
   const float alpha = 1.0f / (1.0f + expf(-logit));
   flags[i] = fl;
-  if (cnt > 0) {
-    float4* r = rec + 4 * (size_t)i;
-    r[0] = make_float4(cx, cy, Q00, Q01);
-    r[1] = make_float4(Q10, Q11, alpha, zc);
-    r[2] = make_float4(g0, g1, rgb[3 * i], rgb[3 * i + 1]);
-    r[3] = make_float4(rgb[3 * i + 2], n0, n1, nz);
+  float4* r = s_rec + 4 * threadIdx.x;      // culled surfels: the slot is written too, and never read
+  r[0] = make_float4(cx, cy, Q00, Q01);
+  r[1] = make_float4(Q10, Q11, alpha, zc);
+  r[2] = make_float4(g0, g1, cr, cg);
+  r[3] = make_float4(cb, n0, n1, nz);
   }
+  __syncthreads();
+  {
+    const int nb = min(256, N - (int)(blockIdx.x * blockDim.x));
+    float4* out = rec + 4 * (size_t)blockIdx.x * blockDim.x;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int e = threadIdx.x + 256 * k;
+      if (e < 4 * nb) out[e] = s_rec[e];
+    }
   }
   // tile-sort binning: count the (tile, surfel) pairs per tile with fire-and-forget RED atomics; surfels covering
   // many tiles (oversized splats) are expanded by the whole warp
