@@ -117,6 +117,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   const size_t px = (size_t)max_w * (size_t)max_h;
 #define A(call) if (e == cudaSuccess) e = (call)
   A(dalloc(ctx, &ctx->rec, N * 4));
+  A(dalloc(ctx, &ctx->bbox, N));
   A(dalloc(ctx, &ctx->rect, N * 4));
   A(dalloc(ctx, &ctx->count, N));
   A(dalloc(ctx, &ctx->offset, N + 1));
@@ -159,7 +160,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
 void satsplat_destroy(satsplat_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
-  void* ptrs[] = {ctx->rec, ctx->rect, ctx->count, ctx->offset, ctx->depth_key, ctx->flags, ctx->vrec, ctx->block_sums,
+  void* ptrs[] = {ctx->rec, ctx->bbox, ctx->rect, ctx->count, ctx->offset, ctx->depth_key, ctx->flags, ctx->vrec, ctx->block_sums,
                   ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->tile_count,
                   ctx->tile_start, ctx->worklist, ctx->wl_count, ctx->px_a,
                   ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in, ctx->e2e_up,

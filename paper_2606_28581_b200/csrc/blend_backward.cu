@@ -2,13 +2,16 @@
 //
 // Per pixel: epilogue backward first (gradients of the 3x4 colour correction, the ambient light, the
 // reprojection constants; scatter into the sun-depth gradient), then the tile list is walked in REVERSE order:
-// T_i is recovered as T_{i+1}/(1 - a_i) and the suffix sum S_i = sum_{k>i} w_k phi_k is carried.  The walk only
-// produces, per contributing (pixel, surfel) pair, the three scalars the gradients are linear in (dL/d rho,
-// dL/d z, w) and the pair's local coordinates; the lanes of a warp that hit the same surfel append them,
-// ballot-compacted, to a small per-warp segment buffer in shared memory.  Every eight segments the warp turns
-// into eight teams of 4 lanes: a team walks one segment with all lanes busy, accumulates the 18 gradient moments
-// of that surfel, reduces them over its 4 lanes (transposed butterfly) and adds them to the surfel's moment
-// record with 16-byte vector REDs.  FP32-issue bound.
+// T_i is recovered as T_{i+1}/(1 - a_i) and the suffix sum S_i = sum_{k>i} w_k phi_k is carried.
+//
+// A warp owns an 8x4 pixel block and walks the tile's list on its own (no CTA barrier in the walk): per group of
+// 32 list entries it culls by bounding box (one entry per lane, ballot) and gathers only the survivors' records
+// into its shared-memory slots.  The walk only produces, per contributing (pixel, surfel) pair, the three scalars
+// the gradients are linear in (dL/d rho, dL/d z, w) and the pair's local coordinates; the lanes that hit the same
+// surfel append them, ballot-compacted, to a per-warp segment buffer.  Every eight segments the warp turns into
+// eight teams of 4 lanes: a team walks one segment with all lanes busy, accumulates the 18 gradient moments of
+// that surfel, reduces them over its 4 lanes (transposed butterfly) and adds them to the surfel's moment record
+// with 16-byte vector REDs.  FP32-issue bound.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -19,6 +22,7 @@ struct BwdParams {
   const uint32_t* ranges;
   const uint32_t* vals;
   const float4* rec;
+  const float4* bbox;
   const float4* v_rgba;
   const float4* v_geom;
   const float4* v_aux;
@@ -32,14 +36,13 @@ struct BwdParams {
 };
 
 #ifndef SATSPLAT_BWD_WARPS
-#define SATSPLAT_BWD_WARPS 8
+#define SATSPLAT_BWD_WARPS 4
 #endif
 #ifndef SATSPLAT_BWD_MINB
-#define SATSPLAT_BWD_MINB 3
+#define SATSPLAT_BWD_MINB 6
 #endif
 constexpr int kWarpsB = SATSPLAT_BWD_WARPS;   // warps per CTA: 8 = one 16x16 tile, 4 = its upper or lower half
 constexpr int kThreadsB = 32 * kWarpsB;
-constexpr int kBatchB = kThreadsB;
 #ifndef SATSPLAT_BWD_TEAM
 #define SATSPLAT_BWD_TEAM 4
 #endif
@@ -117,14 +120,12 @@ __device__ __forceinline__ float warp_reduce32_transposed(float (&v)[32], int la
 template <bool DEPTH_ONLY>
 __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_kernel(const __grid_constant__ BwdParams P) {
   constexpr int kRecV = DEPTH_ONLY ? 3 : 4;
-  __shared__ float4 s_rec[kBatchB][kRecV];
-  __shared__ float4 s_bb[kBatchB];
-  __shared__ uint32_t s_id[kBatchB];
+  __shared__ float4 s_wrec[kWarpsB][32][kRecV];   // per warp: records of the current group's survivors
+  __shared__ int2 s_widx[kWarpsB][32];            //           and their (list index, surfel id)
   // per warp: pending pairs (s, t, w, source lane | low-pass flag) and their local coordinates: (u, v), or (dx, dy)
   // for low-pass pairs; kSegs segments of up to 32 pairs each (dynamic shared memory: kPairBytes per CTA)
   extern __shared__ float4 s_dyn[];
   __shared__ float s_red[kWarpsB][24];
-  __shared__ int s_max[kWarpsB];
 
   // CTA blockIdx.y holds warps [blockIdx.y * kWarpsB, +kWarpsB) of tile column blockIdx.x; a tile has 8 warps (8x4 px each)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -226,16 +227,6 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       }
     }
   }
-  // ---- CTA-wide maximum of `last` ----
-  {
-    const int m = __reduce_max_sync(0xffffffffu, last);
-    if (lane == 0) s_max[warp] = m;
-  }
-  __syncthreads();
-  int max_last = 0;
-#pragma unroll
-  for (int w = 0; w < kWarpsB; ++w) max_last = max(max_last, s_max[w]);
-
   const float TfvT = Tf * vT;
   float Ssum = 0.f;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -302,78 +293,86 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
     __syncwarp();
   };
 
-  const int nb = (max_last + kBatchB - 1) / kBatchB;
-  for (int b = nb - 1; b >= 0; --b) {
-    const int rel0 = b * kBatchB;
-    const int n = min(kBatchB, max_last - rel0);
-    if ((int)threadIdx.x < n) {
-      const uint32_t id = P.vals[start + rel0 + threadIdx.x];
-      const float4* r = P.rec + 4 * (size_t)id;
-      s_id[threadIdx.x] = id;
-      const float4 q0 = r[0], q1 = r[1];
-      s_rec[threadIdx.x][0] = q0;
-      s_rec[threadIdx.x][1] = q1;
-      s_rec[threadIdx.x][2] = r[2];
-      if (!DEPTH_ONLY) s_rec[threadIdx.x][3] = r[3];
-      s_bb[threadIdx.x] = splat_bbox(q0, q1);
+  // ---- the walk: every warp is on its own (no CTA barrier below this line) ----
+  // The tile list is consumed in groups of 32 entries, last group first.  Per group: lane l takes entry l, tests its
+  // bounding box against the warp's 8x4 block (ballot), and the survivors' records are gathered into the warp's
+  // shared-memory slots in walk order.  Surfel ids are fetched two groups ahead and boxes one group ahead, so only
+  // the record gather waits on memory.
+  const int wlast = __reduce_max_sync(0xffffffffu, last);   // nothing beyond this index matters to this warp
+  float4 (*const wrec)[kRecV] = s_wrec[warp];
+  int2* const widx = s_widx[warp];
+  const unsigned gt_mask = ~((2u << lane) - 1u);
+  constexpr uint32_t kNoId = 0xffffffffu;
+  auto fetch_id = [&](int cc) -> uint32_t {
+    const int idx = cc * 32 + lane;
+    return (cc >= 0 && idx < wlast) ? P.vals[start + idx] : kNoId;
+  };
+  const float4 bb_none = make_float4(1e30f, -1e30f, 1e30f, -1e30f);
+  int c = (wlast + 31) / 32 - 1;
+  uint32_t id_cur = fetch_id(c);
+  float4 bb_cur = id_cur != kNoId ? P.bbox[id_cur] : bb_none;
+  uint32_t id_nxt = fetch_id(c - 1);
+  for (; c >= 0; --c) {
+    const float4 bb_nxt = id_nxt != kNoId ? P.bbox[id_nxt] : bb_none;
+    const uint32_t id_nn = fetch_id(c - 2);
+    const bool hit = bb_cur.x <= wx1 && bb_cur.y >= wx0 && bb_cur.z <= wy1 && bb_cur.w >= wy0;
+    const unsigned mask = __ballot_sync(0xffffffffu, hit);
+    const int nsurv = __popc(mask);
+    if (hit) {
+      const int slot = __popc(mask & gt_mask);   // highest list index first
+      const float4* r = P.rec + 4 * (size_t)id_cur;
+      const float4 q0 = r[0], q1 = r[1], q2 = r[2];
+      wrec[slot][0] = q0; wrec[slot][1] = q1; wrec[slot][2] = q2;
+      if (!DEPTH_ONLY) wrec[slot][3] = r[3];
+      widx[slot] = make_int2(c * 32 + lane, (int)id_cur);
     }
-    __syncthreads();
-    const int wlast = __reduce_max_sync(0xffffffffu, last);   // nothing beyond this index matters to this warp
-    for (int g0 = ((n - 1) >> 5) << 5; g0 >= 0; g0 -= 32) {
-      bool hit = false;
-      if (g0 + lane < n && rel0 + g0 + lane < wlast) {
-        const float4 bb = s_bb[g0 + lane];
-        hit = bb.x <= wx1 && bb.y >= wx0 && bb.z <= wy1 && bb.w >= wy0;
-      }
-      unsigned mask = __ballot_sync(0xffffffffu, hit);
-      while (mask) {
-        const int bit = 31 - __clz(mask);
-        mask &= ~(1u << bit);
-        const int j = g0 + bit;
-        const float4* e = s_rec[j];
-        const float4 r0 = e[0], r1 = e[1];
-        const float dx = px - r0.x, dy = py - r0.y;
-        const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
-        const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);
-        const float rho = fminf(rho3, rho2);
-        const float aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
-        const float a = fminf(kAlphaMax, aG);
-        const bool active = (rel0 + j < last) && (rho <= kRhoCut) && (a >= kAlphaMin);
-        const unsigned hm = __ballot_sync(0xffffffffu, active);
-        if (hm == 0) continue;
-        if (active) {
-          const float4 r2 = e[2];
-          const bool lowpass = !(rho3 <= rho2);
-          const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
-          const float zs = z - zref;
-          const float rc = fast_rcp(1.0f - a);
-          const float Ti = T * rc;
-          const float w = a * Ti;
-          float phi, v_z;
-          if (DEPTH_ONLY) {
-            phi = vD * zs;
-            v_z = w * vD;
-          } else {
-            const float4 r3 = e[3];
-            const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
-            phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
-            v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((rel0 + j == mi) ? vmed : 0.f);
-          }
-          const float v_a = Ti * phi - (Ssum + TfvT) * rc;
-          Ssum += w * phi;
-          T = Ti;
-          const float v_rho = (aG < kAlphaMax) ? -0.5f * aG * v_a : 0.f;   // alpha' = alpha G unless clamped
-          const int pos = nseg * 32 + __popc(hm & lt_mask);
-          p4[pos] = make_float4(v_rho, v_z, w, __int_as_float(lane | (lowpass ? 32 : 0)));
-          p2[pos] = lowpass ? make_float2(dx, dy) : make_float2(u, v);
+    __syncwarp();
+    for (int sv = 0; sv < nsurv; ++sv) {
+      const float4* e = wrec[sv];
+      const int2 ji = widx[sv];
+      const float4 r0 = e[0], r1 = e[1];
+      const float dx = px - r0.x, dy = py - r0.y;
+      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
+      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);
+      const float rho = fminf(rho3, rho2);
+      const float aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
+      const float a = fminf(kAlphaMax, aG);
+      const bool active = (ji.x < last) && (rho <= kRhoCut) && (a >= kAlphaMin);
+      const unsigned hm = __ballot_sync(0xffffffffu, active);
+      if (hm == 0) continue;
+      if (active) {
+        const float4 r2 = e[2];
+        const bool lowpass = !(rho3 <= rho2);
+        const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
+        const float zs = z - zref;
+        const float rc = fast_rcp(1.0f - a);
+        const float Ti = T * rc;
+        const float w = a * Ti;
+        float phi, v_z;
+        if (DEPTH_ONLY) {
+          phi = vD * zs;
+          v_z = w * vD;
+        } else {
+          const float4 r3 = e[3];
+          const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
+          phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
+          v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((ji.x == mi) ? vmed : 0.f);
         }
-        const int cnt = __popc(hm);
-        if (team == nseg) { my_cnt = cnt; my_id = s_id[j]; }
-        wmax = max(wmax, cnt);
-        if (++nseg == kSegs) flush();
+        const float v_a = Ti * phi - (Ssum + TfvT) * rc;
+        Ssum += w * phi;
+        T = Ti;
+        const float v_rho = (aG < kAlphaMax) ? -0.5f * aG * v_a : 0.f;   // alpha' = alpha G unless clamped
+        const int pos = nseg * 32 + __popc(hm & lt_mask);
+        p4[pos] = make_float4(v_rho, v_z, w, __int_as_float(lane | (lowpass ? 32 : 0)));
+        p2[pos] = lowpass ? make_float2(dx, dy) : make_float2(u, v);
       }
+      const int cnt = __popc(hm);
+      if (team == nseg) { my_cnt = cnt; my_id = (uint32_t)ji.y; }
+      wmax = max(wmax, cnt);
+      if (++nseg == kSegs) flush();
     }
-    __syncthreads();
+    __syncwarp();
+    id_cur = id_nxt; bb_cur = bb_nxt; id_nxt = id_nn;
   }
   if (nseg) flush();
 }
@@ -387,6 +386,7 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.ranges = c->ranges;
   P.vals = c->vals[c->sorted];
   P.rec = c->rec;
+  P.bbox = c->bbox;
   P.v_rgba = reinterpret_cast<const float4*>(v_rgba);
   P.v_geom = reinterpret_cast<const float4*>(v_geom);
   P.v_aux = reinterpret_cast<const float4*>(v_aux);

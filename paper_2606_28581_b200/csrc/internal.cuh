@@ -121,6 +121,7 @@ struct satsplat_ctx {
   int64_t scratch_bytes;
   // per-surfel
   float4* rec;            // [N*4]
+  float4* bbox;           // [N] conservative screen-space box of each record (splat_bbox), for the blend kernels' culling
   uint16_t* rect;         // [N*4]
   uint32_t* count;        // [N]
   uint32_t* offset;       // [N+1] exclusive scan

@@ -21,7 +21,7 @@ __device__ __forceinline__ int tile_of(float v, int T) {
 __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, const float* __restrict__ means,
                                                          const float* __restrict__ quats, const float* __restrict__ scales,
                                                          const float* __restrict__ logits, const float* __restrict__ rgb,
-                                                         float4* __restrict__ rec, ushort4* __restrict__ rect,
+                                                         float4* __restrict__ rec, float4* __restrict__ bbox, ushort4* __restrict__ rect,
                                                          uint32_t* __restrict__ count, uint32_t* __restrict__ depth_key,
                                                          uint8_t* __restrict__ flags, uint32_t* __restrict__ tile_count) {
   // records leave through shared memory so that the CTA's 256 x 64 B go out as one contiguous float4 stream
@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   r[1] = make_float4(Q10, Q11, alpha, zc);
   r[2] = make_float4(g0, g1, cr, cg);
   r[3] = make_float4(cb, n0, n1, nz);
+  bbox[i] = splat_bbox(r[0], r[1]);
   }
   __syncthreads();
   {
@@ -135,7 +136,7 @@ cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, co
   const int threads = 256;
   const int blocks = (int)((N + threads - 1) / threads);
   ++g_kernel_launches;
-  preprocess_kernel<<<blocks, threads, 0, s>>>(c->cam, (int)N, means, quats, scales, logits, rgb, c->rec,
+  preprocess_kernel<<<blocks, threads, 0, s>>>(c->cam, (int)N, means, quats, scales, logits, rgb, c->rec, c->bbox,
                                                reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags,
                                                c->binning_mode == SATSPLAT_BINNING_TILESORT ? c->tile_count : nullptr);
   return cudaGetLastError();
