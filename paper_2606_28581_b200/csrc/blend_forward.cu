@@ -3,12 +3,12 @@
 // Gaussian evaluated through the exact per-splat affine map u = Q (x - c) (Eq. 9), and (a5) the Eq. 1 epilogue
 // (colour correction + soft shadow test against the sun-view depth map) fused after the loop.
 //
-// One CTA per tile, one thread per pixel; a warp covers an 8x4 pixel block.  Splat records are staged through
-// shared memory in batches of 256 together with a conservative bounding box.  Per group of 32 entries, lane l turns
-// entry l's box into the bit mask of the block's pixels it covers; a 32x32 bit transpose across the warp (5 shuffles)
-// hands every pixel the mask of entries whose box covers it, and each pixel then walks only its own candidates, in
-// list order (the walk diverges across lanes; the per-pair test and the blend are exactly those of Eq. 9/12/14).
-// FP32-issue bound.
+// One thread per pixel; a warp owns an 8x4 pixel block and walks the tile's list on its own (no CTA barrier).  Per
+// group of 32 list entries, lane l turns entry l's precomputed bounding box into the bit mask of the block's pixels
+// it covers; entries with a non-empty mask have their records gathered into the warp's shared-memory slots; a 32x32
+// bit transpose across the warp (5 shuffles) hands every pixel the mask of entries whose box covers it, and each
+// pixel then walks only its own candidates, in list order (the walk diverges across lanes; the per-pair test and
+// the blend are exactly those of Eq. 9/12/14).  FP32-issue bound.
 #include "internal.cuh"
 
 namespace satsplat {
@@ -19,6 +19,7 @@ struct FwdParams {
   const uint32_t* ranges;
   const uint32_t* vals;
   const float4* rec;
+  const float4* bbox;
   float4* out_rgba;
   float4* out_geom;
   float4* out_aux;
@@ -30,7 +31,14 @@ struct FwdParams {
   int32_t* px_contrib;
 };
 
-constexpr int kBatch = 256;
+#ifndef SATSPLAT_FWD_WARPS
+#define SATSPLAT_FWD_WARPS 4
+#endif
+#ifndef SATSPLAT_FWD_MINB
+#define SATSPLAT_FWD_MINB 8
+#endif
+constexpr int kWarpsF = SATSPLAT_FWD_WARPS;   // warps per CTA; a 16x16 tile is 8 warps (8x4 px each)
+constexpr int kThreadsF = 32 * kWarpsF;
 
 // 32x32 bit-matrix transpose across the warp: lane l passes row l, and receives column l (bit b = bit l of lane b's row).
 __device__ __forceinline__ uint32_t warp_transpose_bits(uint32_t x, int lane) {
@@ -56,87 +64,110 @@ __device__ __forceinline__ uint32_t block_cover_mask(const float4 bb, float wx0,
 }
 
 template <bool DEPTH_ONLY>
-__global__ void __launch_bounds__(256, 4) blend_forward_kernel(const __grid_constant__ FwdParams P) {
-  // staged records as four float4 planes (lanes of a warp read different entries at the same time) + bounding boxes
-  __shared__ float4 s_r0[kBatch], s_r1[kBatch], s_r2[kBatch], s_r3[DEPTH_ONLY ? 1 : kBatch];
-  __shared__ float4 s_bb[kBatch];
+__global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_kernel(const __grid_constant__ FwdParams P) {
+  // per warp, double buffered: the records of a group's survivors as four float4 planes (lanes of a warp read
+  // different entries at the same time)
+  __shared__ float4 s_r0[2][kWarpsF][32], s_r1[2][kWarpsF][32], s_r2[2][kWarpsF][32], s_r3[2][DEPTH_ONLY ? 1 : kWarpsF][32];
 
-  const int tile = blockIdx.y * P.cam.TX + blockIdx.x;
-  const uint32_t start = P.ranges[2 * tile], end = P.ranges[2 * tile + 1];
+  // CTA blockIdx.y holds warps [blockIdx.y * kWarpsF, +kWarpsF) of tile column blockIdx.x
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int ix = blockIdx.x * kTile + (warp & 1) * 8 + (lane & 7);
-  const int iy = blockIdx.y * kTile + (warp >> 1) * 4 + (lane >> 3);
+  const int gw = blockIdx.y * kWarpsF + warp, ty = gw >> 3, wi = gw & 7;
+  const int tile = ty * P.cam.TX + blockIdx.x;
+  const uint32_t start = P.ranges[2 * tile], end = P.ranges[2 * tile + 1];
+  const int bx0 = blockIdx.x * kTile + (wi & 1) * 8, by0 = ty * kTile + (wi >> 1) * 4;
+  const int ix = bx0 + (lane & 7), iy = by0 + (lane >> 3);
   const bool inside = ix < P.cam.W && iy < P.cam.H;
   const float px = (float)ix + 0.5f, py = (float)iy + 0.5f;
-  // first pixel centre of this warp's 8x4 block
-  const float wx0 = (float)(blockIdx.x * kTile + (warp & 1) * 8) + 0.5f;
-  const float wy0 = (float)(blockIdx.y * kTile + (warp >> 1) * 4) + 0.5f;
+  const float wx0 = (float)bx0 + 0.5f, wy0 = (float)by0 + 0.5f;   // first pixel centre of this warp's 8x4 block
 
   float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
   float M1 = 0.f, M2 = 0.f, L = 0.f, zref = 0.f, med = P.cam.z_bg;
   int mi = -1, last = 0, visited = 0, ncontrib = 0;
   bool done = !inside;
 
-  for (uint32_t base = start; base < end; base += kBatch) {
-    if (__syncthreads_and(done)) break;
-    const uint32_t idx = base + threadIdx.x;
-    if (idx < end) {
-      const float4* r = P.rec + 4 * (size_t)P.vals[idx];
-      const float4 q0 = r[0], q1 = r[1];
-      s_r0[threadIdx.x] = q0;
-      s_r1[threadIdx.x] = q1;
-      s_r2[threadIdx.x] = r[2];
-      if (!DEPTH_ONLY) s_r3[threadIdx.x] = r[3];
-      s_bb[threadIdx.x] = splat_bbox(q0, q1);
+  // Every warp walks the tile's list on its own (no CTA barrier), in groups of 32 entries, software-pipelined:
+  // surfel ids are fetched three groups ahead, boxes two groups ahead, and the survivors' records are gathered one
+  // group ahead with asynchronous copies into the other half of the double buffer.
+  const int len = (int)(end - start);
+  const int ngroups = (len + 31) >> 5;
+  constexpr uint32_t kNoId = 0xffffffffu;
+  auto fetch_id = [&](int cc) -> uint32_t {
+    const int idx = cc * 32 + lane;
+    return idx < len ? P.vals[start + idx] : kNoId;
+  };
+  const float4 bb_none = make_float4(1e30f, -1e30f, 1e30f, -1e30f);
+  auto fetch_bb = [&](uint32_t id) -> float4 { return id != kNoId ? P.bbox[id] : bb_none; };
+  // lane l turns entry l's bounding box into the mask of block pixels it covers; survivors (non-empty masks) have
+  // their records gathered into the warp's slots (slot = lane) of buffer `buf`
+  auto gather = [&](uint32_t id, uint32_t cover, int buf) {
+    if (cover != 0u) {
+      const float4* r = P.rec + 4 * (size_t)id;
+      cp_async16(&s_r0[buf][warp][lane], r);
+      cp_async16(&s_r1[buf][warp][lane], r + 1);
+      cp_async16(&s_r2[buf][warp][lane], r + 2);
+      if (!DEPTH_ONLY) cp_async16(&s_r3[buf][warp][lane], r + 3);
     }
-    __syncthreads();
-    const int n = min(kBatch, (int)(end - base));
-    const int rel0 = (int)(base - start);
-    for (int g0 = 0; g0 < n; g0 += 32) {
-      if (__all_sync(0xffffffffu, done)) break;   // this warp's 8x4 pixels are all finished
-      // per-pixel candidate lists of this group of 32 entries: lane l turns entry l's bounding box into the mask of
-      // block pixels it covers; the transpose hands every pixel the mask of entries that cover it
-      uint32_t cover = 0u;
-      if (g0 + lane < n) cover = block_cover_mask(s_bb[g0 + lane], wx0, wy0);
-      uint32_t m = warp_transpose_bits(cover, lane);
-      if (done) m = 0u;
-      // every pixel walks its own candidates, in list order
-      while (m) {
-        const int j = g0 + __ffs(m) - 1;
-        m &= m - 1;
-        const float4 r0 = s_r0[j], r1 = s_r1[j];
-        const float dx = px - r0.x, dy = py - r0.y;
-        const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
-        const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
-        const float rho = fminf(rho3, rho2);
-        if (!(rho <= kRhoCut)) continue;
-        const float G = fast_exp2(rho * kNegHalfLog2e);                         // exp(-rho/2)
-        const float a = fminf(kAlphaMax, r1.z * G);
-        if (a < kAlphaMin) continue;
-        const float Tn = T * (1.0f - a);
-        if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
-        const float w = a * T;
-        const float4 r2 = s_r2[j];
-        const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
-        if (DEPTH_ONLY) {
-          M1 += w * z;
-        } else {
-          const float4 r3 = s_r3[j];
-          if (ncontrib == 0) zref = z;
-          const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
-          if (T > 0.5f) { med = z; mi = rel0 + j; }
-          L += w * (zs * zs * (1.0f - T) + M2 - 2.0f * zs * M1);
-          C0 += w * r2.z; C1 += w * r2.w; C2 += w * r3.x;
-          N0 += w * r3.y; N1 += w * r3.z; N2 += w * r3.w;
-          M1 += w * zs;
-          M2 += w * zs * zs;
-        }
-        T = Tn;
-        last = rel0 + j + 1;
-        ++ncontrib;
+    cp_async_commit();
+  };
+  uint32_t id_a = fetch_id(0), id_b = fetch_id(1), id_c = fetch_id(2);   // groups c, c+1, c+2
+  float4 bb_a = fetch_bb(id_a);
+  float4 bb_b = fetch_bb(id_b);
+  uint32_t cover = block_cover_mask(bb_a, wx0, wy0);
+  gather(id_a, cover, 0);
+  for (int c = 0; c < ngroups; ++c) {
+    if (__all_sync(0xffffffffu, done)) break;   // this warp's 8x4 pixels are all finished
+    // next group: boxes -> cover masks -> record gather in flight while this group is walked
+    const uint32_t cover_n = block_cover_mask(bb_b, wx0, wy0);
+    gather(id_b, cover_n, (c + 1) & 1);
+    const float4 bb_c = fetch_bb(id_c);
+    const uint32_t id_d = fetch_id(c + 3);
+    // the 32x32 bit transpose hands every pixel the mask of entries whose box covers it
+    uint32_t m = warp_transpose_bits(cover, lane);
+    if (done) m = 0u;
+    cp_async_wait<1>();   // this group's records have landed
+    __syncwarp();
+    const int buf = c & 1;
+    const int rel0 = c * 32;
+    // every pixel walks its own candidates, in list order
+    while (m) {
+      const int j = __ffs(m) - 1;
+      m &= m - 1;
+      const float4 r0 = s_r0[buf][warp][j], r1 = s_r1[buf][warp][j];
+      const float dx = px - r0.x, dy = py - r0.y;
+      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
+      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
+      const float rho = fminf(rho3, rho2);
+      if (!(rho <= kRhoCut)) continue;
+      const float G = fast_exp2(rho * kNegHalfLog2e);                         // exp(-rho/2)
+      const float a = fminf(kAlphaMax, r1.z * G);
+      if (a < kAlphaMin) continue;
+      const float Tn = T * (1.0f - a);
+      if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
+      const float w = a * T;
+      const float4 r2 = s_r2[buf][warp][j];
+      const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
+      if (DEPTH_ONLY) {
+        M1 += w * z;
+      } else {
+        const float4 r3 = s_r3[buf][warp][j];
+        if (ncontrib == 0) zref = z;
+        const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
+        if (T > 0.5f) { med = z; mi = rel0 + j; }
+        L += w * (zs * zs * (1.0f - T) + M2 - 2.0f * zs * M1);
+        C0 += w * r2.z; C1 += w * r2.w; C2 += w * r3.x;
+        N0 += w * r3.y; N1 += w * r3.z; N2 += w * r3.w;
+        M1 += w * zs;
+        M2 += w * zs * zs;
       }
+      T = Tn;
+      last = rel0 + j + 1;
+      ++ncontrib;
     }
+    __syncwarp();
+    cover = cover_n;
+    id_b = id_c; bb_b = bb_c; id_c = id_d;
   }
+  cp_async_wait<0>();
   if (!inside) return;
   if (visited == 0) visited = (int)(end - start);
   const size_t o = (size_t)iy * P.cam.W + ix;
@@ -185,6 +216,7 @@ cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* o
   P.ranges = c->ranges;
   P.vals = c->vals[c->sorted];
   P.rec = c->rec;
+  P.bbox = c->bbox;
   P.out_rgba = reinterpret_cast<float4*>(out_rgba);
   P.out_geom = reinterpret_cast<float4*>(out_geom);
   P.out_aux = reinterpret_cast<float4*>(out_aux);
@@ -194,12 +226,12 @@ cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* o
   P.px_i = c->px_i;
   P.px_visited = c->px_visited;
   P.px_contrib = c->px_contrib;
-  const dim3 grid(c->cam.TX, c->cam.TY);
+  const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsF));
   ++g_kernel_launches;
   if (depth_only)
-    blend_forward_kernel<true><<<grid, 256, 0, s>>>(P);
+    blend_forward_kernel<true><<<grid, kThreadsF, 0, s>>>(P);
   else
-    blend_forward_kernel<false><<<grid, 256, 0, s>>>(P);
+    blend_forward_kernel<false><<<grid, kThreadsF, 0, s>>>(P);
   return cudaGetLastError();
 }
 

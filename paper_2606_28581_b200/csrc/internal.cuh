@@ -36,6 +36,15 @@ __device__ __forceinline__ float fast_rcp(float x) {
   return y;
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS), and the wait for all but the n most recent commit groups
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // ---- device-side camera ------------------------------------------------------------------------------------
 struct DevCamera {
   int W, H, TX, TY;
