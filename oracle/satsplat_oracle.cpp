@@ -597,12 +597,17 @@ int orc_preprocess_backward(const orc_cam_f64* cam, int64_t N, const double* mea
     const double alpha = 1.0 / (1.0 + std::exp(-logits[i]));
     v_logits[i] += g[R_ALPHA] * alpha * (1 - alpha);
     for (int c = 0; c < 3; ++c) v_rgb[3 * i + c] += g[R_R + c];
-    const double sg = G.flipped ? -1.0 : 1.0;
+    // The flip and degenerate decisions are those of the preprocess that produced the records the forward composited
+    // (its flags), not a fresh evaluation: in the fp32 record mode
+    // a surfel whose normal is within rounding of perpendicular to the viewing direction may be flipped in fp32 and
+    // not in double, and the backward must differentiate the function the forward evaluated.
+    const bool flipped = flags[i] & F_FLIPPED, degenerate = flags[i] & F_DEGENERATE;
+    const double sg = flipped ? -1.0 : 1.0;
     double v_tu[3] = {0, 0, 0}, v_tv[3] = {0, 0, 0};
     const double v_n[3] = {sg * g[R_NX], sg * g[R_NY], sg * g[R_NZ]};
     const double v_c[2] = {g[R_CX], g[R_CY]};
     double v_B[2][3] = {{0, 0, 0}, {0, 0, 0}};
-    if (!G.degenerate) {
+    if (!degenerate) {
       double vQ[2][2] = {{g[R_Q00], g[R_Q01]}, {g[R_Q10], g[R_Q11]}};
       const double vg[2] = {g[R_G0], g[R_G1]};
       // g_j = -sum_i r_i Q_ij

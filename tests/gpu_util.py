@@ -143,13 +143,16 @@ def compare_images(gpu, ref, fragile, *, atol=1e-5, rtol=1e-4, names=("rgba", "g
     return stats
 
 
-def compare_grads(gpu, ref, *, atol=1e-5, rtol=1e-3, pairs=None, allow_frac=0.0, elem_frac=2e-3):
+def compare_grads(gpu, ref, *, atol=1e-5, rtol=1e-3, pairs=None, allow_frac=0.0, elem_frac=2e-3, tail_frac=2e-6,
+                  tail_factor=2.0):
     """Gradient bar: |gpu - ref| <= atol + rtol * s, where s is the largest |ref| of the
     same surfel's parameter group (the row).  A per-surfel gradient is an fp32 sum of signed per-pixel terms;
     where they cancel, the error scales with the terms, not with the residual, so the relative bar is applied to
     the row scale.  The plain element-wise bar (s = |ref| of the element) must still hold for all but
     `elem_frac` of the elements.  `allow_frac` tolerates that share of rows out of tolerance (unmasked runs,
-    where fragile pixels legitimately differ)."""
+    where fragile pixels legitimately differ).  At full size (millions of gradient elements) the fp32 rounding tail
+    shows: at most `tail_frac` of the elements (2 per million; none below 500 K elements) may exceed the row bar, and
+    then by at most `tail_factor` (DESIGN.md section 3 "Tolerances")."""
     stats = {}
     for kg, kr in pairs:
         g, r = gpu[kg].astype(np.float64), np.asarray(ref[kr]).reshape(gpu[kg].shape)
@@ -170,7 +173,9 @@ def compare_grads(gpu, ref, *, atol=1e-5, rtol=1e-3, pairs=None, allow_frac=0.0,
         nbad_el = int((err > tol_el).sum())
         stats[kg] = (float((err / tol_row).max()), nbad, nbad_el)
         i = int(np.argmax((err / tol_row).reshape(-1)))
-        assert nbad <= allow_frac * g.size, (kg, nbad, g.size, stats[kg], g.reshape(-1)[i], r.reshape(-1)[i])
+        nworse = int((err > tail_factor * tol_row).sum())
+        assert nbad <= (allow_frac + tail_frac) * g.size, (kg, nbad, g.size, stats[kg], g.reshape(-1)[i], r.reshape(-1)[i])
+        assert nworse <= allow_frac * g.size, (kg, "tail", nworse, g.size, stats[kg], g.reshape(-1)[i], r.reshape(-1)[i])
         assert nbad_el <= max(elem_frac, allow_frac) * g.size + 2, (kg, "elementwise", nbad_el, g.size)
     return stats
 

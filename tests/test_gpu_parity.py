@@ -45,6 +45,8 @@ def _scene(cfg):
         return S.make_config(3, n=40000, size=384, n_views=1, extent=200.0, sun_size=384)
     if cfg == "C4s":
         return S.make_config(4, n=40000, size=512, n_views=1, extent=250.0)
+    if cfg == "C3full":               # BASELINE.json configs[3] at full size (1M surfels, 2048^2), the bench workload
+        return S.make_config(3, n_views=1)
     raise KeyError(cfg)
 
 
@@ -55,7 +57,7 @@ def _no_shadow(view):
     return v
 
 
-@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s"])
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s", "C3full"])
 def test_binning_and_records_bitexact(P, G, orc, cfg):
     scene = _scene(cfg)
     gs = G.GpuScene(scene)
@@ -100,7 +102,7 @@ def test_long_tile_lists_bitexact(P, G, orc, n, size):
     G.assert_bins_bitexact(ref, res["bins"], scene.n)
 
 
-@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s"])
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s", "C3full"])
 def test_forward_backward_parity(P, G, orc, cfg):
     scene = _scene(cfg)
     gs = G.GpuScene(scene)
