@@ -169,6 +169,10 @@ void satsplat_destroy(satsplat_ctx* ctx) {
     if (p) cudaFree(p);
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  for (int i = 0; i < 2; ++i)
+    if (ctx->e2e_stream[i]) cudaStreamDestroy(ctx->e2e_stream[i]);
+  for (int i = 0; i < 4; ++i)
+    if (ctx->e2e_ev[i]) cudaEventDestroy(ctx->e2e_ev[i]);
   free(ctx);
 }
 
@@ -427,7 +431,15 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
     CU(dalloc(ctx, &ctx->e2e_up, mpx * 12));
     CU(dalloc(ctx, &ctx->e2e_out, mpx * 12));
     CU(dalloc(ctx, &ctx->e2e_grads, (size_t)ctx->max_surfels * 13 + 32));
+    for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
+    for (int i = 0; i < 4; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[i], cudaEventDisableTiming));
   }
+  // Three queues: the caller's stream carries the surfel upload and every kernel; the upstream gradients (only
+  // needed by the backward) go up on a second stream while the sun and view forward passes run, and the images come
+  // down on a third while the backward runs (PCIe is full duplex).
+  cudaStream_t s_up = ctx->e2e_stream[0], s_down = ctx->e2e_stream[1];
+  cudaEvent_t ev_start = ctx->e2e_ev[0], ev_up = ctx->e2e_ev[1], ev_fwd = ctx->e2e_ev[2], ev_img = ctx->e2e_ev[3];
+  CU(cudaEventRecord(ev_start, s));
   float* d_means = ctx->e2e_in;
   float* d_quats = d_means + 3 * (size_t)ctx->max_surfels;
   float* d_scales = d_quats + 4 * (size_t)ctx->max_surfels;
@@ -440,11 +452,13 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   CU(cudaMemcpyAsync(d_rgb, h_rgb, n * 12, cudaMemcpyHostToDevice, s));
   float* d_up[3] = {nullptr, nullptr, nullptr};
   const float* h_up[3] = {h_v_rgba, h_v_geom, h_v_aux};
+  CU(cudaStreamWaitEvent(s_up, ev_start, 0));
   for (int k = 0; k < 3; ++k)
     if (h_up[k]) {
       d_up[k] = ctx->e2e_up + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
-      CU(cudaMemcpyAsync(d_up[k], h_up[k], px * 16, cudaMemcpyHostToDevice, s));
+      CU(cudaMemcpyAsync(d_up[k], h_up[k], px * 16, cudaMemcpyHostToDevice, s_up));
     }
+  CU(cudaEventRecord(ev_up, s_up));
   float* d_out[3];
   for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
   float* g = ctx->e2e_grads;
@@ -471,6 +485,13 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   }
   if ((rc = satsplat_preprocess(ctx, cam, N, d_means, d_quats, d_scales, d_logits, d_rgb, stream))) return rc;
   if ((rc = satsplat_render_forward(ctx, &sh, d_out[0], d_out[1], d_out[2], stream))) return rc;
+  CU(cudaEventRecord(ev_fwd, s));
+  float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};
+  CU(cudaStreamWaitEvent(s_down, ev_fwd, 0));
+  for (int k = 0; k < 3; ++k)
+    if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s_down));
+  CU(cudaEventRecord(ev_img, s_down));
+  CU(cudaStreamWaitEvent(s, ev_up, 0));
   if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_means, g_quats, g_scales, g_logits, g_rgb, g_dF,
                                      g_cc, g_amb, d_vsun, nullptr, stream)))
     return rc;
@@ -478,11 +499,9 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
     // the sun camera is derived from F' (cascade, Fig. 1); its 2x4 gradient is not chained here (NEXT-2)
     if ((rc = satsplat_shadow_map_backward(sun_ctx, d_vsun, g_means, g_quats, g_scales, g_logits, nullptr, stream))) return rc;
   }
-  float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};
-  for (int k = 0; k < 3; ++k)
-    if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s));
   CU(cudaMemcpyAsync(h_grads, g, (n * 13 + 23) * sizeof(float), cudaMemcpyDeviceToHost, s));
   CU(cudaStreamSynchronize(s));
+  CU(cudaEventSynchronize(ev_img));
   return SATSPLAT_OK;
 }
 

@@ -168,6 +168,8 @@ struct satsplat_ctx {
   float* e2e_up;          // upstream grads (3 images)
   float* e2e_out;         // images
   float* e2e_grads;       // N*13 + 23
+  cudaStream_t e2e_stream[2];   // upload of the upstream gradients / download of the images, beside the caller's stream
+  cudaEvent_t e2e_ev[4];
   // profiling
   int profiling;
   cudaEvent_t ev[2 * SATSPLAT_NUM_STAGES];
