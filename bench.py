@@ -33,6 +33,10 @@ INST_CONTRIB_FWD = 25.0   # extra per contributing pair, forward (view pass; the
 INST_CONTRIB_BWD = 90.0   # extra per contributing pair, backward (view pass; sun pass: 50)
 INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN = 6.0, 50.0
 FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.965 GHz = 37.2 T lane-instr/s
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the view-pass kernels at C3, from the committed
+# `ncu --set full` capture (a profiler number is never a bench value: it only fills roofline.traffic)
+NCU_SOURCE = "profiles/r1_kernels_final.md"
+NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": None, "blend_fwd": None}
 
 
 def parse():
@@ -259,17 +263,22 @@ def timed(torch, dist, world, fn, items):
     return max_over_ranks(torch, dist, world, e0.elapsed_time(e1), "cuda")
 
 
-def stage_profile(job, vi, peaks):
-    """Per-stage device ms (CUDA events recorded by the library on the launching stream), pair counts, and the
-    algorithmic work of each kernel for view `vi`."""
+def stage_profile(job, views, peaks):
+    """Per-stage device ms (CUDA events recorded by the library on the launching stream around every kernel of a
+    stage), averaged over the launches of the bench's step views; pair counts and the algorithmic work of each kernel
+    (of the last view)."""
     torch, P = job.torch, job.P
     job.ctx.set_profiling(True)
     if job.sctx:
         job.sctx.set_profiling(True)
-    job.step(vi)
-    torch.cuda.synchronize()
-    ms_view = job.ctx.stage_ms()
-    ms_sun = job.sctx.stage_ms() if job.sctx else {}
+    ms_view, ms_sun = {}, {}
+    for vi in views:
+        job.step(vi)
+        torch.cuda.synchronize()
+        for acc, ctx in ((ms_view, job.ctx), (ms_sun, job.sctx)):
+            if ctx:
+                for k, v in ctx.stage_ms().items():
+                    acc[k] = acc.get(k, 0.0) + v / len(views)
     job.ctx.set_profiling(False)
     if job.sctx:
         job.sctx.set_profiling(False)
@@ -285,13 +294,15 @@ def stage_profile(job, vi, peaks):
     # algorithmic bytes: per surfel / per key / per pixel figures of SURVEY.md 8(d)
     work = {
         "preprocess": ("hbm", n * 137.0),
-        "scan": ("hbm", n * 12.0),
-        "duplicate": ("hbm", n * 16.0 + K * 12.0),
-        "sort": ("hbm", K * (passes * 36.0)),
-        "ranges": ("hbm", K * 8.0 + tiles * 8.0),
+        # tile-sort binning (the default mode): one-CTA scan of the tile counters, scatter of (depth, id) entries,
+        # per-tile sort; the radix option's figures are (8 + 24 P) B / pair, P = ceil((32 + log2 tiles) / 8) passes
+        "scan": ("hbm", tiles * 12.0),
+        "duplicate": ("hbm", n * 16.0 + K * 8.0),
+        "sort": ("hbm", K * 20.0),
+        "ranges": ("hbm", 0.0),
         "blend_fwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_FWD),
         "blend_bwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_BWD),
-        "chain_bwd": ("hbm", n * (64.0 * 2 + 40.0 + 52.0 * 2)),
+        "chain_bwd": ("hbm", n * (80.0 * 2 + 45.0 + 52.0 * 2)),
     }
     stages = {}
     for k, ms in ms_view.items():
@@ -343,11 +354,12 @@ def run_ours(args):
                 config=workload_config(scene, args, world), clocks=clocks, gpu_launches=int(launches),
                 fwd_ms_per_step=ms_fwd / args.steps, fwd_mpixel_s=world * px / 1e6 / (ms_fwd / args.steps * 1e-3))
     if rank == 0:
-        stages, pairs, _ = stage_profile(job, step_views[0], peaks)
+        stages, pairs, _ = stage_profile(job, step_views, peaks)
         dom = max(stages, key=lambda k: stages[k]["ms"])
         d = stages[dom]
         line["roofline"] = dict(kernel=dom, bound=d["bound"], achieved=d["achieved"], peak=d["peak"], unit=d["unit"], frac=d["frac"],
-                                traffic=None, peak_source=("derived: 148 SM x 128 FP32 lanes x 1.965 GHz (DESIGN.md section 5)" if d["bound"] == "alu"
+                                traffic=NCU_DRAM_BYTES_PER_LAUNCH.get(dom), traffic_source=NCU_SOURCE, launches_averaged=len(step_views),
+                                peak_source=("derived: 148 SM x 128 FP32 lanes x 1.965 GHz (DESIGN.md section 5)" if d["bound"] == "alu"
                                                            else peaks["source"] + " HBM copy"),
                                 kernel_ms=d["ms"])
         line["stages"] = stages

@@ -327,50 +327,67 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       widx[slot] = make_int2(c * 32 + lane, (int)id_cur);
     }
     __syncwarp();
-    for (int sv = 0; sv < nsurv; ++sv) {
-      const float4* e = wrec[sv];
-      const int2 ji = widx[sv];
-      const float4 r0 = e[0], r1 = e[1];
-      const float dx = px - r0.x, dy = py - r0.y;
-      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;
-      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);
-      const float rho = fminf(rho3, rho2);
-      const float aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
-      const float a = fminf(kAlphaMax, aG);
-      const bool active = (ji.x < last) && (rho <= kRhoCut) && (a >= kAlphaMin);
-      const unsigned hm = __ballot_sync(0xffffffffu, active);
-      if (hm == 0) continue;
-      if (active) {
-        const float4 r2 = e[2];
-        const bool lowpass = !(rho3 <= rho2);
-        const float z = lowpass ? r1.w : r1.w + (r2.x * dx + r2.y * dy);
+    // the depth-only pass evaluates two survivors per trip (independent instruction streams for the scheduler) and
+    // composites them in order; the view pass has no registers to spare for that and takes them one by one
+    struct Eval { const float4* e; int2 ji; float dx, dy, u, v, rho3, rho2, aG, a, zc; bool active; };
+    auto evaluate = [&](int sv) -> Eval {
+      Eval E;
+      E.e = wrec[sv];
+      E.ji = widx[sv];
+      const float4 r0 = E.e[0], r1 = E.e[1];
+      E.dx = px - r0.x; E.dy = py - r0.y;
+      E.u = r0.z * E.dx + r0.w * E.dy; E.v = r1.x * E.dx + r1.y * E.dy;
+      E.rho3 = E.u * E.u + E.v * E.v; E.rho2 = 2.0f * (E.dx * E.dx + E.dy * E.dy);
+      const float rho = fminf(E.rho3, E.rho2);
+      E.aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
+      E.a = fminf(kAlphaMax, E.aG);
+      E.zc = r1.w;
+      E.active = (E.ji.x < last) && (rho <= kRhoCut) && (E.a >= kAlphaMin);
+      return E;
+    };
+    auto composite = [&](const Eval& E) {
+      const unsigned hm = __ballot_sync(0xffffffffu, E.active);
+      if (hm == 0) return;
+      if (E.active) {
+        const float4 r2 = E.e[2];
+        const bool lowpass = !(E.rho3 <= E.rho2);
+        const float z = lowpass ? E.zc : E.zc + (r2.x * E.dx + r2.y * E.dy);
         const float zs = z - zref;
-        const float rc = fast_rcp(1.0f - a);
+        const float rc = fast_rcp(1.0f - E.a);
         const float Ti = T * rc;
-        const float w = a * Ti;
+        const float w = E.a * Ti;
         float phi, v_z;
         if (DEPTH_ONLY) {
           phi = vD * zs;
           v_z = w * vD;
         } else {
-          const float4 r3 = e[3];
+          const float4 r3 = E.e[3];
           const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
           phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
-          v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((ji.x == mi) ? vmed : 0.f);
+          v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((E.ji.x == mi) ? vmed : 0.f);
         }
         const float v_a = Ti * phi - (Ssum + TfvT) * rc;
         Ssum += w * phi;
         T = Ti;
-        const float v_rho = (aG < kAlphaMax) ? -0.5f * aG * v_a : 0.f;   // alpha' = alpha G unless clamped
+        const float v_rho = (E.aG < kAlphaMax) ? -0.5f * E.aG * v_a : 0.f;   // alpha' = alpha G unless clamped
         const int pos = nseg * 32 + __popc(hm & lt_mask);
         p4[pos] = make_float4(v_rho, v_z, w, __int_as_float(lane | (lowpass ? 32 : 0)));
-        p2[pos] = lowpass ? make_float2(dx, dy) : make_float2(u, v);
+        p2[pos] = lowpass ? make_float2(E.dx, E.dy) : make_float2(E.u, E.v);
       }
       const int cnt = __popc(hm);
-      if (team == nseg) { my_cnt = cnt; my_id = (uint32_t)ji.y; }
+      if (team == nseg) { my_cnt = cnt; my_id = (uint32_t)E.ji.y; }
       wmax = max(wmax, cnt);
       if (++nseg == kSegs) flush();
+    };
+    int sv = 0;
+    if (DEPTH_ONLY) {
+      for (; sv + 1 < nsurv; sv += 2) {
+        const Eval E0 = evaluate(sv), E1 = evaluate(sv + 1);
+        composite(E0);
+        composite(E1);
+      }
     }
+    for (; sv < nsurv; ++sv) composite(evaluate(sv));
     __syncwarp();
     id_cur = id_nxt; bb_cur = bb_nxt; id_nxt = id_nn;
   }
