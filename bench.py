@@ -36,7 +36,7 @@ FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.96
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the view-pass kernels at C3, from the committed
 # `ncu --set full` capture (a profiler number is never a bench value: it only fills roofline.traffic)
 NCU_SOURCE = "profiles/r1_kernels_final.md"
-NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": None, "blend_fwd": None}
+NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": 784.7e6, "blend_fwd": 529.6e6}
 
 
 def parse():
