@@ -191,6 +191,8 @@ class Job:
         self.g = dict(m=z(n, 3), q=z(n, 4), s=z(n, 2), l=z(n), c=z(n, 3), dF=z(8), cc=z(12), amb=z(3))
         self.cams, self.up = {}, {}
         self.device = device
+        # the view pass's preprocess + binning do not depend on the sun pass: they run on a second stream beside it
+        self.side = torch.cuda.Stream(device=device) if self.shadows else None
 
     def prepare_view(self, vi):
         if vi in self.cams:
@@ -214,11 +216,16 @@ class Job:
 
     def forward(self, vi):
         cam, sun_cam, _ = self.cams[vi]
+        sh = self.shading(vi)
         if self.shadows:
+            cur = self.torch.cuda.current_stream()
+            self.side.wait_stream(cur)
+            self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb, stream=self.side)
             self.sctx.preprocess(sun_cam, self.means, self.quats, self.scales, self.logits, self.rgb)
             self.sctx.shadow_map(self.sun_depth)
-        sh = self.shading(vi)
-        self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb)
+            cur.wait_stream(self.side)
+        else:
+            self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb)
         self.ctx.render_forward(sh, *self.out)
         return sh
 
