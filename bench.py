@@ -37,6 +37,9 @@ FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.96
 # `ncu --set full` capture (a profiler number is never a bench value: it only fills roofline.traffic)
 NCU_SOURCE = "profiles/r1_kernels_final.md"
 NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": 784.7e6, "blend_fwd": 529.6e6}
+# executed warp-instructions and issue-slot utilisation of the same capture (the kernels cull before they evaluate:
+# they execute fewer lane-instructions than the algorithmic count the roofline fraction is quoted on)
+NCU_EXECUTED = {"blend_bwd": dict(warp_inst=675.5e6, issue_active_pct=72.8), "blend_fwd": dict(warp_inst=324.7e6, issue_active_pct=78.3)}
 
 
 def parse():
@@ -366,6 +369,7 @@ def run_ours(args):
         d = stages[dom]
         line["roofline"] = dict(kernel=dom, bound=d["bound"], achieved=d["achieved"], peak=d["peak"], unit=d["unit"], frac=d["frac"],
                                 traffic=NCU_DRAM_BYTES_PER_LAUNCH.get(dom), traffic_source=NCU_SOURCE, launches_averaged=len(step_views),
+                                executed=NCU_EXECUTED.get(dom),
                                 peak_source=("derived: 148 SM x 128 FP32 lanes x 1.965 GHz (DESIGN.md section 5)" if d["bound"] == "alu"
                                                            else peaks["source"] + " HBM copy"),
                                 kernel_ms=d["ms"])
