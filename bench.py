@@ -191,7 +191,7 @@ class Job:
         self.out = [torch.empty(v.height, v.width, 4, device=device) for _ in range(3)]
         self.sun_depth = z(v.sun_height, v.sun_width) if self.shadows else None
         self.v_sun = z(v.sun_height, v.sun_width) if self.shadows else None
-        self.g = dict(m=z(n, 3), q=z(n, 4), s=z(n, 2), l=z(n), c=z(n, 3), dF=z(8), cc=z(12), amb=z(3))
+        self.g = dict(m=z(n, 3), q=z(n, 4), s=z(n, 2), l=z(n), c=z(n, 3), dF=z(8), cc=z(12), amb=z(3), rep=z(8), dFs=z(8))
         self.cams, self.up = {}, {}
         self.device = device
         # the view pass's preprocess + binning do not depend on the sun pass: they run on a second stream beside it
@@ -241,9 +241,12 @@ class Job:
         if self.shadows:
             self.v_sun.zero_()
         self.ctx.render_backward(sh, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"], g["cc"], g["amb"],
-                                 self.v_sun, None)
+                                 self.v_sun, g["rep"] if self.shadows else None)
         if self.shadows:
-            self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], None)
+            self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], g["dFs"])
+            # cascade (Fig. 1): the sun camera is derived from F' = F + dF
+            v = self.scene.views[vi]
+            self.P.sun_camera_backward(self.cams[vi][0], v.sun_azimuth, v.sun_elevation, v.sun_viewport, g["dFs"], g["rep"], g["dF"])
 
 
 def max_over_ranks(torch, dist, world, value, device):

@@ -92,6 +92,19 @@ int64_t satsplat_scratch_bytes(const satsplat_ctx* ctx);  /* device bytes owned 
 int satsplat_sun_camera(const satsplat_camera* view, float azimuth, float elevation, int32_t sun_w, int32_t sun_h,
                         const float viewport[4], satsplat_camera* sun_out, float reproj_out[8]);
 
+/* Cascade camera optimisation (Fig. 1 :159): the sun camera is DERIVED from the refined view camera
+ * F' = F + dF, so what reaches the sun camera's 2x4 matrix (v_dF_sun of satsplat_shadow_map_backward) and the
+ * reprojection constants (v_reproj of satsplat_render_backward) flows back into dF.  This is the adjoint of
+ * satsplat_sun_camera with respect to F': for a camera built by Eq. 16 the reprojection is
+ * x_s = diag(sc) x - sc (B' s) h + t, so only its k_h column depends on F', and
+ *   v_dF[r][c] += sc_r (v_F_sun[r][c] - s_c (v_F_sun[r][2] + v_reproj[r][2]))   c = 0,1,2   (s_2 = 1)
+ *   v_dF[r][3] += sc_r  v_F_sun[r][3].
+ * `view`, `viewport` HOST (same values as given to satsplat_sun_camera); v_F_sun, v_reproj DEVICE [8] (either may be
+ * NULL = zero); v_dF DEVICE [8], accumulated into.  One tiny kernel on `stream`, no host synchronisation.
+ * Errors: SATSPLAT_E_INVALID (NULL view / viewport / v_dF, zero elevation), SATSPLAT_E_CUDA. */
+int satsplat_sun_camera_backward(const satsplat_camera* view, float azimuth, float elevation, const float viewport[4],
+                                 const float* v_F_sun, const float* v_reproj, float* v_dF, satsplat_stream stream);
+
 /* ---- hot path ------------------------------------------------------------------------------------------ */
 /* (a1)+(a2) per-surfel preprocess and binning (PAPER.md:97-131 Eq. 6-12; :140).  Per surfel: rotation from the
  * quaternion, M = B' R S' (Eq. 8), Q = M^-1 (Eq. 10), centre c, height depth z_c (Eq. 11), depth slope, opacity,

@@ -66,7 +66,7 @@ def lib():
     if _LIB is None:
         _LIB = C.CDLL(build())
         for name in ("orc_preprocess_f32", "orc_preprocess_f64", "orc_bin", "orc_forward", "orc_backward",
-                     "orc_preprocess_backward", "orc_sun_camera", "orc_num_threads"):
+                     "orc_preprocess_backward", "orc_sun_camera", "orc_sun_camera_backward", "orc_num_threads"):
             getattr(_LIB, name).restype = C.c_int
     return _LIB
 
@@ -260,6 +260,16 @@ def sun_camera(Fp, azimuth, elevation, viewport):
                               _p(F_sun), _p(reproj))
     assert rc == 0
     return F_sun, reproj
+
+
+def sun_camera_backward(Fp, azimuth, elevation, viewport, v_F_sun, v_reproj):
+    """Adjoint of sun_camera with respect to Fp = F + dF (= the gradient that reaches dF through the cascade,
+    PAPER.md:155-176).  Returns v_Fp [8] (double)."""
+    v_Fp = np.zeros(8)
+    rc = lib().orc_sun_camera_backward(_p(_f64(Fp)), C.c_double(azimuth), C.c_double(elevation), _p(_f64(viewport)),
+                                       _p(_f64(v_F_sun)), _p(_f64(v_reproj)), _p(v_Fp))
+    assert rc == 0
+    return v_Fp
 
 
 # ------------------------------------------------------------------------------------------------

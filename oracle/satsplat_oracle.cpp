@@ -697,6 +697,68 @@ int orc_sun_camera(const double* Fp, double azimuth, double elevation, const dou
   return 0;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Adjoint of orc_sun_camera with respect to Fp = F + dF (cascade camera optimisation, Fig. 1:
+// the sun camera is derived from the refined view camera, so the gradients that reach the sun camera's 2x4 matrix
+// (sun pass) and the reprojection constants (shadow test) flow back into dF).  Written as the reverse of the steps of
+// orc_sun_camera, one by one, without using that the result simplifies.  v_Fp is accumulated into.
+// ---------------------------------------------------------------------------------------------------
+int orc_sun_camera_backward(const double* Fp, double azimuth, double elevation, const double* viewport,
+                            const double* v_F_sun, const double* v_reproj, double* v_Fp) {
+  const double s[3] = {std::cos(azimuth) / std::tan(elevation), std::sin(azimuth) / std::tan(elevation), 1.0};
+  // ---- forward values that the adjoint needs ----
+  double Bs[2][3];
+  for (int r = 0; r < 2; ++r) {
+    const double* B = Fp + 4 * r;
+    const double Bs3 = B[0] * s[0] + B[1] * s[1] + B[2] * s[2];
+    Bs[r][0] = viewport[r] * B[0]; Bs[r][1] = viewport[r] * B[1]; Bs[r][2] = viewport[r] * (B[2] - Bs3);
+  }
+  const double B2[2][2] = {{Fp[0], Fp[1]}, {Fp[4], Fp[5]}};
+  const double det = B2[0][0] * B2[1][1] - B2[0][1] * B2[1][0];
+  if (!(std::fabs(det) > 0)) return -1;
+  const double Bi[2][2] = {{B2[1][1] / det, -B2[0][1] / det}, {-B2[1][0] / det, B2[0][0] / det}};
+  double Rx[2][2];
+  for (int r = 0; r < 2; ++r) {
+    Rx[r][0] = Bs[r][0] * Bi[0][0] + Bs[r][1] * Bi[1][0];
+    Rx[r][1] = Bs[r][0] * Bi[0][1] + Bs[r][1] * Bi[1][1];
+  }
+  // ---- reverse ----
+  double vBs[2][3], vbs[2], vBi[2][2] = {{0, 0}, {0, 0}};
+  for (int r = 0; r < 2; ++r) {
+    const double* vr = v_reproj + 4 * r;
+    const double* vf = v_F_sun + 4 * r;
+    // reproj[r][2] = Bs[r][2] - (Rx0 Fp[2] + Rx1 Fp[6]);  reproj[r][3] = bs[r] - (Rx0 Fp[3] + Rx1 Fp[7])
+    const double vRx0 = vr[0] - vr[2] * Fp[2] - vr[3] * Fp[3];
+    const double vRx1 = vr[1] - vr[2] * Fp[6] - vr[3] * Fp[7];
+    v_Fp[2] += -vr[2] * Rx[r][0]; v_Fp[6] += -vr[2] * Rx[r][1];
+    v_Fp[3] += -vr[3] * Rx[r][0]; v_Fp[7] += -vr[3] * Rx[r][1];
+    // Rx0 = Bs0 Bi00 + Bs1 Bi10;  Rx1 = Bs0 Bi01 + Bs1 Bi11
+    vBs[r][0] = vf[0] + vRx0 * Bi[0][0] + vRx1 * Bi[0][1];
+    vBs[r][1] = vf[1] + vRx0 * Bi[1][0] + vRx1 * Bi[1][1];
+    vBs[r][2] = vf[2] + vr[2];
+    vbs[r] = vf[3] + vr[3];
+    vBi[0][0] += vRx0 * Bs[r][0]; vBi[1][0] += vRx0 * Bs[r][1];
+    vBi[0][1] += vRx1 * Bs[r][0]; vBi[1][1] += vRx1 * Bs[r][1];
+  }
+  // Bi = B2^-1  =>  v_B2 = -Bi^T v_Bi Bi^T
+  double tmp[2][2], vB2[2][2];
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b) tmp[a][b] = Bi[0][a] * vBi[0][b] + Bi[1][a] * vBi[1][b];
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b) vB2[a][b] = -(tmp[a][0] * Bi[b][0] + tmp[a][1] * Bi[b][1]);
+  v_Fp[0] += vB2[0][0]; v_Fp[1] += vB2[0][1]; v_Fp[4] += vB2[1][0]; v_Fp[5] += vB2[1][1];
+  // Bs[r] = sc_r (B0, B1, B2 - B.s),  bs[r] = sc_r B3 + tr_r
+  for (int r = 0; r < 2; ++r) {
+    const double sc = viewport[r];
+    const double vBs3 = -sc * vBs[r][2];                 // through the B.s term
+    v_Fp[4 * r + 0] += sc * vBs[r][0] + vBs3 * s[0];
+    v_Fp[4 * r + 1] += sc * vBs[r][1] + vBs3 * s[1];
+    v_Fp[4 * r + 2] += sc * vBs[r][2] + vBs3 * s[2];
+    v_Fp[4 * r + 3] += sc * vbs[r];
+  }
+  return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -94,6 +94,7 @@ def lib():
         vp, i64, i32, f32 = C.c_void_p, C.c_int64, C.c_int32, C.c_float
         L.satsplat_create.argtypes = [C.POINTER(vp), C.c_int, i64, i32, i32, i64]
         L.satsplat_sun_camera.argtypes = [C.POINTER(Camera), f32, f32, i32, i32, C.POINTER(f32), C.POINTER(Camera), C.POINTER(f32)]
+        L.satsplat_sun_camera_backward.argtypes = [C.POINTER(Camera), f32, f32, C.POINTER(f32), vp, vp, vp, vp]
         L.satsplat_preprocess.argtypes = [vp, C.POINTER(Camera), i64, vp, vp, vp, vp, vp, vp]
         L.satsplat_render_forward.argtypes = [vp, C.POINTER(Shading), vp, vp, vp, vp]
         L.satsplat_shadow_map.argtypes = [vp, vp, vp]
@@ -157,6 +158,16 @@ def sun_camera(view: Camera, azimuth, elevation, sun_w, sun_h, viewport):
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
     return out, list(rep)
+
+
+def sun_camera_backward(view: Camera, azimuth, elevation, viewport, v_F_sun, v_reproj, v_dF, stream=None):
+    """satsplat_sun_camera_backward: v_dF (device [8]) += adjoint of the Eq. 16 sun camera applied to the device
+    vectors v_F_sun / v_reproj (either may be None)."""
+    vp = (C.c_float * 4)(*[float(x) for x in viewport])
+    rc = lib().satsplat_sun_camera_backward(C.byref(view), float(azimuth), float(elevation), vp, _ptr(v_F_sun), _ptr(v_reproj),
+                                            _ptr(v_dF), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
 
 
 class Context:

@@ -219,6 +219,17 @@ int satsplat_sun_camera(const satsplat_camera* view, float azimuth, float elevat
   return SATSPLAT_OK;
 }
 
+int satsplat_sun_camera_backward(const satsplat_camera* view, float azimuth, float elevation, const float viewport[4],
+                                 const float* v_F_sun, const float* v_reproj, float* v_dF, satsplat_stream stream) {
+  if (!view || !viewport || !v_dF) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera_backward: NULL argument");
+  const double te = tan((double)elevation);
+  if (!(fabs(te) > 1e-12)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera_backward: elevation must be non-zero");
+  const float s0 = (float)(cos((double)azimuth) / te), s1 = (float)(sin((double)azimuth) / te);   // Eq. S2
+  cudaError_t e = launch_sun_camera_backward(viewport[0], viewport[1], s0, s1, v_F_sun, v_reproj, v_dF, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_sun_camera_backward: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
                         const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
                         satsplat_stream stream) {

@@ -203,6 +203,24 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
   return cudaGetLastError();
 }
 
+// adjoint of the Eq. 16 sun camera with respect to F' (include/satsplat.h: satsplat_sun_camera_backward)
+__global__ void sun_camera_backward_kernel(float sc0, float sc1, float s0, float s1, const float* __restrict__ v_F_sun,
+                                           const float* __restrict__ v_reproj, float* __restrict__ v_dF) {
+  const int r = threadIdx.x >> 2, c = threadIdx.x & 3;   // 8 threads: one per entry of the 2x4 matrix
+  if (r >= 2) return;
+  const float sc = r ? sc1 : sc0;
+  const float vs = v_F_sun ? v_F_sun[4 * r + c] : 0.f;
+  const float vs2 = (v_F_sun ? v_F_sun[4 * r + 2] : 0.f) + (v_reproj ? v_reproj[4 * r + 2] : 0.f);
+  const float sdir = c == 0 ? s0 : (c == 1 ? s1 : (c == 2 ? 1.0f : 0.0f));
+  v_dF[4 * r + c] += sc * (vs - sdir * vs2);
+}
+cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1, const float* v_F_sun, const float* v_reproj,
+                                       float* v_dF, cudaStream_t s) {
+  ++g_kernel_launches;
+  sun_camera_backward_kernel<<<1, 32, 0, s>>>(sc0, sc1, s0, s1, v_F_sun, v_reproj, v_dF);
+  return cudaGetLastError();
+}
+
 __global__ void add_small_kernel(float* dst, const float* src, int n) {
   if ((int)threadIdx.x < n) dst[threadIdx.x] += src[threadIdx.x];
 }

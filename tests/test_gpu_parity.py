@@ -332,3 +332,58 @@ def test_iteration_host_matches_device_path(P, G, orc):
     np.testing.assert_allclose(g[:3 * n].reshape(n, 3), tot, rtol=1e-3, atol=1e-4)   # atomics: order differs run to run
     np.testing.assert_allclose(g[13 * n:13 * n + 8], res["grads"]["v_dF"], rtol=2e-3, atol=1e-2)
     ctx.close(); sctx.close()
+
+
+def test_sun_camera_backward_matches_oracle(P, G, orc):
+    """Cascade adjoint (satsplat_sun_camera_backward): closed-form device kernel against the oracle's
+    step-by-step adjoint of Eq. 16 on random cotangents; NULL inputs; accumulation."""
+    import torch
+    rng = np.random.default_rng(11)
+    scene = S.make_config(2, n=2000, size=128, n_views=3, extent=32.0, sun_size=160)
+    for view in scene.views:
+        cam = P.Camera.from_view(view)
+        Fp = (view.F.astype(np.float32) + view.dF.astype(np.float32)).astype(np.float64).reshape(8)
+        vF, vR = rng.normal(0, 1, 8), rng.normal(0, 1, 8)
+        ref = orc.sun_camera_backward(Fp, view.sun_azimuth, view.sun_elevation, view.sun_viewport, vF, vR)
+        acc0 = rng.normal(0, 1, 8).astype(np.float32)
+        out = G.t(acc0.copy())
+        P.sun_camera_backward(cam, view.sun_azimuth, view.sun_elevation, view.sun_viewport, G.t(vF), G.t(vR), out)
+        got = out.cpu().numpy().astype(np.float64) - acc0
+        np.testing.assert_allclose(got, ref, rtol=1e-5, atol=1e-5 * np.abs(ref).max())
+        out2 = torch.zeros(8, device="cuda")
+        P.sun_camera_backward(cam, view.sun_azimuth, view.sun_elevation, view.sun_viewport, None, G.t(vR), out2)
+        ref2 = orc.sun_camera_backward(Fp, view.sun_azimuth, view.sun_elevation, view.sun_viewport, np.zeros(8), vR)
+        np.testing.assert_allclose(out2.cpu().numpy(), ref2, rtol=1e-5, atol=1e-5 * max(np.abs(ref2).max(), 1e-6))
+    with pytest.raises(P.SatsplatError):
+        P.sun_camera_backward(cam, 0.3, 0.0, view.sun_viewport, None, None, out2)
+
+
+def test_cascade_total_camera_delta_gradient(P, G, orc):
+    """Total dL/d(dF) of one iteration through the cascade (Fig. 1): view-pass v_dF + adjoint of the sun camera applied to
+    the sun pass's v_dF_sun and the shadow test's v_reproj, CUDA path against the oracle, masked on fragile pixels."""
+    scene = S.make_config(2, n=20000, size=256, n_views=2, extent=64.0, sun_size=384)
+    gs = G.GpuScene(scene)
+    nth = orc.num_threads()
+    import torch
+    for vi, view in enumerate(scene.views):
+        up = S.upstream_grads(scene.seed, vi, view.height, view.width)
+        ref = orc.view_iteration(scene, view, do_backward=False, threads=nth)
+        fragile = G.fragile_mask(ref["fwd"]["margins"])
+        upm = [u.copy() for u in up]
+        for u in upm:
+            u[fragile] = 0
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        Fp = (view.F.astype(np.float32) + view.dF.astype(np.float32)).astype(np.float64).reshape(8)
+        cas_ref = orc.sun_camera_backward(Fp, view.sun_azimuth, view.sun_elevation, view.sun_viewport,
+                                          refb["sun_grads"]["v_dF"], refb["bwd"]["v_reproj"])
+        tot_ref = refb["grads"]["v_dF"] + cas_ref
+        res = G.gpu_view_iteration(P, gs, view, sun_view=ref["sun_view"], reproj=ref["reproj"], upstream=upm, want_debug=False)
+        tot = G.t(res["grads"]["v_dF"])
+        P.sun_camera_backward(P.Camera.from_view(view), view.sun_azimuth, view.sun_elevation, view.sun_viewport,
+                              G.t(res["sun_grads"]["v_dF_sun"]), G.t(res["grads"]["v_reproj"]), tot)
+        torch.cuda.synchronize()
+        got = tot.cpu().numpy().astype(np.float64)
+        scale = np.abs(tot_ref).max()
+        assert np.abs(cas_ref).max() > 1e-3 * scale                      # the cascade term is not negligible here
+        assert np.abs(got - tot_ref).max() <= 1e-2 * scale, (got, tot_ref, cas_ref)
+        print("cascade", vi, "total", tot_ref, "err/scale", np.abs(got - tot_ref).max() / scale)

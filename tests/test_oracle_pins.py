@@ -542,3 +542,92 @@ def test_p12_identity_cases(c0, orc):
     np.testing.assert_allclose(f2["rgba"][..., :3], exp, atol=1e-14)
     for k in ("geom", "aux"):
         np.testing.assert_array_equal(f2[k], f_tile[k])
+
+
+# ------------------------------------------------------------------------------------------------ P14
+def test_p14_sun_camera_adjoint_fd_and_closed_form(orc):
+    """Cascade: the sun camera and the reprojection constants are functions of F' = F + dF.
+    (a) the adjoint of Eq. 16 + viewport against central finite differences of the forward helper;
+    (b) the mathematics fixes the result: for a sun camera built by Eq. 16 the reprojection collapses to
+        x_s = diag(sc) x - sc (B s) h + t, so the columns R_x and k_0 do not depend on F' at all and only k_h does."""
+    rng = np.random.default_rng(5)
+    for trial in range(4):
+        Fp = np.array([[2.0, 0.1, 0.3, 40.0], [-0.15, -1.9, 0.8, 70.0]]).reshape(8) + rng.normal(0, 0.1, 8)
+        az, el = rng.uniform(0, 2 * np.pi), np.radians(rng.uniform(30, 70))
+        vp = np.array([rng.uniform(0.5, 2), rng.uniform(0.5, 2), rng.normal(0, 5), rng.normal(0, 5)])
+        vF, vR = rng.normal(0, 1, 8), rng.normal(0, 1, 8)
+        g = orc.sun_camera_backward(Fp, az, el, vp, vF, vR)
+
+        def f(x):
+            Fs, rp = orc.sun_camera(x, az, el, vp)
+            return float(Fs @ vF + rp @ vR)
+        for k in range(8):
+            e = np.zeros(8); e[k] = 1e-6
+            fd = (f(Fp + e) - f(Fp - e)) / 2e-6
+            assert abs(fd - g[k]) < 1e-7 * max(1.0, np.abs(g).max()), (trial, k, fd, g[k])
+        # (b) closed form
+        Fs, rp = orc.sun_camera(Fp, az, el, vp)
+        s = np.array([np.cos(az) / np.tan(el), np.sin(az) / np.tan(el), 1.0])
+        B = Fp.reshape(2, 4)[:, :3]
+        expect = np.array([[vp[0], 0, -vp[0] * (B[0] @ s), vp[2]], [0, vp[1], -vp[1] * (B[1] @ s), vp[3]]]).reshape(8)
+        np.testing.assert_allclose(rp, expect, rtol=1e-11, atol=1e-10)
+        only_const = np.zeros(8); only_const[[0, 1, 3, 4, 5, 7]] = rng.normal(0, 1, 6)
+        np.testing.assert_allclose(orc.sun_camera_backward(Fp, az, el, vp, np.zeros(8), only_const), 0, atol=1e-9)
+
+
+def test_p14_cascade_total_dF_finite_differences(orc):
+    """The whole cascade in one objective: dF moves the view camera, the sun camera built from it (Eq. 16), the sun
+    depth map rendered with that camera, and the reprojection of the shadow test.  Total analytic gradient
+    = view-pass v_dF + sun_camera_backward(sun-pass v_dF, v_reproj), against finite differences (cut-offs off)."""
+    rng = np.random.default_rng(77)
+    n, W, H, Ws, Hs = 12, 16, 16, 24, 24
+    F, d = S.affine_camera(0.5, math.radians(20), 0.7, W, H, (4, 4, 0))
+    means = np.concatenate([rng.uniform(1.0, 7.0, (n, 2)), rng.normal(0, 1.0, (n, 1))], 1)
+    quats = rng.normal(0, 1, (n, 4)); quats[:, 0] += 3.0
+    scales, logits, rgb = rng.uniform(0.8, 2.0, (n, 2)), rng.normal(0.5, 1, n), rng.uniform(0, 1, (n, 3))
+    cc = (np.concatenate([np.eye(3), np.zeros((3, 1))], 1) + rng.normal(0, 0.1, (3, 4))).reshape(12)
+    ambient = rng.uniform(0.2, 0.5, 3)
+    az, el = 0.9, math.radians(50)
+    vp = np.array([1.3, 1.3, 4.0, 6.0])
+    view = make_view(W, H, F, view_dir=d, b_z=12.0, z_bg=16.0, bg=(0.2, 0.1, 0.3))
+    up = [rng.normal(0, 1, (H, W, 4)) for _ in range(3)]
+    up[2][..., 2:] = 0
+    order = np.argsort(-means[:, 2], kind="stable").astype(np.uint32)
+    F64 = view.F.astype(np.float64)
+    sdir = -np.array([np.cos(az) * np.cos(el), np.sin(az) * np.cos(el), np.sin(el)])
+
+    def run(dF, need_grad=False):
+        Fp = F64.reshape(8) + dF
+        F_sun, reproj = orc.sun_camera(Fp, az, el, vp)
+        sun_view = make_view(Ws, Hs, F_sun.astype(np.float32), view_dir=sdir, b_z=12.0, z_bg=16.0, bg=(0, 0, 0))
+        pre_s = orc.preprocess_f64(sun_view, means, quats, scales, logits, rgb, F=F_sun, dF=np.zeros(8))
+        fs = orc.forward(Ws, Hs, 12.0, 16.0, np.zeros(3), pre_s["rec"], pre_s["flags"], order, orc.Shading(), options=7)
+        sun_depth = fs["geom"][..., 3] + fs["aux"][..., 3] * 16.0
+        sh = orc.Shading(cc=cc, ambient=ambient, sun_depth=sun_depth, reproj=reproj, bias=0.5, slope=4.0)
+        pre = orc.preprocess_f64(view, means, quats, scales, logits, rgb, F=F64, dF=dF)
+        out = orc.forward(W, H, 12.0, 16.0, view.bg_rgb, pre["rec"], pre["flags"], order, sh, options=7)
+        loss = (out["rgba"] * up[0]).sum() + (out["geom"] * up[1]).sum() + (out["aux"] * up[2]).sum()
+        if not need_grad:
+            return loss, out
+        bw = orc.backward(W, H, 12.0, 16.0, view.bg_rgb, pre["rec"], pre["flags"], order, sh, *up, options=7)
+        g = orc.preprocess_backward(view, means, quats, scales, logits, pre["flags"], bw["v_rec"], F=F64, dF=dF)
+        v_sd = bw["v_sun_depth"]
+        vg = np.zeros((Hs, Ws, 4)); vg[..., 3] = v_sd
+        vr = np.zeros((Hs, Ws, 4)); vr[..., 3] = -16.0 * v_sd
+        bs = orc.backward(Ws, Hs, 12.0, 16.0, np.zeros(3), pre_s["rec"], pre_s["flags"], order, orc.Shading(), vr, vg, None,
+                          options=7)
+        gs = orc.preprocess_backward(sun_view, means, quats, scales, logits, pre_s["flags"], bs["v_rec"], F=F_sun,
+                                     dF=np.zeros(8))
+        total = g["v_dF"] + orc.sun_camera_backward(Fp, az, el, vp, gs["v_dF"], bw["v_reproj"])
+        return loss, out, total, g["v_dF"]
+
+    dF0 = rng.normal(0, 1e-2, 8)
+    _, out, total, direct = run(dF0, need_grad=True)
+    V = out["aux"][..., 2]
+    assert V.min() < 0.5 and V.max() > 0.8                       # the shadow test is exercised
+    assert np.abs(total - direct).max() > 1e-2 * np.abs(total).max()   # the cascade term matters in this problem
+    scale = np.abs(total).max()
+    for k in range(8):
+        e = np.zeros(8); e[k] = 1e-6 * max(1.0, abs(F64.reshape(8)[k]))
+        fd = (run(dF0 + e)[0] - run(dF0 - e)[0]) / (2 * e[k])
+        assert abs(fd - total[k]) < 2e-5 * scale, (k, fd, total[k], direct[k])
