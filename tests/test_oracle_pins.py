@@ -631,3 +631,53 @@ def test_p14_cascade_total_dF_finite_differences(orc):
         e = np.zeros(8); e[k] = 1e-6 * max(1.0, abs(F64.reshape(8)[k]))
         fd = (run(dF0 + e)[0] - run(dF0 - e)[0]) / (2 * e[k])
         assert abs(fd - total[k]) < 2e-5 * scale, (k, fd, total[k], direct[k])
+
+
+# ------------------------------------------------------------------------------------------------ P15
+def _adam_problem(seed=3, n=50):
+    rng = np.random.default_rng(seed)
+    params = dict(means=rng.normal(0, 5, (n, 3)), quats=rng.normal(0, 1, (n, 4)), scales=rng.uniform(0.2, 2.0, (n, 2)),
+                  logits=rng.normal(0, 2, n), rgb=rng.uniform(0, 1, (n, 3)))
+    lrs = dict(means=0.075, quats=0.001, scales=0.001, logits=0.05, rgb=0.0025)   # PAPER.md:349 (+ opacity: argument)
+    return rng, params, lrs
+
+
+def test_p15_adam_first_step_closed_form():
+    """t = 1 from zero state: m^ = g, v^ = g^2, so the step is lr g / (|g| + eps) whatever b1, b2 are."""
+    from oracle import adam
+    rng, params, lrs = _adam_problem()
+    grads = {k: rng.normal(0, 1, v.shape) * 10.0 ** rng.uniform(-4, 2) for k, v in params.items()}
+    state = {k: (np.zeros_like(v), np.zeros_like(v)) for k, v in params.items()}
+    new, st = adam.adam_step(params, grads, state, lrs, beta1=0.8, beta2=0.95, eps=1e-8, step=1)
+    for k in adam.GROUPS:
+        g = grads[k] * (params[k] if k == "scales" else 1.0)
+        step = lrs[k] * g / (np.abs(g) + 1e-8)
+        expect = params[k] * np.exp(-step) if k == "scales" else params[k] - step
+        np.testing.assert_allclose(new[k], expect, rtol=1e-12, atol=1e-14)
+        np.testing.assert_allclose(st[k][0], 0.2 * g, rtol=1e-12)
+        np.testing.assert_allclose(st[k][1], 0.05 * g * g, rtol=1e-12)
+    assert (new["scales"] > 0).all()
+
+
+def test_p15_adam_matches_torch_optimizer_over_several_steps():
+    """torch.optim.Adam (an independent library routine) on the same sequence of gradients; the scale group is handed to
+    torch as theta = log s with the chain-ruled gradient, which is what "stepped in log space" means."""
+    import torch
+    from oracle import adam
+    rng, params, lrs = _adam_problem(seed=8)
+    tp = {k: torch.tensor(np.log(v) if k == "scales" else v, dtype=torch.float64, requires_grad=True) for k, v in params.items()}
+    opt = torch.optim.Adam([dict(params=[tp[k]], lr=lrs[k]) for k in adam.GROUPS], betas=(0.9, 0.999), eps=1e-8)
+    state = {k: (np.zeros_like(v), np.zeros_like(v)) for k, v in params.items()}
+    cur = {k: v.copy() for k, v in params.items()}
+    for t in range(1, 8):
+        grads = {k: rng.normal(0, 1, v.shape) * (1.0 + 0.3 * t) for k, v in params.items()}
+        cur_before = cur
+        cur, state = adam.adam_step(cur, grads, state, lrs, step=t)
+        for k in adam.GROUPS:
+            g = grads[k] * (cur_before[k] if k == "scales" else 1.0)
+            tp[k].grad = torch.tensor(g, dtype=torch.float64)
+        opt.step()
+        for k in adam.GROUPS:
+            ref = tp[k].detach().numpy()
+            ref = np.exp(ref) if k == "scales" else ref
+            np.testing.assert_allclose(cur[k], ref, rtol=1e-10, atol=1e-12)
