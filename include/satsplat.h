@@ -157,6 +157,28 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
                             const float* h_v_geom, const float* h_v_aux, float* h_out_rgba, float* h_out_geom,
                             float* h_out_aux, float* h_grads, satsplat_stream stream);
 
+/* ---- optimiser step ------------------------------------------------------- */
+/* One Adam step [Kingma & Ba 2015, Alg. 1] over the five surfel groups with per-group learning rates (PAPER.md:349:
+ * 0.075 means, 0.0025 colour, 0.001 quaternions and scales; the paper names no opacity rate, no betas and no epsilon:
+ * all are arguments).  theta <- theta - lr m^/(sqrt(v^) + eps) with m^ = m/(1 - beta1^t), v^ = v/(1 - beta2^t); the
+ * scale group is stepped in log space (theta = log s, dL/dtheta = s dL/ds, s <- s exp(-step)) so that the linear
+ * scales of this library stay positive, and its state is that of log s.
+ * HOST struct.  lr[] in the order means, quats, scales, opacity logits, rgb; step = t >= 1. */
+typedef struct {
+  float lr[5];
+  float beta1, beta2, eps;
+  int32_t step;
+} satsplat_adam;
+/* Floats in each of the two state arrays for N surfels (13 N rounded so that every group starts 16-byte aligned). */
+int64_t satsplat_adam_state_floats(int64_t N);
+/* All pointers DEVICE, fp32, 16-byte aligned.  Parameters are updated in place; gradients are read only; adam_m and
+ * adam_v (satsplat_adam_state_floats(N) floats each, zero before the first step) are caller-owned state, updated in
+ * place.  One kernel on `stream`, no host synchronisation.  Errors: SATSPLAT_E_INVALID (NULL pointer, N < 0,
+ * step < 1, beta outside [0,1)), SATSPLAT_E_CUDA. */
+int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, float* opacity_logits, float* rgb,
+                       const float* v_means, const float* v_quats, const float* v_scales, const float* v_opacity_logits,
+                       const float* v_rgb, float* adam_m, float* adam_v, const satsplat_adam* hp, satsplat_stream stream);
+
 /* ---- status, test and profiling access ------------------------------------------------------------------ */
 /* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
  * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */

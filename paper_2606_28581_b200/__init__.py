@@ -48,6 +48,11 @@ class Camera(C.Structure):
         return cls.make(v.width, v.height, v.F, v.dF, v.view_dir, v.b_z, v.z_bg, v.bg_rgb)
 
 
+class Adam(C.Structure):
+    """satsplat_adam (include/satsplat.h): lr in the order means, quats, scales, opacity logits, rgb."""
+    _fields_ = [("lr", C.c_float * 5), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
+
+
 class Shading(C.Structure):
     """satsplat_shading (include/satsplat.h)."""
     _fields_ = [("cc", C.c_float * 12), ("ambient", C.c_float * 3), ("shadows_on", C.c_int32),
@@ -95,6 +100,9 @@ def lib():
         L.satsplat_create.argtypes = [C.POINTER(vp), C.c_int, i64, i32, i32, i64]
         L.satsplat_sun_camera.argtypes = [C.POINTER(Camera), f32, f32, i32, i32, C.POINTER(f32), C.POINTER(Camera), C.POINTER(f32)]
         L.satsplat_sun_camera_backward.argtypes = [C.POINTER(Camera), f32, f32, C.POINTER(f32), vp, vp, vp, vp]
+        L.satsplat_adam_state_floats.restype = C.c_int64
+        L.satsplat_adam_state_floats.argtypes = [i64]
+        L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
         L.satsplat_preprocess.argtypes = [vp, C.POINTER(Camera), i64, vp, vp, vp, vp, vp, vp]
         L.satsplat_render_forward.argtypes = [vp, C.POINTER(Shading), vp, vp, vp, vp]
         L.satsplat_shadow_map.argtypes = [vp, vp, vp]
@@ -166,6 +174,23 @@ def sun_camera_backward(view: Camera, azimuth, elevation, viewport, v_F_sun, v_r
     vp = (C.c_float * 4)(*[float(x) for x in viewport])
     rc = lib().satsplat_sun_camera_backward(C.byref(view), float(azimuth), float(elevation), vp, _ptr(v_F_sun), _ptr(v_reproj),
                                             _ptr(v_dF), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def adam_state_floats(n) -> int:
+    return int(lib().satsplat_adam_state_floats(int(n)))
+
+
+def adam_step(n, means, quats, scales, opacity_logits, rgb, v_means, v_quats, v_scales, v_opacity_logits, v_rgb, adam_m, adam_v,
+              lr, beta1=0.9, beta2=0.999, eps=1e-8, step=1, stream=None):
+    """satsplat_adam_step: one fused Adam step over the five surfel groups, in place (device tensors)."""
+    hp = Adam()
+    hp.lr[:] = [float(x) for x in lr]
+    hp.beta1, hp.beta2, hp.eps, hp.step = float(beta1), float(beta2), float(eps), int(step)
+    rc = lib().satsplat_adam_step(int(n), _ptr(means), _ptr(quats), _ptr(scales), _ptr(opacity_logits), _ptr(rgb), _ptr(v_means),
+                                  _ptr(v_quats), _ptr(v_scales), _ptr(v_opacity_logits), _ptr(v_rgb), _ptr(adam_m), _ptr(adam_v),
+                                  C.byref(hp), _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
 

@@ -230,6 +230,29 @@ int satsplat_sun_camera_backward(const satsplat_camera* view, float azimuth, flo
   return SATSPLAT_OK;
 }
 
+int64_t satsplat_adam_state_floats(int64_t N) {
+  static const int width[5] = {3, 4, 2, 1, 3};
+  int64_t t = 0;
+  for (int k = 0; k < 5; ++k) t += (N * width[k] + 3) & ~(int64_t)3;
+  return t;
+}
+
+int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, float* opacity_logits, float* rgb,
+                       const float* v_means, const float* v_quats, const float* v_scales, const float* v_opacity_logits,
+                       const float* v_rgb, float* adam_m, float* adam_v, const satsplat_adam* hp, satsplat_stream stream) {
+  if (N < 0 || !hp) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step: bad argument");
+  if (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb || !v_means || !v_quats || !v_scales ||
+                !v_opacity_logits || !v_rgb || !adam_m || !adam_v))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step: NULL pointer");
+  if (hp->step < 1 || !(hp->beta1 >= 0.f && hp->beta1 < 1.f) || !(hp->beta2 >= 0.f && hp->beta2 < 1.f))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step: step must be >= 1 and the betas in [0, 1)");
+  float* const params[5] = {means, quats, scales, opacity_logits, rgb};
+  const float* const grads[5] = {v_means, v_quats, v_scales, v_opacity_logits, v_rgb};
+  cudaError_t e = launch_adam(N, params, grads, adam_m, adam_v, hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_adam_step: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
                         const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
                         satsplat_stream stream) {

@@ -387,3 +387,46 @@ def test_cascade_total_camera_delta_gradient(P, G, orc):
         assert np.abs(cas_ref).max() > 1e-3 * scale                      # the cascade term is not negligible here
         assert np.abs(got - tot_ref).max() <= 1e-2 * scale, (got, tot_ref, cas_ref)
         print("cascade", vi, "total", tot_ref, "err/scale", np.abs(got - tot_ref).max() / scale)
+
+
+@pytest.mark.parametrize("n", [1, 5, 1023, 40001])
+def test_adam_step_matches_oracle(P, G, n):
+    """satsplat_adam_step (fp32, fused over the five groups) against the numpy float64 oracle over several steps, on
+    sizes that exercise the ragged float4 tails (group sizes 3n, 4n, 2n, n, 3n) and more than one grid pass."""
+    import torch
+    from oracle import adam
+    rng = np.random.default_rng(100 + n)
+    params = dict(means=rng.normal(0, 50, (n, 3)), quats=rng.normal(0, 1, (n, 4)), scales=rng.uniform(0.2, 2.0, (n, 2)),
+                  logits=rng.normal(0, 2, n), rgb=rng.uniform(0, 1, (n, 3)))
+    params = {k: v.astype(np.float32).astype(np.float64) for k, v in params.items()}
+    lrs = dict(means=0.075, quats=0.001, scales=0.001, logits=0.05, rgb=0.0025)
+    dp = {k: G.t(v) for k, v in params.items()}
+    ns = P.adam_state_floats(n)
+    assert ns >= 13 * n and ns % 4 == 0
+    dm, dv = torch.zeros(ns, device="cuda"), torch.zeros(ns, device="cuda")
+    state = {k: (np.zeros_like(v), np.zeros_like(v)) for k, v in params.items()}
+    cur = params
+    for t_ in range(1, 6):
+        grads = {k: (rng.normal(0, 1, v.shape) * 10.0 ** rng.uniform(-3, 1)).astype(np.float32).astype(np.float64) for k, v in params.items()}
+        cur, state = adam.adam_step(cur, grads, state, lrs, step=t_)
+        dg = {k: G.t(v) for k, v in grads.items()}
+        P.adam_step(n, dp["means"], dp["quats"], dp["scales"], dp["logits"], dp["rgb"], dg["means"], dg["quats"], dg["scales"],
+                    dg["logits"], dg["rgb"], dm, dv, [lrs[k] for k in adam.GROUPS], step=t_)
+        for k in adam.GROUPS:
+            got = dp[k].cpu().numpy().astype(np.float64)
+            # one step moves a value by at most lr; fp32 arithmetic of the step itself: 1e-5 relative to the step size
+            tol = 2e-6 * np.abs(cur[k]) + 2e-5 * lrs[k] * (np.abs(cur[k]) if k == "scales" else 1.0) * t_
+            assert (np.abs(got - cur[k]) <= tol).all(), (k, t_, np.abs(got - cur[k]).max())
+    # state layout: groups at 16-byte aligned offsets, in the order of the learning rates
+    off = 0
+    for k in adam.GROUPS:
+        sz = params[k].size
+        # m is a signed fp32 sum of five terms: absolute error ~ ulp of the largest term
+        np.testing.assert_allclose(dm[off:off + sz].cpu().numpy(), state[k][0].reshape(-1), rtol=2e-5,
+                                   atol=1e-6 * np.abs(state[k][0]).max())
+        np.testing.assert_allclose(dv[off:off + sz].cpu().numpy(), state[k][1].reshape(-1), rtol=2e-5, atol=1e-12)
+        off += (sz + 3) // 4 * 4
+    assert (dp["scales"] > 0).all()
+    with pytest.raises(P.SatsplatError):
+        P.adam_step(n, dp["means"], dp["quats"], dp["scales"], dp["logits"], dp["rgb"], dg["means"], dg["quats"], dg["scales"],
+                    dg["logits"], dg["rgb"], dm, dv, [0.1] * 5, step=0)
