@@ -681,3 +681,91 @@ def test_p15_adam_matches_torch_optimizer_over_several_steps():
             ref = tp[k].detach().numpy()
             ref = np.exp(ref) if k == "scales" else ref
             np.testing.assert_allclose(cur[k], ref, rtol=1e-10, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------ P16
+def test_p16_depth_normals_of_a_world_plane():
+    """Eq. 13 on the depth image of a tilted world plane seen by an affine camera: every interior pixel must return the
+    plane's normal.  The depth image is built independently of the backprojection formula: each pixel's parallel ray
+    (direction = null space of B) is intersected with the plane n0 . (p - q) = 0."""
+    from oracle import losses
+    W, H = 40, 32
+    F, d = S.affine_camera(0.5, math.radians(25), 0.9, W, H, (10, 8, 0))
+    Fp = np.asarray(F, np.float64).reshape(2, 4)
+    B, b = Fp[:, :3], Fp[:, 3]
+    ray = np.cross(B[0], B[1]); ray /= np.linalg.norm(ray)
+    n0 = np.array([0.15, -0.25, 1.0]); n0 /= np.linalg.norm(n0)
+    q = np.array([10.0, 8.0, 3.0])
+    b_z = 20.0
+    zv = np.zeros((H, W))
+    for j in range(H):
+        for i in range(W):
+            x = np.array([i + 0.5, j + 0.5])
+            p0 = np.linalg.lstsq(B, x - b, rcond=None)[0]          # some point on the pixel's ray
+            t = (n0 @ (q - p0)) / (n0 @ ray)
+            zv[j, i] = b_z - (p0 + t * ray)[2]
+    N, _, interior, _ = losses.depth_normals(zv, Fp, d)
+    expect = n0 if n0 @ np.asarray(d, np.float64) < 0 else -n0      # facing the sensor
+    assert np.abs(N[interior] - expect).max() < 1e-9
+    assert (N[~interior] == 0).all() and interior.sum() == (W - 2) * (H - 2)
+
+
+def test_p16_ssim_identities_and_brute_force_window():
+    from oracle import losses
+    rng = np.random.default_rng(4)
+    g = losses.gaussian_window()
+    assert abs(g.sum() - 1) < 1e-15 and np.allclose(g, g[::-1]) and len(g) == 11
+    I = rng.uniform(0, 1, (24, 30, 3))
+    m, _ = losses.ssim_map_and_grad(I, I.copy())
+    assert np.abs(m - 1).max() < 1e-12                              # identical images, borders included
+    # constant images away from the (zero-padded) border: variances vanish, SSIM = (2ab + C1)/(a^2 + b^2 + C1)
+    a, b = 0.3, 0.7
+    m, _ = losses.ssim_map_and_grad(np.full((30, 30, 3), a), np.full((30, 30, 3), b))
+    np.testing.assert_allclose(m[10:20, 10:20], (2 * a * b + losses.C1) / (a * a + b * b + losses.C1), rtol=1e-9)
+    # brute force at a few pixels: 2-D window = outer(g, g), zero outside the image
+    J = rng.uniform(0, 1, (24, 30, 3))
+    m, _ = losses.ssim_map_and_grad(I, J)
+    G2 = np.outer(g, g)
+    for (y, x) in [(0, 0), (3, 28), (12, 15), (23, 7)]:
+        def win(A):
+            acc = np.zeros(3)
+            for dy in range(-5, 6):
+                for dx in range(-5, 6):
+                    yy, xx = y + dy, x + dx
+                    if 0 <= yy < 24 and 0 <= xx < 30:
+                        acc += G2[dy + 5, dx + 5] * A[yy, xx]
+            return acc
+        mu1, mu2 = win(I), win(J)
+        s11, s22, s12 = win(I * I) - mu1 ** 2, win(J * J) - mu2 ** 2, win(I * J) - mu1 * mu2
+        ref = ((2 * mu1 * mu2 + losses.C1) * (2 * s12 + losses.C2)) / ((mu1 ** 2 + mu2 ** 2 + losses.C1) * (s11 + s22 + losses.C2))
+        np.testing.assert_allclose(m[y, x], ref, rtol=1e-10)
+
+
+def test_p16_loss_upstream_gradients_finite_differences():
+    """d(total)/d(rgba, geom, aux) against central finite differences (alpha's stop-gradient copy held fixed)."""
+    from oracle import losses
+    rng = np.random.default_rng(9)
+    W, H = 20, 18
+    F, d = S.affine_camera(0.5, math.radians(20), 0.7, W, H, (5, 4, 0))
+    rgba = rng.uniform(0.1, 0.9, (H, W, 4))
+    geom = np.concatenate([rng.normal(0, 0.5, (H, W, 3)), rng.uniform(8, 12, (H, W, 1))], -1)
+    aux = rng.uniform(0, 1, (H, W, 4))
+    target = rng.uniform(0, 1, (H, W, 3))
+    args = dict(Fp=F, view_dir=d, b_z=15.0, z_bg=14.0, w_l1=0.8, w_ssim=0.2, w_dist=0.05, w_normal=0.05)
+    A0 = rgba[..., 3].copy()
+    terms, v_rgba, v_geom, v_aux = losses.loss_and_upstream(rgba, geom, aux, target, alpha_sg=A0, **args)
+    assert 0 < terms["ssim"] < 1 and terms["l1"] > 0 and 0 < terms["normal"] < 2
+    arrs, grads = dict(rgba=rgba, geom=geom, aux=aux), dict(rgba=v_rgba, geom=v_geom, aux=v_aux)
+
+    def total(**over):
+        a = {**arrs, **over}
+        return losses.loss_and_upstream(a["rgba"], a["geom"], a["aux"], target, alpha_sg=A0, **args)[0]["total"]
+    for name in ("rgba", "geom", "aux"):
+        base, g = arrs[name], grads[name]
+        gs = np.abs(g).max()
+        for _ in range(40):
+            idx = (rng.integers(H), rng.integers(W), rng.integers(4))
+            e = np.zeros_like(base); e[idx] = 1e-6
+            fd = (total(**{name: base + e}) - total(**{name: base - e})) / 2e-6
+            assert abs(fd - g[idx]) < 1e-6 * gs + 1e-10, (name, idx, fd, g[idx])
+    assert np.abs(v_geom[..., 3]).max() > 0 and np.abs(v_rgba[..., 3]).max() > 0     # the depth path is exercised
