@@ -403,6 +403,22 @@ def run_ours(args):
         line["adam"] = dict(ms=ms_adam, bound="hbm", achieved=ab / (ms_adam * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
                             frac=ab / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_surfel=13 * 28,
                             note="fused Adam over the 13 N surfel parameters; not included in value / ms_per_step")
+    # ---- the loss stage, timed on its own on the last rendered view ----
+    if rank == 0:
+        vi = step_views[-1]
+        cam = job.cams[vi][0]
+        tgt = torch.rand(job.H, job.W, 4, device=device)
+        scr = torch.empty(P.loss_scratch_floats(job.W, job.H), device=device)
+        vv = [torch.empty(job.H, job.W, 4, device=device) for _ in range(3)]
+        sums = torch.zeros(8, device=device)
+        run_loss = lambda _: P.loss_upstream(cam, job.out[0], job.out[1], job.out[2], tgt, scr, vv[0], vv[1], vv[2], sums)
+        for _ in range(3):
+            run_loss(0)
+        ms_loss = timed(torch, None, 1, run_loss, range(20)) / 20
+        lb = px * 240.0
+        line["loss_stage"] = dict(ms=ms_loss, bound="hbm", achieved=lb / (ms_loss * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                                  frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=240,
+                                  note="L1 + SSIM + distortion + normal consistency -> upstream gradients (2 kernels); not included in value / ms_per_step")
     # ---- end to end through the C ABI with HOST buffers ----
     if not args.no_e2e:
         vi = step_views[0]

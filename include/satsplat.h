@@ -179,6 +179,29 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
                        const float* v_means, const float* v_quats, const float* v_scales, const float* v_opacity_logits,
                        const float* v_rgb, float* adam_m, float* adam_v, const satsplat_adam* hp, satsplat_stream stream);
 
+/* ---- loss stage ----------------------------------------------------------- */
+/* L = w_l1 mean|I - I*| + w_ssim (1 - mean SSIM(I, I*)) + w_dist mean(L_dist) + w_normal mean(1 - A_sg N_r . N_d)
+ * (PAPER.md:349 lists the terms and weights 0.8 / 0.2 / 0.05 / 0.05; :133-138 Eq. 13 defines N_d) and its gradients with
+ * respect to the three rendered images = the upstream gradients of satsplat_render_backward.
+ *   I = out_rgba.xyz, A = out_rgba.w, N_r = out_geom.xyz (alpha-weighted rendered normal), D = out_geom.w,
+ *   L_dist = out_aux.y; means over the H W pixels (and 3 channels for L1 / SSIM).
+ *   SSIM: 11x11 Gaussian window, sigma 1.5, zero padding, C1 = 0.01^2, C2 = 0.03^2, per channel.
+ *   N_d (Eq. 13): normal of the world point map backprojected from the background-composited depth
+ *   z_v = D + (1 - A) z_bg with F' = F + dF (height h = b_z - z_v), central differences on interior pixels, zero on
+ *   the one-pixel border, oriented towards the sensor; A_sg = alpha with stop-gradient (2DGS's normal consistency).
+ * HOST: cam, w.  DEVICE, fp32, 16-byte aligned: the three rendered images and target_rgba [H,W,4] (4th channel of
+ * the target ignored); scratch (satsplat_loss_scratch_floats(W, H) floats); v_rgba / v_geom / v_aux [H,W,4] are
+ * OVERWRITTEN with dL/d(out_rgba, out_geom, out_aux); loss_sums [8]: [0] sum |I - I*| (divide by 3 H W), [1] sum of the
+ * SSIM map (3 H W), [2] sum L_dist (H W), [3] sum (1 - A N_r.N_d) (H W), rest zero.  Two kernels on `stream`, no host
+ * synchronisation.  Errors: SATSPLAT_E_INVALID (NULL pointer, singular camera), SATSPLAT_E_CUDA. */
+typedef struct {
+  float w_l1, w_ssim, w_dist, w_normal;
+} satsplat_loss_weights;
+int64_t satsplat_loss_scratch_floats(int32_t width, int32_t height);
+int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weights* w, const float* out_rgba,
+                           const float* out_geom, const float* out_aux, const float* target_rgba, float* scratch,
+                           float* v_rgba, float* v_geom, float* v_aux, float* loss_sums, satsplat_stream stream);
+
 /* ---- status, test and profiling access ------------------------------------------------------------------ */
 /* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
  * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */

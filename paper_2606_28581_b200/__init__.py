@@ -48,6 +48,11 @@ class Camera(C.Structure):
         return cls.make(v.width, v.height, v.F, v.dF, v.view_dir, v.b_z, v.z_bg, v.bg_rgb)
 
 
+class LossWeights(C.Structure):
+    """satsplat_loss_weights (include/satsplat.h); PAPER.md:349: 0.8, 0.2, 0.05, 0.05."""
+    _fields_ = [("w_l1", C.c_float), ("w_ssim", C.c_float), ("w_dist", C.c_float), ("w_normal", C.c_float)]
+
+
 class Adam(C.Structure):
     """satsplat_adam (include/satsplat.h): lr in the order means, quats, scales, opacity logits, rgb."""
     _fields_ = [("lr", C.c_float * 5), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
@@ -100,6 +105,9 @@ def lib():
         L.satsplat_create.argtypes = [C.POINTER(vp), C.c_int, i64, i32, i32, i64]
         L.satsplat_sun_camera.argtypes = [C.POINTER(Camera), f32, f32, i32, i32, C.POINTER(f32), C.POINTER(Camera), C.POINTER(f32)]
         L.satsplat_sun_camera_backward.argtypes = [C.POINTER(Camera), f32, f32, C.POINTER(f32), vp, vp, vp, vp]
+        L.satsplat_loss_scratch_floats.restype = C.c_int64
+        L.satsplat_loss_scratch_floats.argtypes = [i32, i32]
+        L.satsplat_loss_upstream.argtypes = [C.POINTER(Camera), C.POINTER(LossWeights)] + [vp] * 10
         L.satsplat_adam_state_floats.restype = C.c_int64
         L.satsplat_adam_state_floats.argtypes = [i64]
         L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
@@ -174,6 +182,21 @@ def sun_camera_backward(view: Camera, azimuth, elevation, viewport, v_F_sun, v_r
     vp = (C.c_float * 4)(*[float(x) for x in viewport])
     rc = lib().satsplat_sun_camera_backward(C.byref(view), float(azimuth), float(elevation), vp, _ptr(v_F_sun), _ptr(v_reproj),
                                             _ptr(v_dF), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def loss_scratch_floats(width, height) -> int:
+    return int(lib().satsplat_loss_scratch_floats(int(width), int(height)))
+
+
+def loss_upstream(cam: Camera, out_rgba, out_geom, out_aux, target_rgba, scratch, v_rgba, v_geom, v_aux, loss_sums,
+                  w_l1=0.8, w_ssim=0.2, w_dist=0.05, w_normal=0.05, stream=None):
+    """satsplat_loss_upstream: fills v_rgba / v_geom / v_aux with dL/d(rendered images) and loss_sums[0:4] with the sums of
+    |I - I*|, the SSIM map, the distortion and the normal term (device tensors)."""
+    w = LossWeights(float(w_l1), float(w_ssim), float(w_dist), float(w_normal))
+    rc = lib().satsplat_loss_upstream(C.byref(cam), C.byref(w), _ptr(out_rgba), _ptr(out_geom), _ptr(out_aux), _ptr(target_rgba),
+                                      _ptr(scratch), _ptr(v_rgba), _ptr(v_geom), _ptr(v_aux), _ptr(loss_sums), _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
 

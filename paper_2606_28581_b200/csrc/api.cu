@@ -230,6 +230,41 @@ int satsplat_sun_camera_backward(const satsplat_camera* view, float azimuth, flo
   return SATSPLAT_OK;
 }
 
+int64_t satsplat_loss_scratch_floats(int32_t width, int32_t height) { return (int64_t)12 * width * height; }
+
+int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weights* w, const float* out_rgba,
+                           const float* out_geom, const float* out_aux, const float* target_rgba, float* scratch,
+                           float* v_rgba, float* v_geom, float* v_aux, float* loss_sums, satsplat_stream stream) {
+  if (!cam || !w || !out_rgba || !out_geom || !out_aux || !target_rgba || !scratch || !v_rgba || !v_geom || !v_aux || !loss_sums)
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_loss_upstream: NULL argument");
+  if (cam->width <= 0 || cam->height <= 0) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_loss_upstream: bad image size");
+  // Eq. 13 constants: p_s = (B2^-1 (x - b - B3 h), h), h = b_z - z_v, is affine in z_v, so with the central differences
+  // dx, dy of z_v:  grad_x p x grad_y p = c0 + dx c1 + dy c2
+  double Fp[8];
+  for (int i = 0; i < 8; ++i) Fp[i] = (double)(float)(cam->F[i] + cam->dF[i]);
+  const double det = Fp[0] * Fp[5] - Fp[1] * Fp[4];
+  if (!(fabs(det) > 0)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_loss_upstream: singular camera");
+  const double Bi[2][2] = {{Fp[5] / det, -Fp[1] / det}, {-Fp[4] / det, Fp[0] / det}};
+  const double k[3] = {Bi[0][0] * Fp[2] + Bi[0][1] * Fp[6], Bi[1][0] * Fp[2] + Bi[1][1] * Fp[6], -1.0};
+  const double ax[3] = {2.0 * Bi[0][0], 2.0 * Bi[1][0], 0.0}, ay[3] = {2.0 * Bi[0][1], 2.0 * Bi[1][1], 0.0};
+  auto cross = [](const double* a, const double* b, double* c) {
+    c[0] = a[1] * b[2] - a[2] * b[1]; c[1] = a[2] * b[0] - a[0] * b[2]; c[2] = a[0] * b[1] - a[1] * b[0];
+  };
+  double c0[3], c1[3], c2[3];
+  cross(ax, ay, c0); cross(k, ay, c1); cross(ax, k, c2);
+  LossHost L;
+  L.W = cam->width; L.H = cam->height;
+  L.w_l1 = w->w_l1; L.w_ssim = w->w_ssim; L.w_dist = w->w_dist; L.w_normal = w->w_normal;
+  for (int i = 0; i < 3; ++i) { L.c0[i] = (float)c0[i]; L.c1[i] = (float)c1[i]; L.c2[i] = (float)c2[i]; }
+  L.sgn = (c0[0] * cam->view_dir[0] + c0[1] * cam->view_dir[1] + c0[2] * cam->view_dir[2]) > 0 ? -1.f : 1.f;
+  L.z_bg = cam->z_bg;
+  L.rgba = out_rgba; L.geom = out_geom; L.aux = out_aux; L.target = target_rgba;
+  L.scratch = scratch; L.v_rgba = v_rgba; L.v_geom = v_geom; L.v_aux = v_aux; L.sums = loss_sums;
+  cudaError_t e = launch_losses(L, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_loss_upstream: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 int64_t satsplat_adam_state_floats(int64_t N) {
   static const int width[5] = {3, 4, 2, 1, 3};
   int64_t t = 0;

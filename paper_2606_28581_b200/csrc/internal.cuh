@@ -200,6 +200,14 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
                                   const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
                                   float* v_rgb, float* v_dF, cudaStream_t s);
 cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s);
+struct LossHost {   // arguments of the loss stage (losses.cu)
+  int W, H;
+  float w_l1, w_ssim, w_dist, w_normal;
+  float c0[3], c1[3], c2[3], sgn, z_bg;
+  const float *rgba, *geom, *aux, *target;
+  float *scratch, *v_rgba, *v_geom, *v_aux, *sums;
+};
+cudaError_t launch_losses(const LossHost& L, cudaStream_t s);
 cudaError_t launch_adam(int64_t N, float* const params[5], const float* const grads[5], float* m, float* v, const float lrs[5],
                         float beta1, float beta2, float eps, int step, cudaStream_t s);
 cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1, const float* v_F_sun, const float* v_reproj,

@@ -430,3 +430,46 @@ def test_adam_step_matches_oracle(P, G, n):
     with pytest.raises(P.SatsplatError):
         P.adam_step(n, dp["means"], dp["quats"], dp["scales"], dp["logits"], dp["rgb"], dg["means"], dg["quats"], dg["scales"],
                     dg["logits"], dg["rgb"], dm, dv, [0.1] * 5, step=0)
+
+
+@pytest.mark.parametrize("cfg", ["C0_ragged", "C1s"])
+def test_loss_stage_matches_oracle(P, G, orc, cfg):
+    """satsplat_loss_upstream on REAL rendered images (CUDA forward) against the numpy float64 oracle fed the same fp32
+    images: loss terms and the three upstream gradient images; ragged image sizes included (77 x 100)."""
+    import torch
+    from oracle import losses
+    scene = _scene(cfg)
+    gs = G.GpuScene(scene)
+    view = _no_shadow(scene.views[0])
+    res = G.gpu_view_iteration(P, gs, view, do_backward=False, want_debug=False)
+    H, W = view.height, view.width
+    rng = np.random.default_rng(5)
+    # target: the render itself, shifted and perturbed (a plausible "ground truth" with structure)
+    target = np.clip(np.roll(res["rgba"][..., :3], 2, axis=1) + rng.normal(0, 0.05, (H, W, 3)), 0, 1).astype(np.float32)
+    t4 = np.concatenate([target, np.zeros((H, W, 1), np.float32)], -1)
+    cam = P.Camera.from_view(view)
+    Fp = (view.F.astype(np.float32) + view.dF.astype(np.float32)).astype(np.float64)
+    terms, r_rgba, r_geom, r_aux = losses.loss_and_upstream(res["rgba"], res["geom"], res["aux"], target, Fp, view.view_dir,
+                                                            view.b_z, view.z_bg)
+    d = [G.t(res[k]) for k in ("rgba", "geom", "aux")]
+    scratch = torch.empty(P.loss_scratch_floats(W, H), device="cuda")
+    v = [torch.full((H, W, 4), float("nan"), device="cuda") for _ in range(3)]
+    sums = torch.full((8,), float("nan"), device="cuda")
+    P.loss_upstream(cam, d[0], d[1], d[2], G.t(t4), scratch, v[0], v[1], v[2], sums)
+    torch.cuda.synchronize()
+    s = sums.cpu().numpy().astype(np.float64)
+    npx = H * W
+    got = dict(l1=s[0] / (3 * npx), ssim=s[1] / (3 * npx), distortion=s[2] / npx, normal=s[3] / npx)
+    for k, gv in got.items():
+        assert abs(gv - terms[k]) <= 2e-5 * max(abs(terms[k]), 1e-3), (k, gv, terms[k])
+    assert (s[4:] == 0).all()
+    for name, gpu, ref in (("v_rgba", v[0], r_rgba), ("v_geom", v[1], r_geom), ("v_aux", v[2], r_aux)):
+        g = gpu.cpu().numpy().astype(np.float64)
+        assert np.isfinite(g).all(), name
+        for ch in range(4):
+            scale = np.abs(ref[..., ch]).max()
+            err = np.abs(g[..., ch] - ref[..., ch]).max()
+            # fp32 stencil arithmetic: SSIM variances are differences of blurred moments (cancellation ~1e-7 / C2)
+            assert err <= 2e-4 * scale + 1e-12, (name, ch, err, scale)
+    assert np.abs(r_geom[..., 3]).max() > 0 and terms["ssim"] < 0.99
+    print(cfg, terms)
