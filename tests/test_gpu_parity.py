@@ -473,3 +473,43 @@ def test_loss_stage_matches_oracle(P, G, orc, cfg):
             assert err <= 2e-4 * scale + 1e-12, (name, ch, err, scale)
     assert np.abs(r_geom[..., 3]).max() > 0 and terms["ssim"] < 0.99
     print(cfg, terms)
+
+
+def test_optimisation_steps_reduce_the_loss(P, G):
+    """The pieces as one training loop (forward -> loss stage -> backward -> Adam), all through the C ABI: starting from a
+    perturbed copy of the C0 scene, 30 steps towards the image rendered from the unperturbed scene must cut the loss."""
+    import torch
+    scene = S.make_config(0)
+    view = _no_shadow(scene.views[0])
+    H, W, n = view.height, view.width, scene.n
+    cam = P.Camera.from_view(view)
+    ctx = P.Context(n, W, H, 16 * n)
+    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, depth_bias=view.depth_bias, slope=view.slope)
+    gs = G.GpuScene(scene)
+    out = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    ctx.preprocess(cam, gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+    ctx.render_forward(sh, *out)
+    target = out[0].clone()
+    rng = np.random.default_rng(0)
+    p = [G.t(scene.means + rng.normal(0, 0.05, scene.means.shape)), gs.quats.clone(), G.t(scene.scales * rng.uniform(0.8, 1.25, scene.scales.shape)),
+         gs.logits.clone(), G.t(np.clip(scene.rgb + rng.normal(0, 0.15, scene.rgb.shape), 0, 1))]
+    ns = P.adam_state_floats(n)
+    am, av = torch.zeros(ns, device="cuda"), torch.zeros(ns, device="cuda")
+    scratch = torch.empty(P.loss_scratch_floats(W, H), device="cuda")
+    v = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    sums = torch.zeros(8, device="cuda")
+    lr = [0.01, 0.001, 0.005, 0.02, 0.01]
+    hist = []
+    for step in range(1, 31):
+        ctx.preprocess(cam, *p)
+        ctx.render_forward(sh, *out)
+        P.loss_upstream(cam, out[0], out[1], out[2], target, scratch, v[0], v[1], v[2], sums, w_dist=0.0, w_normal=0.0)
+        g = [torch.zeros_like(t_) for t_ in p]
+        ctx.render_backward(sh, v[0], v[1], v[2], *g)
+        s = sums.cpu().numpy()
+        hist.append(0.8 * s[0] / (3 * H * W) + 0.2 * (1 - s[1] / (3 * H * W)))
+        P.adam_step(n, *p, *g, am, av, lr, step=step)
+    ctx.close()
+    assert np.isfinite(hist).all()
+    assert hist[-1] < 0.6 * hist[0], hist
+    assert (p[2] > 0).all()
