@@ -53,6 +53,7 @@ def parse():
     ap.add_argument("--size", type=int, default=None, help="override view size (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-graphs", action="store_true", help="launch every kernel of a step from the host instead of replaying one CUDA graph per view")
     return ap.parse_args()
 
 
@@ -165,7 +166,7 @@ def run_reference(args):
 def workload_config(scene, args, world):
     v = scene.views[0]
     return dict(workload=f"C{args.config} benchmark-shaped site (BASELINE.json configs[{args.config}])", surfels=scene.n,
-                view=f"{v.width}x{v.height}", sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
+                view=f"{v.width}x{v.height}", cuda_graphs=not getattr(args, "no_graphs", False), sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
                 views=len(scene.views), shadows=bool(v.shadows_on), parallelism=f"views sharded over {world} rank(s), no collective",
                 l2="per-step working set (records, keys, per-pixel state, images: >0.8 GB) exceeds the 126 MB L2; views cycle")
 
@@ -354,8 +355,25 @@ def run_ours(args):
     launches0 = P.kernel_launches()
     sampler = ClockSampler(local)
     sampler.start()
-    ms_total = timed(torch, dist, world, job.step, step_views)
-    launches = P.kernel_launches() - launches0
+    run_step = job.step
+    launches_per_step = None
+    if not args.no_graphs:
+        # one CUDA graph per view (the camera is baked into the kernel arguments): a step is one graph launch
+        graphs = {}
+        for vi in sorted(set(step_views)):
+            l0 = P.kernel_launches()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                job.step(vi)
+            graphs[vi] = g
+            launches_per_step = P.kernel_launches() - l0
+        for vi in step_views[:3]:
+            graphs[vi].replay()
+        torch.cuda.synchronize()
+        run_step = lambda vi: graphs[vi].replay()
+        launches0 = P.kernel_launches()
+    ms_total = timed(torch, dist, world, run_step, step_views)
+    launches = P.kernel_launches() - launches0 if launches_per_step is None else launches_per_step * len(step_views)
     clocks = sampler.stop()
     ms_fwd = timed(torch, dist, world, job.forward, step_views)
     px = job.W * job.H
