@@ -660,10 +660,10 @@ cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s) {
 
 cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_done[64] = {};   // per device: the dynamic shared-memory limit is a per-device function attribute
+  if (!attr_done[c->device & 63]) {
     cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
-    attr_set = true;
+    attr_done[c->device & 63] = true;
   }
   g_kernel_launches += 3;
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(

@@ -418,11 +418,11 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   if (want_red) cudaMemsetAsync(c->red_buf, 0, 32 * sizeof(float), s);
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));
   constexpr int kPairBytes = kWarpsB * kSegs * 32 * (int)(sizeof(float4) + sizeof(float2));
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_done[64] = {};   // per device: the dynamic shared-memory limit is a per-device function attribute
+  if (!attr_done[c->device & 63]) {
     cudaFuncSetAttribute(blend_backward_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
     cudaFuncSetAttribute(blend_backward_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
-    attr_set = true;
+    attr_done[c->device & 63] = true;
   }
   ++g_kernel_launches;
   if (depth_only)

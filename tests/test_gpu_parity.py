@@ -513,3 +513,37 @@ def test_optimisation_steps_reduce_the_loss(P, G):
     assert np.isfinite(hist).all()
     assert hist[-1] < 0.6 * hist[0], hist
     assert (p[2] > 0).all()
+
+
+@pytest.mark.parametrize("hw", [(1, 1), (2, 5), (3, 3), (17, 33)])
+def test_loss_stage_tiny_and_ragged_images(P, G, hw):
+    """Degenerate image sizes: no interior pixel for Eq. 13 (H or W < 3), windows larger than the image, ragged tiles.
+    Synthetic image contents (the loss stage does not care where its inputs come from)."""
+    import torch
+    from oracle import losses
+    H, W = hw
+    rng = np.random.default_rng(H * 100 + W)
+    F, d = S.affine_camera(0.5, math.radians(15), 0.4, max(W, 4), max(H, 4), (2, 2, 0))
+    cam = P.Camera.make(W, H, np.asarray(F).reshape(-1), np.zeros(8, np.float32), d, 15.0, 14.0, (0, 0, 0))
+    rgba = rng.uniform(0.05, 0.95, (H, W, 4)).astype(np.float32)
+    geom = np.concatenate([rng.normal(0, 0.5, (H, W, 3)), rng.uniform(8, 12, (H, W, 1))], -1).astype(np.float32)
+    aux = rng.uniform(0, 1, (H, W, 4)).astype(np.float32)
+    target = rng.uniform(0, 1, (H, W, 3)).astype(np.float32)
+    t4 = np.concatenate([target, np.zeros((H, W, 1), np.float32)], -1)
+    terms, r_rgba, r_geom, r_aux = losses.loss_and_upstream(rgba, geom, aux, target, np.asarray(F, np.float32).astype(np.float64), d, 15.0, 14.0)
+    scratch = torch.empty(max(P.loss_scratch_floats(W, H), 4), device="cuda")
+    v = [torch.full((H, W, 4), float("nan"), device="cuda") for _ in range(3)]
+    sums = torch.zeros(8, device="cuda")
+    P.loss_upstream(cam, G.t(rgba), G.t(geom), G.t(aux), G.t(t4), scratch, v[0], v[1], v[2], sums)
+    s = sums.cpu().numpy().astype(np.float64)
+    npx = H * W
+    got = dict(l1=s[0] / (3 * npx), ssim=s[1] / (3 * npx), distortion=s[2] / npx, normal=s[3] / npx)
+    for k, gv in got.items():
+        assert abs(gv - terms[k]) <= 1e-5 * max(abs(terms[k]), 1e-2), (k, gv, terms[k])
+    for gpu, ref in ((v[0], r_rgba), (v[1], r_geom), (v[2], r_aux)):
+        g = gpu.cpu().numpy().astype(np.float64)
+        assert np.isfinite(g).all()
+        assert np.abs(g - ref).max() <= 2e-4 * max(np.abs(ref).max(), 1e-12) + 1e-12
+    if H < 3 or W < 3:
+        assert abs(terms["normal"] - 1.0) < 1e-12 and np.abs(r_geom).max() == 0    # no interior pixel: N_d = 0 everywhere
+
