@@ -769,3 +769,64 @@ def test_p16_loss_upstream_gradients_finite_differences():
             fd = (total(**{name: base + e}) - total(**{name: base - e})) / 2e-6
             assert abs(fd - g[idx]) < 1e-6 * gs + 1e-10, (name, idx, fd, g[idx])
     assert np.abs(v_geom[..., 3]).max() > 0 and np.abs(v_rgba[..., 3]).max() > 0     # the depth path is exercised
+
+
+# ------------------------------------------------------------------------------------------------ P17
+def test_p17_area_weights_plane_and_inverse_cdf():
+    """a = |dx x dy|.  A tilted plane has the same weight cell^2 sqrt(1 + a^2 + b^2) in every cell (finite
+    differences are exact for planes, one-sided ones included); the inverse transform on a hand-made weight row."""
+    from oracle import init
+    cell = 0.5
+    yy, xx = np.meshgrid(np.arange(7) + 0.5, np.arange(9) + 0.5, indexing="ij")
+    h = 0.8 * xx * cell - 1.7 * yy * cell + 3.0
+    np.testing.assert_allclose(init.area_weights(h, cell), cell * cell * math.sqrt(1 + 0.8 ** 2 + 1.7 ** 2), rtol=1e-12)
+    w = np.array([[1.0, 3.0], [2.0, 2.0]])            # cumulative 1, 4, 6, 8
+    got = init.sample_cells(w, np.array([0.0, 0.124, 0.125, 0.49, 0.5, 0.74, 0.75, 0.999999]))
+    assert got.tolist() == [0, 0, 1, 1, 2, 2, 3, 3]
+
+
+def test_p17_facades_receive_their_share_of_samples():
+    """A box building on flat ground: the cells on the wall ring carry the extra area |dh| * cell per unit length, and the
+    sampled fraction follows the weights (PAPER.md:186 'building facades ... more likely to be selected')."""
+    from oracle import init
+    rng = np.random.default_rng(2)
+    cell, n = 0.5, 200000
+    h = np.zeros((60, 60)); h[20:40, 20:40] = 12.0
+    w = init.area_weights(h, cell)
+    wall = w > 1.5 * cell * cell
+    assert wall.sum() > 0                                         # a two-cell-wide ring (central differences)
+    out = init.init_from_dsm(h, cell, (0.0, 0.0), rng.uniform(0, 1, n), rng.uniform(0, 1, n), rng.uniform(0, 1, n))
+    frac = wall.ravel()[out["cells"]].mean()
+    expect = w[wall].sum() / w.sum()
+    assert abs(frac - expect) < 4 * math.sqrt(expect * (1 - expect) / n)
+    assert expect > 5 * wall.mean()                                # far more than their share of the footprint
+
+
+def test_p17_frames_quaternions_and_knn_scale():
+    from oracle import init
+    from scipy.spatial.transform import Rotation
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        hx, hy = rng.normal(0, 3, 2)
+        R = init.frame(hx, hy)
+        np.testing.assert_allclose(R.T @ R, np.eye(3), atol=1e-12)
+        assert abs(np.linalg.det(R) - 1) < 1e-12
+        n = np.array([-hx, -hy, 1.0]); n /= np.linalg.norm(n)
+        np.testing.assert_allclose(R[:, 2], n, atol=1e-12)
+        # t_u is the world x axis made orthogonal to n: in the plane of (e_x, n), on e_x's side
+        assert abs(R[:, 0] @ np.cross(n, [1.0, 0, 0])) < 1e-12 and R[0, 0] > 0
+        q = init.rotation_to_quat(R)
+        assert q[0] >= 0 and abs(np.linalg.norm(q) - 1) < 1e-12
+        np.testing.assert_allclose(Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix(), R, atol=1e-12)
+    # kNN scale against brute force
+    h = rng.normal(0, 1, (30, 30)).cumsum(0).cumsum(1) * 0.05
+    n = 300
+    out = init.init_from_dsm(h, 0.5, (10.0, -5.0), rng.uniform(0, 1, n), rng.uniform(0, 1, n), rng.uniform(0, 1, n))
+    P_ = out["means"]
+    D = np.linalg.norm(P_[:, None, :] - P_[None, :, :], axis=-1)
+    D.sort(axis=1)
+    np.testing.assert_allclose(out["scales"][:, 0], D[:, 1:4].mean(1), rtol=1e-12)
+    assert (out["scales"][:, 0] == out["scales"][:, 1]).all()
+    # centres lie on their cell's tangent plane and inside the cell
+    col = np.floor((P_[:, 0] - 10.0) / 0.5).astype(int); row = np.floor((P_[:, 1] + 5.0) / 0.5).astype(int)
+    assert (row * 30 + col == out["cells"]).all()
