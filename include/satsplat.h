@@ -202,6 +202,25 @@ int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weigh
                            const float* out_geom, const float* out_aux, const float* target_rgba, float* scratch,
                            float* v_rgba, float* v_geom, float* v_aux, float* loss_sums, satsplat_stream stream);
 
+/* ---- geometry-aware initialisation ----------------------------------------- */
+/* Surfels from a DSM.  dsm[row, col] heights on a regular grid of spacing `cell`; the centre of
+ * cell (row, col) is at (origin_x + (col + 0.5) cell, origin_y + (row + 0.5) cell).
+ *   area-weighted sampling (:186): weight a = |dx x dy| = cell^2 sqrt(1 + h_x^2 + h_y^2) with finite-difference slopes
+ *     (central inside, one-sided on the border); sample k takes the first cell, in row-major order, whose cumulative
+ *     weight exceeds u[k] * total (cumulative sum in double precision); its centre is
+ *     (origin + (col + jx[k], row + jy[k]) cell, h + h_x (jx - 0.5) cell + h_y (jy - 0.5) cell) (tangent-plane lift);
+ *     u, jx, jy in [0, 1) are the CALLER's random numbers;
+ *   orientation (:192): n = (-h_x, -h_y, 1)/|.|, t_u = world x axis made orthogonal to n (Gram-Schmidt), t_v = n x t_u,
+ *     quaternion (w, x, y, z) of R = [t_u | t_v | n], w >= 0;
+ *   scale (:194): s_u = s_v = mean distance to the 3 nearest other sampled centres (exact kNN); `cell` if N <= 3.
+ * All pointers DEVICE: dsm [dsm_h, dsm_w], u / jx / jy [N], scratch (satsplat_init_scratch_bytes bytes, 16-byte aligned),
+ * outputs means [N,3], quats [N,4], scales [N,2] fp32 and, if not NULL, cells_out [N] int32 (the sampled row-major cell
+ * index).  Nine kernels on `stream`, no host synchronisation.  Errors: SATSPLAT_E_INVALID, SATSPLAT_E_CUDA. */
+int64_t satsplat_init_scratch_bytes(int32_t dsm_w, int32_t dsm_h, int64_t N);
+int satsplat_init_from_dsm(const float* dsm, int32_t dsm_w, int32_t dsm_h, float cell, float origin_x, float origin_y, int64_t N,
+                           const float* u, const float* jx, const float* jy, void* scratch, float* means, float* quats,
+                           float* scales, int32_t* cells_out, satsplat_stream stream);
+
 /* ---- status, test and profiling access ------------------------------------------------------------------ */
 /* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
  * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */

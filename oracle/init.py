@@ -24,8 +24,16 @@ import numpy as np
 def slopes(dsm, cell):
     """h_x (along columns) and h_y (along rows): central differences inside, one-sided on the border."""
     h = np.asarray(dsm, np.float64)
-    hy, hx = np.gradient(h, cell)          # np.gradient: central interior, first-order one-sided at the edges
-    return hx, hy
+
+    def diff(a, axis):
+        a = np.moveaxis(a, axis, 0)
+        d = np.zeros_like(a)
+        if a.shape[0] > 1:                  # an axis of length 1 has no neighbour: slope 0
+            d[1:-1] = (a[2:] - a[:-2]) / (2.0 * cell)
+            d[0] = (a[1] - a[0]) / cell
+            d[-1] = (a[-1] - a[-2]) / cell
+        return np.moveaxis(d, 0, axis)
+    return diff(h, 1), diff(h, 0)
 
 
 def area_weights(dsm, cell):

@@ -108,6 +108,9 @@ def lib():
         L.satsplat_loss_scratch_floats.restype = C.c_int64
         L.satsplat_loss_scratch_floats.argtypes = [i32, i32]
         L.satsplat_loss_upstream.argtypes = [C.POINTER(Camera), C.POINTER(LossWeights)] + [vp] * 10
+        L.satsplat_init_scratch_bytes.restype = C.c_int64
+        L.satsplat_init_scratch_bytes.argtypes = [i32, i32, i64]
+        L.satsplat_init_from_dsm.argtypes = [vp, i32, i32, f32, f32, f32, i64] + [vp] * 9
         L.satsplat_adam_state_floats.restype = C.c_int64
         L.satsplat_adam_state_floats.argtypes = [i64]
         L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
@@ -199,6 +202,24 @@ def loss_upstream(cam: Camera, out_rgba, out_geom, out_aux, target_rgba, scratch
                                       _ptr(scratch), _ptr(v_rgba), _ptr(v_geom), _ptr(v_aux), _ptr(loss_sums), _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def init_from_dsm(dsm, cell, origin, u, jx, jy, want_cells=False, stream=None):
+    """satsplat_init_from_dsm: dsm [H,W] and the random numbers u, jx, jy [N] are device tensors; returns device tensors
+    (means [N,3], quats [N,4], scales [N,2][, cells [N] int32])."""
+    _check(dsm, torch.float32, 2)
+    H, W = dsm.shape
+    n = int(u.numel())
+    dev = dsm.device
+    scratch = torch.empty(max(int(lib().satsplat_init_scratch_bytes(W, H, n)), 16), dtype=torch.uint8, device=dev)
+    means, quats, scales = (torch.empty(n, k, device=dev) for k in (3, 4, 2))
+    cells = torch.empty(n, dtype=torch.int32, device=dev) if want_cells else None
+    rc = lib().satsplat_init_from_dsm(dsm.data_ptr(), W, H, float(cell), float(origin[0]), float(origin[1]), n, _ptr(u), _ptr(jx),
+                                      _ptr(jy), scratch.data_ptr(), means.data_ptr(), quats.data_ptr(), scales.data_ptr(),
+                                      None if cells is None else cells.data_ptr(), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+    return (means, quats, scales, cells) if want_cells else (means, quats, scales)
 
 
 def adam_state_floats(n) -> int:

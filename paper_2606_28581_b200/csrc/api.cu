@@ -265,6 +265,23 @@ int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weigh
   return SATSPLAT_OK;
 }
 
+int64_t satsplat_init_scratch_bytes(int32_t dsm_w, int32_t dsm_h, int64_t N) {
+  if (dsm_w <= 0 || dsm_h <= 0 || N < 0) return 0;
+  return init_scratch_bytes(dsm_w, dsm_h, N);
+}
+
+int satsplat_init_from_dsm(const float* dsm, int32_t dsm_w, int32_t dsm_h, float cell, float origin_x, float origin_y, int64_t N,
+                           const float* u, const float* jx, const float* jy, void* scratch, float* means, float* quats,
+                           float* scales, int32_t* cells_out, satsplat_stream stream) {
+  if (!dsm || dsm_w <= 0 || dsm_h <= 0 || !(cell > 0.f) || N < 0) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_init_from_dsm: bad argument");
+  if (N > 0 && (!u || !jx || !jy || !scratch || !means || !quats || !scales))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_init_from_dsm: NULL pointer");
+  cudaError_t e = launch_init_from_dsm(dsm, dsm_w, dsm_h, cell, origin_x, origin_y, N, u, jx, jy, scratch, means, quats, scales,
+                                       cells_out, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_init_from_dsm: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 int64_t satsplat_adam_state_floats(int64_t N) {
   static const int width[5] = {3, 4, 2, 1, 3};
   int64_t t = 0;

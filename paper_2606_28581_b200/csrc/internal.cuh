@@ -208,6 +208,10 @@ struct LossHost {   // arguments of the loss stage (losses.cu)
   float *scratch, *v_rgba, *v_geom, *v_aux, *sums;
 };
 cudaError_t launch_losses(const LossHost& L, cudaStream_t s);
+int64_t init_scratch_bytes(int W, int H, int64_t N);
+cudaError_t launch_init_from_dsm(const float* dsm, int W, int H, float cell, float ox, float oy, int64_t N, const float* u,
+                                 const float* jx, const float* jy, void* scratch, float* means, float* quats, float* scales,
+                                 int32_t* cells_out, cudaStream_t s);
 cudaError_t launch_adam(int64_t N, float* const params[5], const float* const grads[5], float* m, float* v, const float lrs[5],
                         float beta1, float beta2, float eps, int step, cudaStream_t s);
 cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1, const float* v_F_sun, const float* v_reproj,
