@@ -830,3 +830,64 @@ def test_p17_frames_quaternions_and_knn_scale():
     # centres lie on their cell's tangent plane and inside the cell
     col = np.floor((P_[:, 0] - 10.0) / 0.5).astype(int); row = np.floor((P_[:, 1] + 5.0) / 0.5).astype(int)
     assert (row * 30 + col == out["cells"]).all()
+
+
+# ------------------------------------------------------------------------------------------------ P18
+def test_p18_relocation_factors_preserve_centre_opacity_and_profile_integral():
+    """The two things the 3DGS-MCMC relocation [22] is built to preserve, checked without its formula: N copies of
+    opacity o' composited at the centre give the old opacity, and the composited 1-D profile through the centre keeps its
+    integral (numerical quadrature of 1 - (1 - o' g_{s'}(x))^N against alpha s sqrt(2 pi))."""
+    from oracle import relocate
+    assert relocate.relocation_factors(0.37, 1) == (pytest.approx(0.37, rel=1e-15), pytest.approx(1.0, rel=1e-14))
+    x = np.linspace(-60, 60, 2_400_001)
+    for alpha in (0.02, 0.5, 0.93, 0.999):
+        for n in (2, 3, 7, 20, 51):
+            o_new, f = relocate.relocation_factors(alpha, n)
+            assert abs(1 - (1 - o_new) ** n - alpha) < 1e-12
+            s_old = 1.7
+            s_new = s_old * f
+            prof = 1 - (1 - o_new * np.exp(-x * x / (2 * s_new * s_new))) ** n
+            integral = np.trapezoid(prof, x)
+            assert abs(integral - alpha * s_old * math.sqrt(2 * math.pi)) < 1e-8 * integral, (alpha, n)
+            assert 0 < f and s_new > 0
+
+
+def test_p18_relocate_hand_example_and_degenerate_cases():
+    from oracle import relocate
+    sig_inv = lambda a: math.log(a / (1 - a))
+    alphas = np.array([0.5, 0.001, 0.25, 0.004, 0.25])                 # surfels 1 and 3 are dead (<= 0.005)
+    n = 5
+    rng = np.random.default_rng(0)
+    means, quats, scales, rgb = rng.normal(0, 1, (n, 3)), rng.normal(0, 1, (n, 4)), rng.uniform(0.5, 2, (n, 2)), rng.uniform(0, 1, (n, 3))
+    logits = np.array([sig_inv(a) for a in alphas])
+    st = lambda: dict(means=np.ones((n, 3)), quats=np.ones((n, 4)), scales=np.ones((n, 2)), logits=np.ones(n), rgb=np.ones((n, 3)))
+    # live cumulative weights: [0.5, 0.5, 0.75, 0.75, 1.0]; u = 0.6 -> surfel 2, u = 0.1 -> surfel 0
+    u = np.array([0.9, 0.6, 0.9, 0.1, 0.9])
+    out = relocate.relocate(means, quats, scales, logits, rgb, st(), st(), u)
+    assert out["dead"].tolist() == [False, True, False, True, False]
+    assert out["src"].tolist() == [-1, 2, -1, 0, -1] and out["ratio"].tolist() == [2, 1, 2, 1, 1]
+    for d, j in ((1, 2), (3, 0)):
+        o_new, f = relocate.relocation_factors(alphas[j], 2)
+        for k in ("means", "quats", "rgb"):
+            np.testing.assert_array_equal(out[k][d], [means, quats, rgb][["means", "quats", "rgb"].index(k)][j])
+        np.testing.assert_allclose(out["scales"][d], scales[j] * f, rtol=1e-14)
+        np.testing.assert_allclose(out["scales"][j], scales[j] * f, rtol=1e-14)
+        assert abs(1 / (1 + math.exp(-out["logits"][d])) - o_new) < 1e-14 and out["logits"][j] == out["logits"][d]
+        np.testing.assert_array_equal(out["means"][j], means[j])
+    # surfel 4 untouched, bit for bit; Adam state zeroed exactly on the four touched surfels
+    for k, a in (("means", means), ("quats", quats), ("scales", scales), ("logits", logits), ("rgb", rgb)):
+        np.testing.assert_array_equal(out[k][4], a[4])
+    assert out["adam_m"]["means"][[0, 1, 2, 3]].sum() == 0 and (out["adam_m"]["means"][4] == 1).all()
+    assert out["adam_v"]["logits"].tolist() == [0, 0, 0, 0, 1]
+    # nothing dead / nothing alive: nothing moves
+    same = relocate.relocate(means, quats, scales, np.full(n, 1.0), rgb, None, None, u)
+    np.testing.assert_array_equal(same["scales"], scales)
+    none_alive = relocate.relocate(means, quats, scales, np.full(n, -20.0), rgb, None, None, u)
+    np.testing.assert_array_equal(none_alive["means"], means)
+    # many copies of one source: the cap n_max applies to the factors
+    logits2 = np.array([sig_inv(0.8)] + [-20.0] * 60)
+    big = relocate.relocate(np.zeros((61, 3)), np.ones((61, 4)), np.ones((61, 2)), logits2, np.zeros((61, 3)), None, None,
+                            np.full(61, 0.5))
+    o51, f51 = relocate.relocation_factors(0.8, 51)
+    np.testing.assert_allclose(big["scales"], f51, rtol=1e-12)
+    assert big["ratio"][0] == 61
