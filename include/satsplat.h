@@ -221,6 +221,24 @@ int satsplat_init_from_dsm(const float* dsm, int32_t dsm_w, int32_t dsm_h, float
                            const float* u, const float* jx, const float* jy, void* scratch, float* means, float* quats,
                            float* scales, int32_t* cells_out, satsplat_stream stream);
 
+/* ---- relocation of dead surfels (second half) ------------------------------ */
+/* PAPER.md:200 "use the 3DGS-MCMC [22] strategy to relocate Gaussians during training".  A surfel is DEAD if
+ * sigmoid(logit) <= o_min ([22]: 0.005; decided on the logit).  Every dead surfel draws a live source j with probability
+ * proportional to opacity: the first j, in index order, whose cumulative live opacity exceeds u[d] * total (double
+ * precision; u in [0,1) are the CALLER's random numbers, only those of dead surfels are read).  A source drawn by n - 1
+ * dead surfels (n capped at n_max; [22]: 51) and its n - 1 copies all get opacity o' = 1 - (1 - alpha)^(1/n) (clamped to
+ * [o_min, 1 - 1e-7]) and scales multiplied by alpha / D, D = sum_{i=1..n} sum_{k<i} C(i-1,k) (-1)^k o'^(k+1) / sqrt(k+1):
+ * the n copies composited at the centre give alpha back and the composited profile keeps its integral.  A dead surfel
+ * also takes the source's centre, rotation and colour.  The Adam state (layout of satsplat_adam_step; both NULL = none) of
+ * every dead surfel and every drawn source is cleared.  No live surfel: nothing moves.
+ * All pointers DEVICE; parameters and state are updated in place; scratch: satsplat_relocate_scratch_bytes(N) bytes,
+ * 16-byte aligned; src_out [N] int32 (may be NULL): source index of a relocated surfel, -1 otherwise.  Seven kernels on
+ * `stream`, no host synchronisation.  Errors: SATSPLAT_E_INVALID, SATSPLAT_E_CUDA. */
+int64_t satsplat_relocate_scratch_bytes(int64_t N);
+int satsplat_relocate(int64_t N, float* means, float* quats, float* scales, float* opacity_logits, float* rgb, float* adam_m,
+                      float* adam_v, const float* u, float o_min, int32_t n_max, void* scratch, int32_t* src_out,
+                      satsplat_stream stream);
+
 /* ---- status, test and profiling access ------------------------------------------------------------------ */
 /* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
  * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */

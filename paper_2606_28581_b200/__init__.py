@@ -111,6 +111,9 @@ def lib():
         L.satsplat_init_scratch_bytes.restype = C.c_int64
         L.satsplat_init_scratch_bytes.argtypes = [i32, i32, i64]
         L.satsplat_init_from_dsm.argtypes = [vp, i32, i32, f32, f32, f32, i64] + [vp] * 9
+        L.satsplat_relocate_scratch_bytes.restype = C.c_int64
+        L.satsplat_relocate_scratch_bytes.argtypes = [i64]
+        L.satsplat_relocate.argtypes = [i64] + [vp] * 8 + [f32, i32, vp, vp, vp]
         L.satsplat_adam_state_floats.restype = C.c_int64
         L.satsplat_adam_state_floats.argtypes = [i64]
         L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
@@ -220,6 +223,18 @@ def init_from_dsm(dsm, cell, origin, u, jx, jy, want_cells=False, stream=None):
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
     return (means, quats, scales, cells) if want_cells else (means, quats, scales)
+
+
+def relocate(n, means, quats, scales, opacity_logits, rgb, adam_m, adam_v, u, o_min=0.005, n_max=51, want_src=False, stream=None):
+    """satsplat_relocate: dead surfels (opacity <= o_min) are redrawn onto live ones, in place (device tensors)."""
+    scratch = torch.empty(max(int(lib().satsplat_relocate_scratch_bytes(int(n))), 16), dtype=torch.uint8, device=means.device)
+    src = torch.empty(int(n), dtype=torch.int32, device=means.device) if want_src else None
+    rc = lib().satsplat_relocate(int(n), _ptr(means), _ptr(quats), _ptr(scales), _ptr(opacity_logits), _ptr(rgb), _ptr(adam_m),
+                                 _ptr(adam_v), _ptr(u), float(o_min), int(n_max), scratch.data_ptr(),
+                                 None if src is None else src.data_ptr(), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+    return src
 
 
 def adam_state_floats(n) -> int:

@@ -282,6 +282,21 @@ int satsplat_init_from_dsm(const float* dsm, int32_t dsm_w, int32_t dsm_h, float
   return SATSPLAT_OK;
 }
 
+int64_t satsplat_relocate_scratch_bytes(int64_t N) { return N < 0 ? 0 : relocate_scratch_bytes(N); }
+
+int satsplat_relocate(int64_t N, float* means, float* quats, float* scales, float* opacity_logits, float* rgb, float* adam_m,
+                      float* adam_v, const float* u, float o_min, int32_t n_max, void* scratch, int32_t* src_out,
+                      satsplat_stream stream) {
+  if (N < 0 || !(o_min > 0.f && o_min < 1.f) || n_max < 1 || (adam_m == nullptr) != (adam_v == nullptr))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_relocate: bad argument");
+  if (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb || !u || !scratch))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_relocate: NULL pointer");
+  cudaError_t e = launch_relocate(N, means, quats, scales, opacity_logits, rgb, adam_m, adam_v, u, o_min, n_max, scratch, src_out,
+                                  (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_relocate: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 int64_t satsplat_adam_state_floats(int64_t N) {
   static const int width[5] = {3, 4, 2, 1, 3};
   int64_t t = 0;

@@ -261,6 +261,18 @@ __global__ void __launch_bounds__(128) knn_scale_kernel(KnnGrid G, long long N, 
   scales[2 * i + 1] = s;
 }
 
+// in-place inclusive cumulative sum of M doubles (three launches); partial needs M / 4096 + 9 doubles, total = partial + nb
+int64_t cdf_scan_partials(int64_t M) { return (M + kScanChunk - 1) / kScanChunk + 9; }
+cudaError_t launch_cdf_scan(double* w, long long M, double* partial, double** total_out, cudaStream_t s) {
+  const int nb = (int)((M + kScanChunk - 1) / kScanChunk);
+  *total_out = partial + nb;
+  g_kernel_launches += 3;
+  cdf_partials_kernel<<<nb, kScanBlock, 0, s>>>(w, M, partial);
+  cdf_top_kernel<<<1, kScanBlock, 0, s>>>(partial, nb, partial + nb);
+  cdf_apply_kernel<<<nb, kScanBlock, 0, s>>>(w, M, partial);
+  return cudaGetLastError();
+}
+
 int64_t init_scratch_bytes(int W, int H, int64_t N) {
   const int64_t M = (int64_t)W * H;
   const int64_t nb = (M + kScanChunk - 1) / kScanChunk;

@@ -209,6 +209,11 @@ struct LossHost {   // arguments of the loss stage (losses.cu)
 };
 cudaError_t launch_losses(const LossHost& L, cudaStream_t s);
 int64_t init_scratch_bytes(int W, int H, int64_t N);
+int64_t cdf_scan_partials(int64_t M);
+cudaError_t launch_cdf_scan(double* w, long long M, double* partial, double** total_out, cudaStream_t s);
+int64_t relocate_scratch_bytes(int64_t N);
+cudaError_t launch_relocate(int64_t N, float* means, float* quats, float* scales, float* logits, float* rgb, float* adam_m,
+                            float* adam_v, const float* u, float o_min, int n_max, void* scratch, int32_t* src_out, cudaStream_t s);
 cudaError_t launch_init_from_dsm(const float* dsm, int W, int H, float cell, float ox, float oy, int64_t N, const float* u,
                                  const float* jx, const float* jy, void* scratch, float* means, float* quats, float* scales,
                                  int32_t* cells_out, cudaStream_t s);

@@ -583,3 +583,46 @@ def test_init_from_dsm_matches_oracle(P, G, shape, n):
         ok = np.abs(s - ref["scales"]) <= 2e-4 * ref["scales"] + 2e-5
         assert (~ok).sum() <= 8 * (~same).sum()
     assert (s[:, 0] == s[:, 1]).all() and (s > 0).all()
+
+
+@pytest.mark.parametrize("n,frac_dead", [(1, 1.0), (7, 0.3), (5000, 0.02), (50000, 0.5), (300, 0.98)])
+def test_relocate_matches_oracle(P, G, n, frac_dead):
+    """satsplat_relocate against the plain-loop oracle: which surfels are dead, which source each draws (index work: exact),
+    the new scales / logits, the copied parameters, the cleared Adam state, and that untouched surfels are bit-identical.
+    frac_dead = 0.98 makes single sources collect more copies than n_max."""
+    import torch
+    from oracle import relocate, adam
+    rng = np.random.default_rng(n)
+    f32 = lambda a: np.asarray(a, np.float32)
+    means, quats, scales, rgb = f32(rng.normal(0, 10, (n, 3))), f32(rng.normal(0, 1, (n, 4))), f32(rng.uniform(0.2, 2, (n, 2))), f32(rng.uniform(0, 1, (n, 3)))
+    logits = f32(rng.normal(0.5, 1.5, n))
+    dead = rng.uniform(0, 1, n) < frac_dead
+    logits[dead] = f32(rng.uniform(-12, -5.4, dead.sum()))               # sigmoid(-5.4) = 0.0045 <= 0.005
+    u = np.minimum(f32(rng.uniform(0, 1, n)), np.float32(0.99999994))
+    ns = P.adam_state_floats(n)
+    am, av = f32(rng.normal(0, 1, ns)), f32(rng.uniform(0, 1, ns))
+
+    def split_state(flat):
+        out, off = {}, 0
+        for k, wdt in zip(adam.GROUPS, (3, 4, 2, 1, 3)):
+            out[k] = flat[off:off + n * wdt].reshape((n, wdt) if wdt > 1 else (n,)).astype(np.float64)
+            off += (n * wdt + 3) // 4 * 4
+        return out
+    ref = relocate.relocate(means, quats, scales, logits, rgb, split_state(am), split_state(av), u)
+    d = [G.t(a) for a in (means, quats, scales, logits, rgb)]
+    dm, dv = G.t(am), G.t(av)
+    src = P.relocate(n, *d, dm, dv, G.t(u), want_src=True)
+    torch.cuda.synchronize()
+    src = src.cpu().numpy().astype(np.int64)
+    assert np.array_equal(src, ref["src"])                               # same dead set, same sources
+    touched = ref["dead"] & (ref["src"] >= 0) | (ref["ratio"] > 1)
+    for k, t_, a in zip(("means", "quats", "scales", "logits", "rgb"), d, (means, quats, scales, logits, rgb)):
+        g = t_.cpu().numpy()
+        assert np.array_equal(g[~touched], a[~touched]), k                # untouched: bit for bit
+        np.testing.assert_allclose(g.astype(np.float64), ref[k], rtol=3e-6, atol=1e-6)
+    gm, gv = split_state(dm.cpu().numpy()), split_state(dv.cpu().numpy())
+    for k in adam.GROUPS:
+        np.testing.assert_array_equal(gm[k], ref["adam_m"][k])
+        np.testing.assert_array_equal(gv[k], ref["adam_v"][k])
+    if frac_dead == 0.98:
+        assert ref["ratio"].max() > 51
