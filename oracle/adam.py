@@ -16,6 +16,8 @@ Readings where the paper is silent (rows 19-20):
     theta = log s, dL/dtheta = s dL/ds, s <- s exp(-lr m^/(sqrt(v^) + eps)); its Adam state is that of theta.
 Pins: tests/test_oracle_pins.py P15 (first-step closed form, torch.optim.Adam as an independent routine, log-space
 equivalence).
+PARITY UNPINNED against the paper for the opacity learning rate, the betas and epsilon (arguments) and the log-space
+stepping of the scales.
 """
 from __future__ import annotations
 

@@ -15,6 +15,8 @@ Readings (DESIGN.md section 2 rows 26-29; the paper gives the idea, not the disc
   * orientation (:192): n = (-h_x, -h_y, 1)/|.|, t_u = Gram-Schmidt of the world x axis against n, t_v = n x t_u,
     R = [t_u | t_v | n], quaternion (w, x, y, z) with w >= 0;
   * scale (:194): s_u = s_v = mean Euclidean distance to the k = 3 nearest other sampled centres.
+PARITY UNPINNED against the paper for the discretisation (difference stencils, jitter, tangent-plane lift, k = 3, the
+reference axis of the Gram-Schmidt step); the formulas the paper does print (|dx x dy|, orthonormal frame) are pinned (P17).
 """
 from __future__ import annotations
 

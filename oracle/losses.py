@@ -20,6 +20,8 @@ Definitions and readings (DESIGN.md section 2 rows 21-25; the paper gives names,
     (one constant per camera).
 Pins: tests/test_oracle_pins.py P16 (planar depth -> plane normal, SSIM identities and a brute-force window sum,
 finite differences of the total).
+PARITY UNPINNED against the paper for the SSIM window / constants, the depth map behind Eq. 13, the border rule and the
+2DGS form of the normal term (the paper names them without formulas): this build's stated conventions.
 """
 from __future__ import annotations
 

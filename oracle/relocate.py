@@ -19,6 +19,8 @@ restated here is that paper's relocation, derived from what it must preserve (re
   5. a dead surfel takes the source's centre, rotation and colour and the new (scale, logit); the source takes the new
      (scale, logit); the Adam state (m, v) of both is reset to zero.  If there is no live surfel nothing moves.
 Pins: tests/test_oracle_pins.py P18.
+PARITY UNPINNED against the SatSplat paper (it cites [22] without restating the rule); what the rule must preserve IS
+pinned (P18, by quadrature).
 """
 from __future__ import annotations
 
