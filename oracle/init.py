@@ -5,7 +5,7 @@ spacing.
 TEST INFRASTRUCTURE ONLY: imported by tests/ only; shares no code with paper_2606_28581_b200/.  numpy float64, scipy's
 cKDTree as the library kNN routine, each step in the paper's order.
 
-Readings (DESIGN.md section 2 rows 26-29; the paper gives the idea, not the discretisation):
+Readings (DESIGN.md section 2 row 25; the paper gives the idea, not the discretisation):
   * DSM h[row, col] on a regular grid of spacing `cell`, cell centre (col + 0.5, row + 0.5) * cell + origin;
     local tangents by finite differences (central inside, one-sided on the border):
     dx = (cell, 0, h_x cell), dy = (0, cell, h_y cell), weight a = |dx x dy| = cell^2 sqrt(1 + h_x^2 + h_y^2)  (:186);

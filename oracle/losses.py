@@ -5,7 +5,7 @@ with the upstream gradients (v_rgba, v_geom, v_aux) that the rasteriser's backwa
 TEST INFRASTRUCTURE ONLY: imported by tests/ and bench.py's cpu_baseline leg; shares no code with
 paper_2606_28581_b200/.  Plain numpy, float64, every step written out in the order of the definitions below.
 
-Definitions and readings (DESIGN.md section 2 rows 21-25; the paper gives names, references and weights only):
+Definitions and readings (DESIGN.md section 2 rows 21-24; the paper gives names, references and weights only):
   L = w_l1 mean|I - I*| + w_ssim (1 - mean SSIM(I, I*)) + w_dist mean(L_dist) + w_normal mean(1 - A_sg N_r . N_d)
   * means over all H W pixels (and the 3 channels for L1 / SSIM);
   * SSIM [Wang et al. 2004] as used by 3DGS: 11x11 Gaussian window, sigma 1.5, zero padding, C1 = 0.01^2, C2 = 0.03^2,

@@ -5,7 +5,7 @@ TEST INFRASTRUCTURE ONLY: imported by tests/ only; shares no code with paper_260
 loops, in the order of the steps below.
 
 The SatSplat paper only cites [22] (Kheradmand et al., "3D Gaussian Splatting as Markov Chain Monte Carlo"); the rule
-restated here is that paper's relocation, derived from what it must preserve (readings: DESIGN.md section 2 rows 27-28):
+restated here is that paper's relocation, derived from what it must preserve (readings: DESIGN.md section 2 row 26):
   1. alpha_i = sigmoid(logit_i); surfel i is DEAD if alpha_i <= o_min (0.005 in [22]).
   2. every dead surfel d draws a live source j with probability proportional to alpha_j: inverse transform on the cumulative
      sum of the live opacities in index order with the caller's uniform number u_d (first j whose cumulative weight exceeds
