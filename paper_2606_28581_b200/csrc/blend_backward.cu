@@ -228,6 +228,8 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
     }
   }
   const float TfvT = Tf * vT;
+  const float zmean = A > 0.f ? M1 / A : 0.f;          // weighted mean depth of the pixel (shifted frame)
+  const float zvar = A > 0.f ? fmaxf(M2 - M1 * zmean, 0.f) : 0.f;
   float Ssum = 0.f;
   const unsigned lt_mask = (1u << lane) - 1u;
   const int team = lane / kTeam, tl = lane % kTeam;
@@ -362,9 +364,11 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
           v_z = w * vD;
         } else {
           const float4 r3 = E.e[3];
-          const float psi = zs * zs * A - 2.0f * zs * M1 + M2;
+          // psi = z^2 A - 2 z M1 + M2 = A (z - m)^2 + (M2 - M1^2 / A) with m = M1 / A: no cancellation per pair
+          const float dz = zs - zmean;
+          const float psi = A * dz * dz + zvar;
           phi = va0 * r2.z + va1 * r2.w + va2 * r3.x + vN0 * r3.y + vN1 * r3.z + vN2 * r3.w + vD * zs + vL * psi;
-          v_z = w * (vD + 2.0f * vL * (zs * A - M1)) + ((E.ji.x == mi) ? vmed : 0.f);
+          v_z = w * (vD + 2.0f * vL * A * dz) + ((E.ji.x == mi) ? vmed : 0.f);
         }
         const float v_a = Ti * phi - (Ssum + TfvT) * rc;
         Ssum += w * phi;

@@ -142,14 +142,14 @@ def test_forward_backward_parity(P, G, orc, cfg):
                 assert (np.abs(g_b - r_b) <= 1e-4 + 5e-2 * row).all(), k
             gg = {k: (np.where(big.reshape(-1, *([1] * (v.ndim - 1))), 0, v) if k in per_surfel else v) for k, v in gg.items()}
             gr = {k: (np.where(big.reshape(-1, *([1] * (np.asarray(v).ndim - 1))), 0, v) if k in per_surfel else v) for k, v in gr.items()}
-        # C4 also composites 20 pairs per pixel over depth ranges of tens of metres: the fp32 depth / distortion terms
-        # (psi = z^2 A - 2 z M1 + M2 and the suffix sums) lose ~1e-4 per pixel, and 2e-4 of the geometry rows end up outside
-        # the 1e-3 row bar (colour rows, which carry no depth term, agree to 1e-7).  Bar for this stress config: at most
-        # 5e-4 of the elements outside the row bar, none beyond 30x.
+        # C4 also composites 20 pairs per pixel over depth ranges of tens of metres (fp32 depth / distortion terms and
+        # suffix sums): a few rows per million end up outside the 1e-3 row bar (colour rows, which carry no depth term,
+        # agree to 1e-7).  Bar for this stress config: at most 2e-5 of the elements outside the row bar, none beyond 10x
+        # (DESIGN.md section 3).
         gstats = G.compare_grads(gg, gr, pairs=G.GRAD_PAIRS if cfg != "C4full" else G.GRAD_PAIRS[:5],
-                                 allow_frac=5e-4 if cfg == "C4full" else 0.0)
+                                 allow_frac=2e-5 if cfg == "C4full" else 0.0)
         if cfg == "C4full":
-            assert max(v[0] for v in gstats.values()) < 30.0, gstats
+            assert max(v[0] for v in gstats.values()) < 10.0, gstats
             assert gstats["v_rgb"][1] == 0
         if cfg == "C4full":     # v_dF is one global sum over all surfels, the oversized ones included
             np.testing.assert_allclose(resb["grads"]["v_dF"], refb["grads"]["v_dF"], rtol=2e-3, atol=2e-3 * np.abs(refb["grads"]["v_dF"]).max())
