@@ -142,7 +142,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->px_i, px));
   A(dalloc(ctx, &ctx->px_visited, px));
   A(dalloc(ctx, &ctx->px_contrib, px));
-  A(dalloc(ctx, &ctx->red_buf, 64));
+  A(dalloc(ctx, &ctx->red_buf, satsplat::kRedCopies * 32));
   A(cudaMemset(ctx->vrec, 0, N ? N * satsplat::kVrec * sizeof(float) : 4));
   A(cudaMemset(ctx->status, 0, sizeof(Status)));
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i) A(cudaEventCreate(&ctx->ev[i]));

@@ -125,7 +125,6 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
   // per warp: pending pairs (s, t, w, source lane | low-pass flag) and their local coordinates: (u, v), or (dx, dy)
   // for low-pass pairs; kSegs segments of up to 32 pairs each (dynamic shared memory: kPairBytes per CTA)
   extern __shared__ float4 s_dyn[];
-  __shared__ float s_red[kWarpsB][24];
 
   // CTA blockIdx.y holds warps [blockIdx.y * kWarpsB, +kWarpsB) of tile column blockIdx.x; a tile has 8 warps (8x4 px each)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -214,17 +213,11 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       vT += -vA + va0 * P.cam.bg[0] + va1 * P.cam.bg[1] + va2 * P.cam.bg[2];   // A = 1 - T_f ; albedo = C + T_f bg
       vT -= vD * zref;                                                          // D = M1' + z_ref (1 - T_f)
     }
-    // ---- reduce the 23 epilogue gradients over the CTA (transposed butterfly, then shared memory), one atomic each ----
+    // ---- reduce the 23 epilogue gradients over the warp (transposed butterfly); one RED per value into one of kRedCopies
+    // copies of the 23-vector (spread by warp: no hot address, and no CTA barrier); add_small sums the copies ----
     if (P.red) {
       const float r = warp_reduce32_transposed(red, lane);
-      if (lane < 24) s_red[warp][lane] = r;
-      __syncthreads();
-      if (threadIdx.x < 23) {
-        float r = 0.f;
-#pragma unroll
-        for (int w = 0; w < kWarpsB; ++w) r += s_red[w][threadIdx.x];
-        if (r != 0.f) atomicAdd(P.red + threadIdx.x, r);
-      }
+      if (lane < 23 && r != 0.f) atomicAdd(P.red + (gw & (kRedCopies - 1)) * 32 + lane, r);
     }
   }
   const float TfvT = Tf * vT;
@@ -419,7 +412,7 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.v_sun_depth = v_sun_depth;
   const bool want_red = !depth_only && (v_cc || v_ambient || v_reproj);
   P.red = want_red ? c->red_buf : nullptr;
-  if (want_red) cudaMemsetAsync(c->red_buf, 0, 32 * sizeof(float), s);
+  if (want_red) cudaMemsetAsync(c->red_buf, 0, kRedCopies * 32 * sizeof(float), s);
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));
   constexpr int kPairBytes = kWarpsB * kSegs * 32 * (int)(sizeof(float4) + sizeof(float2));
   static bool attr_done[64] = {};   // per device: the dynamic shared-memory limit is a per-device function attribute

@@ -221,8 +221,13 @@ cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1,
   return cudaGetLastError();
 }
 
+// dst[k] += sum over the kRedCopies copies of src[copy * 32 + k]
 __global__ void add_small_kernel(float* dst, const float* src, int n) {
-  if ((int)threadIdx.x < n) dst[threadIdx.x] += src[threadIdx.x];
+  if ((int)threadIdx.x < n) {
+    float a = 0.f;
+    for (int c = 0; c < kRedCopies; ++c) a += src[c * 32 + threadIdx.x];
+    dst[threadIdx.x] += a;
+  }
 }
 cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s) {
   ++g_kernel_launches;

@@ -69,6 +69,7 @@ struct DevShading {
 // The first two float4 are all the per-pair test needs; the last two are only read by contributing pairs.
 // Gradient records (vrec) are kVrec floats of per-surfel moments: layout in blend_backward.cu.
 constexpr int kVrec = 20;
+constexpr int kRedCopies = 64;   // copies of the 23 epilogue-gradient sums (cc, ambient, reproj) the backward spreads its REDs over
 
 // sort configuration
 constexpr int kSortThreads = 256;
