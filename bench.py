@@ -166,7 +166,7 @@ def run_reference(args):
 def workload_config(scene, args, world):
     v = scene.views[0]
     return dict(workload=f"C{args.config} benchmark-shaped site (BASELINE.json configs[{args.config}])", surfels=scene.n,
-                view=f"{v.width}x{v.height}", cuda_graphs=not getattr(args, "no_graphs", False), sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
+                view=f"{v.width}x{v.height}", cuda_graphs=(not getattr(args, "no_graphs", False)) and world == 1, sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
                 views=len(scene.views), shadows=bool(v.shadows_on), parallelism=f"views sharded over {world} rank(s), no collective",
                 l2="per-step working set (records, keys, per-pixel state, images: >0.8 GB) exceeds the 126 MB L2; views cycle")
 
@@ -357,7 +357,8 @@ def run_ours(args):
     sampler.start()
     run_step = job.step
     launches_per_step = None
-    if not args.no_graphs:
+    use_graphs = not args.no_graphs and world == 1   # multi-rank runs launch from the host (no capture beside the NCCL watchdog)
+    if use_graphs:
         # one CUDA graph per view (the camera is baked into the kernel arguments): a step is one graph launch
         graphs = {}
         for vi in sorted(set(step_views)):
