@@ -36,10 +36,10 @@ FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.96
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the view-pass kernels at C3, from the committed
 # `ncu --set full` capture (a profiler number is never a bench value: it only fills roofline.traffic)
 NCU_SOURCE = "profiles/r1_kernels_final.md"
-NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": 784.7e6, "blend_fwd": 529.6e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": 784.4e6, "blend_fwd": 528.7e6}
 # executed warp-instructions and issue-slot utilisation of the same capture (the kernels cull before they evaluate:
 # they execute fewer lane-instructions than the algorithmic count the roofline fraction is quoted on)
-NCU_EXECUTED = {"blend_bwd": dict(warp_inst=675.5e6, issue_active_pct=72.8), "blend_fwd": dict(warp_inst=324.7e6, issue_active_pct=78.3)}
+NCU_EXECUTED = {"blend_bwd": dict(warp_inst=671.3e6, issue_active_pct=73.9), "blend_fwd": dict(warp_inst=324.7e6, issue_active_pct=78.4)}
 
 
 def parse():
