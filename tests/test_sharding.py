@@ -63,3 +63,37 @@ def test_views_for_rank_single_process_cycles():
     import bench
     assert bench.views_for_rank(0, 1, 20, 23) == [i % 20 for i in range(23)]
     assert bench.views_for_rank(3, 8, 20, 3) == [3, 11, 19]
+
+
+def _ref_worker(rank, out):
+    import contextlib
+    import io
+    import json
+    import bench
+    os.environ.update(RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank))
+    buf = io.StringIO()
+    with contextlib.redirect_stdout(buf):
+        sys.argv = ["bench.py", "--impl", "reference", "--config", "0", "--steps", "1", "--warmup", "0", "--gpus", "2"]
+        bench.main()
+    txt = buf.getvalue().strip()
+    out.put((rank, json.loads(txt) if txt else None))
+
+
+@pytest.mark.timeout(300)
+def test_reference_arm_runs_on_rank0_only():
+    """`bench.py --impl reference` under a 2-rank launch: rank 0 times the oracle and prints the JSON line, the other rank
+    exits without work or output (tier contract for the reference arm)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_ref_worker, args=(r, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict(q.get(timeout=250) for _ in range(2))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert got[1] is None
+    line = got[0]
+    assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "Mpixel/s"
