@@ -197,6 +197,7 @@ class Job:
         self.device = device
         # the view pass's preprocess + binning do not depend on the sun pass: they run on a second stream beside it
         self.side = torch.cuda.Stream(device=device) if self.shadows else None
+        self.overlap = True     # False: everything on one stream (the per-stage timers then see each kernel alone)
 
     def prepare_view(self, vi):
         if vi in self.cams:
@@ -221,7 +222,11 @@ class Job:
     def forward(self, vi):
         cam, sun_cam, _ = self.cams[vi]
         sh = self.shading(vi)
-        if self.shadows:
+        if self.shadows and not self.overlap:
+            self.sctx.preprocess(sun_cam, self.means, self.quats, self.scales, self.logits, self.rgb)
+            self.sctx.shadow_map(self.sun_depth)
+            self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb)
+        elif self.shadows:
             cur = self.torch.cuda.current_stream()
             self.side.wait_stream(cur)
             self.ctx.preprocess(cam, self.means, self.quats, self.scales, self.logits, self.rgb, stream=self.side)
@@ -285,6 +290,7 @@ def stage_profile(job, views, peaks):
     job.ctx.set_profiling(True)
     if job.sctx:
         job.sctx.set_profiling(True)
+    job.overlap = False
     ms_view, ms_sun = {}, {}
     for vi in views:
         job.step(vi)
@@ -296,6 +302,7 @@ def stage_profile(job, views, peaks):
     job.ctx.set_profiling(False)
     if job.sctx:
         job.sctx.set_profiling(False)
+    job.overlap = True
     nv, nc = job.ctx.debug_planes()
     pairs = dict(view_evaluated=int(nv.sum().item()), view_contributing=int(nc.sum().item()), view_K=job.ctx.sync_status())
     if job.sctx:
