@@ -146,6 +146,8 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(cudaMemset(ctx->vrec, 0, N ? N * satsplat::kVrec * sizeof(float) : 4));
   A(cudaMemset(ctx->status, 0, sizeof(Status)));
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i) A(cudaEventCreate(&ctx->ev[i]));
+  A(cudaStreamCreateWithFlags(&ctx->bin_stream, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) A(cudaEventCreateWithFlags(&ctx->bin_ev[i], cudaEventDisableTiming));
 #undef A
   if (e != cudaSuccess) {
     fail(nullptr, SATSPLAT_E_CUDA, "satsplat_create: %s", cudaGetErrorString(e));
@@ -169,6 +171,9 @@ void satsplat_destroy(satsplat_ctx* ctx) {
     if (p) cudaFree(p);
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  if (ctx->bin_stream) cudaStreamDestroy(ctx->bin_stream);
+  for (int i = 0; i < 2; ++i)
+    if (ctx->bin_ev[i]) cudaEventDestroy(ctx->bin_ev[i]);
   for (int i = 0; i < 2; ++i)
     if (ctx->e2e_stream[i]) cudaStreamDestroy(ctx->e2e_stream[i]);
   for (int i = 0; i < 4; ++i)

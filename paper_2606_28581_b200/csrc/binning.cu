@@ -374,10 +374,13 @@ cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
 // single CTA: exclusive scan of tile_count[tiles]; writes ranges, K, overflow; resets the cursors and the worklist.
 // Chunks of 1024 x 8 counters are staged through shared memory so that every global access is coalesced.
 constexpr int kTileScanItems = 8;
+constexpr int kTileSortWarpMax = 1024;    // entries one warp sorts in registers (32 per lane)
 __global__ void __launch_bounds__(1024) tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_start,
                                                          uint32_t* __restrict__ ranges, Status* status, uint32_t capacity,
-                                                         uint32_t* __restrict__ wl_count) {
+                                                         uint32_t* __restrict__ wl_count, uint32_t* __restrict__ worklist) {
   __shared__ uint32_t s_warp[33];
+  __shared__ uint32_t s_wl[2];   // lengths of the mid / large worklists (tiles too long for the one-warp register sort)
+  if (threadIdx.x < 2) s_wl[threadIdx.x] = 0u;
   __shared__ uint32_t s_cnt[1024 * kTileScanItems + 8];
   __shared__ uint32_t s_total;
   constexpr int kChunk = 1024 * kTileScanItems;
@@ -418,16 +421,22 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int tiles, uint32_t* __
       tile_start[base + i] = st;
       const bool empty = en == st || overflow;      // overflow: nothing is rendered (outputs undefined, no OOB access)
       reinterpret_cast<uint2*>(ranges)[base + i] = empty ? make_uint2(0u, 0u) : make_uint2(st, en);
+      const uint32_t len = empty ? 0u : en - st;
+      if (len > 256u) {                             // dispatch by list length (see tile_sort_kernel)
+        if (len > (uint32_t)kTileSortWarpMax) worklist[tiles + atomicAdd(&s_wl[1], 1u)] = (uint32_t)(base + i);
+        else worklist[atomicAdd(&s_wl[0], 1u)] = (uint32_t)(base + i);
+      }
     }
     carry += chunk_total;
     __syncthreads();
   }
+  __syncthreads();
   if (threadIdx.x == 0) {
     status->K = total;
     status->overflow = overflow ? 1u : 0u;
-    wl_count[0] = 0;
+    wl_count[0] = s_wl[0];
     wl_count[1] = 0;
-    wl_count[2] = 0;
+    wl_count[2] = s_wl[1];
     wl_count[3] = 0;
   }
 }
@@ -505,7 +514,6 @@ __device__ __forceinline__ void bitonic_sort_asc(uint64_t* buf, uint32_t n, uint
 }
 
 constexpr int kTileSortWarps = 8;         // warps (= tiles) per CTA
-constexpr int kTileSortWarpMax = 1024;    // entries one warp sorts in registers (32 per lane)
 constexpr int kTileSortCtaMax = 16384;    // entries one CTA sorts in shared memory (large-tile kernel)
 
 // Warp-wide bitonic sort of 32*E 64-bit values held in registers, blocked layout: element index of v[e] is
@@ -578,13 +586,7 @@ __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tile
   if (lane == 0) cursor[t] = 0;   // leave the per-tile counters zero for the next preprocess on this context
   const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
   if (n == 0) return;
-  if (n > 256u) {
-    if (lane == 0) {
-      if (n > (uint32_t)kTileSortWarpMax) worklist[tiles + atomicAdd(wl_count + 2, 1u)] = (uint32_t)t;
-      else worklist[atomicAdd(wl_count, 1u)] = (uint32_t)t;
-    }
-    return;
-  }
+  if (n > 256u) return;           // on a worklist (built by tile_scan_kernel): sorted by the mid / large kernels beside this one
   const uint64_t hi = (uint64_t)(uint32_t)t << 32;
   if (n <= 64) tile_sort_warp<2>(entries + s, n, hi, keys + s, vals + s, lane);
   else if (n <= 128) tile_sort_warp<4>(entries + s, n, hi, keys + s, vals + s, lane);
@@ -646,7 +648,8 @@ __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* _
 cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
   ++g_kernel_launches;
-  tile_scan_kernel<<<1, 1024, 0, s>>>(tiles, c->tile_count, c->tile_start, c->ranges, c->status, (uint32_t)c->max_dup, c->wl_count);
+  tile_scan_kernel<<<1, 1024, 0, s>>>(tiles, c->tile_count, c->tile_start, c->ranges, c->status, (uint32_t)c->max_dup, c->wl_count,
+                                      c->worklist);
   return cudaGetLastError();
 }
 
@@ -666,11 +669,17 @@ cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
     attr_done[c->device & 63] = true;
   }
   g_kernel_launches += 3;
+  // the three kernels work on disjoint tiles (the worklists come from tile_scan_kernel): the few long lists, whose
+  // one-tile latency sets the duration of their kernels, are sorted on a second stream beside the many short ones
+  cudaEventRecord(c->bin_ev[0], s);
+  cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
+  tile_sort_mid_kernel<<<148 * 4, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
+                                                                            c->worklist + tiles, c->wl_count);
+  cudaEventRecord(c->bin_ev[1], c->bin_stream);
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(
       tiles, c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count, c->tile_count);
-  tile_sort_mid_kernel<<<148 * 4, 128, 0, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
-  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, s>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist + tiles,
-                                                               c->wl_count);
+  cudaStreamWaitEvent(s, c->bin_ev[1], 0);
   c->sorted = 0;
   return cudaGetLastError();
 }

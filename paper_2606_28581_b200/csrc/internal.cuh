@@ -150,6 +150,8 @@ struct satsplat_ctx {
   uint32_t* worklist;     // [2*tiles] tiles too long for the small-tile sort: mid list, then large list
   uint32_t* wl_count;     // [4] mid length, mid cursor, large length, large cursor
   int binning_mode;       // SATSPLAT_BINNING_TILESORT (default) or SATSPLAT_BINNING_RADIX
+  cudaStream_t bin_stream;   // the long tile lists are sorted on this stream beside the short ones (forked from / joined to the caller's)
+  cudaEvent_t bin_ev[2];
   satsplat::Status* status;
   // per-pixel state kept for the backward
   float4* px_a;           // (T_f, z_ref, M1', M2')
