@@ -67,32 +67,38 @@ def ssim_map_and_grad(I, J):
     return m, grad
 
 
-def depth_normal_constants(Fp, view_dir):
-    """c = c0 + dx c1 + dy c2 with dx = z_v(i+1,j) - z_v(i-1,j), dy = z_v(i,j+1) - z_v(i,j-1) (p_s is affine in z_v)."""
+def world_points(zv, Fp, b_z):
+    """The point map p_s of Eq. 13: every pixel centre x = (j + .5, i + .5) backprojected to world
+    coordinates with its depth: h = b_z - z_v (Eq. 11), p_xy = B2^-1 (x - b - B3 h), p_z = h, F' = [B2 B3 | b]."""
     Fp = np.asarray(Fp, np.float64).reshape(2, 4)
-    B2, B3 = Fp[:, :2], Fp[:, 2]
+    B2, B3, b = Fp[:, :2], Fp[:, 2], Fp[:, 3]
     Bi = np.linalg.inv(B2)
-    k = np.array([*(Bi @ B3), -1.0])                     # d p_s / d z_v  (h = b_z - z_v)
-    ax = np.array([*(2.0 * Bi[:, 0]), 0.0])              # p(i+1) - p(i-1) at constant depth
-    ay = np.array([*(2.0 * Bi[:, 1]), 0.0])
-    c0, c1, c2 = np.cross(ax, ay), np.cross(k, ay), np.cross(ax, k)
-    sgn = -1.0 if float(c0 @ np.asarray(view_dir, np.float64)) > 0 else 1.0
-    return c0, c1, c2, sgn
-
-
-def depth_normals(zv, Fp, view_dir):
-    """N_d [H, W, 3] of Eq. 13 (zero on the border) and the intermediate c, for the backward."""
-    c0, c1, c2, sgn = depth_normal_constants(Fp, view_dir)
     H, W = zv.shape
-    dx, dy = np.zeros((H, W)), np.zeros((H, W))
-    dx[1:-1, 1:-1] = zv[1:-1, 2:] - zv[1:-1, :-2]        # x = column index
-    dy[1:-1, 1:-1] = zv[2:, 1:-1] - zv[:-2, 1:-1]        # y = row index
-    c = c0 + dx[..., None] * c1 + dy[..., None] * c2
-    N = sgn * c / np.linalg.norm(c, axis=-1, keepdims=True)
+    x = np.stack(np.meshgrid(np.arange(W) + 0.5, np.arange(H) + 0.5), -1)      # [H, W, 2] = (column, row) centres
+    h = b_z - zv
+    pxy = (x - b - h[..., None] * B3) @ Bi.T
+    return np.concatenate([pxy, h[..., None]], -1), Bi, B3
+
+
+def depth_normals(zv, Fp, view_dir, b_z):
+    """Eq. 13 as written: N_d = (grad_x p_s x grad_y p_s) / |.| with central differences of the point map on the
+    interior pixels, zero on the one-pixel border; oriented towards the sensor by one sign per camera (the sign that
+    makes the normal of a constant-depth map face the sensor).  Returns N_d [H, W, 3], the cross product c, the two
+    difference maps, the interior mask and the sign."""
+    p, _, _ = world_points(zv, Fp, b_z)
+    H, W = zv.shape
+    gx, gy = np.zeros((H, W, 3)), np.zeros((H, W, 3))
+    gx[1:-1, 1:-1] = p[1:-1, 2:] - p[1:-1, :-2]          # x = column index
+    gy[1:-1, 1:-1] = p[2:, 1:-1] - p[:-2, 1:-1]          # y = row index
+    c = np.cross(gx, gy)
+    flat, _, _ = world_points(np.zeros((3, 3)), Fp, b_z)
+    c_flat = np.cross(flat[1, 2] - flat[1, 0], flat[2, 1] - flat[0, 1])
+    sgn = -1.0 if float(c_flat @ np.asarray(view_dir, np.float64)) > 0 else 1.0
     interior = np.zeros((H, W), bool)
     interior[1:-1, 1:-1] = True
-    N[~interior] = 0.0
-    return N, c, interior, (c1, c2, sgn)
+    cn = np.linalg.norm(c, axis=-1, keepdims=True)
+    N = np.where(interior[..., None], sgn * c / np.where(cn > 0, cn, 1.0), 0.0)
+    return N, c, gx, gy, interior, sgn
 
 
 def loss_and_upstream(rgba, geom, aux, target, Fp, view_dir, b_z, z_bg, w_l1=0.8, w_ssim=0.2, w_dist=0.05, w_normal=0.05,
@@ -118,7 +124,7 @@ def loss_and_upstream(rgba, geom, aux, target, Fp, view_dir, b_z, z_bg, w_l1=0.8
     # ---- normal consistency ----
     D, Nr = geom[..., 3], geom[..., :3]
     zv = D + (1.0 - A) * z_bg
-    Nd, c, interior, (c1, c2, sgn) = depth_normals(zv, Fp, view_dir)
+    Nd, c, gx, gy, interior, sgn = depth_normals(zv, Fp, view_dir, b_z)
     Asg = A if alpha_sg is None else np.asarray(alpha_sg, np.float64)
     dot = (Nr * Nd).sum(-1)
     normal = (1.0 - Asg * dot).mean()
@@ -126,15 +132,21 @@ def loss_and_upstream(rgba, geom, aux, target, Fp, view_dir, b_z, z_bg, w_l1=0.8
     v_Nd = -w_normal * Asg[..., None] * Nr / npx
     # N = sgn c/|c|  =>  v_c = sgn (v_N - n (n . v_N)) / |c| with n = c/|c|
     cn = np.linalg.norm(c, axis=-1, keepdims=True)
+    cn = np.where(interior[..., None], cn, 1.0)
     n = c / cn
     v_c = sgn * (v_Nd - n * (n * v_Nd).sum(-1, keepdims=True)) / cn
     v_c[~interior] = 0.0
-    v_dx, v_dy = (v_c * c1).sum(-1), (v_c * c2).sum(-1)
-    v_zv = np.zeros((H, W))
-    v_zv[1:-1, 2:] += v_dx[1:-1, 1:-1]
-    v_zv[1:-1, :-2] -= v_dx[1:-1, 1:-1]
-    v_zv[2:, 1:-1] += v_dy[1:-1, 1:-1]
-    v_zv[:-2, 1:-1] -= v_dy[1:-1, 1:-1]
+    # c = gx x gy  =>  v_gx = gy x v_c,  v_gy = v_c x gx;  the differences scatter to the four neighbours of the point map
+    v_gx, v_gy = np.cross(gy, v_c), np.cross(v_c, gx)
+    v_p = np.zeros((H, W, 3))
+    v_p[1:-1, 2:] += v_gx[1:-1, 1:-1]
+    v_p[1:-1, :-2] -= v_gx[1:-1, 1:-1]
+    v_p[2:, 1:-1] += v_gy[1:-1, 1:-1]
+    v_p[:-2, 1:-1] -= v_gy[1:-1, 1:-1]
+    # p_xy = B2^-1 (x - b - B3 h), p_z = h, h = b_z - z_v  =>  d p / d z_v = (B2^-1 B3, -1)
+    _, Bi, B3 = world_points(zv, Fp, b_z)
+    k = np.array([*(Bi @ B3), -1.0])
+    v_zv = v_p @ k
     v_geom[..., 3] += v_zv                                # z_v = D + (1 - A) z_bg
     v_rgba[..., 3] += -z_bg * v_zv
     total = w_l1 * l1 + w_ssim * (1.0 - ssim) + w_dist * dist + w_normal * normal

@@ -211,7 +211,7 @@ def forward(width, height, b_z, z_bg, bg, rec, flags, lists, shading: Shading, o
     H, W = int(height), int(width)
     out = dict(rgba=np.zeros((H, W, 4)), geom=np.zeros((H, W, 4)), aux=np.zeros((H, W, 4)),
                albedo=np.zeros((H, W, 3)), last=np.zeros((H, W), np.int32), med_idx=np.zeros((H, W), np.int32),
-               margins=np.zeros((H, W, 6)), counters=np.zeros(2, np.int64))
+               margins=np.zeros((H, W, 6)), counters=np.zeros(5, np.int64))
     sh = shading.c()
     rc = lib().orc_forward(C.byref(cfg), C.byref(sh), _p(rec), _p(flags), _p(out["rgba"]), _p(out["geom"]),
                            _p(out["aux"]), _p(out["albedo"]), _p(out["last"]), _p(out["med_idx"]),

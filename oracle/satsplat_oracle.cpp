@@ -312,6 +312,7 @@ struct PixelState {
   int32_t mi;          // surfel id of the median-depth contributor, -1 if none
   int32_t n_visited;   // list entries visited (including the one that triggered the stop)
   int64_t n_contrib;
+  int64_t n_lowpass, n_clamped, n_degenerate;   // composited pairs on the low-pass branch / with alpha clamped / of degenerate surfels
   double margin[6];    // smallest distance to each decision: rho cut, alpha skip, T stop, median, branch, clamp
 };
 
@@ -324,6 +325,7 @@ void composite_pixel(const orc_render& cfg, const double* rec, const uint8_t* fl
   S.mi = -1;
   S.n_visited = 0;
   S.n_contrib = 0;
+  S.n_lowpass = S.n_clamped = S.n_degenerate = 0;
   for (double& m : S.margin) m = std::numeric_limits<double>::infinity();
   if (hits) hits->clear();
   const double inf = std::numeric_limits<double>::infinity();
@@ -367,6 +369,9 @@ void composite_pixel(const orc_render& cfg, const double* rec, const uint8_t* fl
     if (hits) hits->push_back(Hit{id, a, G, S.T, w, z, u, v, dx, dy, lowpass, !(aG < kAlphaMax)});
     S.T = Tn;
     ++S.n_contrib;
+    if (lowpass) ++S.n_lowpass;
+    if (!(aG < kAlphaMax)) ++S.n_clamped;
+    if (flags[id] & F_DEGENERATE) ++S.n_degenerate;
   }
 }
 
@@ -432,13 +437,14 @@ extern "C" {
 
 // out_rgba [H,W,4] = (I rgb, A);  out_geom [H,W,4] = (N xyz, D);  out_aux [H,W,4] = (median depth,
 // distortion, V, T_final);  albedo [H,W,3] (pre-correction, incl. T*bg);  last [H,W] = list entries
-// visited;  med_idx [H,W];  margins [H,W,6];  counters[2] = (evaluated pairs, contributing pairs).
+// visited;  med_idx [H,W];  margins [H,W,6];  counters[5] = (evaluated pairs, contributing pairs, and of the
+// contributing pairs: on the low-pass branch of Eq. 12, with alpha clamped at alpha_max, of degenerate surfels).
 int orc_forward(const orc_render* cfg, const orc_shading* sh, const double* rec, const uint8_t* flags,
                 double* out_rgba, double* out_geom, double* out_aux, double* albedo, int32_t* last,
                 int32_t* med_idx, double* margins, int64_t* counters) {
   const int W = cfg->width, H = cfg->height;
-  int64_t evaluated = 0, contributing = 0;
-#pragma omp parallel for schedule(dynamic, 4) num_threads(cfg->threads > 0 ? cfg->threads : 1) reduction(+ : evaluated, contributing)
+  int64_t evaluated = 0, contributing = 0, n_lowpass = 0, n_clamped = 0, n_degenerate = 0;
+#pragma omp parallel for schedule(dynamic, 4) num_threads(cfg->threads > 0 ? cfg->threads : 1) reduction(+ : evaluated, contributing, n_lowpass, n_clamped, n_degenerate)
   for (int iy = 0; iy < H; ++iy) {
     for (int ix = 0; ix < W; ++ix) {
       const uint32_t* list; int64_t len;
@@ -459,9 +465,13 @@ int orc_forward(const orc_render* cfg, const orc_shading* sh, const double* rec,
       if (margins) for (int k = 0; k < 6; ++k) margins[6 * o + k] = S.margin[k];
       evaluated += S.n_visited;
       contributing += S.n_contrib;
+      n_lowpass += S.n_lowpass; n_clamped += S.n_clamped; n_degenerate += S.n_degenerate;
     }
   }
-  if (counters) { counters[0] = evaluated; counters[1] = contributing; }
+  if (counters) {
+    counters[0] = evaluated; counters[1] = contributing;
+    counters[2] = n_lowpass; counters[3] = n_clamped; counters[4] = n_degenerate;
+  }
   return 0;
 }
 

@@ -497,6 +497,148 @@ def test_p8_finite_differences_with_cutoffs(orc):
         assert bad <= 1, (name, bad)
 
 
+# ------------------------------------------------------------------- P8b-d: the three branches of Eq. 12's backward
+def _branch_fd_problem(orc, P, *, options=7, hold_flags=False, W=16, H=16, seed=5):
+    """A finite-difference problem on hand-made surfel populations (view pass, shadows off).  With `hold_flags` the
+    per-surfel decisions (degenerate, flipped) are those of the unperturbed inputs, as in the record mode the GPU
+    path is compared in (reading 4: a degenerate surfel passes no gradient through Q, g)."""
+    rng = np.random.default_rng(seed)
+    F, d = S.affine_camera(0.5, math.radians(20), 0.7, W, H, (4, 4, 0))
+    view = make_view(W, H, F, view_dir=d, b_z=12.0, z_bg=16.0, bg=(0.2, 0.1, 0.3))
+    up = [rng.normal(0, 1, (H, W, 4)) for _ in range(3)]
+    up[2][..., 2:] = 0
+    order = np.argsort(-np.asarray(P["means"])[:, 2], kind="stable").astype(np.uint32)
+    base_flags = orc.preprocess_f64(view, P["means"], P["quats"], P["scales"], P["logits"], P["rgb"],
+                                    F=view.F.astype(np.float64), dF=P["dF"])["flags"].copy()
+
+    def run(Pv, need_grad=False):
+        sh = orc.Shading(cc=Pv["cc"], ambient=Pv["ambient"])
+        pre = orc.preprocess_f64(view, Pv["means"], Pv["quats"], Pv["scales"], Pv["logits"], Pv["rgb"],
+                                 F=view.F.astype(np.float64), dF=Pv["dF"])
+        rec, flags = pre["rec"], pre["flags"]
+        if hold_flags:
+            # keep the stored normal on the side the unperturbed preprocess chose, and the degenerate decision as it was
+            resign = ((flags ^ base_flags) & orc.F_FLIPPED) != 0
+            rec[resign, 13:16] *= -1.0
+            flags = base_flags
+        out = orc.forward(W, H, view.b_z, view.z_bg, view.bg_rgb, rec, flags, order, sh, options=options)
+        loss = (out["rgba"] * up[0]).sum() + (out["geom"] * up[1]).sum() + (out["aux"] * up[2]).sum()
+        if not need_grad:
+            return loss, out
+        bw = orc.backward(W, H, view.b_z, view.z_bg, view.bg_rgb, rec, flags, order, sh, *up, options=options)
+        g = orc.preprocess_backward(view, Pv["means"], Pv["quats"], Pv["scales"], Pv["logits"], flags, bw["v_rec"],
+                                    F=view.F.astype(np.float64), dF=Pv["dF"])
+        grads = dict(means=g["v_means"], quats=g["v_quats"], scales=g["v_scales"], logits=g["v_logits"], rgb=g["v_rgb"],
+                     dF=g["v_dF"], cc=bw["v_cc"], ambient=bw["v_ambient"])
+        return loss, out, grads
+
+    return view, run
+
+
+def _pair_table(orc, view, P):
+    """(pixel, surfel) pair quantities straight from the definitions (numpy, no oracle arithmetic): alpha * G with
+    the Eq. 12 exponent, which term of Eq. 12 is active."""
+    pre = orc.preprocess_f64(view, P["means"], P["quats"], P["scales"], P["logits"], P["rgb"],
+                             F=view.F.astype(np.float64), dF=P["dF"])
+    r = pre["rec"]
+    px, py = pixel_grid(view.width, view.height)
+    dx, dy = px[..., None] - r[:, 0], py[..., None] - r[:, 1]
+    u, v = r[:, 2] * dx + r[:, 3] * dy, r[:, 4] * dx + r[:, 5] * dy
+    deg = (pre["flags"] & orc.F_DEGENERATE) != 0
+    rho3 = np.where(deg, np.inf, u * u + v * v)
+    rho2 = 2.0 * (dx * dx + dy * dy)
+    aG = r[:, 9] * np.exp(-0.5 * np.minimum(rho3, rho2))
+    return dict(aG=aG, lowpass=~(rho3 <= rho2), rho3=rho3, rho2=rho2, flags=pre["flags"])
+
+
+def _common_groups(rng, n):
+    return dict(rgb=rng.uniform(0, 1, (n, 3)), dF=rng.normal(0, 1e-2, 8),
+                cc=(np.concatenate([np.eye(3), np.zeros((3, 1))], 1) + rng.normal(0, 0.1, (3, 4))).reshape(12),
+                ambient=rng.uniform(0.2, 0.5, 3))
+
+
+def test_p8b_alpha_clamp_branch_finite_differences(orc):
+    """alpha' = min(alpha_max, alpha G) (reading 7): where the clamp is active neither the opacity nor the
+    Gaussian receives a gradient.  Large, nearly opaque surfels so that many pairs sit on the clamp."""
+    rng = np.random.default_rng(41)
+    n = 12
+    quats = rng.normal(0, 0.15, (n, 4)); quats[:, 0] += 1.0
+    logits = np.where(np.arange(n) % 2 == 0, rng.uniform(7.0, 10.0, n), rng.normal(0.5, 1.0, n))
+    P = dict(means=np.concatenate([rng.uniform(0.5, 7.5, (n, 2)), rng.normal(0, 1.0, (n, 1))], 1), quats=quats,
+             scales=rng.uniform(2.5, 6.0, (n, 2)), logits=logits, **_common_groups(rng, n))
+    view, run = _branch_fd_problem(orc, P)
+    T = _pair_table(orc, view, P)
+    clamped = T["aG"] >= 0.99
+    assert clamped.sum() >= 10, clamped.sum()                       # the branch is exercised ...
+    assert np.abs(T["aG"] - 0.99).min() > 2e-5                      # ... and no pair sits on the switch itself
+    out, _ = _check_fd(P, run, ["means", "quats", "scales", "logits", "rgb", "dF", "cc", "ambient"], rtol=2e-6)
+    assert out["counters"][3] == clamped.sum()                      # the oracle takes the same branch for the same pairs
+
+
+def test_p8c_lowpass_branch_finite_differences(orc):
+    """Eq. 12 low-pass term: rho = 2 |x - c|^2 wins for sub-pixel and steeply tilted surfels; its gradient goes to the
+    centre only (no Q, no g), and the depth falls back to z_c.  Cut-offs off, every parameter group."""
+    rng = np.random.default_rng(43)
+    n = 14
+    # half the surfels sub-pixel (0.05-0.2 m at 0.5 m GSD), the others needle-like: sub-pixel across, pixels along,
+    # tilted up to 70 degrees, so that both terms of Eq. 12 are active on significant pairs of the same surfel
+    scales = np.where((np.arange(n) % 2 == 0)[:, None], rng.uniform(0.05, 0.2, (n, 2)),
+                      np.stack([rng.uniform(0.06, 0.2, n), rng.uniform(1.0, 2.5, n)], 1))
+    ang = rng.uniform(0.0, math.radians(70), n)
+    axis = rng.normal(0, 1, (n, 3)); axis[:, 2] *= 0.3
+    axis /= np.linalg.norm(axis, axis=1, keepdims=True)
+    quats = np.concatenate([np.cos(ang / 2)[:, None], np.sin(ang / 2)[:, None] * axis], 1) * rng.uniform(0.5, 2.0, (n, 1))
+    P = dict(means=np.concatenate([rng.uniform(1.0, 7.0, (n, 2)), rng.normal(0, 0.5, (n, 1))], 1), quats=quats,
+             scales=scales, logits=rng.normal(1.0, 1.0, n), **_common_groups(rng, n))
+    view, run = _branch_fd_problem(orc, P)
+    T = _pair_table(orc, view, P)
+    sig = T["aG"] > 1e-4                                            # pairs that matter to the loss
+    lp = T["lowpass"] & sig
+    assert lp.sum() >= 30 and lp.sum() >= 0.3 * sig.sum(), (lp.sum(), sig.sum())
+    assert (~T["lowpass"] & sig).sum() >= 10                        # the Eq. 9 term is active beside it
+    # no significant pair sits on the switch between the two terms (the depth jumps there)
+    assert np.abs(T["rho3"] - T["rho2"])[sig].min() > 1e-3
+    out, _ = _check_fd(P, run, ["means", "quats", "scales", "logits", "rgb", "dF", "cc", "ambient"], h=1e-7, rtol=2e-6)
+    assert out["counters"][2] == T["lowpass"].sum()
+
+
+def test_p8d_degenerate_surfels_pass_no_gradient_through_Q_and_g(orc):
+    """Exactly edge-on surfels (det(B'RS') = 0): low-pass term only, depth z_c, and with the per-surfel
+    decisions held fixed the objective does not depend on their scales, nor on their rotation except through the
+    blended normal (reading 4)."""
+    rng = np.random.default_rng(47)
+    n = 12
+    W = H = 16
+    F, d = S.affine_camera(0.5, math.radians(20), 0.7, W, H, (4, 4, 0))
+    quats = rng.normal(0, 0.3, (n, 4)); quats[:, 0] += 1.5
+    common = _common_groups(rng, n)
+    Bp = (np.asarray(F, np.float64).reshape(2, 4) + common["dF"].reshape(2, 4))[:, :3]
+    ray = np.cross(Bp[0], Bp[1])            # the parallel-ray direction of F' = F + dF (PAPER.md:165)
+    edge = [2, 7]
+    for i in edge:                          # frame with the ray direction inside the surfel plane: t_u = ray
+        tu = ray / np.linalg.norm(ray)
+        tv = np.cross(rng.normal(0, 1, 3), tu); tv /= np.linalg.norm(tv)
+        nn = np.cross(tu, tv)
+        R = np.stack([tu, tv, nn], 1)
+        w = 0.5 * math.sqrt(max(1e-12, 1 + R[0, 0] + R[1, 1] + R[2, 2]))
+        quats[i] = [w, (R[2, 1] - R[1, 2]) / (4 * w), (R[0, 2] - R[2, 0]) / (4 * w), (R[1, 0] - R[0, 1]) / (4 * w)]
+    means = np.concatenate([rng.uniform(1.0, 7.0, (n, 2)), rng.normal(0, 1.0, (n, 1))], 1)
+    means[edge, 2] = [2.5, 1.8]            # in front of most of the others
+    logits = rng.normal(0.5, 1.0, n); logits[edge] = [1.5, 2.5]
+    P = dict(means=means, quats=quats, scales=rng.uniform(0.6, 2.0, (n, 2)), logits=logits, **common)
+    view, run = _branch_fd_problem(orc, P, hold_flags=True)
+    T = _pair_table(orc, view, P)
+    deg = (T["flags"] & orc.F_DEGENERATE) != 0
+    assert deg[edge].all() and deg.sum() == len(edge)
+    assert (T["aG"][..., deg] > 1e-2).sum() >= 10                   # the degenerate surfels are seen
+    out, _ = _check_fd(P, run, ["means", "quats", "scales", "logits", "rgb", "dF", "cc", "ambient"], rtol=2e-6)
+    assert out["counters"][4] == deg.sum() * W * H                  # cut-offs off: every pixel composites them
+    _, _, grads = run(P, need_grad=True)
+    assert np.all(grads["scales"][edge] == 0.0)                     # nothing flows through Q or g ...
+    assert np.abs(grads["means"][edge]).min() > 1e-6 and np.abs(grads["logits"][edge]).min() > 1e-6   # ... but the rest does
+    assert np.abs(grads["quats"][edge]).max() > 1e-6                # (the rotation still moves the blended normal)
+
+
 # ----------------------------------------------------------------------------------------- P11 / P12
 def test_p11_shadow_test_closed_form(orc):
     W = H = 24
@@ -704,10 +846,24 @@ def test_p16_depth_normals_of_a_world_plane():
             p0 = np.linalg.lstsq(B, x - b, rcond=None)[0]          # some point on the pixel's ray
             t = (n0 @ (q - p0)) / (n0 @ ray)
             zv[j, i] = b_z - (p0 + t * ray)[2]
-    N, _, interior, _ = losses.depth_normals(zv, Fp, d)
+    N, c, _, _, interior, sgn = losses.depth_normals(zv, Fp, d, b_z)
     expect = n0 if n0 @ np.asarray(d, np.float64) < 0 else -n0      # facing the sensor
     assert np.abs(N[interior] - expect).max() < 1e-9
     assert (N[~interior] == 0).all() and interior.sum() == (W - 2) * (H - 2)
+    # cross-check on a non-planar depth image: p_s is affine in z_v, so the cross product of the central differences
+    # factors as c = c0 + dx c1 + dy c2 with dx, dy the central differences of the depth alone (the form a kernel
+    # would evaluate); the oracle itself is Eq. 13 as written
+    rng = np.random.default_rng(9)
+    zv2 = zv + rng.normal(0, 0.3, zv.shape)
+    N2, c2_, _, _, _, _ = losses.depth_normals(zv2, Fp, d, b_z)
+    Bi = np.linalg.inv(Fp[:, :2])
+    k = np.array([*(Bi @ Fp[:, 2]), -1.0])
+    ax, ay = np.array([*(2.0 * Bi[:, 0]), 0.0]), np.array([*(2.0 * Bi[:, 1]), 0.0])
+    dx = zv2[1:-1, 2:] - zv2[1:-1, :-2]
+    dy = zv2[2:, 1:-1] - zv2[:-2, 1:-1]
+    fact = np.cross(ax, ay) + dx[..., None] * np.cross(k, ay) + dy[..., None] * np.cross(ax, k)
+    np.testing.assert_allclose(c2_[1:-1, 1:-1], fact, rtol=1e-10, atol=1e-12)
+    assert np.abs(np.linalg.norm(N2[1:-1, 1:-1], axis=-1) - 1).max() < 1e-12
 
 
 def test_p16_ssim_identities_and_brute_force_window():
