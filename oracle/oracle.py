@@ -222,9 +222,10 @@ def forward(width, height, b_z, z_bg, bg, rec, flags, lists, shading: Shading, o
 
 
 def backward(width, height, b_z, z_bg, bg, rec, flags, lists, shading: Shading, v_rgba, v_geom, v_aux,
-             options=0, threads=1):
+             options=0, threads=1, twin=False):
     """Analytic backward (step E) of epilogue + compositor.  Returns v_rec [N,16], v_cc [12], v_ambient [3],
-    v_reproj [8], v_sun_depth [Hs,Ws] or None."""
+    v_reproj [8], v_sun_depth [Hs,Ws] or None.  `twin`: also the absolute-value twins a_* of the same sums (the
+    rounding-error scale of every gradient value, see orc_backward)."""
     cfg, keep = _render_cfg(width, height, b_z, z_bg, bg, lists, options, threads)
     rec = _f64(rec)
     flags = np.ascontiguousarray(flags, np.uint8)
@@ -233,23 +234,42 @@ def backward(width, height, b_z, z_bg, bg, rec, flags, lists, shading: Shading, 
     v_sun = None if shading.sun_depth is None else np.zeros_like(shading.sun_depth)
     sh = shading.c()
     a = [None if x is None else _f64(x) for x in (v_rgba, v_geom, v_aux)]
+    tw = dict(a_rec=None, a_cc=None, a_ambient=None, a_reproj=None, a_sun_depth=None)
+    if twin:
+        tw = dict(a_rec=np.zeros_like(rec), a_cc=np.zeros(12), a_ambient=np.zeros(3), a_reproj=np.zeros(8),
+                  a_sun_depth=None if v_sun is None else np.zeros_like(v_sun))
     rc = lib().orc_backward(C.byref(cfg), C.byref(sh), _p(rec), _p(flags), _p(a[0]), _p(a[1]), _p(a[2]), _p(v_rec),
-                            _p(v_cc), _p(v_amb), _p(v_rep), _p(v_sun))
+                            _p(v_cc), _p(v_amb), _p(v_rep), _p(v_sun), _p(tw["a_rec"]), _p(tw["a_cc"]), _p(tw["a_ambient"]),
+                            _p(tw["a_reproj"]), _p(tw["a_sun_depth"]))
     assert rc == 0
     del keep
-    return dict(v_rec=v_rec, v_cc=v_cc, v_ambient=v_amb, v_reproj=v_rep, v_sun_depth=v_sun)
+    out = dict(v_rec=v_rec, v_cc=v_cc, v_ambient=v_amb, v_reproj=v_rep, v_sun_depth=v_sun)
+    if twin:
+        out.update(tw)
+    return out
 
 
-def preprocess_backward(view, means, quats, scales, logits, flags, v_rec, F=None, dF=None):
+def preprocess_backward(view, means, quats, scales, logits, flags, v_rec, F=None, dF=None, a_rec=None):
+    """Per-surfel chain.  With `a_rec` (the twin of v_rec from backward(twin=True)) also returns the twins a_means,
+    a_quats, a_scales, a_logits, a_rgb, a_dF."""
     n = means.shape[0]
     out = dict(v_means=np.zeros((n, 3)), v_quats=np.zeros((n, 4)), v_scales=np.zeros((n, 2)), v_logits=np.zeros(n),
                v_rgb=np.zeros((n, 3)), v_dF=np.zeros(8))
+    tw = dict(a_means=None, a_quats=None, a_scales=None, a_logits=None, a_rgb=None, a_dF=None)
+    if a_rec is not None:
+        a_rec = _f64(a_rec)
+        tw = dict(a_means=np.zeros((n, 3)), a_quats=np.zeros((n, 4)), a_scales=np.zeros((n, 2)), a_logits=np.zeros(n),
+                  a_rgb=np.zeros((n, 3)), a_dF=np.zeros(8))
     cam = _cam64(view, F, dF)
     rc = lib().orc_preprocess_backward(C.byref(cam), C.c_int64(n), _p(_f64(means)), _p(_f64(quats)), _p(_f64(scales)),
                                        _p(_f64(logits)), _p(np.ascontiguousarray(flags, np.uint8)), _p(_f64(v_rec)),
                                        _p(out["v_means"]), _p(out["v_quats"]), _p(out["v_scales"]),
-                                       _p(out["v_logits"]), _p(out["v_rgb"]), _p(out["v_dF"]))
+                                       _p(out["v_logits"]), _p(out["v_rgb"]), _p(out["v_dF"]), _p(a_rec),
+                                       _p(tw["a_means"]), _p(tw["a_quats"]), _p(tw["a_scales"]), _p(tw["a_logits"]),
+                                       _p(tw["a_rgb"]), _p(tw["a_dF"]))
     assert rc == 0
+    if a_rec is not None:
+        out.update(tw)
     return out
 
 
@@ -309,7 +329,7 @@ def render_pass(view, scene, *, tile_mode=True, threads=1):
 
 
 def view_iteration(scene, view, upstream=None, sun_upstream=None, *, tile_mode=True, threads=1,
-                   do_backward=True):
+                   do_backward=True, twin=False):
     """Full forward(+backward) of one view with record mode `float` (the fp32 record is the
     interface between preprocess and blend).  Returns a dict of outputs and gradients (all float64)."""
     res = {}
@@ -333,9 +353,9 @@ def view_iteration(scene, view, upstream=None, sun_upstream=None, *, tile_mode=T
         return res
     v_rgba, v_geom, v_aux = upstream
     bw = backward(view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, main["rec64"], main["flags"],
-                  main["lists"], shading, v_rgba, v_geom, v_aux, threads=threads)
+                  main["lists"], shading, v_rgba, v_geom, v_aux, threads=threads, twin=twin)
     g = preprocess_backward(view, scene.means, scene.quats, scene.scales, scene.opacity_logits, main["flags"],
-                            bw["v_rec"])
+                            bw["v_rec"], a_rec=bw.get("a_rec"))
     res.update(bwd=bw, grads=g)
     if view.shadows_on:
         v_sd = bw["v_sun_depth"]
@@ -345,8 +365,8 @@ def view_iteration(scene, view, upstream=None, sun_upstream=None, *, tile_mode=T
         vg = np.zeros((Hs, Ws, 4)); vg[..., 3] = v_sd             # sun_depth = D + (1 - A) z_bg
         vr = np.zeros((Hs, Ws, 4)); vr[..., 3] = -sun_view.z_bg * v_sd
         bs = backward(sun_view.width, sun_view.height, sun_view.b_z, sun_view.z_bg, np.zeros(3), sun["rec64"],
-                      sun["flags"], sun["lists"], Shading(), vr, vg, None, threads=threads)
+                      sun["flags"], sun["lists"], Shading(), vr, vg, None, threads=threads, twin=twin)
         gs = preprocess_backward(sun_view, scene.means, scene.quats, scene.scales, scene.opacity_logits,
-                                 sun["flags"], bs["v_rec"])
+                                 sun["flags"], bs["v_rec"], a_rec=bs.get("a_rec"))
         res.update(sun_bwd=bs, sun_grads=gs)
     return res

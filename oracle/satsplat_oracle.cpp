@@ -480,14 +480,26 @@ int orc_forward(const orc_render* cfg, const orc_shading* sh, const double* rec,
 // v_aux channels: (d median, d distortion, ignored, ignored).  All outputs are accumulated into (+=).
 // v_rec [N,16] in the canonical record layout (gradient w.r.t. the flipped normal as stored).
 // ---------------------------------------------------------------------------------------------------
+//
+// Rounding-error twin (tests only; every a_* pointer may be NULL).  a_rec [N,16], a_cc, a_ambient, a_reproj and
+// a_sun_depth receive, for every gradient value above, the sum of the ABSOLUTE values of the per-pixel / per-pair
+// terms that are added into it, each term itself being formed from absolute values of its factors (running error
+// analysis: a floating-point evaluation of the same sums in precision eps is off by at most c eps a_* for a modest
+// c that counts the operations per term and the length of the sum).  The twin is evaluated on the same gradient
+// written in the depth frame shifted to the pixel's first contributor (z - z_0) and with the distortion adjoint in
+// its centred form psi_i = A (z_i - m)^2 + (M2 - M1^2 / A), m = M1 / A: identical gradients, but their terms do not
+// carry the cancellation of the raw depths (z ~ b_z), so a_* measures the conditioning of the sums, not of that frame.
 int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec, const uint8_t* flags,
                  const double* v_rgba, const double* v_geom, const double* v_aux, double* v_rec,
-                 double* v_cc, double* v_ambient, double* v_reproj, double* v_sun_depth) {
+                 double* v_cc, double* v_ambient, double* v_reproj, double* v_sun_depth,
+                 double* a_rec, double* a_cc, double* a_ambient, double* a_reproj, double* a_sun_depth) {
   const int W = cfg->width, H = cfg->height;
 #pragma omp parallel num_threads(cfg->threads > 0 ? cfg->threads : 1)
   {
     std::vector<Hit> hits;
+    std::vector<double> aphi;
     double l_cc[12] = {0}, l_amb[3] = {0}, l_rep[8] = {0};
+    double t_cc[12] = {0}, t_amb[3] = {0}, t_rep[8] = {0};   // twins
 #pragma omp for schedule(dynamic, 4)
     for (int iy = 0; iy < H; ++iy) {
       for (int ix = 0; ix < W; ++ix) {
@@ -512,6 +524,9 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
           l_amb[c] += v_shade * (1 - E.V);
           for (int k = 0; k < 3; ++k) l_cc[4 * c + k] += v_albedoC[c] * E.albedo[k];
           l_cc[4 * c + 3] += v_albedoC[c];
+          t_amb[c] += std::fabs(v_shade * (1 - E.V));
+          for (int k = 0; k < 3; ++k) t_cc[4 * c + k] += std::fabs(v_albedoC[c] * E.albedo[k]);
+          t_cc[4 * c + 3] += std::fabs(v_albedoC[c]);
         }
         for (int k = 0; k < 3; ++k)
           v_albedo[k] = sh->cc[k] * v_albedoC[0] + sh->cc[4 + k] * v_albedoC[1] + sh->cc[8 + k] * v_albedoC[2];
@@ -528,6 +543,12 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
             atomic_add(&v_sun_depth[E.y1 * SW + E.x0], v_ds * E.fy * (1 - E.fx));
             atomic_add(&v_sun_depth[E.y1 * SW + E.x1], v_ds * E.fy * E.fx);
           }
+          if (a_sun_depth) {
+            atomic_add(&a_sun_depth[E.y0 * SW + E.x0], std::fabs(v_ds * (1 - E.fy) * (1 - E.fx)));
+            atomic_add(&a_sun_depth[E.y0 * SW + E.x1], std::fabs(v_ds * (1 - E.fy) * E.fx));
+            atomic_add(&a_sun_depth[E.y1 * SW + E.x0], std::fabs(v_ds * E.fy * (1 - E.fx)));
+            atomic_add(&a_sun_depth[E.y1 * SW + E.x1], std::fabs(v_ds * E.fy * E.fx));
+          }
           // d d_s / d x_s through the bilinear weights
           const double dds_dx = (1 - E.fy) * (D[E.y0 * SW + E.x1] - D[E.y0 * SW + E.x0]) + E.fy * (D[E.y1 * SW + E.x1] - D[E.y1 * SW + E.x0]);
           const double dds_dy = (1 - E.fx) * (D[E.y1 * SW + E.x0] - D[E.y0 * SW + E.x0]) + E.fx * (D[E.y1 * SW + E.x1] - D[E.y0 * SW + E.x1]);
@@ -537,6 +558,8 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
           for (int r = 0; r < 2; ++r) {
             l_rep[4 * r + 0] += v_xs[r] * px; l_rep[4 * r + 1] += v_xs[r] * py;
             l_rep[4 * r + 2] += v_xs[r] * E.h; l_rep[4 * r + 3] += v_xs[r];
+            t_rep[4 * r + 0] += std::fabs(v_xs[r] * px); t_rep[4 * r + 1] += std::fabs(v_xs[r] * py);
+            t_rep[4 * r + 2] += std::fabs(v_xs[r] * E.h); t_rep[4 * r + 3] += std::fabs(v_xs[r]);
           }
           vD += v_zv;             // z_v = D + T_f z_bg
           vT += cfg->z_bg * v_zv;
@@ -546,6 +569,11 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
         // ---- compositor backward, reverse order ----
         const double A = 1 - S.T, M1 = S.M1, M2 = S.M2, Tf = S.T;
         double Ssum = 0;  // sum_{k>i} w_k phi_k
+        // twin: shifted depth frame and centred distortion adjoint (see the header of this function)
+        const double z0 = hits.empty() ? 0.0 : hits[0].z;
+        const double zm = A > 0 ? M1 / A : 0.0, zvar = A > 0 ? std::max(M2 - M1 * M1 / A, 0.0) : 0.0;
+        const double t_vT = std::fabs(vT - vD * z0);   // per-pixel scalars enter the twin by their absolute value
+        double t_Ssum = 0;
         for (int64_t h = (int64_t)hits.size() - 1; h >= 0; --h) {
           const Hit& X = hits[h];
           const double* r = rec + R_SIZE * X.id;
@@ -560,6 +588,34 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
           double v_G = 0;
           if (!X.clamped) { atomic_add(&g[R_ALPHA], X.G * v_a); v_G = r[R_ALPHA] * v_a; }
           const double v_rho = -0.5 * X.G * v_G;
+          if (a_rec) {
+            double* t = a_rec + R_SIZE * X.id;
+            const double dzm = X.z - zm;
+            double t_phi = std::fabs(vD * (X.z - z0)) + std::fabs(vL) * (A * dzm * dzm + zvar);
+            for (int c = 0; c < 3; ++c) t_phi += std::fabs(v_albedo[c] * r[R_R + c]) + std::fabs(vN[c] * r[R_NX + c]);
+            const double t_va = X.T * t_phi + (t_Ssum + Tf * t_vT) / (1 - X.a);
+            t_Ssum += X.w * t_phi;
+            for (int c = 0; c < 3; ++c) { atomic_add(&t[R_R + c], std::fabs(X.w * v_albedo[c])); atomic_add(&t[R_NX + c], std::fabs(X.w * vN[c])); }
+            const double t_vz = X.w * (std::fabs(vD) + 2 * std::fabs(vL) * A * std::fabs(dzm)) + ((int32_t)X.id == S.mi ? std::fabs(vmed) : 0.0);
+            double t_vG = 0;
+            if (!X.clamped) { atomic_add(&t[R_ALPHA], X.G * t_va); t_vG = r[R_ALPHA] * t_va; }
+            const double t_vrho = 0.5 * X.G * t_vG;
+            atomic_add(&t[R_ZC], t_vz);
+            double t_vd[2];
+            if (!X.lowpass) {
+              const double tu = 2 * std::fabs(X.u) * t_vrho, tv = 2 * std::fabs(X.v) * t_vrho;
+              atomic_add(&t[R_G0], t_vz * std::fabs(X.dx)); atomic_add(&t[R_G1], t_vz * std::fabs(X.dy));
+              t_vd[0] = t_vz * std::fabs(r[R_G0]) + std::fabs(r[R_Q00]) * tu + std::fabs(r[R_Q10]) * tv;
+              t_vd[1] = t_vz * std::fabs(r[R_G1]) + std::fabs(r[R_Q01]) * tu + std::fabs(r[R_Q11]) * tv;
+              atomic_add(&t[R_Q00], tu * std::fabs(X.dx)); atomic_add(&t[R_Q01], tu * std::fabs(X.dy));
+              atomic_add(&t[R_Q10], tv * std::fabs(X.dx)); atomic_add(&t[R_Q11], tv * std::fabs(X.dy));
+            } else {
+              t_vd[0] = 2 * kInvSigma2 * std::fabs(X.dx) * t_vrho;
+              t_vd[1] = 2 * kInvSigma2 * std::fabs(X.dy) * t_vrho;
+            }
+            atomic_add(&t[R_CX], t_vd[0]);
+            atomic_add(&t[R_CY], t_vd[1]);
+          }
           double v_d[2];
           atomic_add(&g[R_ZC], v_z);
           if (!X.lowpass) {
@@ -583,6 +639,9 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
       if (v_cc) for (int k = 0; k < 12; ++k) v_cc[k] += l_cc[k];
       if (v_ambient) for (int k = 0; k < 3; ++k) v_ambient[k] += l_amb[k];
       if (v_reproj) for (int k = 0; k < 8; ++k) v_reproj[k] += l_rep[k];
+      if (a_cc) for (int k = 0; k < 12; ++k) a_cc[k] += t_cc[k];
+      if (a_ambient) for (int k = 0; k < 3; ++k) a_ambient[k] += t_amb[k];
+      if (a_reproj) for (int k = 0; k < 8; ++k) a_reproj[k] += t_rep[k];
     }
   }
   return 0;
@@ -592,12 +651,76 @@ int orc_backward(const orc_render* cfg, const orc_shading* sh, const double* rec
 // E (per-surfel chain): record gradients -> gradients of (p, q, s, logit, rgb) and of dF (Eq. 15).
 // All outputs accumulated into (+=).
 // ---------------------------------------------------------------------------------------------------
+// Twin (tests only; a_rec NULL = off): the absolute sums a_rec of orc_backward pushed through the absolute values of
+// the same chain, term by term, into a_means ... a_dF (accumulated into).
 int orc_preprocess_backward(const orc_cam_f64* cam, int64_t N, const double* means, const double* quats,
                             const double* scales, const double* logits, const uint8_t* flags,
                             const double* v_rec, double* v_means, double* v_quats, double* v_scales,
-                            double* v_logits, double* v_rgb, double* v_dF) {
+                            double* v_logits, double* v_rgb, double* v_dF,
+                            const double* a_rec, double* a_means, double* a_quats, double* a_scales,
+                            double* a_logits, double* a_rgb, double* a_dF) {
   for (int64_t i = 0; i < N; ++i) {
     if (flags[i] & F_CULLED) continue;
+    if (a_rec) {
+      const double* p = means + 3 * i;
+      const double* q = quats + 4 * i;
+      const double* sc = scales + 2 * i;
+      const double* t = a_rec + R_SIZE * i;
+      SurfelGeom G;
+      surfel_geom(cam, p, q, sc, G);
+      auto ab = [](double x) { return std::fabs(x); };
+      const double alpha = 1.0 / (1.0 + std::exp(-logits[i]));
+      a_logits[i] += t[R_ALPHA] * alpha * (1 - alpha);
+      for (int c = 0; c < 3; ++c) a_rgb[3 * i + c] += t[R_R + c];
+      double t_tu[3] = {0, 0, 0}, t_tv[3] = {0, 0, 0};
+      const double t_n[3] = {t[R_NX], t[R_NY], t[R_NZ]};
+      const double t_c[2] = {t[R_CX], t[R_CY]};
+      double t_B[2][3] = {{0, 0, 0}, {0, 0, 0}};
+      if (!(flags[i] & F_DEGENERATE)) {
+        double tQ[2][2] = {{t[R_Q00], t[R_Q01]}, {t[R_Q10], t[R_Q11]}};
+        const double tg[2] = {t[R_G0], t[R_G1]};
+        double t_r[2];
+        for (int a = 0; a < 2; ++a) {
+          t_r[a] = tg[0] * ab(G.Q[a][0]) + tg[1] * ab(G.Q[a][1]);
+          for (int b = 0; b < 2; ++b) tQ[a][b] += ab(G.r[a]) * tg[b];
+        }
+        double tmp[2][2], tM[2][2];
+        for (int a = 0; a < 2; ++a)
+          for (int b = 0; b < 2; ++b) tmp[a][b] = ab(G.Q[0][a]) * tQ[0][b] + ab(G.Q[1][a]) * tQ[1][b];
+        for (int a = 0; a < 2; ++a)
+          for (int b = 0; b < 2; ++b) tM[a][b] = tmp[a][0] * ab(G.Q[b][0]) + tmp[a][1] * ab(G.Q[b][1]);
+        a_scales[2 * i] += tM[0][0] * ab(G.au[0]) + tM[1][0] * ab(G.au[1]) + t_r[0] * ab(G.tu[2]);
+        a_scales[2 * i + 1] += tM[0][1] * ab(G.av[0]) + tM[1][1] * ab(G.av[1]) + t_r[1] * ab(G.tv[2]);
+        const double t_au[2] = {sc[0] * tM[0][0], sc[0] * tM[1][0]};
+        const double t_av[2] = {sc[1] * tM[0][1], sc[1] * tM[1][1]};
+        for (int c = 0; c < 3; ++c) {
+          t_tu[c] += ab(G.B[0][c]) * t_au[0] + ab(G.B[1][c]) * t_au[1];
+          t_tv[c] += ab(G.B[0][c]) * t_av[0] + ab(G.B[1][c]) * t_av[1];
+          for (int r = 0; r < 2; ++r) t_B[r][c] += t_au[r] * ab(G.tu[c]) + t_av[r] * ab(G.tv[c]);
+        }
+        t_tu[2] += sc[0] * t_r[0];
+        t_tv[2] += sc[1] * t_r[1];
+      }
+      for (int c = 0; c < 3; ++c) {
+        a_means[3 * i + c] += ab(G.B[0][c]) * t_c[0] + ab(G.B[1][c]) * t_c[1];
+        for (int r = 0; r < 2; ++r) t_B[r][c] += t_c[r] * ab(p[c]);
+      }
+      a_means[3 * i + 2] += t[R_ZC];
+      for (int r = 0; r < 2; ++r) {
+        for (int c = 0; c < 3; ++c) a_dF[4 * r + c] += t_B[r][c];
+        a_dF[4 * r + 3] += t_c[r];
+      }
+      const double Gm[3][3] = {{t_tu[0], t_tv[0], t_n[0]}, {t_tu[1], t_tv[1], t_n[1]}, {t_tu[2], t_tv[2], t_n[2]}};
+      const double w = ab(G.w), x = ab(G.x), y = ab(G.y), z = ab(G.z);
+      double tq[4];
+      tq[0] = 2 * (x * (Gm[2][1] + Gm[1][2]) + y * (Gm[0][2] + Gm[2][0]) + z * (Gm[1][0] + Gm[0][1]));
+      tq[1] = 2 * (2 * x * (Gm[1][1] + Gm[2][2]) + y * (Gm[0][1] + Gm[1][0]) + z * (Gm[0][2] + Gm[2][0]) + w * (Gm[2][1] + Gm[1][2]));
+      tq[2] = 2 * (x * (Gm[0][1] + Gm[1][0]) + 2 * y * (Gm[0][0] + Gm[2][2]) + z * (Gm[1][2] + Gm[2][1]) + w * (Gm[0][2] + Gm[2][0]));
+      tq[3] = 2 * (x * (Gm[0][2] + Gm[2][0]) + y * (Gm[1][2] + Gm[2][1]) + 2 * z * (Gm[0][0] + Gm[1][1]) + w * (Gm[1][0] + Gm[0][1]));
+      const double qh[4] = {w, x, y, z};
+      const double dotq = qh[0] * tq[0] + qh[1] * tq[1] + qh[2] * tq[2] + qh[3] * tq[3];
+      for (int k = 0; k < 4; ++k) a_quats[4 * i + k] += (tq[k] + qh[k] * dotq) / G.qn;
+    }
     const double* p = means + 3 * i;
     const double* q = quats + 4 * i;
     const double* s = scales + 2 * i;

@@ -639,6 +639,49 @@ def test_p8d_degenerate_surfels_pass_no_gradient_through_Q_and_g(orc):
     assert np.abs(grads["quats"][edge]).max() > 1e-6                # (the rotation still moves the blended normal)
 
 
+# ------------------------------------------------------------------------------- P19: the rounding-error twin
+def test_p19_absolute_value_twin_bounds_and_is_not_vacuous(c0, orc):
+    """The a_* twins of the backward (sum of |per-pair term| pushed through |chain Jacobian|) are what the GPU
+    parity bar scales its rounding allowance with, so they are pinned by what the mathematics fixes:
+    (a) triangle inequality: a >= |v| for every gradient value;
+    (b) a == v where every term has the same sign (colour gradient under a non-negative upstream image);
+    (c) the gradients are linear in the upstream images: scaling the upstream of every pixel by its own factor
+        (1 + d_p), |d_p| <= delta, moves no gradient value by more than delta * a;
+    (d) not vacuous: on C0 the typical a / |v| is a small number."""
+    scene, view, tile = c0[0], c0[1], c0[2]
+    up = S.upstream_grads(scene.seed, 0, view.height, view.width)
+    sh = orc.Shading(cc=view.cc, ambient=view.ambient)
+    args = (view.width, view.height, view.b_z, view.z_bg, view.bg_rgb, tile["rec64"], tile["flags"], tile["lists"], sh)
+
+    def grads(upstream, twin):
+        bw = orc.backward(*args, *upstream, threads=orc.num_threads(), twin=twin)
+        g = orc.preprocess_backward(view, scene.means, scene.quats, scene.scales, scene.opacity_logits, tile["flags"],
+                                    bw["v_rec"], a_rec=bw.get("a_rec"))
+        g.update(v_cc=bw["v_cc"], v_ambient=bw["v_ambient"])
+        if twin:
+            g.update(a_cc=bw["a_cc"], a_ambient=bw["a_ambient"])
+        return g
+
+    g = grads(up, True)
+    names = ["means", "quats", "scales", "logits", "rgb", "dF", "cc"]
+    for k in names:
+        v, a = g["v_" + k], g["a_" + k]
+        assert (a >= np.abs(v) * (1 - 1e-12) - 1e-300).all(), k                              # (a)
+        if v.size > 32:     # per-surfel groups (the global sums dF, cc cancel over a thousand surfels by themselves)
+            nz = np.abs(v) > 1e-9 * np.abs(v).max()
+            assert np.median(a[nz] / np.abs(v[nz])) < 25, (k, np.median(a[nz] / np.abs(v[nz])))  # (d)
+    rng = np.random.default_rng(5)
+    delta = 1e-3
+    fac = 1 + delta * rng.choice([-1.0, 1.0], (view.height, view.width, 1))
+    g2 = grads([u * fac for u in up], False)
+    for k in names:
+        assert (np.abs(g2["v_" + k] - g["v_" + k]) <= delta * g["a_" + k] * (1 + 1e-9) + 1e-18).all(), k   # (c)
+    pos = [np.abs(up[0]) * np.array([1, 1, 1, 0.0]), None, None]
+    gp = grads(pos, True)
+    np.testing.assert_allclose(gp["a_rgb"], np.abs(gp["v_rgb"]), rtol=1e-12, atol=1e-300)      # (b): w v_albedo >= 0 ...
+    assert (gp["v_rgb"] >= 0).all() and gp["v_rgb"].max() > 0                                  # ... with C0's identity CC
+
+
 # ----------------------------------------------------------------------------------------- P11 / P12
 def test_p11_shadow_test_closed_form(orc):
     W = H = 24
