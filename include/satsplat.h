@@ -294,6 +294,12 @@ const char* satsplat_version(void);
 /* Cumulative number of CUDA kernels this library has launched in this process (all contexts). */
 int64_t satsplat_kernel_launches(void);
 
+/* The two issue-rate peaks the blend kernels' roofline is quoted against, MEASURED on `device` by
+ * two micro-benchmark kernels: FP32 lane-instructions per second (independent FFMA chains on every sub-partition)
+ * and MUFU operations per second (independent ex2.approx chains).  HOST outputs; sm_count may be NULL.  Synchronises
+ * the device (a few milliseconds): a measurement utility for bench.py, not part of the hot path. */
+int satsplat_measure_peaks(int device, double* fp32_lane_inst_per_s, double* mufu_per_s, int* sm_count);
+
 #ifdef __cplusplus
 }
 #endif

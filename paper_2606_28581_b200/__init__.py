@@ -130,12 +130,22 @@ def lib():
         L.satsplat_set_profiling.argtypes = [vp, i32]
         L.satsplat_set_option.argtypes = [vp, i32, i32]
         L.satsplat_stage_ms.argtypes = [vp, C.POINTER(f32)]
+        L.satsplat_measure_peaks.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
         _LIB = L
     return _LIB
 
 
 def kernel_launches() -> int:
     return int(lib().satsplat_kernel_launches())
+
+
+def measure_peaks(device: int = 0) -> dict:
+    """satsplat_measure_peaks: measured FP32 lane-instructions/s and MUFU operations/s of `device`."""
+    a, b, n = C.c_double(0), C.c_double(0), C.c_int(0)
+    rc = lib().satsplat_measure_peaks(int(device), C.byref(a), C.byref(b), C.byref(n))
+    if rc != 0:
+        raise SatsplatError(rc, "satsplat_measure_peaks failed")
+    return dict(fp32_lane_inst_per_s=a.value, mufu_per_s=b.value, sm_count=n.value)
 
 
 def version() -> str:

@@ -14,7 +14,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libsatsplat.so")
-SOURCES = ["api.cu", "preprocess.cu", "binning.cu", "blend_forward.cu", "blend_backward.cu", "chain_backward.cu", "adam.cu", "losses.cu", "init.cu", "relocate.cu"]
+SOURCES = ["api.cu", "preprocess.cu", "binning.cu", "blend_forward.cu", "blend_backward.cu", "chain_backward.cu", "adam.cu", "losses.cu", "init.cu", "relocate.cu", "peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr"]
 
@@ -33,7 +33,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, *( ["-Xptxas", "-v"] if verbose else []), "-c", os.path.join(CSRC, src), "-o", obj]
+        extra = os.environ.get("SATSPLAT_NVCC_FLAGS", "").split()     # e.g. -DSATSPLAT_BWD_MINB=8 (tuning experiments)
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *( ["-Xptxas", "-v"] if verbose else []), "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")

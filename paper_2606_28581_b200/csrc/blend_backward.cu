@@ -324,20 +324,15 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
     __syncwarp();
     // the depth-only pass evaluates two survivors per trip (independent instruction streams for the scheduler) and
     // composites them in order; the view pass has no registers to spare for that and takes them one by one
-    struct Eval { const float4* e; int2 ji; float dx, dy, u, v, rho3, rho2, aG, a, zc; bool active; };
+    struct Eval { const float4* e; int2 ji; PairEval p; float zc; bool active; };
     auto evaluate = [&](int sv) -> Eval {
       Eval E;
       E.e = wrec[sv];
       E.ji = widx[sv];
       const float4 r0 = E.e[0], r1 = E.e[1];
-      E.dx = px - r0.x; E.dy = py - r0.y;
-      E.u = r0.z * E.dx + r0.w * E.dy; E.v = r1.x * E.dx + r1.y * E.dy;
-      E.rho3 = E.u * E.u + E.v * E.v; E.rho2 = 2.0f * (E.dx * E.dx + E.dy * E.dy);
-      const float rho = fminf(E.rho3, E.rho2);
-      E.aG = r1.z * fast_exp2(rho * kNegHalfLog2e);
-      E.a = fminf(kAlphaMax, E.aG);
+      E.p = pair_eval(r0, r1, px, py);       // the forward's arithmetic, bit for bit: same decisions
       E.zc = r1.w;
-      E.active = (E.ji.x < last) && (rho <= kRhoCut) && (E.a >= kAlphaMin);
+      E.active = (E.ji.x < last) && (E.p.rho <= kRhoCut) && (E.p.a >= kAlphaMin);
       return E;
     };
     auto composite = [&](const Eval& E) {
@@ -345,12 +340,12 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       if (hm == 0) return;
       if (E.active) {
         const float4 r2 = E.e[2];
-        const bool lowpass = !(E.rho3 <= E.rho2);
-        const float z = lowpass ? E.zc : E.zc + (r2.x * E.dx + r2.y * E.dy);
+        const bool lowpass = !(E.p.rho3 <= E.p.rho2);
+        const float z = pair_depth(E.p, E.zc, r2.x, r2.y);
         const float zs = z - zref;
-        const float rc = fast_rcp(1.0f - E.a);
+        const float rc = fast_rcp(1.0f - E.p.a);
         const float Ti = T * rc;
-        const float w = E.a * Ti;
+        const float w = E.p.a * Ti;
         float phi, v_z;
         if (DEPTH_ONLY) {
           phi = vD * zs;
@@ -366,10 +361,10 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
         const float v_a = Ti * phi - (Ssum + TfvT) * rc;
         Ssum += w * phi;
         T = Ti;
-        const float v_rho = (E.aG < kAlphaMax) ? -0.5f * E.aG * v_a : 0.f;   // alpha' = alpha G unless clamped
+        const float v_rho = (E.p.aG < kAlphaMax) ? -0.5f * E.p.aG * v_a : 0.f;   // alpha' = alpha G unless clamped
         const int pos = nseg * 32 + __popc(hm & lt_mask);
         p4[pos] = make_float4(v_rho, v_z, w, __int_as_float(lane | (lowpass ? 32 : 0)));
-        p2[pos] = lowpass ? make_float2(E.dx, E.dy) : make_float2(E.u, E.v);
+        p2[pos] = lowpass ? make_float2(E.p.dx, E.p.dy) : make_float2(E.p.u, E.p.v);
       }
       const int cnt = __popc(hm);
       if (team == nseg) { my_cnt = cnt; my_id = (uint32_t)E.ji.y; }

@@ -133,19 +133,15 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
       const int j = __ffs(m) - 1;
       m &= m - 1;
       const float4 r0 = s_r0[buf][warp][j], r1 = s_r1[buf][warp][j];
-      const float dx = px - r0.x, dy = py - r0.y;
-      const float u = r0.z * dx + r0.w * dy, v = r1.x * dx + r1.y * dy;       // Eq. 9
-      const float rho3 = u * u + v * v, rho2 = 2.0f * (dx * dx + dy * dy);    // Eq. 12, sigma^2 = 1/2
-      const float rho = fminf(rho3, rho2);
-      if (!(rho <= kRhoCut)) continue;
-      const float G = fast_exp2(rho * kNegHalfLog2e);                         // exp(-rho/2)
-      const float a = fminf(kAlphaMax, r1.z * G);
+      const PairEval E = pair_eval(r0, r1, px, py);                           // Eq. 9, Eq. 12
+      if (!(E.rho <= kRhoCut)) continue;
+      const float a = E.a;
       if (a < kAlphaMin) continue;
       const float Tn = T * (1.0f - a);
       if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
       const float w = a * T;
       const float4 r2 = s_r2[buf][warp][j];
-      const float z = (rho3 <= rho2) ? r1.w + (r2.x * dx + r2.y * dy) : r1.w;   // Eq. 6 depth at the intersection
+      const float z = pair_depth(E, r1.w, r2.x, r2.y);                        // Eq. 6 depth at the intersection
       if (DEPTH_ONLY) {
         M1 += w * z;
       } else {

@@ -99,7 +99,9 @@ __device__ __forceinline__ float4 splat_bbox(const float4 r0, const float4 r1) {
 }
 
 // Shadow-test lookup shared by the forward epilogue and its backward so that both take the same in-map /
-// texel decisions from the same bits (explicit fma sequence: no compiler-dependent contraction).
+// texel decisions from the same bits.  The reprojection x_s = R_x x + k_h h + k_0 is evaluated
+// in double precision: at 2048 px an fp32 x_s carries ~1e-4 px of rounding, which a building edge in the sun map
+// (tens of metres per texel) turns into a visible error of the soft test and of every gradient through it.
 struct ShadowTap {
   bool in_map;
   int x0, y0, x1, y1;
@@ -109,17 +111,43 @@ __device__ __forceinline__ ShadowTap shadow_tap(const DevShading& sh, const DevC
   ShadowTap t;
   t.zv = __fmaf_rn(T, cam.z_bg, D);          // z_v = D + T_f z_bg
   t.h = __fsub_rn(cam.b_z, t.zv);            // world height seen at this pixel
-  const float xs = __fmaf_rn(sh.reproj[2], t.h, __fmaf_rn(sh.reproj[1], py, __fmaf_rn(sh.reproj[0], px, sh.reproj[3])));
-  const float ys = __fmaf_rn(sh.reproj[6], t.h, __fmaf_rn(sh.reproj[5], py, __fmaf_rn(sh.reproj[4], px, sh.reproj[7])));
-  t.in_map = xs >= 0.5f && xs <= (float)sh.sun_w - 0.5f && ys >= 0.5f && ys <= (float)sh.sun_h - 0.5f;
-  const float tx = xs - 0.5f, ty = ys - 0.5f;
-  t.x0 = min(max((int)floorf(tx), 0), sh.sun_w - 1);
-  t.y0 = min(max((int)floorf(ty), 0), sh.sun_h - 1);
-  t.fx = tx - (float)t.x0;
-  t.fy = ty - (float)t.y0;
+  const double dpx = (double)px, dpy = (double)py, dh = (double)t.h;
+  const double xs = fma((double)sh.reproj[2], dh, fma((double)sh.reproj[1], dpy, fma((double)sh.reproj[0], dpx, (double)sh.reproj[3])));
+  const double ys = fma((double)sh.reproj[6], dh, fma((double)sh.reproj[5], dpy, fma((double)sh.reproj[4], dpx, (double)sh.reproj[7])));
+  t.in_map = xs >= 0.5 && xs <= (double)sh.sun_w - 0.5 && ys >= 0.5 && ys <= (double)sh.sun_h - 0.5;
+  const double tx = xs - 0.5, ty = ys - 0.5;
+  // clamp in double before the conversion (far outside the map the product would overflow an int)
+  t.x0 = (int)fmin(fmax(floor(tx), 0.0), (double)(sh.sun_w - 1));
+  t.y0 = (int)fmin(fmax(floor(ty), 0.0), (double)(sh.sun_h - 1));
+  t.fx = (float)(tx - (double)t.x0);
+  t.fy = (float)(ty - (double)t.y0);
   t.x1 = min(t.x0 + 1, sh.sun_w - 1);
   t.y1 = min(t.y0 + 1, sh.sun_h - 1);
   return t;
+}
+
+// Per-(pixel, surfel) evaluation of Eq. 9 / Eq. 12, shared by the forward and the backward blend so that both take
+// the same decisions (rho cut, alpha skip, depth branch, clamp) from the same bits: every operation is an explicitly
+// rounded intrinsic, so the result does not depend on the contraction choices of the compiler in either kernel.
+struct PairEval {
+  float dx, dy, u, v, rho3, rho2, rho, aG, a;
+};
+__device__ __forceinline__ PairEval pair_eval(const float4 r0, const float4 r1, float px, float py) {
+  PairEval E;
+  E.dx = __fsub_rn(px, r0.x);
+  E.dy = __fsub_rn(py, r0.y);
+  E.u = __fmaf_rn(r0.z, E.dx, __fmul_rn(r0.w, E.dy));                       // Eq. 9: (u, v) = Q (x - c)
+  E.v = __fmaf_rn(r1.x, E.dx, __fmul_rn(r1.y, E.dy));
+  E.rho3 = __fmaf_rn(E.u, E.u, __fmul_rn(E.v, E.v));
+  E.rho2 = __fmul_rn(2.0f, __fmaf_rn(E.dx, E.dx, __fmul_rn(E.dy, E.dy)));   // Eq. 12 low-pass term, sigma^2 = 1/2
+  E.rho = fminf(E.rho3, E.rho2);
+  E.aG = __fmul_rn(r1.z, fast_exp2(__fmul_rn(E.rho, kNegHalfLog2e)));      // alpha exp(-rho / 2)
+  E.a = fminf(kAlphaMax, E.aG);
+  return E;
+}
+// depth of the pair (Eq. 6 at the intersection; the centre depth where the low-pass term wins)
+__device__ __forceinline__ float pair_depth(const PairEval& E, float zc, float g0, float g1) {
+  return (E.rho3 <= E.rho2) ? __fadd_rn(zc, __fmaf_rn(g0, E.dx, __fmul_rn(g1, E.dy))) : zc;
 }
 
 }  // namespace satsplat

@@ -45,11 +45,51 @@ def _scene(cfg):
         return S.make_config(3, n=40000, size=384, n_views=1, extent=200.0, sun_size=384)
     if cfg == "C4s":
         return S.make_config(4, n=40000, size=512, n_views=1, extent=250.0)
+    if cfg == "C1full":               # BASELINE.json configs[1] at full size (200k surfels, 512^2 views, dF and CC gradients)
+        return S.make_config(1, n_views=3)
+    if cfg == "C2full":               # BASELINE.json configs[2] at full size (C1 scene, 1024^2 sun maps)
+        return S.make_config(2, n_views=2)
+    if cfg == "C0_branches":          # the three branches of Eq. 12's backward, populated on purpose (pins P8b-d)
+        return _branch_scene()
     if cfg == "C3full":               # BASELINE.json configs[3] at full size (1M surfels, 2048^2), the bench workload
         return S.make_config(3, n_views=1)
     if cfg == "C4full":               # BASELINE.json configs[4] at full size (4M surfels, 4096^2, oversized splats)
         return S.make_config(4, n_views=1)
     raise KeyError(cfg)
+
+
+def _branch_scene():
+    """C0 with three hand-made populations: nearly opaque large surfels (alpha' sits on the 0.99 clamp), sub-pixel and
+    needle-like steeply tilted surfels (the low-pass term of Eq. 12 wins), and surfels whose plane contains the viewing
+    ray (det(B'RS') = 0: degenerate, PAPER.md:126)."""
+    sc = S.make_config(0)
+    rng = np.random.default_rng(77)
+    view = sc.views[0]
+    n = sc.n
+    a, b, c_ = slice(0, 64), slice(64, 192), slice(192, 224)
+    # alpha G >= 0.99 needs rho <= 2 ln(alpha / 0.99) ~ 0.02: large splats (sigma 8-16 px) so that the clamped core spans
+    # several pixels; placed below the rest of the scene so that they are composited last and hide nothing
+    sc.opacity_logits[a] = rng.uniform(8.0, 12.0, 64).astype(np.float32)
+    sc.scales[a] = rng.uniform(4.0, 8.0, (64, 2)).astype(np.float32)
+    sc.means[a, 2] = rng.uniform(-9.0, -7.0, 64).astype(np.float32)
+    nb = 128
+    sc.scales[b] = np.where((np.arange(nb) % 2 == 0)[:, None], rng.uniform(0.05, 0.2, (nb, 2)),
+                            np.stack([rng.uniform(0.06, 0.2, nb), rng.uniform(1.0, 2.5, nb)], 1)).astype(np.float32)
+    ang = rng.uniform(0.0, math.radians(70), nb)
+    axis = rng.normal(0, 1, (nb, 3)); axis[:, 2] *= 0.3
+    axis /= np.linalg.norm(axis, axis=1, keepdims=True)
+    sc.quats[b] = np.concatenate([np.cos(ang / 2)[:, None], np.sin(ang / 2)[:, None] * axis], 1).astype(np.float32)
+    sc.opacity_logits[b] = rng.normal(1.5, 0.7, nb).astype(np.float32)
+    Fp = (view.F.astype(np.float32) + view.dF.astype(np.float32)).astype(np.float64).reshape(2, 4)
+    ray = np.cross(Fp[0, :3], Fp[1, :3]); ray /= np.linalg.norm(ray)
+    for i in range(192, 224):                   # frame with t_u = the parallel-ray direction (edge-on)
+        tv = np.cross(rng.normal(0, 1, 3), ray); tv /= np.linalg.norm(tv)
+        R = np.stack([ray, tv, np.cross(ray, tv)], 1)
+        w = 0.5 * math.sqrt(max(1e-12, 1 + R[0, 0] + R[1, 1] + R[2, 2]))
+        sc.quats[i] = [w, (R[2, 1] - R[1, 2]) / (4 * w), (R[0, 2] - R[2, 0]) / (4 * w), (R[1, 0] - R[0, 1]) / (4 * w)]
+    sc.scales[c_] = rng.uniform(0.05, 0.3, (32, 2)).astype(np.float32)
+    sc.opacity_logits[c_] = rng.normal(1.5, 0.7, 32).astype(np.float32)
+    return sc
 
 
 def _no_shadow(view):
@@ -59,7 +99,7 @@ def _no_shadow(view):
     return v
 
 
-@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s", "C3full", "C4full"])
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C0_branches", "C1s", "C3s", "C4s", "C1full", "C3full", "C4full"])
 def test_binning_and_records_bitexact(P, G, orc, cfg):
     scene = _scene(cfg)
     gs = G.GpuScene(scene)
@@ -104,7 +144,7 @@ def test_long_tile_lists_bitexact(P, G, orc, n, size):
     G.assert_bins_bitexact(ref, res["bins"], scene.n)
 
 
-@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C1s", "C3s", "C4s", "C3full", "C4full"])
+@pytest.mark.parametrize("cfg", ["C0", "C0_ragged", "C0_branches", "C1s", "C3s", "C4s", "C1full", "C3full", "C4full"])
 def test_forward_backward_parity(P, G, orc, cfg):
     scene = _scene(cfg)
     gs = G.GpuScene(scene)
@@ -113,62 +153,48 @@ def test_forward_backward_parity(P, G, orc, cfg):
         view = _no_shadow(view)
         up = S.upstream_grads(scene.seed, vi, view.height, view.width)
         ref = orc.view_iteration(scene, view, do_backward=False, threads=nth)
+        if cfg == "C0_branches":     # all three branches of Eq. 12's backward are populated (contributing pairs of each kind)
+            cnt = ref["fwd"]["counters"]
+            assert cnt[2] > 200 and cnt[3] > 100 and cnt[4] > 20, cnt
+            assert ((ref["main_pass"]["flags"] & 2) != 0).sum() >= 16
         fragile = G.fragile_mask(ref["fwd"]["margins"])
         res = G.gpu_view_iteration(P, gs, view, do_backward=False)
-        # fragility is per decision: C4's 20 composited pairs per pixel (C3: 7) put 0.52 % of the pixels within the
-        # margins of some cut-off, just above the 0.5 % bound used for the other configs
-        stats = G.compare_images(res, ref["fwd"], fragile, max_fragile_frac=1.5e-2 if cfg == "C4full" else 5e-3)
+        # fragility is per decision: C4's 20 composited pairs per pixel (C3: 7) and C1's flat-ground tie density put
+        # 0.5-1.2 % of the pixels within the margins of some cut-off
+        stats = G.compare_images(res, ref["fwd"], fragile, max_fragile_frac=1.5e-2 if cfg in ("C4full", "C1full", "C0_branches") else 5e-3)
         # pair counts: same decisions on every non-fragile pixel
         ok = ~fragile
         assert np.array_equal(res["n_visited"][ok], ref["fwd"]["last"][ok])
         assert int(res["n_contrib"][ok].sum()) > 0
-        # ---- gradients, upstream masked on fragile pixels ----
+        # ---- gradients, upstream masked on fragile pixels: ONE bar, every element, no share allowed to miss it ----
         upm = [u.copy() for u in up]
         for u in upm:
             u[fragile] = 0
-        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth, twin=True)
         resb = G.gpu_view_iteration(P, gs, view, upstream=upm, want_debug=False)
-        gg, gr = resb["grads"], refb["grads"]
-        if cfg == "C4full":
-            # C4's 0.1 % tail of 10-40 m splats covers 10^3-10^4 pixels each: their gradients are fp32 sums of 10^4-10^5
-            # signed pair terms that cancel to ~1e-5 of their magnitude.  The per-surfel bar is asserted on the body of
-            # the distribution (scales <= 5 m); the oversized rows get the same bar relative to 50x their row scale.
-            big = scene.scales.max(1) > 5.0
-            assert 0 < big.sum() < 0.01 * scene.n
-            per_surfel = [k for k, _ in G.GRAD_PAIRS if k != "v_dF"]
-            for k in per_surfel:
-                g_b, r_b = gg[k][big].astype(np.float64), np.asarray(gr[k])[big].reshape(gg[k][big].shape)
-                row = np.abs(r_b).max(-1, keepdims=True) if r_b.ndim > 1 else np.abs(r_b)
-                assert (np.abs(g_b - r_b) <= 1e-4 + 5e-2 * row).all(), k
-            gg = {k: (np.where(big.reshape(-1, *([1] * (v.ndim - 1))), 0, v) if k in per_surfel else v) for k, v in gg.items()}
-            gr = {k: (np.where(big.reshape(-1, *([1] * (np.asarray(v).ndim - 1))), 0, v) if k in per_surfel else v) for k, v in gr.items()}
-        # C4 also composites 20 pairs per pixel over depth ranges of tens of metres (fp32 depth / distortion terms and
-        # suffix sums): a few rows per million end up outside the 1e-3 row bar (colour rows, which carry no depth term,
-        # agree to 1e-7).  Bar for this stress config: at most 2e-5 of the elements outside the row bar, none beyond 10x
-        # (DESIGN.md section 3).
-        gstats = G.compare_grads(gg, gr, pairs=G.GRAD_PAIRS if cfg != "C4full" else G.GRAD_PAIRS[:5],
-                                 allow_frac=2e-5 if cfg == "C4full" else 0.0)
-        if cfg == "C4full":
-            assert max(v[0] for v in gstats.values()) < 10.0, gstats
-            assert gstats["v_rgb"][1] == 0
-        if cfg == "C4full":     # v_dF is one global sum over all surfels, the oversized ones included
-            np.testing.assert_allclose(resb["grads"]["v_dF"], refb["grads"]["v_dF"], rtol=2e-3, atol=2e-3 * np.abs(refb["grads"]["v_dF"]).max())
-        G.compare_grads(resb["grads"], refb["bwd"], pairs=[("v_cc", "v_cc"), ("v_ambient", "v_ambient")])
-        # ---- unmasked: fragile pixels may legitimately differ; bounded share of elements ----
-        refu = orc.view_iteration(scene, view, upstream=up, threads=nth)
+        gstats = G.compare_grads(resb["grads"], refb["grads"], refb["grads"], G.GRAD_PAIRS)
+        gstats.update(G.compare_grads(resb["grads"], refb["bwd"], refb["bwd"], G.EPI_PAIRS))
+        # ---- unmasked: a pixel whose decision flips moves the gradients of the surfels it touches.  SURVEY 8(c) F: every
+        # element outside the bar belongs to a surfel touched by a fragile pixel, and they are <= 1e-4 of all elements ----
+        refu = orc.view_iteration(scene, view, upstream=up, threads=nth, twin=True)
         resu = G.gpu_view_iteration(P, gs, view, upstream=up, want_debug=False)
-        if cfg != "C4full":
-            G.compare_grads(resu["grads"], refu["grads"], pairs=G.GRAD_PAIRS[:5], allow_frac=2e-3 if fragile.any() else 0.0)
-        print(cfg, vi, "fragile", int(fragile.sum()), "img err/tol", stats, "grad err/tol", gstats)
+        touched = G.touched_by(fragile, ref["main_pass"]["rec"], ref["main_pass"]["flags"])
+        ust = G.compare_grads(resu["grads"], refu["grads"], refu["grads"], G.GRAD_PAIRS[:5], exempt={k[0]: touched for k in G.GRAD_PAIRS[:5]})
+        n_out = sum(v["exempt_bad"] for v in ust.values())
+        assert n_out <= max(1e-4 * 13 * scene.n, 3 * int(fragile.sum() > 0)), (n_out, scene.n)
+        print(cfg, vi, "fragile", int(fragile.sum()), "img err/tol", stats, "masked", {k: (round(v["c_needed"], 1), v["beyond_plain"]) for k, v in gstats.items()},
+              "unmasked outside (touched rows)", n_out, "touched", float(touched.mean()))
 
 
-@pytest.mark.parametrize("cfg", ["C2s", "C3full"])
+@pytest.mark.parametrize("cfg", ["C2s", "C2full", "C3full"])
 def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
     """C2-shaped (and the C3 bench workload at full size): sun pass (depth only) -> view pass with the fused shadow + colour epilogue -> both backwards.
     Each stage is compared with identical inputs on both sides (the oracle's fp32 sun camera / sun map / sun-map
     gradient are the inputs of the next GPU stage), then once end to end."""
     import torch
     scene = S.make_config(2, n=20000, size=256, n_views=2, extent=64.0, sun_size=384) if cfg == "C2s" else _scene(cfg)
+    if cfg == "C2full":
+        assert scene.n == 200000 and scene.views[0].sun_width == 1024 and scene.views[0].width == 512
     gs = G.GpuScene(scene)
     nth = orc.num_threads()
     for vi, view in enumerate(scene.views):
@@ -199,44 +225,53 @@ def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
         gpu = dict(rgba=out[0].cpu().numpy(), geom=out[1].cpu().numpy(), aux=out[2].cpu().numpy())
         f = ref["fwd"]
         fragile = G.fragile_mask(f["margins"])
-        # conditioning of the shadow lookup: x_s carries ~2 ulp(2048) of fp32 rounding and z_v ~1e-5; V moves by
-        # slope V (1-V) (range of the bilinear footprint * dx + dz)
+        # Conditioning of the shadow lookup: z_v (three fp32 roundings at the magnitude of the depth)
+        # moves x_s through k_h and the looked-up depth through the slope of the sun map inside the bilinear footprint;
+        # dV = slope V (1 - V) dgap,  dgap = dz (1 + |k_h|_1 range(footprint)).  x_s itself is evaluated in double.
         V = f["aux"][..., 2]
         zv = f["geom"][..., 3] + f["aux"][..., 3] * view.z_bg
         h = view.b_z - zv
         py, px = np.meshgrid(np.arange(view.height) + 0.5, np.arange(view.width) + 0.5, indexing="ij")
-        xs = reproj[0] * px + reproj[1] * py + reproj[2] * h + reproj[3] - 0.5
-        ys = reproj[4] * px + reproj[5] * py + reproj[6] * h + reproj[7] - 0.5
+        rp = reproj.astype(np.float64)
+        xs = rp[0] * px + rp[1] * py + rp[2] * h + rp[3] - 0.5
+        ys = rp[4] * px + rp[5] * py + rp[6] * h + rp[7] - 0.5
         x0 = np.clip(np.floor(xs).astype(int), 0, view.sun_width - 2); y0 = np.clip(np.floor(ys).astype(int), 0, view.sun_height - 2)
         tex = np.stack([sun_map32[y0, x0], sun_map32[y0, x0 + 1], sun_map32[y0 + 1, x0], sun_map32[y0 + 1, x0 + 1]], -1).astype(np.float64)
         rng_ = tex.max(-1) - tex.min(-1)
-        dV = view.slope * V * (1 - V) * (rng_ * 1e-3 + 3e-5)
+        dz = 4.0 * G.EPS32 * max(abs(view.z_bg), abs(view.b_z))
+        dgap = dz * (1.0 + (abs(rp[2]) + abs(rp[6])) * rng_)
+        dV = view.slope * V * (1 - V) * dgap
         # texel-border crossings flip the footprint: fragile
         fr = np.minimum(np.abs(xs - np.round(xs)), np.abs(ys - np.round(ys)))
-        fragile |= (fr < 1e-3) & (rng_ > 1e-3)
+        fragile |= (fr < 1e-4) & (rng_ > 1e-3)
         albC = np.abs(f["albedo"] @ view.cc.reshape(3, 4)[:, :3].T.astype(np.float64) + view.cc.reshape(3, 4)[:, 3])
         ex_rgba = np.zeros_like(f["rgba"]); ex_rgba[..., :3] = albC * dV[..., None]
         ex_aux = np.zeros_like(f["aux"]); ex_aux[..., 2] = dV
-        stats = G.compare_images(gpu, f, fragile, extra_tol=dict(rgba=ex_rgba, aux=ex_aux), max_fragile_frac=2e-2)
+        stats = G.compare_images(gpu, f, fragile, extra_tol=dict(rgba=ex_rgba, aux=ex_aux), max_fragile_frac=1.5e-2)
         assert V.min() < 0.3 and V.max() > 0.9       # shadows really are exercised
+        assert np.median(dV) < 2e-5                  # the conditioning allowance is small against the image bar almost everywhere
         # ---- stage 3: view backward (masked upstream) ----
         upm = [u.copy() for u in up]
         for u in upm:
             u[fragile] = 0
-        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth, twin=True)
+        # every term that passes through the soft test carries the relative conditioning error kappa = 2 slope dgap of its
+        # pixel: its scale is the oracle's own twin for the colour upstream scaled by kappa (an upper bound: it also
+        # counts the colour path)
+        kap = [np.zeros_like(u) for u in upm]
+        kap[0][..., :3] = upm[0][..., :3] * (2.0 * view.slope * dgap)[..., None]
+        refk = orc.view_iteration(scene, view, upstream=kap, threads=nth, twin=True)
         g = gs.zeros_grads()
         v_sun = torch.zeros_like(d_sun)
         ctx.render_backward(shading, G.t(upm[0]), G.t(upm[1]), G.t(upm[2]), g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"],
                             g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"], v_sun, g["v_reproj"])
         gn = {k: v.cpu().numpy() for k, v in g.items()}
-        # gradients that pass through dV/dgap inherit the conditioning of the lookup: looser relative bar there
-        # (at full size 0.22 % of the v_means ELEMENTS sit outside their own-magnitude bar while every row is inside
-        # the row bar: small components of rows dominated by the shadow term; element share bound 0.5 % here)
-        gst = G.compare_grads(gn, refb["grads"], pairs=G.GRAD_PAIRS, rtol=5e-3, atol=1e-4, allow_frac=1e-3, elem_frac=5e-3)
-        G.compare_grads(gn, refb["bwd"], pairs=[("v_cc", "v_cc"), ("v_ambient", "v_ambient"), ("v_reproj", "v_reproj")], rtol=5e-3, atol=1e-3)
+        gn["v_sun_depth"] = v_sun.cpu().numpy()
+        gst = G.compare_grads(gn, refb["grads"], refb["grads"], G.GRAD_PAIRS, extra={k[0]: refk["grads"][k[2]] for k in G.GRAD_PAIRS})
+        epi = G.EPI_PAIRS + [("v_reproj", "v_reproj", "a_reproj"), ("v_sun_depth", "v_sun_depth", "a_sun_depth")]
+        gst.update(G.compare_grads(gn, refb["bwd"], refb["bwd"], epi, extra={k[0]: refk["bwd"][k[2]] for k in epi}))
         vs_ref = refb["bwd"]["v_sun_depth"]
-        vs_err = np.abs(v_sun.cpu().numpy().astype(np.float64) - vs_ref)
-        assert (vs_err > 1e-4 + 5e-3 * np.abs(vs_ref)).mean() < 1e-3
+        assert np.abs(vs_ref).max() > 0
         ctx.close()
         # ---- stage 4: sun backward with the ORACLE's fp32 sun-map gradient as input (masked on fragile sun pixels) ----
         vsd = vs_ref.astype(np.float32)
@@ -246,8 +281,9 @@ def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
         vr = np.zeros((Hs, Ws, 4)); vr[..., 3] = -sun_view.z_bg * vsd.astype(np.float64)
         sp = ref["sun_pass"]
         bs = orc.backward(Ws, Hs, sun_view.b_z, sun_view.z_bg, np.zeros(3), sp["rec64"], sp["flags"], sp["lists"], orc.Shading(),
-                          vr, vg, None, threads=nth)
-        gsr = orc.preprocess_backward(sun_view, scene.means, scene.quats, scene.scales, scene.opacity_logits, sp["flags"], bs["v_rec"])
+                          vr, vg, None, threads=nth, twin=True)
+        gsr = orc.preprocess_backward(sun_view, scene.means, scene.quats, scene.scales, scene.opacity_logits, sp["flags"], bs["v_rec"],
+                                      a_rec=bs["a_rec"])
         sctx = P.Context(scene.n, Ws, Hs, 16 * scene.n)
         sctx.preprocess(P.Camera.from_view(sun_view), gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
         tmp = torch.empty(Hs, Ws, device="cuda")
@@ -255,10 +291,13 @@ def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
         g2 = gs.zeros_grads()
         sctx.shadow_map_backward(G.t(vsd), g2["v_means"], g2["v_quats"], g2["v_scales"], g2["v_logits"], g2["v_dF_sun"])
         g2n = {k: v.cpu().numpy() for k, v in g2.items()}
-        G.compare_grads(g2n, gsr, pairs=[("v_means", "v_means"), ("v_quats", "v_quats"), ("v_scales", "v_scales"),
-                                         ("v_logits", "v_logits"), ("v_dF_sun", "v_dF")])
+        sst = G.compare_grads(g2n, gsr, gsr, [("v_means", "v_means", "a_means"), ("v_quats", "v_quats", "a_quats"),
+                                              ("v_scales", "v_scales", "a_scales"), ("v_logits", "v_logits", "a_logits"),
+                                              ("v_dF_sun", "v_dF", "a_dF")])
         sctx.close()
-        print(cfg, vi, "fragile", int(fragile.sum()), "sun fragile", int(sfrag.sum()), stats, gst)
+        print(cfg, vi, "fragile", int(fragile.sum()), "sun fragile", int(sfrag.sum()), stats,
+              {k: (round(v["c_needed"], 1), v["beyond_plain"], round(v["max_err_over_tol"], 3)) for k, v in gst.items()},
+              {k: (round(v["c_needed"], 1), v["beyond_plain"]) for k, v in sst.items()})
 
 
 def test_edge_cases_and_errors(P, G, orc):
@@ -461,6 +500,24 @@ def test_adam_step_matches_oracle(P, G, n):
                     dg["logits"], dg["rgb"], dm, dv, [0.1] * 5, step=0)
 
 
+def _loss_grad_close(name, g, ref, npx, z_bg=1.0):
+    """Element-wise bar of the loss stage: |gpu - ref| <= atol + rtol |ref| in the natural unit of an upstream-gradient
+    image, 1 / (number of pixels) (every loss term is a mean over pixels): atol = 5e-5 / npx, rtol = 1e-3.  The
+    absolute part is the fp32 conditioning of the SSIM derivative (variances are differences of blurred moments:
+    ~1e-7 of cancellation divided by C2 = 9e-4) and of Eq. 13's normalisation.  The alpha channel of v_rgba is
+    -z_bg times the depth gradient (z_v = D + (1 - A) z_bg): its unit is z_bg / npx."""
+    g = g.astype(np.float64)
+    assert np.isfinite(g).all(), name
+    err = np.abs(g - ref) * npx
+    unit = np.ones(g.shape[-1])
+    if name == "v_rgba":
+        unit[3] = max(1.0, abs(z_bg))
+    tol = 5e-5 * unit + 1e-3 * np.abs(ref) * npx
+    worst = float((err / tol).max())
+    assert worst <= 1.0, (name, worst, np.argwhere(err > tol)[:5])
+    return worst
+
+
 @pytest.mark.parametrize("cfg", ["C0_ragged", "C1s"])
 def test_loss_stage_matches_oracle(P, G, orc, cfg):
     """satsplat_loss_upstream on REAL rendered images (CUDA forward) against the numpy float64 oracle fed the same fp32
@@ -493,13 +550,7 @@ def test_loss_stage_matches_oracle(P, G, orc, cfg):
         assert abs(gv - terms[k]) <= 2e-5 * max(abs(terms[k]), 1e-3), (k, gv, terms[k])
     assert (s[4:] == 0).all()
     for name, gpu, ref in (("v_rgba", v[0], r_rgba), ("v_geom", v[1], r_geom), ("v_aux", v[2], r_aux)):
-        g = gpu.cpu().numpy().astype(np.float64)
-        assert np.isfinite(g).all(), name
-        for ch in range(4):
-            scale = np.abs(ref[..., ch]).max()
-            err = np.abs(g[..., ch] - ref[..., ch]).max()
-            # fp32 stencil arithmetic: SSIM variances are differences of blurred moments (cancellation ~1e-7 / C2)
-            assert err <= 2e-4 * scale + 1e-12, (name, ch, err, scale)
+        _loss_grad_close(name, gpu.cpu().numpy(), ref, npx, view.z_bg)
     assert np.abs(r_geom[..., 3]).max() > 0 and terms["ssim"] < 0.99
     print(cfg, terms)
 
@@ -569,10 +620,8 @@ def test_loss_stage_tiny_and_ragged_images(P, G, hw):
     got = dict(l1=s[0] / (3 * npx), ssim=s[1] / (3 * npx), distortion=s[2] / npx, normal=s[3] / npx)
     for k, gv in got.items():
         assert abs(gv - terms[k]) <= 1e-5 * max(abs(terms[k]), 1e-2), (k, gv, terms[k])
-    for gpu, ref in ((v[0], r_rgba), (v[1], r_geom), (v[2], r_aux)):
-        g = gpu.cpu().numpy().astype(np.float64)
-        assert np.isfinite(g).all()
-        assert np.abs(g - ref).max() <= 2e-4 * max(np.abs(ref).max(), 1e-12) + 1e-12
+    for name, gpu, ref in (("v_rgba", v[0], r_rgba), ("v_geom", v[1], r_geom), ("v_aux", v[2], r_aux)):
+        _loss_grad_close(name, gpu.cpu().numpy(), ref, npx, 14.0)
     if H < 3 or W < 3:
         assert abs(terms["normal"] - 1.0) < 1e-12 and np.abs(r_geom).max() == 0    # no interior pixel: N_d = 0 everywhere
 
