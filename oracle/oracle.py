@@ -27,16 +27,41 @@ REC = dict(cx=0, cy=1, q00=2, q01=3, q10=4, q11=5, zc=6, g0=7, g1=8, alpha=9, r=
 TILE = 16
 
 
+def _compile(out: str, opt: list) -> None:
+    tmp = out + f".tmp{os.getpid()}"
+    cmd = ["g++", *opt, "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC", _SRC, "-o", tmp]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, out)
+
+
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (building the checker is not using it)."""
+    """Compile the oracle with gcc (building the checker is not using it).  Portable -O2 build: the .so travels."""
     with _LOCK:
         if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-            tmp = _SO + f".tmp{os.getpid()}"
-            cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
-                   "-shared", "-fPIC", _SRC, "-o", tmp]
-            subprocess.run(cmd, check=True)
-            os.replace(tmp, _SO)
+            _compile(_SO, ["-O2"])
     return _SO
+
+
+def use_native_build() -> str:
+    """The timed baseline's build (-O3 -march=native -ffp-contract=off), compiled ON the host it
+    runs on (the file name carries the host's CPU model, so a copy made on another machine is never loaded).  Same
+    source, same arithmetic (no fast-math, no contraction); only bench.py's CPU legs switch to it, before first use."""
+    global _LIB
+    import hashlib
+    import platform
+    model = platform.machine()
+    try:
+        with open("/proc/cpuinfo") as f:
+            model += "".join(l for l in f if l.startswith(("model name", "flags")))[:20000]
+    except OSError:
+        pass
+    so = os.path.join(_HERE, f"libsatsplat_oracle_native_{hashlib.sha1(model.encode()).hexdigest()[:10]}.so")
+    with _LOCK:
+        if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+            _compile(so, ["-O3", "-march=native"])
+        _LIB = None
+    lib(so)
+    return so
 
 
 class _CamF32(C.Structure):
@@ -61,12 +86,13 @@ class _Render(C.Structure):
                 ("ranges", C.c_void_p), ("list_len", C.c_int64), ("options", C.c_int32), ("threads", C.c_int32)]
 
 
-def lib():
+def lib(path: str = None):
     global _LIB
     if _LIB is None:
-        _LIB = C.CDLL(build())
+        _LIB = C.CDLL(path or build())
         for name in ("orc_preprocess_f32", "orc_preprocess_f64", "orc_bin", "orc_forward", "orc_backward",
-                     "orc_preprocess_backward", "orc_sun_camera", "orc_sun_camera_backward", "orc_num_threads"):
+                     "orc_preprocess_backward", "orc_sun_camera", "orc_sun_camera_backward", "orc_nearby_camera",
+                     "orc_nearby_camera_backward", "orc_num_threads"):
             getattr(_LIB, name).restype = C.c_int
     return _LIB
 
@@ -288,6 +314,23 @@ def sun_camera_backward(Fp, azimuth, elevation, viewport, v_F_sun, v_reproj):
     v_Fp = np.zeros(8)
     rc = lib().orc_sun_camera_backward(_p(_f64(Fp)), C.c_double(azimuth), C.c_double(elevation), _p(_f64(viewport)),
                                        _p(_f64(v_F_sun)), _p(_f64(v_reproj)), _p(v_Fp))
+    assert rc == 0
+    return v_Fp
+
+
+def nearby_camera(Fp, d_azimuth, d_elevation):
+    """Nearby camera of PAPER.md:176: azimuth / elevation of d_main = B_x x B_y perturbed, then Eq. 16.  Returns
+    F_near [8] and (azimuth, elevation) of the main direction (double)."""
+    F_near, ang = np.zeros(8), np.zeros(2)
+    rc = lib().orc_nearby_camera(_p(_f64(Fp)), C.c_double(d_azimuth), C.c_double(d_elevation), _p(F_near), _p(ang))
+    assert rc == 0
+    return F_near, ang
+
+
+def nearby_camera_backward(Fp, d_azimuth, d_elevation, v_F_near):
+    """Adjoint of nearby_camera with respect to Fp.  Returns v_Fp [8] (double)."""
+    v_Fp = np.zeros(8)
+    rc = lib().orc_nearby_camera_backward(_p(_f64(Fp)), C.c_double(d_azimuth), C.c_double(d_elevation), _p(_f64(v_F_near)), _p(v_Fp))
     assert rc == 0
     return v_Fp
 

@@ -892,6 +892,85 @@ int orc_sun_camera_backward(const double* Fp, double azimuth, double elevation, 
   return 0;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Nearby camera (Fig. 1): "we compute the azimuth and elevation angle of the original camera viewing
+// direction d_main.  We then add small random perturbations to the angles to create a new viewing direction.  Then
+// apply the same projection matrix transformation as Eq. (16)".  d_main = B_x x B_y is the nullspace of
+// B_xy; its angles are taken on the ray pointing up (towards the sensor), in the convention of Eq. S2 (azimuth from +X
+// towards +Y, elevation above the horizon), so that a zero perturbation returns the input camera: B u = 0 leaves the
+// third column unchanged.  The offset column is kept (as for the sun camera: b_sun = b').  DESIGN.md reading 27.
+// angles_out (may be NULL) = (azimuth, elevation) of the main direction.
+// ---------------------------------------------------------------------------------------------------
+int orc_nearby_camera(const double* Fp, double d_azimuth, double d_elevation, double* F_near, double* angles_out) {
+  const double* Bx = Fp;
+  const double* By = Fp + 4;
+  const double d[3] = {Bx[1] * By[2] - Bx[2] * By[1], Bx[2] * By[0] - Bx[0] * By[2], Bx[0] * By[1] - Bx[1] * By[0]};
+  const double dn = std::sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+  if (!(dn > 0)) return -1;
+  const double sg = d[2] < 0 ? -1.0 : 1.0;                       // the ray that points up
+  const double u[3] = {sg * d[0] / dn, sg * d[1] / dn, sg * d[2] / dn};
+  const double az = std::atan2(u[1], u[0]), el = std::asin(u[2]);
+  if (angles_out) { angles_out[0] = az; angles_out[1] = el; }
+  const double a2 = az + d_azimuth, e2 = el + d_elevation;
+  const double s[3] = {std::cos(a2) / std::tan(e2), std::sin(a2) / std::tan(e2), 1.0};   // Eq. S2 for the new direction
+  for (int r = 0; r < 2; ++r) {
+    const double* B = Fp + 4 * r;
+    const double Bs = B[0] * s[0] + B[1] * s[1] + B[2] * s[2];
+    F_near[4 * r + 0] = B[0];
+    F_near[4 * r + 1] = B[1];
+    F_near[4 * r + 2] = B[2] - Bs;                               // Eq. 16: B (I - [0 0 s])
+    F_near[4 * r + 3] = B[3];
+  }
+  return 0;
+}
+
+// Adjoint of orc_nearby_camera with respect to Fp (the gradient a nearby-view render sends back into dF through the
+// cascade), the reverse of its steps one by one.  v_Fp is accumulated into.
+int orc_nearby_camera_backward(const double* Fp, double d_azimuth, double d_elevation, const double* v_F_near, double* v_Fp) {
+  const double* Bx = Fp;
+  const double* By = Fp + 4;
+  const double d[3] = {Bx[1] * By[2] - Bx[2] * By[1], Bx[2] * By[0] - Bx[0] * By[2], Bx[0] * By[1] - Bx[1] * By[0]};
+  const double dn = std::sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+  if (!(dn > 0)) return -1;
+  const double sg = d[2] < 0 ? -1.0 : 1.0;
+  const double u[3] = {sg * d[0] / dn, sg * d[1] / dn, sg * d[2] / dn};
+  const double az = std::atan2(u[1], u[0]), el = std::asin(u[2]);
+  const double a2 = az + d_azimuth, e2 = el + d_elevation;
+  const double ct = 1.0 / std::tan(e2);
+  const double s[3] = {std::cos(a2) * ct, std::sin(a2) * ct, 1.0};
+  // ---- reverse: F_near[r] = (B0, B1, B2 - B.s, B3) ----
+  double vs[3] = {0, 0, 0};
+  for (int r = 0; r < 2; ++r) {
+    const double* B = Fp + 4 * r;
+    const double* vf = v_F_near + 4 * r;
+    v_Fp[4 * r + 0] += vf[0] - vf[2] * s[0];
+    v_Fp[4 * r + 1] += vf[1] - vf[2] * s[1];
+    v_Fp[4 * r + 2] += vf[2] - vf[2] * s[2];
+    v_Fp[4 * r + 3] += vf[3];
+    for (int k = 0; k < 3; ++k) vs[k] += -vf[2] * B[k];
+  }
+  // s = (cos a2 ct, sin a2 ct, 1), ct = 1 / tan e2
+  const double v_a2 = vs[0] * (-std::sin(a2) * ct) + vs[1] * (std::cos(a2) * ct);
+  const double v_ct = vs[0] * std::cos(a2) + vs[1] * std::sin(a2);
+  const double v_e2 = -v_ct / (std::sin(e2) * std::sin(e2));
+  // az = atan2(u1, u0), el = asin(u2)
+  const double h2 = u[0] * u[0] + u[1] * u[1];
+  if (!(h2 > 0)) return -2;                                      // exactly nadir: the azimuth is undefined
+  double vu[3] = {v_a2 * (-u[1] / h2), v_a2 * (u[0] / h2), v_e2 / std::sqrt(1.0 - u[2] * u[2])};
+  // u = sg d / |d|
+  const double dot = u[0] * vu[0] + u[1] * vu[1] + u[2] * vu[2];
+  double vd[3];
+  for (int k = 0; k < 3; ++k) vd[k] = sg * (vu[k] - u[k] * dot) / dn;
+  // d = Bx x By  =>  v_Bx = By x v_d,  v_By = v_d x Bx
+  v_Fp[0] += By[1] * vd[2] - By[2] * vd[1];
+  v_Fp[1] += By[2] * vd[0] - By[0] * vd[2];
+  v_Fp[2] += By[0] * vd[1] - By[1] * vd[0];
+  v_Fp[4] += vd[1] * Bx[2] - vd[2] * Bx[1];
+  v_Fp[5] += vd[2] * Bx[0] - vd[0] * Bx[2];
+  v_Fp[6] += vd[0] * Bx[1] - vd[1] * Bx[0];
+  return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -760,6 +760,54 @@ def test_p14_sun_camera_adjoint_fd_and_closed_form(orc):
         np.testing.assert_allclose(orc.sun_camera_backward(Fp, az, el, vp, np.zeros(8), only_const), 0, atol=1e-9)
 
 
+def test_p20_nearby_camera_nullspace_identity_roundtrip_and_adjoint(orc):
+    """Nearby camera of the cascade (Fig. 1 :159; reading 27), pinned by what the text fixes:
+    (a) zero perturbation returns the input camera (d_main is the nullspace of B_xy, PAPER.md:165);
+    (b) the new viewing direction s' is the nullspace of B_nearby (S5-S6 applied to the new direction);
+    (c) round trip: the azimuth / elevation of the nearby camera's OWN main direction B_x x B_y are the perturbed angles;
+    (d) the angles of a camera built from a known direction by the scene recipe are that direction's (independent of the
+        cross product: the recipe's d is an input here);
+    (e) the adjoint against central finite differences of the forward."""
+    rng = np.random.default_rng(12)
+    for trial in range(6):
+        theta, psi = math.radians(rng.uniform(5, 35)), rng.uniform(0, 2 * math.pi)
+        F, d = S.affine_camera(0.4, theta, psi, 512, 512, (10.0, -20.0, 5.0))
+        Fp = np.asarray(F, np.float64).reshape(8) + rng.normal(0, 1e-3, 8)
+        B = Fp.reshape(2, 4)[:, :3]
+        # (a)
+        F0, ang = orc.nearby_camera(Fp, 0.0, 0.0)
+        np.testing.assert_allclose(F0, Fp, rtol=0, atol=1e-12 * np.abs(Fp).max())
+        # (d) the up-pointing ray of the unperturbed recipe camera is -d: off-nadir theta <=> elevation 90 deg - theta
+        _, ang_clean = orc.nearby_camera(np.asarray(F, np.float64).reshape(8), 0.0, 0.0)
+        up_ray = -np.asarray(d, np.float64)
+        assert abs(ang_clean[1] - (math.pi / 2 - theta)) < 1e-6
+        assert abs(math.remainder(ang_clean[0] - math.atan2(up_ray[1], up_ray[0]), 2 * math.pi)) < 1e-5
+        # (b), (c)
+        da, de = rng.normal(0, 0.05), rng.normal(0, 0.03)
+        Fn, _ = orc.nearby_camera(Fp, da, de)
+        a2, e2 = ang[0] + da, ang[1] + de
+        s2 = np.array([math.cos(a2) / math.tan(e2), math.sin(a2) / math.tan(e2), 1.0])
+        Bn = Fn.reshape(2, 4)[:, :3]
+        assert np.abs(Bn @ s2).max() < 1e-10 * np.abs(Bn).max()
+        assert np.array_equal(Fn.reshape(2, 4)[:, [0, 1, 3]], Fp.reshape(2, 4)[:, [0, 1, 3]])    # Eq. 16 only touches column 3
+        _, ang_n = orc.nearby_camera(Fn, 0.0, 0.0)
+        assert abs(math.remainder(ang_n[0] - a2, 2 * math.pi)) < 1e-9 and abs(ang_n[1] - e2) < 1e-9
+        # a point moved along the new direction keeps its nearby-image position (definition of a viewing direction)
+        p = rng.normal(0, 30, 3)
+        assert np.abs(Bn @ (p + 7.0 * s2) - Bn @ p).max() < 1e-8
+        # (e)
+        vF = rng.normal(0, 1, 8)
+        g = orc.nearby_camera_backward(Fp, da, de, vF)
+        for k in range(8):
+            h = 1e-6 * max(1.0, abs(Fp[k]))
+            e = np.zeros(8); e[k] = h
+            fd = (orc.nearby_camera(Fp + e, da, de)[0] @ vF - orc.nearby_camera(Fp - e, da, de)[0] @ vF) / (2 * h)
+            assert abs(fd - g[k]) < 2e-6 * max(1.0, np.abs(g).max()), (trial, k, fd, g[k])
+    # a gradient that only reaches the untouched columns passes straight through
+    only = np.zeros(8); only[[0, 1, 3, 4, 5, 7]] = 1.0
+    np.testing.assert_allclose(orc.nearby_camera_backward(Fp, 0.02, -0.01, only), only, atol=1e-12)
+
+
 def test_p14_cascade_total_dF_finite_differences(orc):
     """The whole cascade in one objective: dF moves the view camera, the sun camera built from it (Eq. 16), the sun
     depth map rendered with that camera, and the reprojection of the shadow test.  Total analytic gradient
