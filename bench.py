@@ -3,18 +3,24 @@
 
     python bench.py --gpus N --steps K --warmup W            # the CUDA path (hand-written sm_100a kernels)
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands, on the host cores
+    python bench.py --record-traffic <ncu raw csv>           # refresh profiles/r2_traffic.json from an ncu capture
 
 A "step" is one full training-view iteration of the hot path: sun pass (preprocess,
 binning, depth-only compositing) -> view pass (preprocess, binning, compositing of colour/alpha/depth/normal/
 median/distortion with the fused colour-correction + shadow epilogue) -> backward of both passes (epilogue
-backward, reverse compositing, per-surfel chain, dF / CC reductions).  Views cycle through the config's 20 views.
-Prints ONE JSON line (rank 0).
+backward, reverse compositing, per-surfel chain, dF / CC reductions) -> cascade chain of the sun camera into dF.
+Views cycle through the config's 20 views.  With --gpus N > 1 (one process per GPU: under torchrun, or spawned by this
+script when WORLD_SIZE is unset) the views are sharded over the ranks and every step ends with ONE NCCL all-reduce
+(sum) of the packed 13 N surfel gradients, overlapped with the next step.  Prints ONE JSON line
+(rank 0).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -32,14 +38,9 @@ INST_EVAL = 17.0          # per evaluated (pixel, list entry) pair: Eq. 9 + Eq. 
 INST_CONTRIB_FWD = 25.0   # extra per contributing pair, forward (view pass; the depth-only sun pass: 6)
 INST_CONTRIB_BWD = 90.0   # extra per contributing pair, backward (view pass; sun pass: 50)
 INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN = 6.0, 50.0
-FP32_PEAK_TINST = 148 * 128 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 1.965 GHz = 37.2 T lane-instr/s
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the view-pass kernels at C3, from the committed
-# `ncu --set full` capture (a profiler number is never a bench value: it only fills roofline.traffic)
-NCU_SOURCE = "profiles/r1_kernels_final.md"
-NCU_DRAM_BYTES_PER_LAUNCH = {"blend_bwd": 784.4e6, "blend_fwd": 528.7e6}
-# executed warp-instructions and issue-slot utilisation of the same capture (the kernels cull before they evaluate:
-# they execute fewer lane-instructions than the algorithmic count the roofline fraction is quoted on)
-NCU_EXECUTED = {"blend_bwd": dict(warp_inst=671.3e6, issue_active_pct=73.9), "blend_fwd": dict(warp_inst=324.7e6, issue_active_pct=78.4)}
+SM_LANES = 128            # FP32 lanes per SM; derived peak = SMs x 128 x clock, measured one beside it
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
+CSRC = os.path.join(ROOT, "paper_2606_28581_b200", "csrc")
 
 
 def parse():
@@ -53,7 +54,11 @@ def parse():
     ap.add_argument("--size", type=int, default=None, help="override view size (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the Adam / loss / init stage timings")
     ap.add_argument("--no-graphs", action="store_true", help="launch every kernel of a step from the host instead of replaying one CUDA graph per view")
+    ap.add_argument("--no-allreduce", action="store_true", help="N > 1: leave the per-rank gradients un-reduced")
+    ap.add_argument("--record-traffic", default=None, metavar="NCU_RAW_CSV",
+                    help="write profiles/r2_traffic.json from `ncu -i <rep> --page raw --csv` output and exit")
     return ap.parse_args()
 
 
@@ -63,6 +68,53 @@ def load_peaks():
         d = json.load(open(p))
         return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def csrc_hash() -> str:
+    """Content hash of the CUDA sources (the GPU box has no .git): ties the ncu-derived fields to the kernels they
+    were captured on."""
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            h.update(open(os.path.join(CSRC, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def record_traffic(raw_csv: str):
+    """profiles/r2_traffic.json <- per-kernel DRAM bytes, executed warp-instructions and issue utilisation of one
+    `ncu --set full` capture (first launch of each kernel name in the file), with the hash of the sources."""
+    import csv
+    rows = list(csv.reader(open(raw_csv)))
+    hdr = rows[0]
+    col = {h: i for i, h in enumerate(hdr)}
+    out = {}
+    for r in rows[2:]:
+        name = r[col["Kernel Name"]]
+        key = ("blend_bwd" if "blend_backward" in name else "blend_fwd" if "blend_forward" in name else name.split("(")[0].split("::")[-1])
+        key += "_sun" if ("<1>" in name or "(bool)1" in name) else ""
+        if key in out:
+            continue
+        f = lambda k: float(r[col[k]]) if k in col and r[col[k]] not in ("", "n/a") else None
+        unit = rows[1][col["dram__bytes_read.sum"]].lower() if "dram__bytes_read.sum" in col else "byte"
+        mul = dict(byte=1.0, kbyte=1e3, mbyte=1e6, gbyte=1e9).get(unit, 1.0)
+        rd, wr = f("dram__bytes_read.sum"), f("dram__bytes_write.sum")
+        out[key] = dict(dram_bytes=(rd + wr) * mul if rd is not None and wr is not None else None,
+                        warp_inst=f("smsp__inst_executed.sum"),
+                        issue_active_pct=f("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+                        ncu_us=f("gpu__time_duration.sum"))
+    json.dump(dict(csrc_sha256=csrc_hash(), source=os.path.basename(raw_csv), kernels=out), open(TRAFFIC_JSON, "w"), indent=1)
+    print("wrote", TRAFFIC_JSON, list(out))
+
+
+def load_traffic():
+    """ncu-derived fields of the roofline line; None when the committed capture was taken on other kernel sources."""
+    if not os.path.exists(TRAFFIC_JSON):
+        return None, "no capture committed"
+    d = json.load(open(TRAFFIC_JSON))
+    if d.get("csrc_sha256") != csrc_hash():
+        return None, f"stale: profiles/r2_traffic.json was captured on sources {d.get('csrc_sha256')}, these are {csrc_hash()}"
+    return d["kernels"], "profiles/r2_traffic.json (ncu --set full, same sources)"
 
 
 def make_scene(args):
@@ -78,63 +130,150 @@ def make_scene(args):
 
 def views_for_rank(rank: int, world: int, n_views: int, steps: int):
     """View index of every step of this rank: ranks start on different views and stride by the world size, so
-    that the ranks of one job render disjoint views (independent units, no data-path collective)."""
+    that the ranks of one job render disjoint views (independent units; the only exchange is the gradient sum)."""
     return [(rank + s * world) % n_views for s in range(steps)]
 
 
+def packed_offsets(n: int):
+    """Float offsets of the five surfel-gradient groups (means 3N, quats 4N, scales 2N, logits N, rgb 3N) in the ONE
+    buffer that is all-reduced; every group starts on a 16-byte boundary.  Returns (offsets[5], total floats)."""
+    off, t = [], 0
+    for w in (3, 4, 2, 1, 3):
+        off.append(t)
+        t += (n * w + 3) // 4 * 4
+    return off, t
+
+
+def allreduce_sum(dist, flat):
+    """The one collective of the data-parallel path: sum over ranks of the packed surfel gradients."""
+    dist.all_reduce(flat, op=dist.ReduceOp.SUM)
+    return flat
+
+
+def spawn_command(args, port: int):
+    """Command line that launches this bench as one process per GPU (used when --gpus N > 1 and WORLD_SIZE is unset)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)]
+    return cmd + [a for a in sys.argv[1:]]
+
+
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+    """SM clock + throttle reasons through NVML every ~2 ms, started BEFORE the warm-up; only the samples whose host
+    time falls inside the timed window are reported (so even a 40 ms timed region has samples).  Falls back to
+    `nvidia-smi -lms` when NVML cannot be loaded."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown"}
 
     def __init__(self, index):
-        self.index, self.proc, self.rows = index, None, []
+        self.index, self.rows, self.stop_flag, self.thread, self.mode = index, [], False, None, None
 
     def start(self):
-        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.mode = "nvml"
+            self.thread = threading.Thread(target=self._loop_nvml, daemon=True)
         except Exception:
-            self.proc = None
+            self.mode = "nvidia-smi"
+            self.thread = threading.Thread(target=self._loop_smi, daemon=True)
+        self.thread.start()
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append(line.strip())
-
-    def stop(self):
-        if not self.proc:
-            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
-            f = [x.strip() for x in r.split(",")]
+    def _loop_nvml(self):
+        nv = self.nv
+        while not self.stop_flag:
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
-                for nm, v in zip(names, f[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(nm)
+                t = time.perf_counter()
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.rows.append((t, float(mhz), int(rs)))
             except Exception:
                 pass
-        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
-                    reasons=sorted(reasons), samples=len(sm))
+            time.sleep(0.002)
+
+    def _loop_smi(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.sw_power_cap,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.hw_thermal_slowdown")
+        try:
+            proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20"],
+                                    stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.mode = None
+            return
+        self.proc = proc
+        for line in proc.stdout:
+            f = [x.strip() for x in line.split(",")]
+            try:
+                bits = sum(b for b, v in zip((0x4, 0x8, 0x20, 0x40), f[2:6]) if v.lower().startswith("active"))
+                self.max_mhz = float(f[1])
+                self.rows.append((time.perf_counter(), float(f[0]), bits))
+            except Exception:
+                pass
+            if self.stop_flag:
+                break
+        proc.terminate()
+
+    def stop(self, t0, t1):
+        time.sleep(0.03)
+        self.stop_flag = True
+        if getattr(self, "proc", None):
+            self.proc.terminate()
+        if self.mode is None or not self.rows:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["clock sampling unavailable"], samples=0)
+        inside = [r for r in self.rows if t0 <= r[0] <= t1]
+        reasons = set()
+        for r in inside:
+            for bit, nm in self.REASONS.items():
+                if r[2] & bit:
+                    reasons.add(nm)
+        return dict(sm_mhz=float(np.median([r[1] for r in inside])) if inside else None, sm_max_mhz=getattr(self, "max_mhz", None),
+                    reasons=sorted(reasons), samples=len(inside), samples_total=len(self.rows), source=self.mode)
 
 
 # ------------------------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample
 # ------------------------------------------------------------------------------------------------------------
-def oracle_iteration_seconds(scene, view_index):
+def oracle_iteration_seconds(scene, view_index, threads=None, do_backward=True):
     import satsplat_scenes as S
     from oracle import oracle as orc
     view = scene.views[view_index]
     up = S.upstream_grads(scene.seed, view_index, view.height, view.width)
-    nth = orc.num_threads()
+    nth = threads or orc.num_threads()
     t0 = time.perf_counter()
-    orc.view_iteration(scene, view, upstream=up, threads=nth)
+    orc.view_iteration(scene, view, upstream=up if do_backward else None, threads=nth, do_backward=do_backward)
     return time.perf_counter() - t0, nth
+
+
+def oracle_flags():
+    return "-O3 -march=native -ffp-contract=off -fno-fast-math -fopenmp (BASELINE.md section 3), compiled on this host"
+
+
+def cpu_baseline_block(scene, view_index, px, nviews):
+    """The oracle timed on the host cores, beside the GPU number: all threads fwd and fwd+bwd on one full view of the
+    workload, and ONE thread on a bounded sample (a C1-sized scene: 200k surfels, one 512^2 view with its sun pass)."""
+    import satsplat_scenes as S
+    from oracle import oracle as orc
+    orc.use_native_build()
+    dt, nth = oracle_iteration_seconds(scene, view_index)
+    dt_f, _ = oracle_iteration_seconds(scene, view_index, do_backward=False)
+    small = S.make_config(2, n_views=1)
+    spx = small.views[0].width * small.views[0].height
+    dt1, _ = oracle_iteration_seconds(small, 0, threads=1)
+    dt1n, _ = oracle_iteration_seconds(small, 0, threads=nth)
+    return dict(value=px / 1e6 / dt, unit=UNIT, cores=nth, kind="oracle", seconds=dt, fwd_seconds=dt_f, fwd_value=px / 1e6 / dt_f,
+                sample=f"1 full view iteration (view {view_index} of {nviews}) of the same workload, {nth} threads; forward alone timed too",
+                flags=oracle_flags(),
+                single_thread=dict(value=spx / 1e6 / dt1, unit=UNIT, seconds=dt1, all_threads_seconds=dt1n, cores=1,
+                                   sample="C2-sized scene (200k surfels, one 512^2 view + 1024^2 sun map), full iteration, 1 thread"))
 
 
 def run_reference(args):
@@ -142,7 +281,7 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import oracle as orc
-    orc.build()
+    orc.use_native_build()
     scene = make_scene(args)
     steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)   # bounded: each step is ~10 s of CPU work
     for w in range(warm):
@@ -158,16 +297,19 @@ def run_reference(args):
     line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=0, steps=steps, warmup=warm, ms_per_step=ms,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
                 config=workload_config(scene, args, 1),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=nth, kind="oracle", sample=sample),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=nth, kind="oracle", sample=sample, flags=oracle_flags()),
                 e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
 
 
 def workload_config(scene, args, world):
     v = scene.views[0]
+    par = (f"views sharded over {world} ranks; one NCCL all-reduce (sum) of the packed 13 N surfel gradients per step" if world > 1
+           else "1 rank")
     return dict(workload=f"C{args.config} benchmark-shaped site (BASELINE.json configs[{args.config}])", surfels=scene.n,
-                view=f"{v.width}x{v.height}", cuda_graphs=(not getattr(args, "no_graphs", False)) and world == 1, sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
-                views=len(scene.views), shadows=bool(v.shadows_on), parallelism=f"views sharded over {world} rank(s), no collective",
+                view=f"{v.width}x{v.height}", cuda_graphs=("one graph for all views (device-resident cameras)" if (not getattr(args, "no_graphs", False)) and world == 1 else False),
+                sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
+                views=len(scene.views), shadows=bool(v.shadows_on), parallelism=par,
                 l2="per-step working set (records, keys, per-pixel state, images: >0.8 GB) exceeds the 126 MB L2; views cycle")
 
 
@@ -177,7 +319,7 @@ def workload_config(scene, args, world):
 class Job:
     """Device-resident state of one rank: surfels, two contexts (view + sun), outputs, gradient buffers."""
 
-    def __init__(self, P, torch, scene, device):
+    def __init__(self, P, torch, scene, device, n_grad_buffers=1):
         self.P, self.torch, self.scene = P, torch, scene
         dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(device)
         self.means, self.quats, self.scales = dev(scene.means), dev(scene.quats), dev(scene.scales)
@@ -192,9 +334,33 @@ class Job:
         self.out = [torch.empty(v.height, v.width, 4, device=device) for _ in range(3)]
         self.sun_depth = z(v.sun_height, v.sun_width) if self.shadows else None
         self.v_sun = z(v.sun_height, v.sun_width) if self.shadows else None
-        self.g = dict(m=z(n, 3), q=z(n, 4), s=z(n, 2), l=z(n), c=z(n, 3), dF=z(8), cc=z(12), amb=z(3), rep=z(8), dFs=z(8))
-        self.cams, self.up = {}, {}
+        # the 13 N surfel gradients live in ONE packed buffer (what a data-parallel job all-reduces), followed by the
+        # small per-camera vectors: dF(8) cc(12) ambient(3) reproj(8) dF_sun(8), which stay local to the rank
+        off, tot = packed_offsets(n)
+        self.flat_floats = tot
+        self.gbufs = []
+        for _ in range(n_grad_buffers):
+            flat = z(tot + 40)
+            g = dict(flat=flat, surfel=flat[:tot],
+                     m=flat[off[0]:off[0] + 3 * n].view(n, 3), q=flat[off[1]:off[1] + 4 * n].view(n, 4),
+                     s=flat[off[2]:off[2] + 2 * n].view(n, 2), l=flat[off[3]:off[3] + n], c=flat[off[4]:off[4] + 3 * n].view(n, 3),
+                     dF=flat[tot:tot + 8], cc=flat[tot + 8:tot + 20], amb=flat[tot + 20:tot + 23], rep=flat[tot + 24:tot + 32],
+                     dFs=flat[tot + 32:tot + 40])
+            self.gbufs.append(g)
+        self.g = self.gbufs[0]
+        self.cams = {}
         self.device = device
+        # one set of upstream gradient images ~ N(0,1), shared by all views (synthetic; the loss stage would write them)
+        gen = torch.Generator(device=device)
+        gen.manual_seed(scene.seed + 1000)
+        self.up_shared = [torch.randn(v.height, v.width, 4, device=device, generator=gen) for _ in range(3)]
+        self.up_shared[2][..., 2:] = 0
+        # (f2) device-resident cameras: per-view constants, the learnable dF [V,8], the current view index, the camera block
+        self.table = P.view_params_table(scene.views, device=device)
+        self.dF_all = dev(np.stack([vw.dF for vw in scene.views]))
+        self.v_dF_all = z(len(scene.views), 8)
+        self.idx = torch.zeros(1, dtype=torch.int32, device=device)
+        self.block = z(P.CAMERA_BLOCK_FLOATS)
         # the view pass's preprocess + binning do not depend on the sun pass: they run on a second stream beside it
         self.side = torch.cuda.Stream(device=device) if self.shadows else None
         self.overlap = True     # False: everything on one stream (the per-stage timers then see each kernel alone)
@@ -207,11 +373,6 @@ class Job:
         sun_cam, rep = (P.sun_camera(cam, v.sun_azimuth, v.sun_elevation, v.sun_width, v.sun_height, v.sun_viewport)
                         if self.shadows else (None, None))
         self.cams[vi] = (cam, sun_cam, rep)
-        gen = torch.Generator(device=self.device)
-        gen.manual_seed(self.scene.seed + 1000 + 7919 * vi)
-        up = [torch.randn(v.height, v.width, 4, device=self.device, generator=gen) for _ in range(3)]
-        up[2][..., 2:] = 0
-        self.up[vi] = up
 
     def shading(self, vi, with_sun=True):
         v = self.scene.views[vi]
@@ -238,12 +399,11 @@ class Job:
         self.ctx.render_forward(sh, *self.out)
         return sh
 
-    def step(self, vi):
-        g = self.g
-        for t in g.values():
-            t.zero_()
+    def step(self, vi, buf=0):
+        g = self.gbufs[buf]
+        g["flat"].zero_()
         sh = self.forward(vi)
-        up = self.up[vi]
+        up = self.up_shared
         if self.shadows:
             self.v_sun.zero_()
         self.ctx.render_backward(sh, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"], g["cc"], g["amb"],
@@ -255,6 +415,36 @@ class Job:
             self.P.sun_camera_backward(self.cams[vi][0], v.sun_azimuth, v.sun_elevation, v.sun_viewport, g["dFs"], g["rep"], g["dF"])
 
 
+    def step_device(self, stride=1, buf=0):
+        """The same iteration with every camera read from the device-resident block: the view is
+        selected by the device index, nothing of it is baked into kernel arguments, so ONE captured graph of this function
+        serves all views and all optimiser steps (dF lives in self.dF_all on the device)."""
+        P, g, surf = self.P, self.gbufs[buf], (self.means, self.quats, self.scales, self.logits, self.rgb)
+        g["flat"].zero_()
+        P.camera_chain(self.table, self.dF_all, self.idx, self.block)
+        v = self.scene.views[0]
+        if self.shadows:
+            cur = self.torch.cuda.current_stream()
+            self.side.wait_stream(cur)
+            self.ctx.preprocess_device(self.W, self.H, self.block, P.CAM_VIEW, *surf, stream=self.side)
+            self.sctx.preprocess_device(v.sun_width, v.sun_height, self.block, P.CAM_SUN, *surf)
+            self.sctx.shadow_map(self.sun_depth)
+            cur.wait_stream(self.side)
+            self.v_sun.zero_()
+        else:
+            self.ctx.preprocess_device(self.W, self.H, self.block, P.CAM_VIEW, *surf)
+        self.ctx.render_forward_device(self.block, self.sun_depth, *self.out)
+        up = self.up_shared
+        self.ctx.render_backward_device(self.block, self.sun_depth, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"],
+                                        g["cc"], g["amb"], self.v_sun, g["rep"] if self.shadows else None)
+        if self.shadows:
+            self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], g["dFs"])
+        # cascade (PAPER.md Fig. 1): view-pass dF gradient + adjoint of the sun camera / reprojection -> this view's row of v_dF_all
+        P.camera_chain_backward(self.table, self.dF_all, self.idx, g["dF"], g["dFs"] if self.shadows else None,
+                                g["rep"] if self.shadows else None, None, self.v_dF_all)
+        P.advance_view_index(self.idx, stride, len(self.scene.views))
+
+
 def max_over_ranks(torch, dist, world, value, device):
     """MAX all-reduce of a per-rank scalar (device timings are reported as the max over ranks)."""
     if world <= 1:
@@ -264,28 +454,37 @@ def max_over_ranks(torch, dist, world, value, device):
     return float(t.item())
 
 
-def timed(torch, dist, world, fn, items):
+def timed(torch, dist, world, fn, items, per_step=False):
     """Time fn(item) over items with CUDA events on the current stream; barrier + synchronize on both sides;
-    returns the max over ranks of the elapsed milliseconds."""
+    returns the max over ranks of the elapsed milliseconds (and, with per_step, this rank's per-item times and the
+    host-clock window of the timed region)."""
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(items) + 1 if per_step else 2)]
     torch.cuda.synchronize()
-    e0.record()
-    for it in items:
+    t0 = time.perf_counter()
+    ev[0].record()
+    for k, it in enumerate(items):
         fn(it)
-    e1.record()
+        if per_step:
+            ev[k + 1].record()
+    if not per_step:
+        ev[1].record()
     torch.cuda.synchronize()
+    t1 = time.perf_counter()
     if world > 1:
         dist.barrier()
-    return max_over_ranks(torch, dist, world, e0.elapsed_time(e1), "cuda")
+    total = max_over_ranks(torch, dist, world, ev[0].elapsed_time(ev[-1]), "cuda")
+    if per_step:
+        return total, [ev[k].elapsed_time(ev[k + 1]) for k in range(len(items))], (t0, t1)
+    return total
 
 
-def stage_profile(job, views, peaks):
+def stage_profile(job, views, peaks, fp32_peak_tinst):
     """Per-stage device ms (CUDA events recorded by the library on the launching stream around every kernel of a
     stage), averaged over the launches of the bench's step views; pair counts and the algorithmic work of each kernel
-    (of the last view)."""
+    (of the last view), for both passes."""
     torch, P = job.torch, job.P
     job.ctx.set_profiling(True)
     if job.sctx:
@@ -308,30 +507,42 @@ def stage_profile(job, views, peaks):
     if job.sctx:
         snv, snc = job.sctx.debug_planes()
         pairs.update(sun_evaluated=int(snv.sum().item()), sun_contributing=int(snc.sum().item()), sun_K=job.sctx.sync_status())
-    n, K = job.n, pairs["view_K"]
+    n = job.n
     tiles = ((job.W + 15) // 16) * ((job.H + 15) // 16)
-    passes = (32 + max(1, (tiles - 1).bit_length()) + 7) // 8
     px = job.W * job.H
-    # algorithmic bytes: per surfel / per key / per pixel figures of SURVEY.md 8(d)
-    work = {
-        "preprocess": ("hbm", n * 137.0),
-        # tile-sort binning (the default mode): one-CTA scan of the tile counters, scatter of (depth, id) entries,
-        # per-tile sort; the radix option's figures are (8 + 24 P) B / pair, P = ceil((32 + log2 tiles) / 8) passes
-        "scan": ("hbm", tiles * 12.0),
-        "duplicate": ("hbm", n * 16.0 + K * 8.0),
-        "sort": ("hbm", K * 20.0),
-        "ranges": ("hbm", 0.0),
-        "blend_fwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_FWD),
-        "blend_bwd": ("alu", pairs["view_evaluated"] * INST_EVAL + pairs["view_contributing"] * INST_CONTRIB_BWD),
-        "chain_bwd": ("hbm", n * (80.0 * 2 + 45.0 + 52.0 * 2)),
-    }
+
+    def work(pass_):   # algorithmic bytes / lane-instructions (per surfel / key / pair figures of SURVEY.md 8(d))
+        K, ev, co = pairs[f"{pass_}_K"], pairs[f"{pass_}_evaluated"], pairs[f"{pass_}_contributing"]
+        cf, cb = (INST_CONTRIB_FWD, INST_CONTRIB_BWD) if pass_ == "view" else (INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN)
+        return {
+            "preprocess": ("hbm", n * 137.0, None),
+            "scan": ("hbm", tiles * 12.0, None),
+            "duplicate": ("hbm", n * 16.0 + K * 8.0, None),
+            "sort": ("hbm", K * 20.0, None),
+            "ranges": ("hbm", 0.0, None),
+            "blend_fwd": ("alu", ev * INST_EVAL + co * cf, co * (INST_EVAL + cf)),
+            "blend_bwd": ("alu", ev * INST_EVAL + co * cb, co * (INST_EVAL + cb)),
+            "chain_bwd": ("hbm", n * (80.0 * 2 + 45.0 + 52.0 * 2), None),
+        }
+
     stages = {}
+    wv, ws = work("view"), (work("sun") if job.sctx else None)
     for k, ms in ms_view.items():
-        bound, w = work[k]
-        ach = w / (ms * 1e-3) / (1e12 if bound == "alu" else 1e9) if ms > 0 else 0.0
-        peak = FP32_PEAK_TINST if bound == "alu" else peaks["hbm_gbs"]
-        stages[k] = dict(ms=ms, sun_ms=ms_sun.get(k, 0.0), bound=bound, achieved=ach, peak=peak,
-                         unit="Tinst/s" if bound == "alu" else "GB/s", frac=ach / peak if peak else None)
+        bound, w, useful = wv[k]
+        peak = fp32_peak_tinst if bound == "alu" else peaks["hbm_gbs"]
+        scale = 1e12 if bound == "alu" else 1e9
+        ach = w / (ms * 1e-3) / scale if ms > 0 else 0.0
+        st = dict(ms=ms, sun_ms=ms_sun.get(k, 0.0), bound=bound, achieved=ach, peak=peak, unit="Tinst/s" if bound == "alu" else "GB/s",
+                  frac=ach / peak if peak else None, roofline_ms=w / scale / peak * 1e3)
+        if useful is not None and ms > 0:
+            st["useful_frac"] = useful / (ms * 1e-3) / scale / peak          # contributing pairs only
+        if ws is not None and ms_sun.get(k, 0.0) > 0:
+            _, w2, u2 = ws[k]
+            st["sun_frac"] = w2 / (ms_sun[k] * 1e-3) / scale / peak
+            st["sun_roofline_ms"] = w2 / scale / peak * 1e3
+            if u2 is not None:
+                st["sun_useful_frac"] = u2 / (ms_sun[k] * 1e-3) / scale / peak
+        stages[k] = st
     return stages, pairs, px
 
 
@@ -348,129 +559,146 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
     peaks = load_peaks()
+    sampler = ClockSampler(local)
+    sampler.start()                      # before the warm-up: the samples of the timed window are picked out afterwards
+    # the two issue-rate peaks of the blend kernels' roofline, measured on this device
+    mp = P.measure_peaks(local)
+    derived_tinst = mp["sm_count"] * SM_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+    fp32_peak = mp["fp32_lane_inst_per_s"] / 1e12
     scene = make_scene(args)
-    job = Job(P, torch, scene, device)
+    allreduce = world > 1 and not args.no_allreduce
+    job = Job(P, torch, scene, device, n_grad_buffers=2 if allreduce else 1)
     nviews = len(scene.views)
     warm_views = views_for_rank(rank, world, nviews, args.warmup)
     step_views = views_for_rank(rank + args.warmup * world, world, nviews, args.steps)
     for vi in set(warm_views + step_views):
         job.prepare_view(vi)
+    comm = torch.cuda.Stream(device=device) if allreduce else None
+    state = dict(k=0, pending=[None, None])
+
+    def dp_step(vi):
+        """One data-parallel step: this rank's view, then the all-reduce of its packed gradients on the communication
+        stream, overlapped with the next step (which writes the other gradient buffer)."""
+        b = state["k"] & 1
+        cur = torch.cuda.current_stream()
+        if state["pending"][b] is not None:
+            cur.wait_event(state["pending"][b])          # the all-reduce that last used this buffer has finished
+        job.step(vi, buf=b)
+        done = torch.cuda.Event()
+        done.record(cur)
+        comm.wait_event(done)
+        with torch.cuda.stream(comm):
+            allreduce_sum(dist, job.gbufs[b]["surfel"])
+            fin = torch.cuda.Event()
+            fin.record(comm)
+        state["pending"][b] = fin
+        state["k"] += 1
+
+    def drain():
+        for e in state["pending"]:
+            if e is not None:
+                torch.cuda.current_stream().wait_event(e)
+
+    run_step = dp_step if allreduce else job.step
     for vi in warm_views:
-        job.step(vi)
+        run_step(vi)
+    if allreduce:
+        drain()
     torch.cuda.synchronize()
-    k_ok = job.ctx.sync_status()     # raises on capacity overflow
+    job.ctx.sync_status()     # raises on capacity overflow
     launches0 = P.kernel_launches()
-    sampler = ClockSampler(local)
-    sampler.start()
-    run_step = job.step
     launches_per_step = None
     use_graphs = not args.no_graphs and world == 1   # multi-rank runs launch from the host (no capture beside the NCCL watchdog)
     if use_graphs:
-        # one CUDA graph per view (the camera is baked into the kernel arguments): a step is one graph launch
-        graphs = {}
-        for vi in sorted(set(step_views)):
-            l0 = P.kernel_launches()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                job.step(vi)
-            graphs[vi] = g
-            launches_per_step = P.kernel_launches() - l0
-        for vi in step_views[:3]:
-            graphs[vi].replay()
+        # ONE CUDA graph for all views and all steps: the cameras are device-resident (row f2), the graph advances the view
+        # index itself; a step is one graph launch
+        job.idx.fill_(step_views[0])
+        job.step_device()                      # warm-up of the device path outside the capture
         torch.cuda.synchronize()
-        run_step = lambda vi: graphs[vi].replay()
+        l0 = P.kernel_launches()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            job.step_device()
+        launches_per_step = P.kernel_launches() - l0
+        for _ in range(3):
+            graph.replay()
+        torch.cuda.synchronize()
+        job.idx.fill_(step_views[0])           # views step_views[0], +1, ... (mod the number of views): the same sequence
+        job.v_dF_all.zero_()
+        run_step = lambda vi: graph.replay()
         launches0 = P.kernel_launches()
-    ms_total = timed(torch, dist, world, run_step, step_views)
+    if allreduce:
+        def timed_steps(vi):
+            dp_step(vi)
+        ms_total, per_step, window = timed(torch, dist, world, timed_steps, step_views, per_step=True)
+        drain()
+        torch.cuda.synchronize()
+    else:
+        ms_total, per_step, window = timed(torch, dist, world, run_step, step_views, per_step=True)
     launches = P.kernel_launches() - launches0 if launches_per_step is None else launches_per_step * len(step_views)
-    clocks = sampler.stop()
+    clocks = sampler.stop(*window)
     ms_fwd = timed(torch, dist, world, job.forward, step_views)
     px = job.W * job.H
     ms_step = ms_total / args.steps
     value = world * px / 1e6 / (ms_step * 1e-3)
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms_step,
+                ms_median=float(np.median(per_step)), ms_min=float(np.min(per_step)),
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 config=workload_config(scene, args, world), clocks=clocks, gpu_launches=int(launches),
                 fwd_ms_per_step=ms_fwd / args.steps, fwd_mpixel_s=world * px / 1e6 / (ms_fwd / args.steps * 1e-3))
+    if allreduce:
+        line["allreduce"] = dict(bytes_per_step=job.flat_floats * 4, collective="ncclAllReduce(sum) of the packed surfel gradients",
+                                 overlapped_with="the next step's kernels (double-buffered gradient buffer, communication stream)")
     if rank == 0:
-        stages, pairs, _ = stage_profile(job, step_views, peaks)
+        stages, pairs, _ = stage_profile(job, step_views, peaks, fp32_peak)
         dom = max(stages, key=lambda k: stages[k]["ms"])
         d = stages[dom]
+        traffic, traffic_src = load_traffic()
+        t_dom = (traffic or {}).get(dom)
         line["roofline"] = dict(kernel=dom, bound=d["bound"], achieved=d["achieved"], peak=d["peak"], unit=d["unit"], frac=d["frac"],
-                                traffic=NCU_DRAM_BYTES_PER_LAUNCH.get(dom), traffic_source=NCU_SOURCE, launches_averaged=len(step_views),
-                                executed=NCU_EXECUTED.get(dom),
-                                peak_source=("derived: 148 SM x 128 FP32 lanes x 1.965 GHz (DESIGN.md section 5)" if d["bound"] == "alu"
-                                                           else peaks["source"] + " HBM copy"),
-                                kernel_ms=d["ms"])
+                                useful_frac=d.get("useful_frac"),
+                                traffic=t_dom["dram_bytes"] if t_dom else None, traffic_source=traffic_src, launches_averaged=len(step_views),
+                                executed=dict(warp_inst=t_dom["warp_inst"], issue_active_pct=t_dom["issue_active_pct"]) if t_dom else None,
+                                peak_source=("measured: satsplat_measure_peaks (independent FFMA chains on every sub-partition of this device)"
+                                             if d["bound"] == "alu" else peaks["source"] + " HBM copy (MEASURED_PEAKS.json)"),
+                                peak_derived=derived_tinst if d["bound"] == "alu" else None,
+                                peak_derived_how=f"{mp['sm_count']} SMs x {SM_LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz",
+                                mufu_peak_measured_tops=mp["mufu_per_s"] / 1e12, kernel_ms=d["ms"])
         line["stages"] = stages
         line["pairs"] = pairs
         sun_ms = sum(s["sun_ms"] for s in stages.values())
         view_ms = sum(s["ms"] for s in stages.values())
-        # whole-iteration roofline: sum over kernels of their own roofline time (both passes)
-        roof_ms = 0.0
-        for k, s in stages.items():
-            if s["frac"]:
-                roof_ms += s["ms"] * s["frac"]
-        line["iteration"] = dict(view_pass_kernel_ms=view_ms, sun_pass_kernel_ms=sun_ms, view_pass_roofline_ms=roof_ms,
-                                 view_pass_frac_of_roofline=roof_ms / view_ms if view_ms else None,
-                                 scratch_gb=(job.ctx.scratch_bytes + (job.sctx.scratch_bytes if job.sctx else 0)) / 1e9,
-                                 peak_mem_gb=torch.cuda.max_memory_allocated() / 1e9 + (job.ctx.scratch_bytes + (job.sctx.scratch_bytes if job.sctx else 0)) / 1e9)
-    # ---- the optimiser step, timed on its own: it is not part of the metric's iteration ----
-    if rank == 0:
-        ns = P.adam_state_floats(scene.n)
-        am, av = torch.zeros(ns, device=device), torch.zeros(ns, device=device)
-        pp = [t.clone() for t in (job.means, job.quats, job.scales, job.logits, job.rgb)]
-        gg = [job.g[k] for k in ("m", "q", "s", "l", "c")]
-        lr = [0.075, 0.001, 0.001, 0.05, 0.0025]     # PAPER.md:349 (opacity: not stated, 3DGS's value)
-        for t_ in range(1, 4):
-            P.adam_step(scene.n, *pp, *gg, am, av, lr, step=t_)
-        ms_adam = timed(torch, None, 1, lambda t_: P.adam_step(scene.n, *pp, *gg, am, av, lr, step=t_), range(4, 4 + 20)) / 20
-        ab = scene.n * 13 * 28.0
-        line["adam"] = dict(ms=ms_adam, bound="hbm", achieved=ab / (ms_adam * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                            frac=ab / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_surfel=13 * 28,
-                            note="fused Adam over the 13 N surfel parameters; not included in value / ms_per_step")
-    # ---- the loss stage, timed on its own on the last rendered view ----
-    if rank == 0:
-        vi = step_views[-1]
-        cam = job.cams[vi][0]
-        tgt = torch.rand(job.H, job.W, 4, device=device)
-        scr = torch.empty(P.loss_scratch_floats(job.W, job.H), device=device)
-        vv = [torch.empty(job.H, job.W, 4, device=device) for _ in range(3)]
-        sums = torch.zeros(8, device=device)
-        run_loss = lambda _: P.loss_upstream(cam, job.out[0], job.out[1], job.out[2], tgt, scr, vv[0], vv[1], vv[2], sums)
-        for _ in range(3):
-            run_loss(0)
-        ms_loss = timed(torch, None, 1, run_loss, range(20)) / 20
-        lb = px * 240.0
-        line["loss_stage"] = dict(ms=ms_loss, bound="hbm", achieved=lb / (ms_loss * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                                  frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=240,
-                                  note="L1 + SSIM + distortion + normal consistency -> upstream gradients (2 kernels); not included in value / ms_per_step")
-    # ---- geometry-aware initialisation: one-time work, timed once on a DSM of the site's size ----
-    if rank == 0:
-        side = int(round(1000.0 / 0.3)) if args.config in (3, 4) else 512
-        gen = torch.Generator(device=device); gen.manual_seed(1)
-        dsm = torch.cumsum(torch.randn(side, side, device=device, generator=gen) * 0.05, 1)
-        dsm[side // 4: side // 3, side // 4: side // 2] += 25.0
-        uu = [torch.rand(scene.n, device=device, generator=gen).clamp_(max=0.99999994) for _ in range(3)]
-        P.init_from_dsm(dsm, 0.3, (0.0, 0.0), *uu)
-        ms_init = timed(torch, None, 1, lambda _: P.init_from_dsm(dsm, 0.3, (0.0, 0.0), *uu), range(3)) / 3
-        line["init_stage"] = dict(ms=ms_init, dsm=f"{side}x{side}", samples=scene.n,
-                                  note="area-weighted sampling + frames + exact 3-NN scale from a DSM (9 kernels); one-time, not part of the iteration")
+        # whole-iteration roofline: sum over kernels of their own roofline time, BOTH passes
+        roof_view = sum(s["roofline_ms"] for s in stages.values())
+        roof_sun = sum(s.get("sun_roofline_ms", 0.0) for s in stages.values())
+        scratch = (job.ctx.scratch_bytes + (job.sctx.scratch_bytes if job.sctx else 0)) / 1e9
+        line["iteration"] = dict(view_pass_kernel_ms=view_ms, sun_pass_kernel_ms=sun_ms, view_pass_roofline_ms=roof_view,
+                                 sun_pass_roofline_ms=roof_sun,
+                                 view_pass_frac_of_roofline=roof_view / view_ms if view_ms else None,
+                                 sun_pass_frac_of_roofline=roof_sun / sun_ms if sun_ms else None,
+                                 frac_of_roofline=(roof_view + roof_sun) / (view_ms + sun_ms) if view_ms + sun_ms else None,
+                                 frac_of_roofline_vs_step=(roof_view + roof_sun) / ms_step,
+                                 scratch_gb=scratch, peak_mem_gb=torch.cuda.max_memory_allocated() / 1e9 + scratch)
+    if rank == 0 and not args.no_extras:
+        extras(line, args, job, P, torch, scene, device, peaks, step_views, px)
     # ---- end to end through the C ABI with HOST buffers ----
     if not args.no_e2e:
         vi = step_views[0]
         v = scene.views[vi]
         pin = lambda t: t.detach().cpu().contiguous().pin_memory()
         h_in = [pin(x) for x in (job.means, job.quats, job.scales, job.logits, job.rgb)]
-        h_up = [pin(u) for u in job.up[vi]]
+        h_up = [pin(u) for u in job.up_shared]
         h_out = [torch.empty(v.height, v.width, 4).pin_memory() for _ in range(3)]
         h_g = torch.empty(scene.n * 13 + 23).pin_memory()
-        cam, sun_cam, rep = job.cams[vi]
-        sh = P.Shading.make(cc=v.cc, ambient=v.ambient, reproj=rep, depth_bias=v.depth_bias, slope=v.slope)
+        cam = job.cams[vi][0]
+        sun = P.Sun.from_view(v) if job.shadows else None
+        sh = P.Shading.make(cc=v.cc, ambient=v.ambient, depth_bias=v.depth_bias, slope=v.slope)
         sh.shadows_on = 1 if job.shadows else 0
+        P.reserve_host_staging(job.ctx, job.sctx)
 
         def e2e_step(_):
-            P.iteration_host(job.ctx, job.sctx, cam, sun_cam, sh, scene.n, *h_in, *h_up, *h_out, h_g)
+            P.iteration_host(job.ctx, job.sctx, cam, sun, sh, scene.n, *h_in, *h_up, *h_out, h_g)
         for _ in range(2):
             e2e_step(0)
         n_e2e = max(3, min(args.steps, 10))
@@ -486,26 +714,71 @@ def run_ours(args):
         h2d = scene.n * 56 + 3 * px * 16
         d2h = 3 * px * 16 + (scene.n * 13 + 23) * 4
         line["e2e"] = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                           ms_per_step=1e3 * dt / n_e2e, steps=n_e2e, api="satsplat_iteration_host (pinned host buffers)")
+                           ms_per_step=1e3 * dt / n_e2e, steps=n_e2e,
+                           api="satsplat_iteration_host (pinned host buffers; same work as the device step, cascade chain included)")
     # ---- the oracle beside it (rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import oracle as orc
-        orc.build()
-        dt, nth = oracle_iteration_seconds(scene, step_views[0])
-        line["cpu_baseline"] = dict(value=px / 1e6 / dt, unit=UNIT, cores=nth, kind="oracle", seconds=dt,
-                                    sample=f"1 full view iteration (view {step_views[0]} of {nviews}) of the same workload, {nth} threads")
+        line["cpu_baseline"] = cpu_baseline_block(scene, step_views[0], px, nviews)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
+def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
+    """The NEXT rows of SURVEY.md section 8 that sit outside the metric's iteration, each timed on its own."""
+    # ---- the optimiser step (row f3) ----
+    ns = P.adam_state_floats(scene.n)
+    am, av = torch.zeros(ns, device=device), torch.zeros(ns, device=device)
+    pp = [t.clone() for t in (job.means, job.quats, job.scales, job.logits, job.rgb)]
+    gg = [job.g[k] for k in ("m", "q", "s", "l", "c")]
+    lr = [0.075, 0.001, 0.001, 0.05, 0.0025]     # PAPER.md:349 (opacity: not stated, 3DGS's value)
+    for t_ in range(1, 4):
+        P.adam_step(scene.n, *pp, *gg, am, av, lr, step=t_)
+    ms_adam = timed(torch, None, 1, lambda t_: P.adam_step(scene.n, *pp, *gg, am, av, lr, step=t_), range(4, 4 + 20)) / 20
+    ab = scene.n * 13 * 28.0
+    line["adam"] = dict(ms=ms_adam, bound="hbm", achieved=ab / (ms_adam * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                        frac=ab / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_surfel=13 * 28,
+                        note="fused Adam over the 13 N surfel parameters; not included in value / ms_per_step")
+    # ---- the loss stage (row f1), on the last rendered view ----
+    vi = step_views[-1]
+    cam = job.cams[vi][0]
+    tgt = torch.rand(job.H, job.W, 4, device=device)
+    scr = torch.empty(P.loss_scratch_floats(job.W, job.H), device=device)
+    vv = [torch.empty(job.H, job.W, 4, device=device) for _ in range(3)]
+    sums = torch.zeros(8, device=device)
+    run_loss = lambda _: P.loss_upstream(cam, job.out[0], job.out[1], job.out[2], tgt, scr, vv[0], vv[1], vv[2], sums)
+    for _ in range(3):
+        run_loss(0)
+    ms_loss = timed(torch, None, 1, run_loss, range(20)) / 20
+    lb = px * 240.0
+    line["loss_stage"] = dict(ms=ms_loss, bound="hbm", achieved=lb / (ms_loss * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                              frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=240,
+                              note="L1 + SSIM + distortion + normal consistency -> upstream gradients (2 kernels); not included in value / ms_per_step")
+    # ---- geometry-aware initialisation (row f4): one-time work, on a DSM of the site's size ----
+    side = int(round(1000.0 / 0.3)) if args.config in (3, 4) else 512
+    gen = torch.Generator(device=device); gen.manual_seed(1)
+    dsm = torch.cumsum(torch.randn(side, side, device=device, generator=gen) * 0.05, 1)
+    dsm[side // 4: side // 3, side // 4: side // 2] += 25.0
+    uu = [torch.rand(scene.n, device=device, generator=gen).clamp_(max=0.99999994) for _ in range(3)]
+    P.init_from_dsm(dsm, 0.3, (0.0, 0.0), *uu)
+    ms_init = timed(torch, None, 1, lambda _: P.init_from_dsm(dsm, 0.3, (0.0, 0.0), *uu), range(3)) / 3
+    line["init_stage"] = dict(ms=ms_init, dsm=f"{side}x{side}", samples=scene.n,
+                              note="area-weighted sampling + frames + exact 3-NN scale from a DSM (9 kernels); one-time, not part of the iteration")
+
+
 def main():
     args = parse()
+    if args.record_traffic:
+        record_traffic(args.record_traffic)
+        return
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_ours(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not launched by torchrun: start one process per GPU ourselves and hand over
+        sys.exit(subprocess.call(spawn_command(args, free_port())))
+    run_ours(args)
 
 
 if __name__ == "__main__":

@@ -74,7 +74,7 @@ typedef struct {
 } satsplat_shading;
 
 /* ---- lifetime ------------------------------------------------------------------------------------------ */
-/* Allocates all scratch on `device` (cudaMalloc; the only allocating call).  max_duplicates bounds K, the
+/* Allocates all scratch on `device` (cudaMalloc; the only allocating call besides satsplat_reserve_host_staging).  max_duplicates bounds K, the
  * number of (tile, surfel) pairs of one pass. */
 int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t max_width, int32_t max_height,
                     int64_t max_duplicates);
@@ -144,18 +144,107 @@ int satsplat_shadow_map_backward(satsplat_ctx* sun_ctx, const float* v_sun_depth
                                  float* v_scales, float* v_opacity_logits, float* v_dF_sun /*[8]*/,
                                  satsplat_stream stream);
 
+/* The sun of one view: angles (radians; azimuth from +X toward +Y, elevation above the horizon, Eq. S2), the size of
+ * its depth map and the 2-D viewport (scale x, scale y, shift x, shift y) that fits the flattened footprint in it. */
+typedef struct {
+  float azimuth, elevation;
+  int32_t width, height;
+  float viewport[4];
+} satsplat_sun;
+
+/* ---- (f2) device-resident cameras: the cascade camera chain of PAPER.md:155-176, Fig. 1 --------------------------------
+ * With dF stepped on the device by the optimiser every iteration, cameras baked into kernel arguments would force a
+ * re-capture of the step's CUDA graph per view and per step.  Here the per-view constants live in a DEVICE array of
+ * satsplat_view_params, dF in a DEVICE [V,8] array, the current view in a DEVICE int32, and satsplat_camera_chain
+ * (one tiny kernel) builds from them a DEVICE camera block:
+ *   floats [0,16) view camera, [16,32) sun camera, [32,48) nearby camera, each (F'[8], view_dir[3], b_z, z_bg, bg[3]);
+ *   [48,76) the view's shading constants: cc[12], ambient[3], reproj[8], depth_bias, slope; [76,80) unused.
+ * The *_device calls read their camera / shading from that block through a pointer. */
+#define SATSPLAT_CAMERA_BLOCK_FLOATS 80
+#define SATSPLAT_CAM_VIEW 0
+#define SATSPLAT_CAM_SUN 1
+#define SATSPLAT_CAM_NEARBY 2
+
+typedef struct {            /* constants of one view; fill with satsplat_view_params_fill, then copy to the device */
+  float F[8];               /* 2x4 world -> pixel (Eq. 2, 7); dF is NOT here: it is the learnable [V,8] array          */
+  float view_dir[3];
+  float b_z;
+  float z_bg;
+  float bg_rgb[3];
+  float cc[12];             /* Eq. 1 */
+  float ambient[3];
+  float depth_bias;
+  float slope;
+  float nearby_d_azimuth;   /* perturbation of the azimuth / elevation of d_main = B_x x B_y for the nearby camera     */
+  float nearby_d_elevation; /* (PAPER.md:176); radians                                                                 */
+  float pad0;
+  float sun_viewport[4];
+  double sun_s[2];          /* (cos phi / tan theta, sin phi / tan theta) of Eq. S2, from the sun angles (metadata)     */
+  float sun_view_dir[3];
+  float pad1;
+} satsplat_view_params;
+
+/* HOST helper: fills `out` from the host structs (`shading` gives cc, ambient, depth_bias, slope; `sun` the angles and
+ * viewport; both may be NULL = identity colour correction / no sun).  The trigonometry of Eq. S2 is done here, once,
+ * in double, exactly as satsplat_sun_camera does it, so that the device-built sun camera is bit-equal to the helper's. */
+int satsplat_view_params_fill(const satsplat_camera* cam, const satsplat_shading* shading, const satsplat_sun* sun,
+                              float nearby_d_azimuth, float nearby_d_elevation, satsplat_view_params* out);
+
+/* Builds the camera block of view *view_index (DEVICE int32; NULL = view 0) from views[V] and dF[V,8] (DEVICE; dF may be
+ * NULL = zero): F' = F + dF (Eq. 15), sun camera + reprojection constants (Eq. 16 + viewport, bit-equal to
+ * satsplat_sun_camera), nearby camera, shading constants.  One kernel, no host synchronisation. */
+int satsplat_camera_chain(const satsplat_view_params* views, const float* dF, const int32_t* view_index, float* block,
+                          satsplat_stream stream);
+
+/* Adjoint of satsplat_camera_chain with respect to dF: v_dF_all[*view_index] += v_dF_view (the view pass's own gradient,
+ * DEVICE [8]) + adjoint of the sun camera applied to v_F_sun (sun pass) and v_reproj (shadow test) + adjoint of the
+ * nearby camera applied to v_F_nearby (a nearby-view pass).  Any of the four [8] inputs may be NULL (= zero).
+ * v_dF_all DEVICE [V,8], accumulated into. */
+int satsplat_camera_chain_backward(const satsplat_view_params* views, const float* dF, const int32_t* view_index,
+                                   const float* v_dF_view, const float* v_F_sun, const float* v_reproj, const float* v_F_nearby,
+                                   float* v_dF_all, satsplat_stream stream);
+
+/* *view_index = (*view_index + stride) % n_views on the device (so that a captured graph can walk through the views). */
+int satsplat_advance_view_index(int32_t* view_index, int32_t stride, int32_t n_views, satsplat_stream stream);
+
+/* satsplat_preprocess with the camera `which` (SATSPLAT_CAM_*) of a DEVICE camera block; width / height (host values,
+ * fixed per context) size the grid.  The context then renders from the device camera: satsplat_shadow_map,
+ * satsplat_shadow_map_backward work unchanged; the view pass uses the two *_device calls below. */
+int satsplat_preprocess_device(satsplat_ctx* ctx, int32_t width, int32_t height, const float* block, int32_t which, int64_t N,
+                               const float* means, const float* quats, const float* scales, const float* opacity_logits,
+                               const float* rgb, satsplat_stream stream);
+
+/* satsplat_render_forward / satsplat_render_backward with cc, ambient, reproj, depth_bias, slope read from the block;
+ * sun_depth DEVICE [sun_height, sun_width] or NULL (= shadows off).  SATSPLAT_E_STATE unless the context was
+ * preprocessed by satsplat_preprocess_device. */
+int satsplat_render_forward_device(satsplat_ctx* ctx, const float* block, const float* sun_depth, int32_t sun_width,
+                                   int32_t sun_height, float* out_rgba, float* out_geom, float* out_aux, satsplat_stream stream);
+int satsplat_render_backward_device(satsplat_ctx* ctx, const float* block, const float* sun_depth, int32_t sun_width,
+                                    int32_t sun_height, const float* v_rgba, const float* v_geom, const float* v_aux,
+                                    float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
+                                    float* v_dF /*[8]*/, float* v_cc /*[12]*/, float* v_ambient /*[3]*/,
+                                    float* v_sun_depth /*[Hs,Ws]*/, float* v_reproj /*[8]*/, satsplat_stream stream);
+
+
+/* Allocates the device staging buffers satsplat_iteration_host needs (sized for the contexts' maxima) and its two
+ * copy streams.  The only allocating call besides satsplat_create; idempotent; `sun_ctx` may be NULL. */
+int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx);
+
 /* One whole training-view iteration with HOST buffers (end-to-end leg of the benchmark): copies the surfels and
- * upstream gradients host->device, runs sun pass (if shading->shadows_on; `sun_cam` then non-NULL and
- * shading->sun_depth ignored) + view pass forward + backward of both, copies images and gradients back, and
- * synchronises `stream`.  h_* are HOST pointers (pinned memory recommended); h_grads = packed
- * [N*13 + 8 + 12 + 3] floats: means(3N) quats(4N) scales(2N) logits(N) rgb(3N) dF(8) cc(12) ambient(3).
- * `sun_ctx` may be NULL when shadows are off. */
+ * upstream gradients host->device, builds the sun camera and the reprojection constants from F' = F + dF (Eq. 16;
+ * shading->reproj / sun_depth are ignored when shading->shadows_on), runs sun pass + view pass forward + backward of
+ * both + the cascade chain of the sun camera back into dF (Fig. 1), copies images and gradients back, and
+ * synchronises `stream`: exactly the work of the staged device calls.  h_* are HOST pointers (pinned memory
+ * recommended); h_grads = packed [N*13 + 8 + 12 + 3] floats: means(3N) quats(4N) scales(2N) logits(N) rgb(3N) dF(8)
+ * cc(12) ambient(3), any N (the device staging is padded to 16-byte boundaries internally).  All sizes are validated
+ * before the first copy.  `sun_ctx` / `sun` may be NULL when shadows are off.  SATSPLAT_E_STATE if
+ * satsplat_reserve_host_staging has not been called. */
 int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
-                            const satsplat_camera* sun_cam, const satsplat_shading* shading, int64_t N,
+                            const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
                             const float* h_means, const float* h_quats, const float* h_scales,
-                            const float* h_opacity_logits, const float* h_rgb, const float* h_v_rgba,
-                            const float* h_v_geom, const float* h_v_aux, float* h_out_rgba, float* h_out_geom,
-                            float* h_out_aux, float* h_grads, satsplat_stream stream);
+                            const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                            const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                            float* h_grads, satsplat_stream stream);
 
 /* ---- optimiser step ------------------------------------------------------- */
 /* One Adam step [Kingma & Ba 2015, Alg. 1] over the five surfel groups with per-group learning rates (PAPER.md:349:

@@ -81,6 +81,32 @@ class Shading(C.Structure):
         return s
 
 
+class Sun(C.Structure):
+    """satsplat_sun (include/satsplat.h)."""
+    _fields_ = [("azimuth", C.c_float), ("elevation", C.c_float), ("width", C.c_int32), ("height", C.c_int32),
+                ("viewport", C.c_float * 4)]
+
+    @classmethod
+    def from_view(cls, v):
+        s = cls()
+        s.azimuth, s.elevation = float(v.sun_azimuth), float(v.sun_elevation)
+        s.width, s.height = int(v.sun_width), int(v.sun_height)
+        s.viewport[:] = [float(x) for x in v.sun_viewport]
+        return s
+
+
+class ViewParams(C.Structure):
+    """satsplat_view_params (include/satsplat.h): the constants of one view of the device-resident camera chain."""
+    _fields_ = [("F", C.c_float * 8), ("view_dir", C.c_float * 3), ("b_z", C.c_float), ("z_bg", C.c_float), ("bg_rgb", C.c_float * 3),
+                ("cc", C.c_float * 12), ("ambient", C.c_float * 3), ("depth_bias", C.c_float), ("slope", C.c_float),
+                ("nearby_d_azimuth", C.c_float), ("nearby_d_elevation", C.c_float), ("pad0", C.c_float),
+                ("sun_viewport", C.c_float * 4), ("sun_s", C.c_double * 2), ("sun_view_dir", C.c_float * 3), ("pad1", C.c_float)]
+
+
+CAMERA_BLOCK_FLOATS = 80
+CAM_VIEW, CAM_SUN, CAM_NEARBY = 0, 1, 2
+
+
 def build(force: bool = False) -> str:
     from .build import build as _b
     return _b(force=force)
@@ -122,7 +148,8 @@ def lib():
         L.satsplat_shadow_map.argtypes = [vp, vp, vp]
         L.satsplat_render_backward.argtypes = [vp, C.POINTER(Shading)] + [vp] * 14
         L.satsplat_shadow_map_backward.argtypes = [vp] * 8
-        L.satsplat_iteration_host.argtypes = [vp, vp, C.POINTER(Camera), C.POINTER(Camera), C.POINTER(Shading), i64] + [vp] * 13
+        L.satsplat_iteration_host.argtypes = [vp, vp, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading), i64] + [vp] * 13
+        L.satsplat_reserve_host_staging.argtypes = [vp, vp]
         L.satsplat_sync_status.argtypes = [vp, C.POINTER(i64), vp]
         L.satsplat_debug_bins.argtypes = [vp, C.POINTER(i64)] + [C.POINTER(vp)] * 5 + [vp]
         L.satsplat_debug_records.argtypes = [vp, vp, vp, vp]
@@ -130,6 +157,13 @@ def lib():
         L.satsplat_set_profiling.argtypes = [vp, i32]
         L.satsplat_set_option.argtypes = [vp, i32, i32]
         L.satsplat_stage_ms.argtypes = [vp, C.POINTER(f32)]
+        L.satsplat_view_params_fill.argtypes = [C.POINTER(Camera), C.POINTER(Shading), C.POINTER(Sun), f32, f32, C.POINTER(ViewParams)]
+        L.satsplat_camera_chain.argtypes = [vp] * 5
+        L.satsplat_camera_chain_backward.argtypes = [vp] * 9
+        L.satsplat_advance_view_index.argtypes = [vp, i32, i32, vp]
+        L.satsplat_preprocess_device.argtypes = [vp, i32, i32, vp, i32, i64, vp, vp, vp, vp, vp, vp]
+        L.satsplat_render_forward_device.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, vp]
+        L.satsplat_render_backward_device.argtypes = [vp, vp, vp, i32, i32] + [vp] * 14
         L.satsplat_measure_peaks.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
         _LIB = L
     return _LIB
@@ -198,6 +232,45 @@ def sun_camera_backward(view: Camera, azimuth, elevation, viewport, v_F_sun, v_r
     vp = (C.c_float * 4)(*[float(x) for x in viewport])
     rc = lib().satsplat_sun_camera_backward(C.byref(view), float(azimuth), float(elevation), vp, _ptr(v_F_sun), _ptr(v_reproj),
                                             _ptr(v_dF), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def view_params_table(views, nearby=None, device="cuda"):
+    """Device-resident array of satsplat_view_params for `views` (objects with the fields of satsplat_scenes.View), built
+    with satsplat_view_params_fill (HOST) and copied up once.  `nearby[i]` = (d_azimuth, d_elevation) of view i's nearby
+    camera.  Returns a uint8 device tensor [V, sizeof(satsplat_view_params)]."""
+    arr = (ViewParams * len(views))()
+    for i, v in enumerate(views):
+        cam = Camera.from_view(v)
+        sh = Shading.make(cc=v.cc, ambient=v.ambient, depth_bias=v.depth_bias, slope=v.slope)
+        sun = Sun.from_view(v) if getattr(v, "shadows_on", False) else None
+        da, de = (0.0, 0.0) if nearby is None else nearby[i]
+        rc = lib().satsplat_view_params_fill(C.byref(cam), C.byref(sh), None if sun is None else C.byref(sun), float(da), float(de),
+                                             C.byref(arr[i]))
+        if rc:
+            raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+    raw = torch.frombuffer(bytearray(bytes(arr)), dtype=torch.uint8).view(len(views), C.sizeof(ViewParams))
+    return raw.to(device)
+
+
+def camera_chain(views_dev, dF_dev, view_index_dev, block_dev, stream=None):
+    """satsplat_camera_chain: block_dev (device fp32 [80]) <- cameras of view *view_index_dev (device int32 [1])."""
+    rc = lib().satsplat_camera_chain(_ptr(views_dev, torch.uint8), _ptr(dF_dev), _ptr(view_index_dev, torch.int32), _ptr(block_dev), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def camera_chain_backward(views_dev, dF_dev, view_index_dev, v_dF_view, v_F_sun, v_reproj, v_F_nearby, v_dF_all, stream=None):
+    """satsplat_camera_chain_backward: v_dF_all[view] += v_dF_view + cascade adjoints (device tensors; inputs may be None)."""
+    rc = lib().satsplat_camera_chain_backward(_ptr(views_dev, torch.uint8), _ptr(dF_dev), _ptr(view_index_dev, torch.int32), _ptr(v_dF_view), _ptr(v_F_sun),
+                                              _ptr(v_reproj), _ptr(v_F_nearby), _ptr(v_dF_all), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def advance_view_index(view_index_dev, stride, n_views, stream=None):
+    rc = lib().satsplat_advance_view_index(_ptr(view_index_dev, torch.int32), int(stride), int(n_views), _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
 
@@ -304,6 +377,29 @@ class Context:
         self._rc(lib().satsplat_preprocess(self._h, C.byref(cam), n, _ptr(means), _ptr(quats), _ptr(scales),
                                            _ptr(opacity_logits), _ptr(rgb), _stream(stream)))
 
+    def preprocess_device(self, width, height, block, which, means, quats, scales, opacity_logits, rgb, stream=None):
+        """satsplat_preprocess_device: camera `which` (CAM_*) of the device camera block `block` (fp32 [80])."""
+        n = int(means.shape[0])
+        self._keep["in"] = (means, quats, scales, opacity_logits, rgb, block)
+        cam = Camera()
+        cam.width, cam.height = int(width), int(height)
+        self.cam, self.n = cam, n
+        self._rc(lib().satsplat_preprocess_device(self._h, int(width), int(height), _ptr(block), int(which), n, _ptr(means), _ptr(quats),
+                                                  _ptr(scales), _ptr(opacity_logits), _ptr(rgb), _stream(stream)))
+
+    def render_forward_device(self, block, sun_depth, out_rgba=None, out_geom=None, out_aux=None, stream=None):
+        sh, sw = (0, 0) if sun_depth is None else (int(sun_depth.shape[0]), int(sun_depth.shape[1]))
+        self._rc(lib().satsplat_render_forward_device(self._h, _ptr(block), _ptr(sun_depth), sw, sh, _ptr(out_rgba), _ptr(out_geom),
+                                                      _ptr(out_aux), _stream(stream)))
+
+    def render_backward_device(self, block, sun_depth, v_rgba, v_geom, v_aux, v_means, v_quats, v_scales, v_opacity_logits, v_rgb,
+                               v_dF=None, v_cc=None, v_ambient=None, v_sun_depth=None, v_reproj=None, stream=None):
+        sh, sw = (0, 0) if sun_depth is None else (int(sun_depth.shape[0]), int(sun_depth.shape[1]))
+        self._rc(lib().satsplat_render_backward_device(self._h, _ptr(block), _ptr(sun_depth), sw, sh, _ptr(v_rgba), _ptr(v_geom),
+                                                       _ptr(v_aux), _ptr(v_means), _ptr(v_quats), _ptr(v_scales), _ptr(v_opacity_logits),
+                                                       _ptr(v_rgb), _ptr(v_dF), _ptr(v_cc), _ptr(v_ambient), _ptr(v_sun_depth),
+                                                       _ptr(v_reproj), _stream(stream)))
+
     def render_forward(self, shading: Shading, out_rgba=None, out_geom=None, out_aux=None, stream=None):
         self._rc(lib().satsplat_render_forward(self._h, C.byref(shading), _ptr(out_rgba), _ptr(out_geom), _ptr(out_aux), _stream(stream)))
 
@@ -374,9 +470,14 @@ class Context:
         return dict(zip(STAGES, [float(x) for x in ms]))
 
 
-def iteration_host(ctx: Context, sun_ctx, cam: Camera, sun_cam, shading: Shading, n, h_means, h_quats, h_scales, h_logits,
+def reserve_host_staging(ctx: Context, sun_ctx=None):
+    """satsplat_reserve_host_staging: allocate the device staging of iteration_host (explicit, never lazy)."""
+    ctx._rc(lib().satsplat_reserve_host_staging(ctx._h, None if sun_ctx is None else sun_ctx._h))
+
+
+def iteration_host(ctx: Context, sun_ctx, cam: Camera, sun, shading: Shading, n, h_means, h_quats, h_scales, h_logits,
                    h_rgb, h_v_rgba, h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, stream=None):
-    """satsplat_iteration_host: one full training-view iteration with HOST (pinned CPU) tensors."""
+    """satsplat_iteration_host: one full training-view iteration with HOST (pinned CPU) tensors; `sun` is a Sun."""
     def hp(t):
         if t is None:
             return None
@@ -384,7 +485,7 @@ def iteration_host(ctx: Context, sun_ctx, cam: Camera, sun_cam, shading: Shading
             raise ValueError("expected contiguous fp32 CPU tensors")
         return t.data_ptr()
     rc = lib().satsplat_iteration_host(ctx._h, None if sun_ctx is None else sun_ctx._h, C.byref(cam),
-                                       None if sun_cam is None else C.byref(sun_cam), C.byref(shading), int(n), hp(h_means),
+                                       None if sun is None else C.byref(sun), C.byref(shading), int(n), hp(h_means),
                                        hp(h_quats), hp(h_scales), hp(h_logits), hp(h_rgb), hp(h_v_rgba), hp(h_v_geom),
                                        hp(h_v_aux), hp(h_out_rgba), hp(h_out_geom), hp(h_out_aux), hp(h_grads), _stream(stream))
     ctx._rc(rc)

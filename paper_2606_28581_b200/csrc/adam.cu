@@ -84,7 +84,8 @@ cudaError_t launch_adam(int64_t N, float* const params[5], const float* const gr
   A.inv_sqrt_c2 = (float)(1.0 / sqrt(1.0 - pow((double)beta2, (double)step)));
   const long long blocks = (vec + 255) / 256;
   ++g_kernel_launches;
-  adam_kernel<<<(int)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, s>>>(A);
+  const int64_t cap = (int64_t)current_sm_count() * 16;
+  adam_kernel<<<(int)(blocks < cap ? blocks : cap), 256, 0, s>>>(A);
   return cudaGetLastError();
 }
 

@@ -5,12 +5,13 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include "camera_math.cuh"
 #include "internal.cuh"
 
 using namespace satsplat;
 
 namespace satsplat {
-long long g_kernel_launches = 0;
+std::atomic<long long> g_kernel_launches{0};
 }
 
 namespace {
@@ -91,7 +92,7 @@ extern "C" {
 
 const char* satsplat_version(void) { return "satsplat-b200 0.1 (sm_100a)"; }
 
-int64_t satsplat_kernel_launches(void) { return (int64_t)g_kernel_launches; }
+int64_t satsplat_kernel_launches(void) { return (int64_t)g_kernel_launches.load(); }
 
 const char* satsplat_last_error(const satsplat_ctx* ctx) { return ctx ? ctx->err : g_err; }
 
@@ -112,6 +113,9 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   ctx->max_w = max_w;
   ctx->max_h = max_h;
   cudaError_t e = cudaSetDevice(device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
+  if (e == cudaSuccess) e = init_blend_backward_attrs();
+  if (e == cudaSuccess) e = init_binning_attrs();
   const size_t N = (size_t)max_surfels, K = (size_t)max_dup;
   const size_t tiles = (size_t)((max_w + kTile - 1) / kTile) * (size_t)((max_h + kTile - 1) / kTile);
   const size_t px = (size_t)max_w * (size_t)max_h;
@@ -189,32 +193,12 @@ int satsplat_sun_camera(const satsplat_camera* view, float azimuth, float elevat
   if (!(fabs(te) > 1e-12)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: elevation must be non-zero");
   double Fp[8];
   for (int i = 0; i < 8; ++i) Fp[i] = (double)(float)(view->F[i] + view->dF[i]);  // the camera the rasteriser uses
-  const double s[3] = {cos((double)azimuth) / te, sin((double)azimuth) / te, 1.0};  // Eq. S2
-  double S[2][4];
-  for (int r = 0; r < 2; ++r) {
-    const double* B = Fp + 4 * r;
-    const double Bs = B[0] * s[0] + B[1] * s[1] + B[2] * s[2];
-    const double sc = viewport[r], tr = viewport[2 + r];
-    S[r][0] = sc * B[0];
-    S[r][1] = sc * B[1];
-    S[r][2] = sc * (B[2] - Bs);  // Eq. 16: B (I - [0 0 s])
-    S[r][3] = sc * B[3] + tr;
-  }
-  const double det = Fp[0] * Fp[5] - Fp[1] * Fp[4];
-  if (!(fabs(det) > 0)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: singular view camera");
-  const double Bi[2][2] = {{Fp[5] / det, -Fp[1] / det}, {-Fp[4] / det, Fp[0] / det}};
+  const double s0 = cos((double)azimuth) / te, s1 = sin((double)azimuth) / te;     // Eq. S2
   memset(sun_out, 0, sizeof(*sun_out));
   sun_out->width = sun_w;
   sun_out->height = sun_h;
-  for (int r = 0; r < 2; ++r) {
-    for (int c = 0; c < 4; ++c) sun_out->F[4 * r + c] = (float)S[r][c];
-    const double Rx0 = S[r][0] * Bi[0][0] + S[r][1] * Bi[1][0];
-    const double Rx1 = S[r][0] * Bi[0][1] + S[r][1] * Bi[1][1];
-    reproj_out[4 * r + 0] = (float)Rx0;
-    reproj_out[4 * r + 1] = (float)Rx1;
-    reproj_out[4 * r + 2] = (float)(S[r][2] - (Rx0 * Fp[2] + Rx1 * Fp[6]));
-    reproj_out[4 * r + 3] = (float)(S[r][3] - (Rx0 * Fp[3] + Rx1 * Fp[7]));
-  }
+  if (!sun_camera_math(Fp, s0, s1, viewport, sun_out->F, reproj_out))             // Eq. 16 + viewport; shared with the device chain
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_sun_camera: singular view camera");
   const double ce = cos((double)elevation);
   sun_out->view_dir[0] = (float)(-cos((double)azimuth) * ce);
   sun_out->view_dir[1] = (float)(-sin((double)azimuth) * ce);
@@ -325,18 +309,10 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
   return SATSPLAT_OK;
 }
 
-int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
-                        const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
-                        satsplat_stream stream) {
-  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_preprocess: ctx is NULL");
-  if (!cam || N < 0 || (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb)))
-    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: NULL argument");
-  if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: N exceeds max_surfels");
-  if (cam->width <= 0 || cam->height <= 0 || cam->width > ctx->max_w || cam->height > ctx->max_h)
-    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: image size exceeds the context");
-  cudaStream_t s = (cudaStream_t)stream;
-  CU(cudaSetDevice(ctx->device));
-  set_camera(ctx, cam);
+namespace {
+// (a1) + (a2) on the context's current camera (host copy in ctx->cam, or the device record ctx->cam_dev)
+int preprocess_common(satsplat_ctx* ctx, int64_t N, const float* means, const float* quats, const float* scales,
+                      const float* opacity_logits, const float* rgb, cudaStream_t s) {
   ctx->N = N;
   ctx->in_means = means; ctx->in_quats = quats; ctx->in_scales = scales; ctx->in_logits = opacity_logits;
   ctx->preprocessed = 0;
@@ -359,21 +335,104 @@ int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N
   ctx->preprocessed = 1;
   return SATSPLAT_OK;
 }
+}  // namespace
+
+int satsplat_preprocess(satsplat_ctx* ctx, const satsplat_camera* cam, int64_t N, const float* means,
+                        const float* quats, const float* scales, const float* opacity_logits, const float* rgb,
+                        satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_preprocess: ctx is NULL");
+  if (!cam || N < 0 || (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb)))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: NULL argument");
+  if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: N exceeds max_surfels");
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > ctx->max_w || cam->height > ctx->max_h)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess: image size exceeds the context");
+  CU(cudaSetDevice(ctx->device));
+  set_camera(ctx, cam);
+  ctx->cam_dev = nullptr;
+  return preprocess_common(ctx, N, means, quats, scales, opacity_logits, rgb, (cudaStream_t)stream);
+}
+
+int satsplat_preprocess_device(satsplat_ctx* ctx, int32_t width, int32_t height, const float* block, int32_t which, int64_t N,
+                               const float* means, const float* quats, const float* scales, const float* opacity_logits,
+                               const float* rgb, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_preprocess_device: ctx is NULL");
+  if (!block || which < 0 || which > 2 || N < 0 || (N > 0 && (!means || !quats || !scales || !opacity_logits || !rgb)))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess_device: bad argument");
+  if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess_device: N exceeds max_surfels");
+  if (width <= 0 || height <= 0 || width > ctx->max_w || height > ctx->max_h)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_preprocess_device: image size exceeds the context");
+  CU(cudaSetDevice(ctx->device));
+  memset(&ctx->cam, 0, sizeof(ctx->cam));           // the float fields live on the device; only the sizes are host values
+  ctx->cam.W = width;
+  ctx->cam.H = height;
+  ctx->cam.TX = (width + kTile - 1) / kTile;
+  ctx->cam.TY = (height + kTile - 1) / kTile;
+  ctx->cam_dev = block + kCamFloats * which;
+  return preprocess_common(ctx, N, means, quats, scales, opacity_logits, rgb, (cudaStream_t)stream);
+}
+
+namespace {
+int forward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev, float* out_rgba, float* out_geom, float* out_aux,
+                   cudaStream_t s) {
+  clear_stage_marks(ctx, {5, 6, 7});
+  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, sh_dev, out_rgba, out_geom, out_aux, nullptr, false, s)); }
+  ctx->forwarded = 1;
+  ctx->depth_only = 0;
+  return SATSPLAT_OK;
+}
+
+int backward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
+                    const float* v_aux, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
+                    float* v_dF, float* v_cc, float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s) {
+  clear_stage_marks(ctx, {6, 7});
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
+    CU(launch_blend_backward(ctx, sh, sh_dev, v_rgba, v_geom, v_aux, nullptr, false, v_cc, v_ambient, v_sun_depth, v_reproj, s));
+    if (v_cc) CU(launch_add_small(v_cc, ctx->red_buf, 12, s));
+    if (v_ambient) CU(launch_add_small(v_ambient, ctx->red_buf + 12, 3, s));
+    if (v_reproj) CU(launch_add_small(v_reproj, ctx->red_buf + 15, 8, s));
+  }
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
+    CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
+                             v_opacity_logits, v_rgb, v_dF, s));
+  }
+  return SATSPLAT_OK;
+}
+
+// shading of the *_device calls: the float constants come from the block, the sun map and its size from the caller
+DevShading device_shading(const float* sun_depth, int32_t sun_w, int32_t sun_h) {
+  DevShading d;
+  memset(&d, 0, sizeof(d));
+  d.shadows_on = sun_depth ? 1 : 0;
+  d.sun_depth = sun_depth;
+  d.sun_w = sun_w;
+  d.sun_h = sun_h;
+  return d;
+}
+}  // namespace
 
 int satsplat_render_forward(satsplat_ctx* ctx, const satsplat_shading* shading, float* out_rgba, float* out_geom,
                             float* out_aux, satsplat_stream stream) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_forward: ctx is NULL");
   if (!ctx->preprocessed) return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_forward: call satsplat_preprocess first");
+  if (ctx->cam_dev) return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_forward: device camera in use, call satsplat_render_forward_device");
   if (shading && shading->shadows_on && (!shading->sun_depth || shading->sun_width <= 0 || shading->sun_height <= 0))
     return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_forward: shadows_on without a sun depth map");
-  cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
-  const DevShading sh = make_shading(shading);
-  clear_stage_marks(ctx, {5, 6, 7});
-  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, out_rgba, out_geom, out_aux, nullptr, false, s)); }
-  ctx->forwarded = 1;
-  ctx->depth_only = 0;
-  return SATSPLAT_OK;
+  return forward_common(ctx, make_shading(shading), nullptr, out_rgba, out_geom, out_aux, (cudaStream_t)stream);
+}
+
+int satsplat_render_forward_device(satsplat_ctx* ctx, const float* block, const float* sun_depth, int32_t sun_width,
+                                   int32_t sun_height, float* out_rgba, float* out_geom, float* out_aux, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_forward_device: ctx is NULL");
+  if (!ctx->preprocessed || !ctx->cam_dev)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_forward_device: call satsplat_preprocess_device first");
+  if (!block || (sun_depth && (sun_width <= 0 || sun_height <= 0)))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_forward_device: bad argument");
+  CU(cudaSetDevice(ctx->device));
+  return forward_common(ctx, device_shading(sun_depth, sun_width, sun_height), block + kBlockShading, out_rgba, out_geom, out_aux,
+                        (cudaStream_t)stream);
 }
 
 int satsplat_shadow_map(satsplat_ctx* ctx, float* sun_depth_out, satsplat_stream stream) {
@@ -384,7 +443,7 @@ int satsplat_shadow_map(satsplat_ctx* ctx, float* sun_depth_out, satsplat_stream
   CU(cudaSetDevice(ctx->device));
   const DevShading sh = make_shading(nullptr);
   clear_stage_marks(ctx, {5, 6, 7});
-  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, nullptr, nullptr, nullptr, sun_depth_out, true, s)); }
+  { StageTimer t(ctx, SATSPLAT_STAGE_BLEND_FWD, s); CU(launch_blend_forward(ctx, sh, nullptr, nullptr, nullptr, nullptr, sun_depth_out, true, s)); }
   ctx->forwarded = 1;
   ctx->depth_only = 1;
   return SATSPLAT_OK;
@@ -397,25 +456,27 @@ int satsplat_render_backward(satsplat_ctx* ctx, const satsplat_shading* shading,
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_backward: ctx is NULL");
   if (!ctx->forwarded || ctx->depth_only)
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_backward: call satsplat_render_forward first");
-  if (shading && shading->shadows_on && !shading->sun_depth)
+  if (ctx->cam_dev) return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_backward: device camera in use, call satsplat_render_backward_device");
+  if (shading && shading->shadows_on && (!shading->sun_depth || shading->sun_width <= 0 || shading->sun_height <= 0))
     return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_backward: shadows_on without a sun depth map");
-  cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
-  const DevShading sh = make_shading(shading);
-  clear_stage_marks(ctx, {6, 7});
-  {
-    StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
-    CU(launch_blend_backward(ctx, sh, v_rgba, v_geom, v_aux, nullptr, false, v_cc, v_ambient, v_sun_depth, v_reproj, s));
-    if (v_cc) CU(launch_add_small(v_cc, ctx->red_buf, 12, s));
-    if (v_ambient) CU(launch_add_small(v_ambient, ctx->red_buf + 12, 3, s));
-    if (v_reproj) CU(launch_add_small(v_reproj, ctx->red_buf + 15, 8, s));
-  }
-  {
-    StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
-    CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
-                             v_opacity_logits, v_rgb, v_dF, s));
-  }
-  return SATSPLAT_OK;
+  return backward_common(ctx, make_shading(shading), nullptr, v_rgba, v_geom, v_aux, v_means, v_quats, v_scales, v_opacity_logits,
+                         v_rgb, v_dF, v_cc, v_ambient, v_sun_depth, v_reproj, (cudaStream_t)stream);
+}
+
+int satsplat_render_backward_device(satsplat_ctx* ctx, const float* block, const float* sun_depth, int32_t sun_width,
+                                    int32_t sun_height, const float* v_rgba, const float* v_geom, const float* v_aux,
+                                    float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
+                                    float* v_dF, float* v_cc, float* v_ambient, float* v_sun_depth, float* v_reproj,
+                                    satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_render_backward_device: ctx is NULL");
+  if (!ctx->forwarded || ctx->depth_only || !ctx->cam_dev)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_render_backward_device: call satsplat_render_forward_device first");
+  if (!block || (sun_depth && (sun_width <= 0 || sun_height <= 0)))
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_render_backward_device: bad argument");
+  CU(cudaSetDevice(ctx->device));
+  return backward_common(ctx, device_shading(sun_depth, sun_width, sun_height), block + kBlockShading, v_rgba, v_geom, v_aux, v_means,
+                         v_quats, v_scales, v_opacity_logits, v_rgb, v_dF, v_cc, v_ambient, v_sun_depth, v_reproj, (cudaStream_t)stream);
 }
 
 int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, float* v_means, float* v_quats,
@@ -430,13 +491,75 @@ int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, fl
   clear_stage_marks(ctx, {6, 7});
   {
     StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
-    CU(launch_blend_backward(ctx, sh, nullptr, nullptr, nullptr, v_sun_depth, true, nullptr, nullptr, nullptr, nullptr, s));
+    CU(launch_blend_backward(ctx, sh, nullptr, nullptr, nullptr, nullptr, v_sun_depth, true, nullptr, nullptr, nullptr, nullptr, s));
   }
   {
     StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
     CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
                              v_opacity_logits, nullptr, v_dF_sun, s));
   }
+  return SATSPLAT_OK;
+}
+
+int satsplat_view_params_fill(const satsplat_camera* cam, const satsplat_shading* shading, const satsplat_sun* sun,
+                              float nearby_d_azimuth, float nearby_d_elevation, satsplat_view_params* out) {
+  if (!cam || !out) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_view_params_fill: NULL argument");
+  memset(out, 0, sizeof(*out));
+  memcpy(out->F, cam->F, sizeof(out->F));
+  memcpy(out->view_dir, cam->view_dir, sizeof(out->view_dir));
+  out->b_z = cam->b_z;
+  out->z_bg = cam->z_bg;
+  memcpy(out->bg_rgb, cam->bg_rgb, sizeof(out->bg_rgb));
+  out->cc[0] = out->cc[5] = out->cc[10] = 1.f;
+  out->depth_bias = 0.5f;
+  out->slope = 4.f;
+  if (shading) {
+    memcpy(out->cc, shading->cc, sizeof(out->cc));
+    memcpy(out->ambient, shading->ambient, sizeof(out->ambient));
+    out->depth_bias = shading->depth_bias;
+    out->slope = shading->slope;
+  }
+  out->nearby_d_azimuth = nearby_d_azimuth;
+  out->nearby_d_elevation = nearby_d_elevation;
+  out->sun_viewport[0] = out->sun_viewport[1] = 1.f;
+  out->sun_s[0] = out->sun_s[1] = 0.0;
+  out->sun_view_dir[2] = -1.f;
+  if (sun) {
+    const double te = tan((double)sun->elevation);
+    if (!(fabs(te) > 1e-12)) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_view_params_fill: elevation must be non-zero");
+    out->sun_s[0] = cos((double)sun->azimuth) / te;   // Eq. S2, exactly as satsplat_sun_camera
+    out->sun_s[1] = sin((double)sun->azimuth) / te;
+    memcpy(out->sun_viewport, sun->viewport, sizeof(out->sun_viewport));
+    const double ce = cos((double)sun->elevation);
+    out->sun_view_dir[0] = (float)(-cos((double)sun->azimuth) * ce);
+    out->sun_view_dir[1] = (float)(-sin((double)sun->azimuth) * ce);
+    out->sun_view_dir[2] = (float)(-sin((double)sun->elevation));
+  }
+  return SATSPLAT_OK;
+}
+
+int satsplat_camera_chain(const satsplat_view_params* views, const float* dF, const int32_t* view_index, float* block,
+                          satsplat_stream stream) {
+  if (!views || !block) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_camera_chain: NULL argument");
+  const cudaError_t e = launch_camera_chain(views, dF, view_index, block, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_camera_chain: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
+int satsplat_camera_chain_backward(const satsplat_view_params* views, const float* dF, const int32_t* view_index,
+                                   const float* v_dF_view, const float* v_F_sun, const float* v_reproj, const float* v_F_nearby,
+                                   float* v_dF_all, satsplat_stream stream) {
+  if (!views || !v_dF_all) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_camera_chain_backward: NULL argument");
+  const cudaError_t e = launch_camera_chain_backward(views, dF, view_index, v_dF_view, v_F_sun, v_reproj, v_F_nearby, v_dF_all,
+                                                     (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_camera_chain_backward: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
+int satsplat_advance_view_index(int32_t* view_index, int32_t stride, int32_t n_views, satsplat_stream stream) {
+  if (!view_index || n_views <= 0) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_advance_view_index: bad argument");
+  const cudaError_t e = launch_advance_index(view_index, stride, n_views, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_advance_view_index: %s", cudaGetErrorString(e));
   return SATSPLAT_OK;
 }
 
@@ -515,8 +638,43 @@ int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out) {
   return SATSPLAT_OK;
 }
 
+namespace {
+// float offset of sub-array k of the packed surfel staging (means 3N, quats 4N, scales 2N, logits N, rgb 3N): every
+// sub-array starts on a 16-byte boundary whatever N is (the kernels use float4 / float2 accesses on them)
+inline size_t align4(size_t x) { return (x + 3) & ~(size_t)3; }
+struct Pack { size_t off[6]; };
+inline Pack pack_offsets(size_t n) {
+  static const int w[5] = {3, 4, 2, 1, 3};
+  Pack p;
+  p.off[0] = 0;
+  for (int k = 0; k < 5; ++k) p.off[k + 1] = p.off[k] + align4(n * (size_t)w[k]);
+  return p;
+}
+}  // namespace
+
+int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_reserve_host_staging: ctx is NULL");
+  CU(cudaSetDevice(ctx->device));
+  if (!ctx->e2e_in) {
+    const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
+    const Pack pk = pack_offsets((size_t)ctx->max_surfels);
+    CU(dalloc(ctx, &ctx->e2e_in, pk.off[5] + 4));
+    CU(dalloc(ctx, &ctx->e2e_up, mpx * 12));
+    CU(dalloc(ctx, &ctx->e2e_out, mpx * 12));
+    CU(dalloc(ctx, &ctx->e2e_grads, pk.off[5] + 64));
+    for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
+    for (int i = 0; i < 4; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[i], cudaEventDisableTiming));
+  }
+  if (sun_ctx && !sun_ctx->e2e_out) {
+    const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
+    const cudaError_t e = dalloc(sun_ctx, &sun_ctx->e2e_out, mpx * 2);   // sun map + its gradient
+    if (e != cudaSuccess) return fail(ctx, SATSPLAT_E_CUDA, "satsplat_reserve_host_staging: %s", cudaGetErrorString(e));
+  }
+  return SATSPLAT_OK;
+}
+
 int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
-                            const satsplat_camera* sun_cam, const satsplat_shading* shading, int64_t N,
+                            const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
                             const float* h_means, const float* h_quats, const float* h_scales,
                             const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
                             const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
@@ -524,38 +682,43 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_iteration_host: ctx is NULL");
   if (!cam || !shading || !h_means || !h_quats || !h_scales || !h_logits || !h_rgb || !h_grads || N <= 0)
     return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: NULL argument");
+  // every size is checked before the first copy is enqueued
   if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: N exceeds max_surfels");
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > ctx->max_w || cam->height > ctx->max_h)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: image size exceeds the context");
   const bool shadows = shading->shadows_on != 0;
-  if (shadows && (!sun_ctx || !sun_cam)) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: shadows need sun_ctx and sun_cam");
+  if (shadows) {
+    if (!sun_ctx || !sun) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: shadows need sun_ctx and sun");
+    if (N > sun_ctx->max_surfels || sun->width <= 0 || sun->height <= 0 || sun->width > sun_ctx->max_w || sun->height > sun_ctx->max_h)
+      return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: sun map size or N exceeds the sun context");
+  }
+  if (!ctx->e2e_in || (shadows && !sun_ctx->e2e_out))
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: call satsplat_reserve_host_staging first");
   cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
-  const size_t n = (size_t)N, px = (size_t)cam->width * cam->height;
-  const size_t spx = shadows ? (size_t)sun_cam->width * sun_cam->height : 0;
-  if (!ctx->e2e_in) {  // staging buffers: allocated on first use, sized for the context's maxima
-    const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
-    CU(dalloc(ctx, &ctx->e2e_in, (size_t)ctx->max_surfels * 13));
-    CU(dalloc(ctx, &ctx->e2e_up, mpx * 12));
-    CU(dalloc(ctx, &ctx->e2e_out, mpx * 12));
-    CU(dalloc(ctx, &ctx->e2e_grads, (size_t)ctx->max_surfels * 13 + 32));
-    for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
-    for (int i = 0; i < 4; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[i], cudaEventDisableTiming));
+  // the sun camera and the reprojection constants are derived from F' = F + dF (Eq. 16, cascade of Fig. 1)
+  satsplat_camera sun_cam;
+  satsplat_shading sh = *shading;
+  if (shadows) {
+    const int rc0 = satsplat_sun_camera(cam, sun->azimuth, sun->elevation, sun->width, sun->height, sun->viewport, &sun_cam, sh.reproj);
+    if (rc0) return fail(ctx, rc0, "satsplat_iteration_host: %s", satsplat_last_error(nullptr));
   }
+  const size_t n = (size_t)N, px = (size_t)cam->width * cam->height;
+  const size_t spx = shadows ? (size_t)sun->width * sun->height : 0;
   // Three queues: the caller's stream carries the surfel upload and every kernel; the upstream gradients (only
   // needed by the backward) go up on a second stream while the sun and view forward passes run, and the images come
   // down on a third while the backward runs (PCIe is full duplex).
   cudaStream_t s_up = ctx->e2e_stream[0], s_down = ctx->e2e_stream[1];
   cudaEvent_t ev_start = ctx->e2e_ev[0], ev_up = ctx->e2e_ev[1], ev_fwd = ctx->e2e_ev[2], ev_img = ctx->e2e_ev[3];
   CU(cudaEventRecord(ev_start, s));
-  float* d_means = ctx->e2e_in;
-  float* d_quats = d_means + 3 * (size_t)ctx->max_surfels;
-  float* d_scales = d_quats + 4 * (size_t)ctx->max_surfels;
-  float* d_logits = d_scales + 2 * (size_t)ctx->max_surfels;
-  float* d_rgb = d_logits + (size_t)ctx->max_surfels;
-  CU(cudaMemcpyAsync(d_means, h_means, n * 12, cudaMemcpyHostToDevice, s));
-  CU(cudaMemcpyAsync(d_quats, h_quats, n * 16, cudaMemcpyHostToDevice, s));
-  CU(cudaMemcpyAsync(d_scales, h_scales, n * 8, cudaMemcpyHostToDevice, s));
-  CU(cudaMemcpyAsync(d_logits, h_logits, n * 4, cudaMemcpyHostToDevice, s));
-  CU(cudaMemcpyAsync(d_rgb, h_rgb, n * 12, cudaMemcpyHostToDevice, s));
+  const Pack pk = pack_offsets(n);
+  float* d_in[5];
+  const float* h_in[5] = {h_means, h_quats, h_scales, h_logits, h_rgb};
+  static const int width[5] = {3, 4, 2, 1, 3};
+  for (int k = 0; k < 5; ++k) {
+    d_in[k] = ctx->e2e_in + pk.off[k];
+    CU(cudaMemcpyAsync(d_in[k], h_in[k], n * width[k] * sizeof(float), cudaMemcpyHostToDevice, s));
+  }
   float* d_up[3] = {nullptr, nullptr, nullptr};
   const float* h_up[3] = {h_v_rgba, h_v_geom, h_v_aux};
   CU(cudaStreamWaitEvent(s_up, ev_start, 0));
@@ -567,29 +730,26 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   CU(cudaEventRecord(ev_up, s_up));
   float* d_out[3];
   for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+  // device gradients: the five surfel groups at 16-byte aligned offsets, then dF(8) cc(12) ambient(3) reproj(8) dF_sun(8)
   float* g = ctx->e2e_grads;
-  CU(cudaMemsetAsync(g, 0, (n * 13 + 23) * sizeof(float), s));
-  float *g_means = g, *g_quats = g + 3 * n, *g_scales = g + 7 * n, *g_logits = g + 9 * n, *g_rgb = g + 10 * n;
-  float *g_dF = g + 13 * n, *g_cc = g_dF + 8, *g_amb = g_cc + 12;
-  satsplat_shading sh = *shading;
+  CU(cudaMemsetAsync(g, 0, (pk.off[5] + 40) * sizeof(float), s));
+  float* g_grp[5];
+  for (int k = 0; k < 5; ++k) g_grp[k] = g + pk.off[k];
+  float *g_dF = g + pk.off[5], *g_cc = g_dF + 8, *g_amb = g_cc + 12, *g_rep = g_dF + 24, *g_dFs = g_dF + 32;
   float* d_sun = nullptr;
   float* d_vsun = nullptr;
   int rc;
   if (shadows) {
-    if (!sun_ctx->e2e_out) {
-      const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
-      CU(dalloc(sun_ctx, &sun_ctx->e2e_out, mpx * 2));
-    }
     d_sun = sun_ctx->e2e_out;
     d_vsun = d_sun + (size_t)sun_ctx->max_w * sun_ctx->max_h;
-    if ((rc = satsplat_preprocess(sun_ctx, sun_cam, N, d_means, d_quats, d_scales, d_logits, d_rgb, stream))) return rc;
+    if ((rc = satsplat_preprocess(sun_ctx, &sun_cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
     if ((rc = satsplat_shadow_map(sun_ctx, d_sun, stream))) return rc;
     CU(cudaMemsetAsync(d_vsun, 0, spx * sizeof(float), s));
     sh.sun_depth = d_sun;
-    sh.sun_width = sun_cam->width;
-    sh.sun_height = sun_cam->height;
+    sh.sun_width = sun->width;
+    sh.sun_height = sun->height;
   }
-  if ((rc = satsplat_preprocess(ctx, cam, N, d_means, d_quats, d_scales, d_logits, d_rgb, stream))) return rc;
+  if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
   if ((rc = satsplat_render_forward(ctx, &sh, d_out[0], d_out[1], d_out[2], stream))) return rc;
   CU(cudaEventRecord(ev_fwd, s));
   float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};
@@ -598,14 +758,21 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
     if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s_down));
   CU(cudaEventRecord(ev_img, s_down));
   CU(cudaStreamWaitEvent(s, ev_up, 0));
-  if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_means, g_quats, g_scales, g_logits, g_rgb, g_dF,
-                                     g_cc, g_amb, d_vsun, nullptr, stream)))
+  if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_grp[0], g_grp[1], g_grp[2], g_grp[3], g_grp[4], g_dF,
+                                     g_cc, g_amb, d_vsun, shadows ? g_rep : nullptr, stream)))
     return rc;
   if (shadows) {
-    // the sun camera is derived from F' (cascade, Fig. 1); its 2x4 gradient is not chained here (NEXT-2)
-    if ((rc = satsplat_shadow_map_backward(sun_ctx, d_vsun, g_means, g_quats, g_scales, g_logits, nullptr, stream))) return rc;
+    if ((rc = satsplat_shadow_map_backward(sun_ctx, d_vsun, g_grp[0], g_grp[1], g_grp[2], g_grp[3], g_dFs, stream))) return rc;
+    // cascade: the gradients of the sun camera and of the reprojection constants flow back into dF (Eq. 16 adjoint)
+    if ((rc = satsplat_sun_camera_backward(cam, sun->azimuth, sun->elevation, sun->viewport, g_dFs, g_rep, g_dF, stream))) return rc;
   }
-  CU(cudaMemcpyAsync(h_grads, g, (n * 13 + 23) * sizeof(float), cudaMemcpyDeviceToHost, s));
+  // h_grads stays packed (means 3N, quats 4N, scales 2N, logits N, rgb 3N, dF 8, cc 12, ambient 3)
+  size_t ho = 0;
+  for (int k = 0; k < 5; ++k) {
+    CU(cudaMemcpyAsync(h_grads + ho, g_grp[k], n * width[k] * sizeof(float), cudaMemcpyDeviceToHost, s));
+    ho += n * width[k];
+  }
+  CU(cudaMemcpyAsync(h_grads + ho, g_dF, 23 * sizeof(float), cudaMemcpyDeviceToHost, s));
   CU(cudaStreamSynchronize(s));
   CU(cudaEventSynchronize(ev_img));
   return SATSPLAT_OK;

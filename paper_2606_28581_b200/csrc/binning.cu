@@ -355,7 +355,7 @@ cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
   cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
   ++g_kernel_launches;
-  ranges_kernel<<<148 * 8, 256, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[c->sorted], c->ranges);
+  ranges_kernel<<<c->sm_count * 8, 256, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[c->sorted], c->ranges);
   return cudaGetLastError();
 }
 
@@ -519,7 +519,7 @@ constexpr int kTileSortCtaMax = 16384;    // entries one CTA sorts in shared mem
 // Warp-wide bitonic sort of 32*E 64-bit values held in registers, blocked layout: element index of v[e] is
 // lane*E + e.  Strides >= E exchange through shuffles (run-time loop: the body is the same for every stride), strides
 // below E are register-to-register.  Only the loop over e is unrolled, so the code stays small (an earlier fully
-// unrolled version spent 40 % of its issue slots waiting on the instruction cache, profiles/r1_binning.md).
+// unrolled version spent 40 % of its issue slots waiting on the instruction cache).
 template <int E>
 __device__ __forceinline__ void warp_bitonic_regs(uint64_t (&v)[E], int lane) {
   for (int k = 2; k <= 32 * E; k <<= 1) {
@@ -645,6 +645,10 @@ __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* _
   }
 }
 
+cudaError_t init_binning_attrs() {
+  return cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
+}
+
 cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
   ++g_kernel_launches;
@@ -663,18 +667,13 @@ cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s) {
 
 cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
-  static bool attr_done[64] = {};   // per device: the dynamic shared-memory limit is a per-device function attribute
-  if (!attr_done[c->device & 63]) {
-    cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
-    attr_done[c->device & 63] = true;
-  }
   g_kernel_launches += 3;
   // the three kernels work on disjoint tiles (the worklists come from tile_scan_kernel): the few long lists, whose
   // one-tile latency sets the duration of their kernels, are sorted on a second stream beside the many short ones
   cudaEventRecord(c->bin_ev[0], s);
   cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
-  tile_sort_mid_kernel<<<148 * 4, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
-  tile_sort_large_kernel<<<74, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
+  tile_sort_mid_kernel<<<c->sm_count * 4, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_large_kernel<<<(c->sm_count + 1) / 2, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
                                                                             c->worklist + tiles, c->wl_count);
   cudaEventRecord(c->bin_ev[1], c->bin_stream);
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(

@@ -19,6 +19,8 @@ namespace satsplat {
 struct BwdParams {
   DevCamera cam;
   DevShading sh;
+  const float* cam_dev;   // device-resident camera / shading records (DEV instantiations only)
+  const float* sh_dev;
   const uint32_t* ranges;
   const uint32_t* vals;
   const float4* rec;
@@ -117,8 +119,10 @@ __device__ __forceinline__ float warp_reduce32_transposed(float (&v)[32], int la
   return v[0];
 }
 
-template <bool DEPTH_ONLY>
+template <bool DEPTH_ONLY, bool DEV>
 __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_kernel(const __grid_constant__ BwdParams P) {
+  const CamRef<DEV> cam{P.cam, P.cam_dev};
+  const ShRef<DEV> sh{P.sh, P.sh_dev};
   constexpr int kRecV = DEPTH_ONLY ? 3 : 4;
   __shared__ float4 s_wrec[kWarpsB][32][kRecV];   // per warp: records of the current group's survivors
   __shared__ int2 s_widx[kWarpsB][32];            //           and their (list index, surfel id)
@@ -150,7 +154,7 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
     if (DEPTH_ONLY) {
       // sun_depth = sum w (z - z_bg) + z_bg  (since sum w + T_f = 1): phi = v (z - z_bg), no T_f term
       vD = P.v_sun_in[o];
-      zref = P.cam.z_bg;
+      zref = cam.z_bg();
     }
   }
   if (!DEPTH_ONLY) {
@@ -165,15 +169,18 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       if (P.v_rgba) { const float4 t = P.v_rgba[o]; vI0 = t.x; vI1 = t.y; vI2 = t.z; vA = t.w; }
       if (P.v_geom) { const float4 t = P.v_geom[o]; vN0 = t.x; vN1 = t.y; vN2 = t.z; vD = t.w; }
       if (P.v_aux) { const float4 t = P.v_aux[o]; vmed = t.x; vL = t.y; }
-      const float* cc = P.sh.cc;
+      float cc[12];
+#pragma unroll
+      for (int k = 0; k < 12; ++k) cc[k] = sh.cc(k);
+      const float am0 = sh.ambient(0), am1 = sh.ambient(1), am2 = sh.ambient(2);
       const float V = b.w;
       const float ac0 = cc[0] * b.x + cc[1] * b.y + cc[2] * b.z + cc[3];
       const float ac1 = cc[4] * b.x + cc[5] * b.y + cc[6] * b.z + cc[7];
       const float ac2 = cc[8] * b.x + cc[9] * b.y + cc[10] * b.z + cc[11];
-      const float s0 = V + (1.f - V) * P.sh.ambient[0], s1 = V + (1.f - V) * P.sh.ambient[1], s2 = V + (1.f - V) * P.sh.ambient[2];
+      const float s0 = V + (1.f - V) * am0, s1 = V + (1.f - V) * am1, s2 = V + (1.f - V) * am2;
       const float vs0 = vI0 * ac0, vs1 = vI1 * ac1, vs2 = vI2 * ac2;     // d/d shade
       const float vc0 = vI0 * s0, vc1 = vI1 * s1, vc2 = vI2 * s2;        // d/d corrected albedo
-      const float vV = vs0 * (1.f - P.sh.ambient[0]) + vs1 * (1.f - P.sh.ambient[1]) + vs2 * (1.f - P.sh.ambient[2]);
+      const float vV = vs0 * (1.f - am0) + vs1 * (1.f - am1) + vs2 * (1.f - am2);
       red[0] = vc0 * b.x; red[1] = vc0 * b.y; red[2] = vc0 * b.z; red[3] = vc0;
       red[4] = vc1 * b.x; red[5] = vc1 * b.y; red[6] = vc1 * b.z; red[7] = vc1;
       red[8] = vc2 * b.x; red[9] = vc2 * b.y; red[10] = vc2 * b.z; red[11] = vc2;
@@ -183,7 +190,7 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       va2 = cc[2] * vc0 + cc[6] * vc1 + cc[10] * vc2;
       if (P.sh.shadows_on) {
         const float D = __fmaf_rn(zref, A, M1);
-        const ShadowTap t = shadow_tap(P.sh, P.cam, px, py, D, Tf);
+        const ShadowTap t = shadow_tap(sh, cam, P.sh.sun_w, P.sh.sun_h, px, py, D, Tf);
         if (t.in_map) {
           const int x0 = t.x0, y0 = t.y0, x1 = t.x1, y1 = t.y1;
           const float fx = t.fx, fy = t.fy, h = t.h;
@@ -191,7 +198,7 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
           const int SW = P.sh.sun_w;
           const float d00 = __ldg(Dm + y0 * SW + x0), d01 = __ldg(Dm + y0 * SW + x1);
           const float d10 = __ldg(Dm + y1 * SW + x0), d11 = __ldg(Dm + y1 * SW + x1);
-          const float v_gap = -P.sh.slope * V * (1.f - V) * vV;
+          const float v_gap = -sh.slope() * V * (1.f - V) * vV;
           float v_zv = v_gap;
           const float v_ds = -v_gap;
           if (P.v_sun_depth) {
@@ -203,14 +210,14 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
           const float dds_dx = (1.f - fy) * (d01 - d00) + fy * (d11 - d10);
           const float dds_dy = (1.f - fx) * (d10 - d00) + fx * (d11 - d01);
           const float v_xs = v_ds * dds_dx, v_ys = v_ds * dds_dy;
-          v_zv -= P.sh.reproj[2] * v_xs + P.sh.reproj[6] * v_ys;   // h = b_z - z_v
+          v_zv -= sh.reproj(2) * v_xs + sh.reproj(6) * v_ys;   // h = b_z - z_v
           red[15] = v_xs * px; red[16] = v_xs * py; red[17] = v_xs * h; red[18] = v_xs;
           red[19] = v_ys * px; red[20] = v_ys * py; red[21] = v_ys * h; red[22] = v_ys;
           vD += v_zv;                 // z_v = D + T_f z_bg
-          vT += P.cam.z_bg * v_zv;
+          vT += cam.z_bg() * v_zv;
         }
       }
-      vT += -vA + va0 * P.cam.bg[0] + va1 * P.cam.bg[1] + va2 * P.cam.bg[2];   // A = 1 - T_f ; albedo = C + T_f bg
+      vT += -vA + va0 * cam.bg(0) + va1 * cam.bg(1) + va2 * cam.bg(2);   // A = 1 - T_f ; albedo = C + T_f bg
       vT -= vD * zref;                                                          // D = M1' + z_ref (1 - T_f)
     }
     // ---- reduce the 23 epilogue gradients over the warp (transposed butterfly); one RED per value into one of kRedCopies
@@ -386,12 +393,25 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
   if (nseg) flush();
 }
 
-cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* v_rgba, const float* v_geom,
+constexpr int kPairBytesB = kWarpsB * kSegs * 32 * (int)(sizeof(float4) + sizeof(float2));
+
+// the dynamic shared-memory limit is a per-device function attribute: set for the current device by satsplat_create
+cudaError_t init_blend_backward_attrs() {
+  cudaError_t e = cudaFuncSetAttribute(blend_backward_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytesB);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(blend_backward_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytesB);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(blend_backward_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytesB);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(blend_backward_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytesB);
+  return e;
+}
+
+cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
                                   const float* v_aux, const float* v_sun_depth_in, bool depth_only, float* v_cc,
                                   float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s) {
   BwdParams P;
   P.cam = c->cam;
   P.sh = sh;
+  P.cam_dev = c->cam_dev;
+  P.sh_dev = sh_dev;
   P.ranges = c->ranges;
   P.vals = c->vals[c->sorted];
   P.rec = c->rec;
@@ -409,18 +429,16 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.red = want_red ? c->red_buf : nullptr;
   if (want_red) cudaMemsetAsync(c->red_buf, 0, kRedCopies * 32 * sizeof(float), s);
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));
-  constexpr int kPairBytes = kWarpsB * kSegs * 32 * (int)(sizeof(float4) + sizeof(float2));
-  static bool attr_done[64] = {};   // per device: the dynamic shared-memory limit is a per-device function attribute
-  if (!attr_done[c->device & 63]) {
-    cudaFuncSetAttribute(blend_backward_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
-    cudaFuncSetAttribute(blend_backward_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairBytes);
-    attr_done[c->device & 63] = true;
-  }
+  constexpr int kPairBytes = kPairBytesB;
   ++g_kernel_launches;
-  if (depth_only)
-    blend_backward_kernel<true><<<grid, kThreadsB, kPairBytes, s>>>(P);
-  else
-    blend_backward_kernel<false><<<grid, kThreadsB, kPairBytes, s>>>(P);
+  const bool dev = c->cam_dev != nullptr;
+  if (depth_only) {
+    if (dev) blend_backward_kernel<true, true><<<grid, kThreadsB, kPairBytes, s>>>(P);
+    else blend_backward_kernel<true, false><<<grid, kThreadsB, kPairBytes, s>>>(P);
+  } else {
+    if (dev) blend_backward_kernel<false, true><<<grid, kThreadsB, kPairBytes, s>>>(P);
+    else blend_backward_kernel<false, false><<<grid, kThreadsB, kPairBytes, s>>>(P);
+  }
   return cudaGetLastError();
 }
 

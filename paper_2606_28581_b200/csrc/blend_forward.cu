@@ -16,6 +16,8 @@ namespace satsplat {
 struct FwdParams {
   DevCamera cam;
   DevShading sh;
+  const float* cam_dev;   // device-resident camera / shading records (DEV instantiations only)
+  const float* sh_dev;
   const uint32_t* ranges;
   const uint32_t* vals;
   const float4* rec;
@@ -63,8 +65,10 @@ __device__ __forceinline__ uint32_t block_cover_mask(const float4 bb, float wx0,
   return cols * ((rows * 0x00204081u) & 0x01010101u);
 }
 
-template <bool DEPTH_ONLY>
+template <bool DEPTH_ONLY, bool DEV>
 __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_kernel(const __grid_constant__ FwdParams P) {
+  const CamRef<DEV> cam{P.cam, P.cam_dev};
+  const ShRef<DEV> sh{P.sh, P.sh_dev};
   // per warp, double buffered: the records of a group's survivors as four float4 planes (lanes of a warp read
   // different entries at the same time)
   __shared__ float4 s_r0[2][kWarpsF][32], s_r1[2][kWarpsF][32], s_r2[2][kWarpsF][32], s_r3[2][DEPTH_ONLY ? 1 : kWarpsF][32];
@@ -81,7 +85,7 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
   const float wx0 = (float)bx0 + 0.5f, wy0 = (float)by0 + 0.5f;   // first pixel centre of this warp's 8x4 block
 
   float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f;
-  float M1 = 0.f, M2 = 0.f, L = 0.f, zref = 0.f, med = P.cam.z_bg;
+  float M1 = 0.f, M2 = 0.f, L = 0.f, zref = 0.f, med = cam.z_bg();
   int mi = -1, last = 0, visited = 0, ncontrib = 0;
   bool done = !inside;
 
@@ -169,15 +173,15 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
   const size_t o = (size_t)iy * P.cam.W + ix;
   const float A = 1.0f - T;
   if (DEPTH_ONLY) {
-    P.sun_depth_out[o] = M1 + T * P.cam.z_bg;
+    P.sun_depth_out[o] = M1 + T * cam.z_bg();
     P.px_a[o] = make_float4(T, 0.f, 0.f, 0.f);
     P.px_i[o] = make_int2(last, -1);
   } else {
     const float D = __fmaf_rn(zref, A, M1);
-    const float al0 = C0 + T * P.cam.bg[0], al1 = C1 + T * P.cam.bg[1], al2 = C2 + T * P.cam.bg[2];
+    const float al0 = C0 + T * cam.bg(0), al1 = C1 + T * cam.bg(1), al2 = C2 + T * cam.bg(2);
     float V = 1.0f;
     if (P.sh.shadows_on) {
-      const ShadowTap t = shadow_tap(P.sh, P.cam, px, py, D, T);
+      const ShadowTap t = shadow_tap(sh, cam, P.sh.sun_w, P.sh.sun_h, px, py, D, T);
       if (t.in_map) {
         const float* Dm = P.sh.sun_depth;
         const int SW = P.sh.sun_w;
@@ -185,14 +189,13 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
         const float d10 = __ldg(Dm + t.y1 * SW + t.x0), d11 = __ldg(Dm + t.y1 * SW + t.x1);
         const float ds = (1.f - t.fy) * ((1.f - t.fx) * d00 + t.fx * d01) + t.fy * ((1.f - t.fx) * d10 + t.fx * d11);
         const float gap = t.zv - ds;
-        V = 1.0f / (1.0f + __expf(P.sh.slope * (gap - P.sh.bias)));
+        V = 1.0f / (1.0f + __expf(sh.slope() * (gap - sh.bias())));
       }
     }
-    const float* cc = P.sh.cc;
-    const float ac0 = cc[0] * al0 + cc[1] * al1 + cc[2] * al2 + cc[3];
-    const float ac1 = cc[4] * al0 + cc[5] * al1 + cc[6] * al2 + cc[7];
-    const float ac2 = cc[8] * al0 + cc[9] * al1 + cc[10] * al2 + cc[11];
-    const float s0 = V + (1.f - V) * P.sh.ambient[0], s1 = V + (1.f - V) * P.sh.ambient[1], s2 = V + (1.f - V) * P.sh.ambient[2];
+    const float ac0 = sh.cc(0) * al0 + sh.cc(1) * al1 + sh.cc(2) * al2 + sh.cc(3);
+    const float ac1 = sh.cc(4) * al0 + sh.cc(5) * al1 + sh.cc(6) * al2 + sh.cc(7);
+    const float ac2 = sh.cc(8) * al0 + sh.cc(9) * al1 + sh.cc(10) * al2 + sh.cc(11);
+    const float s0 = V + (1.f - V) * sh.ambient(0), s1 = V + (1.f - V) * sh.ambient(1), s2 = V + (1.f - V) * sh.ambient(2);
     if (P.out_rgba) P.out_rgba[o] = make_float4(ac0 * s0, ac1 * s1, ac2 * s2, A);   // Eq. 1
     if (P.out_geom) P.out_geom[o] = make_float4(N0, N1, N2, D);
     if (P.out_aux) P.out_aux[o] = make_float4(med, L, V, T);
@@ -204,11 +207,13 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
   P.px_contrib[o] = ncontrib;
 }
 
-cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* out_rgba, float* out_geom, float* out_aux,
-                                 float* sun_depth_out, bool depth_only, cudaStream_t s) {
+cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, float* out_rgba, float* out_geom,
+                                 float* out_aux, float* sun_depth_out, bool depth_only, cudaStream_t s) {
   FwdParams P;
   P.cam = c->cam;
   P.sh = sh;
+  P.cam_dev = c->cam_dev;
+  P.sh_dev = sh_dev;
   P.ranges = c->ranges;
   P.vals = c->vals[c->sorted];
   P.rec = c->rec;
@@ -224,10 +229,14 @@ cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* o
   P.px_contrib = c->px_contrib;
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsF));
   ++g_kernel_launches;
-  if (depth_only)
-    blend_forward_kernel<true><<<grid, kThreadsF, 0, s>>>(P);
-  else
-    blend_forward_kernel<false><<<grid, kThreadsF, 0, s>>>(P);
+  const bool dev = c->cam_dev != nullptr;   // the view's shading record travels with a device camera (sh_dev is NULL for depth-only passes)
+  if (depth_only) {
+    if (dev) blend_forward_kernel<true, true><<<grid, kThreadsF, 0, s>>>(P);
+    else blend_forward_kernel<true, false><<<grid, kThreadsF, 0, s>>>(P);
+  } else {
+    if (dev) blend_forward_kernel<false, true><<<grid, kThreadsF, 0, s>>>(P);
+    else blend_forward_kernel<false, false><<<grid, kThreadsF, 0, s>>>(P);
+  }
   return cudaGetLastError();
 }
 

@@ -14,7 +14,8 @@ __device__ __forceinline__ float warp_sum_f(float v) {
   return v;
 }
 
-__global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int N, const float* __restrict__ means,
+template <bool DEV>
+__global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera camv, const float* __restrict__ cam_dev, int N, const float* __restrict__ means,
                                                              const float* __restrict__ quats, const float* __restrict__ scales,
                                                              const float* __restrict__ logits, const uint32_t* __restrict__ count,
                                                              const uint8_t* __restrict__ flags, float4* __restrict__ vrec,
@@ -84,8 +85,9 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera cam, int 
   if (cnt > 0) {
     const float4 m0 = s_v[5 * t], m1 = s_v[5 * t + 1], m2 = s_v[5 * t + 2], m3 = s_v[5 * t + 3], m4 = s_v[5 * t + 4];
     const float p0 = s_p[3 * t], p1 = s_p[3 * t + 1], p2 = s_p[3 * t + 2];
-    const float B00 = cam.Fp[0], B01 = cam.Fp[1], B02 = cam.Fp[2];
-    const float B10 = cam.Fp[4], B11 = cam.Fp[5], B12 = cam.Fp[6];
+    const CamRef<DEV> camr{camv, cam_dev};
+    const float B00 = camr.Fp(0), B01 = camr.Fp(1), B02 = camr.Fp(2);
+    const float B10 = camr.Fp(4), B11 = camr.Fp(5), B12 = camr.Fp(6);
     const float qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
     const float inv = 1.0f / qn;
     const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
@@ -197,9 +199,13 @@ cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const flo
                                   float* v_rgb, float* v_dF, cudaStream_t s) {
   if (c->N == 0) return cudaSuccess;
   ++g_kernel_launches;
-  chain_backward_kernel<<<(int)((c->N + 255) / 256), 256, 0, s>>>(c->cam, (int)c->N, means, quats, scales, logits, c->count,
-                                                                  c->flags, reinterpret_cast<float4*>(c->vrec), v_means,
-                                                                  v_quats, v_scales, v_logits, v_rgb, v_dF);
+  const int grid = (int)((c->N + 255) / 256);
+  if (c->cam_dev)
+    chain_backward_kernel<true><<<grid, 256, 0, s>>>(c->cam, c->cam_dev, (int)c->N, means, quats, scales, logits, c->count, c->flags,
+                                                     reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF);
+  else
+    chain_backward_kernel<false><<<grid, 256, 0, s>>>(c->cam, nullptr, (int)c->N, means, quats, scales, logits, c->count, c->flags,
+                                                      reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF);
   return cudaGetLastError();
 }
 

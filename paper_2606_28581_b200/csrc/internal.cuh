@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/satsplat.h"
 
 namespace satsplat {
@@ -64,6 +66,35 @@ struct DevShading {
   float bias, slope;
 };
 
+// ---- device-resident camera block (row f2: satsplat_camera_chain writes it, the *_device calls read it) ---------------
+// floats [0,16) view camera, [16,32) sun camera, [32,48) nearby camera, each (Fp[8], view_dir[3], b_z, z_bg, bg[3]);
+// [48,76) shading of the view: cc[12], ambient[3], reproj[8], depth_bias, slope, 3 unused;  SATSPLAT_CAMERA_BLOCK_FLOATS = 80
+constexpr int kCamFloats = 16;
+constexpr int kBlockShading = 48;
+
+// Camera / shading values of a kernel: kernel-argument copies (DEV = false: the host-struct calls) or loads from the
+// device-resident block (DEV = true).  W, H, TX, TY, the sun map pointer and its size are host-known in both modes.
+template <bool DEV>
+struct CamRef {
+  const DevCamera& c;
+  const float* d;   // 16-float camera record of the block (DEV only)
+  __device__ __forceinline__ float Fp(int k) const { return DEV ? __ldg(d + k) : c.Fp[k]; }
+  __device__ __forceinline__ float vd(int k) const { return DEV ? __ldg(d + 8 + k) : c.vd[k]; }
+  __device__ __forceinline__ float b_z() const { return DEV ? __ldg(d + 11) : c.b_z; }
+  __device__ __forceinline__ float z_bg() const { return DEV ? __ldg(d + 12) : c.z_bg; }
+  __device__ __forceinline__ float bg(int k) const { return DEV ? __ldg(d + 13 + k) : c.bg[k]; }
+};
+template <bool DEV>
+struct ShRef {
+  const DevShading& s;
+  const float* d;   // 28-float shading record of the block (DEV only)
+  __device__ __forceinline__ float cc(int k) const { return DEV ? __ldg(d + k) : s.cc[k]; }
+  __device__ __forceinline__ float ambient(int k) const { return DEV ? __ldg(d + 12 + k) : s.ambient[k]; }
+  __device__ __forceinline__ float reproj(int k) const { return DEV ? __ldg(d + 15 + k) : s.reproj[k]; }
+  __device__ __forceinline__ float bias() const { return DEV ? __ldg(d + 23) : s.bias; }
+  __device__ __forceinline__ float slope() const { return DEV ? __ldg(d + 24) : s.slope; }
+};
+
 // ---- record layout in HBM: 4 x float4 = 64 B per surfel, 64-B aligned --------------------------------------
 //   r0 = (c_x, c_y, Q00, Q01)   r1 = (Q10, Q11, alpha, z_c)   r2 = (g0, g1, red, green)   r3 = (blue, n_x, n_y, n_z)
 // The first two float4 are all the per-pair test needs; the last two are only read by contributing pairs.
@@ -75,7 +106,7 @@ constexpr int kRedCopies = 64;   // copies of the 23 epilogue-gradient sums (cc,
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 8;
 constexpr int kSortTile = kSortThreads * kSortItems;  // 2048 keys
-constexpr int kSortBlocks = 148 * 2;                  // fixed grid: K lives on the device
+constexpr int kSortBlocks = 296;                      // fixed grid of the radix passes (K lives on the device; sizes the digit table)
 
 struct Status {           // device-resident status words
   unsigned int K;         // duplicated keys of the last preprocess (may exceed capacity)
@@ -107,22 +138,23 @@ struct ShadowTap {
   int x0, y0, x1, y1;
   float fx, fy, h, zv;
 };
-__device__ __forceinline__ ShadowTap shadow_tap(const DevShading& sh, const DevCamera& cam, float px, float py, float D, float T) {
+template <class SH, class CAM>
+__device__ __forceinline__ ShadowTap shadow_tap(const SH& sh, const CAM& cam, int sun_w, int sun_h, float px, float py, float D, float T) {
   ShadowTap t;
-  t.zv = __fmaf_rn(T, cam.z_bg, D);          // z_v = D + T_f z_bg
-  t.h = __fsub_rn(cam.b_z, t.zv);            // world height seen at this pixel
+  t.zv = __fmaf_rn(T, cam.z_bg(), D);        // z_v = D + T_f z_bg
+  t.h = __fsub_rn(cam.b_z(), t.zv);          // world height seen at this pixel
   const double dpx = (double)px, dpy = (double)py, dh = (double)t.h;
-  const double xs = fma((double)sh.reproj[2], dh, fma((double)sh.reproj[1], dpy, fma((double)sh.reproj[0], dpx, (double)sh.reproj[3])));
-  const double ys = fma((double)sh.reproj[6], dh, fma((double)sh.reproj[5], dpy, fma((double)sh.reproj[4], dpx, (double)sh.reproj[7])));
-  t.in_map = xs >= 0.5 && xs <= (double)sh.sun_w - 0.5 && ys >= 0.5 && ys <= (double)sh.sun_h - 0.5;
+  const double xs = fma((double)sh.reproj(2), dh, fma((double)sh.reproj(1), dpy, fma((double)sh.reproj(0), dpx, (double)sh.reproj(3))));
+  const double ys = fma((double)sh.reproj(6), dh, fma((double)sh.reproj(5), dpy, fma((double)sh.reproj(4), dpx, (double)sh.reproj(7))));
+  t.in_map = xs >= 0.5 && xs <= (double)sun_w - 0.5 && ys >= 0.5 && ys <= (double)sun_h - 0.5;
   const double tx = xs - 0.5, ty = ys - 0.5;
   // clamp in double before the conversion (far outside the map the product would overflow an int)
-  t.x0 = (int)fmin(fmax(floor(tx), 0.0), (double)(sh.sun_w - 1));
-  t.y0 = (int)fmin(fmax(floor(ty), 0.0), (double)(sh.sun_h - 1));
+  t.x0 = (int)fmin(fmax(floor(tx), 0.0), (double)(sun_w - 1));
+  t.y0 = (int)fmin(fmax(floor(ty), 0.0), (double)(sun_h - 1));
   t.fx = (float)(tx - (double)t.x0);
   t.fy = (float)(ty - (double)t.y0);
-  t.x1 = min(t.x0 + 1, sh.sun_w - 1);
-  t.y1 = min(t.y0 + 1, sh.sun_h - 1);
+  t.x1 = min(t.x0 + 1, sun_w - 1);
+  t.y1 = min(t.y0 + 1, sun_h - 1);
   return t;
 }
 
@@ -154,6 +186,7 @@ __device__ __forceinline__ float pair_depth(const PairEval& E, float zc, float g
 
 struct satsplat_ctx {
   int device;
+  int sm_count;           // multiprocessors of `device` (grid sizing of the fixed-grid kernels)
   int64_t max_surfels, max_dup;
   int32_t max_w, max_h;
   int64_t scratch_bytes;
@@ -191,6 +224,7 @@ struct satsplat_ctx {
   float* red_buf;         // small reduction scratch (dF, cc, ambient, reproj)
   // host state
   satsplat::DevCamera cam;
+  const float* cam_dev;   // device-resident camera record (16 floats of a camera block) of the last satsplat_preprocess_device, else NULL
   int64_t N;
   const float *in_means, *in_quats, *in_scales, *in_logits;  // caller buffers of the last preprocess (chain backward)
   int preprocessed, forwarded, depth_only;
@@ -210,7 +244,14 @@ struct satsplat_ctx {
 
 namespace satsplat {
 
-extern long long g_kernel_launches;  // cumulative kernel launches of this process (bench.py's gpu_launches)
+extern std::atomic<long long> g_kernel_launches;  // cumulative kernel launches of this process (bench.py's gpu_launches)
+
+// multiprocessors of the current device (for the kernels launched without a context)
+inline int current_sm_count() {
+  int dev = 0, n = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  return n;
+}
 
 // launchers (each enqueues on `s`, returns the cudaError_t of the launch)
 cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, const float* quats, const float* scales,
@@ -222,9 +263,10 @@ cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s);
 cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s);
 cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s);
 cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s);
-cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, float* out_rgba, float* out_geom, float* out_aux,
-                                 float* sun_depth_out, bool depth_only, cudaStream_t s);
-cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* v_rgba, const float* v_geom,
+// sh_dev: 28-float shading record of a device camera block (NULL: the values of `sh`); the camera comes from c->cam_dev / c->cam
+cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, float* out_rgba, float* out_geom,
+                                 float* out_aux, float* sun_depth_out, bool depth_only, cudaStream_t s);
+cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
                                   const float* v_aux, const float* v_sun_depth_in, bool depth_only, float* v_cc,
                                   float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s);
 cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
@@ -252,6 +294,15 @@ cudaError_t launch_adam(int64_t N, float* const params[5], const float* const gr
                         float beta1, float beta2, float eps, int step, cudaStream_t s);
 cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1, const float* v_F_sun, const float* v_reproj,
                                        float* v_dF, cudaStream_t s);
+cudaError_t launch_camera_chain(const satsplat_view_params* views, const float* dF_all, const int32_t* view_index, float* block,
+                                cudaStream_t s);
+cudaError_t launch_camera_chain_backward(const satsplat_view_params* views, const float* dF_all, const int32_t* view_index,
+                                         const float* v_dF_view, const float* v_F_sun, const float* v_reproj, const float* v_F_nearby,
+                                         float* v_dF_all, cudaStream_t s);
+cudaError_t launch_advance_index(int32_t* view_index, int32_t stride, int32_t n_views, cudaStream_t s);
+// per-device function attributes (dynamic shared-memory limits) of the kernels that need them; called by satsplat_create
+cudaError_t init_blend_backward_attrs();
+cudaError_t init_binning_attrs();
 cudaError_t launch_export_records(satsplat_ctx* c, float* records_out, uint8_t* flags_out, cudaStream_t s);
 
 }  // namespace satsplat

@@ -18,7 +18,8 @@ __device__ __forceinline__ int tile_of(float v, int T) {
   return (int)t;
 }
 
-__global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, const float* __restrict__ means,
+template <bool DEV>
+__global__ void __launch_bounds__(256) preprocess_kernel(DevCamera camv, const float* __restrict__ cam_dev, int N, const float* __restrict__ means,
                                                          const float* __restrict__ quats, const float* __restrict__ scales,
                                                          const float* __restrict__ logits, const float* __restrict__ rgb,
                                                          float4* __restrict__ rec, float4* __restrict__ bbox, ushort4* __restrict__ rect,
@@ -26,6 +27,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
                                                          uint8_t* __restrict__ flags, uint32_t* __restrict__ tile_count) {
   // records leave through shared memory so that the CTA's 256 x 64 B go out as one contiguous float4 stream
   __shared__ float4 s_rec[256 * 4];
+  const CamRef<DEV> camr{camv, cam_dev};
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   int cnt = 0, tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
   if (i < N) {
@@ -34,8 +36,8 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   const float4 q = reinterpret_cast<const float4*>(quats)[i];
   const float2 sc = reinterpret_cast<const float2*>(scales)[i];
   const float logit = logits[i];
-  const float B00 = cam.Fp[0], B01 = cam.Fp[1], B02 = cam.Fp[2], b0 = cam.Fp[3];
-  const float B10 = cam.Fp[4], B11 = cam.Fp[5], B12 = cam.Fp[6], b1 = cam.Fp[7];
+  const float B00 = camr.Fp(0), B01 = camr.Fp(1), B02 = camr.Fp(2), b0 = camr.Fp(3);
+  const float B10 = camr.Fp(4), B11 = camr.Fp(5), B12 = camr.Fp(6), b1 = camr.Fp(7);
   uint8_t fl = 0;
   // 1. normalise the quaternion (w,x,y,z)
   const float n2 = __fmaf_rn(q.w, q.w, __fmaf_rn(q.z, q.z, __fmaf_rn(q.y, q.y, __fmul_rn(q.x, q.x))));
@@ -55,7 +57,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   const float cx = __fmaf_rn(B02, pz, __fmaf_rn(B01, py, __fmaf_rn(B00, px, b0)));
   const float cy = __fmaf_rn(B12, pz, __fmaf_rn(B11, py, __fmaf_rn(B10, px, b1)));
   // 5. height depth (Eq. 11) and order-preserving key
-  const float zc = __fsub_rn(cam.b_z, pz);
+  const float zc = __fsub_rn(camr.b_z(), pz);
   uint32_t k = __float_as_uint(zc);
   k = (k & 0x80000000u) ? ~k : (k | 0x80000000u);
   // 6. extent
@@ -67,10 +69,10 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
                     !isfinite(cx) || !isfinite(cy) || !isfinite(extx) || !isfinite(exty) || !isfinite(zc);
   if (!cull) {
     // 7. tile rect
-    tx0 = min(max(tile_of(__fsub_rn(cx, extx), cam.TX), 0), cam.TX);
-    tx1 = min(max(tile_of(__fadd_rn(cx, extx), cam.TX) + 1, 0), cam.TX);
-    ty0 = min(max(tile_of(__fsub_rn(cy, exty), cam.TY), 0), cam.TY);
-    ty1 = min(max(tile_of(__fadd_rn(cy, exty), cam.TY) + 1, 0), cam.TY);
+    tx0 = min(max(tile_of(__fsub_rn(cx, extx), camv.TX), 0), camv.TX);
+    tx1 = min(max(tile_of(__fadd_rn(cx, extx), camv.TX) + 1, 0), camv.TX);
+    ty0 = min(max(tile_of(__fsub_rn(cy, exty), camv.TY), 0), camv.TY);
+    ty1 = min(max(tile_of(__fadd_rn(cy, exty), camv.TY) + 1, 0), camv.TY);
   } else {
     fl |= F_CULLED;
   }
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
     g0 = -__fmaf_rn(r1, Q10, __fmul_rn(r0, Q00));
     g1 = -__fmaf_rn(r1, Q11, __fmul_rn(r0, Q01));
   }
-  const float dotv = __fmaf_rn(nz, cam.vd[2], __fmaf_rn(n1, cam.vd[1], __fmul_rn(n0, cam.vd[0])));
+  const float dotv = __fmaf_rn(nz, camr.vd(2), __fmaf_rn(n1, camr.vd(1), __fmul_rn(n0, camr.vd(0))));
   if (dotv > 0.0f) { n0 = -n0; n1 = -n1; nz = -nz; fl |= F_FLIPPED; }
   const float alpha = 1.0f / (1.0f + expf(-logit));
   flags[i] = fl;
@@ -116,7 +118,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
   if (tile_count == nullptr) return;
   if (cnt > 0 && cnt <= 16) {
     for (int ty = ty0; ty < ty1; ++ty)
-      for (int tx = tx0; tx < tx1; ++tx) atomicAdd(tile_count + ty * cam.TX + tx, 1u);
+      for (int tx = tx0; tx < tx1; ++tx) atomicAdd(tile_count + ty * camv.TX + tx, 1u);
   }
   unsigned big = __ballot_sync(0xffffffffu, cnt > 16);
   const int lane = threadIdx.x & 31;
@@ -126,7 +128,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera cam, int N, c
     const int c2 = __shfl_sync(0xffffffffu, cnt, src);
     const int x0 = __shfl_sync(0xffffffffu, tx0, src), y0 = __shfl_sync(0xffffffffu, ty0, src);
     const int w = __shfl_sync(0xffffffffu, tx1, src) - x0;
-    for (int q = lane; q < c2; q += 32) atomicAdd(tile_count + (y0 + q / w) * cam.TX + x0 + q % w, 1u);
+    for (int q = lane; q < c2; q += 32) atomicAdd(tile_count + (y0 + q / w) * camv.TX + x0 + q % w, 1u);
   }
 }
 
@@ -136,9 +138,13 @@ cudaError_t launch_preprocess(satsplat_ctx* c, int64_t N, const float* means, co
   const int threads = 256;
   const int blocks = (int)((N + threads - 1) / threads);
   ++g_kernel_launches;
-  preprocess_kernel<<<blocks, threads, 0, s>>>(c->cam, (int)N, means, quats, scales, logits, rgb, c->rec, c->bbox,
-                                               reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags,
-                                               c->binning_mode == SATSPLAT_BINNING_TILESORT ? c->tile_count : nullptr);
+  uint32_t* tc = c->binning_mode == SATSPLAT_BINNING_TILESORT ? c->tile_count : nullptr;
+  if (c->cam_dev)
+    preprocess_kernel<true><<<blocks, threads, 0, s>>>(c->cam, c->cam_dev, (int)N, means, quats, scales, logits, rgb, c->rec, c->bbox,
+                                                       reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags, tc);
+  else
+    preprocess_kernel<false><<<blocks, threads, 0, s>>>(c->cam, nullptr, (int)N, means, quats, scales, logits, rgb, c->rec, c->bbox,
+                                                        reinterpret_cast<ushort4*>(c->rect), c->count, c->depth_key, c->flags, tc);
   return cudaGetLastError();
 }
 

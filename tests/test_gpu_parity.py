@@ -368,25 +368,38 @@ def test_oversized_splats_cooperative_duplication(P, G, orc):
     G.compare_images(res, f, G.fragile_mask(f["margins"]))
 
 
-def test_iteration_host_matches_device_path(P, G, orc):
-    """The end-to-end HOST-buffer entry point gives the same result as the staged device calls."""
+@pytest.mark.parametrize("n", [8000, 1023])
+def test_iteration_host_matches_device_path(P, G, orc, n):
+    """The end-to-end HOST-buffer entry point does exactly the work of the staged device calls (both passes, both
+    backwards, the cascade chain of the sun camera into dF), for an N that is not a multiple of 4 too (the device staging
+    is padded to 16-byte boundaries; the host arrays stay packed).  A consistency test of two entry points of the CUDA
+    path, not parity evidence."""
     import torch
-    scene = S.make_config(2, n=8000, size=128, n_views=1, extent=40.0, sun_size=192)
+    scene = S.make_config(2, n=n, size=128, n_views=1, extent=40.0, sun_size=192)
     view = scene.views[0]
     gs = G.GpuScene(scene)
     cam = P.Camera.from_view(view)
+    sun = P.Sun.from_view(view)
     sun_cam, rep = P.sun_camera(cam, view.sun_azimuth, view.sun_elevation, view.sun_width, view.sun_height, view.sun_viewport)
     up = S.upstream_grads(scene.seed, 0, view.height, view.width)
-    n = scene.n
     ctx = P.Context(n, view.width, view.height, 16 * n)
     sctx = P.Context(n, view.sun_width, view.sun_height, 16 * n)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
     h_out = [torch.empty(view.height, view.width, 4).pin_memory() for _ in range(3)]
     h_g = torch.empty(n * 13 + 23).pin_memory()
-    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, reproj=rep, depth_bias=view.depth_bias, slope=view.slope)
+    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, depth_bias=view.depth_bias, slope=view.slope)
     sh.shadows_on = 1
-    P.iteration_host(ctx, sctx, cam, sun_cam, sh, n, pin(scene.means), pin(scene.quats), pin(scene.scales), pin(scene.opacity_logits),
-                     pin(scene.rgb), pin(up[0]), pin(up[1]), pin(up[2]), h_out[0], h_out[1], h_out[2], h_g)
+    args = (ctx, sctx, cam, sun, sh, n, pin(scene.means), pin(scene.quats), pin(scene.scales), pin(scene.opacity_logits),
+            pin(scene.rgb), pin(up[0]), pin(up[1]), pin(up[2]), h_out[0], h_out[1], h_out[2], h_g)
+    with pytest.raises(P.SatsplatError) as e:          # staging is explicit, never lazy
+        P.iteration_host(*args)
+    assert e.value.code == P.E_STATE
+    P.reserve_host_staging(ctx, sctx)
+    big = P.Camera.from_view(view); big.width = view.width + 16
+    with pytest.raises(P.SatsplatError) as e:          # rejected before any copy is enqueued
+        P.iteration_host(ctx, sctx, big, *args[3:])
+    assert e.value.code == P.E_INVALID
+    P.iteration_host(*args)
     # staged device path
     class SV: pass
     sv = SV(); sv.width, sv.height = view.sun_width, view.sun_height
@@ -396,9 +409,20 @@ def test_iteration_host_matches_device_path(P, G, orc):
     np.testing.assert_allclose(h_out[0].numpy(), res["rgba"], rtol=0, atol=0)
     np.testing.assert_allclose(h_out[1].numpy(), res["geom"], rtol=0, atol=0)
     g = h_g.numpy()
-    tot = res["grads"]["v_means"] + res["sun_grads"]["v_means"]
-    np.testing.assert_allclose(g[:3 * n].reshape(n, 3), tot, rtol=1e-3, atol=1e-4)   # atomics: order differs run to run
-    np.testing.assert_allclose(g[13 * n:13 * n + 8], res["grads"]["v_dF"], rtol=2e-3, atol=1e-2)
+    off = 0
+    for k, wdt in (("v_means", 3), ("v_quats", 4), ("v_scales", 2), ("v_logits", 1), ("v_rgb", 3)):
+        tot = res["grads"][k] + (res["sun_grads"][k] if k != "v_rgb" else 0)
+        got = g[off:off + wdt * n].reshape(tot.shape)
+        np.testing.assert_allclose(got, tot, rtol=1e-3, atol=1e-4 * max(1.0, np.abs(tot).max()))   # atomics: order differs run to run
+        off += wdt * n
+    # dF with the cascade chained in, exactly as the staged calls + satsplat_sun_camera_backward give it
+    tot_dF = G.t(res["grads"]["v_dF"])
+    P.sun_camera_backward(cam, view.sun_azimuth, view.sun_elevation, view.sun_viewport, G.t(res["sun_grads"]["v_dF_sun"]),
+                          G.t(res["grads"]["v_reproj"]), tot_dF)
+    torch.cuda.synchronize()
+    ref_dF = tot_dF.cpu().numpy()
+    np.testing.assert_allclose(g[off:off + 8], ref_dF, rtol=2e-3, atol=2e-3 * np.abs(ref_dF).max())
+    np.testing.assert_allclose(g[off + 8:off + 20], res["grads"]["v_cc"], rtol=2e-3, atol=2e-3 * np.abs(res["grads"]["v_cc"]).max())
     ctx.close(); sctx.close()
 
 
@@ -704,3 +728,183 @@ def test_relocate_matches_oracle(P, G, n, frac_dead):
         np.testing.assert_array_equal(gv[k], ref["adam_v"][k])
     if frac_dead == 0.98:
         assert ref["ratio"].max() > 51
+
+
+# ------------------------------------------------------------------------------------------------------------
+# (f2) device-resident cameras: the cascade camera chain
+# ------------------------------------------------------------------------------------------------------------
+def _chain_setup(P, G, scene, nearby):
+    import torch
+    table = P.view_params_table(scene.views, nearby=nearby)
+    dF_all = G.t(np.stack([v.dF for v in scene.views]).astype(np.float32))
+    idx = torch.zeros(1, dtype=torch.int32, device="cuda")
+    block = torch.zeros(P.CAMERA_BLOCK_FLOATS, device="cuda")
+    return table, dF_all, idx, block
+
+
+def test_camera_chain_matches_host_helper_and_oracle(P, G, orc):
+    """satsplat_camera_chain (device kernel) per view: F' = F + dF bit-equal to the fp32 sum; sun camera and reprojection
+    constants BIT-EQUAL to the host helper satsplat_sun_camera (and so within its tolerance of the oracle's Eq. 16); nearby
+    camera against the oracle; zero perturbation = the view camera; shading constants copied.  Then the
+    adjoint (satsplat_camera_chain_backward) against the oracle's step-by-step adjoints, only the selected row touched."""
+    import torch
+    scene = S.make_config(2, n=2000, size=128, n_views=4, extent=32.0, sun_size=160)
+    rng = np.random.default_rng(3)
+    nearby = [(0.0, 0.0)] + [(float(rng.normal(0, 0.05)), float(rng.normal(0, 0.03))) for _ in scene.views[1:]]
+    table, dF_all, idx, block = _chain_setup(P, G, scene, nearby)
+    v_all = torch.zeros_like(dF_all)
+    for vi, view in enumerate(scene.views):
+        idx.fill_(vi)
+        P.camera_chain(table, dF_all, idx, block)
+        b = block.cpu().numpy()
+        Fp32 = view.F.astype(np.float32) + view.dF.astype(np.float32)
+        assert np.array_equal(b[0:8].view(np.uint32), Fp32.view(np.uint32))
+        np.testing.assert_array_equal(b[8:11], view.view_dir.astype(np.float32))
+        assert b[11] == np.float32(view.b_z) and b[12] == np.float32(view.z_bg)
+        cam = P.Camera.from_view(view)
+        sun_cam, rep = P.sun_camera(cam, view.sun_azimuth, view.sun_elevation, view.sun_width, view.sun_height, view.sun_viewport)
+        assert np.array_equal(b[16:24].view(np.uint32), np.array(sun_cam.F[:], np.float32).view(np.uint32))      # bit-equal
+        assert np.array_equal(b[63:71].view(np.uint32), np.array(rep, np.float32).view(np.uint32))
+        np.testing.assert_array_equal(b[24:27], np.array(sun_cam.view_dir[:], np.float32))
+        Fs_ref, rep_ref = orc.sun_camera(Fp32.astype(np.float64), view.sun_azimuth, view.sun_elevation, view.sun_viewport)
+        np.testing.assert_allclose(b[16:24], Fs_ref, rtol=2e-6, atol=1e-4)
+        np.testing.assert_allclose(b[63:71], rep_ref, rtol=2e-6, atol=1e-4)
+        # nearby camera against the oracle
+        da, de = nearby[vi]
+        Fn_ref, ang = orc.nearby_camera(Fp32.astype(np.float64), da, de)
+        np.testing.assert_allclose(b[32:40], Fn_ref, rtol=2e-6, atol=2e-6 * np.abs(Fn_ref).max())
+        if vi == 0:
+            np.testing.assert_allclose(b[32:40], Fp32, rtol=1e-6, atol=1e-6 * np.abs(Fp32).max())     # zero perturbation
+            np.testing.assert_allclose(b[40:43], view.view_dir, atol=5e-3)     # direction of F' = F + dF, close to that of F
+        else:
+            assert np.abs(b[32:40] - Fp32).max() > 1e-4 * np.abs(Fp32).max()
+        a2, e2 = ang[0] + da, ang[1] + de
+        np.testing.assert_allclose(b[40:43], -np.array([np.cos(a2) * np.cos(e2), np.sin(a2) * np.cos(e2), np.sin(e2)]), atol=2e-6)
+        # shading constants
+        np.testing.assert_array_equal(b[48:60], view.cc.astype(np.float32))
+        np.testing.assert_array_equal(b[60:63], view.ambient.astype(np.float32))
+        assert b[71] == np.float32(view.depth_bias) and b[72] == np.float32(view.slope)
+        # ---- adjoint ----
+        vV, vS, vR, vN = (rng.normal(0, 1, 8) for _ in range(4))
+        P.camera_chain_backward(table, dF_all, idx, G.t(vV), G.t(vS), G.t(vR), G.t(vN), v_all)
+        ref = (vV.astype(np.float32).astype(np.float64)
+               + orc.sun_camera_backward(Fp32.astype(np.float64), view.sun_azimuth, view.sun_elevation, view.sun_viewport,
+                                         vS.astype(np.float32), vR.astype(np.float32))
+               + orc.nearby_camera_backward(Fp32.astype(np.float64), da, de, vN.astype(np.float32)))
+        got = v_all.cpu().numpy()
+        np.testing.assert_allclose(got[vi], ref, rtol=2e-5, atol=2e-5 * np.abs(ref).max())
+        assert (got[vi + 1:] == 0).all()                 # only the selected row is touched
+    # NULL inputs, index advance
+    v2 = torch.zeros_like(dF_all)
+    idx.fill_(1)
+    P.camera_chain_backward(table, dF_all, idx, None, None, None, None, v2)
+    assert (v2 == 0).all()
+    P.advance_view_index(idx, 3, len(scene.views))
+    assert int(idx.item()) == 0
+
+
+def test_device_camera_path_equals_host_path_and_one_graph_serves_all_views(P, G, orc):
+    """The *_device calls (camera and shading read from the device block) give the results of the host-struct calls bit
+    for bit, view after view, from ONE captured CUDA graph that walks the views by itself, and again after dF has been
+    changed on the device (no re-capture); the nearby-camera pass rendered through the device path matches the oracle run
+    on the oracle's own nearby camera."""
+    import torch
+    import copy
+    scene = S.make_config(2, n=6000, size=128, n_views=3, extent=40.0, sun_size=192)
+    gs = G.GpuScene(scene)
+    n, V = scene.n, len(scene.views)
+    v0 = scene.views[0]
+    W, H, SW, SH = v0.width, v0.height, v0.sun_width, v0.sun_height
+    nearby = [(0.03, -0.02)] * V
+    table, dF_all, idx, block = _chain_setup(P, G, scene, nearby)
+    ctx, sctx = P.Context(n, W, H, 16 * n), P.Context(n, SW, SH, 16 * n)
+    up = [G.t(u) for u in S.upstream_grads(scene.seed, 0, H, W)]
+    out = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    sun_depth, v_sun = torch.empty(SH, SW, device="cuda"), torch.zeros(SH, SW, device="cuda")
+    g = gs.zeros_grads()
+    v_dF_all = torch.zeros_like(dF_all)
+    surf = (gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+
+    def step():
+        for t_ in g.values():
+            t_.zero_()
+        v_sun.zero_()
+        P.camera_chain(table, dF_all, idx, block)
+        sctx.preprocess_device(SW, SH, block, P.CAM_SUN, *surf)
+        sctx.shadow_map(sun_depth)
+        ctx.preprocess_device(W, H, block, P.CAM_VIEW, *surf)
+        ctx.render_forward_device(block, sun_depth, *out)
+        ctx.render_backward_device(block, sun_depth, up[0], up[1], up[2], g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"],
+                                   g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"], v_sun, g["v_reproj"])
+        sctx.shadow_map_backward(v_sun, g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"], g["v_dF_sun"])
+        P.camera_chain_backward(table, dF_all, idx, g["v_dF"], g["v_dF_sun"], g["v_reproj"], None, v_dF_all)
+
+    step()                                   # warm-up outside the capture
+    torch.cuda.synchronize()
+    v_dF_all.zero_()
+    idx.zero_()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+        P.advance_view_index(idx, 1, V)
+    idx.zero_()
+    v_dF_all.zero_()
+
+    def host_reference(view):
+        cam = P.Camera.from_view(view)
+        sun_cam, rep = P.sun_camera(cam, view.sun_azimuth, view.sun_elevation, SW, SH, view.sun_viewport)
+        sv = type("SV", (), {})()
+        sv.width, sv.height, sv.F, sv.dF, sv.view_dir = SW, SH, np.array(sun_cam.F[:]), np.zeros(8), np.array(sun_cam.view_dir[:])
+        sv.b_z, sv.z_bg, sv.bg_rgb = sun_cam.b_z, sun_cam.z_bg, np.zeros(3)
+        res = G.gpu_view_iteration(P, gs, view, sun_view=sv, reproj=rep, upstream=[u.cpu().numpy() for u in up], want_debug=False)
+        tot = G.t(res["grads"]["v_dF"])
+        P.sun_camera_backward(cam, view.sun_azimuth, view.sun_elevation, view.sun_viewport, G.t(res["sun_grads"]["v_dF_sun"]),
+                              G.t(res["grads"]["v_reproj"]), tot)
+        return res, tot.cpu().numpy()
+
+    views = [copy.copy(v) for v in scene.views]
+    for rnd in range(2):                     # second round: dF changed on the device, same graph
+        if rnd == 1:
+            delta = (np.random.default_rng(9).normal(0, 2e-3, (V, 8)) * np.abs(np.stack([v.F for v in views]))).astype(np.float32)
+            dF_all += G.t(delta)
+            for vi, v in enumerate(views):
+                v.dF = (v.dF.astype(np.float32) + delta[vi]).astype(np.float32)
+            v_dF_all.zero_()
+        for vi, view in enumerate(views):
+            assert int(idx.item()) == vi
+            graph.replay()
+            torch.cuda.synchronize()
+            res, dF_ref = host_reference(view)
+            assert np.array_equal(out[0].cpu().numpy(), res["rgba"]) and np.array_equal(out[1].cpu().numpy(), res["geom"])
+            assert np.array_equal(sun_depth.cpu().numpy(), res["sun_depth"])
+            tot = res["grads"]["v_means"] + res["sun_grads"]["v_means"]
+            np.testing.assert_allclose(g["v_means"].cpu().numpy(), tot, rtol=1e-3, atol=1e-4 * max(1.0, np.abs(tot).max()))
+            np.testing.assert_allclose(v_dF_all[vi].cpu().numpy(), dF_ref, rtol=2e-3, atol=2e-3 * np.abs(dF_ref).max())
+        assert int(idx.item()) == 0
+    # ---- the nearby camera pass through the device path against the oracle on the oracle's nearby camera ----
+    view = views[1]
+    idx.fill_(1)
+    P.camera_chain(table, dF_all, idx, block)
+    nctx = P.Context(n, W, H, 16 * n)
+    nctx.preprocess_device(W, H, block, P.CAM_NEARBY, *surf)
+    nout = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    nctx.render_forward_device(block, None, *nout)
+    Fp32 = view.F.astype(np.float32) + view.dF.astype(np.float32)
+    Fn_ref, ang = orc.nearby_camera(Fp32.astype(np.float64), *nearby[1])
+    nv = _no_shadow(view)
+    a2, e2 = ang[0] + nearby[1][0], ang[1] + nearby[1][1]
+    nv.F, nv.dF = block[32:40].cpu().numpy(), np.zeros(8, np.float32)        # the fp32 camera the kernels consumed ...
+    np.testing.assert_allclose(nv.F, Fn_ref, rtol=2e-6, atol=2e-6 * np.abs(Fn_ref).max())   # ... which is the oracle's
+    nv.view_dir = (-np.array([np.cos(a2) * np.cos(e2), np.sin(a2) * np.cos(e2), np.sin(e2)])).astype(np.float32)
+    ref = orc.render_pass(nv, scene)
+    G.assert_bins_bitexact(ref, nctx.debug_bins(), n)
+    f = orc.forward(W, H, nv.b_z, nv.z_bg, nv.bg_rgb, ref["rec64"], ref["flags"], ref["lists"], orc.Shading(cc=nv.cc, ambient=nv.ambient),
+                    threads=orc.num_threads())
+    gpu = dict(rgba=nout[0].cpu().numpy(), geom=nout[1].cpu().numpy(), aux=nout[2].cpu().numpy())
+    G.compare_images(gpu, f, G.fragile_mask(f["margins"]))
+    # calls out of order / mixed modes are refused
+    with pytest.raises(P.SatsplatError) as e:
+        nctx.render_forward(P.Shading.make(), *nout)
+    assert e.value.code == P.E_STATE
+    for c in (ctx, sctx, nctx):
+        c.close()

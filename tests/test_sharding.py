@@ -18,6 +18,12 @@ def _free_port():
         return s.getsockname()[1]
 
 
+def _fake_view_gradient(vi, tot):
+    import torch
+    g = torch.Generator().manual_seed(1000 + vi)
+    return torch.randn(tot, generator=g, dtype=torch.float64)
+
+
 def _worker(rank, world, port, out):
     import torch
     import torch.distributed as dist
@@ -31,8 +37,16 @@ def _worker(rank, world, port, out):
         gathered = [None] * world
         dist.all_gather_object(gathered, (warm_views, step_views))
         ms = bench.max_over_ranks(torch, dist, world, 10.0 + 5.0 * rank, "cpu")
+        # the one collective of the data-parallel path: every rank fills the packed gradient buffer with the (fake)
+        # gradients of ITS views; after the all-reduce every rank holds the sum over all views of all ranks
+        n = 37                                              # not a multiple of 4: the group offsets are padded
+        off, tot = bench.packed_offsets(n)
+        flat = torch.zeros(tot, dtype=torch.float64)
+        for vi in step_views:
+            flat += _fake_view_gradient(vi, tot)
+        bench.allreduce_sum(dist, flat)
         if rank == 0:
-            out.put((gathered, ms))
+            out.put((gathered, ms, flat.numpy().copy(), off, tot))
     finally:
         dist.destroy_process_group()
 
@@ -46,7 +60,7 @@ def test_views_shard_over_two_ranks_gloo():
     procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
     for p in procs:
         p.start()
-    gathered, ms = q.get(timeout=100)
+    gathered, ms, flat, off, tot = q.get(timeout=100)
     for p in procs:
         p.join(60)
         assert p.exitcode == 0
@@ -57,6 +71,11 @@ def test_views_shard_over_two_ranks_gloo():
         assert a != b
     assert set(s0).isdisjoint(s1) and set(w0).isdisjoint(w1)
     assert sorted(w0 + w1 + s0 + s1) == list(range(18))   # consecutive views, no gap, no overlap
+    # all-reduced buffer = sum over ALL timed views of the single-rank gradients
+    import numpy as np
+    want = sum(_fake_view_gradient(vi, tot) for vi in s0 + s1).numpy()
+    np.testing.assert_allclose(flat, want, rtol=1e-12, atol=1e-12)
+    assert off == [0, 112, 260, 336, 376] and tot == 488 and all(o % 4 == 0 for o in off)   # 16-byte aligned groups, N = 37
 
 
 def test_views_for_rank_single_process_cycles():
@@ -97,3 +116,25 @@ def test_reference_arm_runs_on_rank0_only():
     line = got[0]
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "Mpixel/s"
+
+
+def test_gpus_flag_spawns_one_process_per_gpu(monkeypatch):
+    """`python bench.py --gpus 2` without WORLD_SIZE launches two ranks itself (torch.distributed.run on 127.0.0.1) and
+    hands over; under torchrun (WORLD_SIZE set) it does not spawn again."""
+    import bench
+    calls = []
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: calls.append(cmd) or 0)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "2", "--steps", "4", "--warmup", "3"])
+    with pytest.raises(SystemExit) as e:
+        bench.main()
+    assert e.value.code == 0 and len(calls) == 1
+    cmd = calls[0]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    assert cmd[-6:] == ["--gpus", "2", "--steps", "4", "--warmup", "3"] and cmd[-7].endswith("bench.py")
+    # under a launcher: no second spawn (run_ours is reached; stub it out)
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    reached = []
+    monkeypatch.setattr(bench, "run_ours", lambda a: reached.append(a.gpus))
+    bench.main()
+    assert reached == [2] and len(calls) == 1
