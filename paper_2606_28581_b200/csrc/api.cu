@@ -128,7 +128,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->depth_key, N));
   A(dalloc(ctx, &ctx->flags, N));
   A(dalloc(ctx, &ctx->vrec, N * satsplat::kVrec));
-  A(dalloc(ctx, &ctx->block_sums, N / 4096 + 2));
+  A(dalloc(ctx, &ctx->block_sums, (N / 4096 > tiles / 2048 ? N / 4096 : tiles / 2048) + 2));
   A(dalloc(ctx, &ctx->keys[0], K));
   A(dalloc(ctx, &ctx->keys[1], K));
   A(dalloc(ctx, &ctx->vals[0], K));
@@ -136,11 +136,11 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->hist, (size_t)256 * kSortBlocks));
   A(dalloc(ctx, &ctx->ranges, tiles * 2));
   A(dalloc(ctx, &ctx->status, 1));
-  A(dalloc(ctx, &ctx->tile_count, tiles));
+  A(dalloc(ctx, &ctx->tile_count, tiles * satsplat::kCtrStride));
   A(dalloc(ctx, &ctx->tile_start, tiles));
   A(dalloc(ctx, &ctx->worklist, tiles * 2));
   A(dalloc(ctx, &ctx->wl_count, 4));
-  A(cudaMemset(ctx->tile_count, 0, tiles * sizeof(uint32_t)));
+  A(cudaMemset(ctx->tile_count, 0, tiles * satsplat::kCtrStride * sizeof(uint32_t)));
   A(dalloc(ctx, &ctx->px_a, px));
   A(dalloc(ctx, &ctx->px_b, px));
   A(dalloc(ctx, &ctx->px_i, px));

@@ -371,80 +371,120 @@ cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
 // at most once per tile.  4 launches instead of 25, ~10x less traffic.
 // ============================================================================================================
 
-// single CTA: exclusive scan of tile_count[tiles]; writes ranges, K, overflow; resets the cursors and the worklist.
-// Chunks of 1024 x 8 counters are staged through shared memory so that every global access is coalesced.
+// Exclusive scan of tile_count[tiles] in two multi-CTA kernels (a single CTA took 18 us for the 64 KB of a 2048^2 view):
+//  A. every CTA scans its 2048 counters (8 per thread, loaded as two uint4) and leaves the CTA-local exclusive prefix in
+//     tile_start and its total in block_sums;
+//  B. every CTA adds the totals of the CTAs before it (a handful of values), writes the tile ranges (= the scan), turns
+//     the counters into scatter cursors that start at the tile's first position, and files the long lists on the
+//     worklists of the mid / large sort kernels.  K and the overflow flag come from the 64-bit grand total.
+constexpr int kTileScanThreads = 256;
 constexpr int kTileScanItems = 8;
-constexpr int kTileSortWarpMax = 1024;    // entries one warp sorts in registers (32 per lane)
-__global__ void __launch_bounds__(1024) tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_start,
-                                                         uint32_t* __restrict__ ranges, Status* status, uint32_t capacity,
-                                                         uint32_t* __restrict__ wl_count, uint32_t* __restrict__ worklist) {
+constexpr int kTileScanChunk = kTileScanThreads * kTileScanItems;   // 2048 tiles per CTA
+#ifndef SATSPLAT_SORT_SMALL_MAX
+#define SATSPLAT_SORT_SMALL_MAX 256
+#endif
+constexpr int kTileSortSmallMax = SATSPLAT_SORT_SMALL_MAX;    // entries one warp sorts in registers in the small-tile kernel (4 or 8 per lane)
+constexpr int kTileSortMergeMax = 1024;   // entries the 4-warp merge kernel handles (4 chunks of <= 256)
+
+__global__ void __launch_bounds__(kTileScanThreads) tile_scan_partial_kernel(int tiles, const uint32_t* __restrict__ tile_count,
+                                                                             uint32_t* __restrict__ tile_start,
+                                                                             uint32_t* __restrict__ block_sums,
+                                                                             uint32_t* __restrict__ wl_count) {
   __shared__ uint32_t s_warp[33];
-  __shared__ uint32_t s_wl[2];   // lengths of the mid / large worklists (tiles too long for the one-warp register sort)
-  if (threadIdx.x < 2) s_wl[threadIdx.x] = 0u;
-  __shared__ uint32_t s_cnt[1024 * kTileScanItems + 8];
-  __shared__ uint32_t s_total;
-  constexpr int kChunk = 1024 * kTileScanItems;
-  // pass 1: total (decides overflow before any range is written)
-  uint32_t sum = 0;
-  for (int i = threadIdx.x; i < tiles; i += 1024) sum += tile_count[i];
+  if (blockIdx.x == 0 && threadIdx.x < 4) wl_count[threadIdx.x] = 0u;   // worklist lengths / cursors of this pass
+  const int i0 = blockIdx.x * kTileScanChunk + threadIdx.x * kTileScanItems;
+  uint32_t v[kTileScanItems];
+  if (kCtrStride == 1 && i0 + kTileScanItems <= tiles) {
+    const uint4 a = reinterpret_cast<const uint4*>(tile_count + i0)[0], b = reinterpret_cast<const uint4*>(tile_count + i0)[1];
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  } else {
+#pragma unroll
+    for (int k = 0; k < kTileScanItems; ++k) v[k] = i0 + k < tiles ? tile_count[(size_t)(i0 + k) * kCtrStride] : 0u;
+  }
+  uint32_t part = 0;
+#pragma unroll
+  for (int k = 0; k < kTileScanItems; ++k) part += v[k];
   uint32_t total;
-  block_exclusive_scan(sum, s_warp, &total);
-  const bool overflow = total > capacity;
-  uint32_t carry = 0;
-  for (int base = 0; base < tiles; base += kChunk) {
-    const int n = min(kChunk, tiles - base);
-    for (int i = threadIdx.x; i < n; i += 1024) {
-      s_cnt[i] = tile_count[base + i];
-      tile_count[base + i] = 0;                     // becomes the scatter cursor
-    }
-    __syncthreads();
-    uint32_t v[kTileScanItems], part = 0;
+  uint32_t run = block_exclusive_scan(part, s_warp, &total);
 #pragma unroll
-    for (int k = 0; k < kTileScanItems; ++k) {
-      const int i = threadIdx.x * kTileScanItems + k;
-      v[k] = i < n ? s_cnt[i] : 0u;
-      part += v[k];
-    }
-    uint32_t chunk_total;
-    uint32_t run = carry + block_exclusive_scan(part, s_warp, &chunk_total);
-#pragma unroll
-    for (int k = 0; k < kTileScanItems; ++k) {
-      const int i = threadIdx.x * kTileScanItems + k;
-      if (i < n) s_cnt[i] = run;                    // exclusive prefix, back in place
-      run += v[k];
-    }
-    if (threadIdx.x == 1023) s_total = run;         // = carry + chunk_total
-    __syncthreads();
-    for (int i = threadIdx.x; i < n; i += 1024) {
-      const uint32_t st = s_cnt[i];
-      const uint32_t en = (i + 1 < n) ? s_cnt[i + 1] : s_total;
-      tile_start[base + i] = st;
-      const bool empty = en == st || overflow;      // overflow: nothing is rendered (outputs undefined, no OOB access)
-      reinterpret_cast<uint2*>(ranges)[base + i] = empty ? make_uint2(0u, 0u) : make_uint2(st, en);
-      const uint32_t len = empty ? 0u : en - st;
-      if (len > 256u) {                             // dispatch by list length (see tile_sort_kernel)
-        if (len > (uint32_t)kTileSortWarpMax) worklist[tiles + atomicAdd(&s_wl[1], 1u)] = (uint32_t)(base + i);
-        else worklist[atomicAdd(&s_wl[0], 1u)] = (uint32_t)(base + i);
-      }
-    }
-    carry += chunk_total;
-    __syncthreads();
+  for (int k = 0; k < kTileScanItems; ++k) {
+    if (i0 + k < tiles) tile_start[i0 + k] = run;
+    run += v[k];
   }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    status->K = total;
-    status->overflow = overflow ? 1u : 0u;
-    wl_count[0] = s_wl[0];
-    wl_count[1] = 0;
-    wl_count[2] = s_wl[1];
-    wl_count[3] = 0;
-  }
+  if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
 }
 
+__global__ void __launch_bounds__(kTileScanThreads) tile_scan_finish_kernel(int tiles, int nblocks, uint32_t* __restrict__ cursor,
+                                                                            const uint32_t* __restrict__ tile_start,
+                                                                            const uint32_t* __restrict__ block_sums,
+                                                                            uint32_t* __restrict__ ranges, Status* status,
+                                                                            uint32_t capacity, uint32_t* __restrict__ wl_count,
+                                                                            uint32_t* __restrict__ worklist) {
+  // one tile per thread; this CTA's tiles lie inside chunk `cb` of kernel A
+  __shared__ unsigned long long s_red[2][kTileScanThreads / 32];
+  __shared__ unsigned long long s_off[2];
+  const int i = blockIdx.x * kTileScanThreads + threadIdx.x;
+  const int cb = (blockIdx.x * kTileScanThreads) / kTileScanChunk;
+  // offset of the chunk = sum of the chunk totals before it; grand total in 64 bits (it may exceed 2^32: flagged as overflow)
+  unsigned long long before = 0, all = 0;
+  for (int b = threadIdx.x; b < nblocks; b += kTileScanThreads) {
+    const unsigned long long t = block_sums[b];
+    all += t;
+    if (b < cb) before += t;
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    before += __shfl_xor_sync(0xffffffffu, before, d);
+    all += __shfl_xor_sync(0xffffffffu, all, d);
+  }
+  if ((threadIdx.x & 31) == 0) { s_red[0][threadIdx.x >> 5] = before; s_red[1][threadIdx.x >> 5] = all; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long a = 0, b = 0;
+    for (int w = 0; w < kTileScanThreads / 32; ++w) { a += s_red[0][w]; b += s_red[1][w]; }
+    s_off[0] = a; s_off[1] = b;
+  }
+  __syncthreads();
+  const unsigned long long total = s_off[1];
+  const bool overflow = total > (unsigned long long)capacity;
+  const uint32_t off = (uint32_t)s_off[0];
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    status->K = total > 0xffffffffull ? 0xffffffffu : (uint32_t)total;
+    status->overflow = overflow ? 1u : 0u;
+  }
+  const int lane = threadIdx.x & 31;
+  uint32_t len = 0;
+  if (i < tiles) {
+    const bool last_of_chunk = (i + 1 == tiles) || ((i + 1) % kTileScanChunk == 0);
+    const uint32_t st = off + tile_start[i];
+    const uint32_t en = off + (last_of_chunk ? block_sums[cb] : tile_start[i + 1]);
+    const bool empty = en == st || overflow;         // overflow: nothing is rendered (outputs undefined, no OOB access)
+    reinterpret_cast<uint2*>(ranges)[i] = empty ? make_uint2(0u, 0u) : make_uint2(st, en);
+    cursor[(size_t)i * kCtrStride] = st;             // the scatter appends at cursor++ (the sort kernel clears it again)
+    len = empty ? 0u : en - st;
+  }
+  // long lists go to the worklists (warp-aggregated appends): [0, tiles) merge kernel, [tiles, 2 tiles) large kernel
+  const bool mid = len > (uint32_t)kTileSortSmallMax && len <= (uint32_t)kTileSortMergeMax;
+  const bool big = len > (uint32_t)kTileSortMergeMax;
+  const unsigned mm = __ballot_sync(0xffffffffu, mid), mb = __ballot_sync(0xffffffffu, big);
+  uint32_t bm = 0, bb = 0;
+  if (lane == 0) {
+    if (mm) bm = atomicAdd(wl_count + 0, (uint32_t)__popc(mm));
+    if (mb) bb = atomicAdd(wl_count + 2, (uint32_t)__popc(mb));
+  }
+  bm = __shfl_sync(0xffffffffu, bm, 0);
+  bb = __shfl_sync(0xffffffffu, bb, 0);
+  const unsigned lt = (1u << lane) - 1u;
+  if (mid) worklist[bm + __popc(mm & lt)] = (uint32_t)i;
+  if (big) worklist[tiles + bb + __popc(mb & lt)] = (uint32_t)i;
+}
+
+// Appends (depth bits << 32 | surfel id) to the segment of every tile of the surfel's rect: position = cursor[tile]++ (the
+// cursors start at the tiles' first positions).  The returning atomics of up to four tiles are issued back to back
+// before the first store (one L2 round trip instead of four).
 __global__ void __launch_bounds__(256) tile_scatter_kernel(int N, int TX, const ushort4* __restrict__ rect,
                                                            const uint32_t* __restrict__ count,
-                                                           const uint32_t* __restrict__ depth_key,
-                                                           const uint32_t* __restrict__ tile_start, uint32_t* __restrict__ cursor,
+                                                           const uint32_t* __restrict__ depth_key, uint32_t* __restrict__ cursor,
                                                            const Status* __restrict__ status, uint64_t* __restrict__ entries) {
   if (status->overflow) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -457,11 +497,18 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int N, int TX, const 
   }
   if (cnt && cnt <= kDupCoopThreshold) {
     const uint64_t e = ((uint64_t)dk << 32) | (uint32_t)i;
-    for (int ty = r.y; ty < r.w; ++ty)
-      for (int tx = r.x; tx < r.z; ++tx) {
-        const int t = ty * TX + tx;
-        entries[tile_start[t] + atomicAdd(cursor + t, 1u)] = e;
+    const uint32_t w = (uint32_t)(r.z - r.x);
+    for (uint32_t q0 = 0; q0 < cnt; q0 += 4) {
+      uint32_t pos[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t q = q0 + k;
+        if (q < cnt) pos[k] = atomicAdd(cursor + (size_t)((r.y + q / w) * TX + r.x + q % w) * kCtrStride, 1u);
       }
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (q0 + k < cnt) entries[pos[k]] = e;
+    }
   }
   unsigned big = __ballot_sync(0xffffffffu, cnt > kDupCoopThreshold);
   while (big) {
@@ -476,7 +523,7 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int N, int TX, const 
     const uint64_t e = ((uint64_t)k2 << 32) | id;
     for (uint32_t q = lane; q < c2; q += 32) {
       const int t = (y0 + (int)(q / (uint32_t)w)) * TX + x0 + (int)(q % (uint32_t)w);
-      entries[tile_start[t] + atomicAdd(cursor + t, 1u)] = e;
+      entries[atomicAdd(cursor + (size_t)t * kCtrStride, 1u)] = e;
     }
   }
 }
@@ -571,60 +618,110 @@ __device__ __noinline__ void tile_sort_warp(const uint64_t* __restrict__ in, uin
   }
 }
 
-// Tiles are dispatched by list length so that each kernel keeps the register budget (and occupancy) of its own
-// variants: <= 256 entries here (2/4/8 registers per lane), 257..1024 in tile_sort_mid_kernel (16/32 per lane),
-// longer ones in tile_sort_large_kernel (one CTA per tile).  Worklists: [0, tiles) mid, [tiles, 2 tiles) large;
-// wl_count = {mid length, mid cursor, large length, large cursor}.
+// same, sorted (depth, id) composites left in shared memory (a chunk of the merge kernel)
+template <int E>
+__device__ __noinline__ void chunk_sort_warp(const uint64_t* __restrict__ in, uint32_t n, uint64_t* __restrict__ out, int lane) {
+  uint64_t v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const uint32_t i = lane * E + e;
+    v[e] = i < n ? in[i] : ~0ull;
+  }
+  warp_bitonic_regs<E>(v, lane);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const uint32_t i = lane * E + e;
+    if (i < n) out[i] = v[e];
+  }
+}
+
+// Tiles are dispatched by list length: <= 256 entries here (one warp per tile, 2 / 4 / 8 registers per lane), 257..1024 in
+// tile_sort_merge_kernel (one 4-warp CTA per tile), longer ones in tile_sort_large_kernel (one 1024-thread CTA per tile).
+// At C3 a fifth of the tiles hold more than 256 entries (walls stack surfels along the ray) and carry half of the
+// pairs.  Worklists: [0, tiles) merge, [tiles, 2 tiles) large; wl_count = {merge length, merge cursor, large length,
+// large cursor}.
 __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tiles, const uint32_t* __restrict__ ranges,
                                                                         const uint64_t* __restrict__ entries,
                                                                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                                                        uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count,
                                                                         uint32_t* __restrict__ cursor) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = blockIdx.x * kTileSortWarps + warp;
   if (t >= tiles) return;
-  if (lane == 0) cursor[t] = 0;   // leave the per-tile counters zero for the next preprocess on this context
+  if (lane == 0) cursor[(size_t)t * kCtrStride] = 0;   // leave the per-tile counters zero for the next preprocess on this context
   const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
   if (n == 0) return;
-  if (n > 256u) return;           // on a worklist (built by tile_scan_kernel): sorted by the mid / large kernels beside this one
+  if (n > (uint32_t)kTileSortSmallMax) return;   // on a worklist (built by the scan): sorted by the merge / large kernels beside this one
   const uint64_t hi = (uint64_t)(uint32_t)t << 32;
   if (n <= 64) tile_sort_warp<2>(entries + s, n, hi, keys + s, vals + s, lane);
-  else if (n <= 128) tile_sort_warp<4>(entries + s, n, hi, keys + s, vals + s, lane);
+  else if (kTileSortSmallMax <= 128 || n <= 128) tile_sort_warp<4>(entries + s, n, hi, keys + s, vals + s, lane);
   else tile_sort_warp<8>(entries + s, n, hi, keys + s, vals + s, lane);
 }
 
-__global__ void __launch_bounds__(128) tile_sort_mid_kernel(const uint32_t* __restrict__ ranges, const uint64_t* __restrict__ entries,
-                                                            uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                                            const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
-  const int lane = threadIdx.x & 31;
+// number of elements of the sorted range a[0, n) that are smaller than x (all values are distinct)
+__device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t n, uint64_t x) {
+  uint32_t lo = 0;
+  while (n > 0) {
+    const uint32_t h = n >> 1;
+    const bool right = a[lo + h] < x;
+    lo = right ? lo + h + 1 : lo;
+    n = right ? n - h - 1 : h;
+  }
+  return lo;
+}
+
+// Lists of 257..1024 entries: the CTA's four warps each sort a quarter in registers (<= 256 entries, 2/4/8 per lane),
+// then two merge rounds in shared memory by rank: an element's place in the merge of two sorted runs is its own index
+// plus the number of smaller elements in the other run (binary search; the (depth, id) composites are distinct).
+__global__ void __launch_bounds__(128) tile_sort_merge_kernel(const uint32_t* __restrict__ ranges, const uint64_t* __restrict__ entries,
+                                                              uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                              const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
+  __shared__ uint64_t s_a[kTileSortMergeMax], s_b[kTileSortMergeMax];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t total = wl_count[0];
-  for (;;) {
-    uint32_t item = 0;
-    if (lane == 0) item = atomicAdd(wl_count + 1, 1u);
-    item = __shfl_sync(0xffffffffu, item, 0);
-    if (item >= total) return;
+  // items are dealt round-robin to the CTAs: a shared work counter costs one same-address atomic per item, which at
+  // ~13 ns each was the whole duration of this kernel (3000 items per pass)
+  for (uint32_t item = blockIdx.x; item < total; item += gridDim.x) {
+    __syncthreads();
     const uint32_t t = worklist[item];
     const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
+    const uint32_t c = (n + 3) >> 2;                         // quarter length (<= 256)
+    {
+      const uint32_t b = min((uint32_t)warp * c, n), e = min(b + c, n);
+      if (c <= 64) chunk_sort_warp<2>(entries + s + b, e - b, s_a + b, lane);
+      else if (c <= 128) chunk_sort_warp<4>(entries + s + b, e - b, s_a + b, lane);
+      else chunk_sort_warp<8>(entries + s + b, e - b, s_a + b, lane);
+    }
+    __syncthreads();
+    // round 1: quarters (0,1) and (2,3)
+    for (uint32_t i = threadIdx.x; i < n; i += 128) {
+      const uint32_t q = i / c, sib = q ^ 1u;
+      const uint32_t sb = min(sib * c, n), se = min(sb + c, n);
+      const uint64_t x = s_a[i];
+      // ties cannot occur; the run that comes first wins "equal" by construction of lower_bound on distinct values
+      s_b[(q & ~1u) * c + (i - q * c) + lower_bound_u64(s_a + sb, se - sb, x)] = x;
+    }
+    __syncthreads();
+    // round 2: halves [0, h) and [h, n), straight to the output
+    const uint32_t h = min(2u * c, n);
     const uint64_t hi = (uint64_t)t << 32;
-    if (n <= 512) tile_sort_warp<16>(entries + s, n, hi, keys + s, vals + s, lane);
-    else tile_sort_warp<32>(entries + s, n, hi, keys + s, vals + s, lane);
+    for (uint32_t i = threadIdx.x; i < n; i += 128) {
+      const uint64_t x = s_b[i];
+      const uint32_t o = i < h ? i + lower_bound_u64(s_b + h, n - h, x) : (i - h) + lower_bound_u64(s_b, h, x);
+      keys[s + o] = hi | (x >> 32);
+      vals[s + o] = (uint32_t)x;
+    }
   }
 }
 
-// tiles with more than kTileSortWarpMax entries (oversized splats; tiny images): one 1024-thread CTA
+// tiles with more than kTileSortMergeMax entries (oversized splats; tiny images): one 1024-thread CTA
 // per worklist item, in shared memory up to kTileSortCtaMax entries, else in place in global memory.
 __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* __restrict__ ranges, uint64_t* __restrict__ entries,
                                                                uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
                                                                const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
   extern __shared__ uint64_t s_big[];
-  __shared__ uint32_t s_item;
   const uint32_t total = wl_count[2];
-  for (;;) {
+  for (uint32_t item = blockIdx.x; item < total; item += gridDim.x) {
     __syncthreads();
-    if (threadIdx.x == 0) s_item = atomicAdd(wl_count + 3, 1u);
-    __syncthreads();
-    const uint32_t item = s_item;
-    if (item >= total) return;
     const uint32_t t = worklist[item];
     const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
     uint64_t* buf;
@@ -651,9 +748,11 @@ cudaError_t init_binning_attrs() {
 
 cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
-  ++g_kernel_launches;
-  tile_scan_kernel<<<1, 1024, 0, s>>>(tiles, c->tile_count, c->tile_start, c->ranges, c->status, (uint32_t)c->max_dup, c->wl_count,
-                                      c->worklist);
+  const int nblocks = (tiles + kTileScanChunk - 1) / kTileScanChunk;
+  g_kernel_launches += 2;
+  tile_scan_partial_kernel<<<nblocks, kTileScanThreads, 0, s>>>(tiles, c->tile_count, c->tile_start, c->block_sums, c->wl_count);
+  tile_scan_finish_kernel<<<(tiles + kTileScanThreads - 1) / kTileScanThreads, kTileScanThreads, 0, s>>>(tiles, nblocks, c->tile_count, c->tile_start, c->block_sums, c->ranges,
+                                                              c->status, (uint32_t)c->max_dup, c->wl_count, c->worklist);
   return cudaGetLastError();
 }
 
@@ -661,23 +760,23 @@ cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s) {
   if (N == 0) return cudaSuccess;
   ++g_kernel_launches;
   tile_scatter_kernel<<<(int)((N + 255) / 256), 256, 0, s>>>((int)N, c->cam.TX, reinterpret_cast<const ushort4*>(c->rect), c->count,
-                                                             c->depth_key, c->tile_start, c->tile_count, c->status, c->keys[1]);
+                                                             c->depth_key, c->tile_count, c->status, c->keys[1]);
   return cudaGetLastError();
 }
 
 cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
   g_kernel_launches += 3;
-  // the three kernels work on disjoint tiles (the worklists come from tile_scan_kernel): the few long lists, whose
-  // one-tile latency sets the duration of their kernels, are sorted on a second stream beside the many short ones
+  // the three kernels work on disjoint tiles (the worklists come from the scan): the long lists are sorted on a second
+  // stream beside the many short ones
   cudaEventRecord(c->bin_ev[0], s);
   cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
-  tile_sort_mid_kernel<<<c->sm_count * 4, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_merge_kernel<<<c->sm_count * 8, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
   tile_sort_large_kernel<<<(c->sm_count + 1) / 2, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
-                                                                            c->worklist + tiles, c->wl_count);
+                                                                                               c->worklist + tiles, c->wl_count);
   cudaEventRecord(c->bin_ev[1], c->bin_stream);
-  tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(
-      tiles, c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count, c->tile_count);
+  tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(tiles, c->ranges, c->keys[1], c->keys[0],
+                                                                                                 c->vals[0], c->tile_count);
   cudaStreamWaitEvent(s, c->bin_ev[1], 0);
   c->sorted = 0;
   return cudaGetLastError();

@@ -102,6 +102,13 @@ struct ShRef {
 constexpr int kVrec = 20;
 constexpr int kRedCopies = 64;   // copies of the 23 epilogue-gradient sums (cc, ambient, reproj) the backward spreads its REDs over
 
+// Per-tile pair counters / scatter cursors are spaced kCtrStride words apart: the 2 M returning atomics of a C3 pass land on
+// 16 K counters; packed, 32 of them share a 128-byte line and serialise in one L2 atomic unit (measured)
+#ifndef SATSPLAT_CTR_STRIDE
+#define SATSPLAT_CTR_STRIDE 8
+#endif
+constexpr int kCtrStride = SATSPLAT_CTR_STRIDE;
+
 // sort configuration
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 8;

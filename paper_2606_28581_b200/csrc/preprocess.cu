@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera camv, const f
   if (tile_count == nullptr) return;
   if (cnt > 0 && cnt <= 16) {
     for (int ty = ty0; ty < ty1; ++ty)
-      for (int tx = tx0; tx < tx1; ++tx) atomicAdd(tile_count + ty * camv.TX + tx, 1u);
+      for (int tx = tx0; tx < tx1; ++tx) atomicAdd(tile_count + (size_t)(ty * camv.TX + tx) * kCtrStride, 1u);
   }
   unsigned big = __ballot_sync(0xffffffffu, cnt > 16);
   const int lane = threadIdx.x & 31;
@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(256) preprocess_kernel(DevCamera camv, const f
     const int c2 = __shfl_sync(0xffffffffu, cnt, src);
     const int x0 = __shfl_sync(0xffffffffu, tx0, src), y0 = __shfl_sync(0xffffffffu, ty0, src);
     const int w = __shfl_sync(0xffffffffu, tx1, src) - x0;
-    for (int q = lane; q < c2; q += 32) atomicAdd(tile_count + (y0 + q / w) * camv.TX + x0 + q % w, 1u);
+    for (int q = lane; q < c2; q += 32) atomicAdd(tile_count + (size_t)((y0 + q / w) * camv.TX + x0 + q % w) * kCtrStride, 1u);
   }
 }
 
