@@ -697,25 +697,42 @@ def run_ours(args):
         sh.shadows_on = 1 if job.shadows else 0
         P.reserve_host_staging(job.ctx, job.sctx)
 
+        hargs = (cam, sun, sh, scene.n, *h_in, *h_up, *h_out, h_g)
+
         def e2e_step(_):
-            P.iteration_host(job.ctx, job.sctx, cam, sun, sh, scene.n, *h_in, *h_up, *h_out, h_g)
+            P.iteration_host(job.ctx, job.sctx, *hargs)
         for _ in range(2):
             e2e_step(0)
         n_e2e = max(3, min(args.steps, 10))
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for i in range(n_e2e):
-            e2e_step(i)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(torch, dist, world, dt, "cuda")
+
+        def wall(fn):
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            t0 = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            return max_over_ranks(torch, dist, world, time.perf_counter() - t0, "cuda")
+
+        def serial():
+            for i in range(n_e2e):
+                e2e_step(i)
+
+        def pipelined():   # the begin / end pair: the upload of step i+1 crosses PCIe while the kernels of step i run
+            P.iteration_host_begin(job.ctx, job.sctx, 0, *hargs)
+            for i in range(1, n_e2e):
+                P.iteration_host_begin(job.ctx, job.sctx, i & 1, *hargs)
+                P.iteration_host_end(job.ctx, (i - 1) & 1)
+            P.iteration_host_end(job.ctx, (n_e2e - 1) & 1)
+        dt_serial = wall(serial)
+        pipelined()
+        dt = wall(pipelined)
         h2d = scene.n * 56 + 3 * px * 16
         d2h = 3 * px * 16 + (scene.n * 13 + 23) * 4
         line["e2e"] = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                           ms_per_step=1e3 * dt / n_e2e, steps=n_e2e,
-                           api="satsplat_iteration_host (pinned host buffers; same work as the device step, cascade chain included)")
+                           ms_per_step=1e3 * dt / n_e2e, steps=n_e2e, serial_ms_per_step=1e3 * dt_serial / n_e2e,
+                           api="satsplat_iteration_host_begin / _end, two steps in flight (pinned host buffers; same work as the device "
+                               "step, cascade chain included); serial_ms_per_step = one blocking satsplat_iteration_host per step")
     # ---- the oracle beside it (rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline_block(scene, step_views[0], px, nviews)

@@ -246,6 +246,19 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
                             const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
                             float* h_grads, satsplat_stream stream);
 
+/* The same iteration split in two, so that the copies of consecutive steps overlap (the upload of step i+1 crosses PCIe
+ * while the kernels of step i run): _begin enqueues everything for one step on staging slot `slot` (0 or 1) and returns
+ * without synchronising; _end blocks until that step's images and gradients are in the host buffers.  A slot can be
+ * begun again only after its _end (SATSPLAT_E_STATE otherwise); the host buffers of a step must stay valid and
+ * untouched until its _end.  satsplat_iteration_host == _begin(slot 0) + _end(slot 0). */
+int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                                  const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                                  const float* h_means, const float* h_quats, const float* h_scales,
+                                  const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                                  const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                                  float* h_grads, satsplat_stream stream);
+int satsplat_iteration_host_end(satsplat_ctx* ctx, int32_t slot);
+
 /* ---- optimiser step ------------------------------------------------------- */
 /* One Adam step [Kingma & Ba 2015, Alg. 1] over the five surfel groups with per-group learning rates (PAPER.md:349:
  * 0.075 means, 0.0025 colour, 0.001 quaternions and scales; the paper names no opacity rate, no betas and no epsilon:

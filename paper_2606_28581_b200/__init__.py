@@ -150,6 +150,8 @@ def lib():
         L.satsplat_shadow_map_backward.argtypes = [vp] * 8
         L.satsplat_iteration_host.argtypes = [vp, vp, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading), i64] + [vp] * 13
         L.satsplat_reserve_host_staging.argtypes = [vp, vp]
+        L.satsplat_iteration_host_begin.argtypes = [vp, vp, i32, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading), i64] + [vp] * 13
+        L.satsplat_iteration_host_end.argtypes = [vp, i32]
         L.satsplat_sync_status.argtypes = [vp, C.POINTER(i64), vp]
         L.satsplat_debug_bins.argtypes = [vp, C.POINTER(i64)] + [C.POINTER(vp)] * 5 + [vp]
         L.satsplat_debug_records.argtypes = [vp, vp, vp, vp]
@@ -473,6 +475,29 @@ class Context:
 def reserve_host_staging(ctx: Context, sun_ctx=None):
     """satsplat_reserve_host_staging: allocate the device staging of iteration_host (explicit, never lazy)."""
     ctx._rc(lib().satsplat_reserve_host_staging(ctx._h, None if sun_ctx is None else sun_ctx._h))
+
+
+def _host_ptr(t):
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise ValueError("expected contiguous fp32 CPU tensors")
+    return t.data_ptr()
+
+
+def iteration_host_begin(ctx: Context, sun_ctx, slot, cam: Camera, sun, shading: Shading, n, h_means, h_quats, h_scales, h_logits,
+                         h_rgb, h_v_rgba, h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, stream=None):
+    """satsplat_iteration_host_begin: enqueue one iteration with HOST tensors on staging slot 0 / 1; no synchronisation."""
+    hp = _host_ptr
+    ctx._rc(lib().satsplat_iteration_host_begin(ctx._h, None if sun_ctx is None else sun_ctx._h, int(slot), C.byref(cam),
+                                                None if sun is None else C.byref(sun), C.byref(shading), int(n), hp(h_means),
+                                                hp(h_quats), hp(h_scales), hp(h_logits), hp(h_rgb), hp(h_v_rgba), hp(h_v_geom),
+                                                hp(h_v_aux), hp(h_out_rgba), hp(h_out_geom), hp(h_out_aux), hp(h_grads), _stream(stream)))
+
+
+def iteration_host_end(ctx: Context, slot):
+    """satsplat_iteration_host_end: wait until the step begun on `slot` has delivered its images and gradients."""
+    ctx._rc(lib().satsplat_iteration_host_end(ctx._h, int(slot)))
 
 
 def iteration_host(ctx: Context, sun_ctx, cam: Camera, sun, shading: Shading, n, h_means, h_quats, h_scales, h_logits,

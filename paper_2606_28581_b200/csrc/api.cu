@@ -169,8 +169,8 @@ void satsplat_destroy(satsplat_ctx* ctx) {
   void* ptrs[] = {ctx->rec, ctx->bbox, ctx->rect, ctx->count, ctx->offset, ctx->depth_key, ctx->flags, ctx->vrec, ctx->block_sums,
                   ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->tile_count,
                   ctx->tile_start, ctx->worklist, ctx->wl_count, ctx->px_a,
-                  ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in, ctx->e2e_up,
-                  ctx->e2e_out, ctx->e2e_grads};
+                  ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in[0], ctx->e2e_in[1],
+                  ctx->e2e_up[0], ctx->e2e_up[1], ctx->e2e_out[0], ctx->e2e_out[1], ctx->e2e_grads[0], ctx->e2e_grads[1]};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
@@ -180,8 +180,8 @@ void satsplat_destroy(satsplat_ctx* ctx) {
     if (ctx->bin_ev[i]) cudaEventDestroy(ctx->bin_ev[i]);
   for (int i = 0; i < 2; ++i)
     if (ctx->e2e_stream[i]) cudaStreamDestroy(ctx->e2e_stream[i]);
-  for (int i = 0; i < 4; ++i)
-    if (ctx->e2e_ev[i]) cudaEventDestroy(ctx->e2e_ev[i]);
+  for (int i = 0; i < 10; ++i)
+    if (ctx->e2e_ev[i / 5][i % 5]) cudaEventDestroy(ctx->e2e_ev[i / 5][i % 5]);
   free(ctx);
 }
 
@@ -655,33 +655,35 @@ inline Pack pack_offsets(size_t n) {
 int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_reserve_host_staging: ctx is NULL");
   CU(cudaSetDevice(ctx->device));
-  if (!ctx->e2e_in) {
+  if (!ctx->e2e_in[0]) {
     const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
     const Pack pk = pack_offsets((size_t)ctx->max_surfels);
-    CU(dalloc(ctx, &ctx->e2e_in, pk.off[5] + 4));
-    CU(dalloc(ctx, &ctx->e2e_up, mpx * 12));
-    CU(dalloc(ctx, &ctx->e2e_out, mpx * 12));
-    CU(dalloc(ctx, &ctx->e2e_grads, pk.off[5] + 64));
+    for (int k = 0; k < 2; ++k) {
+      CU(dalloc(ctx, &ctx->e2e_in[k], pk.off[5] + 4));
+      CU(dalloc(ctx, &ctx->e2e_up[k], mpx * 12));
+      CU(dalloc(ctx, &ctx->e2e_out[k], mpx * 12));
+      CU(dalloc(ctx, &ctx->e2e_grads[k], pk.off[5] + 64));
+      for (int i = 0; i < 5; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
+    }
     for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
-    for (int i = 0; i < 4; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[i], cudaEventDisableTiming));
   }
-  if (sun_ctx && !sun_ctx->e2e_out) {
+  if (sun_ctx && !sun_ctx->e2e_out[0]) {
     const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
-    const cudaError_t e = dalloc(sun_ctx, &sun_ctx->e2e_out, mpx * 2);   // sun map + its gradient
+    const cudaError_t e = dalloc(sun_ctx, &sun_ctx->e2e_out[0], mpx * 2);   // sun map + its gradient
     if (e != cudaSuccess) return fail(ctx, SATSPLAT_E_CUDA, "satsplat_reserve_host_staging: %s", cudaGetErrorString(e));
   }
   return SATSPLAT_OK;
 }
 
-int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
-                            const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
-                            const float* h_means, const float* h_quats, const float* h_scales,
-                            const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
-                            const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
-                            float* h_grads, satsplat_stream stream) {
+int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                                  const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                                  const float* h_means, const float* h_quats, const float* h_scales,
+                                  const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                                  const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                                  float* h_grads, satsplat_stream stream) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_iteration_host: ctx is NULL");
-  if (!cam || !shading || !h_means || !h_quats || !h_scales || !h_logits || !h_rgb || !h_grads || N <= 0)
-    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: NULL argument");
+  if (!cam || !shading || !h_means || !h_quats || !h_scales || !h_logits || !h_rgb || !h_grads || N <= 0 || slot < 0 || slot > 1)
+    return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: bad argument");
   // every size is checked before the first copy is enqueued
   if (N > ctx->max_surfels) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: N exceeds max_surfels");
   if (cam->width <= 0 || cam->height <= 0 || cam->width > ctx->max_w || cam->height > ctx->max_h)
@@ -692,8 +694,9 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
     if (N > sun_ctx->max_surfels || sun->width <= 0 || sun->height <= 0 || sun->width > sun_ctx->max_w || sun->height > sun_ctx->max_h)
       return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: sun map size or N exceeds the sun context");
   }
-  if (!ctx->e2e_in || (shadows && !sun_ctx->e2e_out))
+  if (!ctx->e2e_in[0] || (shadows && !sun_ctx->e2e_out[0]))
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: call satsplat_reserve_host_staging first");
+  if (ctx->e2e_busy[slot]) return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host_begin: slot still in flight (call _end)");
   cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
   // the sun camera and the reprojection constants are derived from F' = F + dF (Eq. 16, cascade of Fig. 1)
@@ -705,33 +708,33 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   }
   const size_t n = (size_t)N, px = (size_t)cam->width * cam->height;
   const size_t spx = shadows ? (size_t)sun->width * sun->height : 0;
-  // Three queues: the caller's stream carries the surfel upload and every kernel; the upstream gradients (only
-  // needed by the backward) go up on a second stream while the sun and view forward passes run, and the images come
-  // down on a third while the backward runs (PCIe is full duplex).
+  // Three queues.  Every host->device copy of the step goes up on the upload stream as soon as it is enqueued: while the
+  // caller's stream is still busy with the kernels of the previous step (other slot), this step's 257 MB are already
+  // crossing PCIe.  The caller's stream carries the kernels; the images come down on the download stream while the
+  // backward runs, the gradients after it (PCIe is full duplex).
   cudaStream_t s_up = ctx->e2e_stream[0], s_down = ctx->e2e_stream[1];
-  cudaEvent_t ev_start = ctx->e2e_ev[0], ev_up = ctx->e2e_ev[1], ev_fwd = ctx->e2e_ev[2], ev_img = ctx->e2e_ev[3];
-  CU(cudaEventRecord(ev_start, s));
+  cudaEvent_t* ev = ctx->e2e_ev[slot];   // 0 surfels up, 1 upstream up, 2 forward done, 3 backward done, 4 everything down
   const Pack pk = pack_offsets(n);
   float* d_in[5];
   const float* h_in[5] = {h_means, h_quats, h_scales, h_logits, h_rgb};
   static const int width[5] = {3, 4, 2, 1, 3};
   for (int k = 0; k < 5; ++k) {
-    d_in[k] = ctx->e2e_in + pk.off[k];
-    CU(cudaMemcpyAsync(d_in[k], h_in[k], n * width[k] * sizeof(float), cudaMemcpyHostToDevice, s));
+    d_in[k] = ctx->e2e_in[slot] + pk.off[k];
+    CU(cudaMemcpyAsync(d_in[k], h_in[k], n * width[k] * sizeof(float), cudaMemcpyHostToDevice, s_up));
   }
+  CU(cudaEventRecord(ev[0], s_up));
   float* d_up[3] = {nullptr, nullptr, nullptr};
   const float* h_up[3] = {h_v_rgba, h_v_geom, h_v_aux};
-  CU(cudaStreamWaitEvent(s_up, ev_start, 0));
   for (int k = 0; k < 3; ++k)
     if (h_up[k]) {
-      d_up[k] = ctx->e2e_up + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+      d_up[k] = ctx->e2e_up[slot] + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
       CU(cudaMemcpyAsync(d_up[k], h_up[k], px * 16, cudaMemcpyHostToDevice, s_up));
     }
-  CU(cudaEventRecord(ev_up, s_up));
+  CU(cudaEventRecord(ev[1], s_up));
   float* d_out[3];
-  for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+  for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out[slot] + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
   // device gradients: the five surfel groups at 16-byte aligned offsets, then dF(8) cc(12) ambient(3) reproj(8) dF_sun(8)
-  float* g = ctx->e2e_grads;
+  float* g = ctx->e2e_grads[slot];
   CU(cudaMemsetAsync(g, 0, (pk.off[5] + 40) * sizeof(float), s));
   float* g_grp[5];
   for (int k = 0; k < 5; ++k) g_grp[k] = g + pk.off[k];
@@ -739,8 +742,9 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   float* d_sun = nullptr;
   float* d_vsun = nullptr;
   int rc;
+  CU(cudaStreamWaitEvent(s, ev[0], 0));
   if (shadows) {
-    d_sun = sun_ctx->e2e_out;
+    d_sun = sun_ctx->e2e_out[0];
     d_vsun = d_sun + (size_t)sun_ctx->max_w * sun_ctx->max_h;
     if ((rc = satsplat_preprocess(sun_ctx, &sun_cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
     if ((rc = satsplat_shadow_map(sun_ctx, d_sun, stream))) return rc;
@@ -751,13 +755,12 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
   }
   if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
   if ((rc = satsplat_render_forward(ctx, &sh, d_out[0], d_out[1], d_out[2], stream))) return rc;
-  CU(cudaEventRecord(ev_fwd, s));
+  CU(cudaEventRecord(ev[2], s));
   float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};
-  CU(cudaStreamWaitEvent(s_down, ev_fwd, 0));
+  CU(cudaStreamWaitEvent(s_down, ev[2], 0));
   for (int k = 0; k < 3; ++k)
     if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s_down));
-  CU(cudaEventRecord(ev_img, s_down));
-  CU(cudaStreamWaitEvent(s, ev_up, 0));
+  CU(cudaStreamWaitEvent(s, ev[1], 0));
   if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_grp[0], g_grp[1], g_grp[2], g_grp[3], g_grp[4], g_dF,
                                      g_cc, g_amb, d_vsun, shadows ? g_rep : nullptr, stream)))
     return rc;
@@ -766,16 +769,40 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
     // cascade: the gradients of the sun camera and of the reprojection constants flow back into dF (Eq. 16 adjoint)
     if ((rc = satsplat_sun_camera_backward(cam, sun->azimuth, sun->elevation, sun->viewport, g_dFs, g_rep, g_dF, stream))) return rc;
   }
+  CU(cudaEventRecord(ev[3], s));
   // h_grads stays packed (means 3N, quats 4N, scales 2N, logits N, rgb 3N, dF 8, cc 12, ambient 3)
+  CU(cudaStreamWaitEvent(s_down, ev[3], 0));
   size_t ho = 0;
   for (int k = 0; k < 5; ++k) {
-    CU(cudaMemcpyAsync(h_grads + ho, g_grp[k], n * width[k] * sizeof(float), cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(h_grads + ho, g_grp[k], n * width[k] * sizeof(float), cudaMemcpyDeviceToHost, s_down));
     ho += n * width[k];
   }
-  CU(cudaMemcpyAsync(h_grads + ho, g_dF, 23 * sizeof(float), cudaMemcpyDeviceToHost, s));
-  CU(cudaStreamSynchronize(s));
-  CU(cudaEventSynchronize(ev_img));
+  CU(cudaMemcpyAsync(h_grads + ho, g_dF, 23 * sizeof(float), cudaMemcpyDeviceToHost, s_down));
+  CU(cudaEventRecord(ev[4], s_down));
+  ctx->e2e_busy[slot] = 1;
   return SATSPLAT_OK;
+}
+
+int satsplat_iteration_host_end(satsplat_ctx* ctx, int32_t slot) {
+  if (!ctx || slot < 0 || slot > 1) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host_end: bad argument");
+  if (!ctx->e2e_busy[slot]) return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host_end: no begin on this slot");
+  CU(cudaSetDevice(ctx->device));
+  ctx->e2e_busy[slot] = 0;
+  CU(cudaEventSynchronize(ctx->e2e_ev[slot][4]));   // images and gradients are in the host buffers
+  CU(cudaEventSynchronize(ctx->e2e_ev[slot][3]));
+  return SATSPLAT_OK;
+}
+
+int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam,
+                            const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                            const float* h_means, const float* h_quats, const float* h_scales,
+                            const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                            const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                            float* h_grads, satsplat_stream stream) {
+  const int rc = satsplat_iteration_host_begin(ctx, sun_ctx, 0, cam, sun, shading, N, h_means, h_quats, h_scales, h_logits, h_rgb,
+                                               h_v_rgba, h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, stream);
+  if (rc) return rc;
+  return satsplat_iteration_host_end(ctx, 0);
 }
 
 }  // extern "C"

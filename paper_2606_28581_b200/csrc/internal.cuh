@@ -236,12 +236,14 @@ struct satsplat_ctx {
   const float *in_means, *in_quats, *in_scales, *in_logits;  // caller buffers of the last preprocess (chain backward)
   int preprocessed, forwarded, depth_only;
   // e2e staging buffers (lazily sized inside create)
-  float* e2e_in;          // means..rgb
-  float* e2e_up;          // upstream grads (3 images)
-  float* e2e_out;         // images
-  float* e2e_grads;       // N*13 + 23
-  cudaStream_t e2e_stream[2];   // upload of the upstream gradients / download of the images, beside the caller's stream
-  cudaEvent_t e2e_ev[4];
+  // host-buffer iteration (satsplat_iteration_host*): two staging slots so that the copies of consecutive steps overlap
+  float* e2e_in[2];       // means..rgb, sub-arrays at 16-byte aligned offsets
+  float* e2e_up[2];       // upstream gradients (3 images)
+  float* e2e_out[2];      // images (view ctx); slot 0 of a sun ctx: sun map + its gradient
+  float* e2e_grads[2];    // surfel gradient groups + dF cc ambient reproj dF_sun
+  cudaStream_t e2e_stream[2];   // uploads / downloads, beside the caller's stream
+  cudaEvent_t e2e_ev[2][5];     // per slot: surfels up, upstream up, forward done, backward done, everything down
+  int e2e_busy[2];              // slot has a begin without its end
   // profiling
   int profiling;
   cudaEvent_t ev[2 * SATSPLAT_NUM_STAGES];

@@ -423,6 +423,22 @@ def test_iteration_host_matches_device_path(P, G, orc, n):
     ref_dF = tot_dF.cpu().numpy()
     np.testing.assert_allclose(g[off:off + 8], ref_dF, rtol=2e-3, atol=2e-3 * np.abs(ref_dF).max())
     np.testing.assert_allclose(g[off + 8:off + 20], res["grads"]["v_cc"], rtol=2e-3, atol=2e-3 * np.abs(res["grads"]["v_cc"]).max())
+    # begin / end: two steps in flight on the two staging slots give what two serial calls give
+    h_out2 = [[torch.empty(view.height, view.width, 4).pin_memory() for _ in range(3)] for _ in range(2)]
+    h_g2 = [torch.empty(n * 13 + 23).pin_memory() for _ in range(2)]
+    P.iteration_host_begin(ctx, sctx, 0, *args[2:14], *h_out2[0], h_g2[0])
+    with pytest.raises(P.SatsplatError) as e:          # a slot cannot be begun twice
+        P.iteration_host_begin(ctx, sctx, 0, *args[2:14], *h_out2[0], h_g2[0])
+    assert e.value.code == P.E_STATE
+    P.iteration_host_begin(ctx, sctx, 1, *args[2:14], *h_out2[1], h_g2[1])
+    P.iteration_host_end(ctx, 0)
+    P.iteration_host_end(ctx, 1)
+    with pytest.raises(P.SatsplatError):
+        P.iteration_host_end(ctx, 1)
+    for k in range(2):
+        for a, b in zip(h_out2[k], h_out):
+            assert torch.equal(a, b)
+        np.testing.assert_allclose(h_g2[k].numpy(), g, rtol=1e-3, atol=1e-4 * max(1.0, np.abs(g).max()))
     ctx.close(); sctx.close()
 
 
