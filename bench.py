@@ -507,12 +507,18 @@ def stage_profile(job, views, peaks, fp32_peak_tinst):
     if job.sctx:
         snv, snc = job.sctx.debug_planes()
         pairs.update(sun_evaluated=int(snv.sum().item()), sun_contributing=int(snc.sum().item()), sun_K=job.sctx.sync_status())
+        # the sun-pass backward only has work on the texels some view pixel looked up (the others have no upstream gradient
+        # and are skipped exactly): its algorithmic work counts the pairs of those texels only
+        live = (job.v_sun != 0).to(snv.dtype)
+        pairs.update(sun_bwd_evaluated=int((snv * live).sum().item()), sun_bwd_contributing=int((snc * live).sum().item()),
+                     sun_live_texel_share=float(live.float().mean().item()))
     n = job.n
     tiles = ((job.W + 15) // 16) * ((job.H + 15) // 16)
     px = job.W * job.H
 
     def work(pass_):   # algorithmic bytes / lane-instructions (per surfel / key / pair figures of SURVEY.md 8(d))
         K, ev, co = pairs[f"{pass_}_K"], pairs[f"{pass_}_evaluated"], pairs[f"{pass_}_contributing"]
+        evb, cob = pairs.get(f"{pass_}_bwd_evaluated", ev), pairs.get(f"{pass_}_bwd_contributing", co)
         cf, cb = (INST_CONTRIB_FWD, INST_CONTRIB_BWD) if pass_ == "view" else (INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN)
         return {
             "preprocess": ("hbm", n * 137.0, None),
@@ -521,7 +527,7 @@ def stage_profile(job, views, peaks, fp32_peak_tinst):
             "sort": ("hbm", K * 20.0, None),
             "ranges": ("hbm", 0.0, None),
             "blend_fwd": ("alu", ev * INST_EVAL + co * cf, co * (INST_EVAL + cf)),
-            "blend_bwd": ("alu", ev * INST_EVAL + co * cb, co * (INST_EVAL + cb)),
+            "blend_bwd": ("alu", evb * INST_EVAL + cob * cb, cob * (INST_EVAL + cb)),
             "chain_bwd": ("hbm", n * (80.0 * 2 + 45.0 + 52.0 * 2), None),
         }
 

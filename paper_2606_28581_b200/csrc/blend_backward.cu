@@ -155,6 +155,9 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       // sun_depth = sum w (z - z_bg) + z_bg  (since sum w + T_f = 1): phi = v (z - z_bg), no T_f term
       vD = P.v_sun_in[o];
       zref = cam.z_bg();
+      // A texel no view pixel looked up has no upstream gradient (40-60 % of a sun map at C3): every gradient term of its
+      // pairs is exactly zero, so it takes no part in the walk (a block of such texels skips the walk altogether).
+      if (vD == 0.f) last = 0;
     }
   }
   if (!DEPTH_ONLY) {
@@ -219,6 +222,10 @@ __global__ void __launch_bounds__(kThreadsB, SATSPLAT_BWD_MINB) blend_backward_k
       }
       vT += -vA + va0 * cam.bg(0) + va1 * cam.bg(1) + va2 * cam.bg(2);   // A = 1 - T_f ; albedo = C + T_f bg
       vT -= vD * zref;                                                          // D = M1' + z_ref (1 - T_f)
+      // a pixel without any upstream gradient (masked out of the loss) contributes exact zeros: it skips the walk
+      if (vI0 == 0.f && vI1 == 0.f && vI2 == 0.f && vA == 0.f && vN0 == 0.f && vN1 == 0.f && vN2 == 0.f && vD == 0.f && vmed == 0.f &&
+          vL == 0.f)
+        last = 0;
     }
     // ---- reduce the 23 epilogue gradients over the warp (transposed butterfly); one RED per value into one of kRedCopies
     // copies of the 23-vector (spread by warp: no hot address, and no CTA barrier); add_small sums the copies ----

@@ -39,6 +39,9 @@ struct FwdParams {
 #ifndef SATSPLAT_FWD_MINB
 #define SATSPLAT_FWD_MINB 8
 #endif
+#ifndef SATSPLAT_FWD_BULK
+#define SATSPLAT_FWD_BULK 0   // 1: gather the records with one 64-byte cp.async.bulk each, completion on an mbarrier (measured trial)
+#endif
 constexpr int kWarpsF = SATSPLAT_FWD_WARPS;   // warps per CTA; a 16x16 tile is 8 warps (8x4 px each)
 constexpr int kThreadsF = 32 * kWarpsF;
 
@@ -53,6 +56,27 @@ __device__ __forceinline__ uint32_t warp_transpose_bits(uint32_t x, int lane) {
   }
   return x;
 }
+
+#if SATSPLAT_FWD_BULK
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}\n" ::"r"(smem_u32(b)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+               "r"(bytes), "r"(smem_u32(b))
+               : "memory");
+}
+#endif
 
 // Bit p (p = 8 * row + column) set iff pixel p of the 8x4 block whose first pixel centre is (wx0, wy0) lies inside the
 // bounding box bb = (x_min, x_max, y_min, y_max).
@@ -71,7 +95,13 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
   const ShRef<DEV> sh{P.sh, P.sh_dev};
   // per warp, double buffered: the records of a group's survivors as four float4 planes (lanes of a warp read
   // different entries at the same time)
+#if SATSPLAT_FWD_BULK
+  constexpr int kRecF = DEPTH_ONLY ? 3 : 4;
+  __shared__ __align__(64) float4 s_rec[2][kWarpsF][32][kRecF];   // records as they sit in HBM (one bulk copy each)
+  __shared__ __align__(8) uint64_t s_bar[2][kWarpsF];             // one mbarrier per warp and buffer
+#else
   __shared__ float4 s_r0[2][kWarpsF][32], s_r1[2][kWarpsF][32], s_r2[2][kWarpsF][32], s_r3[2][DEPTH_ONLY ? 1 : kWarpsF][32];
+#endif
 
   // CTA blockIdx.y holds warps [blockIdx.y * kWarpsF, +kWarpsF) of tile column blockIdx.x
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -103,6 +133,21 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
   auto fetch_bb = [&](uint32_t id) -> float4 { return id != kNoId ? P.bbox[id] : bb_none; };
   // lane l turns entry l's bounding box into the mask of block pixels it covers; survivors (non-empty masks) have
   // their records gathered into the warp's slots (slot = lane) of buffer `buf`
+#if SATSPLAT_FWD_BULK
+  if (lane == 0) { mbar_init(&s_bar[0][warp], 1); mbar_init(&s_bar[1][warp], 1); }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncwarp();
+  uint32_t bar_phase = 0u;   // bit b: parity the next wait on buffer b expects
+  auto gather = [&](uint32_t id, uint32_t cover, int buf) {
+    // the buffer was last read with ordinary loads: order them before the asynchronous-proxy writes
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const unsigned surv = __ballot_sync(0xffffffffu, cover != 0u);
+    if (lane == 0) mbar_expect_tx(&s_bar[buf][warp], (uint32_t)__popc(surv) * 16u * kRecF);
+    __syncwarp();
+    if (cover != 0u) bulk_g2s(&s_rec[buf][warp][lane][0], P.rec + 4 * (size_t)id, 16u * kRecF, &s_bar[buf][warp]);
+  };
+#else
   auto gather = [&](uint32_t id, uint32_t cover, int buf) {
     if (cover != 0u) {
       const float4* r = P.rec + 4 * (size_t)id;
@@ -113,12 +158,14 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
     }
     cp_async_commit();
   };
+#endif
   uint32_t id_a = fetch_id(0), id_b = fetch_id(1), id_c = fetch_id(2);   // groups c, c+1, c+2
   float4 bb_a = fetch_bb(id_a);
   float4 bb_b = fetch_bb(id_b);
   uint32_t cover = block_cover_mask(bb_a, wx0, wy0);
   gather(id_a, cover, 0);
-  for (int c = 0; c < ngroups; ++c) {
+  int c = 0;
+  for (; c < ngroups; ++c) {
     if (__all_sync(0xffffffffu, done)) break;   // this warp's 8x4 pixels are all finished
     // next group: boxes -> cover masks -> record gather in flight while this group is walked
     const uint32_t cover_n = block_cover_mask(bb_b, wx0, wy0);
@@ -128,15 +175,24 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
     // the 32x32 bit transpose hands every pixel the mask of entries whose box covers it
     uint32_t m = warp_transpose_bits(cover, lane);
     if (done) m = 0u;
-    cp_async_wait<1>();   // this group's records have landed
-    __syncwarp();
     const int buf = c & 1;
+#if SATSPLAT_FWD_BULK
+    mbar_wait(&s_bar[buf][warp], (bar_phase >> buf) & 1u);   // this group's records have landed
+    bar_phase ^= 1u << buf;
+#else
+    cp_async_wait<1>();   // this group's records have landed
+#endif
+    __syncwarp();
     const int rel0 = c * 32;
     // every pixel walks its own candidates, in list order
     while (m) {
       const int j = __ffs(m) - 1;
       m &= m - 1;
+#if SATSPLAT_FWD_BULK
+      const float4 r0 = s_rec[buf][warp][j][0], r1 = s_rec[buf][warp][j][1];
+#else
       const float4 r0 = s_r0[buf][warp][j], r1 = s_r1[buf][warp][j];
+#endif
       const PairEval E = pair_eval(r0, r1, px, py);                           // Eq. 9, Eq. 12
       if (!(E.rho <= kRhoCut)) continue;
       const float a = E.a;
@@ -144,12 +200,20 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
       const float Tn = T * (1.0f - a);
       if (Tn < kTMin) { done = true; visited = rel0 + j + 1; break; }
       const float w = a * T;
+#if SATSPLAT_FWD_BULK
+      const float4 r2 = s_rec[buf][warp][j][2];
+#else
       const float4 r2 = s_r2[buf][warp][j];
+#endif
       const float z = pair_depth(E, r1.w, r2.x, r2.y);                        // Eq. 6 depth at the intersection
       if (DEPTH_ONLY) {
         M1 += w * z;
       } else {
+#if SATSPLAT_FWD_BULK
+        const float4 r3 = s_rec[buf][warp][j][kRecF - 1];
+#else
         const float4 r3 = s_r3[buf][warp][j];
+#endif
         if (ncontrib == 0) zref = z;
         const float zs = z - zref;   // distortion accumulated in a per-pixel shifted depth frame (fp32 cancellation)
         if (T > 0.5f) { med = z; mi = rel0 + j; }
@@ -167,7 +231,13 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
     cover = cover_n;
     id_b = id_c; bb_b = bb_c; id_c = id_d;
   }
+#if SATSPLAT_FWD_BULK
+  // exactly one armed phase is left unconsumed (group c, whether the loop broke off or ran out): its copies may still
+  // be in flight and must land before the CTA can exit
+  mbar_wait(&s_bar[c & 1][warp], (bar_phase >> (c & 1)) & 1u);
+#else
   cp_async_wait<0>();
+#endif
   if (!inside) return;
   if (visited == 0) visited = (int)(end - start);
   const size_t o = (size_t)iy * P.cam.W + ix;
