@@ -20,6 +20,7 @@ import argparse
 import hashlib
 import json
 import os
+import re
 import socket
 import subprocess
 import sys
@@ -92,7 +93,8 @@ def record_traffic(raw_csv: str):
     for r in rows[2:]:
         name = r[col["Kernel Name"]]
         key = ("blend_bwd" if "blend_backward" in name else "blend_fwd" if "blend_forward" in name else name.split("(")[0].split("::")[-1])
-        key += "_sun" if ("<1>" in name or "(bool)1" in name) else ""
+        m = re.search(r"kernel<\s*(?:\(bool\))?\s*(\d|true|false)", name)     # first template argument: DEPTH_ONLY (the sun pass)
+        key += "_sun" if (m and m.group(1) in ("1", "true") and key.startswith("blend_")) else ""
         if key in out:
             continue
         f = lambda k: float(r[col[k]]) if k in col and r[col[k]] not in ("", "n/a") else None

@@ -61,14 +61,19 @@ __global__ void __launch_bounds__(kScanThreads) scan_block_sums_kernel(int N, co
 __global__ void __launch_bounds__(1024) scan_top_kernel(int nblocks, uint32_t* __restrict__ block_sums, Status* status,
                                                          uint32_t capacity) {
   __shared__ uint32_t s_warp[33];
+  __shared__ unsigned long long s_big[32];
   // one block; each thread owns a contiguous chunk
   const int per = (nblocks + 1023) / 1024;
   const int b0 = threadIdx.x * per;
   uint32_t sum = 0;
+  unsigned long long sum64 = 0;   // the grand total in 64 bits: a sum beyond 2^32 must be flagged, not wrapped
   for (int k = 0; k < per; ++k)
-    if (b0 + k < nblocks) sum += block_sums[b0 + k];
+    if (b0 + k < nblocks) { sum += block_sums[b0 + k]; sum64 += block_sums[b0 + k]; }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) sum64 += __shfl_xor_sync(0xffffffffu, sum64, d);
+  if ((threadIdx.x & 31) == 0) s_big[threadIdx.x >> 5] = sum64;
   uint32_t total;
-  uint32_t run = block_exclusive_scan(sum, s_warp, &total);
+  uint32_t run = block_exclusive_scan(sum, s_warp, &total);   // (contains the barriers that publish s_big)
   for (int k = 0; k < per; ++k)
     if (b0 + k < nblocks) {
       const uint32_t v = block_sums[b0 + k];
@@ -76,8 +81,10 @@ __global__ void __launch_bounds__(1024) scan_top_kernel(int nblocks, uint32_t* _
       run += v;
     }
   if (threadIdx.x == 0) {
-    status->K = total;
-    status->overflow = total > capacity ? 1u : 0u;
+    unsigned long long t64 = 0;
+    for (int w = 0; w < 32; ++w) t64 += s_big[w];
+    status->K = t64 > 0xffffffffull ? 0xffffffffu : (uint32_t)t64;
+    status->overflow = t64 > (unsigned long long)capacity ? 1u : 0u;
   }
 }
 
