@@ -58,6 +58,9 @@ def parse():
     ap.add_argument("--no-extras", action="store_true", help="skip the Adam / loss / init stage timings")
     ap.add_argument("--no-graphs", action="store_true", help="launch every kernel of a step from the host instead of replaying one CUDA graph per view")
     ap.add_argument("--no-allreduce", action="store_true", help="N > 1: leave the per-rank gradients un-reduced")
+    ap.add_argument("--dp-path", action="store_true",
+                    help="run the data-parallel code path (NCCL group, gradient all-reduce on the communication stream, host-launched "
+                         "steps) even with one rank: a functional check of that path on a single GPU, not a scaling number")
     ap.add_argument("--record-traffic", default=None, metavar="NCU_RAW_CSV",
                     help="write profiles/r2_traffic.json from `ncu -i <rep> --page raw --csv` output and exit")
     return ap.parse_args()
@@ -306,10 +309,11 @@ def run_reference(args):
 
 def workload_config(scene, args, world):
     v = scene.views[0]
-    par = (f"views sharded over {world} ranks; one NCCL all-reduce (sum) of the packed 13 N surfel gradients per step" if world > 1
-           else "1 rank")
+    par = (f"views sharded over {world} rank(s); one NCCL all-reduce (sum) of the packed 13 N surfel gradients per step"
+           if (world > 1 or getattr(args, "dp_path", False)) else "1 rank")
     return dict(workload=f"C{args.config} benchmark-shaped site (BASELINE.json configs[{args.config}])", surfels=scene.n,
-                view=f"{v.width}x{v.height}", cuda_graphs=("one graph for all views (device-resident cameras)" if (not getattr(args, "no_graphs", False)) and world == 1 else False),
+                view=f"{v.width}x{v.height}", cuda_graphs=("one graph for all views (device-resident cameras)"
+                             if (not getattr(args, "no_graphs", False)) and world == 1 and not getattr(args, "dp_path", False) else False),
                 sun_map=f"{v.sun_width}x{v.sun_height}" if v.shadows_on else None,
                 views=len(scene.views), shadows=bool(v.shadows_on), parallelism=par,
                 l2="per-step working set (records, keys, per-pixel state, images: >0.8 GB) exceeds the 126 MB L2; views cycle")
@@ -564,7 +568,10 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     device = torch.device("cuda", local)
-    if world > 1:
+    dp = world > 1 or args.dp_path     # the data-parallel path: NCCL group, one all-reduce per step
+    if dp:
+        if "MASTER_ADDR" not in os.environ:
+            os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(free_port()), RANK="0", WORLD_SIZE="1")
         dist.init_process_group("nccl", device_id=device)
     peaks = load_peaks()
     sampler = ClockSampler(local)
@@ -574,7 +581,7 @@ def run_ours(args):
     derived_tinst = mp["sm_count"] * SM_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
     fp32_peak = mp["fp32_lane_inst_per_s"] / 1e12
     scene = make_scene(args)
-    allreduce = world > 1 and not args.no_allreduce
+    allreduce = dp and not args.no_allreduce
     job = Job(P, torch, scene, device, n_grad_buffers=2 if allreduce else 1)
     nviews = len(scene.views)
     warm_views = views_for_rank(rank, world, nviews, args.warmup)
@@ -616,7 +623,7 @@ def run_ours(args):
     job.ctx.sync_status()     # raises on capacity overflow
     launches0 = P.kernel_launches()
     launches_per_step = None
-    use_graphs = not args.no_graphs and world == 1   # multi-rank runs launch from the host (no capture beside the NCCL watchdog)
+    use_graphs = not args.no_graphs and not dp   # data-parallel runs launch from the host (no capture beside the NCCL watchdog)
     if use_graphs:
         # ONE CUDA graph for all views and all steps: the cameras are device-resident (row f2), the graph advances the view
         # index itself; a step is one graph launch
@@ -746,7 +753,7 @@ def run_ours(args):
         line["cpu_baseline"] = cpu_baseline_block(scene, step_views[0], px, nviews)
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
+    if dp:
         dist.destroy_process_group()
 
 
