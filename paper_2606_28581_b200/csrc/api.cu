@@ -388,14 +388,12 @@ int backward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev
   {
     StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
     CU(launch_blend_backward(ctx, sh, sh_dev, v_rgba, v_geom, v_aux, nullptr, false, v_cc, v_ambient, v_sun_depth, v_reproj, s));
-    if (v_cc) CU(launch_add_small(v_cc, ctx->red_buf, 12, s));
-    if (v_ambient) CU(launch_add_small(v_ambient, ctx->red_buf + 12, 3, s));
-    if (v_reproj) CU(launch_add_small(v_reproj, ctx->red_buf + 15, 8, s));
   }
   {
     StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
+    const bool epi = v_cc || v_ambient || v_reproj;   // their partial sums sit in red_buf; the chain kernel's first CTA delivers them
     CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
-                             v_opacity_logits, v_rgb, v_dF, s));
+                             v_opacity_logits, v_rgb, v_dF, epi ? ctx->red_buf : nullptr, v_cc, v_ambient, v_reproj, s));
   }
   return SATSPLAT_OK;
 }
@@ -496,7 +494,7 @@ int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, fl
   {
     StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
     CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
-                             v_opacity_logits, nullptr, v_dF_sun, s));
+                             v_opacity_logits, nullptr, v_dF_sun, nullptr, nullptr, nullptr, nullptr, s));
   }
   return SATSPLAT_OK;
 }

@@ -21,8 +21,21 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera camv, con
                                                              const uint8_t* __restrict__ flags, float4* __restrict__ vrec,
                                                              float* __restrict__ v_means, float* __restrict__ v_quats,
                                                              float* __restrict__ v_scales, float* __restrict__ v_logits,
-                                                             float* __restrict__ v_rgb, float* __restrict__ v_dF) {
+                                                             float* __restrict__ v_rgb, float* __restrict__ v_dF,
+                                                             const float* __restrict__ epi, float* __restrict__ v_cc,
+                                                             float* __restrict__ v_ambient, float* __restrict__ v_reproj) {
   __shared__ float s_red[8][8];
+  // the 23 epilogue gradients of the blend backward (kRedCopies partial copies in `epi`) are summed into the caller's
+  // v_cc / v_ambient / v_reproj by the first CTA: no launch of their own
+  if (epi && blockIdx.x == 0 && threadIdx.x < 23) {
+    const int k = threadIdx.x;
+    float* dst = k < 12 ? (v_cc ? v_cc + k : nullptr) : (k < 15 ? (v_ambient ? v_ambient + (k - 12) : nullptr) : (v_reproj ? v_reproj + (k - 15) : nullptr));
+    if (dst) {
+      float a = 0.f;
+      for (int c = 0; c < kRedCopies; ++c) a += epi[c * 32 + k];
+      *dst += a;
+    }
+  }
   // The CTA's 256 surfels are contiguous in every array: the 80-B moment records and the 12-B rows (means, v_means,
   // v_rgb) are moved between HBM and shared memory as coalesced float4 streams, and every load of the kernel is
   // issued before the first use (one DRAM round trip).
@@ -196,16 +209,24 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera camv, con
 
 cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
                                   const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
-                                  float* v_rgb, float* v_dF, cudaStream_t s) {
-  if (c->N == 0) return cudaSuccess;
+                                  float* v_rgb, float* v_dF, const float* epi, float* v_cc, float* v_ambient, float* v_reproj,
+                                  cudaStream_t s) {
+  if (c->N == 0) {   // no surfel: only the epilogue sums are left to deliver (background pixels still feed the colour correction)
+    if (epi && v_cc) launch_add_small(v_cc, epi, 12, s);
+    if (epi && v_ambient) launch_add_small(v_ambient, epi + 12, 3, s);
+    if (epi && v_reproj) launch_add_small(v_reproj, epi + 15, 8, s);
+    return cudaGetLastError();
+  }
   ++g_kernel_launches;
   const int grid = (int)((c->N + 255) / 256);
   if (c->cam_dev)
     chain_backward_kernel<true><<<grid, 256, 0, s>>>(c->cam, c->cam_dev, (int)c->N, means, quats, scales, logits, c->count, c->flags,
-                                                     reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF);
+                                                     reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF, epi, v_cc, v_ambient,
+                                                     v_reproj);
   else
     chain_backward_kernel<false><<<grid, 256, 0, s>>>(c->cam, nullptr, (int)c->N, means, quats, scales, logits, c->count, c->flags,
-                                                      reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF);
+                                                      reinterpret_cast<float4*>(c->vrec), v_means, v_quats, v_scales, v_logits, v_rgb, v_dF, epi, v_cc, v_ambient,
+                                                     v_reproj);
   return cudaGetLastError();
 }
 

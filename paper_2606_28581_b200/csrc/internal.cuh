@@ -280,7 +280,8 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
                                   float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s);
 cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
                                   const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
-                                  float* v_rgb, float* v_dF, cudaStream_t s);
+                                  float* v_rgb, float* v_dF, const float* epi, float* v_cc, float* v_ambient, float* v_reproj,
+                                  cudaStream_t s);
 cudaError_t launch_add_small(float* dst, const float* src, int n, cudaStream_t s);
 struct LossHost {   // arguments of the loss stage (losses.cu)
   int W, H;
