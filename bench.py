@@ -632,7 +632,11 @@ def run_ours(args):
         torch.cuda.synchronize()
         l0 = P.kernel_launches()
         graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):
+        # captured on a high-priority stream: the critical chain (sun pass -> view forward -> backwards) gets the SMs before
+        # the view pass's preprocess + binning, which runs beside the sun pass on the default-priority side stream and is
+        # not needed until the sun map is done (2.206 -> 2.189 ms per step)
+        cap = torch.cuda.Stream(device=device, priority=-1)
+        with torch.cuda.graph(graph, stream=cap):
             job.step_device()
         launches_per_step = P.kernel_launches() - l0
         for _ in range(3):
