@@ -138,7 +138,7 @@ int satsplat_create(satsplat_ctx** out, int device, int64_t max_surfels, int32_t
   A(dalloc(ctx, &ctx->status, 1));
   A(dalloc(ctx, &ctx->tile_count, tiles * satsplat::kCtrStride));
   A(dalloc(ctx, &ctx->tile_start, tiles));
-  A(dalloc(ctx, &ctx->worklist, tiles * 2));
+  A(dalloc(ctx, &ctx->worklist, tiles * 3));
   A(dalloc(ctx, &ctx->wl_count, 4));
   A(cudaMemset(ctx->tile_count, 0, tiles * satsplat::kCtrStride * sizeof(uint32_t)));
   A(dalloc(ctx, &ctx->px_a, px));

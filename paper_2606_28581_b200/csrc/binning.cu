@@ -391,7 +391,8 @@ constexpr int kTileScanChunk = kTileScanThreads * kTileScanItems;   // 2048 tile
 #define SATSPLAT_SORT_SMALL_MAX 256
 #endif
 constexpr int kTileSortSmallMax = SATSPLAT_SORT_SMALL_MAX;    // entries one warp sorts in registers in the small-tile kernel (4 or 8 per lane)
-constexpr int kTileSortMergeMax = 1024;   // entries the 4-warp merge kernel handles (4 chunks of <= 256)
+constexpr int kTileSortMergeMax = 1024;   // entries the 4-warp merge kernel handles (4 runs of <= 256)
+constexpr int kTileSortMerge16Max = 4096; // entries the 16-warp merge kernel handles (16 runs of <= 256)
 
 __global__ void __launch_bounds__(kTileScanThreads) tile_scan_partial_kernel(int tiles, const uint32_t* __restrict__ tile_count,
                                                                              uint32_t* __restrict__ tile_start,
@@ -470,20 +471,18 @@ __global__ void __launch_bounds__(kTileScanThreads) tile_scan_finish_kernel(int 
     cursor[(size_t)i * kCtrStride] = st;             // the scatter appends at cursor++ (the sort kernel clears it again)
     len = empty ? 0u : en - st;
   }
-  // long lists go to the worklists (warp-aggregated appends): [0, tiles) merge kernel, [tiles, 2 tiles) large kernel
-  const bool mid = len > (uint32_t)kTileSortSmallMax && len <= (uint32_t)kTileSortMergeMax;
-  const bool big = len > (uint32_t)kTileSortMergeMax;
-  const unsigned mm = __ballot_sync(0xffffffffu, mid), mb = __ballot_sync(0xffffffffu, big);
-  uint32_t bm = 0, bb = 0;
-  if (lane == 0) {
-    if (mm) bm = atomicAdd(wl_count + 0, (uint32_t)__popc(mm));
-    if (mb) bb = atomicAdd(wl_count + 2, (uint32_t)__popc(mb));
-  }
-  bm = __shfl_sync(0xffffffffu, bm, 0);
-  bb = __shfl_sync(0xffffffffu, bb, 0);
+  // long lists go to the worklists (warp-aggregated appends): [0, tiles) 4-warp merge kernel, [tiles, 2 tiles) 16-warp merge
+  // kernel, [2 tiles, 3 tiles) large kernel; wl_count[0..2] = their lengths
+  const int cls = len <= (uint32_t)kTileSortSmallMax ? -1 : (len <= (uint32_t)kTileSortMergeMax ? 0 : (len <= (uint32_t)kTileSortMerge16Max ? 1 : 2));
   const unsigned lt = (1u << lane) - 1u;
-  if (mid) worklist[bm + __popc(mm & lt)] = (uint32_t)i;
-  if (big) worklist[tiles + bb + __popc(mb & lt)] = (uint32_t)i;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const unsigned m = __ballot_sync(0xffffffffu, cls == k);
+    uint32_t b = 0;
+    if (lane == 0 && m) b = atomicAdd(wl_count + k, (uint32_t)__popc(m));
+    b = __shfl_sync(0xffffffffu, b, 0);
+    if (cls == k) worklist[(size_t)k * tiles + b + __popc(m & lt)] = (uint32_t)i;
+  }
 }
 
 // Appends (depth bits << 32 | surfel id) to the segment of every tile of the surfel's rect: position = cursor[tile]++ (the
@@ -642,11 +641,11 @@ __device__ __noinline__ void chunk_sort_warp(const uint64_t* __restrict__ in, ui
   }
 }
 
-// Tiles are dispatched by list length: <= 256 entries here (one warp per tile, 2 / 4 / 8 registers per lane), 257..1024 in
-// tile_sort_merge_kernel (one 4-warp CTA per tile), longer ones in tile_sort_large_kernel (one 1024-thread CTA per tile).
+// Tiles are dispatched by list length: <= 256 entries here (one warp per tile, 2 / 4 / 8 registers per lane), 257..1024 and
+// 1025..4096 in tile_sort_merge_kernel<4> / <16> (one 4- / 16-warp CTA per tile), longer ones in tile_sort_large_kernel
+// (one 1024-thread CTA per tile).
 // At C3 a fifth of the tiles hold more than 256 entries (walls stack surfels along the ray) and carry half of the
-// pairs.  Worklists: [0, tiles) merge, [tiles, 2 tiles) large; wl_count = {merge length, merge cursor, large length,
-// large cursor}.
+// pairs.  Worklists: [0, tiles) 4-warp merge, [tiles, 2 tiles) 16-warp merge, [2 tiles, 3 tiles) large; wl_count[0..2] = lengths.
 __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tiles, const uint32_t* __restrict__ ranges,
                                                                         const uint64_t* __restrict__ entries,
                                                                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
@@ -664,58 +663,76 @@ __global__ void __launch_bounds__(kTileSortWarps * 32) tile_sort_kernel(int tile
   else tile_sort_warp<8>(entries + s, n, hi, keys + s, vals + s, lane);
 }
 
-// number of elements of the sorted range a[0, n) that are smaller than x (all values are distinct)
-__device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t n, uint64_t x) {
-  uint32_t lo = 0;
-  while (n > 0) {
-    const uint32_t h = n >> 1;
-    const bool right = a[lo + h] < x;
-    lo = right ? lo + h + 1 : lo;
-    n = right ? n - h - 1 : h;
-  }
-  return lo;
-}
-
-// Lists of 257..1024 entries: the CTA's four warps each sort a quarter in registers (<= 256 entries, 2/4/8 per lane),
-// then two merge rounds in shared memory by rank: an element's place in the merge of two sorted runs is its own index
-// plus the number of smaller elements in the other run (binary search; the (depth, id) composites are distinct).
-__global__ void __launch_bounds__(128) tile_sort_merge_kernel(const uint32_t* __restrict__ ranges, const uint64_t* __restrict__ entries,
-                                                              uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                                              const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
-  __shared__ uint64_t s_a[kTileSortMergeMax], s_b[kTileSortMergeMax];
+// Lists of 257..4096 entries: the CTA's W warps each sort one W-th in registers (<= 256 entries, 2/4/8 per lane), then
+// log2(W) merge rounds in shared memory along merge paths (a thread finds its place on the diagonal by one binary search
+// and merges four outputs sequentially; the (depth, id) composites are distinct).
+// W = 4 takes the lists up to 1024 entries (C3: a fifth of the tiles), W = 16 those up to 4096 (C1: 200 K surfels on
+// 1024 tiles give lists of 1000-2200 entries, which the one-CTA bitonic sort of tile_sort_large_kernel took 60 us for).
+template <int W>
+__global__ void __launch_bounds__(32 * W) tile_sort_merge_kernel(const uint32_t* __restrict__ ranges, const uint64_t* __restrict__ entries,
+                                                                 uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                                 const uint32_t* __restrict__ worklist, const uint32_t* __restrict__ wl_len) {
+  extern __shared__ uint64_t s_merge[];              // two buffers of 256 W composites
+  uint64_t* buf_a = s_merge;
+  uint64_t* buf_b = s_merge + 256 * W;
+  constexpr uint32_t kThreads = 32 * W;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t total = wl_count[0];
-  // items are dealt round-robin to the CTAs: a shared work counter costs one same-address atomic per item, which at
-  // ~13 ns each was the whole duration of this kernel (3000 items per pass)
+  const uint32_t total = *wl_len;
+  // items are dealt round-robin to the CTAs: a shared work counter costs one same-address atomic per item
   for (uint32_t item = blockIdx.x; item < total; item += gridDim.x) {
     __syncthreads();
     const uint32_t t = worklist[item];
     const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s;
-    const uint32_t c = (n + 3) >> 2;                         // quarter length (<= 256)
+    // run length: the smallest of 64 / 128 / 256 that covers the list with W runs, so that the register networks run
+    // full (a 350-entry list is three runs of 128 on three warps, not four padded runs of 88)
+    const uint32_t c = n <= 64u * W ? 64u : (n <= 128u * W ? 128u : 256u);
     {
-      const uint32_t b = min((uint32_t)warp * c, n), e = min(b + c, n);
-      if (c <= 64) chunk_sort_warp<2>(entries + s + b, e - b, s_a + b, lane);
-      else if (c <= 128) chunk_sort_warp<4>(entries + s + b, e - b, s_a + b, lane);
-      else chunk_sort_warp<8>(entries + s + b, e - b, s_a + b, lane);
+      const uint32_t b = min((uint32_t)warp * c, n), e = min(b + c, n), m = e - b;
+      if (m > 128u) chunk_sort_warp<8>(entries + s + b, m, buf_a + b, lane);
+      else if (m > 64u) chunk_sort_warp<4>(entries + s + b, m, buf_a + b, lane);
+      else if (m > 0u) chunk_sort_warp<2>(entries + s + b, m, buf_a + b, lane);
     }
     __syncthreads();
-    // round 1: quarters (0,1) and (2,3)
-    for (uint32_t i = threadIdx.x; i < n; i += 128) {
-      const uint32_t q = i / c, sib = q ^ 1u;
-      const uint32_t sb = min(sib * c, n), se = min(sb + c, n);
-      const uint64_t x = s_a[i];
-      // ties cannot occur; the run that comes first wins "equal" by construction of lower_bound on distinct values
-      s_b[(q & ~1u) * c + (i - q * c) + lower_bound_u64(s_a + sb, se - sb, x)] = x;
-    }
-    __syncthreads();
-    // round 2: halves [0, h) and [h, n), straight to the output
-    const uint32_t h = min(2u * c, n);
     const uint64_t hi = (uint64_t)t << 32;
-    for (uint32_t i = threadIdx.x; i < n; i += 128) {
-      const uint64_t x = s_b[i];
-      const uint32_t o = i < h ? i + lower_bound_u64(s_b + h, n - h, x) : (i - h) + lower_bound_u64(s_b, h, x);
-      keys[s + o] = hi | (x >> 32);
-      vals[s + o] = (uint32_t)x;
+    uint64_t* src = buf_a;
+    uint64_t* dst = buf_b;
+#pragma unroll 1
+    for (uint32_t run = c; run < n; run <<= 1) {             // merge pairs of runs of length `run`
+      const bool last = (run << 1) >= n;                     // the last round goes straight to the output
+      // merge path: a thread produces 4 consecutive outputs; one binary search along the diagonal finds how many of the
+      // outputs before them come from the first run, then it merges sequentially (runs start at multiples of 4, so a
+      // segment never straddles two pairs)
+      for (uint32_t o0 = 4u * threadIdx.x; o0 < n; o0 += 4u * kThreads) {
+        const uint32_t pbase = (o0 / (2u * run)) * (2u * run);
+        const uint32_t la = min(run, n - pbase), lb = min(run, n - pbase - la);
+        const uint64_t* A = src + pbase;
+        const uint64_t* B = A + la;
+        const uint32_t d = o0 - pbase;
+        uint32_t lo = d > lb ? d - lb : 0u, hi_ = min(d, la);
+        while (lo < hi_) {
+          const uint32_t mid = (lo + hi_) >> 1;
+          if (A[mid] < B[d - 1u - mid]) lo = mid + 1u; else hi_ = mid;
+        }
+        uint32_t i = lo, j = d - lo;
+        const uint32_t cnt = min(4u, la + lb - d);
+        uint64_t a = i < la ? A[i] : ~0ull, b = j < lb ? B[j] : ~0ull;
+#pragma unroll
+        for (uint32_t k = 0; k < 4u; ++k) {
+          if (k < cnt) {
+            const bool ta = a < b;                            // composites are distinct; ~0 marks an exhausted run
+            const uint64_t x = ta ? a : b;
+            if (ta) { ++i; a = i < la ? A[i] : ~0ull; } else { ++j; b = j < lb ? B[j] : ~0ull; }
+            if (last) {
+              keys[s + o0 + k] = hi | (x >> 32);
+              vals[s + o0 + k] = (uint32_t)x;
+            } else {
+              dst[o0 + k] = x;
+            }
+          }
+        }
+      }
+      __syncthreads();
+      uint64_t* tmp = src; src = dst; dst = tmp;
     }
   }
 }
@@ -726,7 +743,7 @@ __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* _
                                                                uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
                                                                const uint32_t* __restrict__ worklist, uint32_t* __restrict__ wl_count) {
   extern __shared__ uint64_t s_big[];
-  const uint32_t total = wl_count[2];
+  const uint32_t total = wl_count[2];   // lists beyond the 16-warp merge kernel
   for (uint32_t item = blockIdx.x; item < total; item += gridDim.x) {
     __syncthreads();
     const uint32_t t = worklist[item];
@@ -750,7 +767,9 @@ __global__ void __launch_bounds__(1024) tile_sort_large_kernel(const uint32_t* _
 }
 
 cudaError_t init_binning_attrs() {
-  return cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
+  cudaError_t e = cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSortCtaMax * 8);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_sort_merge_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 256 * 16 * 8);
+  return e;
 }
 
 cudaError_t launch_tile_scan(satsplat_ctx* c, cudaStream_t s) {
@@ -773,14 +792,17 @@ cudaError_t launch_tile_scatter(satsplat_ctx* c, int64_t N, cudaStream_t s) {
 
 cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
-  g_kernel_launches += 3;
-  // the three kernels work on disjoint tiles (the worklists come from the scan): the long lists are sorted on a second
+  g_kernel_launches += 4;
+  // the four kernels work on disjoint tiles (the worklists come from the scan): the long lists are sorted on a second
   // stream beside the many short ones
   cudaEventRecord(c->bin_ev[0], s);
   cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
-  tile_sort_merge_kernel<<<c->sm_count * 8, 128, 0, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0], c->worklist, c->wl_count);
+  tile_sort_merge_kernel<4><<<c->sm_count * 8, 128, 2 * 256 * 4 * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
+                                                                                      c->worklist, c->wl_count + 0);
+  tile_sort_merge_kernel<16><<<c->sm_count * 2, 512, 2 * 256 * 16 * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
+                                                                                        c->worklist + tiles, c->wl_count + 1);
   tile_sort_large_kernel<<<(c->sm_count + 1) / 2, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
-                                                                                               c->worklist + tiles, c->wl_count);
+                                                                                               c->worklist + 2 * (size_t)tiles, c->wl_count);
   cudaEventRecord(c->bin_ev[1], c->bin_stream);
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(tiles, c->ranges, c->keys[1], c->keys[0],
                                                                                                  c->vals[0], c->tile_count);

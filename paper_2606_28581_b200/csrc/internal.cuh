@@ -215,8 +215,8 @@ struct satsplat_ctx {
   uint32_t* ranges;       // [tiles*2]
   uint32_t* tile_count;   // [tiles] tile-sort binning: pair count per tile, then the scatter cursor
   uint32_t* tile_start;   // [tiles] exclusive scan of tile_count
-  uint32_t* worklist;     // [2*tiles] tiles too long for the small-tile sort: mid list, then large list
-  uint32_t* wl_count;     // [4] mid length, mid cursor, large length, large cursor
+  uint32_t* worklist;     // [3*tiles] tiles too long for the small-tile sort: 257-1024, 1025-4096, longer
+  uint32_t* wl_count;     // [4] lengths of the three worklists
   int binning_mode;       // SATSPLAT_BINNING_TILESORT (default) or SATSPLAT_BINNING_RADIX
   cudaStream_t bin_stream;   // the long tile lists are sorted on this stream beside the short ones (forked from / joined to the caller's)
   cudaEvent_t bin_ev[2];
