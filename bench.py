@@ -370,6 +370,7 @@ class Job:
         # the view pass's preprocess + binning do not depend on the sun pass: they run on a second stream beside it
         self.side = torch.cuda.Stream(device=device) if self.shadows else None
         self.overlap = True     # False: everything on one stream (the per-stage timers then see each kernel alone)
+        self.split = False      # True while step_device runs: contexts in SATSPLAT_OPT_SPLIT_BACKWARD mode
 
     def prepare_view(self, vi):
         if vi in self.cams:
@@ -406,6 +407,10 @@ class Job:
         return sh
 
     def step(self, vi, buf=0):
+        if self.split:          # the host-struct step uses the unsplit backward calls
+            self.ctx.set_option(self.P.OPT_SPLIT_BACKWARD, 0)
+            self.sctx.set_option(self.P.OPT_SPLIT_BACKWARD, 0)
+            self.split = False
         g = self.gbufs[buf]
         g["flat"].zero_()
         sh = self.forward(vi)
@@ -426,6 +431,10 @@ class Job:
         selected by the device index, nothing of it is baked into kernel arguments, so ONE captured graph of this function
         serves all views and all optimiser steps (dF lives in self.dF_all on the device)."""
         P, g, surf = self.P, self.gbufs[buf], (self.means, self.quats, self.scales, self.logits, self.rgb)
+        if self.shadows and not self.split:
+            self.ctx.set_option(P.OPT_SPLIT_BACKWARD, 1)
+            self.sctx.set_option(P.OPT_SPLIT_BACKWARD, 1)
+            self.split = True
         g["flat"].zero_()
         P.camera_chain(self.table, self.dF_all, self.idx, self.block)
         v = self.scene.views[0]
@@ -441,10 +450,20 @@ class Job:
             self.ctx.preprocess_device(self.W, self.H, self.block, P.CAM_VIEW, *surf)
         self.ctx.render_forward_device(self.block, self.sun_depth, *self.out)
         up = self.up_shared
-        self.ctx.render_backward_device(self.block, self.sun_depth, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"],
-                                        g["cc"], g["amb"], self.v_sun, g["rep"] if self.shadows else None)
         if self.shadows:
-            self.sctx.shadow_map_backward(self.v_sun, g["m"], g["q"], g["s"], g["l"], g["dFs"])
+            # split backward calls: the view pass's per-surfel chain (HBM-bound) runs on the side stream beside the sun pass's
+            # blend backward (issue-bound); the sun pass's chain follows both (the two chains share the gradient buffers)
+            cur = self.torch.cuda.current_stream()
+            self.ctx.render_backward_device(self.block, self.sun_depth, up[0], up[1], up[2], None, None, None, None, None,
+                                            v_sun_depth=self.v_sun)
+            self.side.wait_stream(cur)
+            self.ctx.backward_chain(g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"], g["cc"], g["amb"], g["rep"], stream=self.side)
+            self.sctx.shadow_map_backward(self.v_sun, None, None, None, None)
+            cur.wait_stream(self.side)
+            self.sctx.backward_chain(g["m"], g["q"], g["s"], g["l"], None, g["dFs"])
+        else:
+            self.ctx.render_backward_device(self.block, None, up[0], up[1], up[2], g["m"], g["q"], g["s"], g["l"], g["c"], g["dF"],
+                                            g["cc"], g["amb"], None, None)
         # cascade (Fig. 1): view-pass dF gradient + adjoint of the sun camera / reprojection -> this view's row of v_dF_all
         P.camera_chain_backward(self.table, self.dF_all, self.idx, g["dF"], g["dFs"] if self.shadows else None,
                                 g["rep"] if self.shadows else None, None, self.v_dF_all)
@@ -715,6 +734,10 @@ def run_ours(args):
         sh = P.Shading.make(cc=v.cc, ambient=v.ambient, depth_bias=v.depth_bias, slope=v.slope)
         sh.shadows_on = 1 if job.shadows else 0
         P.reserve_host_staging(job.ctx, job.sctx)
+        if job.split:            # the host-buffer entry point runs the unsplit backward calls
+            job.ctx.set_option(P.OPT_SPLIT_BACKWARD, 0)
+            job.sctx.set_option(P.OPT_SPLIT_BACKWARD, 0)
+            job.split = False
 
         hargs = (cam, sun, sh, scene.n, *h_in, *h_up, *h_out, h_g)
 

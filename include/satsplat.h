@@ -354,6 +354,15 @@ int satsplat_debug_bins(satsplat_ctx* ctx, int64_t* K, const uint64_t** keys, co
                         const uint32_t** tile_ranges, const uint16_t** rects, const uint32_t** counts,
                         satsplat_stream stream);
 
+/* Second half of a backward call made with SATSPLAT_OPT_SPLIT_BACKWARD = 1 on `ctx`: turns the moment records the blend half
+ * left into surfel gradients (accumulated into v_means ... v_rgb, DEVICE, any may be NULL; v_rgb is ignored for a
+ * depth-only context), reduces v_dF and delivers v_cc / v_ambient / v_reproj.  Must run after the blend half (stream
+ * order or an event) and before the next backward on `ctx`; two chains that accumulate into the same gradient buffers must
+ * be ordered by the caller.  SATSPLAT_E_STATE if no split backward is pending. */
+int satsplat_backward_chain(satsplat_ctx* ctx, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
+                            float* v_dF /*[8]*/, float* v_cc /*[12]*/, float* v_ambient /*[3]*/, float* v_reproj /*[8]*/,
+                            satsplat_stream stream);
+
 /* Copies the per-surfel records of the last preprocess into records_out (DEVICE [N,16] fp32) in the canonical
  * order (c_x, c_y, Q00, Q01, Q10, Q11, z_c, g0, g1, alpha, r, g, b, n_x, n_y, n_z) and flags_out (DEVICE [N] uint8:
  * bit0 culled, bit1 degenerate, bit2 normal flipped). */
@@ -387,6 +396,12 @@ int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out);
  *       SATSPLAT_BINNING_RADIX              per-surfel scan -> key duplication -> stable 8-bit LSD radix sort of the
  *                                           64-bit keys -> range detection; the general-purpose device sort */
 #define SATSPLAT_OPT_BINNING 0
+/*   SATSPLAT_OPT_SPLIT_BACKWARD (0 default / 1): with 1, satsplat_render_backward, satsplat_render_backward_device and
+ *     satsplat_shadow_map_backward stop after their blend half (epilogue backward + reverse compositing: per-surfel moment
+ *     records, v_sun_depth and the epilogue sums stay in the context; their v_means ... v_reproj arguments are ignored and
+ *     may be NULL) and satsplat_backward_chain runs the per-surfel chain.  For callers that overlap the chain of one pass
+ *     (HBM-bound) with the blend backward of the next pass (issue-bound) on two streams. */
+#define SATSPLAT_OPT_SPLIT_BACKWARD 1
 #define SATSPLAT_BINNING_TILESORT 0
 #define SATSPLAT_BINNING_RADIX 1
 int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value);

@@ -17,6 +17,7 @@ _LIB = None
 
 OK, E_INVALID, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4
 OPT_BINNING, BINNING_TILESORT, BINNING_RADIX = 0, 0, 1
+OPT_SPLIT_BACKWARD = 1
 STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_fwd", "blend_bwd", "chain_bwd")
 
 
@@ -166,6 +167,7 @@ def lib():
         L.satsplat_preprocess_device.argtypes = [vp, i32, i32, vp, i32, i64, vp, vp, vp, vp, vp, vp]
         L.satsplat_render_forward_device.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.satsplat_render_backward_device.argtypes = [vp, vp, vp, i32, i32] + [vp] * 14
+        L.satsplat_backward_chain.argtypes = [vp] * 11
         L.satsplat_measure_peaks.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
         _LIB = L
     return _LIB
@@ -413,6 +415,12 @@ class Context:
         self._rc(lib().satsplat_render_backward(self._h, C.byref(shading), _ptr(v_rgba), _ptr(v_geom), _ptr(v_aux), _ptr(v_means),
                                                 _ptr(v_quats), _ptr(v_scales), _ptr(v_opacity_logits), _ptr(v_rgb), _ptr(v_dF),
                                                 _ptr(v_cc), _ptr(v_ambient), _ptr(v_sun_depth), _ptr(v_reproj), _stream(stream)))
+
+    def backward_chain(self, v_means, v_quats, v_scales, v_opacity_logits, v_rgb=None, v_dF=None, v_cc=None, v_ambient=None,
+                       v_reproj=None, stream=None):
+        """satsplat_backward_chain: second half of a backward call made with OPT_SPLIT_BACKWARD = 1."""
+        self._rc(lib().satsplat_backward_chain(self._h, _ptr(v_means), _ptr(v_quats), _ptr(v_scales), _ptr(v_opacity_logits), _ptr(v_rgb),
+                                               _ptr(v_dF), _ptr(v_cc), _ptr(v_ambient), _ptr(v_reproj), _stream(stream)))
 
     def shadow_map_backward(self, v_sun_depth, v_means, v_quats, v_scales, v_opacity_logits, v_dF_sun=None, stream=None):
         self._rc(lib().satsplat_shadow_map_backward(self._h, _ptr(v_sun_depth), _ptr(v_means), _ptr(v_quats), _ptr(v_scales),

@@ -385,13 +385,19 @@ int backward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev
                     const float* v_aux, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
                     float* v_dF, float* v_cc, float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s) {
   clear_stage_marks(ctx, {6, 7});
+  // the 23 epilogue sums (cc, ambient, reproj) are left in red_buf by the blend; the chain kernel's first CTA delivers them
+  const bool epi = ctx->split_backward || v_cc || v_ambient || v_reproj;
   {
     StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
-    CU(launch_blend_backward(ctx, sh, sh_dev, v_rgba, v_geom, v_aux, nullptr, false, v_cc, v_ambient, v_sun_depth, v_reproj, s));
+    CU(launch_blend_backward(ctx, sh, sh_dev, v_rgba, v_geom, v_aux, nullptr, false, epi, v_sun_depth, s));
+  }
+  if (ctx->split_backward) {   // SATSPLAT_OPT_SPLIT_BACKWARD: satsplat_backward_chain finishes the call
+    ctx->chain_pending = 1;
+    ctx->chain_epi = 1;
+    return SATSPLAT_OK;
   }
   {
     StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
-    const bool epi = v_cc || v_ambient || v_reproj;   // their partial sums sit in red_buf; the chain kernel's first CTA delivers them
     CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
                              v_opacity_logits, v_rgb, v_dF, epi ? ctx->red_buf : nullptr, v_cc, v_ambient, v_reproj, s));
   }
@@ -489,12 +495,33 @@ int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, fl
   clear_stage_marks(ctx, {6, 7});
   {
     StageTimer t(ctx, SATSPLAT_STAGE_BLEND_BWD, s);
-    CU(launch_blend_backward(ctx, sh, nullptr, nullptr, nullptr, nullptr, v_sun_depth, true, nullptr, nullptr, nullptr, nullptr, s));
+    CU(launch_blend_backward(ctx, sh, nullptr, nullptr, nullptr, nullptr, v_sun_depth, true, false, nullptr, s));
+  }
+  if (ctx->split_backward) {
+    ctx->chain_pending = 1;
+    ctx->chain_epi = 0;
+    return SATSPLAT_OK;
   }
   {
     StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
     CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
                              v_opacity_logits, nullptr, v_dF_sun, nullptr, nullptr, nullptr, nullptr, s));
+  }
+  return SATSPLAT_OK;
+}
+
+int satsplat_backward_chain(satsplat_ctx* ctx, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
+                            float* v_dF, float* v_cc, float* v_ambient, float* v_reproj, satsplat_stream stream) {
+  if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_backward_chain: ctx is NULL");
+  if (!ctx->chain_pending) return fail(ctx, SATSPLAT_E_STATE, "satsplat_backward_chain: no split backward call is pending on this context");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaSetDevice(ctx->device));
+  ctx->chain_pending = 0;
+  {
+    StageTimer t(ctx, SATSPLAT_STAGE_CHAIN_BWD, s);
+    CU(launch_chain_backward(ctx, ctx->in_means, ctx->in_quats, ctx->in_scales, ctx->in_logits, v_means, v_quats, v_scales,
+                             v_opacity_logits, ctx->depth_only ? nullptr : v_rgb, v_dF, ctx->chain_epi ? ctx->red_buf : nullptr, v_cc,
+                             v_ambient, v_reproj, s));
   }
   return SATSPLAT_OK;
 }
@@ -607,6 +634,11 @@ int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const in
 
 int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_set_option: ctx is NULL");
+  if (option == SATSPLAT_OPT_SPLIT_BACKWARD && (value == 0 || value == 1)) {
+    ctx->split_backward = value;
+    ctx->chain_pending = 0;
+    return SATSPLAT_OK;
+  }
   if (option == SATSPLAT_OPT_BINNING && (value == SATSPLAT_BINNING_TILESORT || value == SATSPLAT_BINNING_RADIX)) {
     ctx->binning_mode = value;
     ctx->preprocessed = 0;
@@ -695,6 +727,8 @@ int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int3
   if (!ctx->e2e_in[0] || (shadows && !sun_ctx->e2e_out[0]))
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: call satsplat_reserve_host_staging first");
   if (ctx->e2e_busy[slot]) return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host_begin: slot still in flight (call _end)");
+  if (ctx->split_backward || (shadows && sun_ctx->split_backward))
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: the contexts are in SATSPLAT_OPT_SPLIT_BACKWARD mode");
   cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
   // the sun camera and the reprojection constants are derived from F' = F + dF (Eq. 16, cascade of Fig. 1)

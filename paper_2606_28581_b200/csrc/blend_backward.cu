@@ -412,8 +412,8 @@ cudaError_t init_blend_backward_attrs() {
 }
 
 cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
-                                  const float* v_aux, const float* v_sun_depth_in, bool depth_only, float* v_cc,
-                                  float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s) {
+                                  const float* v_aux, const float* v_sun_depth_in, bool depth_only, bool want_epilogue_sums,
+                                  float* v_sun_depth, cudaStream_t s) {
   BwdParams P;
   P.cam = c->cam;
   P.sh = sh;
@@ -432,7 +432,7 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.px_i = c->px_i;
   P.vrec = c->vrec;
   P.v_sun_depth = v_sun_depth;
-  const bool want_red = !depth_only && (v_cc || v_ambient || v_reproj);
+  const bool want_red = !depth_only && want_epilogue_sums;
   P.red = want_red ? c->red_buf : nullptr;
   if (want_red) cudaMemsetAsync(c->red_buf, 0, kRedCopies * 32 * sizeof(float), s);
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));

@@ -218,6 +218,9 @@ struct satsplat_ctx {
   uint32_t* worklist;     // [3*tiles] tiles too long for the small-tile sort: 257-1024, 1025-4096, longer
   uint32_t* wl_count;     // [4] lengths of the three worklists
   int binning_mode;       // SATSPLAT_BINNING_TILESORT (default) or SATSPLAT_BINNING_RADIX
+  int split_backward;     // SATSPLAT_OPT_SPLIT_BACKWARD: the backward calls stop after the blend; satsplat_backward_chain finishes
+  int chain_pending;      // a blend backward has left moment records (and epilogue sums: chain_epi) for satsplat_backward_chain
+  int chain_epi;
   cudaStream_t bin_stream;   // the long tile lists are sorted on this stream beside the short ones (forked from / joined to the caller's)
   cudaEvent_t bin_ev[2];
   satsplat::Status* status;
@@ -276,8 +279,8 @@ cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s);
 cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, float* out_rgba, float* out_geom,
                                  float* out_aux, float* sun_depth_out, bool depth_only, cudaStream_t s);
 cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
-                                  const float* v_aux, const float* v_sun_depth_in, bool depth_only, float* v_cc,
-                                  float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s);
+                                  const float* v_aux, const float* v_sun_depth_in, bool depth_only, bool want_epilogue_sums,
+                                  float* v_sun_depth, cudaStream_t s);
 cudaError_t launch_chain_backward(satsplat_ctx* c, const float* means, const float* quats, const float* scales,
                                   const float* logits, float* v_means, float* v_quats, float* v_scales, float* v_logits,
                                   float* v_rgb, float* v_dF, const float* epi, float* v_cc, float* v_ambient, float* v_reproj,

@@ -924,3 +924,52 @@ def test_device_camera_path_equals_host_path_and_one_graph_serves_all_views(P, G
     assert e.value.code == P.E_STATE
     for c in (ctx, sctx, nctx):
         c.close()
+
+
+def test_split_backward_equals_unsplit(P, G, orc):
+    """SATSPLAT_OPT_SPLIT_BACKWARD: blend half + satsplat_backward_chain give what the one-call backward gives (view pass with
+    the epilogue sums, depth-only sun pass), with the view chain on a second stream beside the sun blend as bench.py runs it."""
+    import torch
+    scene = S.make_config(2, n=8000, size=128, n_views=1, extent=40.0, sun_size=192)
+    view = scene.views[0]
+    gs = G.GpuScene(scene)
+    ref = orc.view_iteration(scene, view, do_backward=False, threads=orc.num_threads())
+    up = S.upstream_grads(scene.seed, 0, view.height, view.width)
+    base = G.gpu_view_iteration(P, gs, view, sun_view=ref["sun_view"], reproj=ref["reproj"], upstream=up, want_debug=False)
+    n = scene.n
+    ctx, sctx = P.Context(n, view.width, view.height, 16 * n), P.Context(n, view.sun_width, view.sun_height, 16 * n)
+    surf = (gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+    sctx.preprocess(P.Camera.from_view(ref["sun_view"]), *surf)
+    sun_depth = torch.empty(view.sun_height, view.sun_width, device="cuda")
+    sctx.shadow_map(sun_depth)
+    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, sun_depth=sun_depth, reproj=ref["reproj"], depth_bias=view.depth_bias, slope=view.slope)
+    ctx.preprocess(P.Camera.from_view(view), *surf)
+    out = [torch.empty(view.height, view.width, 4, device="cuda") for _ in range(3)]
+    ctx.render_forward(sh, *out)
+    with pytest.raises(P.SatsplatError) as e:        # nothing pending yet
+        ctx.backward_chain(None, None, None, None)
+    assert e.value.code == P.E_STATE
+    for c in (ctx, sctx):
+        c.set_option(P.OPT_SPLIT_BACKWARD, 1)
+    g, g2 = gs.zeros_grads(), gs.zeros_grads()
+    v_sun = torch.zeros_like(sun_depth)
+    side = torch.cuda.Stream()
+    cur = torch.cuda.current_stream()
+    ctx.render_backward(sh, G.t(up[0]), G.t(up[1]), G.t(up[2]), None, None, None, None, None, v_sun_depth=v_sun)
+    side.wait_stream(cur)
+    ctx.backward_chain(g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"], g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"],
+                       g["v_reproj"], stream=side)
+    sctx.shadow_map_backward(v_sun, None, None, None, None)
+    cur.wait_stream(side)
+    sctx.backward_chain(g2["v_means"], g2["v_quats"], g2["v_scales"], g2["v_logits"], None, g2["v_dF_sun"])
+    torch.cuda.synchronize()
+    with pytest.raises(P.SatsplatError):
+        sctx.backward_chain(None, None, None, None)
+    np.testing.assert_array_equal(v_sun.cpu().numpy() != 0, base["v_sun_depth"] != 0)
+    for k in ("v_means", "v_quats", "v_scales", "v_logits", "v_rgb", "v_dF", "v_cc", "v_ambient", "v_reproj"):
+        a, b = g[k].cpu().numpy(), base["grads"][k]
+        np.testing.assert_allclose(a, b, rtol=1e-3, atol=1e-4 * max(1.0, np.abs(b).max()), err_msg=k)     # atomics: order differs run to run
+    for k in ("v_means", "v_quats", "v_scales", "v_logits", "v_dF_sun"):
+        a, b = g2[k].cpu().numpy(), base["sun_grads"][k]
+        np.testing.assert_allclose(a, b, rtol=1e-3, atol=1e-4 * max(1.0, np.abs(b).max()), err_msg=k)
+    ctx.close(); sctx.close()
