@@ -61,8 +61,8 @@ def parse():
     ap.add_argument("--dp-path", action="store_true",
                     help="run the data-parallel code path (NCCL group, gradient all-reduce on the communication stream, host-launched "
                          "steps) even with one rank: a functional check of that path on a single GPU, not a scaling number")
-    ap.add_argument("--record-traffic", default=None, metavar="NCU_RAW_CSV",
-                    help="write profiles/r2_traffic.json from `ncu -i <rep> --page raw --csv` output and exit")
+    ap.add_argument("--record-traffic", default=None, nargs="+", metavar="NCU_RAW_CSV",
+                    help="write profiles/r2_traffic.json from `ncu -i <rep> --page raw --csv` output file(s) and exit")
     return ap.parse_args()
 
 
@@ -85,14 +85,21 @@ def csrc_hash() -> str:
     return h.hexdigest()[:16]
 
 
-def record_traffic(raw_csv: str):
-    """profiles/r2_traffic.json <- per-kernel DRAM bytes, executed warp-instructions and issue utilisation of one
-    `ncu --set full` capture (first launch of each kernel name in the file), with the hash of the sources."""
+def record_traffic(raw_csvs):
+    """profiles/r2_traffic.json <- per-kernel DRAM bytes, executed warp-instructions and issue utilisation of `ncu --set
+    full` captures (first launch of each kernel name in the files), with the hash of the sources."""
     import csv
-    rows = list(csv.reader(open(raw_csv)))
+    out = {}
+    for raw_csv in raw_csvs:
+        rows = list(csv.reader(open(raw_csv)))
+        _record_rows(rows, out)
+    json.dump(dict(csrc_sha256=csrc_hash(), source=[os.path.basename(f) for f in raw_csvs], kernels=out), open(TRAFFIC_JSON, "w"), indent=1)
+    print("wrote", TRAFFIC_JSON, list(out))
+
+
+def _record_rows(rows, out):
     hdr = rows[0]
     col = {h: i for i, h in enumerate(hdr)}
-    out = {}
     for r in rows[2:]:
         name = r[col["Kernel Name"]]
         key = ("blend_bwd" if "blend_backward" in name else "blend_fwd" if "blend_forward" in name else name.split("(")[0].split("::")[-1])
@@ -108,8 +115,6 @@ def record_traffic(raw_csv: str):
                         warp_inst=f("smsp__inst_executed.sum"),
                         issue_active_pct=f("smsp__issue_active.avg.pct_of_peak_sustained_active"),
                         ncu_us=f("gpu__time_duration.sum"))
-    json.dump(dict(csrc_sha256=csrc_hash(), source=os.path.basename(raw_csv), kernels=out), open(TRAFFIC_JSON, "w"), indent=1)
-    print("wrote", TRAFFIC_JSON, list(out))
 
 
 def load_traffic():
