@@ -137,7 +137,9 @@ __global__ void __launch_bounds__(256) chain_backward_kernel(DevCamera camv, con
       g2.z = m3.x; g2.w = m3.y; g3.x = m3.z; g3.y = m3.w; g3.z = m4.x; g3.w = m4.y;
     }
     // gradient record slots: g0 = (c_x, c_y, M00, M01)  g1 = (M10, M11, alpha, z_c)  g2 = (r_0, r_1, red, green)  g3 = (blue, n_x, n_y, n_z)
-    if (v_logits) v_logits[i] = vlg + g1.z * alpha * (1.0f - alpha);
+    // v_logit = v_alpha alpha (1 - alpha) = -2 (sum s) (1 - alpha), with 1 - alpha = sigmoid(-logit) evaluated directly: for a
+    // nearly opaque surfel (logit 10) the difference 1 - alpha of the rounded alpha carries 1e-3 of relative error
+    if (v_logits) v_logits[i] = vlg - 2.0f * m2.w * (1.0f / (1.0f + expf(lg)));
     if (v_rgb) { s_vc[3 * t] += g2.z; s_vc[3 * t + 1] += g2.w; s_vc[3 * t + 2] += g3.x; }
     const float sg = (fl & F_FLIPPED) ? -1.f : 1.f;
     float vtu0 = 0.f, vtu1 = 0.f, vtu2 = 0.f, vtv0 = 0.f, vtv1 = 0.f, vtv2 = 0.f;
