@@ -294,8 +294,9 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
  * HOST: cam, w.  DEVICE, fp32, 16-byte aligned: the three rendered images and target_rgba [H,W,4] (4th channel of
  * the target ignored); scratch (satsplat_loss_scratch_floats(W, H) floats); v_rgba / v_geom / v_aux [H,W,4] are
  * OVERWRITTEN with dL/d(out_rgba, out_geom, out_aux); loss_sums [8]: [0] sum |I - I*| (divide by 3 H W), [1] sum of the
- * SSIM map (3 H W), [2] sum L_dist (H W), [3] sum (1 - A N_r.N_d) (H W), rest zero.  Two kernels on `stream`, no host
- * synchronisation.  Errors: SATSPLAT_E_INVALID (NULL pointer, singular camera), SATSPLAT_E_CUDA. */
+ * SSIM map (3 H W), [2] sum L_dist (H W), [3] sum (1 - A N_r.N_d) (H W), rest zero.  Three kernels ordered after the
+ * work already queued on `stream` and before any work queued on it later (one of them runs on an internal side stream,
+ * forked and joined with events: capturable in a CUDA graph); no host synchronisation.  Errors: SATSPLAT_E_INVALID (NULL pointer, singular camera), SATSPLAT_E_CUDA. */
 typedef struct {
   float w_l1, w_ssim, w_dist, w_normal;
 } satsplat_loss_weights;

@@ -219,7 +219,7 @@ int satsplat_sun_camera_backward(const satsplat_camera* view, float azimuth, flo
   return SATSPLAT_OK;
 }
 
-int64_t satsplat_loss_scratch_floats(int32_t width, int32_t height) { return (int64_t)12 * width * height; }
+int64_t satsplat_loss_scratch_floats(int32_t width, int32_t height) { return (int64_t)13 * width * height; }
 
 int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weights* w, const float* out_rgba,
                            const float* out_geom, const float* out_aux, const float* target_rgba, float* scratch,

@@ -635,7 +635,7 @@ def test_optimisation_steps_reduce_the_loss(P, G):
     assert (p[2] > 0).all()
 
 
-@pytest.mark.parametrize("hw", [(1, 1), (2, 5), (3, 3), (17, 33)])
+@pytest.mark.parametrize("hw", [(1, 1), (2, 5), (3, 3), (17, 33), (150, 203), (64, 128)])
 def test_loss_stage_tiny_and_ragged_images(P, G, hw):
     """Degenerate image sizes: no interior pixel for Eq. 13 (H or W < 3), windows larger than the image, ragged tiles.
     Synthetic image contents (the loss stage does not care where its inputs come from)."""
@@ -665,6 +665,54 @@ def test_loss_stage_tiny_and_ragged_images(P, G, hw):
     if H < 3 or W < 3:
         assert abs(terms["normal"] - 1.0) < 1e-12 and np.abs(r_geom).max() == 0    # no interior pixel: N_d = 0 everywhere
 
+
+
+def test_loss_stage_full_size_eager_and_captured(P, G):
+    """The loss stage at the benchmark's image size (2048 x 2048: 32 column strips x 13-18 row segments of the rolling
+    kernels, 8192 tiles of the normal-term kernel, the launch configuration bench.py times), EVERY pixel against the
+    float64 oracle; then the same call captured in a CUDA graph (the side-stream fork / join inside the call must be
+    capturable) and replayed: identical images."""
+    import torch
+    from oracle import losses
+    H = W = 2048
+    rng = np.random.default_rng(2048)
+    F, d = S.affine_camera(0.5, math.radians(15), 0.4, W, H, (2, 2, 0))
+    cam = P.Camera.make(W, H, np.asarray(F).reshape(-1), np.zeros(8, np.float32), d, 15.0, 14.0, (0, 0, 0))
+    rgba = rng.uniform(0.05, 0.95, (H, W, 4)).astype(np.float32)
+    geom = np.concatenate([rng.normal(0, 0.5, (H, W, 3)), rng.uniform(8, 12, (H, W, 1))], -1).astype(np.float32)
+    aux = rng.uniform(0, 1, (H, W, 4)).astype(np.float32)
+    t4 = np.concatenate([rng.uniform(0, 1, (H, W, 3)), np.zeros((H, W, 1))], -1).astype(np.float32)
+    terms, r_rgba, r_geom, r_aux = losses.loss_and_upstream(rgba, geom, aux, t4[..., :3], np.asarray(F, np.float32).astype(np.float64),
+                                                            d, 15.0, 14.0)
+    dev = [G.t(a) for a in (rgba, geom, aux, t4)]
+    scratch = torch.empty(P.loss_scratch_floats(W, H), device="cuda")
+    v = [torch.full((H, W, 4), float("nan"), device="cuda") for _ in range(3)]
+    sums = torch.full((8,), float("nan"), device="cuda")
+    P.loss_upstream(cam, *dev, scratch, v[0], v[1], v[2], sums)
+    torch.cuda.synchronize()
+    npx = H * W
+    s = sums.cpu().numpy().astype(np.float64)
+    got = dict(l1=s[0] / (3 * npx), ssim=s[1] / (3 * npx), distortion=s[2] / npx, normal=s[3] / npx)
+    for k, gv in got.items():
+        assert abs(gv - terms[k]) <= 2e-5 * max(abs(terms[k]), 1e-2), (k, gv, terms[k])
+    eager = [t_.cpu().numpy() for t_ in v]
+    for name, gpu, ref in (("v_rgba", eager[0], r_rgba), ("v_geom", eager[1], r_geom), ("v_aux", eager[2], r_aux)):
+        _loss_grad_close(name, gpu, ref, npx, 14.0)
+    del r_rgba, r_geom, r_aux
+    for t_ in v:
+        t_.fill_(float("nan"))
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            P.loss_upstream(cam, *dev, scratch, v[0], v[1], v[2], sums, stream=side)
+        graph.replay()
+        graph.replay()
+    side.synchronize()
+    for t_, e in zip(v, eager):
+        assert np.array_equal(t_.cpu().numpy(), e)
+    assert np.allclose(sums.cpu().numpy()[:4], s[:4], rtol=1e-5)
 
 
 @pytest.mark.parametrize("shape,n", [((1, 1), 1), ((3, 5), 3), ((40, 60), 2000), ((257, 301), 60000)])
