@@ -815,10 +815,11 @@ def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
     for _ in range(3):
         run_loss(0)
     ms_loss = timed(torch, None, 1, run_loss, range(20)) / 20
-    lb = px * 240.0
+    lb = px * 264.0   # 80 (ssim_stats) + 84 (normal_term) + 100 (ssim_adjoint) B / pixel
     line["loss_stage"] = dict(ms=ms_loss, bound="hbm", achieved=lb / (ms_loss * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                              frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=240,
-                              note="L1 + SSIM + distortion + normal consistency -> upstream gradients (2 kernels); not included in value / ms_per_step")
+                              frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=264,
+                              note="L1 + SSIM + distortion + normal consistency -> upstream gradients (3 kernels, the normal term beside "
+                                   "the SSIM statistics on a side stream); not included in value / ms_per_step")
     # ---- geometry-aware initialisation (row f4): one-time work, on a DSM of the site's size ----
     side = int(round(1000.0 / 0.3)) if args.config in (3, 4) else 512
     gen = torch.Generator(device=device); gen.manual_seed(1)
