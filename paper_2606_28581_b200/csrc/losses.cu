@@ -140,10 +140,11 @@ __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_ker
   float w1[6];
 #pragma unroll
   for (int k = 0; k < 6; ++k) { w1[k] = P.g[k]; w2[k] = pk(P.g[k], P.g[k]); }
-  f32x2 accM[11], accE[11];   // pending output rows: (mu_1, mu_2), (E[I^2], E[I*^2])
-  float accX[11];             // E[I I*]
+  // pending output rows: (mu_1, mu_2) and (E[I^2] + E[I*^2], E[I I*]) -- SSIM and its derivatives need the two second
+  // moments only through their sum, so four blurred maps per channel are carried, not five
+  f32x2 accM[11], accS[11];
 #pragma unroll
-  for (int k = 0; k < 11; ++k) { accM[k] = 0ull; accE[k] = 0ull; accX[k] = 0.f; }
+  for (int k = 0; k < 11; ++k) { accM[k] = 0ull; accS[k] = 0ull; }
   float ssim_sum = 0.f;
   const int r_first = ys - kSR, r_last = ye - 1 + kSR;
 #pragma unroll
@@ -172,26 +173,28 @@ __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_ker
         hE = fma2(wab, ab, hE);
         hX = fmaf(wa, b, hX);
       }
+      float h11, h22;
+      upk(hE, h11, h22);
+      const f32x2 hS = pk(h11 + h22, hX);
       // vertical pass: scatter into the pending rows (k = 0 opens a row)
 #pragma unroll
       for (int k = 0; k < 11; ++k) {
         const int s = slot_of(j, k), kk = k < 6 ? k : 10 - k;
         if (k == 0) {
-          accM[s] = mul2(w2[kk], hM); accE[s] = mul2(w2[kk], hE); accX[s] = w1[kk] * hX;
+          accM[s] = mul2(w2[kk], hM); accS[s] = mul2(w2[kk], hS);
         } else {
-          accM[s] = fma2(w2[kk], hM, accM[s]); accE[s] = fma2(w2[kk], hE, accE[s]); accX[s] = fmaf(w1[kk], hX, accX[s]);
+          accM[s] = fma2(w2[kk], hM, accM[s]); accS[s] = fma2(w2[kk], hS, accS[s]);
         }
       }
       const int y = r - kSR;
       if (y >= ys && x < P.W) {   // the completed row
         const int s = slot_of(j, 10);
-        float mu1, mu2, e11, e22;
+        float mu1, mu2, ess, e12;
         upk(accM[s], mu1, mu2);
-        upk(accE[s], e11, e22);
-        const float e12 = accX[s];
-        const float s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
+        upk(accS[s], ess, e12);
+        const float mm = mu1 * mu1 + mu2 * mu2, s12 = e12 - mu1 * mu2;
         const float a = 2.f * mu1 * mu2 + kC1, b = 2.f * s12 + kC2;
-        const float cc = mu1 * mu1 + mu2 * mu2 + kC1, d = s11 + s22 + kC2;
+        const float cc = mm + kC1, d = (ess - mm) + kC2;          // sigma_1^2 + sigma_2^2 = E[I^2] + E[I*^2] - mu_1^2 - mu_2^2
         const float icc = __fdividef(1.0f, cc), id = __fdividef(1.0f, d), icd = icc * id;
         const float m = a * b * icd;
         const float d_mu1 = 2.f * mu2 * b * icd - m * 2.f * mu1 * icc;
