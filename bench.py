@@ -774,12 +774,42 @@ def run_ours(args):
         dt_serial = wall(serial)
         pipelined()
         dt = wall(pipelined)
-        h2d = scene.n * 56 + 3 * px * 16
+        h2d = scene.n * 52 + 3 * px * 16
         d2h = 3 * px * 16 + (scene.n * 13 + 23) * 4
-        line["e2e"] = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+        raster_only = dict(value=world * px / 1e6 / (dt / n_e2e), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
                            ms_per_step=1e3 * dt / n_e2e, steps=n_e2e, serial_ms_per_step=1e3 * dt_serial / n_e2e,
                            api="satsplat_iteration_host_begin / _end, two steps in flight (pinned host buffers; same work as the device "
-                               "step, cascade chain included); serial_ms_per_step = one blocking satsplat_iteration_host per step")
+                               "step, cascade chain included; the upstream-gradient images go up and the rendered images come down); "
+                               "serial_ms_per_step = one blocking satsplat_iteration_host per step")
+        # the call a training loop makes: surfels + target image up, forward -> loss stage on the device -> backward,
+        # gradients + loss sums down.  MORE device work per step than `value` times (the loss stage), a third of the bytes.
+        h_tgt = torch.rand(v.height, v.width, 4).pin_memory()
+        h_sums = torch.empty(8).pin_memory()
+        targs = (cam, sun, sh, scene.n, *h_in, h_tgt, None, h_g, h_sums)
+
+        def t_serial():
+            for i in range(n_e2e):
+                P.training_step_host(job.ctx, job.sctx, *targs)
+
+        def t_pipelined():
+            P.training_step_host_begin(job.ctx, job.sctx, 0, *targs)
+            for i in range(1, n_e2e):
+                P.training_step_host_begin(job.ctx, job.sctx, i & 1, *targs)
+                P.training_step_host_end(job.ctx, (i - 1) & 1)
+            P.training_step_host_end(job.ctx, (n_e2e - 1) & 1)
+        t_serial()
+        dt_ts = wall(t_serial)
+        t_pipelined()
+        dt_t = wall(t_pipelined)
+        assert float(h_sums[0]) > 0 and bool(torch.isfinite(h_g).all())
+        line["e2e"] = dict(value=world * px / 1e6 / (dt_t / n_e2e), unit=UNIT, h2d_bytes_per_step=scene.n * 52 + px * 16,
+                           d2h_bytes_per_step=(scene.n * 13 + 23 + 8) * 4, ms_per_step=1e3 * dt_t / n_e2e, steps=n_e2e,
+                           serial_ms_per_step=1e3 * dt_ts / n_e2e,
+                           api="satsplat_training_step_host_begin / _end, two steps in flight (pinned host buffers): the device step "
+                               "of `value` PLUS the loss stage (L1 + SSIM + distortion + normal consistency) between forward and "
+                               "backward; surfels and the target image go up, gradients and the loss sums come down; "
+                               "serial_ms_per_step = one blocking satsplat_training_step_host per step",
+                           rasteriser_only=raster_only)
     # ---- the oracle beside it (rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline_block(scene, step_views[0], px, nviews)

@@ -226,8 +226,8 @@ int satsplat_render_backward_device(satsplat_ctx* ctx, const float* block, const
                                     float* v_sun_depth /*[Hs,Ws]*/, float* v_reproj /*[8]*/, satsplat_stream stream);
 
 
-/* Allocates the device staging buffers satsplat_iteration_host needs (sized for the contexts' maxima) and its two
- * copy streams.  The only allocating call besides satsplat_create; idempotent; `sun_ctx` may be NULL. */
+/* Allocates the device staging buffers satsplat_iteration_host and satsplat_training_step_host need (sized for the
+ * contexts' maxima; 45 floats per pixel and 26 per surfel for the two slots of the view context) and their two copy streams.  The only allocating call besides satsplat_create; idempotent; `sun_ctx` may be NULL. */
 int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx);
 
 /* One whole training-view iteration with HOST buffers (end-to-end leg of the benchmark): copies the surfels and
@@ -304,6 +304,27 @@ int64_t satsplat_loss_scratch_floats(int32_t width, int32_t height);
 int satsplat_loss_upstream(const satsplat_camera* cam, const satsplat_loss_weights* w, const float* out_rgba,
                            const float* out_geom, const float* out_aux, const float* target_rgba, float* scratch,
                            float* v_rgba, float* v_geom, float* v_aux, float* loss_sums, satsplat_stream stream);
+
+/* One whole TRAINING step with HOST buffers: satsplat_iteration_host with the loss stage in the middle.  Copies the
+ * surfels and the target image host->device, runs sun pass + view pass forward, satsplat_loss_upstream on the rendered
+ * images (its upstream gradients never leave the device), the backward of both passes and the cascade chain, and copies
+ * back the packed gradients (layout of satsplat_iteration_host), the 8 loss sums of satsplat_loss_upstream and, if
+ * h_out_rgba is not NULL, the rendered image.  Per step this moves 13 N + 4 H W floats up and 13 N + 31 floats down
+ * instead of the 13 N + 12 H W up / 13 N + 12 H W down of the rasteriser-only call.  _begin / _end as for
+ * satsplat_iteration_host (the two families share the staging slots: a slot carries one step of either kind at a
+ * time).  h_target_rgba [H,W,4] (4th channel ignored), h_loss_sums [8]: HOST.  Errors as satsplat_iteration_host. */
+int satsplat_training_step_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam, const satsplat_sun* sun,
+                                const satsplat_shading* shading, const satsplat_loss_weights* weights, int64_t N,
+                                const float* h_means, const float* h_quats, const float* h_scales, const float* h_logits,
+                                const float* h_rgb, const float* h_target_rgba, float* h_out_rgba, float* h_grads,
+                                float* h_loss_sums, satsplat_stream stream);
+int satsplat_training_step_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                                      const satsplat_sun* sun, const satsplat_shading* shading,
+                                      const satsplat_loss_weights* weights, int64_t N, const float* h_means,
+                                      const float* h_quats, const float* h_scales, const float* h_logits, const float* h_rgb,
+                                      const float* h_target_rgba, float* h_out_rgba, float* h_grads, float* h_loss_sums,
+                                      satsplat_stream stream);
+int satsplat_training_step_host_end(satsplat_ctx* ctx, int32_t slot);
 
 /* ---- geometry-aware initialisation ----------------------------------------- */
 /* Surfels from a DSM.  dsm[row, col] heights on a regular grid of spacing `cell`; the centre of

@@ -153,6 +153,11 @@ def lib():
         L.satsplat_reserve_host_staging.argtypes = [vp, vp]
         L.satsplat_iteration_host_begin.argtypes = [vp, vp, i32, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading), i64] + [vp] * 13
         L.satsplat_iteration_host_end.argtypes = [vp, i32]
+        L.satsplat_training_step_host_begin.argtypes = [vp, vp, i32, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading),
+                                                        C.POINTER(LossWeights), i64] + [vp] * 10
+        L.satsplat_training_step_host_end.argtypes = [vp, i32]
+        L.satsplat_training_step_host.argtypes = [vp, vp, C.POINTER(Camera), C.POINTER(Sun), C.POINTER(Shading),
+                                                  C.POINTER(LossWeights), i64] + [vp] * 10
         L.satsplat_sync_status.argtypes = [vp, C.POINTER(i64), vp]
         L.satsplat_debug_bins.argtypes = [vp, C.POINTER(i64)] + [C.POINTER(vp)] * 5 + [vp]
         L.satsplat_debug_records.argtypes = [vp, vp, vp, vp]
@@ -501,6 +506,33 @@ def iteration_host_begin(ctx: Context, sun_ctx, slot, cam: Camera, sun, shading:
                                                 None if sun is None else C.byref(sun), C.byref(shading), int(n), hp(h_means),
                                                 hp(h_quats), hp(h_scales), hp(h_logits), hp(h_rgb), hp(h_v_rgba), hp(h_v_geom),
                                                 hp(h_v_aux), hp(h_out_rgba), hp(h_out_geom), hp(h_out_aux), hp(h_grads), _stream(stream)))
+
+
+def training_step_host_begin(ctx: Context, sun_ctx, slot, cam: Camera, sun, shading: Shading, n, h_means, h_quats, h_scales,
+                             h_logits, h_rgb, h_target_rgba, h_out_rgba, h_grads, h_loss_sums,
+                             w_l1=0.8, w_ssim=0.2, w_dist=0.05, w_normal=0.05, stream=None):
+    """satsplat_training_step_host_begin: forward -> loss stage on the device -> backward, HOST tensors (surfels and the
+    target image up; gradients, the 8 loss sums and, if h_out_rgba is not None, the rendered image down); staging slot 0 / 1;
+    no synchronisation."""
+    hp = _host_ptr
+    w = LossWeights(float(w_l1), float(w_ssim), float(w_dist), float(w_normal))
+    ctx._rc(lib().satsplat_training_step_host_begin(ctx._h, None if sun_ctx is None else sun_ctx._h, int(slot), C.byref(cam),
+                                                    None if sun is None else C.byref(sun), C.byref(shading), C.byref(w), int(n),
+                                                    hp(h_means), hp(h_quats), hp(h_scales), hp(h_logits), hp(h_rgb),
+                                                    hp(h_target_rgba), hp(h_out_rgba), hp(h_grads), hp(h_loss_sums), _stream(stream)))
+
+
+def training_step_host_end(ctx: Context, slot):
+    """satsplat_training_step_host_end: wait until the step begun on `slot` has delivered its gradients and loss sums."""
+    ctx._rc(lib().satsplat_training_step_host_end(ctx._h, int(slot)))
+
+
+def training_step_host(ctx: Context, sun_ctx, cam: Camera, sun, shading: Shading, n, h_means, h_quats, h_scales, h_logits, h_rgb,
+                       h_target_rgba, h_out_rgba, h_grads, h_loss_sums, stream=None, **weights):
+    """satsplat_training_step_host: _begin(slot 0) + _end(slot 0)."""
+    training_step_host_begin(ctx, sun_ctx, 0, cam, sun, shading, n, h_means, h_quats, h_scales, h_logits, h_rgb, h_target_rgba,
+                             h_out_rgba, h_grads, h_loss_sums, stream=stream, **weights)
+    training_step_host_end(ctx, 0)
 
 
 def iteration_host_end(ctx: Context, slot):

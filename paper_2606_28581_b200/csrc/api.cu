@@ -170,7 +170,8 @@ void satsplat_destroy(satsplat_ctx* ctx) {
                   ctx->keys[0], ctx->keys[1], ctx->vals[0], ctx->vals[1], ctx->hist, ctx->ranges, ctx->status, ctx->tile_count,
                   ctx->tile_start, ctx->worklist, ctx->wl_count, ctx->px_a,
                   ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in[0], ctx->e2e_in[1],
-                  ctx->e2e_up[0], ctx->e2e_up[1], ctx->e2e_out[0], ctx->e2e_out[1], ctx->e2e_grads[0], ctx->e2e_grads[1]};
+                  ctx->e2e_up[0], ctx->e2e_up[1], ctx->e2e_out[0], ctx->e2e_out[1], ctx->e2e_grads[0], ctx->e2e_grads[1],
+                  ctx->e2e_target[0], ctx->e2e_target[1], ctx->e2e_loss[0], ctx->e2e_loss[1]};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
@@ -693,6 +694,8 @@ int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
       CU(dalloc(ctx, &ctx->e2e_up[k], mpx * 12));
       CU(dalloc(ctx, &ctx->e2e_out[k], mpx * 12));
       CU(dalloc(ctx, &ctx->e2e_grads[k], pk.off[5] + 64));
+      CU(dalloc(ctx, &ctx->e2e_target[k], mpx * 4));
+      CU(dalloc(ctx, &ctx->e2e_loss[k], (size_t)satsplat_loss_scratch_floats(ctx->max_w, ctx->max_h)));
       for (int i = 0; i < 5; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
     }
     for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
@@ -705,13 +708,18 @@ int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
   return SATSPLAT_OK;
 }
 
-int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
-                                  const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
-                                  const float* h_means, const float* h_quats, const float* h_scales,
-                                  const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
-                                  const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
-                                  float* h_grads, satsplat_stream stream) {
+// One step with host buffers.  lw == NULL: the upstream gradients come from the host (h_v_*); lw != NULL (training step):
+// they are written on the device by the loss stage from the rendered images and the uploaded target, and the loss sums
+// come back with the gradients.
+static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                           const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                           const float* h_means, const float* h_quats, const float* h_scales,
+                           const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                           const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                           float* h_grads, const satsplat_loss_weights* lw, const float* h_target, float* h_sums,
+                           satsplat_stream stream) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_iteration_host: ctx is NULL");
+  if (lw && (!h_target || !h_sums)) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_training_step_host: bad argument");
   if (!cam || !shading || !h_means || !h_quats || !h_scales || !h_logits || !h_rgb || !h_grads || N <= 0 || slot < 0 || slot > 1)
     return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: bad argument");
   // every size is checked before the first copy is enqueued
@@ -758,10 +766,13 @@ int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int3
   float* d_up[3] = {nullptr, nullptr, nullptr};
   const float* h_up[3] = {h_v_rgba, h_v_geom, h_v_aux};
   for (int k = 0; k < 3; ++k)
-    if (h_up[k]) {
+    if (lw) {
+      d_up[k] = ctx->e2e_up[slot] + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
+    } else if (h_up[k]) {
       d_up[k] = ctx->e2e_up[slot] + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
       CU(cudaMemcpyAsync(d_up[k], h_up[k], px * 16, cudaMemcpyHostToDevice, s_up));
     }
+  if (lw) CU(cudaMemcpyAsync(ctx->e2e_target[slot], h_target, px * 16, cudaMemcpyHostToDevice, s_up));
   CU(cudaEventRecord(ev[1], s_up));
   float* d_out[3];
   for (int k = 0; k < 3; ++k) d_out[k] = ctx->e2e_out[slot] + (size_t)k * 4 * (size_t)ctx->max_w * ctx->max_h;
@@ -793,6 +804,10 @@ int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int3
   for (int k = 0; k < 3; ++k)
     if (h_out[k]) CU(cudaMemcpyAsync(h_out[k], d_out[k], px * 16, cudaMemcpyDeviceToHost, s_down));
   CU(cudaStreamWaitEvent(s, ev[1], 0));
+  float* const d_sums = g + pk.off[5] + 48;
+  if (lw && (rc = satsplat_loss_upstream(cam, lw, d_out[0], d_out[1], d_out[2], ctx->e2e_target[slot], ctx->e2e_loss[slot], d_up[0],
+                                         d_up[1], d_up[2], d_sums, stream)))
+    return rc;
   if ((rc = satsplat_render_backward(ctx, &sh, d_up[0], d_up[1], d_up[2], g_grp[0], g_grp[1], g_grp[2], g_grp[3], g_grp[4], g_dF,
                                      g_cc, g_amb, d_vsun, shadows ? g_rep : nullptr, stream)))
     return rc;
@@ -810,9 +825,31 @@ int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int3
     ho += n * width[k];
   }
   CU(cudaMemcpyAsync(h_grads + ho, g_dF, 23 * sizeof(float), cudaMemcpyDeviceToHost, s_down));
+  if (lw) CU(cudaMemcpyAsync(h_sums, d_sums, 8 * sizeof(float), cudaMemcpyDeviceToHost, s_down));
   CU(cudaEventRecord(ev[4], s_down));
   ctx->e2e_busy[slot] = 1;
   return SATSPLAT_OK;
+}
+
+int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                                  const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                                  const float* h_means, const float* h_quats, const float* h_scales,
+                                  const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                                  const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                                  float* h_grads, satsplat_stream stream) {
+  return host_step_begin(ctx, sun_ctx, slot, cam, sun, shading, N, h_means, h_quats, h_scales, h_logits, h_rgb, h_v_rgba, h_v_geom,
+                         h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, nullptr, nullptr, nullptr, stream);
+}
+
+int satsplat_training_step_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                                      const satsplat_sun* sun, const satsplat_shading* shading,
+                                      const satsplat_loss_weights* weights, int64_t N, const float* h_means,
+                                      const float* h_quats, const float* h_scales, const float* h_logits, const float* h_rgb,
+                                      const float* h_target_rgba, float* h_out_rgba, float* h_grads, float* h_loss_sums,
+                                      satsplat_stream stream) {
+  if (!weights) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_training_step_host: weights is NULL");
+  return host_step_begin(ctx, sun_ctx, slot, cam, sun, shading, N, h_means, h_quats, h_scales, h_logits, h_rgb, nullptr, nullptr,
+                         nullptr, h_out_rgba, nullptr, nullptr, h_grads, weights, h_target_rgba, h_loss_sums, stream);
 }
 
 int satsplat_iteration_host_end(satsplat_ctx* ctx, int32_t slot) {
@@ -833,6 +870,19 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
                             float* h_grads, satsplat_stream stream) {
   const int rc = satsplat_iteration_host_begin(ctx, sun_ctx, 0, cam, sun, shading, N, h_means, h_quats, h_scales, h_logits, h_rgb,
                                                h_v_rgba, h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, stream);
+  if (rc) return rc;
+  return satsplat_iteration_host_end(ctx, 0);
+}
+
+int satsplat_training_step_host_end(satsplat_ctx* ctx, int32_t slot) { return satsplat_iteration_host_end(ctx, slot); }
+
+int satsplat_training_step_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const satsplat_camera* cam, const satsplat_sun* sun,
+                                const satsplat_shading* shading, const satsplat_loss_weights* weights, int64_t N,
+                                const float* h_means, const float* h_quats, const float* h_scales, const float* h_logits,
+                                const float* h_rgb, const float* h_target_rgba, float* h_out_rgba, float* h_grads,
+                                float* h_loss_sums, satsplat_stream stream) {
+  const int rc = satsplat_training_step_host_begin(ctx, sun_ctx, 0, cam, sun, shading, weights, N, h_means, h_quats, h_scales,
+                                                   h_logits, h_rgb, h_target_rgba, h_out_rgba, h_grads, h_loss_sums, stream);
   if (rc) return rc;
   return satsplat_iteration_host_end(ctx, 0);
 }

@@ -243,7 +243,9 @@ struct satsplat_ctx {
   float* e2e_in[2];       // means..rgb, sub-arrays at 16-byte aligned offsets
   float* e2e_up[2];       // upstream gradients (3 images)
   float* e2e_out[2];      // images (view ctx); slot 0 of a sun ctx: sun map + its gradient
-  float* e2e_grads[2];    // surfel gradient groups + dF cc ambient reproj dF_sun
+  float* e2e_grads[2];    // surfel gradient groups + dF cc ambient reproj dF_sun, loss sums (8) at + 48
+  float* e2e_target[2];   // training step: target image
+  float* e2e_loss[2];     // training step: scratch of the loss stage
   cudaStream_t e2e_stream[2];   // uploads / downloads, beside the caller's stream
   cudaEvent_t e2e_ev[2][5];     // per slot: surfels up, upstream up, forward done, backward done, everything down
   int e2e_busy[2];              // slot has a begin without its end

@@ -137,9 +137,8 @@ __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_ker
     soff += 4ll * P.W; ++srow; sstage = (sstage + 1) & (kStages - 1);
   };
   f32x2 w2[6];
-  float w1[6];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) { w1[k] = P.g[k]; w2[k] = pk(P.g[k], P.g[k]); }
+  for (int k = 0; k < 6; ++k) w2[k] = pk(P.g[k], P.g[k]);
   // pending output rows: (mu_1, mu_2) and (E[I^2] + E[I*^2], E[I I*]) -- SSIM and its derivatives need the two second
   // moments only through their sum, so four blurred maps per channel are carried, not five
   f32x2 accM[11], accS[11];

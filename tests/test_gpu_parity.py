@@ -442,6 +442,70 @@ def test_iteration_host_matches_device_path(P, G, orc, n):
     ctx.close(); sctx.close()
 
 
+@pytest.mark.parametrize("n", [3000, 1023])
+def test_training_step_host_equals_forward_loss_backward(P, G, n):
+    """satsplat_training_step_host (surfels + target up, gradients + loss sums down, the loss stage on the device in the
+    middle) gives what the rasteriser-only host call gives when it is fed the upstream gradients that
+    satsplat_loss_upstream computes from the same rendered images; two steps in flight on the two slots as well.  A
+    consistency test of entry points of the CUDA path (each piece has its own parity test against the oracle)."""
+    import torch
+    scene = S.make_config(2, n=n, size=128, n_views=1, extent=40.0, sun_size=192)
+    view = scene.views[0]
+    H, W = view.height, view.width
+    cam = P.Camera.from_view(view)
+    sun = P.Sun.from_view(view)
+    ctx = P.Context(n, W, H, 16 * n)
+    sctx = P.Context(n, view.sun_width, view.sun_height, 16 * n)
+    P.reserve_host_staging(ctx, sctx)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
+    sh = P.Shading.make(cc=view.cc, ambient=view.ambient, depth_bias=view.depth_bias, slope=view.slope)
+    sh.shadows_on = 1
+    surf = (pin(scene.means), pin(scene.quats), pin(scene.scales), pin(scene.opacity_logits), pin(scene.rgb))
+    rng = np.random.default_rng(11)
+    target = pin(np.concatenate([rng.uniform(0, 1, (H, W, 3)), np.zeros((H, W, 1))], -1))
+    # reference: images from the rasteriser-only call, upstream from the loss stage, gradients from a second call
+    h_out = [torch.empty(H, W, 4).pin_memory() for _ in range(3)]
+    h_g = torch.empty(n * 13 + 23).pin_memory()
+    zero = pin(np.zeros((H, W, 4)))
+    P.iteration_host(ctx, sctx, cam, sun, sh, n, *surf, zero, zero, zero, *h_out, h_g)
+    d = [t_.cuda() for t_ in h_out]
+    scratch = torch.empty(P.loss_scratch_floats(W, H), device="cuda")
+    v = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    sums = torch.zeros(8, device="cuda")
+    P.loss_upstream(cam, d[0], d[1], d[2], target.cuda(), scratch, v[0], v[1], v[2], sums)
+    torch.cuda.synchronize()
+    up = [pin(t_.cpu().numpy()) for t_ in v]
+    P.iteration_host(ctx, sctx, cam, sun, sh, n, *surf, *up, *h_out, h_g)
+    ref_g, ref_s = h_g.numpy().copy(), sums.cpu().numpy()
+    assert np.abs(ref_g[:13 * n]).max() > 0
+    # the training step
+    t_img = torch.full((H, W, 4), float("nan")).pin_memory()
+    t_g = torch.full((n * 13 + 23,), float("nan")).pin_memory()
+    t_s = torch.full((8,), float("nan")).pin_memory()
+    P.training_step_host(ctx, sctx, cam, sun, sh, n, *surf, target, t_img, t_g, t_s)
+    assert torch.equal(t_img, h_out[0])
+    np.testing.assert_allclose(t_s.numpy(), ref_s, rtol=1e-5)
+    tol = 1e-4 * max(1.0, np.abs(ref_g).max())
+    np.testing.assert_allclose(t_g.numpy(), ref_g, rtol=1e-3, atol=tol)          # atomics: order differs run to run
+    # two steps in flight; the rendered image is optional
+    g2 = [torch.full((n * 13 + 23,), float("nan")).pin_memory() for _ in range(2)]
+    s2 = [torch.full((8,), float("nan")).pin_memory() for _ in range(2)]
+    P.training_step_host_begin(ctx, sctx, 0, cam, sun, sh, n, *surf, target, None, g2[0], s2[0])
+    with pytest.raises(P.SatsplatError) as e:
+        P.training_step_host_begin(ctx, sctx, 0, cam, sun, sh, n, *surf, target, None, g2[0], s2[0])
+    assert e.value.code == P.E_STATE
+    P.training_step_host_begin(ctx, sctx, 1, cam, sun, sh, n, *surf, target, None, g2[1], s2[1])
+    P.training_step_host_end(ctx, 0)
+    P.training_step_host_end(ctx, 1)
+    for k in range(2):
+        np.testing.assert_allclose(s2[k].numpy(), ref_s, rtol=1e-5)
+        np.testing.assert_allclose(g2[k].numpy(), ref_g, rtol=1e-3, atol=tol)
+    with pytest.raises(P.SatsplatError) as e:          # the target is not optional
+        P.training_step_host(ctx, sctx, cam, sun, sh, n, *surf, None, None, t_g, t_s)
+    assert e.value.code == P.E_INVALID
+    ctx.close(); sctx.close()
+
+
 def test_sun_camera_backward_matches_oracle(P, G, orc):
     """Cascade adjoint (satsplat_sun_camera_backward): closed-form device kernel against the oracle's
     step-by-step adjoint of Eq. 16 on random cotangents; NULL inputs; accumulation."""
