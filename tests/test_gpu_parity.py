@@ -699,7 +699,7 @@ def test_optimisation_steps_reduce_the_loss(P, G):
     assert (p[2] > 0).all()
 
 
-@pytest.mark.parametrize("hw", [(1, 1), (2, 5), (3, 3), (17, 33), (150, 203), (64, 128)])
+@pytest.mark.parametrize("hw", [(1, 1), (2, 5), (3, 3), (17, 33), (150, 203), (64, 128), (700, 65), (33, 129), (11, 63)])
 def test_loss_stage_tiny_and_ragged_images(P, G, hw):
     """Degenerate image sizes: no interior pixel for Eq. 13 (H or W < 3), windows larger than the image, ragged tiles.
     Synthetic image contents (the loss stage does not care where its inputs come from)."""
