@@ -179,10 +179,10 @@ void satsplat_destroy(satsplat_ctx* ctx) {
   if (ctx->bin_stream) cudaStreamDestroy(ctx->bin_stream);
   for (int i = 0; i < 2; ++i)
     if (ctx->bin_ev[i]) cudaEventDestroy(ctx->bin_ev[i]);
-  for (int i = 0; i < 2; ++i)
+  for (int i = 0; i < 3; ++i)
     if (ctx->e2e_stream[i]) cudaStreamDestroy(ctx->e2e_stream[i]);
-  for (int i = 0; i < 10; ++i)
-    if (ctx->e2e_ev[i / 5][i % 5]) cudaEventDestroy(ctx->e2e_ev[i / 5][i % 5]);
+  for (int i = 0; i < 12; ++i)
+    if (ctx->e2e_ev[i / 6][i % 6]) cudaEventDestroy(ctx->e2e_ev[i / 6][i % 6]);
   free(ctx);
 }
 
@@ -696,9 +696,9 @@ int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
       CU(dalloc(ctx, &ctx->e2e_grads[k], pk.off[5] + 64));
       CU(dalloc(ctx, &ctx->e2e_target[k], mpx * 4));
       CU(dalloc(ctx, &ctx->e2e_loss[k], (size_t)satsplat_loss_scratch_floats(ctx->max_w, ctx->max_h)));
-      for (int i = 0; i < 5; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
+      for (int i = 0; i < 6; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
     }
-    for (int i = 0; i < 2; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
+    for (int i = 0; i < 3; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
   }
   if (sun_ctx && !sun_ctx->e2e_out[0]) {
     const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
@@ -752,8 +752,8 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
   // caller's stream is still busy with the kernels of the previous step (other slot), this step's 257 MB are already
   // crossing PCIe.  The caller's stream carries the kernels; the images come down on the download stream while the
   // backward runs, the gradients after it (PCIe is full duplex).
-  cudaStream_t s_up = ctx->e2e_stream[0], s_down = ctx->e2e_stream[1];
-  cudaEvent_t* ev = ctx->e2e_ev[slot];   // 0 surfels up, 1 upstream up, 2 forward done, 3 backward done, 4 everything down
+  cudaStream_t s_up = ctx->e2e_stream[0], s_down = ctx->e2e_stream[1], s_view = ctx->e2e_stream[2];
+  cudaEvent_t* ev = ctx->e2e_ev[slot];   // 0 surfels up, 1 upstream up, 2 forward done, 3 backward done, 4 everything down, 5 view preprocess done
   const Pack pk = pack_offsets(n);
   float* d_in[5];
   const float* h_in[5] = {h_means, h_quats, h_scales, h_logits, h_rgb};
@@ -787,6 +787,12 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
   int rc;
   CU(cudaStreamWaitEvent(s, ev[0], 0));
   if (shadows) {
+    // the view pass's preprocess + binning needs the surfels only: it runs beside the sun pass.  It follows the caller's
+    // stream up to here (the previous step's backward reads the view context's records) and joins before render_forward.
+    CU(cudaEventRecord(ev[5], s));
+    CU(cudaStreamWaitEvent(s_view, ev[5], 0));
+    if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], (satsplat_stream)s_view))) return rc;
+    CU(cudaEventRecord(ev[5], s_view));
     d_sun = sun_ctx->e2e_out[0];
     d_vsun = d_sun + (size_t)sun_ctx->max_w * sun_ctx->max_h;
     if ((rc = satsplat_preprocess(sun_ctx, &sun_cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
@@ -796,7 +802,8 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
     sh.sun_width = sun->width;
     sh.sun_height = sun->height;
   }
-  if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
+  if (shadows) CU(cudaStreamWaitEvent(s, ev[5], 0));
+  else if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
   if ((rc = satsplat_render_forward(ctx, &sh, d_out[0], d_out[1], d_out[2], stream))) return rc;
   CU(cudaEventRecord(ev[2], s));
   float* h_out[3] = {h_out_rgba, h_out_geom, h_out_aux};

@@ -246,8 +246,8 @@ struct satsplat_ctx {
   float* e2e_grads[2];    // surfel gradient groups + dF cc ambient reproj dF_sun, loss sums (8) at + 48
   float* e2e_target[2];   // training step: target image
   float* e2e_loss[2];     // training step: scratch of the loss stage
-  cudaStream_t e2e_stream[2];   // uploads / downloads, beside the caller's stream
-  cudaEvent_t e2e_ev[2][5];     // per slot: surfels up, upstream up, forward done, backward done, everything down
+  cudaStream_t e2e_stream[3];   // uploads / downloads / view-pass preprocess, beside the caller's stream
+  cudaEvent_t e2e_ev[2][6];     // per slot: surfels up, upstream up, forward done, backward done, everything down, view preprocess done
   int e2e_busy[2];              // slot has a begin without its end
   // profiling
   int profiling;
