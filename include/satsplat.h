@@ -296,7 +296,9 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
  * OVERWRITTEN with dL/d(out_rgba, out_geom, out_aux); loss_sums [8]: [0] sum |I - I*| (divide by 3 H W), [1] sum of the
  * SSIM map (3 H W), [2] sum L_dist (H W), [3] sum (1 - A N_r.N_d) (H W), rest zero.  Three kernels ordered after the
  * work already queued on `stream` and before any work queued on it later (one of them runs on an internal side stream,
- * forked and joined with events: capturable in a CUDA graph); no host synchronisation.  Errors: SATSPLAT_E_INVALID (NULL pointer, singular camera), SATSPLAT_E_CUDA. */
+ * forked and joined with events: capturable in a CUDA graph); no host synchronisation.  The side stream and its two
+ * events are per device and shared by all calls: calls for one device must not be issued from several host threads at
+ * the same time (issue them from one thread, on any streams).  Errors: SATSPLAT_E_INVALID (NULL pointer, singular camera), SATSPLAT_E_CUDA. */
 typedef struct {
   float w_l1, w_ssim, w_dist, w_normal;
 } satsplat_loss_weights;
