@@ -431,7 +431,7 @@ class Job:
             self.P.sun_camera_backward(self.cams[vi][0], v.sun_azimuth, v.sun_elevation, v.sun_viewport, g["dFs"], g["rep"], g["dF"])
 
 
-    def step_device(self, stride=1, buf=0):
+    def step_device(self, stride=1, buf=0, upstream_fn=None):
         """The same iteration with every camera read from the device-resident block: the view is
         selected by the device index, nothing of it is baked into kernel arguments, so ONE captured graph of this function
         serves all views and all optimiser steps (dF lives in self.dF_all on the device)."""
@@ -454,7 +454,7 @@ class Job:
         else:
             self.ctx.preprocess_device(self.W, self.H, self.block, P.CAM_VIEW, *surf)
         self.ctx.render_forward_device(self.block, self.sun_depth, *self.out)
-        up = self.up_shared
+        up = upstream_fn() if upstream_fn else self.up_shared     # upstream_fn: the loss stage on the rendered images (extras)
         if self.shadows:
             # split backward calls: the view pass's per-surfel chain (HBM-bound) runs on the side stream beside the sun pass's
             # blend backward (issue-bound); the sun pass's chain follows both (the two chains share the gradient buffers)
@@ -850,6 +850,32 @@ def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
                               frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=264,
                               note="L1 + SSIM + distortion + normal consistency -> upstream gradients (3 kernels, the normal term beside "
                                    "the SSIM statistics on a side stream); not included in value / ms_per_step")
+    # ---- one whole TRAINING iteration as ONE CUDA graph: camera chain (f2), both passes forward, loss stage (f1), both
+    # backwards, cascade chain, Adam step (f3); device-resident cameras, so the same graph serves all views and steps ----
+    if not args.no_graphs and not args.dp_path and args.gpus == 1:
+        lr_tiny = [1e-7] * 5      # the step is real, the learning rates are tiny so that the synthetic scene stays put
+        surf = [job.means, job.quats, job.scales, job.logits, job.rgb]
+
+        def upstream():
+            P.loss_upstream(cam, job.out[0], job.out[1], job.out[2], tgt, scr, vv[0], vv[1], vv[2], sums)
+            return vv
+
+        def train_iteration():
+            job.step_device(upstream_fn=upstream)
+            P.adam_step(scene.n, *surf, *gg, am, av, lr_tiny, step=100)
+        job.idx.fill_(step_views[0])
+        train_iteration()
+        torch.cuda.synchronize()
+        tgraph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(tgraph, stream=torch.cuda.Stream(device=device, priority=-1)):
+            train_iteration()
+        for _ in range(3):
+            tgraph.replay()
+        ms_train = timed(torch, None, 1, lambda _: tgraph.replay(), range(50)) / 50
+        line["training_iteration"] = dict(ms=ms_train, mpixel_s=px / 1e6 / (ms_train * 1e-3),
+                                          note="ONE graph replay per iteration: the step of `value` + loss stage between forward and "
+                                               "backward + fused Adam over the 13 N parameters (learning rates 1e-7: the synthetic "
+                                               "scene stays put); not included in value / ms_per_step")
     # ---- geometry-aware initialisation (row f4): one-time work, on a DSM of the site's size ----
     side = int(round(1000.0 / 0.3)) if args.config in (3, 4) else 512
     gen = torch.Generator(device=device); gen.manual_seed(1)
