@@ -4,9 +4,10 @@
 // weights :349).  Three kernels:
 //   ssim_stats_kernel    ROLLING column strips: a CTA owns 64 image columns and a run of rows and marches down the rows;
 //                        thread = (column, colour channel).  Per row: the 74 pixels of I and I* (strip + 5-pixel halo)
-//                        are copied into a 4-row ring in shared memory by cp.async (issued three rows ahead; the 4-byte
-//                        copies transpose the float4 pixels into per-channel (I, I*) pairs), the thread blurs the five
-//                        moments (I, I*, I^2, I*^2, I I*) of its channel horizontally (11 taps) and scatters the result
+//                        are copied into an 8-row ring in shared memory by cp.async (issued four rows ahead; the 4-byte
+//                        copies transpose the float4 pixels into per-channel (I, I*) pairs; the CTA barrier per row is an
+//                        mbarrier whose arrive and wait are one row apart), the thread blurs the moments
+//                        (I, I*, I^2 + I*^2, I I*) of its channel horizontally (11 taps) and scatters the result
 //                        into the 11 pending output rows it keeps in REGISTERS (vertical pass: no shared-memory round
 //                        trip, no vertical halo recomputation); the row that completes gives the SSIM value and its
 //                        three partial derivatives (w.r.t. mu_1, E[I^2], E[I I*]), written as one float4 per channel
@@ -83,6 +84,20 @@ __device__ __forceinline__ void cp_async_zfill(unsigned sa, const void* gmem, bo
 
 constexpr int kStages = 4;              // rows in flight in the rolling kernels' shared-memory ring
 
+// mbarrier as a CTA barrier whose two halves are an iteration apart (arrive now, wait at the top of the next row):
+// the warps of a CTA may drift by one row instead of meeting at every row
+__device__ __forceinline__ void mbar_init(unsigned sa, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(sa), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned sa) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sa) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned sa, unsigned parity) {
+  asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}\n" ::"r"(sa),
+               "r"(parity)
+               : "memory");
+}
+
 template <int NT>
 __device__ __forceinline__ float block_sum(float v, float* s_red) {   // NT threads (a multiple of 32, <= 1024); valid in thread 0
 #pragma unroll
@@ -108,7 +123,9 @@ __host__ __device__ constexpr int slot_of(int j, int k) { return (j + 5 - k + 11
 #define SATSPLAT_STATS_MINB 3
 #endif
 __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_kernel(const __grid_constant__ LossParams P) {
-  __shared__ f32x2 s_ab[kStages][3][kSIn];    // ring of staged rows: (I, I*) per channel, zero outside the image
+  constexpr int kRing = 8, kAhead = 4;        // ring of staged rows; a row is copied kAhead rows before it is read
+  __shared__ f32x2 s_ab[kRing][3][kSIn];      // (I, I*) per channel, zero outside the image
+  __shared__ __align__(8) unsigned long long s_bar;
   __shared__ float s_red[kSThreads / 32];
   const int tid = threadIdx.x, col = tid & (kSW - 1), c = tid >> 6;
   const int x0 = blockIdx.x * kSW, x = x0 + col;
@@ -134,7 +151,7 @@ __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_ker
       cp_async_zfill<4>(d + 16 * kSIn, g + 2, ok);
     }
     cp_async_commit();
-    soff += 4ll * P.W; ++srow; sstage = (sstage + 1) & (kStages - 1);
+    soff += 4ll * P.W; ++srow; sstage = (sstage + 1) & (kRing - 1);
   };
   f32x2 w2[6];
 #pragma unroll
@@ -146,17 +163,27 @@ __global__ void __launch_bounds__(kSThreads, SATSPLAT_STATS_MINB) ssim_stats_ker
   for (int k = 0; k < 11; ++k) { accM[k] = 0ull; accS[k] = 0ull; }
   float ssim_sum = 0.f;
   const int r_first = ys - kSR, r_last = ye - 1 + kSR;
+  // Row pipeline.  Phase k of the mbarrier completes when every thread's copies of row r_first + k have landed; a thread
+  // arrives for phase k + 1 at the top of step k (before its arithmetic) and waits for phase k at the top of step k: a
+  // warp runs at most one row ahead of the slowest.  The stage overwritten at step k (row k + 4) was read at step k - 4.
+  const unsigned bar = smem_addr(&s_bar);
+  if (tid == 0) mbar_init(bar, kSThreads);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  __syncthreads();
 #pragma unroll
-  for (int k = 0; k < kStages - 1; ++k) stage_row();
+  for (int k = 0; k < kAhead; ++k) stage_row();
+  cp_async_wait<kAhead - 1>();
+  mbar_arrive(bar);
   for (int r0 = r_first; r0 <= r_last; r0 += 11) {
 #pragma unroll
     for (int j = 0; j < 11; ++j) {
       const int r = r0 + j;
       if (r > r_last) break;
-      const int buf = (r - r_first) & (kStages - 1);
-      cp_async_wait<kStages - 2>();   // this thread's copies of row r have landed ...
-      __syncthreads();                // ... and everybody's; everybody is done with the stage of row r - 1
-      stage_row();                    // row r + 3 into that stage
+      const int it = r - r_first, buf = it & (kRing - 1);
+      mbar_wait(bar, it & 1);         // everybody's copies of row r have landed; everybody is done with row r - 2
+      stage_row();                    // row r + 4 into the stage of row r - 4
+      cp_async_wait<kAhead - 1>();    // this thread's copies of row r + 1 have landed
+      mbar_arrive(bar);
       // horizontal pass of this thread's channel
       const f32x2* const row = &s_ab[buf][c][col];
       f32x2 hM = 0ull, hE = 0ull;
