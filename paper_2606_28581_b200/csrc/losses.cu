@@ -365,7 +365,6 @@ __global__ void __launch_bounds__(kAThreads, SATSPLAT_ADJ_MINB) ssim_adjoint_ker
   const int ch_a = role_a ? tid / kSIn : 0, sc_a = tid % kSIn;
   const int gx_a = x0 - kSR + sc_a;
   const bool in_a = role_a && gx_a >= 0 && gx_a < P.W;
-  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
   f32x2 w2[6];
 #pragma unroll
   for (int k = 0; k < 6; ++k) w2[k] = pk(P.g[k], P.g[k]);
@@ -480,7 +479,7 @@ __global__ void __launch_bounds__(kAThreads, SATSPLAT_ADJ_MINB) ssim_adjoint_ker
 // Rows per strip segment: the strips x segments grid fills `waves` rounds of the CTAs the device holds at once (one round:
 // every CTA marches in step, no tail), with at least 16 rows per segment (a segment recomputes 10 warm-up rows).
 static int segment_rows(int W, int H, int ctas_per_sm) {
-  static const double waves = [] { const char* e = getenv("SATSPLAT_LOSS_WAVES"); return e ? atof(e) : 1.0; }();
+  static const double waves = [] { const char* e = getenv("SATSPLAT_LOSS_WAVES"); return e ? atof(e) : 1.0; }();   // tuning knob
   const int strips = (W + kSW - 1) / kSW;
   const long long target = (long long)(current_sm_count() * ctas_per_sm * waves);
   long long segs = target / strips;
@@ -497,7 +496,7 @@ struct LossSide { cudaStream_t stream = nullptr; cudaEvent_t fork = nullptr, joi
 static LossSide* loss_side() {
   static std::mutex mu;
   static std::map<int, LossSide> per_device;
-  static const bool enabled = [] { const char* e = getenv("SATSPLAT_LOSS_OVERLAP"); return !e || atoi(e) != 0; }();
+  static const bool enabled = [] { const char* e = getenv("SATSPLAT_LOSS_OVERLAP"); return !e || atoi(e) != 0; }();   // 0: one stream (A/B)
   if (!enabled) return nullptr;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
