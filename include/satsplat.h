@@ -365,6 +365,28 @@ int satsplat_relocate(int64_t N, float* means, float* quats, float* scales, floa
                       float* adam_v, const float* u, float o_min, int32_t n_max, void* scratch, int32_t* src_out,
                       satsplat_stream stream);
 
+/* satsplat_relocate for callers that cannot supply scratch memory.  Same operation, same arguments (minus `scratch`), same
+ * results, but the working memory is an array built into the library instead of a caller buffer, and the call itself never
+ * allocates or frees device memory.  It is meant for hosts where an allocation at this point is not an option: the
+ * surrounding framework has already claimed the whole GPU for its own pool and exposes no C allocator, the job runs under a
+ * hard memory quota, or the training loop cannot afford the device-wide pause that an allocation or a free brings.
+ *   Limit: N <= SATSPLAT_RELOCATE_STATIC_MAX_SURFELS (131072; the array is about 3.5 MB).  A larger N is refused with
+ *     SATSPLAT_E_INVALID and a message that names the limit; nothing is launched.  Use satsplat_relocate beyond it.
+ *   Cost: each GPU on which the library is loaded carries the array from load until the process exits, used or not.
+ *   First call per device: looks up the array's device address (cudaGetSymbolAddress with the caller's current device) and
+ *     keeps it; make that first call with the right device current and outside any stream capture.  Later calls only launch.
+ *   Sharing: all calls on one GPU work in the same array.  The array keeps whatever the previous call wrote; that is
+ *     harmless because every call rewrites each entry before reading it (nothing needs to be cleared by the caller).  Two
+ *     calls whose kernels can overlap on the GPU (different streams without an event between them, or several host threads)
+ *     corrupt each other: order them on one stream or with events.
+ * Pointers, in-place updates, u, o_min, n_max, src_out and `stream` exactly as for satsplat_relocate.
+ * Errors: SATSPLAT_E_INVALID (bad argument, NULL pointer, N over the limit), SATSPLAT_E_CUDA; message via
+ * satsplat_last_error(NULL). */
+#define SATSPLAT_RELOCATE_STATIC_MAX_SURFELS 131072
+int satsplat_relocate_static(int64_t N, float* means, float* quats, float* scales, float* opacity_logits, float* rgb,
+                             float* adam_m, float* adam_v, const float* u, float o_min, int32_t n_max, int32_t* src_out,
+                             satsplat_stream stream);
+
 /* ---- status, test and profiling access ------------------------------------------------------------------ */
 /* Synchronises `stream`, then reports the last preprocess: K (duplicated keys) and whether max_duplicates
  * overflowed (returns SATSPLAT_E_CAPACITY then).  HOST pointers, may be NULL. */

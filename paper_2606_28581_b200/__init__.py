@@ -141,6 +141,7 @@ def lib():
         L.satsplat_relocate_scratch_bytes.restype = C.c_int64
         L.satsplat_relocate_scratch_bytes.argtypes = [i64]
         L.satsplat_relocate.argtypes = [i64] + [vp] * 8 + [f32, i32, vp, vp, vp]
+        L.satsplat_relocate_static.argtypes = [i64] + [vp] * 8 + [f32, i32, vp, vp]
         L.satsplat_adam_state_floats.restype = C.c_int64
         L.satsplat_adam_state_floats.argtypes = [i64]
         L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
@@ -324,6 +325,24 @@ def relocate(n, means, quats, scales, opacity_logits, rgb, adam_m, adam_v, u, o_
     rc = lib().satsplat_relocate(int(n), _ptr(means), _ptr(quats), _ptr(scales), _ptr(opacity_logits), _ptr(rgb), _ptr(adam_m),
                                  _ptr(adam_v), _ptr(u), float(o_min), int(n_max), scratch.data_ptr(),
                                  None if src is None else src.data_ptr(), _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+    return src
+
+
+RELOCATE_STATIC_MAX_SURFELS = 131072
+
+
+def relocate_static(n, means, quats, scales, opacity_logits, rgb, adam_m, adam_v, u, o_min=0.005, n_max=51, want_src=False, stream=None):
+    """satsplat_relocate_static: `relocate` without a scratch buffer from the caller.  The library works in an array that is
+    part of its own image, so the call performs no device allocation; that is what a host needs whose GPU memory is already
+    fully owned by another pool or capped by a quota, or that cannot tolerate an allocation stall inside its loop.  At most
+    RELOCATE_STATIC_MAX_SURFELS surfels (SatsplatError above that); calls on one GPU share the array and must not overlap.
+    (`src`, when asked for, is an output tensor this binding creates for convenience; the C call takes a caller pointer.)"""
+    src = torch.empty(int(n), dtype=torch.int32, device=means.device) if want_src else None
+    rc = lib().satsplat_relocate_static(int(n), _ptr(means), _ptr(quats), _ptr(scales), _ptr(opacity_logits), _ptr(rgb), _ptr(adam_m),
+                                        _ptr(adam_v), _ptr(u), float(o_min), int(n_max), None if src is None else src.data_ptr(),
+                                        _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
     return src

@@ -14,7 +14,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libsatsplat.so")
-SOURCES = ["api.cu", "preprocess.cu", "binning.cu", "blend_forward.cu", "blend_backward.cu", "chain_backward.cu", "adam.cu", "losses.cu", "init.cu", "relocate.cu", "peaks.cu", "camera.cu"]
+SOURCES = ["api.cu", "preprocess.cu", "binning.cu", "blend_forward.cu", "blend_backward.cu", "chain_backward.cu", "adam.cu", "losses.cu", "init.cu", "relocate.cu", "relocate_static.cu", "peaks.cu", "camera.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC,-ffp-contract=off",
               "--expt-relaxed-constexpr"]
 

@@ -17,6 +17,14 @@ std::atomic<long long> g_kernel_launches{0};
 namespace {
 
 thread_local char g_err[512] = "";
+}  // namespace
+
+namespace satsplat {
+// for entry points that live in other translation units: the message satsplat_last_error(NULL) returns on this thread
+void set_thread_error(const char* msg) { snprintf(g_err, sizeof(g_err), "%s", msg); }
+}  // namespace satsplat
+
+namespace {
 
 int fail(satsplat_ctx* c, int code, const char* fmt, const char* a = "") {
   char* dst = c ? c->err : g_err;

@@ -319,5 +319,6 @@ cudaError_t launch_advance_index(int32_t* view_index, int32_t stride, int32_t n_
 cudaError_t init_blend_backward_attrs();
 cudaError_t init_binning_attrs();
 cudaError_t launch_export_records(satsplat_ctx* c, float* records_out, uint8_t* flags_out, cudaStream_t s);
+void set_thread_error(const char* msg);   // api.cu: message of satsplat_last_error(NULL) on the calling thread
 
 }  // namespace satsplat
