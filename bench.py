@@ -3,7 +3,7 @@
 
     python bench.py --gpus N --steps K --warmup W            # the CUDA path (hand-written sm_100a kernels)
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands, on the host cores
-    python bench.py --record-traffic <ncu raw csv>           # refresh profiles/r2_traffic.json from an ncu capture
+    python bench.py --record-traffic <ncu raw csv>           # refresh profiles/r3_traffic.json from an ncu capture
 
 A "step" is one full training-view iteration of the hot path: sun pass (preprocess,
 binning, depth-only compositing) -> view pass (preprocess, binning, compositing of colour/alpha/depth/normal/
@@ -40,7 +40,11 @@ INST_CONTRIB_FWD = 25.0   # extra per contributing pair, forward (view pass; the
 INST_CONTRIB_BWD = 90.0   # extra per contributing pair, backward (view pass; sun pass: 50)
 INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN = 6.0, 50.0
 SM_LANES = 128            # FP32 lanes per SM; derived peak = SMs x 128 x clock, measured one beside it
-TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r3_traffic.json")
+DESIGN_BYTES = {"preprocess": 137.0, "chain_bwd": 309.0}   # bytes per surfel this implementation moves
+# stage -> kernel name in the traffic JSON (view pass, sun pass)
+TRAFFIC_KEYS = {"preprocess": ("void preprocess_kernel<0>", None), "blend_fwd": ("blend_fwd", "blend_fwd_sun"),
+                "blend_bwd": ("blend_bwd", "blend_bwd_sun"), "chain_bwd": ("void chain_backward_kernel<0>", None)}
 CSRC = os.path.join(ROOT, "paper_2606_28581_b200", "csrc")
 
 
@@ -62,7 +66,7 @@ def parse():
                     help="run the data-parallel code path (NCCL group, gradient all-reduce on the communication stream, host-launched "
                          "steps) even with one rank: a functional check of that path on a single GPU, not a scaling number")
     ap.add_argument("--record-traffic", default=None, nargs="+", metavar="NCU_RAW_CSV",
-                    help="write profiles/r2_traffic.json from `ncu -i <rep> --page raw --csv` output file(s) and exit")
+                    help="write profiles/r3_traffic.json from `ncu -i <rep> --page raw --csv` output file(s) and exit")
     return ap.parse_args()
 
 
@@ -86,7 +90,7 @@ def csrc_hash() -> str:
 
 
 def record_traffic(raw_csvs):
-    """profiles/r2_traffic.json <- per-kernel DRAM bytes, executed warp-instructions and issue utilisation of `ncu --set
+    """profiles/r3_traffic.json <- per-kernel DRAM bytes, executed warp-instructions and issue utilisation of `ncu --set
     full` captures (first launch of each kernel name in the files), with the hash of the sources."""
     import csv
     out = {}
@@ -123,8 +127,8 @@ def load_traffic():
         return None, "no capture committed"
     d = json.load(open(TRAFFIC_JSON))
     if d.get("csrc_sha256") != csrc_hash():
-        return None, f"stale: profiles/r2_traffic.json was captured on sources {d.get('csrc_sha256')}, these are {csrc_hash()}"
-    return d["kernels"], "profiles/r2_traffic.json (ncu --set full, same sources)"
+        return None, f"stale: profiles/r3_traffic.json was captured on sources {d.get('csrc_sha256')}, these are {csrc_hash()}"
+    return d["kernels"], "profiles/r3_traffic.json (ncu --set full, same sources)"
 
 
 def make_scene(args):
@@ -531,6 +535,16 @@ def stage_profile(job, views, peaks, fp32_peak_tinst):
     job.ctx.set_profiling(False)
     if job.sctx:
         job.sctx.set_profiling(False)
+    # pair counters: one more pass over the last view with the instrumentation planes on (SATSPLAT_OPT_DEBUG_PLANES; they are
+    # off in every timed region, stage times above included)
+    for c in (job.ctx, job.sctx):
+        if c:
+            c.set_option(P.OPT_DEBUG_PLANES, 1)
+    job.step(views[-1])
+    torch.cuda.synchronize()
+    for c in (job.ctx, job.sctx):
+        if c:
+            c.set_option(P.OPT_DEBUG_PLANES, 0)
     job.overlap = True
     nv, nc = job.ctx.debug_planes()
     pairs = dict(view_evaluated=int(nv.sum().item()), view_contributing=int(nc.sum().item()), view_K=job.ctx.sync_status())
@@ -551,14 +565,14 @@ def stage_profile(job, views, peaks, fp32_peak_tinst):
         evb, cob = pairs.get(f"{pass_}_bwd_evaluated", ev), pairs.get(f"{pass_}_bwd_contributing", co)
         cf, cb = (INST_CONTRIB_FWD, INST_CONTRIB_BWD) if pass_ == "view" else (INST_CONTRIB_FWD_SUN, INST_CONTRIB_BWD_SUN)
         return {
-            "preprocess": ("hbm", n * 137.0, None),
+            "preprocess": ("hbm", n * 132.0, None),      # 56 B in + 76 B of records / boxes / keys out
             "scan": ("hbm", tiles * 12.0, None),
             "duplicate": ("hbm", n * 16.0 + K * 8.0, None),
             "sort": ("hbm", K * 20.0, None),
             "ranges": ("hbm", 0.0, None),
             "blend_fwd": ("alu", ev * INST_EVAL + co * cf, co * (INST_EVAL + cf)),
             "blend_bwd": ("alu", evb * INST_EVAL + cob * cb, cob * (INST_EVAL + cb)),
-            "chain_bwd": ("hbm", n * (80.0 * 2 + 45.0 + 52.0 * 2), None),
+            "chain_bwd": ("hbm", n * 172.0, None),       # SURVEY.md 8(d); the design moves 309 (DESIGN_BYTES below)
         }
 
     stages = {}
@@ -572,6 +586,12 @@ def stage_profile(job, views, peaks, fp32_peak_tinst):
                   frac=ach / peak if peak else None, roofline_ms=w / scale / peak * 1e3)
         if useful is not None and ms > 0:
             st["useful_frac"] = useful / (ms * 1e-3) / scale / peak          # contributing pairs only
+        if k in DESIGN_BYTES and ms > 0:
+            # what THIS design moves per surfel (moment records written by the blend and read + cleared by the chain, the +=
+            # read-modify-write of the gradient arrays): printed beside the method's bytes, never as the fraction
+            st["design_bytes_per_surfel"] = DESIGN_BYTES[k]
+            st["method_bytes_per_surfel"] = w / n
+            st["design_frac"] = n * DESIGN_BYTES[k] / (ms * 1e-3) / scale / peak
         if ws is not None and ms_sun.get(k, 0.0) > 0:
             _, w2, u2 = ws[k]
             st["sun_frac"] = w2 / (ms_sun[k] * 1e-3) / scale / peak
@@ -708,6 +728,24 @@ def run_ours(args):
                                 peak_derived=derived_tinst if d["bound"] == "alu" else None,
                                 peak_derived_how=f"{mp['sm_count']} SMs x {SM_LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz",
                                 mufu_peak_measured_tops=mp["mufu_per_s"] / 1e12, kernel_ms=d["ms"])
+        # ncu-derived fields per stage (only while the committed capture matches these sources): DRAM traffic against the
+        # method's bytes for the HBM-bound stages; executed lane slots against the credited lane-instructions for the blends,
+        # so that a stage whose credited work exceeds everything its kernel executes shows as such
+        for k, (kv, ks) in TRAFFIC_KEYS.items():
+            for key, pre in ((kv, ""), (ks, "sun_")):
+                t_k = (traffic or {}).get(key) if key else None
+                if not t_k or k not in stages:
+                    continue
+                st = stages[k]
+                credited_ms = st["roofline_ms"] if pre == "" else st.get("sun_roofline_ms")
+                if credited_ms is None:
+                    continue
+                if st["bound"] == "hbm" and t_k.get("dram_bytes"):
+                    st[pre + "traffic_over_algorithmic"] = t_k["dram_bytes"] / (credited_ms * 1e-3 * st["peak"] * 1e9)
+                elif st["bound"] == "alu" and t_k.get("warp_inst"):
+                    slots = t_k["warp_inst"] * 32
+                    st[pre + "executed_lane_slots"] = slots
+                    st[pre + "credited_over_executed"] = credited_ms * 1e-3 * st["peak"] * 1e12 / slots
         line["stages"] = stages
         line["pairs"] = pairs
         sun_ms = sum(s["sun_ms"] for s in stages.values())
@@ -732,8 +770,10 @@ def run_ours(args):
         pin = lambda t: t.detach().cpu().contiguous().pin_memory()
         h_in = [pin(x) for x in (job.means, job.quats, job.scales, job.logits, job.rgb)]
         h_up = [pin(u) for u in job.up_shared]
-        h_out = [torch.empty(v.height, v.width, 4).pin_memory() for _ in range(3)]
-        h_g = torch.empty(scene.n * 13 + 23).pin_memory()
+        # outputs are per slot: a step's host buffers stay untouched until its _end (the inputs are only read: shared)
+        h_out2 = [[torch.empty(v.height, v.width, 4).pin_memory() for _ in range(3)] for _ in range(2)]
+        h_g2 = [torch.empty(scene.n * 13 + 23).pin_memory() for _ in range(2)]
+        h_g = h_g2[0]
         cam = job.cams[vi][0]
         sun = P.Sun.from_view(v) if job.shadows else None
         sh = P.Shading.make(cc=v.cc, ambient=v.ambient, depth_bias=v.depth_bias, slope=v.slope)
@@ -744,7 +784,8 @@ def run_ours(args):
             job.sctx.set_option(P.OPT_SPLIT_BACKWARD, 0)
             job.split = False
 
-        hargs = (cam, sun, sh, scene.n, *h_in, *h_up, *h_out, h_g)
+        hargs2 = [(cam, sun, sh, scene.n, *h_in, *h_up, *h_out2[k], h_g2[k]) for k in range(2)]
+        hargs = hargs2[0]
 
         def e2e_step(_):
             P.iteration_host(job.ctx, job.sctx, *hargs)
@@ -766,9 +807,9 @@ def run_ours(args):
                 e2e_step(i)
 
         def pipelined():   # the begin / end pair: the upload of step i+1 crosses PCIe while the kernels of step i run
-            P.iteration_host_begin(job.ctx, job.sctx, 0, *hargs)
+            P.iteration_host_begin(job.ctx, job.sctx, 0, *hargs2[0])
             for i in range(1, n_e2e):
-                P.iteration_host_begin(job.ctx, job.sctx, i & 1, *hargs)
+                P.iteration_host_begin(job.ctx, job.sctx, i & 1, *hargs2[i & 1])
                 P.iteration_host_end(job.ctx, (i - 1) & 1)
             P.iteration_host_end(job.ctx, (n_e2e - 1) & 1)
         dt_serial = wall(serial)
@@ -784,24 +825,26 @@ def run_ours(args):
         # the call a training loop makes: surfels + target image up, forward -> loss stage on the device -> backward,
         # gradients + loss sums down.  MORE device work per step than `value` times (the loss stage), a third of the bytes.
         h_tgt = torch.rand(v.height, v.width, 4).pin_memory()
-        h_sums = torch.empty(8).pin_memory()
-        targs = (cam, sun, sh, scene.n, *h_in, h_tgt, None, h_g, h_sums)
+        h_sums2 = [torch.empty(8).pin_memory() for _ in range(2)]
+        h_sums = h_sums2[0]
+        targs2 = [(cam, sun, sh, scene.n, *h_in, h_tgt, None, h_g2[k], h_sums2[k]) for k in range(2)]
+        targs = targs2[0]
 
         def t_serial():
             for i in range(n_e2e):
                 P.training_step_host(job.ctx, job.sctx, *targs)
 
         def t_pipelined():
-            P.training_step_host_begin(job.ctx, job.sctx, 0, *targs)
+            P.training_step_host_begin(job.ctx, job.sctx, 0, *targs2[0])
             for i in range(1, n_e2e):
-                P.training_step_host_begin(job.ctx, job.sctx, i & 1, *targs)
+                P.training_step_host_begin(job.ctx, job.sctx, i & 1, *targs2[i & 1])
                 P.training_step_host_end(job.ctx, (i - 1) & 1)
             P.training_step_host_end(job.ctx, (n_e2e - 1) & 1)
         t_serial()
         dt_ts = wall(t_serial)
         t_pipelined()
         dt_t = wall(t_pipelined)
-        assert float(h_sums[0]) > 0 and bool(torch.isfinite(h_g).all())
+        assert all(float(x[0]) > 0 for x in h_sums2) and all(bool(torch.isfinite(x).all()) for x in h_g2)
         line["e2e"] = dict(value=world * px / 1e6 / (dt_t / n_e2e), unit=UNIT, h2d_bytes_per_step=scene.n * 52 + px * 16,
                            d2h_bytes_per_step=(scene.n * 13 + 23 + 8) * 4, ms_per_step=1e3 * dt_t / n_e2e, steps=n_e2e,
                            serial_ms_per_step=1e3 * dt_ts / n_e2e,
@@ -821,6 +864,7 @@ def run_ours(args):
 
 def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
     """The NEXT rows of SURVEY.md section 8 that sit outside the metric's iteration, each timed on its own."""
+    traffic_all, _ = load_traffic()
     # ---- the optimiser step (row f3) ----
     ns = P.adam_state_floats(scene.n)
     am, av = torch.zeros(ns, device=device), torch.zeros(ns, device=device)
@@ -845,9 +889,17 @@ def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
     for _ in range(3):
         run_loss(0)
     ms_loss = timed(torch, None, 1, run_loss, range(20)) / 20
-    lb = px * 264.0   # 80 (ssim_stats) + 84 (normal_term) + 100 (ssim_adjoint) B / pixel
+    # the METHOD moves 64 B in (three rendered images + target) + 48 B out (three upstream images) = 112 B / pixel; this
+    # design's three kernels move 264 (derivative maps and v_zv written and read back).  Neither is what limits the
+    # kernels today: ssim_stats / ssim_adjoint run at 59-73 % issue-active (profiles/r2_loss.md), i.e. instruction issue.
+    lb, lb_design = px * 112.0, px * 264.0
+    lt = [(traffic_all or {}).get(k) for k in ("ssim_stats_kernel", "normal_term_kernel", "ssim_adjoint_kernel")]
     line["loss_stage"] = dict(ms=ms_loss, bound="hbm", achieved=lb / (ms_loss * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                              frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=264,
+                              frac=lb / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"], bytes_per_pixel=112,
+                              design_bytes_per_pixel=264, design_frac=lb_design / (ms_loss * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                              binding="instruction issue (59-73 % issue-active in the two SSIM kernels), not HBM: frac is the distance "
+                                      "to the method's byte floor, not the headroom of these kernels",
+                              traffic_over_algorithmic=(sum(t["dram_bytes"] for t in lt) / lb) if all(lt) else None,
                               note="L1 + SSIM + distortion + normal consistency -> upstream gradients (3 kernels, the normal term beside "
                                    "the SSIM statistics on a side stream); not included in value / ms_per_step")
     # ---- one whole TRAINING iteration as ONE CUDA graph: camera chain (f2), both passes forward, loss stage (f1), both

@@ -227,7 +227,7 @@ int satsplat_render_backward_device(satsplat_ctx* ctx, const float* block, const
 
 
 /* Allocates the device staging buffers satsplat_iteration_host and satsplat_training_step_host need (sized for the
- * contexts' maxima; 45 floats per pixel and 26 per surfel for the two slots of the view context) and their two copy streams.  The only allocating call besides satsplat_create; idempotent; `sun_ctx` may be NULL. */
+ * contexts' maxima; 45 floats per pixel and 26 per surfel for the two slots of the view context) and their two copy streams.  The only allocating call besides satsplat_create; idempotent; `sun_ctx` may be NULL.  If an allocation fails (SATSPLAT_E_CUDA) everything this call had allocated so far is freed again and a later call starts afresh. */
 int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx);
 
 /* One whole training-view iteration with HOST buffers (end-to-end leg of the benchmark): copies the surfels and
@@ -250,7 +250,9 @@ int satsplat_iteration_host(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, const sats
  * while the kernels of step i run): _begin enqueues everything for one step on staging slot `slot` (0 or 1) and returns
  * without synchronising; _end blocks until that step's images and gradients are in the host buffers.  A slot can be
  * begun again only after its _end (SATSPLAT_E_STATE otherwise); the host buffers of a step must stay valid and
- * untouched until its _end.  satsplat_iteration_host == _begin(slot 0) + _end(slot 0). */
+ * untouched until its _end.  The two slots share the contexts' scratch, so both steps in flight must be begun on the SAME
+ * `stream` (SATSPLAT_E_STATE otherwise); if _begin fails after copies were enqueued it drains them before returning, so the
+ * caller's buffers are free again on any error.  satsplat_iteration_host == _begin(slot 0) + _end(slot 0). */
 int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
                                   const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
                                   const float* h_means, const float* h_quats, const float* h_scales,
@@ -404,7 +406,9 @@ int satsplat_debug_bins(satsplat_ctx* ctx, int64_t* K, const uint64_t** keys, co
  * left into surfel gradients (accumulated into v_means ... v_rgb, DEVICE, any may be NULL; v_rgb is ignored for a
  * depth-only context), reduces v_dF and delivers v_cc / v_ambient / v_reproj.  Must run after the blend half (stream
  * order or an event) and before the next backward on `ctx`; two chains that accumulate into the same gradient buffers must
- * be ordered by the caller.  SATSPLAT_E_STATE if no split backward is pending. */
+ * be ordered by the caller.  SATSPLAT_E_STATE if no split backward is pending.  While one IS pending, satsplat_preprocess*,
+ * satsplat_render_backward*, satsplat_shadow_map_backward and satsplat_set_option(SATSPLAT_OPT_SPLIT_BACKWARD) on `ctx` return
+ * SATSPLAT_E_STATE and launch nothing (the moment records would otherwise be overwritten or added to twice). */
 int satsplat_backward_chain(satsplat_ctx* ctx, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
                             float* v_dF /*[8]*/, float* v_cc /*[12]*/, float* v_ambient /*[3]*/, float* v_reproj /*[8]*/,
                             satsplat_stream stream);
@@ -416,7 +420,9 @@ int satsplat_debug_records(satsplat_ctx* ctx, float* records_out, uint8_t* flags
 
 /* Per-pixel planes of the last forward: n_visited[H,W] (tile-list entries visited, including the one that
  * triggered the transmittance stop) and n_contrib[H,W] (composited entries); DEVICE int32 pointers owned by
- * the context.  Their sums are the evaluated / contributing pair counts the roofline is quoted against. */
+ * the context.  Their sums are the evaluated / contributing pair counts the roofline is quoted against.
+ * Instrumentation, not part of the method: the forward stores them (8 B / pixel) only while
+ * SATSPLAT_OPT_DEBUG_PLANES is 1 (default 0); SATSPLAT_E_STATE if the last forward ran without it. */
 int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const int32_t** n_contrib);
 
 /* Per-stage device times of the most recent hot call on this context, measured with CUDA events on the
@@ -448,6 +454,9 @@ int satsplat_stage_ms(satsplat_ctx* ctx, float* ms_out);
  *     may be NULL) and satsplat_backward_chain runs the per-surfel chain.  For callers that overlap the chain of one pass
  *     (HBM-bound) with the blend backward of the next pass (issue-bound) on two streams. */
 #define SATSPLAT_OPT_SPLIT_BACKWARD 1
+/*   SATSPLAT_OPT_DEBUG_PLANES (0 default / 1): the forward calls also store the per-pixel visit / contribution counters that
+ *     satsplat_debug_planes returns (takes effect at the next forward). */
+#define SATSPLAT_OPT_DEBUG_PLANES 2
 #define SATSPLAT_BINNING_TILESORT 0
 #define SATSPLAT_BINNING_RADIX 1
 int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value);

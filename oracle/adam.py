@@ -14,8 +14,12 @@ Readings where the paper is silent (rows 19-20):
     (the paper lists none for opacity);
   * the library's scales are linear and must stay positive, so the scale group is stepped in log space:
     theta = log s, dL/dtheta = s dL/ds, s <- s exp(-lr m^/(sqrt(v^) + eps)); its Adam state is that of theta.
+  * per-camera groups ("0.0001 for camera delta matrices, and 0.001 for camera gain and bias"; Eq. 15 dF,
+    Eq. 1 [C | c] and the ambient term L_a): one training iteration renders ONE view, so only that view's rows receive a
+    gradient.  Reading: a view's rows, their Adam state and their step counter t_v advance only in the iterations that
+    render the view (per-view Adam; the other views' rows are untouched, not decayed) -- adam_step_cameras below.
 Pins: tests/test_oracle_pins.py P15 (first-step closed form, torch.optim.Adam as an independent routine, log-space
-equivalence).
+equivalence; per-camera groups: every view's subsequence of steps equals torch.optim.Adam run on that view alone).
 PARITY UNPINNED against the paper for the opacity learning rate, the betas and epsilon (arguments) and the log-space
 stepping of the scales.
 """
@@ -44,3 +48,28 @@ def adam_step(params, grads, state, lrs, *, beta1=0.9, beta2=0.999, eps=1e-8, st
         new_p[k] = p * np.exp(-upd) if k == "scales" else p - upd
         new_s[k] = (m, v)
     return new_p, new_s
+
+
+CAMERA_GROUPS = ("dF", "cc", "ambient")     # [V,8] camera deltas (Eq. 15), [V,12] gain and bias (Eq. 1), [V,3] ambient L_a
+
+
+def adam_step_cameras(params, grads, state, steps, view, lrs, *, beta1=0.9, beta2=0.999, eps=1e-8):
+    """One Adam step on the rows of view `view` of the per-camera groups.  `params`: dict of float64 arrays
+    [V,8] / [V,12] / [V,3] keyed by CAMERA_GROUPS; `grads`: dict group -> gradient of THAT view's row ([8] / [12] / [3]);
+    `state`: dict group -> (m, v), arrays shaped like the parameters; `steps`: int array [V], the number of steps each view
+    has taken so far; `lrs`: dict group -> learning rate.  Returns (new_params, new_state, new_steps); the rows of every
+    other view, their state and their counters come back unchanged.  Nothing is modified in place."""
+    steps = np.array(steps, np.int64, copy=True)
+    steps[view] += 1
+    t = int(steps[view])
+    c1, c2 = 1.0 - beta1 ** t, 1.0 - beta2 ** t
+    new_p, new_s = {}, {}
+    for k in CAMERA_GROUPS:
+        p = np.array(params[k], np.float64, copy=True)
+        m, v = (np.array(a, np.float64, copy=True) for a in state[k])
+        g = np.asarray(grads[k], np.float64).reshape(p.shape[1])
+        m[view] = beta1 * m[view] + (1.0 - beta1) * g
+        v[view] = beta2 * v[view] + (1.0 - beta2) * g * g
+        p[view] = p[view] - lrs[k] * (m[view] / c1) / (np.sqrt(v[view] / c2) + eps)
+        new_p[k], new_s[k] = p, (m, v)
+    return new_p, new_s, steps

@@ -18,6 +18,7 @@ _LIB = None
 OK, E_INVALID, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4
 OPT_BINNING, BINNING_TILESORT, BINNING_RADIX = 0, 0, 1
 OPT_SPLIT_BACKWARD = 1
+OPT_DEBUG_PLANES = 2
 STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_fwd", "blend_bwd", "chain_bwd")
 
 

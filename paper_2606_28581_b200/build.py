@@ -24,11 +24,19 @@ def _newest_dep() -> float:
     return max(os.path.getmtime(d) for d in deps)
 
 
+def _flags_stamp() -> str:
+    """Everything besides the sources that decides what the .so contains: a tuning build (SATSPLAT_NVCC_FLAGS=-D...) must not
+    survive as the library a later default test or bench run loads."""
+    return " ".join(NVCC_FLAGS + os.environ.get("SATSPLAT_NVCC_FLAGS", "").split() + SOURCES)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(OUT) and os.path.getmtime(OUT) >= _newest_dep():
+    objdir = os.path.join(HERE, "build")
+    stamp_file = os.path.join(objdir, "flags.stamp")
+    stamp_ok = os.path.exists(stamp_file) and open(stamp_file).read() == _flags_stamp()
+    if not force and stamp_ok and os.path.exists(OUT) and os.path.getmtime(OUT) >= _newest_dep():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
 
     def compile_one(src):
@@ -49,6 +57,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, OUT)
+    with open(stamp_file, "w") as f:
+        f.write(_flags_stamp())
     return OUT
 
 

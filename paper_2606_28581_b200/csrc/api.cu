@@ -179,7 +179,7 @@ void satsplat_destroy(satsplat_ctx* ctx) {
                   ctx->tile_start, ctx->worklist, ctx->wl_count, ctx->px_a,
                   ctx->px_b, ctx->px_i, ctx->px_visited, ctx->px_contrib, ctx->red_buf, ctx->e2e_in[0], ctx->e2e_in[1],
                   ctx->e2e_up[0], ctx->e2e_up[1], ctx->e2e_out[0], ctx->e2e_out[1], ctx->e2e_grads[0], ctx->e2e_grads[1],
-                  ctx->e2e_target[0], ctx->e2e_target[1], ctx->e2e_loss[0], ctx->e2e_loss[1]};
+                  ctx->e2e_target[0], ctx->e2e_target[1], ctx->e2e_loss[0], ctx->e2e_loss[1], ctx->e2e_sun};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (int i = 0; i < 2 * SATSPLAT_NUM_STAGES; ++i)
@@ -319,9 +319,13 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
 }
 
 namespace {
+// The blend half of a split backward accumulates per-surfel moment records with REDs and only the chain clears them: a
+// second blend backward, a new preprocess or an option change in between would leave stale moments for the next chain.
+const char* const kChainPendingMsg = "%s: a split backward is pending on this context; call satsplat_backward_chain first";
 // (a1) + (a2) on the context's current camera (host copy in ctx->cam, or the device record ctx->cam_dev)
 int preprocess_common(satsplat_ctx* ctx, int64_t N, const float* means, const float* quats, const float* scales,
                       const float* opacity_logits, const float* rgb, cudaStream_t s) {
+  if (ctx->chain_pending) return fail(ctx, SATSPLAT_E_STATE, kChainPendingMsg, "satsplat_preprocess");
   ctx->N = N;
   ctx->in_means = means; ctx->in_quats = quats; ctx->in_scales = scales; ctx->in_logits = opacity_logits;
   ctx->preprocessed = 0;
@@ -393,6 +397,7 @@ int forward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev,
 int backward_common(satsplat_ctx* ctx, const DevShading& sh, const float* sh_dev, const float* v_rgba, const float* v_geom,
                     const float* v_aux, float* v_means, float* v_quats, float* v_scales, float* v_opacity_logits, float* v_rgb,
                     float* v_dF, float* v_cc, float* v_ambient, float* v_sun_depth, float* v_reproj, cudaStream_t s) {
+  if (ctx->chain_pending) return fail(ctx, SATSPLAT_E_STATE, kChainPendingMsg, "satsplat_render_backward");
   clear_stage_marks(ctx, {6, 7});
   // the 23 epilogue sums (cc, ambient, reproj) are left in red_buf by the blend; the chain kernel's first CTA delivers them
   const bool epi = ctx->split_backward || v_cc || v_ambient || v_reproj;
@@ -498,6 +503,7 @@ int satsplat_shadow_map_backward(satsplat_ctx* ctx, const float* v_sun_depth, fl
   if (!v_sun_depth) return fail(ctx, SATSPLAT_E_INVALID, "satsplat_shadow_map_backward: v_sun_depth is NULL");
   if (!ctx->forwarded || !ctx->depth_only)
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_shadow_map_backward: call satsplat_shadow_map first");
+  if (ctx->chain_pending) return fail(ctx, SATSPLAT_E_STATE, kChainPendingMsg, "satsplat_shadow_map_backward");
   cudaStream_t s = (cudaStream_t)stream;
   CU(cudaSetDevice(ctx->device));
   const DevShading sh = make_shading(nullptr);
@@ -636,6 +642,8 @@ int satsplat_debug_records(satsplat_ctx* ctx, float* records_out, uint8_t* flags
 int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const int32_t** n_contrib) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_debug_planes: ctx is NULL");
   if (!ctx->forwarded) return fail(ctx, SATSPLAT_E_STATE, "satsplat_debug_planes: no forward pass yet");
+  if (!ctx->planes_valid)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_debug_planes: the last forward ran without SATSPLAT_OPT_DEBUG_PLANES = 1");
   if (n_visited) *n_visited = ctx->px_visited;
   if (n_contrib) *n_contrib = ctx->px_contrib;
   return SATSPLAT_OK;
@@ -644,8 +652,12 @@ int satsplat_debug_planes(satsplat_ctx* ctx, const int32_t** n_visited, const in
 int satsplat_set_option(satsplat_ctx* ctx, int32_t option, int32_t value) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_set_option: ctx is NULL");
   if (option == SATSPLAT_OPT_SPLIT_BACKWARD && (value == 0 || value == 1)) {
+    if (ctx->chain_pending) return fail(ctx, SATSPLAT_E_STATE, kChainPendingMsg, "satsplat_set_option");
     ctx->split_backward = value;
-    ctx->chain_pending = 0;
+    return SATSPLAT_OK;
+  }
+  if (option == SATSPLAT_OPT_DEBUG_PLANES && (value == 0 || value == 1)) {
+    ctx->debug_planes = value;
     return SATSPLAT_OK;
   }
   if (option == SATSPLAT_OPT_BINNING && (value == SATSPLAT_BINNING_TILESORT || value == SATSPLAT_BINNING_RADIX)) {
@@ -691,26 +703,56 @@ inline Pack pack_offsets(size_t n) {
 }
 }  // namespace
 
+namespace {
+// frees whatever a failed satsplat_reserve_host_staging left behind, so that a retry starts from nothing
+void release_staging(satsplat_ctx* ctx) {
+  float** bufs[] = {ctx->e2e_in, ctx->e2e_up, ctx->e2e_out, ctx->e2e_grads, ctx->e2e_target, ctx->e2e_loss};
+  for (float** b : bufs)
+    for (int k = 0; k < 2; ++k)
+      if (b[k]) { cudaFree(b[k]); b[k] = nullptr; }
+  for (int k = 0; k < 2; ++k)
+    for (int i = 0; i < 6; ++i)
+      if (ctx->e2e_ev[k][i]) { cudaEventDestroy(ctx->e2e_ev[k][i]); ctx->e2e_ev[k][i] = nullptr; }
+  for (int i = 0; i < 3; ++i)
+    if (ctx->e2e_stream[i]) { cudaStreamDestroy(ctx->e2e_stream[i]); ctx->e2e_stream[i] = nullptr; }
+}
+
+cudaError_t allocate_staging(satsplat_ctx* ctx) {
+  const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
+  const Pack pk = pack_offsets((size_t)ctx->max_surfels);
+  cudaError_t e;
+#define TRY(call) if ((e = (call)) != cudaSuccess) return e
+  for (int k = 0; k < 2; ++k) {
+    TRY(dalloc(ctx, &ctx->e2e_in[k], pk.off[5] + 4));
+    TRY(dalloc(ctx, &ctx->e2e_up[k], mpx * 12));
+    TRY(dalloc(ctx, &ctx->e2e_out[k], mpx * 12));
+    TRY(dalloc(ctx, &ctx->e2e_grads[k], pk.off[5] + 64));
+    TRY(dalloc(ctx, &ctx->e2e_target[k], mpx * 4));
+    TRY(dalloc(ctx, &ctx->e2e_loss[k], (size_t)satsplat_loss_scratch_floats(ctx->max_w, ctx->max_h)));
+    for (int i = 0; i < 6; ++i) TRY(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
+  }
+  for (int i = 0; i < 3; ++i) TRY(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
+#undef TRY
+  return cudaSuccess;
+}
+}  // namespace
+
 int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
   if (!ctx) return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_reserve_host_staging: ctx is NULL");
   CU(cudaSetDevice(ctx->device));
-  if (!ctx->e2e_in[0]) {
-    const size_t mpx = (size_t)ctx->max_w * ctx->max_h;
-    const Pack pk = pack_offsets((size_t)ctx->max_surfels);
-    for (int k = 0; k < 2; ++k) {
-      CU(dalloc(ctx, &ctx->e2e_in[k], pk.off[5] + 4));
-      CU(dalloc(ctx, &ctx->e2e_up[k], mpx * 12));
-      CU(dalloc(ctx, &ctx->e2e_out[k], mpx * 12));
-      CU(dalloc(ctx, &ctx->e2e_grads[k], pk.off[5] + 64));
-      CU(dalloc(ctx, &ctx->e2e_target[k], mpx * 4));
-      CU(dalloc(ctx, &ctx->e2e_loss[k], (size_t)satsplat_loss_scratch_floats(ctx->max_w, ctx->max_h)));
-      for (int i = 0; i < 6; ++i) CU(cudaEventCreateWithFlags(&ctx->e2e_ev[k][i], cudaEventDisableTiming));
+  if (!ctx->staging_ready) {
+    const int64_t before = ctx->scratch_bytes;
+    const cudaError_t e = allocate_staging(ctx);
+    if (e != cudaSuccess) {      // nothing half-built survives: a later call tries again from scratch
+      release_staging(ctx);
+      ctx->scratch_bytes = before;
+      return fail(ctx, SATSPLAT_E_CUDA, "satsplat_reserve_host_staging: %s", cudaGetErrorString(e));
     }
-    for (int i = 0; i < 3; ++i) CU(cudaStreamCreateWithFlags(&ctx->e2e_stream[i], cudaStreamNonBlocking));
+    ctx->staging_ready = 1;
   }
-  if (sun_ctx && !sun_ctx->e2e_out[0]) {
+  if (sun_ctx && !sun_ctx->e2e_sun) {   // its own field: a context may serve as view context and as sun context
     const size_t mpx = (size_t)sun_ctx->max_w * sun_ctx->max_h;
-    const cudaError_t e = dalloc(sun_ctx, &sun_ctx->e2e_out[0], mpx * 2);   // sun map + its gradient
+    const cudaError_t e = dalloc(sun_ctx, &sun_ctx->e2e_sun, mpx * 2);   // sun map + its gradient
     if (e != cudaSuccess) return fail(ctx, SATSPLAT_E_CUDA, "satsplat_reserve_host_staging: %s", cudaGetErrorString(e));
   }
   return SATSPLAT_OK;
@@ -719,7 +761,7 @@ int satsplat_reserve_host_staging(satsplat_ctx* ctx, satsplat_ctx* sun_ctx) {
 // One step with host buffers.  lw == NULL: the upstream gradients come from the host (h_v_*); lw != NULL (training step):
 // they are written on the device by the loss stage from the rendered images and the uploaded target, and the loss sums
 // come back with the gradients.
-static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+static int host_step_enqueue(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
                            const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
                            const float* h_means, const float* h_quats, const float* h_scales,
                            const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
@@ -740,9 +782,13 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
     if (N > sun_ctx->max_surfels || sun->width <= 0 || sun->height <= 0 || sun->width > sun_ctx->max_w || sun->height > sun_ctx->max_h)
       return fail(ctx, SATSPLAT_E_INVALID, "satsplat_iteration_host: sun map size or N exceeds the sun context");
   }
-  if (!ctx->e2e_in[0] || (shadows && !sun_ctx->e2e_out[0]))
+  if (!ctx->staging_ready || (shadows && !sun_ctx->e2e_sun))
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: call satsplat_reserve_host_staging first");
   if (ctx->e2e_busy[slot]) return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host_begin: slot still in flight (call _end)");
+  // the two slots share the contexts' scratch (records, lists, per-pixel state, moment records, the sun map): their kernels
+  // are ordered only by running on ONE stream
+  if (ctx->e2e_busy[slot ^ 1] && ctx->e2e_caller[slot ^ 1] != (cudaStream_t)stream)
+    return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host_begin: the step in flight on the other slot was begun on a different stream");
   if (ctx->split_backward || (shadows && sun_ctx->split_backward))
     return fail(ctx, SATSPLAT_E_STATE, "satsplat_iteration_host: the contexts are in SATSPLAT_OPT_SPLIT_BACKWARD mode");
   cudaStream_t s = (cudaStream_t)stream;
@@ -801,7 +847,7 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
     CU(cudaStreamWaitEvent(s_view, ev[5], 0));
     if ((rc = satsplat_preprocess(ctx, cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], (satsplat_stream)s_view))) return rc;
     CU(cudaEventRecord(ev[5], s_view));
-    d_sun = sun_ctx->e2e_out[0];
+    d_sun = sun_ctx->e2e_sun;
     d_vsun = d_sun + (size_t)sun_ctx->max_w * sun_ctx->max_h;
     if ((rc = satsplat_preprocess(sun_ctx, &sun_cam, N, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], stream))) return rc;
     if ((rc = satsplat_shadow_map(sun_ctx, d_sun, stream))) return rc;
@@ -843,7 +889,27 @@ static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slo
   if (lw) CU(cudaMemcpyAsync(h_sums, d_sums, 8 * sizeof(float), cudaMemcpyDeviceToHost, s_down));
   CU(cudaEventRecord(ev[4], s_down));
   ctx->e2e_busy[slot] = 1;
+  ctx->e2e_caller[slot] = s;
   return SATSPLAT_OK;
+}
+
+// A failure after the first copy was enqueued (a refused preprocess, a CUDA error) would leave asynchronous copies from and to
+// the caller's buffers in flight on a slot that is not marked busy: drain the queues before reporting it, so that the caller
+// may free or reuse its buffers as soon as _begin has returned an error.
+static int host_step_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,
+                           const satsplat_sun* sun, const satsplat_shading* shading, int64_t N,
+                           const float* h_means, const float* h_quats, const float* h_scales,
+                           const float* h_logits, const float* h_rgb, const float* h_v_rgba, const float* h_v_geom,
+                           const float* h_v_aux, float* h_out_rgba, float* h_out_geom, float* h_out_aux,
+                           float* h_grads, const satsplat_loss_weights* lw, const float* h_target, float* h_sums,
+                           satsplat_stream stream) {
+  const int rc = host_step_enqueue(ctx, sun_ctx, slot, cam, sun, shading, N, h_means, h_quats, h_scales, h_logits, h_rgb, h_v_rgba,
+                                   h_v_geom, h_v_aux, h_out_rgba, h_out_geom, h_out_aux, h_grads, lw, h_target, h_sums, stream);
+  if (rc != SATSPLAT_OK && ctx && ctx->staging_ready) {
+    for (int i = 0; i < 3; ++i) cudaStreamSynchronize(ctx->e2e_stream[i]);
+    cudaStreamSynchronize((cudaStream_t)stream);
+  }
+  return rc;
 }
 
 int satsplat_iteration_host_begin(satsplat_ctx* ctx, satsplat_ctx* sun_ctx, int32_t slot, const satsplat_camera* cam,

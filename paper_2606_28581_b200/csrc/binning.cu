@@ -121,8 +121,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(int N, const u
 cudaError_t launch_scan(satsplat_ctx* c, int64_t N, cudaStream_t s) {
   const int nblocks = (int)((N + kScanTile - 1) / kScanTile);
   if (nblocks == 0) {
-    cudaMemsetAsync(c->status, 0, sizeof(Status), s);
-    return cudaMemsetAsync(c->offset, 0, sizeof(uint32_t), s);
+    const cudaError_t e = cudaMemsetAsync(c->status, 0, sizeof(Status), s);
+    return e != cudaSuccess ? e : cudaMemsetAsync(c->offset, 0, sizeof(uint32_t), s);
   }
   g_kernel_launches += 3;
   scan_block_sums_kernel<<<nblocks, kScanThreads, 0, s>>>((int)N, c->count, c->block_sums);
@@ -360,7 +360,8 @@ __global__ void __launch_bounds__(256) ranges_kernel(const Status* __restrict__ 
 
 cudaError_t launch_ranges(satsplat_ctx* c, cudaStream_t s) {
   const int tiles = c->cam.TX * c->cam.TY;
-  cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
+  const cudaError_t e = cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
+  if (e != cudaSuccess) return e;
   ++g_kernel_launches;
   ranges_kernel<<<c->sm_count * 8, 256, 0, s>>>(c->status, (uint32_t)c->max_dup, c->keys[c->sorted], c->ranges);
   return cudaGetLastError();
@@ -795,18 +796,25 @@ cudaError_t launch_tile_sort(satsplat_ctx* c, cudaStream_t s) {
   g_kernel_launches += 4;
   // the four kernels work on disjoint tiles (the worklists come from the scan): the long lists are sorted on a second
   // stream beside the many short ones
-  cudaEventRecord(c->bin_ev[0], s);
-  cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
+  // a failed fork would let the side-stream sorts race the scatter on keys[1], a failed join would let the blend read
+  // unsorted lists: every event call is checked
+  cudaError_t e = cudaEventRecord(c->bin_ev[0], s);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->bin_stream, c->bin_ev[0], 0);
+  if (e != cudaSuccess) return e;
   tile_sort_merge_kernel<4><<<c->sm_count * 8, 128, 2 * 256 * 4 * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
                                                                                       c->worklist, c->wl_count + 0);
   tile_sort_merge_kernel<16><<<c->sm_count * 2, 512, 2 * 256 * 16 * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
                                                                                         c->worklist + tiles, c->wl_count + 1);
   tile_sort_large_kernel<<<(c->sm_count + 1) / 2, 1024, kTileSortCtaMax * 8, c->bin_stream>>>(c->ranges, c->keys[1], c->keys[0], c->vals[0],
                                                                                                c->worklist + 2 * (size_t)tiles, c->wl_count);
-  cudaEventRecord(c->bin_ev[1], c->bin_stream);
+  e = cudaEventRecord(c->bin_ev[1], c->bin_stream);
   tile_sort_kernel<<<(tiles + kTileSortWarps - 1) / kTileSortWarps, kTileSortWarps * 32, 0, s>>>(tiles, c->ranges, c->keys[1], c->keys[0],
                                                                                                  c->vals[0], c->tile_count);
-  cudaStreamWaitEvent(s, c->bin_ev[1], 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s, c->bin_ev[1], 0);
+  if (e != cudaSuccess) {   // no join: do not let the caller's stream run ahead of the side-stream sorts
+    cudaStreamSynchronize(c->bin_stream);
+    return e;
+  }
   c->sorted = 0;
   return cudaGetLastError();
 }

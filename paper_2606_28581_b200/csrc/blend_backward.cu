@@ -434,7 +434,10 @@ cudaError_t launch_blend_backward(satsplat_ctx* c, const DevShading& sh, const f
   P.v_sun_depth = v_sun_depth;
   const bool want_red = !depth_only && want_epilogue_sums;
   P.red = want_red ? c->red_buf : nullptr;
-  if (want_red) cudaMemsetAsync(c->red_buf, 0, kRedCopies * 32 * sizeof(float), s);
+  if (want_red) {
+    const cudaError_t e = cudaMemsetAsync(c->red_buf, 0, kRedCopies * 32 * sizeof(float), s);
+    if (e != cudaSuccess) return e;
+  }
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsB));
   constexpr int kPairBytes = kPairBytesB;
   ++g_kernel_launches;

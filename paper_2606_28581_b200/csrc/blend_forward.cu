@@ -273,8 +273,10 @@ __global__ void __launch_bounds__(kThreadsF, SATSPLAT_FWD_MINB) blend_forward_ke
     P.px_b[o] = make_float4(al0, al1, al2, V);
     P.px_i[o] = make_int2(last, mi);
   }
-  P.px_visited[o] = visited;
-  P.px_contrib[o] = ncontrib;
+  if (P.px_visited) {   // SATSPLAT_OPT_DEBUG_PLANES: instrumentation, not part of the method
+    P.px_visited[o] = visited;
+    P.px_contrib[o] = ncontrib;
+  }
 }
 
 cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, const float* sh_dev, float* out_rgba, float* out_geom,
@@ -295,8 +297,9 @@ cudaError_t launch_blend_forward(satsplat_ctx* c, const DevShading& sh, const fl
   P.px_a = c->px_a;
   P.px_b = c->px_b;
   P.px_i = c->px_i;
-  P.px_visited = c->px_visited;
-  P.px_contrib = c->px_contrib;
+  P.px_visited = c->debug_planes ? c->px_visited : nullptr;
+  P.px_contrib = c->debug_planes ? c->px_contrib : nullptr;
+  c->planes_valid = c->debug_planes;
   const dim3 grid(c->cam.TX, c->cam.TY * (8 / kWarpsF));
   ++g_kernel_launches;
   const bool dev = c->cam_dev != nullptr;   // the view's shading record travels with a device camera (sh_dev is NULL for depth-only passes)

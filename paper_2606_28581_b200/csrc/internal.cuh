@@ -231,6 +231,8 @@ struct satsplat_ctx {
   int32_t* px_last;       // planes for debug/statistics
   int32_t* px_visited;
   int32_t* px_contrib;
+  int debug_planes;       // SATSPLAT_OPT_DEBUG_PLANES: the forward stores px_visited / px_contrib
+  int planes_valid;       // ... and the last forward did
   float* red_buf;         // small reduction scratch (dF, cc, ambient, reproj)
   // host state
   satsplat::DevCamera cam;
@@ -242,13 +244,16 @@ struct satsplat_ctx {
   // host-buffer iteration (satsplat_iteration_host*): two staging slots so that the copies of consecutive steps overlap
   float* e2e_in[2];       // means..rgb, sub-arrays at 16-byte aligned offsets
   float* e2e_up[2];       // upstream gradients (3 images)
-  float* e2e_out[2];      // images (view ctx); slot 0 of a sun ctx: sun map + its gradient
+  float* e2e_out[2];      // images
   float* e2e_grads[2];    // surfel gradient groups + dF cc ambient reproj dF_sun, loss sums (8) at + 48
   float* e2e_target[2];   // training step: target image
   float* e2e_loss[2];     // training step: scratch of the loss stage
   cudaStream_t e2e_stream[3];   // uploads / downloads / view-pass preprocess, beside the caller's stream
   cudaEvent_t e2e_ev[2][6];     // per slot: surfels up, upstream up, forward done, backward done, everything down, view preprocess done
   int e2e_busy[2];              // slot has a begin without its end
+  cudaStream_t e2e_caller[2];   // the caller's stream of the step in flight on a slot (both slots must use the same one)
+  int staging_ready;            // satsplat_reserve_host_staging allocated everything above (set last, after the last success)
+  float* e2e_sun;               // sun-context role: sun map + its gradient
   // profiling
   int profiling;
   cudaEvent_t ev[2 * SATSPLAT_NUM_STAGES];

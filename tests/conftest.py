@@ -18,3 +18,20 @@ def orc():
     from oracle import oracle
     oracle.build()
     return oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _gradient_bar_log():
+    """After a GPU session: what share of each gradient group lay outside the literal 1e-3 / 1e-5 tolerance and how large a
+    rounding allowance c those elements needed (tests/gpu_util.compare_grads) -> gpurun_out/gradient_bar.json (scratch; the
+    committed summary is profiles/r3_gradient_bar.md)."""
+    yield
+    try:
+        import json
+        import gpu_util
+        if gpu_util.BAR_LOG:
+            os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+            with open(os.path.join(ROOT, "gpurun_out", "gradient_bar.json"), "w") as f:
+                json.dump(gpu_util.BAR_LOG, f, indent=0)
+    except Exception:      # never fail a test session over the log
+        pass

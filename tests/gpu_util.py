@@ -43,6 +43,7 @@ def gpu_view_iteration(P, gs: GpuScene, view, *, sun_view=None, reproj=None, ups
         own.append(ctx)
     if binning is not None:
         ctx.set_option(P.OPT_BINNING, binning)
+    ctx.set_option(P.OPT_DEBUG_PLANES, 1 if want_debug else 0)
     sun_depth = None
     if sun_view is not None:
         if sun_ctx is None:
@@ -144,10 +145,16 @@ def compare_images(gpu, ref, fragile, *, atol=1e-5, rtol=1e-4, names=("rgba", "g
 
 
 EPS32 = 2.0 ** -24      # unit roundoff of fp32 (round to nearest)
-C_ROUND = 256.0         # DESIGN.md section 3 "Gradient bar": roundings a per-pair term passes through, worst case
+C_ROUND = 128.0         # DESIGN.md section 3 "Gradient bar": the largest c any element has needed is 94 (profiles/r3_gradient_bar.md)
+C_ROUND_SHADOW = 256.0  # view backward through the soft shadow test: the derivation's worst case (beside the conditioning term)
 
 
-def compare_grads(gpu, ref, twin, pairs, *, atol=1e-5, rtol=1e-3, c=C_ROUND, extra=None, exempt=None):
+BAR_LOG = []            # one record per (label, gradient group): how much of the third term each comparison used
+MAX_BEYOND_PLAIN = 1e-3  # masked runs: share of a group's elements that may lie outside the literal north_star tolerance
+
+
+def compare_grads(gpu, ref, twin, pairs, *, atol=1e-5, rtol=1e-3, c=C_ROUND, extra=None, exempt=None, label=None,
+                  max_beyond_plain_frac=None):
     """Gradient bar (north_star + DESIGN.md section 3), ONE rule for every gradient the path produces:
 
         |gpu - ref| <= atol + rtol |ref| + c 2^-24 S        element by element,
@@ -157,7 +164,10 @@ def compare_grads(gpu, ref, twin, pairs, *, atol=1e-5, rtol=1e-3, c=C_ROUND, ext
     most c singly rounded operations.  No share of elements may miss it.  `pairs`: (gpu key, ref key, twin key).
     `extra[gpu key]`: a further additive tolerance array computed by the ORACLE (shadow stage: the twin of the
     conditioning of the shadow lookup).  `exempt[gpu key]`: boolean array of elements that may miss the bar
-    (unmasked runs only: rows of surfels touched by a fragile pixel); returned in the statistics."""
+    (unmasked runs only: rows of surfels touched by a fragile pixel); returned in the statistics.
+    `max_beyond_plain_frac`: the third term is the exception, not the bar: at most this share of the elements of a group of
+    1000 elements or more may lie outside the literal `atol + rtol |ref|` (asserted; smaller groups are whole-image sums and
+    are recorded only).  Every call with a `label` is recorded in BAR_LOG (written to gpurun_out/ at session end)."""
     stats = {}
     for kg, kr, kt in pairs:
         g = gpu[kg].astype(np.float64)
@@ -178,6 +188,15 @@ def compare_grads(gpu, ref, twin, pairs, *, atol=1e-5, rtol=1e-3, c=C_ROUND, ext
         need = np.where(S > 0, (err - plain) / (EPS32 * np.maximum(S, 1e-300)), 0.0)
         stats[kg] = dict(max_err_over_tol=float((err / tol).max()) if g.size else 0.0, beyond_plain=int((err > plain).sum()),
                          c_needed=float(need.max()) if g.size else 0.0, exempt_bad=n_exempt)
+        over = need[err > plain]
+        if label is not None:
+            BAR_LOG.append(dict(label=label, group=kg, elements=int(g.size), beyond_plain=stats[kg]["beyond_plain"],
+                                share=stats[kg]["beyond_plain"] / max(g.size, 1), c_needed_max=stats[kg]["c_needed"],
+                                c_needed_p50=float(np.percentile(over, 50)) if over.size else 0.0,
+                                c_needed_p99=float(np.percentile(over, 99)) if over.size else 0.0, c_allowed=float(c),
+                                has_extra=bool(extra is not None and kg in extra), exempt_bad=n_exempt))
+        if max_beyond_plain_frac is not None and g.size >= 1000:
+            assert stats[kg]["beyond_plain"] <= max_beyond_plain_frac * g.size, (kg, "too many elements beyond the plain tolerance", stats[kg], g.size)
         if bad.any():
             i = int(np.argmax(np.where(bad, err / tol, 0).reshape(-1)))
             raise AssertionError((kg, "elements outside the bar", int(bad.sum()), g.size, stats[kg], g.reshape(-1)[i], r.reshape(-1)[i],

@@ -112,7 +112,7 @@ def test_binning_and_records_bitexact(P, G, orc, cfg):
         assert res["K"] == len(ref["keys"]) > 0
 
 
-@pytest.mark.parametrize("cfg", ["C0_ragged", "C1s", "C4s"])
+@pytest.mark.parametrize("cfg", ["C0_ragged", "C1s", "C4s", "C3full", "C4full"])
 def test_binning_radix_mode_bitexact(P, G, orc, cfg):
     """The general-purpose path (per-surfel scan, key duplication, stable LSD radix sort, range detection) gives the
     same bits as the default tile-sort path and the oracle."""
@@ -172,8 +172,9 @@ def test_forward_backward_parity(P, G, orc, cfg):
             u[fragile] = 0
         refb = orc.view_iteration(scene, view, upstream=upm, threads=nth, twin=True)
         resb = G.gpu_view_iteration(P, gs, view, upstream=upm, want_debug=False)
-        gstats = G.compare_grads(resb["grads"], refb["grads"], refb["grads"], G.GRAD_PAIRS)
-        gstats.update(G.compare_grads(resb["grads"], refb["bwd"], refb["bwd"], G.EPI_PAIRS))
+        gstats = G.compare_grads(resb["grads"], refb["grads"], refb["grads"], G.GRAD_PAIRS, label=f"{cfg} view {vi} masked",
+                                 max_beyond_plain_frac=G.MAX_BEYOND_PLAIN)
+        gstats.update(G.compare_grads(resb["grads"], refb["bwd"], refb["bwd"], G.EPI_PAIRS, label=f"{cfg} view {vi} masked"))
         # ---- unmasked: a pixel whose decision flips moves the gradients of the surfels it touches.  SURVEY 8(c) F: every
         # element outside the bar belongs to a surfel touched by a fragile pixel, and they are <= 1e-4 of all elements ----
         refu = orc.view_iteration(scene, view, upstream=up, threads=nth, twin=True)
@@ -267,9 +268,11 @@ def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
                             g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"], v_sun, g["v_reproj"])
         gn = {k: v.cpu().numpy() for k, v in g.items()}
         gn["v_sun_depth"] = v_sun.cpu().numpy()
-        gst = G.compare_grads(gn, refb["grads"], refb["grads"], G.GRAD_PAIRS, extra={k[0]: refk["grads"][k[2]] for k in G.GRAD_PAIRS})
+        gst = G.compare_grads(gn, refb["grads"], refb["grads"], G.GRAD_PAIRS, extra={k[0]: refk["grads"][k[2]] for k in G.GRAD_PAIRS},
+                              label=f"{cfg} view {vi} shadow view-backward", c=G.C_ROUND_SHADOW)
         epi = G.EPI_PAIRS + [("v_reproj", "v_reproj", "a_reproj"), ("v_sun_depth", "v_sun_depth", "a_sun_depth")]
-        gst.update(G.compare_grads(gn, refb["bwd"], refb["bwd"], epi, extra={k[0]: refk["bwd"][k[2]] for k in epi}))
+        gst.update(G.compare_grads(gn, refb["bwd"], refb["bwd"], epi, extra={k[0]: refk["bwd"][k[2]] for k in epi},
+                                   label=f"{cfg} view {vi} shadow view-backward", c=G.C_ROUND_SHADOW))
         vs_ref = refb["bwd"]["v_sun_depth"]
         assert np.abs(vs_ref).max() > 0
         ctx.close()
@@ -293,7 +296,8 @@ def test_shadow_pass_parity_by_stage(P, G, orc, cfg):
         g2n = {k: v.cpu().numpy() for k, v in g2.items()}
         sst = G.compare_grads(g2n, gsr, gsr, [("v_means", "v_means", "a_means"), ("v_quats", "v_quats", "a_quats"),
                                               ("v_scales", "v_scales", "a_scales"), ("v_logits", "v_logits", "a_logits"),
-                                              ("v_dF_sun", "v_dF", "a_dF")])
+                                              ("v_dF_sun", "v_dF", "a_dF")], label=f"{cfg} view {vi} sun-backward",
+                              max_beyond_plain_frac=G.MAX_BEYOND_PLAIN)
         sctx.close()
         print(cfg, vi, "fragile", int(fragile.sum()), "sun fragile", int(sfrag.sum()), stats,
               {k: (round(v["c_needed"], 1), v["beyond_plain"], round(v["max_err_over_tol"], 3)) for k, v in gst.items()},
@@ -544,11 +548,18 @@ def test_cascade_total_camera_delta_gradient(P, G, orc):
         upm = [u.copy() for u in up]
         for u in upm:
             u[fragile] = 0
-        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth)
+        refb = orc.view_iteration(scene, view, upstream=upm, threads=nth, twin=True)
         Fp = (view.F.astype(np.float32) + view.dF.astype(np.float32)).astype(np.float64).reshape(8)
-        cas_ref = orc.sun_camera_backward(Fp, view.sun_azimuth, view.sun_elevation, view.sun_viewport,
-                                          refb["sun_grads"]["v_dF"], refb["bwd"]["v_reproj"])
-        tot_ref = refb["grads"]["v_dF"] + cas_ref
+        cascade = lambda v_F_sun, v_rep: np.asarray(orc.sun_camera_backward(Fp, view.sun_azimuth, view.sun_elevation, view.sun_viewport,
+                                                                            v_F_sun, v_rep), np.float64).reshape(8)
+        cas_ref = cascade(refb["sun_grads"]["v_dF"], refb["bwd"]["v_reproj"])
+        tot_ref = np.asarray(refb["grads"]["v_dF"], np.float64).reshape(8) + cas_ref
+        # twin of the total: the cascade adjoint is linear, so its absolute-value Jacobian (one oracle call per unit vector)
+        # carries the twins of its two inputs; the view pass's own twin is added
+        eye = np.eye(8)
+        J = np.stack([cascade(eye[k], np.zeros(8)) for k in range(8)] + [cascade(np.zeros(8), eye[k]) for k in range(8)], axis=1)
+        a_in = np.concatenate([np.asarray(refb["sun_grads"]["a_dF"], np.float64).reshape(8), np.asarray(refb["bwd"]["a_reproj"], np.float64).reshape(8)])
+        tot_twin = np.asarray(refb["grads"]["a_dF"], np.float64).reshape(8) + np.abs(J) @ a_in
         res = G.gpu_view_iteration(P, gs, view, sun_view=ref["sun_view"], reproj=ref["reproj"], upstream=upm, want_debug=False)
         tot = G.t(res["grads"]["v_dF"])
         P.sun_camera_backward(P.Camera.from_view(view), view.sun_azimuth, view.sun_elevation, view.sun_viewport,
@@ -557,8 +568,11 @@ def test_cascade_total_camera_delta_gradient(P, G, orc):
         got = tot.cpu().numpy().astype(np.float64)
         scale = np.abs(tot_ref).max()
         assert np.abs(cas_ref).max() > 1e-3 * scale                      # the cascade term is not negligible here
-        assert np.abs(got - tot_ref).max() <= 1e-2 * scale, (got, tot_ref, cas_ref)
-        print("cascade", vi, "total", tot_ref, "err/scale", np.abs(got - tot_ref).max() / scale)
+        # the one gradient bar of this file, element by element (the shadow lookup's conditioning term of
+        # test_shadow_pass_parity_by_stage does not apply: the GPU view backward reads the GPU's own sun map here, so that
+        # term is replaced by the oracle's twin of v_reproj, which the cascade carries)
+        st = G.compare_grads(dict(tot=got), dict(tot=tot_ref), dict(tot=tot_twin), [("tot", "tot", "tot")], label=f"cascade total dF view {vi}")
+        print("cascade", vi, "total", tot_ref, "err/scale", np.abs(got - tot_ref).max() / scale, st)
 
 
 @pytest.mark.parametrize("n", [1, 5, 1023, 40001])
@@ -1038,6 +1052,71 @@ def test_device_camera_path_equals_host_path_and_one_graph_serves_all_views(P, G
         c.close()
 
 
+def test_nearby_view_pass_backward_reaches_dF(P, G, orc):
+    """PAPER.md:176 / Fig. 1 carried through its backward: the nearby camera is built on the device from F' = F + dF, the
+    scene is rendered from it, its backward gives the gradient with respect to the nearby camera's 2x4 matrix, and
+    satsplat_camera_chain_backward(v_F_nearby) pulls that back into the view's row of dF.  Against the oracle at every step:
+    orc_backward + orc_preprocess_backward on the oracle's nearby camera (surfel gradients and v_dF of that camera, the one
+    gradient bar), then orc_nearby_camera_backward applied to the ORACLE's own v_dF (twin: |Jacobian| times the oracle's twin)."""
+    import torch
+    scene = S.make_config(2, n=6000, size=128, n_views=2, extent=40.0, sun_size=192)
+    gs = G.GpuScene(scene)
+    n, nth = scene.n, orc.num_threads()
+    view = scene.views[1]
+    W, H = view.width, view.height
+    nearby = [(0.0, 0.0), (0.03, -0.02)]
+    table, dF_all, idx, block = _chain_setup(P, G, scene, nearby)
+    idx.fill_(1)
+    P.camera_chain(table, dF_all, idx, block)
+    surf = (gs.means, gs.quats, gs.scales, gs.logits, gs.rgb)
+    nctx = P.Context(n, W, H, 16 * n)
+    nctx.preprocess_device(W, H, block, P.CAM_NEARBY, *surf)
+    nout = [torch.empty(H, W, 4, device="cuda") for _ in range(3)]
+    nctx.render_forward_device(block, None, *nout)
+    # the oracle's nearby view: its own camera construction (the kernels' fp32 camera is checked against it, then used as the
+    # fp32 input both sides consume, as for every other camera of this file)
+    Fp32 = view.F.astype(np.float32) + view.dF.astype(np.float32)
+    Fn_ref, ang = orc.nearby_camera(Fp32.astype(np.float64), *nearby[1])
+    nv = _no_shadow(view)
+    nv.F, nv.dF = np.asarray(Fn_ref, np.float64).astype(np.float32), np.zeros(8, np.float32)
+    np.testing.assert_allclose(block[32:40].cpu().numpy(), nv.F, rtol=2e-6, atol=2e-6 * np.abs(Fn_ref).max())
+    a2, e2 = ang[0] + nearby[1][0], ang[1] + nearby[1][1]
+    nv.view_dir = (-np.array([np.cos(a2) * np.cos(e2), np.sin(a2) * np.cos(e2), np.sin(e2)])).astype(np.float32)
+    if not np.array_equal(block[32:40].cpu().numpy(), nv.F):
+        # an ulp of difference between the device-built camera and the rounded oracle camera: render what the oracle rendered
+        block[32:40] = G.t(nv.F)
+        nctx.preprocess_device(W, H, block, P.CAM_NEARBY, *surf)
+        nctx.render_forward_device(block, None, *nout)
+    up = S.upstream_grads(scene.seed, 1, H, W)
+    ref = orc.view_iteration(scene, nv, do_backward=False, threads=nth)
+    fragile = G.fragile_mask(ref["fwd"]["margins"])
+    gpu = dict(rgba=nout[0].cpu().numpy(), geom=nout[1].cpu().numpy(), aux=nout[2].cpu().numpy())
+    G.compare_images(gpu, ref["fwd"], fragile)
+    upm = [u.copy() for u in up]
+    for u in upm:
+        u[fragile] = 0
+    refb = orc.view_iteration(scene, nv, upstream=upm, threads=nth, twin=True)
+    g = gs.zeros_grads()
+    nctx.render_backward_device(block, None, G.t(upm[0]), G.t(upm[1]), G.t(upm[2]), g["v_means"], g["v_quats"], g["v_scales"],
+                                g["v_logits"], g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"], None, None)
+    gn = {k: v.cpu().numpy() for k, v in g.items()}
+    G.compare_grads(gn, refb["grads"], refb["grads"], G.GRAD_PAIRS, label="nearby view backward")
+    assert np.abs(refb["grads"]["v_dF"]).max() > 0
+    # ---- into dF ----
+    v_all = torch.zeros_like(dF_all)
+    P.camera_chain_backward(table, dF_all, idx, None, None, None, g["v_dF"], v_all)
+    torch.cuda.synchronize()
+    pull = lambda v: np.asarray(orc.nearby_camera_backward(Fp32.astype(np.float64), nearby[1][0], nearby[1][1], v), np.float64).reshape(8)
+    dF_ref = pull(np.asarray(refb["grads"]["v_dF"], np.float64).reshape(8))
+    J = np.stack([pull(e) for e in np.eye(8)], axis=1)
+    twin = np.abs(J) @ np.asarray(refb["grads"]["a_dF"], np.float64).reshape(8)
+    got = v_all.cpu().numpy().astype(np.float64)
+    assert np.abs(dF_ref).max() > 0 and (got[0] == 0).all()
+    st = G.compare_grads(dict(t=got[1]), dict(t=dF_ref), dict(t=twin), [("t", "t", "t")], label="nearby view -> dF")
+    print("nearby -> dF", dF_ref, got[1], st)
+    nctx.close()
+
+
 def test_split_backward_equals_unsplit(P, G, orc):
     """SATSPLAT_OPT_SPLIT_BACKWARD: blend half + satsplat_backward_chain give what the one-call backward gives (view pass with
     the epilogue sums, depth-only sun pass), with the view chain on a second stream beside the sun blend as bench.py runs it."""
@@ -1068,10 +1147,21 @@ def test_split_backward_equals_unsplit(P, G, orc):
     side = torch.cuda.Stream()
     cur = torch.cuda.current_stream()
     ctx.render_backward(sh, G.t(up[0]), G.t(up[1]), G.t(up[2]), None, None, None, None, None, v_sun_depth=v_sun)
+    # while the chain is pending, everything that would overwrite or double the moment records is refused and launches
+    # nothing: the gradients compared below are those of ONE blend backward
+    for misuse in (lambda: ctx.render_backward(sh, G.t(up[0]), G.t(up[1]), G.t(up[2]), None, None, None, None, None, v_sun_depth=v_sun),
+                   lambda: ctx.preprocess(P.Camera.from_view(view), *surf),
+                   lambda: ctx.set_option(P.OPT_SPLIT_BACKWARD, 0)):
+        with pytest.raises(P.SatsplatError) as e:
+            misuse()
+        assert e.value.code == P.E_STATE and "pending" in str(e.value)
     side.wait_stream(cur)
     ctx.backward_chain(g["v_means"], g["v_quats"], g["v_scales"], g["v_logits"], g["v_rgb"], g["v_dF"], g["v_cc"], g["v_ambient"],
                        g["v_reproj"], stream=side)
     sctx.shadow_map_backward(v_sun, None, None, None, None)
+    with pytest.raises(P.SatsplatError) as e:
+        sctx.shadow_map_backward(v_sun, None, None, None, None)
+    assert e.value.code == P.E_STATE
     cur.wait_stream(side)
     sctx.backward_chain(g2["v_means"], g2["v_quats"], g2["v_scales"], g2["v_logits"], None, g2["v_dF_sun"])
     torch.cuda.synchronize()
