@@ -916,6 +916,46 @@ def test_p15_adam_matches_torch_optimizer_over_several_steps():
             np.testing.assert_allclose(cur[k], ref, rtol=1e-10, atol=1e-12)
 
 
+def test_p15_camera_adam_is_per_view_adam():
+    """Per-camera groups (1e-4 camera deltas, 1e-3 gain and bias): over a sequence of iterations that render
+    one view each, every view's rows follow torch.optim.Adam (an independent routine) run on that view ALONE with the
+    gradients of the iterations that rendered it -- own state, own step counter -- and an iteration leaves the rows, the
+    state and the counters of all other views bit for bit alone."""
+    import torch
+    from oracle import adam
+    rng = np.random.default_rng(21)
+    V = 4
+    width = dict(dF=8, cc=12, ambient=3)
+    lrs = dict(dF=1e-4, cc=1e-3, ambient=1e-3)
+    params = {k: rng.normal(0, 1, (V, w)) for k, w in width.items()}
+    state = {k: (np.zeros((V, w)), np.zeros((V, w))) for k, w in width.items()}
+    steps = np.zeros(V, np.int64)
+    tp = [{k: torch.tensor(params[k][v], dtype=torch.float64, requires_grad=True) for k in adam.CAMERA_GROUPS} for v in range(V)]
+    opts = [torch.optim.Adam([dict(params=[tp[v][k]], lr=lrs[k]) for k in adam.CAMERA_GROUPS], betas=(0.9, 0.999), eps=1e-8) for v in range(V)]
+    order = [0, 2, 2, 1, 0, 2, 3, 2, 0, 0, 1, 2]          # view 2 is rendered five times, view 3 once
+    for it, view in enumerate(order):
+        grads = {k: rng.normal(0, 1, w) * 10.0 ** rng.uniform(-3, 1) for k, w in width.items()}
+        before = {k: params[k].copy() for k in width}, {k: (state[k][0].copy(), state[k][1].copy()) for k in width}, steps.copy()
+        params, state, steps = adam.adam_step_cameras(params, grads, state, steps, view, lrs)
+        for k in adam.CAMERA_GROUPS:
+            tp[view][k].grad = torch.tensor(grads[k], dtype=torch.float64)
+        opts[view].step()
+        others = np.arange(V) != view
+        for k in adam.CAMERA_GROUPS:
+            np.testing.assert_allclose(params[k][view], tp[view][k].detach().numpy(), rtol=1e-12, atol=1e-15)
+            assert np.array_equal(params[k][others], before[0][k][others])
+            assert np.array_equal(state[k][0][others], before[1][k][0][others]) and np.array_equal(state[k][1][others], before[1][k][1][others])
+            assert not np.array_equal(params[k][view], before[0][k][view])
+        assert steps[view] == before[2][view] + 1 and np.array_equal(steps[others], before[2][others])
+    assert steps.tolist() == [4, 2, 5, 1]
+    # first step of a view, whatever the global iteration: lr g / (|g| + eps)
+    p1 = {k: np.zeros((1, w)) for k, w in width.items()}
+    g1 = {k: rng.normal(0, 1, w) for k, w in width.items()}
+    out, _, _ = adam.adam_step_cameras(p1, g1, {k: (np.zeros((1, w)), np.zeros((1, w))) for k, w in width.items()}, np.zeros(1), 0, lrs)
+    for k in adam.CAMERA_GROUPS:
+        np.testing.assert_allclose(out[k][0], -lrs[k] * g1[k] / (np.abs(g1[k]) + 1e-8), rtol=1e-12)
+
+
 # ------------------------------------------------------------------------------------------------ P16
 def test_p16_depth_normals_of_a_world_plane():
     """Eq. 13 on the depth image of a tilted world plane seen by an affine camera: every interior pixel must return the
