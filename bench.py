@@ -435,7 +435,7 @@ class Job:
             self.P.sun_camera_backward(self.cams[vi][0], v.sun_azimuth, v.sun_elevation, v.sun_viewport, g["dFs"], g["rep"], g["dF"])
 
 
-    def step_device(self, stride=1, buf=0, upstream_fn=None):
+    def step_device(self, stride=1, buf=0, upstream_fn=None, camera_step_fn=None):
         """The same iteration with every camera read from the device-resident block: the view is
         selected by the device index, nothing of it is baked into kernel arguments, so ONE captured graph of this function
         serves all views and all optimiser steps (dF lives in self.dF_all on the device)."""
@@ -476,6 +476,8 @@ class Job:
         # cascade (Fig. 1): view-pass dF gradient + adjoint of the sun camera / reprojection -> this view's row of v_dF_all
         P.camera_chain_backward(self.table, self.dF_all, self.idx, g["dF"], g["dFs"] if self.shadows else None,
                                 g["rep"] if self.shadows else None, None, self.v_dF_all)
+        if camera_step_fn:      # the optimiser step of the per-camera groups needs the index of the view just rendered
+            camera_step_fn(g)
         P.advance_view_index(self.idx, stride, len(self.scene.views))
 
 
@@ -912,8 +914,15 @@ def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
             P.loss_upstream(cam, job.out[0], job.out[1], job.out[2], tgt, scr, vv[0], vv[1], vv[2], sums)
             return vv
 
+        nv_ = len(scene.views)
+        cm, cv = torch.zeros(nv_, 23, device=device), torch.zeros(nv_, 23, device=device)
+        csteps = torch.zeros(nv_, dtype=torch.int32, device=device)
+
+        def camera_step(g):     # dF, gain / bias (and ambient) of the rendered view; tiny rates as for the surfels
+            P.adam_step_cameras(job.table, job.idx, job.dF_all, job.v_dF_all, g["cc"], g["amb"], cm, cv, csteps, [1e-9] * 3)
+
         def train_iteration():
-            job.step_device(upstream_fn=upstream)
+            job.step_device(upstream_fn=upstream, camera_step_fn=camera_step)
             P.adam_step(scene.n, *surf, *gg, am, av, lr_tiny, step=100)
         job.idx.fill_(step_views[0])
         train_iteration()
@@ -926,8 +935,9 @@ def extras(line, args, job, P, torch, scene, device, peaks, step_views, px):
         ms_train = timed(torch, None, 1, lambda _: tgraph.replay(), range(50)) / 50
         line["training_iteration"] = dict(ms=ms_train, mpixel_s=px / 1e6 / (ms_train * 1e-3),
                                           note="ONE graph replay per iteration: the step of `value` + loss stage between forward and "
-                                               "backward + fused Adam over the 13 N parameters (learning rates 1e-7: the synthetic "
-                                               "scene stays put); not included in value / ms_per_step")
+                                               "backward + fused Adam over the 13 N parameters + Adam step of the rendered view's camera groups "
+                                               "(dF, gain / bias, ambient; PAPER.md:349) -- a closed step for every learnable group "
+                                               "(learning rates 1e-7 / 1e-9: the synthetic scene stays put); not included in value / ms_per_step")
     # ---- geometry-aware initialisation (row f4): one-time work, on a DSM of the site's size ----
     side = int(round(1000.0 / 0.3)) if args.config in (3, 4) else 512
     gen = torch.Generator(device=device); gen.manual_seed(1)

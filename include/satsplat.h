@@ -283,6 +283,28 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
                        const float* v_means, const float* v_quats, const float* v_scales, const float* v_opacity_logits,
                        const float* v_rgb, float* adam_m, float* adam_v, const satsplat_adam* hp, satsplat_stream stream);
 
+/* The same step for the per-camera groups ("0.0001 for camera delta matrices, and 0.001 for camera gain and
+ * bias"): the row of dF (Eq. 15), the 3x4 [C | c] and the ambient term (Eq. 1) of the view *view_index (DEVICE int32; NULL =
+ * view 0).  One training iteration renders one view, so only that view has a gradient: its 23 values, their state and its
+ * own step counter advance (bias correction from steps[view] + 1); every other view is left untouched.  A schedule such as
+ * "camera loss from iteration 3000" is the caller's: pass lr = 0 until then.
+ *   views     DEVICE [n_views] table (the one satsplat_camera_chain reads); cc and ambient are updated IN it
+ *   dF        DEVICE [n_views,8], updated in place; v_dF_all DEVICE [n_views,8] as accumulated by
+ *             satsplat_camera_chain_backward (the view's row is set to zero afterwards if clear_v_dF != 0); both NULL = group off
+ *   v_cc [12], v_ambient [3]   DEVICE gradients of the rendered view (satsplat_render_backward*); NULL = group off
+ *   adam_m, adam_v DEVICE [n_views,23] (dF 8, cc 12, ambient 3 per view), zero before the first step; steps DEVICE int32
+ *             [n_views], zero before the first step
+ *   hp        HOST; lr[] in the order dF, cc, ambient
+ * One 32-thread kernel on `stream`, no host synchronisation; all view-dependent state is on the device, so a captured graph
+ * serves every view.  Errors: SATSPLAT_E_INVALID, SATSPLAT_E_CUDA. */
+typedef struct {
+  float lr[3];
+  float beta1, beta2, eps;
+} satsplat_camera_adam;
+int satsplat_adam_step_cameras(int32_t n_views, const int32_t* view_index, satsplat_view_params* views, float* dF, float* v_dF_all,
+                               const float* v_cc, const float* v_ambient, float* adam_m, float* adam_v, int32_t* steps,
+                               const satsplat_camera_adam* hp, int32_t clear_v_dF, satsplat_stream stream);
+
 /* ---- loss stage ----------------------------------------------------------- */
 /* L = w_l1 mean|I - I*| + w_ssim (1 - mean SSIM(I, I*)) + w_dist mean(L_dist) + w_normal mean(1 - A_sg N_r . N_d)
  * (PAPER.md:349 lists the terms and weights 0.8 / 0.2 / 0.05 / 0.05; :133-138 Eq. 13 defines N_d) and its gradients with

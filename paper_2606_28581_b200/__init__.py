@@ -60,6 +60,11 @@ class Adam(C.Structure):
     _fields_ = [("lr", C.c_float * 5), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
 
 
+class CameraAdam(C.Structure):
+    """satsplat_camera_adam (include/satsplat.h): lr in the order dF, cc, ambient."""
+    _fields_ = [("lr", C.c_float * 3), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float)]
+
+
 class Shading(C.Structure):
     """satsplat_shading (include/satsplat.h)."""
     _fields_ = [("cc", C.c_float * 12), ("ambient", C.c_float * 3), ("shadows_on", C.c_int32),
@@ -146,6 +151,7 @@ def lib():
         L.satsplat_adam_state_floats.restype = C.c_int64
         L.satsplat_adam_state_floats.argtypes = [i64]
         L.satsplat_adam_step.argtypes = [i64] + [vp] * 12 + [C.POINTER(Adam), vp]
+        L.satsplat_adam_step_cameras.argtypes = [i32] + [vp] * 9 + [C.POINTER(CameraAdam), i32, vp]
         L.satsplat_preprocess.argtypes = [vp, C.POINTER(Camera), i64, vp, vp, vp, vp, vp, vp]
         L.satsplat_render_forward.argtypes = [vp, C.POINTER(Shading), vp, vp, vp, vp]
         L.satsplat_shadow_map.argtypes = [vp, vp, vp]
@@ -364,6 +370,27 @@ def adam_step(n, means, quats, scales, opacity_logits, rgb, v_means, v_quats, v_
                                   C.byref(hp), _stream(stream))
     if rc:
         raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def adam_step_cameras(views_dev, view_index_dev, dF, v_dF_all, v_cc, v_ambient, adam_m, adam_v, steps, lr, beta1=0.9, beta2=0.999,
+                      eps=1e-8, clear_v_dF=True, stream=None):
+    """satsplat_adam_step_cameras: one Adam step on the dF row, [C | c] and ambient of view *view_index_dev, in place
+    (cc / ambient inside the device view table `views_dev`); per-view state [V,23] and step counters [V] (device tensors)."""
+    hp = CameraAdam()
+    hp.lr[:] = [float(x) for x in lr]
+    hp.beta1, hp.beta2, hp.eps = float(beta1), float(beta2), float(eps)
+    rc = lib().satsplat_adam_step_cameras(int(views_dev.shape[0]), _ptr(view_index_dev, torch.int32), _ptr(views_dev, torch.uint8), _ptr(dF),
+                                          _ptr(v_dF_all), _ptr(v_cc), _ptr(v_ambient), _ptr(adam_m), _ptr(adam_v),
+                                          _ptr(steps, torch.int32), C.byref(hp), 1 if clear_v_dF else 0, _stream(stream))
+    if rc:
+        raise SatsplatError(rc, lib().satsplat_last_error(None).decode())
+
+
+def view_table_shading(views_dev):
+    """(cc [V,12], ambient [V,3]) float32 copies read out of a device view table (where satsplat_adam_step_cameras steps them)."""
+    f = views_dev.view(torch.float32).view(views_dev.shape[0], -1)
+    o_cc, o_amb = ViewParams.cc.offset // 4, ViewParams.ambient.offset // 4
+    return f[:, o_cc:o_cc + 12].clone(), f[:, o_amb:o_amb + 3].clone()
 
 
 class Context:

@@ -318,6 +318,21 @@ int satsplat_adam_step(int64_t N, float* means, float* quats, float* scales, flo
   return SATSPLAT_OK;
 }
 
+int satsplat_adam_step_cameras(int32_t n_views, const int32_t* view_index, satsplat_view_params* views, float* dF, float* v_dF_all,
+                               const float* v_cc, const float* v_ambient, float* adam_m, float* adam_v, int32_t* steps,
+                               const satsplat_camera_adam* hp, int32_t clear_v_dF, satsplat_stream stream) {
+  if (n_views <= 0 || !views || !adam_m || !adam_v || !steps || !hp)
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step_cameras: bad argument");
+  if ((dF == nullptr) != (v_dF_all == nullptr))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step_cameras: dF and v_dF_all must both be given or both be NULL");
+  if (!(hp->beta1 >= 0.f && hp->beta1 < 1.f) || !(hp->beta2 >= 0.f && hp->beta2 < 1.f))
+    return fail(nullptr, SATSPLAT_E_INVALID, "satsplat_adam_step_cameras: the betas must be in [0, 1)");
+  cudaError_t e = launch_camera_adam(n_views, view_index, views, dF, v_dF_all, v_cc, v_ambient, adam_m, adam_v, steps, hp->lr, hp->beta1,
+                                     hp->beta2, hp->eps, clear_v_dF ? 1 : 0, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(nullptr, SATSPLAT_E_CUDA, "satsplat_adam_step_cameras: %s", cudaGetErrorString(e));
+  return SATSPLAT_OK;
+}
+
 namespace {
 // The blend half of a split backward accumulates per-surfel moment records with REDs and only the chain clears them: a
 // second blend backward, a new preprocess or an option change in between would leave stale moments for the next chain.

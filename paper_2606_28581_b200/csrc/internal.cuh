@@ -312,6 +312,9 @@ cudaError_t launch_init_from_dsm(const float* dsm, int W, int H, float cell, flo
                                  int32_t* cells_out, cudaStream_t s);
 cudaError_t launch_adam(int64_t N, float* const params[5], const float* const grads[5], float* m, float* v, const float lrs[5],
                         float beta1, float beta2, float eps, int step, cudaStream_t s);
+cudaError_t launch_camera_adam(int n_views, const int32_t* view_index, satsplat_view_params* views, float* dF, float* v_dF_all,
+                               const float* v_cc, const float* v_ambient, float* m, float* v, int32_t* steps, const float lr[3],
+                               float beta1, float beta2, float eps, int clear_v_dF, cudaStream_t s);
 cudaError_t launch_sun_camera_backward(float sc0, float sc1, float s0, float s1, const float* v_F_sun, const float* v_reproj,
                                        float* v_dF, cudaStream_t s);
 cudaError_t launch_camera_chain(const satsplat_view_params* views, const float* dF_all, const int32_t* view_index, float* block,

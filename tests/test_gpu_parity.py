@@ -618,6 +618,69 @@ def test_adam_step_matches_oracle(P, G, n):
                     dg["logits"], dg["rgb"], dm, dv, [0.1] * 5, step=0)
 
 
+def test_camera_adam_step_matches_oracle(P, G):
+    """satsplat_adam_step_cameras against oracle/adam.adam_step_cameras over a sequence of iterations that render one view
+    each (view index on the device): the rendered view's dF row, [C | c] and ambient (the latter two inside the device view
+    table the camera chain reads) follow the oracle, every other view stays bit for bit, counters are per view, the consumed
+    v_dF row is cleared, and the stepped colour correction is what the next camera chain delivers."""
+    import torch
+    from oracle import adam
+    scene = S.make_config(2, n=500, size=64, n_views=4, extent=30.0, sun_size=96)
+    V = len(scene.views)
+    table, dF_all, idx, block = _chain_setup(P, G, scene, [(0.0, 0.0)] * V)
+    rng = np.random.default_rng(5)
+    lrs = dict(dF=1e-4, cc=1e-3, ambient=1e-3)                 # PAPER.md:349
+    cc0, amb0 = P.view_table_shading(table)
+    params = dict(dF=dF_all.cpu().numpy().astype(np.float64), cc=cc0.cpu().numpy().astype(np.float64), ambient=amb0.cpu().numpy().astype(np.float64))
+    state = {k: (np.zeros_like(v), np.zeros_like(v)) for k, v in params.items()}
+    steps = np.zeros(V, np.int64)
+    dm, dv = torch.zeros(V, 23, device="cuda"), torch.zeros(V, 23, device="cuda")
+    dsteps = torch.zeros(V, dtype=torch.int32, device="cuda")
+    v_dF_all = torch.zeros(V, 8, device="cuda")
+    raw0 = table.clone()
+    for it, view in enumerate([0, 2, 2, 1, 0, 2, 3, 2]):
+        grads = {k: (rng.normal(0, 1, params[k].shape[1]) * 10.0 ** rng.uniform(-3, 1)).astype(np.float32).astype(np.float64) for k in adam.CAMERA_GROUPS}
+        params, state, steps = adam.adam_step_cameras(params, grads, state, steps, view, lrs)
+        idx.fill_(view)
+        v_dF_all[view] = G.t(grads["dF"])
+        before = (dF_all.clone(), table.clone())
+        P.adam_step_cameras(table, idx, dF_all, v_dF_all, G.t(grads["cc"]), G.t(grads["ambient"]), dm, dv, dsteps, [lrs[k] for k in adam.CAMERA_GROUPS])
+        torch.cuda.synchronize()
+        cc, amb = P.view_table_shading(table)
+        got = dict(dF=dF_all.cpu().numpy(), cc=cc.cpu().numpy(), ambient=amb.cpu().numpy())
+        others = np.arange(V) != view
+        for k in adam.CAMERA_GROUPS:
+            # one step moves a value by at most lr: fp32 arithmetic of the step is 2e-5 of that, plus the storage rounding
+            tol = 2e-6 * np.abs(params[k][view]) + 2e-5 * lrs[k] * (it + 1)
+            assert (np.abs(got[k][view].astype(np.float64) - params[k][view]) <= tol).all(), (k, it, got[k][view], params[k][view])
+        assert torch.equal(dF_all[torch.from_numpy(others).cuda()], before[0][torch.from_numpy(others).cuda()])
+        assert torch.equal(table[torch.from_numpy(others).cuda()], before[1][torch.from_numpy(others).cuda()])
+        assert (v_dF_all == 0).all()                            # the consumed row was cleared
+        assert dsteps.cpu().numpy().tolist() == steps.tolist()
+    # nothing but cc and ambient changed inside the table
+    o_cc, o_amb = P.ViewParams.cc.offset, P.ViewParams.ambient.offset
+    keep = torch.ones(table.shape[1], dtype=torch.bool, device="cuda")
+    keep[o_cc:o_cc + 48] = False
+    keep[o_amb:o_amb + 12] = False
+    assert torch.equal(table[:, keep], raw0[:, keep])
+    np.testing.assert_allclose(dm.cpu().numpy()[:, :8], state["dF"][0], rtol=2e-5, atol=1e-7 * np.abs(state["dF"][0]).max())
+    np.testing.assert_allclose(dv.cpu().numpy()[:, 8:20], state["cc"][1], rtol=2e-5, atol=1e-12)
+    # the camera chain delivers the stepped constants
+    idx.fill_(2)
+    P.camera_chain(table, dF_all, idx, block)
+    b = block.cpu().numpy()
+    cc, amb = P.view_table_shading(table)
+    assert np.array_equal(b[48:60], cc[2].cpu().numpy()) and np.array_equal(b[60:63], amb[2].cpu().numpy())
+    assert np.array_equal(b[0:8], (np.stack([v.F for v in scene.views]).astype(np.float32)[2] + dF_all[2].cpu().numpy()))
+    # a group whose gradient is NULL is left alone (state and counters of the others still advance)
+    d0, t0 = dF_all.clone(), table.clone()
+    P.adam_step_cameras(table, idx, None, None, None, G.t(np.ones(3, np.float32)), dm, dv, dsteps, [1e-4, 1e-3, 1e-3])
+    cc2, amb2 = P.view_table_shading(table)
+    assert torch.equal(d0, dF_all) and torch.equal(cc2, cc) and not torch.equal(amb2[2], amb[2])
+    with pytest.raises(P.SatsplatError):
+        P.adam_step_cameras(table, idx, dF_all, None, None, None, dm, dv, dsteps, [1e-4, 1e-3, 1e-3])
+
+
 def _loss_grad_close(name, g, ref, npx, z_bg=1.0):
     """Element-wise bar of the loss stage: |gpu - ref| <= atol + rtol |ref| in the natural unit of an upstream-gradient
     image, 1 / (number of pixels) (every loss term is a mean over pixels): atol = 5e-5 / npx, rtol = 1e-3.  The
